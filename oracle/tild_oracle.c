@@ -1,0 +1,652 @@
+/*
+ * tild_oracle.c -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+ *
+ * Plain, slow, double-precision CPU statement of one TILD time step as described in
+ * /root/reference/PAPER.md (arxiv 2302.02474, MATILDA.FT):
+ *   spread -> forward DFT -> pair-kernel multiply + ik gradient -> inverse DFT -> interpolate
+ *   -> harmonic bonds -> GJF Langevin update with Philox4x32-10 noise.
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
+ * call it.  It shares no code, header, table or constant generator with the CUDA path under
+ * paper_2302_02474_b200/csrc/, and neither includes the other.
+ *
+ * Every function cites the PAPER.md passage (or the DESIGN.md reading "A<n>" where the paper is
+ * silent) it follows.  Nothing is blocked, fused or reordered beyond what those passages state.
+ * The only concession to run time is an OpenMP "parallel for" over independent outputs
+ * (lines of the DFT, grid points, particles for gathers); the spread keeps one serial loop per
+ * species so that no atomics or re-association is involved.
+ *
+ * Pins (tests/test_oracle_*.py, all -m "not gpu"): weights vs numerically integrated top-hat
+ * convolutions, partition of unity, first moment; grid mass; DFT vs naive O(M^2) DFT and
+ * numpy.fft; PM force vs a mesh-free k-space sum and vs the direct periodic Gaussian pair sum;
+ * zero net force; bonds vs closed form; GJF(gamma=0) == velocity Verlet; dt^2 energy scaling;
+ * Philox vs cuRAND's host-compiled header.  End-to-end trajectory: "parity unpinned" beyond
+ * those (no reference trajectory exists).
+ *
+ * Build: gcc -O2 -std=c99 -ffp-contract=off -fopenmp -shared -fPIC tild_oracle.c -lm
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#define ORC_MAX_SPECIES 8
+#define ORC_MAX_ORDER 5
+
+typedef struct {
+    int32_t n;          /* particles */
+    int32_t S;          /* species */
+    double L[3];        /* box, orthogonal periodic, origin 0 (A3) */
+    int32_t N[3];       /* grid */
+    int32_t P;          /* nodes per dimension touched by one particle (A1) */
+    double chi[ORC_MAX_SPECIES * ORC_MAX_SPECIES];
+    double kappa;
+    double sigma2;      /* variance of u_G; sigma2 = 2 a^2, L143 */
+    double rho0;        /* n/V, L121 */
+    double k_bond, r0_bond; /* U = k (r - r0)^2 (A10); Eq. 2 L114 has k = 3/(2 b^2), r0 = 0 */
+    int32_t max_bonds;
+    double dt, gamma, kT, mass;
+    uint64_t seed;
+} orc_params;
+
+static const double ORC_PI = 3.14159265358979323846264338327950288;
+
+int orc_struct_size(void) { return (int)sizeof(orc_params); }
+
+void orc_set_threads(int t)
+{
+#ifdef _OPENMP
+    if (t > 0) omp_set_num_threads(t);
+#else
+    (void)t;
+#endif
+}
+int orc_get_threads(void)
+{
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+/* ------------------------------------------------------------------------------------------
+ * O2 Weights.  PAPER.md L223 ("spline interpolation scheme with the weights given in the
+ * appendix of Ref. [40]", Deserno & Holm) and Fig. 1 L231.  Reading A1/A2: P = nodes per
+ * dimension; W^(P) = P-fold convolution of the unit top-hat.  t in [-1/2, 1/2] is the offset of
+ * the particle from the centre of its stencil: from the nearest node for odd P, from the
+ * midpoint between the two nearest nodes for even P.  w[j], j = 0..P-1, runs over the stencil
+ * nodes in increasing coordinate.
+ * ---------------------------------------------------------------------------------------- */
+void orc_weights(int P, double t, double *w)
+{
+    switch (P) {
+    case 1:
+        w[0] = 1.0;
+        break;
+    case 2:
+        w[0] = 0.5 - t;
+        w[1] = 0.5 + t;
+        break;
+    case 3:
+        w[0] = 0.5 * (0.5 - t) * (0.5 - t);
+        w[1] = 0.75 - t * t;
+        w[2] = 0.5 * (0.5 + t) * (0.5 + t);
+        break;
+    case 4:
+        w[0] = (1.0 - 2.0 * t) * (1.0 - 2.0 * t) * (1.0 - 2.0 * t) / 48.0;
+        w[1] = (23.0 - 30.0 * t - 12.0 * t * t + 24.0 * t * t * t) / 48.0;
+        w[2] = (23.0 + 30.0 * t - 12.0 * t * t - 24.0 * t * t * t) / 48.0;
+        w[3] = (1.0 + 2.0 * t) * (1.0 + 2.0 * t) * (1.0 + 2.0 * t) / 48.0;
+        break;
+    case 5: {
+        double t2 = t * t, t3 = t2 * t, t4 = t2 * t2;
+        w[0] = (1.0 - 2.0 * t) * (1.0 - 2.0 * t) * (1.0 - 2.0 * t) * (1.0 - 2.0 * t) / 384.0;
+        w[1] = (19.0 - 44.0 * t + 24.0 * t2 + 16.0 * t3 - 16.0 * t4) / 96.0;
+        w[2] = (115.0 - 120.0 * t2 + 48.0 * t4) / 192.0;
+        w[3] = (19.0 + 44.0 * t + 24.0 * t2 - 16.0 * t3 - 16.0 * t4) / 96.0;
+        w[4] = (1.0 + 2.0 * t) * (1.0 + 2.0 * t) * (1.0 + 2.0 * t) * (1.0 + 2.0 * t) / 384.0;
+        break;
+    }
+    default:
+        for (int j = 0; j < P; ++j) w[j] = 0.0;
+    }
+}
+
+/* ------------------------------------------------------------------------------------------
+ * O1 Index map.  Not in the paper's PM text (nearest: cell binning L205).  Reading A15: the
+ * integer decisions are DEFINED in fp32 so that a double oracle and an fp32 GPU agree bit for
+ * bit: every operation below is one correctly rounded fp32 operation (compile with
+ * -ffp-contract=off; x86-64 SSE has no excess precision).
+ *   s  = fl32(x * inv_h),  inv_h = fl32(N / L)
+ *   even P: c = floorf(s),             t = fl32(fl32(s - c) - 0.5f), first node b = c - P/2 + 1
+ *   odd  P: c' = floorf(fl32(s+0.5f)), t = fl32(s - c'),             first node b = c' - (P-1)/2
+ *   cell   = floorf(s) mod N  (every P);  key = (cx*Ny + cy)*Nz + cz
+ * base[] holds the UNWRAPPED first node b (may be < 0 or + P > N); node j is (b + j) mod N.
+ * ---------------------------------------------------------------------------------------- */
+static int32_t orc_mod(int32_t a, int32_t N)
+{
+    int32_t r = a % N;
+    return r < 0 ? r + N : r;
+}
+
+static void orc_index_1(const orc_params *p, const float *xi, int32_t b[3], float t[3], int32_t c[3])
+{
+    for (int a = 0; a < 3; ++a) {
+        float inv_h = (float)((double)p->N[a] / p->L[a]);
+        float s = xi[a] * inv_h;
+        float fl = floorf(s);
+        c[a] = orc_mod((int32_t)fl, p->N[a]);
+        if (p->P % 2 == 0) {
+            float d = s - fl;
+            t[a] = d - 0.5f;
+            b[a] = (int32_t)fl - p->P / 2 + 1;
+        } else {
+            float sh = s + 0.5f;
+            float cp = floorf(sh);
+            t[a] = s - cp;
+            b[a] = (int32_t)cp - (p->P - 1) / 2;
+        }
+    }
+}
+
+void orc_index_map(const orc_params *p, const float *x, int32_t *base, float *toff, uint32_t *cell_key)
+{
+    for (int i = 0; i < p->n; ++i) {
+        int32_t b[3], c[3];
+        float t[3];
+        orc_index_1(p, x + 3 * (size_t)i, b, t, c);
+        for (int a = 0; a < 3; ++a) {
+            base[3 * (size_t)i + a] = b[a];
+            toff[3 * (size_t)i + a] = t[a];
+        }
+        cell_key[i] = (uint32_t)((c[0] * p->N[1] + c[1]) * p->N[2] + c[2]);
+    }
+}
+
+/* A16: counting sort by cell key.  cell_start[c] = number of particles with key < c
+ * (cell_start[M] = n); perm lists particle ids cell by cell, ascending id inside a cell
+ * (stable). */
+void orc_cell_sort(int32_t n, int32_t M, const uint32_t *cell_key, uint32_t *perm, uint32_t *cell_start)
+{
+    uint32_t *fill = (uint32_t *)calloc((size_t)M + 1, sizeof(uint32_t));
+    for (int32_t c = 0; c <= M; ++c) cell_start[c] = 0;
+    for (int32_t i = 0; i < n; ++i) cell_start[cell_key[i] + 1] += 1;
+    for (int32_t c = 0; c < M; ++c) cell_start[c + 1] += cell_start[c];
+    for (int32_t i = 0; i < n; ++i) {
+        uint32_t c = cell_key[i];
+        perm[cell_start[c] + fill[c]] = (uint32_t)i;
+        fill[c] += 1;
+    }
+    free(fill);
+}
+
+/* ------------------------------------------------------------------------------------------
+ * O3 Spread.  PAPER.md Eq. 1 L110 and L223: "every particle assigns its density contribution
+ * to nearby grid points".  grid[J][gx][gy][gz] = sum over particles of species J of
+ * w_x w_y w_z (raw weights; number density is grid / (h_x h_y h_z)).  z fastest (A17).
+ * ---------------------------------------------------------------------------------------- */
+void orc_spread(const orc_params *p, const float *x, const int32_t *type, double *grid)
+{
+    const int P = p->P;
+    const size_t M = (size_t)p->N[0] * p->N[1] * p->N[2];
+    memset(grid, 0, sizeof(double) * M * (size_t)p->S);
+    for (int i = 0; i < p->n; ++i) {
+        int32_t b[3], c[3];
+        float t[3];
+        double w[3][ORC_MAX_ORDER];
+        orc_index_1(p, x + 3 * (size_t)i, b, t, c);
+        for (int a = 0; a < 3; ++a) orc_weights(P, (double)t[a], w[a]);
+        double *g = grid + (size_t)type[i] * M;
+        for (int jx = 0; jx < P; ++jx) {
+            int gx = orc_mod(b[0] + jx, p->N[0]);
+            for (int jy = 0; jy < P; ++jy) {
+                int gy = orc_mod(b[1] + jy, p->N[1]);
+                for (int jz = 0; jz < P; ++jz) {
+                    int gz = orc_mod(b[2] + jz, p->N[2]);
+                    g[((size_t)gx * p->N[1] + gy) * p->N[2] + gz] += w[0][jx] * w[1][jy] * w[2][jz];
+                }
+            }
+        }
+    }
+}
+
+/* ------------------------------------------------------------------------------------------
+ * O4 / O6 DFT.  PAPER.md L223, L227 ("evaluated in Fourier space using FFTs").  Unnormalised
+ * in both directions:  X[k] = sum_j x[j] exp(sign * 2 pi i j k / n).
+ * Recursive decimation in time on the smallest prime factor p of n (n = p m):
+ *   Y_r[k] = DFT_m of the samples j = r, r+p, r+2p, ...           (r = 0..p-1, k = 0..m-1)
+ *   X[k + q m] = sum_r exp(sign 2 pi i r (k + q m) / n) Y_r[k]    (q = 0..p-1)
+ * data: interleaved (re, im) doubles.
+ * ---------------------------------------------------------------------------------------- */
+static int orc_smallest_factor(int n)
+{
+    for (int f = 2; f * f <= n; ++f)
+        if (n % f == 0) return f;
+    return n;
+}
+
+static void orc_dft_rec(int n, int stride, const double *in, double *out, int sign, int n_top,
+                        const double *tw /* tw[2k] + i tw[2k+1] = exp(sign 2 pi i k / n_top) */)
+{
+    if (n == 1) {
+        out[0] = in[0];
+        out[1] = in[1];
+        return;
+    }
+    const int p = orc_smallest_factor(n);
+    const int m = n / p;
+    for (int r = 0; r < p; ++r) orc_dft_rec(m, stride * p, in + 2 * (size_t)r * stride, out + 2 * (size_t)r * m, sign, n_top, tw);
+    const int step = n_top / n; /* exp(sign 2 pi i a / n) = tw[a * step] */
+    double yr[2 * 64], yi_unused;
+    (void)yi_unused;
+    for (int k = 0; k < m; ++k) {
+        for (int r = 0; r < p; ++r) {
+            yr[2 * r] = out[2 * ((size_t)r * m + k)];
+            yr[2 * r + 1] = out[2 * ((size_t)r * m + k) + 1];
+        }
+        for (int q = 0; q < p; ++q) {
+            double sr = 0.0, si = 0.0;
+            for (int r = 0; r < p; ++r) {
+                long a = ((long)r * (k + (long)q * m)) % n;
+                double c = tw[2 * (a * step)], s = tw[2 * (a * step) + 1];
+                sr += c * yr[2 * r] - s * yr[2 * r + 1];
+                si += c * yr[2 * r + 1] + s * yr[2 * r];
+            }
+            out[2 * ((size_t)k + (size_t)q * m)] = sr;
+            out[2 * ((size_t)k + (size_t)q * m) + 1] = si;
+        }
+    }
+}
+
+/* 1-D DFT of n points, in[j] at in + 2*j*stride, out contiguous. n's prime factors must be <= 61. */
+void orc_dft1d(int n, int stride, const double *in, double *out, int sign)
+{
+    double *tw = (double *)malloc(sizeof(double) * 2 * (size_t)n);
+    for (int k = 0; k < n; ++k) {
+        double ang = (double)sign * 2.0 * ORC_PI * (double)k / (double)n;
+        tw[2 * k] = cos(ang);
+        tw[2 * k + 1] = sin(ang);
+    }
+    orc_dft_rec(n, stride, in, out, sign, n, tw);
+    free(tw);
+}
+
+/* 3-D DFT in place: the 1-D DFT applied along z, then y, then x (separability of the kernel
+ * exp(sign 2 pi i (mx gx/Nx + my gy/Ny + mz gz/Nz))). */
+void orc_dft3d(const int32_t N[3], double *data, int sign)
+{
+    const int Nx = N[0], Ny = N[1], Nz = N[2];
+    for (int axis = 2; axis >= 0; --axis) {
+        const int len = N[axis];
+        const size_t stride = axis == 2 ? 1 : (axis == 1 ? (size_t)Nz : (size_t)Ny * Nz);
+        const size_t nlines = (size_t)Nx * Ny * Nz / len;
+        double *tw = (double *)malloc(sizeof(double) * 2 * (size_t)len);
+        for (int k = 0; k < len; ++k) {
+            double ang = (double)sign * 2.0 * ORC_PI * (double)k / (double)len;
+            tw[2 * k] = cos(ang);
+            tw[2 * k + 1] = sin(ang);
+        }
+#pragma omp parallel
+        {
+            double *line_in = (double *)malloc(sizeof(double) * 2 * (size_t)len);
+            double *line_out = (double *)malloc(sizeof(double) * 2 * (size_t)len);
+#pragma omp for schedule(static)
+            for (long l = 0; l < (long)nlines; ++l) {
+                size_t start;
+                if (axis == 2) start = (size_t)l * Nz;
+                else if (axis == 1) start = ((size_t)l / Nz) * ((size_t)Ny * Nz) + ((size_t)l % Nz);
+                else start = (size_t)l;
+                for (int j = 0; j < len; ++j) {
+                    line_in[2 * j] = data[2 * (start + j * stride)];
+                    line_in[2 * j + 1] = data[2 * (start + j * stride) + 1];
+                }
+                orc_dft_rec(len, 1, line_in, line_out, sign, len, tw);
+                for (int j = 0; j < len; ++j) {
+                    data[2 * (start + j * stride)] = line_out[2 * j];
+                    data[2 * (start + j * stride) + 1] = line_out[2 * j + 1];
+                }
+            }
+            free(line_in);
+            free(line_out);
+        }
+        free(tw);
+    }
+}
+
+/* ------------------------------------------------------------------------------------------
+ * O5 wave numbers and pair coefficients.
+ *   k_a(m) = 2 pi mt / L_a,  mt = m (m <= N/2), m - N (m > N/2).
+ *   Gradient factor: same, but 0 at m = N/2 for even N (A6: keeps the real-space kernel real
+ *   and odd => zero net force).
+ *   u^(k) = exp(-sigma2 |k|^2 / 2): Fourier transform of u_G, PAPER.md L121 (A4, A5).
+ *   c_IJ = (kappa + chi_IJ)/rho0 for I != J, kappa/rho0 for I == J: Eq. 3 L119 + Eq. 4 L123 (A9).
+ * ---------------------------------------------------------------------------------------- */
+static double orc_k(const orc_params *p, int a, int m)
+{
+    int N = p->N[a];
+    int mt = (m <= N / 2) ? m : m - N;
+    return 2.0 * ORC_PI * (double)mt / p->L[a];
+}
+static double orc_kgrad(const orc_params *p, int a, int m)
+{
+    int N = p->N[a];
+    if (N % 2 == 0 && m == N / 2) return 0.0;
+    return orc_k(p, a, m);
+}
+static double orc_cIJ(const orc_params *p, int I, int J)
+{
+    if (I == J) return p->kappa / p->rho0;
+    return (p->kappa + p->chi[I * ORC_MAX_SPECIES + J]) / p->rho0;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * O4-O6 k-space force.  PAPER.md Eq. 18, "becomes a simple multiplication" L227:
+ *   n^_J(m)   = sum_g n_J(g) exp(-2 pi i m.g/N)
+ *   f^_{I,a}(m) = -i k^grad_a(m) u^(k_m) sum_J c_IJ n^_J(m) / V
+ *   f_{I,a}(g)  = sum_m f^_{I,a}(m) exp(+2 pi i m.g/N)
+ * ffield[I][a][g] (real part; the imaginary part is round-off by Hermitian symmetry).
+ * ---------------------------------------------------------------------------------------- */
+void orc_kspace_force(const orc_params *p, const double *grid, double *ffield)
+{
+    const int S = p->S;
+    const size_t M = (size_t)p->N[0] * p->N[1] * p->N[2];
+    const double V = p->L[0] * p->L[1] * p->L[2];
+    double *nhat = (double *)malloc(sizeof(double) * 2 * M * (size_t)S);
+    double *work = (double *)malloc(sizeof(double) * 2 * M);
+    for (int J = 0; J < S; ++J) {
+        double *d = nhat + 2 * M * (size_t)J;
+        for (size_t g = 0; g < M; ++g) {
+            d[2 * g] = grid[(size_t)J * M + g];
+            d[2 * g + 1] = 0.0;
+        }
+        orc_dft3d(p->N, d, -1);
+    }
+    for (int I = 0; I < S; ++I) {
+        for (int a = 0; a < 3; ++a) {
+#pragma omp parallel for schedule(static)
+            for (int mx = 0; mx < p->N[0]; ++mx) {
+                for (int my = 0; my < p->N[1]; ++my) {
+                    for (int mz = 0; mz < p->N[2]; ++mz) {
+                        size_t g = ((size_t)mx * p->N[1] + my) * p->N[2] + mz;
+                        double kx = orc_k(p, 0, mx), ky = orc_k(p, 1, my), kz = orc_k(p, 2, mz);
+                        double uhat = exp(-0.5 * p->sigma2 * (kx * kx + ky * ky + kz * kz));
+                        int m_a = a == 0 ? mx : (a == 1 ? my : mz);
+                        double kg = orc_kgrad(p, a, m_a);
+                        double gr = 0.0, gi = 0.0;
+                        for (int J = 0; J < S; ++J) {
+                            double c = orc_cIJ(p, I, J);
+                            gr += c * nhat[2 * (M * (size_t)J + g)];
+                            gi += c * nhat[2 * (M * (size_t)J + g) + 1];
+                        }
+                        /* -i * (gr + i gi) = gi - i gr */
+                        double f = kg * uhat / V;
+                        work[2 * g] = f * gi;
+                        work[2 * g + 1] = -f * gr;
+                    }
+                }
+            }
+            orc_dft3d(p->N, work, +1);
+            double *out = ffield + ((size_t)I * 3 + a) * M;
+            for (size_t g = 0; g < M; ++g) out[g] = work[2 * g];
+        }
+    }
+    free(nhat);
+    free(work);
+}
+
+/* ------------------------------------------------------------------------------------------
+ * O7a Interpolation.  PAPER.md L227 / Fig. 1: "The same spline weights are used to map
+ * the forces back to the particles."  f[i][a] = sum_g w(g; r_i) ffield[type_i][a][g].
+ * ---------------------------------------------------------------------------------------- */
+void orc_interp(const orc_params *p, const double *ffield, const float *x, const int32_t *type, double *f)
+{
+    const int P = p->P;
+    const size_t M = (size_t)p->N[0] * p->N[1] * p->N[2];
+#pragma omp parallel for schedule(static)
+    for (int i = 0; i < p->n; ++i) {
+        int32_t b[3], c[3];
+        float t[3];
+        double w[3][ORC_MAX_ORDER];
+        orc_index_1(p, x + 3 * (size_t)i, b, t, c);
+        for (int a = 0; a < 3; ++a) orc_weights(P, (double)t[a], w[a]);
+        double acc[3] = {0.0, 0.0, 0.0};
+        for (int jx = 0; jx < P; ++jx) {
+            int gx = orc_mod(b[0] + jx, p->N[0]);
+            for (int jy = 0; jy < P; ++jy) {
+                int gy = orc_mod(b[1] + jy, p->N[1]);
+                for (int jz = 0; jz < P; ++jz) {
+                    int gz = orc_mod(b[2] + jz, p->N[2]);
+                    size_t g = ((size_t)gx * p->N[1] + gy) * p->N[2] + gz;
+                    double ww = w[0][jx] * w[1][jy] * w[2][jz];
+                    for (int a = 0; a < 3; ++a) acc[a] += ww * ffield[((size_t)type[i] * 3 + a) * M + g];
+                }
+            }
+        }
+        for (int a = 0; a < 3; ++a) f[3 * (size_t)i + a] = acc[a];
+    }
+}
+
+/* ------------------------------------------------------------------------------------------
+ * O7b Harmonic bonds.  PAPER.md Eq. 2 L114 (beta U0 = sum 3/(2 b^2) |dr|^2) and L209: every
+ * particle computes its own bonds, Newton's third law not used.  U = k (|d| - r0)^2 (A10), so
+ * the force on i from partner j is -2 k (1 - r0/|d|) d,  d = minimum-image(r_i - r_j).
+ * ADDS into f.
+ * ---------------------------------------------------------------------------------------- */
+static double orc_min_image(double d, double L)
+{
+    return d - L * floor(d / L + 0.5);
+}
+
+void orc_bond_force(const orc_params *p, const double *x, const int32_t *partner, double *f)
+{
+#pragma omp parallel for schedule(static)
+    for (int i = 0; i < p->n; ++i) {
+        for (int s = 0; s < p->max_bonds; ++s) {
+            int32_t j = partner[(size_t)i * p->max_bonds + s];
+            if (j < 0) continue;
+            double d[3], r2 = 0.0;
+            for (int a = 0; a < 3; ++a) {
+                d[a] = orc_min_image(x[3 * (size_t)i + a] - x[3 * (size_t)j + a], p->L[a]);
+                r2 += d[a] * d[a];
+            }
+            double scale = -2.0 * p->k_bond;
+            if (p->r0_bond != 0.0) {
+                double r = sqrt(r2);
+                scale = r > 0.0 ? scale * (1.0 - p->r0_bond / r) : 0.0;
+            }
+            for (int a = 0; a < 3; ++a) f[3 * (size_t)i + a] += scale * d[a];
+        }
+    }
+}
+
+/* Total force F(x): PM part on the fp32-rounded positions (O1 defines the index map on fp32
+ * input), bonds on the double positions. */
+void orc_force(const orc_params *p, const double *x, const int32_t *type, const int32_t *partner, double *f)
+{
+    const size_t M = (size_t)p->N[0] * p->N[1] * p->N[2];
+    float *xf = (float *)malloc(sizeof(float) * 3 * (size_t)p->n);
+    double *grid = (double *)malloc(sizeof(double) * M * (size_t)p->S);
+    double *ff = (double *)malloc(sizeof(double) * M * (size_t)p->S * 3);
+    for (size_t q = 0; q < 3 * (size_t)p->n; ++q) xf[q] = (float)x[q];
+    orc_spread(p, xf, type, grid);
+    orc_kspace_force(p, grid, ff);
+    orc_interp(p, ff, xf, type, f);
+    orc_bond_force(p, x, partner, f);
+    free(xf);
+    free(grid);
+    free(ff);
+}
+
+/* ------------------------------------------------------------------------------------------
+ * O9 Noise.  The paper says GJF "generates thermal noise internally" (L352) and names no
+ * generator; reading A12: Philox4x32-10 (Salmon, Moraes, Dror, Shaw, SC'11), restated here:
+ * ten rounds of
+ *   (c0,c1,c2,c3) <- (hi(M1*c2) ^ c1 ^ k0,  lo(M1*c2),  hi(M0*c0) ^ c3 ^ k1,  lo(M0*c0))
+ * with the key bumped by (W0, W1) between rounds.
+ * ---------------------------------------------------------------------------------------- */
+void orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4])
+{
+    const uint32_t M0 = 0xD2511F53u, M1 = 0xCD9E8D57u, W0 = 0x9E3779B9u, W1 = 0xBB67AE85u;
+    uint32_t c0 = ctr[0], c1 = ctr[1], c2 = ctr[2], c3 = ctr[3];
+    uint32_t k0 = key[0], k1 = key[1];
+    for (int round = 0; round < 10; ++round) {
+        uint64_t p0 = (uint64_t)M0 * c0;
+        uint64_t p1 = (uint64_t)M1 * c2;
+        uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ k0;
+        uint32_t n1 = (uint32_t)p1;
+        uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ k1;
+        uint32_t n3 = (uint32_t)p0;
+        c0 = n0; c1 = n1; c2 = n2; c3 = n3;
+        k0 += W0;
+        k1 += W1;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+/* beta^{step} for particle id: counter = (id, step_lo, step_hi, 0), key = (seed_lo, seed_hi);
+ * u_k = ((x_k >> 8) + 0.5) 2^-24;  Box-Muller;  beta = sqrt(2 gamma kT dt) (z0, z1, z2). */
+void orc_noise(const orc_params *p, uint32_t id, uint64_t step, double beta[3])
+{
+    uint32_t ctr[4] = {id, (uint32_t)(step & 0xffffffffu), (uint32_t)(step >> 32), 0u};
+    uint32_t key[2] = {(uint32_t)(p->seed & 0xffffffffu), (uint32_t)(p->seed >> 32)};
+    uint32_t r[4];
+    orc_philox4x32_10(ctr, key, r);
+    double u[4];
+    for (int k = 0; k < 4; ++k) u[k] = ((double)(r[k] >> 8) + 0.5) * (1.0 / 16777216.0);
+    double r01 = sqrt(-2.0 * log(u[0])), r23 = sqrt(-2.0 * log(u[2]));
+    double z0 = r01 * cos(2.0 * ORC_PI * u[1]);
+    double z1 = r01 * sin(2.0 * ORC_PI * u[1]);
+    double z2 = r23 * cos(2.0 * ORC_PI * u[3]);
+    double amp = sqrt(2.0 * p->gamma * p->kT * p->dt);
+    beta[0] = amp * z0;
+    beta[1] = amp * z1;
+    beta[2] = amp * z2;
+}
+
+/* Standard normals only (for the distribution tests). */
+void orc_normals(uint64_t seed, uint32_t id, uint64_t step, double z[3])
+{
+    orc_params q;
+    memset(&q, 0, sizeof(q));
+    q.seed = seed;
+    q.gamma = 0.5; q.kT = 1.0; q.dt = 1.0; /* amp = 1 */
+    orc_noise(&q, id, step, z);
+}
+
+/* A14 wrap into [0, L). */
+static double orc_wrap(double x, double L)
+{
+    double r = x - L * floor(x / L);
+    if (r >= L) r = 0.0;
+    if (r < 0.0) r = 0.0;
+    return r;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * O8 GJF step.  PAPER.md L352 names the Gronbech-Jensen & Farago integrator (used in Listing 1
+ * L82) without equations; reading A11 takes them from G-J & F, Mol. Phys. 111, 983 (2013):
+ *   b = 1/(1 + gamma dt/2m), a = (1 - gamma dt/2m) b, beta ~ N(0, 2 gamma kT dt) per component
+ *   r' = r + b dt v + (b dt^2/2m) F + (b dt/2m) beta,  wrapped
+ *   F' = F(r')
+ *   v' = a v + (dt/2m)(a F + F') + (b/m) beta
+ * x, v, f updated in place; f holds F(r) on entry and F(r') on exit.  `step` is the index of
+ * the step being taken (noise counter = step + 1, i.e. beta^{n+1} for n -> n+1).
+ * ---------------------------------------------------------------------------------------- */
+void orc_gjf_step(const orc_params *p, double *x, double *v, double *f, const int32_t *type,
+                  const int32_t *partner, uint64_t step)
+{
+    const double m = p->mass, dt = p->dt;
+    const double gh = p->gamma * dt / (2.0 * m);
+    const double b = 1.0 / (1.0 + gh), a = (1.0 - gh) / (1.0 + gh);
+    const size_t n3 = 3 * (size_t)p->n;
+    double *beta = (double *)malloc(sizeof(double) * n3);
+    double *fnew = (double *)malloc(sizeof(double) * n3);
+    for (int i = 0; i < p->n; ++i) {
+        if (p->gamma > 0.0) orc_noise(p, (uint32_t)i, step + 1, beta + 3 * (size_t)i);
+        else beta[3 * (size_t)i] = beta[3 * (size_t)i + 1] = beta[3 * (size_t)i + 2] = 0.0;
+    }
+    for (int i = 0; i < p->n; ++i)
+        for (int c = 0; c < 3; ++c) {
+            size_t q = 3 * (size_t)i + c;
+            double r = x[q] + b * dt * v[q] + (b * dt * dt / (2.0 * m)) * f[q] + (b * dt / (2.0 * m)) * beta[q];
+            x[q] = orc_wrap(r, p->L[c]);
+        }
+    orc_force(p, x, type, partner, fnew);
+    for (size_t q = 0; q < n3; ++q) {
+        v[q] = a * v[q] + (dt / (2.0 * m)) * (a * f[q] + fnew[q]) + (b / m) * beta[q];
+        f[q] = fnew[q];
+    }
+    free(beta);
+    free(fnew);
+}
+
+void orc_run(const orc_params *p, double *x, double *v, double *f, const int32_t *type,
+             const int32_t *partner, uint64_t step0, int32_t nsteps)
+{
+    for (int32_t s = 0; s < nsteps; ++s) orc_gjf_step(p, x, v, f, type, partner, step0 + (uint64_t)s);
+}
+
+/* ------------------------------------------------------------------------------------------
+ * O10 Energy (for the drift check).  e[0] = kinetic = m/2 sum |v|^2; e[1] = bonds, Eq. 2
+ * with U = k (|d| - r0)^2 counted once per bond (slot entries i < j only);
+ * e[2] = non-bonded, Eq. 3-4 L119-123 on the mesh:
+ *   (1/2V) sum_m u^(k_m) sum_IJ c_IJ Re[n^_I(m) conj(n^_J(m))]   (the rho0 shift touches m = 0 only).
+ * ---------------------------------------------------------------------------------------- */
+void orc_energy(const orc_params *p, const double *x, const double *v, const int32_t *type,
+                const int32_t *partner, double e[3])
+{
+    const int S = p->S;
+    const size_t M = (size_t)p->N[0] * p->N[1] * p->N[2];
+    const double V = p->L[0] * p->L[1] * p->L[2];
+    double ke = 0.0, be = 0.0, nb = 0.0;
+    for (size_t q = 0; q < 3 * (size_t)p->n; ++q) ke += 0.5 * p->mass * v[q] * v[q];
+    for (int i = 0; i < p->n; ++i)
+        for (int s = 0; s < p->max_bonds; ++s) {
+            int32_t j = partner[(size_t)i * p->max_bonds + s];
+            if (j < 0 || j < i) continue;
+            double r2 = 0.0;
+            for (int a = 0; a < 3; ++a) {
+                double d = orc_min_image(x[3 * (size_t)i + a] - x[3 * (size_t)j + a], p->L[a]);
+                r2 += d * d;
+            }
+            double dr = sqrt(r2) - p->r0_bond;
+            be += p->k_bond * dr * dr;
+        }
+    float *xf = (float *)malloc(sizeof(float) * 3 * (size_t)p->n);
+    double *grid = (double *)malloc(sizeof(double) * M * (size_t)S);
+    double *nhat = (double *)malloc(sizeof(double) * 2 * M * (size_t)S);
+    for (size_t q = 0; q < 3 * (size_t)p->n; ++q) xf[q] = (float)x[q];
+    orc_spread(p, xf, type, grid);
+    for (int J = 0; J < S; ++J) {
+        double *d = nhat + 2 * M * (size_t)J;
+        for (size_t g = 0; g < M; ++g) {
+            d[2 * g] = grid[(size_t)J * M + g];
+            d[2 * g + 1] = 0.0;
+        }
+        orc_dft3d(p->N, d, -1);
+    }
+    for (int mx = 0; mx < p->N[0]; ++mx)
+        for (int my = 0; my < p->N[1]; ++my)
+            for (int mz = 0; mz < p->N[2]; ++mz) {
+                size_t g = ((size_t)mx * p->N[1] + my) * p->N[2] + mz;
+                double kx = orc_k(p, 0, mx), ky = orc_k(p, 1, my), kz = orc_k(p, 2, mz);
+                double uhat = exp(-0.5 * p->sigma2 * (kx * kx + ky * ky + kz * kz));
+                double acc = 0.0;
+                for (int I = 0; I < S; ++I)
+                    for (int J = 0; J < S; ++J) {
+                        const double *aI = nhat + 2 * (M * (size_t)I + g), *aJ = nhat + 2 * (M * (size_t)J + g);
+                        acc += orc_cIJ(p, I, J) * (aI[0] * aJ[0] + aI[1] * aJ[1]);
+                    }
+                nb += uhat * acc;
+            }
+    nb *= 0.5 / V;
+    free(xf);
+    free(grid);
+    free(nhat);
+    e[0] = ke;
+    e[1] = be;
+    e[2] = nb;
+}

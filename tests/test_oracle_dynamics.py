@@ -1,0 +1,203 @@
+"""Pins for the oracle's bonds (O7b), GJF integrator (O8), noise (O9) and energy (O10).
+
+Bonds: PAPER.md Eq. 2 L114, L209.  GJF: named at L352 (equations from Gronbech-Jensen & Farago 2013,
+DESIGN.md reading A11): gamma = 0 must reduce to velocity Verlet step for step; the energy error must
+scale as dt^2; a free particle must diffuse with D = kT/gamma; a harmonic dimer must sample
+<r^2> = 3 kT / (2 k) (GJF is exact for configurational sampling of a harmonic well).
+Philox: bit-equality with cuRAND's own Philox4x32-10 header compiled for the host (library routine).
+"""
+import ctypes as C
+import os
+import shutil
+import subprocess
+
+import numpy as np
+import pytest
+from scipy import stats
+
+from oracle import tild_oracle as orc
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+
+
+def _p(n, L=(8.0, 8.0, 8.0), N=(8, 8, 8), P=2, S=2, chi=1.0, kappa=5.0, **kw):
+    chim = np.array([[0.0, chi], [chi, 0.0]])
+    return orc.OracleParams(n, S, L, N, P, chim, kappa, 0.5, **kw)
+
+
+def test_bond_force_closed_form_and_minimum_image():
+    L = (8.0, 8.0, 8.0)
+    x = np.array([[0.2, 4.0, 4.0], [7.9, 4.5, 3.0], [1.0, 1.0, 1.0]])
+    bp = np.array([[-1, 1], [0, -1], [-1, -1]], dtype=np.int32)
+    p = _p(3, k_bond=1.5, r0_bond=0.0)
+    f = orc.bond_force(p, x, bp)
+    d = np.array([0.2 - 7.9 + 8.0, -0.5, 1.0])                  # minimum image across the x boundary
+    assert np.allclose(f[0], -2 * 1.5 * d, atol=1e-13)
+    assert np.allclose(f[1], +2 * 1.5 * d, atol=1e-13)
+    assert np.allclose(f[2], 0.0)
+    # rest length r0: F = -2k (1 - r0/|d|) d
+    p2 = _p(3, k_bond=2.0, r0_bond=0.7)
+    f2 = orc.bond_force(p2, x, bp)
+    r = np.linalg.norm(d)
+    assert np.allclose(f2[0], -2 * 2.0 * (1 - 0.7 / r) * d, atol=1e-13)
+
+
+def test_bond_forces_sum_to_zero_on_chains():
+    from paper_2302_02474_b200 import inputs
+    st = inputs.make_state(inputs.C1)
+    p = _p(inputs.C1.n, L=inputs.C1.box, N=(4, 4, 4))
+    f = orc.bond_force(p, st.x.astype(np.float64), st.bond_partner)
+    assert np.abs(f.sum(0)).max() < 1e-10
+    # energy derivative: U = k sum_bonds |d|^2  ->  F = -dU/dx by central differences
+    x = st.x.astype(np.float64)
+    v = np.zeros_like(x)
+    p0 = _p(inputs.C1.n, L=inputs.C1.box, N=(4, 4, 4), chi=0.0, kappa=0.0)
+    eps = 1e-5
+    xp, xm = x.copy(), x.copy()
+    xp[37, 2] += eps
+    xm[37, 2] -= eps
+    dU = (orc.energy(p0, xp, v, st.type, st.bond_partner)[1] - orc.energy(p0, xm, v, st.type, st.bond_partner)[1]) / (2 * eps)
+    assert abs(-dU - f[37, 2]) < 1e-6
+
+
+def _small_melt(seed=3, n_chains=20, nb=6, L=6.0):
+    rng = np.random.default_rng(seed)
+    start = rng.random((n_chains, 1, 3)) * L
+    steps = rng.normal(0, np.sqrt(1 / 3), size=(n_chains, nb, 3))
+    steps[:, 0] = 0
+    x = (start + np.cumsum(steps, axis=1)).reshape(-1, 3) % L
+    n = n_chains * nb
+    ty = np.tile(np.repeat([0, 1], nb // 2), n_chains).astype(np.int32)
+    ids = np.arange(n).reshape(n_chains, nb)
+    prev, nxt = ids - 1, ids + 1
+    prev[:, 0] = -1
+    nxt[:, -1] = -1
+    bp = np.stack([prev.ravel(), nxt.ravel()], 1).astype(np.int32)
+    v = rng.normal(size=(n, 3))
+    return x.astype(np.float32).astype(np.float64), v, ty, bp
+
+
+def test_gjf_gamma0_is_velocity_verlet():
+    x, v, ty, bp = _small_melt()
+    n = x.shape[0]
+    L = 6.0
+    p = _p(n, L=(L,) * 3, N=(12,) * 3, P=3, gamma=0.0, dt=0.01)
+    xo, vo, fo = orc.run(p, x, v, ty, bp, 0, 5)
+    # velocity Verlet written out (Swope et al. 1982), force from the oracle's force routine
+    xv, vv = x.copy(), v.copy()
+    f = orc.force(p, xv, ty, bp)
+    dt = 0.01
+    for _ in range(5):
+        vv = vv + 0.5 * dt * f
+        xv = xv + dt * vv
+        xv = xv - L * np.floor(xv / L)
+        f = orc.force(p, xv, ty, bp)
+        vv = vv + 0.5 * dt * f
+    assert np.abs(xo - xv).max() < 1e-12
+    assert np.abs(vo - vv).max() < 1e-11
+
+
+def test_energy_error_scales_as_dt_squared():
+    x, v, ty, bp = _small_melt(seed=5)
+    n = x.shape[0]
+    L = 6.0
+    T = 0.32
+    devs = []
+    for dt in (0.02, 0.01):
+        p = _p(n, L=(L,) * 3, N=(16,) * 3, P=4, gamma=0.0, dt=dt, kappa=5.0, chi=1.0)
+        e0 = orc.energy(p, x, v, ty, bp).sum()
+        es = []
+        xc, vc, fc = x, v, None
+        nst = int(round(T / dt))
+        chunk = max(1, nst // 8)
+        for s in range(0, nst, chunk):
+            xc, vc, fc = orc.run(p, xc, vc, ty, bp, s, chunk, f=fc)
+            es.append(orc.energy(p, xc, vc, ty, bp).sum())
+        devs.append(np.abs(np.array(es) - e0).max())
+    ratio = devs[0] / devs[1]
+    assert 2.5 < ratio < 6.5, (devs, ratio)
+    assert devs[1] < 1e-2 * abs(e0) + 1.0
+
+
+def test_noise_is_keyed_by_id_and_step_and_has_gjf_variance():
+    p = _p(4, gamma=2.0, kT=1.5, dt=0.01, seed=123456789012345)
+    a = orc.noise(p, 7, 3)
+    assert np.array_equal(a, orc.noise(p, 7, 3))
+    assert not np.array_equal(a, orc.noise(p, 8, 3))
+    assert not np.array_equal(a, orc.noise(p, 7, 4))
+    z = np.array([orc.normals(42, i, 1) for i in range(20000)])
+    assert abs(z.mean()) < 0.02
+    assert np.abs(z.var(axis=0) - 1.0).max() < 0.04
+    assert np.abs(np.corrcoef(z.T) - np.eye(3)).max() < 0.03
+    for c in range(3):
+        assert stats.kstest(z[:, c], "norm").pvalue > 1e-3
+    b = np.array([orc.noise(p, i, 9) for i in range(20000)])
+    assert abs(b.var() / (2 * 2.0 * 1.5 * 0.01) - 1) < 0.03
+
+
+def test_free_particle_diffusion():
+    """No forces (kappa = chi = k_bond = 0): <dr^2> = 6 (kT/gamma) [t - (1 - e^{-gamma t})/gamma] for thermal v0."""
+    n = 3000
+    rng = np.random.default_rng(2)
+    L = 1000.0
+    x = np.full((n, 3), 500.0) + rng.random((n, 3))
+    v = rng.normal(size=(n, 3))
+    ty = np.zeros(n, np.int32)
+    bp = -np.ones((n, 2), np.int32)
+    gamma, dt, nst = 5.0, 0.02, 200
+    p = orc.OracleParams(n, 1, (L,) * 3, (4,) * 3, 1, np.zeros((1, 1)), 0.0, 0.5, k_bond=0.0, gamma=gamma, dt=dt, seed=99)
+    x1, v1, _ = orc.run(p, x, v, ty, bp, 0, nst)
+    t = dt * nst
+    msd = ((x1 - x) ** 2).sum(1).mean()
+    exact = 6 * (1.0 / gamma) * (t - (1 - np.exp(-gamma * t)) / gamma)
+    assert abs(msd / exact - 1) < 0.06, (msd, exact)
+    assert abs((v1 ** 2).mean() - 1.0) < 0.05        # kinetic temperature kT/m = 1 (dt-dependent bias is O(dt^2))
+
+
+def test_harmonic_dimer_samples_boltzmann():
+    """U = k r^2 -> <r^2> = 3 kT/(2k) = 1 for k = 1.5 (Eq. 2: b = 1)."""
+    nd = 1500
+    rng = np.random.default_rng(6)
+    L = 1000.0
+    c = rng.random((nd, 1, 3)) * 900 + 50
+    x = (c + rng.normal(0, 0.4, size=(nd, 2, 3))).reshape(-1, 3)
+    n = 2 * nd
+    v = rng.normal(size=(n, 3))
+    ty = np.zeros(n, np.int32)
+    ids = np.arange(n).reshape(nd, 2)
+    bp = -np.ones((n, 2), np.int32)
+    bp[ids[:, 0], 1] = ids[:, 1]
+    bp[ids[:, 1], 0] = ids[:, 0]
+    p = orc.OracleParams(n, 1, (L,) * 3, (4,) * 3, 1, np.zeros((1, 1)), 0.0, 0.5, k_bond=1.5, gamma=2.0, dt=0.1, seed=5)
+    xc, vc, fc = orc.run(p, x, v, ty, bp, 0, 100)
+    r2 = []
+    for k in range(6):
+        xc, vc, fc = orc.run(p, xc, vc, ty, bp, 100 + 20 * k, 20, f=fc)
+        d = xc[ids[:, 0]] - xc[ids[:, 1]]
+        r2.append((d ** 2).sum(1).mean())
+    assert abs(np.mean(r2) - 1.0) < 0.05, r2
+
+
+@pytest.fixture(scope="module")
+def curand_host(tmp_path_factory):
+    if shutil.which("nvcc") is None:
+        pytest.skip("nvcc not available to host-compile cuRAND's Philox header")
+    out = str(tmp_path_factory.mktemp("philox") / "libphilox_curand_host.so")
+    src = os.path.join(HERE, "helpers", "philox_curand_host.cu")
+    subprocess.run(["nvcc", "-O1", "-Wno-deprecated-gpu-targets", "-shared", "-Xcompiler", "-fPIC", src, "-o", out],
+                   check=True, capture_output=True)
+    return C.CDLL(out)
+
+
+def test_philox_matches_curand_header(curand_host):
+    rng = np.random.default_rng(77)
+    U = C.POINTER(C.c_uint32)
+    cases = [(np.zeros(4, np.uint32), np.zeros(2, np.uint32)),
+             (np.full(4, 0xFFFFFFFF, np.uint32), np.full(2, 0xFFFFFFFF, np.uint32))]
+    for _ in range(500):
+        cases.append((rng.integers(0, 2 ** 32, size=4, dtype=np.uint64).astype(np.uint32),
+                      rng.integers(0, 2 ** 32, size=2, dtype=np.uint64).astype(np.uint32)))
+    for ctr, key in cases:
+        ref = np.zeros(4, np.uint32)
+        curand_host.curand_philox_host(ctr.ctypes.data_as(U), key.ctypes.data_as(U), ref.ctypes.data_as(U))
+        assert np.array_equal(orc.philox4x32_10(ctr, key), ref)

@@ -1,0 +1,244 @@
+"""Pins for the oracle's particle-mesh non-bonded force (O3-O7): normalisation, signs, pair
+coefficients c_IJ, axis order, Nyquist handling.
+
+What fixes the result (Eq. 3-4, u_G L121, Eq. 18):
+  the exact force of the model is  F_i = sum_j c_{I J} (d / sigma^2) u_G(|d|),  d = r_i - r_j (all
+  periodic images), which in Fourier space is  F_i = -(1/V) sum_k i k u^(k) sum_J c_IJ S_J(k) e^{ik.r_i}.
+  The particle-mesh result differs from it only through the assignment function W:
+  (a) for particles sitting exactly at stencil centres the mesh sums are closed forms, so PM must equal
+      a mesh-free k-sum with the discrete transfer factor D(k)^2 to round-off, for every P;
+  (b) for general positions PM equals the k-sum with W^(k)^2 = prod sinc(k h/2)^(2P) up to aliasing,
+      which falls quickly with P and under grid refinement;
+  (c) PM converges to the bare analytic pair force as O(h^2);
+  (d) the net non-bonded force is zero.
+The k-sums and pair sums below are brute force written from those formulas, independent of the oracle.
+"""
+import numpy as np
+import pytest
+
+from oracle import tild_oracle as orc
+
+
+def c_matrix(chi, kappa, rho0):
+    S = chi.shape[0]
+    c = np.full((S, S), kappa / rho0)
+    for i in range(S):
+        for j in range(S):
+            if i != j:
+                c[i, j] += chi[i, j] / rho0
+    return c
+
+
+def ksum_force(x, ty, L, N, chi, kappa, rho0, sigma2, transfer):
+    """F_i = -(1/V) sum_m i k_grad u^(k) T(k) sum_J c_IJ S_J(k) exp(i k.r_i) over the grid's mode set.
+    transfer(kx, ky, kz, h) -> T(k).  Nyquist modes: +pi N/L in u^, 0 in the gradient factor (A6)."""
+    x = np.asarray(x, dtype=np.float64)
+    L = np.asarray(L, dtype=np.float64)
+    V = L.prod()
+    S = chi.shape[0]
+    c = c_matrix(chi, kappa, rho0)
+    ks, kg = [], []
+    for a in range(3):
+        m = np.arange(N[a])
+        mt = np.where(m <= N[a] // 2, m, m - N[a])
+        k = 2 * np.pi * mt / L[a]
+        g = k.copy()
+        if N[a] % 2 == 0:
+            g[N[a] // 2] = 0.0
+        ks.append(k)
+        kg.append(g)
+    KX, KY, KZ = np.meshgrid(*ks, indexing="ij")
+    GX, GY, GZ = np.meshgrid(*kg, indexing="ij")
+    uhat = np.exp(-0.5 * sigma2 * (KX ** 2 + KY ** 2 + KZ ** 2))
+    T = transfer(KX, KY, KZ, L / np.asarray(N))
+    # structure factors S_J(k) = sum_{j in J} exp(-i k.r_j)
+    phase = lambda r: np.exp(-1j * (KX * r[0] + KY * r[1] + KZ * r[2]))
+    SJ = np.zeros((S,) + KX.shape, dtype=np.complex128)
+    for j in range(x.shape[0]):
+        SJ[ty[j]] += phase(x[j])
+    F = np.zeros((x.shape[0], 3))
+    for i in range(x.shape[0]):
+        gI = sum(c[ty[i], J] * SJ[J] for J in range(S))
+        common = uhat * T * gI * np.conj(phase(x[i]))
+        for a, G in enumerate((GX, GY, GZ)):
+            F[i, a] = (-(1j * G) * common).sum().real / V
+    return F
+
+
+def direct_pair_force(x, ty, L, chi, kappa, rho0, sigma2, images=2):
+    """F_i = sum_j sum_images c_IJ (d/sigma^2) u_G(|d|); self-image terms cancel pairwise."""
+    x = np.asarray(x, dtype=np.float64)
+    L = np.asarray(L, dtype=np.float64)
+    c = c_matrix(chi, kappa, rho0)
+    n = x.shape[0]
+    F = np.zeros((n, 3))
+    rng = range(-images, images + 1)
+    norm = (2 * np.pi * sigma2) ** -1.5
+    for i in range(n):
+        for j in range(n):
+            for ax in rng:
+                for ay in rng:
+                    for az in rng:
+                        d = x[i] - x[j] + np.array([ax, ay, az]) * L
+                        r2 = (d ** 2).sum()
+                        F[i] += c[ty[i], ty[j]] * d / sigma2 * norm * np.exp(-r2 / (2 * sigma2))
+    return F
+
+
+def discrete_transfer(P):
+    """Mesh transfer of a particle at its stencil centre (t = 0): sum_j w_j exp(-i k node_j)."""
+    def d1(kh):
+        if P == 1:
+            return np.ones_like(kh)
+        if P == 2:
+            return np.cos(kh / 2)
+        if P == 3:
+            return 0.75 + 0.25 * np.cos(kh)
+        if P == 4:
+            return (23.0 / 24.0) * np.cos(kh / 2) + (1.0 / 24.0) * np.cos(1.5 * kh)
+        raise ValueError
+    return lambda KX, KY, KZ, h: (d1(KX * h[0]) * d1(KY * h[1]) * d1(KZ * h[2])) ** 2
+
+
+def sinc_transfer(P):
+    s = lambda kh: np.sinc(kh / (2 * np.pi))                     # numpy sinc(x) = sin(pi x)/(pi x)
+    return lambda KX, KY, KZ, h: (s(KX * h[0]) * s(KY * h[1]) * s(KZ * h[2])) ** (2 * P)
+
+
+CHI3 = np.array([[0.0, 1.0, 0.3], [1.0, 0.0, 2.0], [0.3, 2.0, 0.0]])
+
+
+@pytest.mark.parametrize("P", [1, 2, 3, 4])
+def test_lattice_particles_equal_closed_form_ksum(P):
+    """(a) exact to round-off; non-cubic box and grid so a transposed axis fails."""
+    rng = np.random.default_rng(100 + P)
+    L, N = (6.0, 4.5, 7.0), (12, 8, 10)
+    h = np.array(L) / np.array(N)
+    n = 14
+    cells = np.stack([rng.integers(0, N[a], size=n) for a in range(3)], axis=1)
+    off = 0.0 if P % 2 == 1 else 0.5
+    x = ((cells + off) * h).astype(np.float32).astype(np.float64)
+    # positions must be exactly representable so that fl32(x * inv_h) gives t = 0: use h-friendly box
+    ty = rng.integers(0, 3, size=n).astype(np.int32)
+    p = orc.OracleParams(n, 3, L, N, P, CHI3, kappa=5.0, sigma2=0.5, rho0=2.0)
+    base, toff, _ = orc.index_map(p, x)
+    assert np.abs(toff).max() < 1e-6
+    F = orc.nonbonded_force(p, x, ty)
+    ref = ksum_force(x, ty, L, N, CHI3, 5.0, 2.0, 0.5, discrete_transfer(P))
+    scale = np.sqrt((ref ** 2).sum(1).mean())
+    assert scale > 1e-3
+    assert np.abs(F - ref).max() < 2e-6 * scale      # fp32 positions: |t| <= 1e-6 instead of exactly 0
+
+
+@pytest.mark.parametrize("P,bound_coarse,bound_fine", [(2, 0.4, 0.08), (3, 0.08, 0.01), (4, 0.03, 0.0015)])
+def test_general_positions_vs_sinc_smeared_ksum(P, bound_coarse, bound_fine):
+    """(b) PM = k-sum with W^(k)^2 up to aliasing; the error falls by > 2^P when h is halved."""
+    rng = np.random.default_rng(7)
+    L = (5.0, 5.0, 5.0)
+    n = 10
+    x = (rng.random((n, 3)) * 5.0).astype(np.float32)
+    ty = rng.integers(0, 2, size=n).astype(np.int32)
+    chi = np.array([[0.0, 1.0], [1.0, 0.0]])
+    errs = []
+    for Ng in (8, 16):
+        N = (Ng,) * 3
+        p = orc.OracleParams(n, 2, L, N, P, chi, kappa=3.0, sigma2=0.5, rho0=2.0)
+        F = orc.nonbonded_force(p, x, ty)
+        ref = ksum_force(x, ty, L, N, chi, 3.0, 2.0, 0.5, sinc_transfer(P))
+        errs.append(np.abs(F - ref).max() / np.sqrt((ref ** 2).sum(1).mean()))
+    assert errs[0] < bound_coarse and errs[1] < bound_fine, errs
+    assert errs[0] / errs[1] > 2 ** P, errs
+
+
+def test_single_gaussian_pair_converges_to_analytic_force():
+    """(c) one A-B pair, chi = 1, kappa = 0 (SURVEY pins): PM -> (chi/rho0) (d/sigma^2) u_G(d) as O(h^2)."""
+    L = (10.0, 10.0, 10.0)
+    x = np.array([[4.1, 5.2, 4.9], [4.9, 4.7, 5.3]], dtype=np.float32)
+    ty = np.array([0, 1], dtype=np.int32)
+    chi = np.array([[0.0, 1.0], [1.0, 0.0]])
+    ref = direct_pair_force(x, ty, L, chi, 0.0, 2.0, 0.5, images=1)
+    assert np.allclose(ref[0], -ref[1])
+    errs = []
+    for Ng in (16, 32, 64):
+        p = orc.OracleParams(2, 2, L, (Ng,) * 3, 4, chi, kappa=0.0, sigma2=0.5, rho0=2.0)
+        F = orc.nonbonded_force(p, x, ty)
+        errs.append(np.abs(F - ref).max() / np.abs(ref).max())
+    # h = 0.625, 0.3125, 0.156: relative error O(P h^2 / (6 sigma^2)) -> 4x per halving
+    assert errs[2] < 0.06, errs
+    assert 2.5 < errs[0] / errs[1] < 5.5 and 3.3 < errs[1] / errs[2] < 4.7, errs   # asymptotically 4
+    # direction and sign: repulsive along d
+    d = (x[0] - x[1]).astype(np.float64)
+    assert np.dot(F[0], d) > 0 and np.dot(F[1], d) < 0
+
+
+def test_direct_pair_sum_equals_full_ksum():
+    """The brute-force references agree with each other (periodic Gaussian pair sum == k-sum with T = 1 on a
+    mode set large enough that u^ has decayed): ties the k-space convention to real space."""
+    rng = np.random.default_rng(1)
+    L = (4.0, 4.0, 4.0)
+    n = 5
+    x = rng.random((n, 3)) * 4.0
+    ty = rng.integers(0, 2, size=n).astype(np.int32)
+    chi = np.array([[0.0, 0.7], [0.7, 0.0]])
+    one = lambda KX, KY, KZ, h: np.ones_like(KX)
+    a = ksum_force(x, ty, L, (21, 21, 21), chi, 2.0, 1.5, 0.5, one)     # odd N: no Nyquist special case
+    b = direct_pair_force(x, ty, L, chi, 2.0, 1.5, 0.5, images=3)
+    assert np.abs(a - b).max() < 1e-9 * np.abs(b).max()
+
+
+@pytest.mark.parametrize("P", [1, 2, 3, 4])
+def test_zero_net_force_and_self_force(P):
+    """(d) momentum conservation to round-off (needs A6), and a lone particle feels no force."""
+    rng = np.random.default_rng(21)
+    L, N = (6.0, 4.5, 7.0), (12, 8, 10)
+    n = 200
+    x = (rng.random((n, 3)) * np.array(L)).astype(np.float32)
+    ty = rng.integers(0, 3, size=n).astype(np.int32)
+    p = orc.OracleParams(n, 3, L, N, P, CHI3, kappa=5.0, sigma2=0.5, rho0=2.0)
+    F = orc.nonbonded_force(p, x, ty)
+    rms = np.sqrt((F ** 2).sum(1).mean())
+    assert np.abs(F.sum(0)).max() < 1e-12 * rms * n
+    p1 = orc.OracleParams(1, 3, L, N, P, CHI3, kappa=5.0, sigma2=0.5, rho0=2.0)
+    F1 = orc.nonbonded_force(p1, x[:1], ty[:1])
+    assert np.abs(F1).max() < 1e-13
+
+
+def test_kappa_only_force_is_species_blind_and_chi_is_antisymmetric_for_pair():
+    rng = np.random.default_rng(4)
+    L, N = (5.0,) * 3, (10,) * 3
+    x = (rng.random((30, 3)) * 5.0).astype(np.float32)
+    ty = rng.integers(0, 2, size=30).astype(np.int32)
+    zero = np.zeros((2, 2))
+    p = orc.OracleParams(30, 2, L, N, 3, zero, kappa=4.0, sigma2=0.5, rho0=2.0)
+    Fa = orc.nonbonded_force(p, x, ty)
+    Fb = orc.nonbonded_force(p, x, 1 - ty)
+    assert np.allclose(Fa, Fb, atol=1e-12)
+    # force is linear in the coefficients: F(kappa, chi) = F(kappa, 0) + F(0, chi)
+    chi = np.array([[0.0, 1.3], [1.3, 0.0]])
+    pc = orc.OracleParams(30, 2, L, N, 3, chi, kappa=0.0, sigma2=0.5, rho0=2.0)
+    pkc = orc.OracleParams(30, 2, L, N, 3, chi, kappa=4.0, sigma2=0.5, rho0=2.0)
+    assert np.allclose(orc.nonbonded_force(pkc, x, ty), Fa + orc.nonbonded_force(pc, x, ty), atol=1e-11)
+
+
+def test_force_is_minus_gradient_of_mesh_energy_up_to_discretisation():
+    """O10 vs O5-O7: central difference of the mesh energy along a particle coordinate approaches the
+    ik-differentiated force as the grid is refined (they are not identical on a mesh)."""
+    rng = np.random.default_rng(8)
+    L = (5.0,) * 3
+    n = 12
+    x = (rng.random((n, 3)) * 5.0)
+    ty = rng.integers(0, 2, size=n).astype(np.int32)
+    chi = np.array([[0.0, 1.0], [1.0, 0.0]])
+    bp = -np.ones((n, 2), dtype=np.int32)
+    v = np.zeros((n, 3))
+    rel = []
+    for Ng in (10, 20):
+        p = orc.OracleParams(n, 2, L, (Ng,) * 3, 4, chi, kappa=3.0, sigma2=0.5, rho0=2.0, k_bond=0.0)
+        F = orc.nonbonded_force(p, x.astype(np.float32), ty)
+        eps = 1e-3
+        xp, xm = x.copy(), x.copy()
+        xp[3, 1] += eps
+        xm[3, 1] -= eps
+        dE = (orc.energy(p, xp, v, ty, bp)[2] - orc.energy(p, xm, v, ty, bp)[2]) / (2 * eps)
+        rel.append(abs(-dE - F[3, 1]) / np.abs(F[3]).max())
+    assert rel[1] < 0.02 and rel[1] < rel[0], rel
