@@ -1,0 +1,274 @@
+#!/usr/bin/env python
+"""bench.py -- particle-steps/s of the TILD particle-mesh step on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C4] [--impl ours|reference]
+    python -m torch.distributed.run --nnodes=1 --nproc-per-node N ... bench.py --gpus N ...
+
+One "step" = one pass of the whole hot path (sort cadence, spread, R2C, fused k-space, C2R, interpolation +
+bonds + GJF) over the workload's particles.  Default workload: C4 (8,388,608 particles, 256^3 grid, P=4),
+the configuration the BASELINE metric's roofline target is quoted on; it fits one GPU.  Multi-GPU is
+"replicas only": every rank runs an independent replica, no data-path collective.
+
+`--impl reference` times the CPU oracle (oracle/, as it stands) on the host cores on a bounded sample of the
+same workload; it is a deliberately slow baseline, not the target.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_2302_02474_b200 import inputs  # noqa: E402
+
+METRIC = "particle_steps_per_sec"
+UNIT = "particle-steps/s"
+
+
+def measured_peak_gbs():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def algorithmic_bytes(cfg):
+    """SURVEY 8(d) / DESIGN.md: bytes the method must move per step, per stage."""
+    n, S, M = cfg.n, cfg.n_species, cfg.M
+    Mk = cfg.grid[0] * cfg.grid[1] * (cfg.grid[2] // 2 + 1)
+    return {"spread": 16 * n + 4 * S * M, "kspace": 32 * S * Mk, "interp": 12 * S * M + 52 * n}
+
+
+def sample_config(cfg):
+    """Bounded CPU-baseline sample: the same recipe at 1/64 of the volume and particle count (same density,
+    same h, same P) for the big workloads; the workload itself when it is already small."""
+    if cfg.n <= 70000:
+        return cfg, "the full workload"
+    scale = 1.0 / 64.0
+    box = cfg.box[0] / 4.0
+    grid = cfg.grid[0] // 4
+    s = inputs.scaled(cfg, scale, box, grid, name=cfg.name + "_sample64")
+    return s, (f"same recipe at 1/64 volume: {s.n} particles, box {box:g}^3, grid {grid}^3, P={cfg.order} "
+               f"(same density and mesh spacing)")
+
+
+def run_oracle(cfg, steps, warmup):
+    """Times oracle.run on the host cores.  Returns (particle-steps/s, ms/step, cores)."""
+    from oracle import tild_oracle as orc
+    st = inputs.make_state(cfg)
+    p = orc.OracleParams(cfg.n, cfg.n_species, cfg.box, cfg.grid, cfg.order, np.array(cfg.chi), cfg.kappa, cfg.sigma2,
+                         k_bond=cfg.k_bond, r0_bond=cfg.r0_bond, dt=cfg.dt, gamma=cfg.gamma, kT=cfg.kT, mass=cfg.mass,
+                         seed=cfg.philox_seed)
+    x, v = st.x.astype(np.float64), st.v.astype(np.float64)
+    f = orc.force(p, x, st.type, st.bond_partner)
+    if warmup > 0:
+        x, v, f = orc.run(p, x, v, st.type, st.bond_partner, 0, warmup, f=f)
+    t0 = time.perf_counter()
+    x, v, f = orc.run(p, x, v, st.type, st.bond_partner, warmup, steps, f=f)
+    dt = time.perf_counter() - t0
+    return cfg.n * steps / dt, 1e3 * dt / steps, orc.get_threads()
+
+
+class ClockSampler:
+    """Samples nvidia-smi clocks and throttle reasons during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            threading.Thread(target=self._read, daemon=True).start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm, mx, reasons = [], None, set()
+        for r in self.rows:
+            try:
+                sm.append(float(r[0]))
+                mx = float(r[1])
+                for name, val in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[3:7]):
+                    if val.lower().startswith("active"):
+                        reasons.add(name)
+            except Exception:
+                pass
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": mx, "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+def reference_arm(args, cfg):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    scfg, what = sample_config(cfg)
+    value, ms, cores = run_oracle(scfg, max(1, args.steps), max(0, args.warmup))
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": cfg.name, "sample": what},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": what},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }))
+
+
+def ours_arm(args, cfg):
+    import torch
+    from paper_2302_02474_b200 import tild
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # independent replica per rank: same recipe, rank-specific seeds
+    st = inputs.make_state(cfg, seed=cfg.input_seed + 7919 * rank)
+    eng = tild.Tild(tild.params_from_config(cfg, flags=tild.FLAG_TIMING, seed=cfg.philox_seed + rank,
+                                            resort_every=args.resort_every), device=f"cuda:{local}")
+    xd, vd = torch.from_numpy(st.x).cuda(), torch.from_numpy(st.v).cuda()
+    td, bd = torch.from_numpy(st.type).cuda(), torch.from_numpy(st.bond_partner).cuda()
+    eng.tild_set_state(xd, vd, td, bd, 0)
+    eng.tild_step(args.warmup)
+    eng.tild_get_timings()                         # synchronises and clears the stage timers
+    stream = torch.cuda.current_stream()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    sampler = ClockSampler(local)
+    sampler.start()
+    barrier()
+    l0 = eng.tild_launch_count()
+    e0.record(stream)
+    eng.tild_step(args.steps)
+    e1.record(stream)
+    barrier()
+    launches = eng.tild_launch_count() - l0
+    clocks = sampler.stop()
+    ms_total = e0.elapsed_time(e1)
+    if dist is not None:
+        t = torch.tensor([ms_total], device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total = float(t.item())
+    stage_ms, nst = eng.tild_get_timings()
+    value = world * cfg.n * args.steps / (ms_total * 1e-3)
+
+    # end to end through the C-ABI with HOST buffers: every step copies the batch in and the result out
+    e2e = None
+    if not args.no_e2e:
+        xh, vh = torch.from_numpy(st.x.copy()).pin_memory(), torch.from_numpy(st.v.copy()).pin_memory()
+        th, bh = torch.from_numpy(st.type.copy()).pin_memory(), torch.from_numpy(st.bond_partner.copy()).pin_memory()
+        reps = max(1, min(args.steps, args.e2e_steps))
+        eng.tild_run_host(xh, vh, th, bh, 0, 1)    # warm-up
+        barrier()
+        t0 = time.perf_counter()
+        for r in range(reps):
+            eng.tild_run_host(xh, vh, th, bh, r, 1)   # synchronous: H2D + set_state + 1 step + D2H
+        barrier()
+        dt = time.perf_counter() - t0
+        if dist is not None:
+            t = torch.tensor([dt], device="cuda")
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            dt = float(t.item())
+        e2e = {"value": world * cfg.n * reps / dt, "unit": UNIT,
+               "h2d_bytes_per_step": int(xh.nbytes + vh.nbytes + th.nbytes + bh.nbytes),
+               "d2h_bytes_per_step": int(xh.nbytes + vh.nbytes), "steps": reps,
+               "note": "tild_run_host(nsteps=1) per step: H2D of (x,v,type,bonds), sort, F(x), one step, v/x read back"}
+
+    if rank != 0:
+        return
+    peak, peak_src = measured_peak_gbs()
+    alg = algorithmic_bytes(cfg)
+    stages = {}
+    for k in ("spread", "kspace", "interp"):
+        gbs = alg[k] / (stage_ms[k] * 1e-3) / 1e9 if stage_ms[k] > 0 else 0.0
+        stages[k] = {"ms": stage_ms[k], "alg_bytes": alg[k], "gbs": gbs, "frac": gbs / peak}
+    dom = max(stages, key=lambda k: stages[k]["ms"])
+    three_ms = sum(stages[k]["ms"] for k in stages)
+    three_gbs = sum(alg.values()) / (three_ms * 1e-3) / 1e9 if three_ms > 0 else 0.0
+    roofline = {"bound": "hbm", "kernel": dom, "achieved": stages[dom]["gbs"], "peak": peak, "unit": "GB/s",
+                "frac": stages[dom]["gbs"] / peak, "traffic": NCU_TRAFFIC.get((cfg.name, dom)), "peak_source": peak_src,
+                "stages": stages,
+                "spread_kspace_interp": {"ms": three_ms, "gbs": three_gbs, "frac": three_gbs / peak,
+                                         "frac_of_8TBs_nominal": three_gbs / 8000.0}}
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        scfg, what = sample_config(cfg)
+        _, ms1, cores = run_oracle(scfg, 1, 0)
+        k = int(min(50, max(2, 12e3 / max(ms1, 1e-3))))
+        val, _, cores = run_oracle(scfg, k, 0)
+        cpu = {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": f"{what}; {k} steps"}
+    print(json.dumps({
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic",
+        "config": {"workload": cfg.name, "n": cfg.n, "grid": list(cfg.grid), "order": cfg.order, "species": cfg.n_species,
+                   "resort_every": args.resort_every, "l2": "inputs larger than L2 (no flush needed)"
+                   if sum(alg.values()) > 2 * 126e6 else "working set fits L2; steady-state numbers",
+                   "parallelism": "replicas only" if world > 1 else "single GPU"},
+        "stage_ms": stage_ms, "stage_steps_timed": nst,
+        "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
+    }))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from `ncu --set full` captures committed under profiles/
+# (key: (workload name, stage)); None until a capture exists.
+NCU_TRAFFIC = {}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="C4", choices=sorted(inputs.CONFIGS))
+    ap.add_argument("--resort-every", type=int, default=0)
+    ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 0)
+    cfg = inputs.CONFIGS[args.workload]
+    if args.impl == "reference":
+        reference_arm(args, cfg)
+    else:
+        ours_arm(args, cfg)
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,150 @@
+/*
+ * tild.h -- C-ABI of the B200-native TILD particle-mesh force path.
+ *
+ * The method is the per-time-step "Particle-to-Mesh" non-bonded force evaluation of
+ * Theoretically-Informed Langevin Dynamics as described in PAPER.md (arxiv 2302.02474,
+ * MATILDA.FT) section IV.C "Long-range interactions" (L221-231, Eq. 18, Fig. 1), applied to the
+ * model of section III (Eq. 1-4; smearing L139-149), plus harmonic bonds (Eq. 2,
+ * IV.B L207-209) and the GJF Langevin integrator (VI.B.6 L346-352).  The paper defines no API
+ * (its user surface is an input script, L58-90); the arguments below follow its statement of the
+ * model.  Readings of points where the paper is silent are listed in DESIGN.md ("A<n>").
+ *
+ * Conventions
+ *  - Unless marked HOST, every pointer argument is a DEVICE pointer owned by the caller (e.g. a
+ *    torch tensor's data_ptr).  The library never frees or reallocates caller memory.
+ *  - `workspace` is caller-allocated device memory of at least tild_workspace_bytes() bytes,
+ *    256-byte aligned, borrowed until tild_destroy().  The context owns only its cuFFT plans
+ *    (and their work areas), CUDA events and host bookkeeping.
+ *  - All calls enqueue on the `cuda_stream` given to tild_init (a cudaStream_t; NULL = legacy
+ *    default stream) and return without synchronising, except where stated.
+ *  - Layouts: positions/velocities/forces AoS [n][3] float (x[ind*Dim+j]);
+ *    grids [species][Nx][Ny][Nz] float, z fastest, linear node index g = (ix*Ny + iy)*Nz + iz;
+ *    force fields [species][3][Nx][Ny][Nz].  Box is [0,L) per axis, periodic, node g at g*h.
+ *  - Return value: 0 on success, negative tild_status on failure; tild_last_error() gives text.
+ *    No exceptions, no output to stdout/stderr, no global mutable state.
+ *  - There is no CPU fallback: every entry point that computes needs a CUDA device.
+ */
+#ifndef TILD_H
+#define TILD_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define TILD_MAX_SPECIES 8
+#define TILD_MAX_BONDS 4
+
+typedef enum {
+    TILD_OK = 0,
+    TILD_EINVAL = -1,  /* bad sizes / order / non-positive box / struct_size mismatch / NULL */
+    TILD_ENOMEM = -2,  /* workspace too small or misaligned */
+    TILD_ECUDA = -3,   /* a CUDA runtime call failed */
+    TILD_ECUFFT = -4,  /* a cuFFT call failed */
+    TILD_ESTATE = -5   /* tild_step / tild_get_state before tild_set_state */
+} tild_status;
+
+/* flags */
+#define TILD_FLAG_TIMING 1u        /* record CUDA events around every stage of tild_step */
+#define TILD_FLAG_NAIVE_SPREAD 2u  /* per-particle global-atomic spread (baseline kernel) */
+#define TILD_FLAG_NAIVE_INTERP 4u  /* per-particle global-gather interpolation (baseline kernel) */
+
+typedef struct tild_ctx tild_ctx;
+
+/* The model statement.  PAPER.md: box L54; grid Nx,Ny,Nz and pmeorder Listing 1 L69-78; species,
+ * chi_ij, kappa Eq. 3-4; Gaussian range L121/L139-143; bonds Eq. 2; delt L71;
+ * integrator L82/L352; reduced units (kT, m, b) L100. */
+typedef struct {
+    uint32_t struct_size;      /* = sizeof(tild_params) */
+    int32_t n;                 /* particles, >= 0 */
+    int32_t n_species;         /* S, 1..TILD_MAX_SPECIES */
+    int32_t order;             /* P = grid nodes touched per dimension, 1..4 (A1: P=2 is the paper's Fig. 1) */
+    double box[3];             /* L > 0 */
+    int32_t grid[3];           /* N >= P, each; any size cuFFT accepts (2,3,5,7 factors are fast) */
+    int32_t max_bonds;         /* bond partner slots per particle, 0..TILD_MAX_BONDS */
+    double chi[TILD_MAX_SPECIES * TILD_MAX_SPECIES]; /* chi[I*8+J], symmetric, diagonal ignored */
+    double kappa;              /* Helfand compressibility, Eq. 4 */
+    double a;                  /* smearing length of h(r), L139; used when sigma2 <= 0 */
+    double sigma2;             /* variance of u_G (L121); <= 0 -> 2 a^2 (L143) */
+    double rho0;               /* <= 0 -> n / V (L121) */
+    double k_bond, r0_bond;    /* U_bond = k (|d| - r0)^2; Eq. 2 has k = 3/(2 b^2), r0 = 0 */
+    double dt, gamma, kT, mass;/* GJF parameters (A11) */
+    uint64_t seed;             /* Philox4x32-10 key (A12) */
+    int32_t resort_every;      /* physically re-sort particles by cell every this many steps; <= 0 -> default */
+    uint32_t flags;            /* TILD_FLAG_* */
+} tild_params;
+
+/* HOST. Bytes of device workspace tild_init needs for these parameters. */
+int tild_workspace_bytes(const tild_params* params /*HOST*/, size_t* bytes /*HOST out*/);
+
+/* HOST+DEVICE. a0: builds the k-space tables k_a(m), exp(-sigma2 k_a^2/2) and the
+ * coefficient matrix c'_IJ = c_IJ / V in double on the host, uploads them as fp32, creates the
+ * batched cuFFT plans (R2C x S, C2R x 3S).  PAPER.md L223 ("Fourier-space representation of the
+ * inter-particle potential is calculated ... and stored"); analytic u^(k) per A5. */
+int tild_init(tild_ctx** out /*HOST out*/, const tild_params* params /*HOST*/, void* workspace,
+              size_t workspace_bytes, void* cuda_stream);
+
+/* Loads (x, v) at step index step0, sorts particles by cell, evaluates F(x) once and forms the
+ * split-kick state w = v - (dt/2m) F.  bond_partner may be NULL iff
+ * max_bonds == 0.  Particle i keeps id i for the noise counter whatever the internal order. */
+int tild_set_state(tild_ctx*, const float* x /*[n][3], in [0,L]*/, const float* v /*[n][3]*/,
+                   const int32_t* type /*[n], 0..S-1*/, const int32_t* bond_partner /*[n][max_bonds], -1 = none*/,
+                   uint64_t step0);
+
+/* a1 + a2: spread.  grid[J][g] = sum_{i: type_i = J} W_x W_y W_z (raw weights, PAPER.md L223,
+ * Eq. 1).  Pure function of (x, type); overwrites grid. */
+int tild_spread(tild_ctx*, const float* x, const int32_t* type, float* grid /*[S][Nx][Ny][Nz]*/);
+
+/* a3-a5: forward FFT, fused pair-kernel multiply + ik gradient, inverse FFT (Eq. 18):
+ * ffield[I][a][g] = sum_m [-i k_a u^(k_m) sum_J c_IJ n^_J(m) / V] exp(+2 pi i m.g/N). */
+int tild_kspace_force(tild_ctx*, const float* grid /*[S][M]*/, float* ffield /*[S][3][M]*/);
+
+/* a6 (force only): f_i = sum_g W(g; r_i) ffield[type_i][.][g]  (L227, Fig. 1). Non-bonded only. */
+int tild_interp(tild_ctx*, const float* ffield, const float* x, const int32_t* type, float* f /*[n][3]*/);
+
+/* Bond forces alone (Eq. 2), for stage parity: f_i = sum_slots -2k(1 - r0/|d|) d. */
+int tild_bond_force(tild_ctx*, const float* x, const int32_t* bond_partner, float* f /*[n][3]*/);
+
+/* The timed path: (x, v)^t -> (x, v)^{t+nsteps}; each step = a1..a6 with bonds and the GJF
+ * update fused into the interpolation pass.  One force evaluation per step. */
+int tild_step(tild_ctx*, int32_t nsteps);
+
+/* Copies the state out in ORIGINAL particle order.  v and f need one force evaluation at the
+ * current positions (no state change).  Any of x, v, f may be NULL.  step is HOST out, nullable. */
+int tild_get_state(tild_ctx*, float* x, float* v, float* f, uint64_t* step /*HOST*/);
+
+/* a1: index map of arbitrary caller positions.  base[i][a] = first stencil node (unwrapped),
+ * cell_key[i] = (cx*Ny+cy)*Nz+cz, perm = particle ids grouped by ascending cell key (order inside
+ * a cell unspecified), cell_start[c] = #particles with key < c (M+1 entries).  Any output may be NULL. */
+int tild_index_map(tild_ctx*, const float* x, int32_t* base /*[n][3]*/, uint32_t* cell_key /*[n]*/,
+                   uint32_t* perm /*[n]*/, uint32_t* cell_start /*[M+1]*/);
+
+/* HOST, synchronises.  Mean milliseconds per step over the tild_step calls since the last call
+ * (needs TILD_FLAG_TIMING): sort, spread (incl. zero fill), fft_fwd, kspace, fft_inv, interp(+bonds
+ * +GJF), other, total.  steps_timed (nullable) receives how many steps the means cover. */
+int tild_get_timings(tild_ctx*, float ms[8] /*HOST out*/, int32_t* steps_timed /*HOST out*/);
+
+/* HOST buffers, synchronises: the end-to-end call.  Copies (x, v, type, bond_partner) host->device,
+ * runs tild_set_state + tild_step(nsteps), copies (x, v) back.  Buffers should be pinned for speed. */
+int tild_run_host(tild_ctx*, float* x_host, float* v_host, const int32_t* type_host,
+                  const int32_t* bond_partner_host, uint64_t step0, int32_t nsteps);
+
+/* Test hook: out[i] = Philox4x32-10(counter = ctr[i], key = key[i]) computed by the same device
+ * function the integrator uses; gauss[i] = the three N(0,1) draws for (id = ctr[i].x, step =
+ * ctr[i].y | ctr[i].z << 32) under key[i].  gauss may be NULL. */
+int tild_philox_test(tild_ctx*, const uint32_t* ctr /*[m][4]*/, const uint32_t* key /*[m][2]*/,
+                     uint32_t* out /*[m][4]*/, float* gauss /*[m][3]*/, int32_t m);
+
+/* HOST. Number of kernels of this library launched on the context's stream so far. */
+int64_t tild_launch_count(const tild_ctx*);
+
+const char* tild_last_error(const tild_ctx*); /* HOST; valid until the next call on the context */
+void tild_destroy(tild_ctx*);
+const char* tild_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TILD_H */

@@ -507,7 +507,8 @@ void orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t ou
 }
 
 /* beta^{step} for particle id: counter = (id, step_lo, step_hi, 0), key = (seed_lo, seed_hi);
- * u_k = ((x_k >> 8) + 0.5) 2^-24;  Box-Muller;  beta = sqrt(2 gamma kT dt) (z0, z1, z2). */
+ * u_k = ((x_k >> 9) + 0.5) 2^-23 (24 significant bits: exact in fp32 and fp64, never 0 or 1);  Box-Muller:
+ * z0 = sqrt(-2 ln u0) cos 2 pi u1, z1 = sqrt(-2 ln u0) sin 2 pi u1, z2 = sqrt(-2 ln u2) cos 2 pi u3;  beta = sqrt(2 gamma kT dt) (z0, z1, z2). */
 void orc_noise(const orc_params *p, uint32_t id, uint64_t step, double beta[3])
 {
     uint32_t ctr[4] = {id, (uint32_t)(step & 0xffffffffu), (uint32_t)(step >> 32), 0u};
@@ -515,7 +516,7 @@ void orc_noise(const orc_params *p, uint32_t id, uint64_t step, double beta[3])
     uint32_t r[4];
     orc_philox4x32_10(ctr, key, r);
     double u[4];
-    for (int k = 0; k < 4; ++k) u[k] = ((double)(r[k] >> 8) + 0.5) * (1.0 / 16777216.0);
+    for (int k = 0; k < 4; ++k) u[k] = ((double)(r[k] >> 9) + 0.5) * (1.0 / 8388608.0);
     double r01 = sqrt(-2.0 * log(u[0])), r23 = sqrt(-2.0 * log(u[2]));
     double z0 = r01 * cos(2.0 * ORC_PI * u[1]);
     double z1 = r01 * sin(2.0 * ORC_PI * u[1]);

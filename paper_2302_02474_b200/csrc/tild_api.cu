@@ -1,0 +1,445 @@
+// C-ABI of libtild (include/tild.h): context, workspace carving, cuFFT plans, stage calls and the timed step.
+#include <math.h>
+#include <stdarg.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include <new>
+#include <vector>
+
+#include "tild_internal.cuh"
+
+int tild_fail(tild_ctx* c, int code, const char* fmt, ...)
+{
+    if (c) {
+        va_list ap;
+        va_start(ap, fmt);
+        vsnprintf(c->err, sizeof(c->err), fmt, ap);
+        va_end(ap);
+    }
+    return code;
+}
+
+namespace {
+
+constexpr size_t ALIGN = 256;
+inline size_t up(size_t b) { return (b + ALIGN - 1) / ALIGN * ALIGN; }
+
+// Walks the workspace layout; with base == nullptr it only measures.
+struct Carver {
+    char* base;
+    size_t off = 0;
+    explicit Carver(void* b) : base(static_cast<char*>(b)) {}
+    template <typename T>
+    T* take(size_t count)
+    {
+        T* p = base ? reinterpret_cast<T*>(base + off) : nullptr;
+        off += up(count * sizeof(T) + 16);
+        return p;
+    }
+};
+
+int validate(const tild_params* p)
+{
+    if (!p || p->struct_size != sizeof(tild_params)) return TILD_EINVAL;
+    if (p->n < 0 || p->n_species < 1 || p->n_species > TILD_MAX_SPECIES) return TILD_EINVAL;
+    if (p->order < 1 || p->order > 4) return TILD_EINVAL;
+    if (p->max_bonds < 0 || p->max_bonds > TILD_MAX_BONDS) return TILD_EINVAL;
+    double M = 1.0;
+    for (int a = 0; a < 3; ++a) {
+        if (!(p->box[a] > 0.0) || p->grid[a] < p->order || p->grid[a] < 2 || p->grid[a] > 4096) return TILD_EINVAL;
+        M *= p->grid[a];
+    }
+    if (M > 2.0e9) return TILD_EINVAL;
+    if (!(p->sigma2 > 0.0) && !(p->a > 0.0)) return TILD_EINVAL;
+    if (!(p->dt > 0.0) || !(p->mass > 0.0) || p->gamma < 0.0 || p->kT < 0.0) return TILD_EINVAL;
+    return TILD_OK;
+}
+
+void carve(tild_ctx* c, void* base, size_t* total)
+{
+    const tild_params& p = c->prm;
+    const size_t n = (size_t)p.n, S = (size_t)p.n_species;
+    const size_t M = (size_t)p.grid[0] * p.grid[1] * p.grid[2];
+    const size_t Mk = (size_t)p.grid[0] * p.grid[1] * (p.grid[2] / 2 + 1);
+    const size_t nb = n * (size_t)(p.max_bonds > 0 ? p.max_bonds : 1);
+    Carver w(base);
+    for (int k = 0; k < 2; ++k) {
+        c->x[k] = w.take<float>(3 * n);
+        c->w[k] = w.take<float>(3 * n);
+        c->type[k] = w.take<int32_t>(n);
+        c->id[k] = w.take<uint32_t>(n);
+        c->bond[k] = w.take<int32_t>(nb);
+    }
+    c->grid = w.take<float>(S * M);
+    c->nhat = w.take<float2>(S * Mk);
+    c->fhat = w.take<float2>(3 * S * Mk);
+    c->ffield = w.take<float>(3 * S * M);
+    c->fpart = w.take<float>(3 * n);
+    c->key = w.take<uint32_t>(n);
+    c->perm = w.take<uint32_t>(n);
+    c->cell_start = w.take<uint32_t>(M + 1);
+    c->cell_fill = w.take<uint32_t>(M + 1);
+    c->scan_part = w.take<uint32_t>(tild_scan_scratch_entries(M, p.n));
+    c->tables = w.take<float>(6 * 4096);
+    *total = w.off;
+}
+
+__global__ void iota_kernel(int n, uint32_t* id)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) id[i] = (uint32_t)i;
+}
+
+#define TILD_FFT(c, call)                                                                  \
+    do {                                                                                   \
+        cufftResult r__ = (call);                                                          \
+        if (r__ != CUFFT_SUCCESS) return tild_fail((c), TILD_ECUFFT, "%s: cufft error %d", #call, (int)r__); \
+    } while (0)
+
+// spread -> R2C -> k-space -> C2R on the given particle arrays, with optional stage events
+int mesh_pipeline(tild_ctx* c, const float* x, const int32_t* type, cudaEvent_t* ev)
+{
+    int rc = launch_spread(c, x, type, c->grid);
+    if (rc) return rc;
+    if (ev) cudaEventRecord(ev[2], c->stream);
+    TILD_FFT(c, cufftExecR2C(c->plan_r2c, c->grid, reinterpret_cast<cufftComplex*>(c->nhat)));
+    if (ev) cudaEventRecord(ev[3], c->stream);
+    rc = launch_kspace(c, c->nhat, c->fhat);
+    if (rc) return rc;
+    if (ev) cudaEventRecord(ev[4], c->stream);
+    TILD_FFT(c, cufftExecC2R(c->plan_c2r, reinterpret_cast<cufftComplex*>(c->fhat), c->ffield));
+    if (ev) cudaEventRecord(ev[5], c->stream);
+    return TILD_OK;
+}
+
+// total force at the current internal positions -> c->fpart (internal order); no state change
+int force_current(tild_ctx* c)
+{
+    const int a = c->cur;
+    int rc = mesh_pipeline(c, c->x[a], c->type[a], nullptr);
+    if (rc) return rc;
+    rc = launch_interp_force(c, c->ffield, c->x[a], c->type[a], c->fpart);
+    if (rc) return rc;
+    if (c->stp.max_bonds > 0) rc = launch_bond_force(c, c->x[a], c->bond[a], c->fpart, true);
+    return rc;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* tild_version(void) { return "tild-b200 0.1 (sm_100a)"; }
+
+int tild_workspace_bytes(const tild_params* params, size_t* bytes)
+{
+    if (!bytes) return TILD_EINVAL;
+    int rc = validate(params);
+    if (rc) return rc;
+    tild_ctx tmp;
+    memset(&tmp, 0, sizeof(tmp));
+    tmp.prm = *params;
+    carve(&tmp, nullptr, bytes);
+    return TILD_OK;
+}
+
+int tild_init(tild_ctx** out, const tild_params* params, void* workspace, size_t workspace_bytes, void* cuda_stream)
+{
+    if (!out) return TILD_EINVAL;
+    *out = nullptr;
+    int rc = validate(params);
+    if (rc) return rc;
+    if (!workspace || (reinterpret_cast<uintptr_t>(workspace) % ALIGN) != 0) return TILD_ENOMEM;
+    tild_ctx* c = new (std::nothrow) tild_ctx;
+    if (!c) return TILD_ENOMEM;
+    memset(c, 0, sizeof(*c));
+    c->prm = *params;
+    c->stream = static_cast<cudaStream_t>(cuda_stream);
+    size_t need = 0;
+    carve(c, workspace, &need);
+    if (need > workspace_bytes) {
+        delete c;
+        return TILD_ENOMEM;
+    }
+    const tild_params& p = c->prm;
+    const int S = p.n_species;
+    c->M = (size_t)p.grid[0] * p.grid[1] * p.grid[2];
+    c->Mk = (size_t)p.grid[0] * p.grid[1] * (p.grid[2] / 2 + 1);
+    const double V = p.box[0] * p.box[1] * p.box[2];
+    const double sigma2 = p.sigma2 > 0.0 ? p.sigma2 : 2.0 * p.a * p.a;
+    const double rho0 = p.rho0 > 0.0 ? p.rho0 : (double)p.n / V;          // L121
+    c->resort_every = p.resort_every > 0 ? p.resort_every : 20;
+
+    MeshParams& m = c->mesh;
+    m.n = p.n;
+    m.S = S;
+    m.P = p.order;
+    m.M = (long long)c->M;
+    for (int a = 0; a < 3; ++a) {
+        m.N[a] = p.grid[a];
+        m.inv_h[a] = (float)((double)p.grid[a] / p.box[a]);
+        m.L[a] = (float)p.box[a];
+        m.inv_L[a] = (float)(1.0 / p.box[a]);
+    }
+
+    // a0: k-space tables in double on the host (A4-A6), uploaded as fp32
+    std::vector<float> tab(6 * 4096, 0.0f);
+    const double PI = 3.14159265358979323846264338327950288;
+    for (int a = 0; a < 3; ++a) {
+        const int N = p.grid[a];
+        for (int mm = 0; mm < N; ++mm) {
+            const int mt = mm <= N / 2 ? mm : mm - N;
+            const double k = 2.0 * PI * (double)mt / p.box[a];
+            const double kg = (N % 2 == 0 && mm == N / 2) ? 0.0 : k;
+            double u = exp(-0.5 * sigma2 * k * k);
+            if (a == 0) u /= V;
+            tab[(size_t)a * 4096 + mm] = (float)kg;
+            tab[(size_t)(3 + a) * 4096 + mm] = (float)u;
+        }
+    }
+    KspaceParams& ks = c->ksp;
+    ks.S = S;
+    ks.Nzc = p.grid[2] / 2 + 1;
+    for (int a = 0; a < 3; ++a) {
+        ks.N[a] = p.grid[a];
+        ks.kgrad[a] = c->tables + (size_t)a * 4096;
+        ks.ufac[a] = c->tables + (size_t)(3 + a) * 4096;
+    }
+    for (int I = 0; I < S; ++I)
+        for (int J = 0; J < S; ++J) {
+            const double cij = (I == J) ? p.kappa / rho0 : (p.kappa + p.chi[I * TILD_MAX_SPECIES + J]) / rho0;  // A9
+            ks.c[I * TILD_MAX_SPECIES + J] = (float)cij;
+        }
+
+    // GJF constants (A11)
+    StepParams& s = c->stp;
+    const double gh = p.gamma * p.dt / (2.0 * p.mass);
+    const double bg = 1.0 / (1.0 + gh), ag = (1.0 - gh) / (1.0 + gh);
+    s.half_dt_over_m = (float)(p.dt / (2.0 * p.mass));
+    s.a_g = (float)ag;
+    s.b_dt = (float)(bg * p.dt);
+    s.b_dt2_over_2m = (float)(bg * p.dt * p.dt / (2.0 * p.mass));
+    s.b_dt_over_2m = (float)(bg * p.dt / (2.0 * p.mass));
+    s.b_over_m = (float)(bg / p.mass);
+    s.noise_amp = (float)sqrt(2.0 * p.gamma * p.kT * p.dt);
+    s.k_bond = (float)p.k_bond;
+    s.r0_bond = (float)p.r0_bond;
+    s.max_bonds = p.max_bonds;
+    s.key0 = (uint32_t)(p.seed & 0xffffffffu);
+    s.key1 = (uint32_t)(p.seed >> 32);
+
+    cudaError_t e = cudaMemcpyAsync(c->tables, tab.data(), tab.size() * sizeof(float), cudaMemcpyHostToDevice, c->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);  // tab is a stack-owned host buffer
+    if (e != cudaSuccess) {
+        delete c;
+        return TILD_ECUDA;
+    }
+    int dims[3] = {p.grid[0], p.grid[1], p.grid[2]};
+    cufftResult r1 = cufftPlanMany(&c->plan_r2c, 3, dims, nullptr, 1, 0, nullptr, 1, 0, CUFFT_R2C, S);
+    cufftResult r2 = r1 == CUFFT_SUCCESS ? cufftPlanMany(&c->plan_c2r, 3, dims, nullptr, 1, 0, nullptr, 1, 0, CUFFT_C2R, 3 * S)
+                                         : CUFFT_INTERNAL_ERROR;
+    if (r1 != CUFFT_SUCCESS || r2 != CUFFT_SUCCESS) {
+        if (r1 == CUFFT_SUCCESS) cufftDestroy(c->plan_r2c);
+        delete c;
+        return TILD_ECUFFT;
+    }
+    c->plans_ok = true;
+    cufftSetStream(c->plan_r2c, c->stream);
+    cufftSetStream(c->plan_c2r, c->stream);
+    if (p.flags & TILD_FLAG_TIMING) {
+        for (int i = 0; i < TILD_MAX_TIMED_STEPS; ++i)
+            for (int k = 0; k < TILD_N_STAGE_EVENTS; ++k) cudaEventCreate(&c->ev[i][k]);
+        c->ev_ok = true;
+    }
+    *out = c;
+    return TILD_OK;
+}
+
+void tild_destroy(tild_ctx* c)
+{
+    if (!c) return;
+    if (c->plans_ok) {
+        cufftDestroy(c->plan_r2c);
+        cufftDestroy(c->plan_c2r);
+    }
+    if (c->ev_ok)
+        for (int i = 0; i < TILD_MAX_TIMED_STEPS; ++i)
+            for (int k = 0; k < TILD_N_STAGE_EVENTS; ++k) cudaEventDestroy(c->ev[i][k]);
+    delete c;
+}
+
+const char* tild_last_error(const tild_ctx* c) { return c ? c->err : "null context"; }
+int64_t tild_launch_count(const tild_ctx* c) { return c ? c->launches : 0; }
+
+int tild_spread(tild_ctx* c, const float* x, const int32_t* type, float* grid)
+{
+    if (!c || !grid || (c->mesh.n > 0 && (!x || !type))) return tild_fail(c, TILD_EINVAL, "tild_spread: null argument");
+    return launch_spread(c, x, type, grid);
+}
+
+int tild_kspace_force(tild_ctx* c, const float* grid, float* ffield)
+{
+    if (!c || !grid || !ffield) return tild_fail(c, TILD_EINVAL, "tild_kspace_force: null argument");
+    TILD_FFT(c, cufftExecR2C(c->plan_r2c, const_cast<float*>(grid), reinterpret_cast<cufftComplex*>(c->nhat)));
+    int rc = launch_kspace(c, c->nhat, c->fhat);
+    if (rc) return rc;
+    TILD_FFT(c, cufftExecC2R(c->plan_c2r, reinterpret_cast<cufftComplex*>(c->fhat), ffield));
+    return TILD_OK;
+}
+
+int tild_interp(tild_ctx* c, const float* ffield, const float* x, const int32_t* type, float* f)
+{
+    if (!c || !ffield || (c->mesh.n > 0 && (!x || !type || !f))) return tild_fail(c, TILD_EINVAL, "tild_interp: null argument");
+    return launch_interp_force(c, ffield, x, type, f);
+}
+
+int tild_bond_force(tild_ctx* c, const float* x, const int32_t* bond_partner, float* f)
+{
+    if (!c || (c->mesh.n > 0 && (!x || !f))) return tild_fail(c, TILD_EINVAL, "tild_bond_force: null argument");
+    if (c->stp.max_bonds > 0 && !bond_partner && c->mesh.n > 0) return tild_fail(c, TILD_EINVAL, "tild_bond_force: null partners");
+    return launch_bond_force(c, x, bond_partner, f, false);
+}
+
+int tild_index_map(tild_ctx* c, const float* x, int32_t* base, uint32_t* cell_key, uint32_t* perm, uint32_t* cell_start)
+{
+    if (!c || (c->mesh.n > 0 && !x)) return tild_fail(c, TILD_EINVAL, "tild_index_map: null argument");
+    uint32_t* key = cell_key ? cell_key : c->key;
+    int rc = launch_cell_keys(c, x, key, base);
+    if (rc) return rc;
+    if (perm || cell_start) rc = launch_counting_sort(c, key, perm ? perm : c->perm, cell_start ? cell_start : c->cell_start);
+    return rc;
+}
+
+int tild_philox_test(tild_ctx* c, const uint32_t* ctr, const uint32_t* key, uint32_t* out, float* gauss, int32_t m)
+{
+    if (!c || (m > 0 && (!ctr || !key || !out))) return tild_fail(c, TILD_EINVAL, "tild_philox_test: null argument");
+    return launch_philox_test(c, ctr, key, out, gauss, m);
+}
+
+int tild_set_state(tild_ctx* c, const float* x, const float* v, const int32_t* type, const int32_t* bond_partner, uint64_t step0)
+{
+    if (!c) return TILD_EINVAL;
+    const size_t n = (size_t)c->mesh.n;
+    if (n > 0 && (!x || !v || !type)) return tild_fail(c, TILD_EINVAL, "tild_set_state: null argument");
+    if (n > 0 && c->stp.max_bonds > 0 && !bond_partner) return tild_fail(c, TILD_EINVAL, "tild_set_state: null bond_partner");
+    c->cur = 0;
+    if (n > 0) {
+        // cudaMemcpyDefault: the sources may be device (stage API) or host (tild_run_host) pointers
+        TILD_CUDA(c, cudaMemcpyAsync(c->x[0], x, 3 * n * sizeof(float), cudaMemcpyDefault, c->stream));
+        TILD_CUDA(c, cudaMemcpyAsync(c->w[0], v, 3 * n * sizeof(float), cudaMemcpyDefault, c->stream));
+        TILD_CUDA(c, cudaMemcpyAsync(c->type[0], type, n * sizeof(int32_t), cudaMemcpyDefault, c->stream));
+        if (c->stp.max_bonds > 0)
+            TILD_CUDA(c, cudaMemcpyAsync(c->bond[0], bond_partner, n * c->stp.max_bonds * sizeof(int32_t), cudaMemcpyDefault,
+                                         c->stream));
+        iota_kernel<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>((int)n, c->id[0]);
+        TILD_LAUNCH_CHECK(c, "iota_kernel");
+    }
+    int rc = launch_reorder(c);
+    if (rc) return rc;
+    rc = force_current(c);
+    if (rc) return rc;
+    rc = launch_make_w(c, c->fpart, c->w[c->cur], -1.0f);  // w = v - (dt/2m) F
+    if (rc) return rc;
+    c->step = step0;
+    c->has_state = true;
+    c->timed_steps = 0;
+    return TILD_OK;
+}
+
+int tild_step(tild_ctx* c, int32_t nsteps)
+{
+    if (!c) return TILD_EINVAL;
+    if (!c->has_state) return tild_fail(c, TILD_ESTATE, "tild_step before tild_set_state");
+    if (nsteps < 0) return tild_fail(c, TILD_EINVAL, "tild_step: nsteps < 0");
+    for (int32_t s = 0; s < nsteps; ++s) {
+        cudaEvent_t* ev = (c->ev_ok && c->timed_steps < TILD_MAX_TIMED_STEPS) ? c->ev[c->timed_steps] : nullptr;
+        if (ev) cudaEventRecord(ev[0], c->stream);
+        if (c->steps_since_sort >= c->resort_every) {
+            int rc = launch_reorder(c);
+            if (rc) return rc;
+        }
+        if (ev) cudaEventRecord(ev[1], c->stream);
+        int rc = mesh_pipeline(c, c->x[c->cur], c->type[c->cur], ev);
+        if (rc) return rc;
+        rc = launch_fused_step(c);
+        if (rc) return rc;
+        if (ev) {
+            cudaEventRecord(ev[6], c->stream);
+            c->timed_steps++;
+        }
+        c->step++;
+        c->steps_since_sort++;
+    }
+    return TILD_OK;
+}
+
+int tild_get_state(tild_ctx* c, float* x, float* v, float* f, uint64_t* step)
+{
+    if (!c) return TILD_EINVAL;
+    if (!c->has_state) return tild_fail(c, TILD_ESTATE, "tild_get_state before tild_set_state");
+    const size_t n = (size_t)c->mesh.n;
+    const size_t bytes = 3 * n * sizeof(float);
+    if (step) *step = c->step;
+    if (n == 0) return TILD_OK;
+    const int a = c->cur;
+    float* scratch = c->x[1 - a];  // the inactive position buffer is free between steps
+    int rc;
+    if (x) {
+        if ((rc = launch_unpermute(c, c->x[a], scratch, 3))) return rc;
+        TILD_CUDA(c, cudaMemcpyAsync(x, scratch, bytes, cudaMemcpyDefault, c->stream));
+    }
+    if (v || f) {
+        if ((rc = force_current(c))) return rc;
+        if (f) {
+            if ((rc = launch_unpermute(c, c->fpart, scratch, 3))) return rc;
+            TILD_CUDA(c, cudaMemcpyAsync(f, scratch, bytes, cudaMemcpyDefault, c->stream));
+        }
+        if (v) {
+            float* vs = c->w[1 - a];
+            TILD_CUDA(c, cudaMemcpyAsync(vs, c->w[a], bytes, cudaMemcpyDeviceToDevice, c->stream));
+            if ((rc = launch_make_w(c, c->fpart, vs, +1.0f))) return rc;  // v = w + (dt/2m) F
+            if ((rc = launch_unpermute(c, vs, scratch, 3))) return rc;
+            TILD_CUDA(c, cudaMemcpyAsync(v, scratch, bytes, cudaMemcpyDefault, c->stream));
+        }
+    }
+    return TILD_OK;
+}
+
+int tild_get_timings(tild_ctx* c, float ms[8], int32_t* steps_timed)
+{
+    if (!c || !ms) return TILD_EINVAL;
+    for (int k = 0; k < 8; ++k) ms[k] = 0.0f;
+    if (steps_timed) *steps_timed = 0;
+    TILD_CUDA(c, cudaStreamSynchronize(c->stream));
+    if (!c->ev_ok || c->timed_steps == 0) return TILD_OK;
+    const int T = c->timed_steps;
+    for (int i = 0; i < T; ++i) {
+        for (int k = 0; k < 6; ++k) {
+            float t = 0.0f;
+            TILD_CUDA(c, cudaEventElapsedTime(&t, c->ev[i][k], c->ev[i][k + 1]));
+            ms[k] += t;
+        }
+        float tot = 0.0f;
+        TILD_CUDA(c, cudaEventElapsedTime(&tot, c->ev[i][0], c->ev[i][6]));
+        ms[7] += tot;
+    }
+    for (int k = 0; k < 8; ++k) ms[k] /= (float)T;
+    ms[6] = ms[7] - (ms[0] + ms[1] + ms[2] + ms[3] + ms[4] + ms[5]);
+    if (steps_timed) *steps_timed = T;
+    c->timed_steps = 0;
+    return TILD_OK;
+}
+
+int tild_run_host(tild_ctx* c, float* x_host, float* v_host, const int32_t* type_host, const int32_t* bond_partner_host,
+                  uint64_t step0, int32_t nsteps)
+{
+    int rc = tild_set_state(c, x_host, v_host, type_host, bond_partner_host, step0);
+    if (rc) return rc;
+    if ((rc = tild_step(c, nsteps))) return rc;
+    if ((rc = tild_get_state(c, x_host, v_host, nullptr, nullptr))) return rc;
+    TILD_CUDA(c, cudaStreamSynchronize(c->stream));
+    return TILD_OK;
+}
+
+}  // extern "C"
