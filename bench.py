@@ -158,7 +158,7 @@ def ours_arm(args, cfg):
 
     # independent replica per rank: same recipe, rank-specific seeds
     st = inputs.make_state(cfg, seed=cfg.input_seed + 7919 * rank)
-    eng = tild.Tild(tild.params_from_config(cfg, flags=tild.FLAG_TIMING, seed=cfg.philox_seed + rank,
+    eng = tild.Tild(tild.params_from_config(cfg, flags=tild.FLAG_TIMING | args.flags, seed=cfg.philox_seed + rank,
                                             resort_every=args.resort_every), device=f"cuda:{local}")
     xd, vd = torch.from_numpy(st.x).cuda(), torch.from_numpy(st.v).cuda()
     td, bd = torch.from_numpy(st.type).cuda(), torch.from_numpy(st.bond_partner).cuda()
@@ -259,6 +259,7 @@ def main():
     ap.add_argument("--workload", default="C4", choices=sorted(inputs.CONFIGS))
     ap.add_argument("--resort-every", type=int, default=0)
     ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--flags", type=int, default=0, help="extra TILD_FLAG_* bits (kernel A/B runs)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

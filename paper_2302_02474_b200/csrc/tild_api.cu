@@ -57,8 +57,55 @@ int validate(const tild_params* p)
     return TILD_OK;
 }
 
+// Tile shape for the shared-memory spread and the tile-major particle order: 8 x 8 x 64 cells (z-long so that a
+// warp of consecutive particles shares z-rows), clipped to the grid, shortened in z while the grid yields fewer
+// than two waves of CTAs, and shrunk until S tiles of (T + halo + 2*margin)^3 u32 fit in shared memory.
+void configure_tiles(tild_ctx* c)
+{
+    const tild_params& p = c->prm;
+    TileParams& t = c->tile;
+    const int lo_halo = p.order >= 3 ? 1 : 0, hi_halo = p.order >= 3 ? 2 : 1;
+    int margin = 1;
+    int T[3] = {8, 8, 64};
+    if (const char* e = getenv("TILD_TILE")) {  // tuning knob: "TX,TY,TZ,margin"
+        int v[4];
+        if (sscanf(e, "%d,%d,%d,%d", &v[0], &v[1], &v[2], &v[3]) == 4 && v[0] > 0 && v[1] > 0 && v[2] > 0 && v[3] >= 0) {
+            T[0] = v[0]; T[1] = v[1]; T[2] = v[2]; margin = v[3];
+        }
+    }
+    for (int a = 0; a < 3; ++a) T[a] = T[a] < p.grid[a] ? T[a] : p.grid[a];
+    auto ntiles = [&]() {
+        long v = 1;
+        for (int a = 0; a < 3; ++a) v *= (p.grid[a] + T[a] - 1) / T[a];
+        return v;
+    };
+    auto smem = [&]() {
+        size_t v = (size_t)p.n_species * sizeof(uint32_t);
+        for (int a = 0; a < 3; ++a) v *= (size_t)(T[a] + lo_halo + hi_halo + 2 * margin);
+        return v;
+    };
+    while (ntiles() < 2 * 148 && T[2] > 8) T[2] /= 2;
+    while (smem() > 100 * 1024 && T[2] > 8) T[2] /= 2;
+    while (smem() > 200 * 1024 && T[0] > 2) { T[0] /= 2; T[1] = T[1] > 2 ? T[1] / 2 : T[1]; }
+    t.lo = lo_halo + margin;
+    t.TV = 1;
+    t.ntiles = 1;
+    for (int a = 0; a < 3; ++a) {
+        t.T[a] = T[a];
+        t.nt[a] = (p.grid[a] + T[a] - 1) / T[a];
+        t.E[a] = T[a] + lo_halo + hi_halo + 2 * margin;
+        t.TV *= T[a];
+        t.ntiles *= t.nt[a];
+    }
+    t.nbins = (unsigned)t.ntiles * (unsigned)t.TV;
+    t.smem_bytes = smem();
+    const size_t M = (size_t)p.grid[0] * p.grid[1] * p.grid[2];
+    c->max_bins = M > t.nbins ? M : t.nbins;
+}
+
 void carve(tild_ctx* c, void* base, size_t* total)
 {
+    configure_tiles(c);
     const tild_params& p = c->prm;
     const size_t n = (size_t)p.n, S = (size_t)p.n_species;
     const size_t M = (size_t)p.grid[0] * p.grid[1] * p.grid[2];
@@ -79,9 +126,12 @@ void carve(tild_ctx* c, void* base, size_t* total)
     c->fpart = w.take<float>(3 * n);
     c->key = w.take<uint32_t>(n);
     c->perm = w.take<uint32_t>(n);
-    c->cell_start = w.take<uint32_t>(M + 1);
-    c->cell_fill = w.take<uint32_t>(M + 1);
-    c->scan_part = w.take<uint32_t>(tild_scan_scratch_entries(M, p.n));
+    c->tile_start = w.take<uint32_t>((size_t)c->tile.nbins + 1);
+    c->cell_start = w.take<uint32_t>(c->max_bins + 1);
+    c->cell_fill = w.take<uint32_t>(c->max_bins + 1);
+    c->scan_part = w.take<uint32_t>(tild_scan_scratch_entries(c->max_bins, p.n));
+    c->stage_x = w.take<float>(3 * n);
+    c->stage_type = w.take<int32_t>(n);
     c->tables = w.take<float>(6 * 4096);
     *total = w.off;
 }
@@ -98,10 +148,12 @@ __global__ void iota_kernel(int n, uint32_t* id)
         if (r__ != CUFFT_SUCCESS) return tild_fail((c), TILD_ECUFFT, "%s: cufft error %d", #call, (int)r__); \
     } while (0)
 
-// spread -> R2C -> k-space -> C2R on the given particle arrays, with optional stage events
+bool naive_spread(const tild_ctx* c) { return (c->prm.flags & TILD_FLAG_NAIVE_SPREAD) != 0; }
+
+// spread -> R2C -> k-space -> C2R on the internal (tile-sorted) particle arrays, with optional stage events
 int mesh_pipeline(tild_ctx* c, const float* x, const int32_t* type, cudaEvent_t* ev)
 {
-    int rc = launch_spread(c, x, type, c->grid);
+    int rc = naive_spread(c) ? launch_spread_naive(c, x, type, c->grid) : launch_spread_tiled(c, c->tile_start, x, type, c->grid);
     if (rc) return rc;
     if (ev) cudaEventRecord(ev[2], c->stream);
     TILD_FFT(c, cufftExecR2C(c->plan_r2c, c->grid, reinterpret_cast<cufftComplex*>(c->nhat)));
@@ -245,6 +297,12 @@ int tild_init(tild_ctx** out, const tild_params* params, void* workspace, size_t
         return TILD_ECUFFT;
     }
     c->plans_ok = true;
+    if ((rc = tild_spread_configure(c)) != TILD_OK) {
+        cufftDestroy(c->plan_r2c);
+        cufftDestroy(c->plan_c2r);
+        delete c;
+        return rc;
+    }
     cufftSetStream(c->plan_r2c, c->stream);
     cufftSetStream(c->plan_c2r, c->stream);
     if (p.flags & TILD_FLAG_TIMING) {
@@ -275,7 +333,10 @@ int64_t tild_launch_count(const tild_ctx* c) { return c ? c->launches : 0; }
 int tild_spread(tild_ctx* c, const float* x, const int32_t* type, float* grid)
 {
     if (!c || !grid || (c->mesh.n > 0 && (!x || !type))) return tild_fail(c, TILD_EINVAL, "tild_spread: null argument");
-    return launch_spread(c, x, type, grid);
+    if (naive_spread(c)) return launch_spread_naive(c, x, type, grid);
+    int rc = launch_stage_sort(c, x, type);  // tile-major sorted copy of the caller's particles
+    if (rc) return rc;
+    return launch_spread_tiled(c, c->cell_start, c->stage_x, c->stage_type, grid);
 }
 
 int tild_kspace_force(tild_ctx* c, const float* grid, float* ffield)
@@ -307,7 +368,7 @@ int tild_index_map(tild_ctx* c, const float* x, int32_t* base, uint32_t* cell_ke
     uint32_t* key = cell_key ? cell_key : c->key;
     int rc = launch_cell_keys(c, x, key, base);
     if (rc) return rc;
-    if (perm || cell_start) rc = launch_counting_sort(c, key, perm ? perm : c->perm, cell_start ? cell_start : c->cell_start);
+    if (perm || cell_start) rc = launch_counting_sort(c, key, c->M, perm ? perm : c->perm, cell_start ? cell_start : c->cell_start);
     return rc;
 }
 

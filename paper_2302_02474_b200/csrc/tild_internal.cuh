@@ -19,6 +19,18 @@ struct MeshParams {
     long long M;     // Nx*Ny*Nz
 };
 
+// Tiling of the cell grid for the shared-memory spread (tild_spread.cu) and the tile-major particle order.
+struct TileParams {
+    int T[3];       // tile edge in cells (clipped to the grid)
+    int nt[3];      // tiles per axis = ceil(N/T)
+    int E[3];       // shared tile edge in nodes = T + stencil halo + 2*margin
+    int lo;         // nodes below the tile's first cell held in shared memory (low halo + margin)
+    int TV;         // T[0]*T[1]*T[2]: sort keys per tile
+    int ntiles;
+    unsigned nbins; // ntiles*TV
+    size_t smem_bytes;
+};
+
 struct KspaceParams {
     int S;
     int N[3];
@@ -49,7 +61,8 @@ struct tild_ctx {
     KspaceParams ksp;
     StepParams stp;
     size_t M, Mk;
-    int ntiles;
+    TileParams tile;
+    size_t max_bins;      // max(M, tile.nbins)
 
     // carved from the caller's workspace
     float* x[2];
@@ -63,12 +76,14 @@ struct tild_ctx {
     float2* fhat;       // [3S][Mk]
     float* ffield;      // [3S][M]
     float* fpart;       // [n][3] scratch forces (internal order)
-    float* stage_x;     // [n][3] scratch for stage calls / get_state
     uint32_t* key;      // [n]
     uint32_t* perm;     // [n]
-    uint32_t* cell_start;  // [M+1]
-    uint32_t* cell_fill;   // [M+1] scatter cursors
-    uint32_t* scan_part;   // block sums for the scan
+    uint32_t* tile_start;  // [tile.nbins+1] tile-major cell offsets of the internal (sorted) state
+    uint32_t* cell_start;  // [max_bins+1] scratch offsets for tild_index_map / stage calls
+    uint32_t* cell_fill;   // [max_bins+1] histogram
+    uint32_t* scan_part;   // block sums for the scan, then rank[n]
+    float* stage_x;        // [n][3] sorted copy of caller positions (stage calls)
+    int32_t* stage_type;   // [n]
     float* tables;      // k-space tables
 
     cufftHandle plan_r2c, plan_c2r;
@@ -102,10 +117,14 @@ int tild_fail(tild_ctx* c, int code, const char* fmt, ...);
     } while (0)
 
 // ---- stage launchers (each enqueues on c->stream) -----------------------------------------------
-int launch_cell_keys(tild_ctx* c, const float* x, uint32_t* key, int32_t* base /*nullable*/);
-int launch_counting_sort(tild_ctx* c, const uint32_t* key, uint32_t* perm, uint32_t* cell_start);
-int launch_reorder(tild_ctx* c);  // sorts the internal state by cell and flips buffers
-int launch_spread(tild_ctx* c, const float* x, const int32_t* type, float* grid);
+int launch_cell_keys(tild_ctx* c, const float* x, uint32_t* key, int32_t* base /*nullable*/);  // row-major cell keys
+int launch_tile_keys(tild_ctx* c, const float* x, uint32_t* key);                              // tile-major cell keys
+int launch_counting_sort(tild_ctx* c, const uint32_t* key, size_t nbins, uint32_t* perm, uint32_t* start);
+int launch_reorder(tild_ctx* c);  // sorts the internal state by tile-major cell and flips buffers
+int launch_stage_sort(tild_ctx* c, const float* x, const int32_t* type);  // caller arrays -> stage_x/stage_type + cell_start
+int launch_spread_naive(tild_ctx* c, const float* x, const int32_t* type, float* grid);
+int launch_spread_tiled(tild_ctx* c, const uint32_t* cell_start, const float* x, const int32_t* type, float* grid);
+int tild_spread_configure(tild_ctx* c);
 int launch_kspace(tild_ctx* c, const float2* nhat, float2* fhat);
 int launch_interp_force(tild_ctx* c, const float* ffield, const float* x, const int32_t* type, float* f);
 int launch_bond_force(tild_ctx* c, const float* x, const int32_t* bond, float* f, bool accumulate);
@@ -114,7 +133,7 @@ int launch_make_w(tild_ctx* c, const float* f, float* w, float sign);  // w += s
 int launch_philox_test(tild_ctx* c, const uint32_t* ctr, const uint32_t* key, uint32_t* out, float* gauss, int m);
 int launch_unpermute(tild_ctx* c, const float* src, float* dst, int ncomp);  // dst[id[i]] = src[i]
 
-size_t tild_scan_scratch_entries(size_t M, int n);
+size_t tild_scan_scratch_entries(size_t nbins, int n);
 
 // ---- device helpers ------------------------------------------------------------------------------
 #ifdef __CUDACC__

@@ -6,7 +6,13 @@
 namespace {
 
 // f_a = sum_{stencil} w_x w_y w_z ffield[type][a][g]
-template <int P>
+//
+// VEC = true (Nz % 4 == 0, 16-byte aligned field): the P nodes of one z-row are contiguous in memory but start at
+// an arbitrary z, so each row is read as the one or two ALIGNED float4 that cover it (LDG.128) and dotted with an
+// 8-wide weight vector holding w_z shifted to the row's offset and zeros elsewhere.  That halves the load
+// instructions of the scalar form; with the particles in tile-major cell order (z fastest) the lanes of a warp
+// read neighbouring z of the same rows, so each load touches few cache lines.
+template <int P, bool VEC>
 __device__ __forceinline__ float3 interp_one(const MeshParams& m, const float* __restrict__ ffield, float px, float py,
                                              float pz, int type)
 {
@@ -21,10 +27,50 @@ __device__ __forceinline__ float3 interp_one(const MeshParams& m, const float* _
     const float* fx = ffield + (size_t)type * 3 * m.M;
     const float* fy = fx + m.M;
     const float* fz = fy + m.M;
+    float3 acc = make_float3(0.f, 0.f, 0.f);
+    if (VEC) {
+        const int bzw = wrap_idx(b[2], m.N[2]);
+        const int a0 = bzw & ~3, off = bzw & 3;
+        const int a1 = (a0 + 4 >= m.N[2]) ? 0 : a0 + 4;
+        const bool two = off + P > 4;
+        float w8[8];
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+            float v = 0.f;
+#pragma unroll
+            for (int j = 0; j < P; ++j)
+                if (k - j >= 0 && k - j <= 3) v = (k - j == off) ? w[2][j] : v;
+            w8[k] = v;
+        }
+#pragma unroll
+        for (int jx = 0; jx < P; ++jx) {
+            const size_t ox = (size_t)wrap_idx(b[0] + jx, m.N[0]) * m.N[1];
+#pragma unroll
+            for (int jy = 0; jy < P; ++jy) {
+                const size_t row = (ox + wrap_idx(b[1] + jy, m.N[1])) * m.N[2];
+                const float wxy = w[0][jx] * w[1][jy];
+                const float* comp[3] = {fx, fy, fz};
+                float d[3];
+#pragma unroll
+                for (int q = 0; q < 3; ++q) {
+                    const float4 v0 = __ldg(reinterpret_cast<const float4*>(comp[q] + row + a0));
+                    float s = w8[0] * v0.x + w8[1] * v0.y + w8[2] * v0.z + w8[3] * v0.w;
+                    if (two) {
+                        const float4 v1 = __ldg(reinterpret_cast<const float4*>(comp[q] + row + a1));
+                        s += w8[4] * v1.x + w8[5] * v1.y + w8[6] * v1.z + w8[7] * v1.w;
+                    }
+                    d[q] = s;
+                }
+                acc.x += wxy * d[0];
+                acc.y += wxy * d[1];
+                acc.z += wxy * d[2];
+            }
+        }
+        return acc;
+    }
     int iz[P];
 #pragma unroll
     for (int j = 0; j < P; ++j) iz[j] = wrap_idx(b[2] + j, m.N[2]);
-    float3 acc = make_float3(0.f, 0.f, 0.f);
 #pragma unroll
     for (int jx = 0; jx < P; ++jx) {
         const size_t ox = (size_t)wrap_idx(b[0] + jx, m.N[0]) * m.N[1];
@@ -67,14 +113,14 @@ __device__ __forceinline__ float3 bond_force_one(const MeshParams& m, const Step
     return f;
 }
 
-template <int P>
+template <int P, bool VEC>
 __global__ void __launch_bounds__(256) interp_force_kernel(MeshParams m, const float* __restrict__ ffield,
                                                            const float* __restrict__ x, const int32_t* __restrict__ type,
                                                            float* __restrict__ f)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= m.n) return;
-    const float3 a = interp_one<P>(m, ffield, x[3 * (size_t)i], x[3 * (size_t)i + 1], x[3 * (size_t)i + 2], type[i]);
+    const float3 a = interp_one<P, VEC>(m, ffield, x[3 * (size_t)i], x[3 * (size_t)i + 1], x[3 * (size_t)i + 2], type[i]);
     f[3 * (size_t)i + 0] = a.x;
     f[3 * (size_t)i + 1] = a.y;
     f[3 * (size_t)i + 2] = a.z;
@@ -103,7 +149,7 @@ __global__ void __launch_bounds__(256) bond_force_kernel(MeshParams m, StepParam
 //   r^{n+1} = wrap(r^n + b dt v^n + (b dt^2/2m) F^n + (b dt/2m) beta)
 //   w^{n+1} = a v^n + (dt/2m) a F^n + (b/m) beta
 // Positions are double-buffered because bonds read the partners' r^n while r^{n+1} is written.
-template <int P>
+template <int P, bool VEC>
 __global__ void __launch_bounds__(256) fused_step_kernel(MeshParams m, StepParams s, uint64_t step_next,
                                                          const float* __restrict__ ffield, const float* __restrict__ x0,
                                                          const float* __restrict__ w0, const int32_t* __restrict__ type,
@@ -113,7 +159,7 @@ __global__ void __launch_bounds__(256) fused_step_kernel(MeshParams m, StepParam
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= m.n) return;
     const float px = x0[3 * (size_t)i], py = x0[3 * (size_t)i + 1], pz = x0[3 * (size_t)i + 2];
-    float3 F = interp_one<P>(m, ffield, px, py, pz, type[i]);
+    float3 F = interp_one<P, VEC>(m, ffield, px, py, pz, type[i]);
     const float3 fb = bond_force_one(m, s, x0, bond, (size_t)i, px, py, pz);
     F.x += fb.x;
     F.y += fb.y;
@@ -162,17 +208,27 @@ __global__ void philox_test_kernel(int m, const uint32_t* __restrict__ ctr, cons
 
 }  // namespace
 
+static bool can_vectorize(const tild_ctx* c, const float* ffield)
+{
+    return (c->mesh.N[2] % 4 == 0) && (reinterpret_cast<uintptr_t>(ffield) % 16 == 0) && !(c->prm.flags & TILD_FLAG_NAIVE_INTERP);
+}
+
 int launch_interp_force(tild_ctx* c, const float* ffield, const float* x, const int32_t* type, float* f)
 {
     const int n = c->mesh.n;
     if (n == 0) return TILD_OK;
     const int nb = (n + 255) / 256;
+    const bool vec = can_vectorize(c, ffield);
+#define IF(PP)                                                                                          \
+    if (vec) interp_force_kernel<PP, true><<<nb, 256, 0, c->stream>>>(c->mesh, ffield, x, type, f);     \
+    else interp_force_kernel<PP, false><<<nb, 256, 0, c->stream>>>(c->mesh, ffield, x, type, f)
     switch (c->mesh.P) {
-    case 1: interp_force_kernel<1><<<nb, 256, 0, c->stream>>>(c->mesh, ffield, x, type, f); break;
-    case 2: interp_force_kernel<2><<<nb, 256, 0, c->stream>>>(c->mesh, ffield, x, type, f); break;
-    case 3: interp_force_kernel<3><<<nb, 256, 0, c->stream>>>(c->mesh, ffield, x, type, f); break;
-    default: interp_force_kernel<4><<<nb, 256, 0, c->stream>>>(c->mesh, ffield, x, type, f); break;
+    case 1: IF(1); break;
+    case 2: IF(2); break;
+    case 3: IF(3); break;
+    default: IF(4); break;
     }
+#undef IF
     TILD_LAUNCH_CHECK(c, "interp_force_kernel");
     return TILD_OK;
 }
@@ -198,7 +254,10 @@ int launch_fused_step(tild_ctx* c)
     if (n > 0) {
         const int nb = (n + 255) / 256;
         const uint64_t sn = c->step + 1;
-#define FS(PP) fused_step_kernel<PP><<<nb, 256, 0, c->stream>>>(c->mesh, c->stp, sn, c->ffield, x0, w0, c->type[a], c->id[a], c->bond[a], x1, w1)
+        const bool vec = can_vectorize(c, c->ffield);
+#define FS(PP)                                                                                                          \
+    if (vec) fused_step_kernel<PP, true><<<nb, 256, 0, c->stream>>>(c->mesh, c->stp, sn, c->ffield, x0, w0, c->type[a], c->id[a], c->bond[a], x1, w1); \
+    else fused_step_kernel<PP, false><<<nb, 256, 0, c->stream>>>(c->mesh, c->stp, sn, c->ffield, x0, w0, c->type[a], c->id[a], c->bond[a], x1, w1)
         switch (c->mesh.P) {
         case 1: FS(1); break;
         case 2: FS(2); break;

@@ -30,6 +30,40 @@ __global__ void __launch_bounds__(256) cell_key_kernel(MeshParams m, const float
     }
 }
 
+// key = tile * TV + local cell (tile-major order; z fastest inside a tile so that consecutive particles share
+// z-rows of the mesh, which is what the interpolation's loads want)
+template <int P>
+__global__ void __launch_bounds__(256) tile_key_kernel(MeshParams m, TileParams tp, const float* __restrict__ x,
+                                                       uint32_t* __restrict__ key)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= m.n) return;
+    int c[3], t[3], b;
+    float off;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        index_1d<P>(x[3 * (size_t)i + a], m.inv_h[a], c[a], b, off);
+        c[a] = wrap_idx(c[a], m.N[a]);
+        t[a] = c[a] / tp.T[a];
+        c[a] -= t[a] * tp.T[a];
+    }
+    const uint32_t tile = (uint32_t)((t[0] * tp.nt[1] + t[1]) * tp.nt[2] + t[2]);
+    key[i] = tile * (uint32_t)tp.TV + (uint32_t)((c[0] * tp.T[1] + c[1]) * tp.T[2] + c[2]);
+}
+
+__global__ void __launch_bounds__(256) gather_stage_kernel(int n, const uint32_t* __restrict__ perm,
+                                                           const float* __restrict__ x0, const int32_t* __restrict__ t0,
+                                                           float* __restrict__ x1, int32_t* __restrict__ t1)
+{
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= n) return;
+    const size_t o = perm[j];
+    x1[3 * (size_t)j + 0] = x0[3 * o + 0];
+    x1[3 * (size_t)j + 1] = x0[3 * o + 1];
+    x1[3 * (size_t)j + 2] = x0[3 * o + 2];
+    t1[j] = t0[o];
+}
+
 // count[key]++ ; rank[i] = arrival order inside the cell
 __global__ void __launch_bounds__(256) histogram_kernel(int n, const uint32_t* __restrict__ key,
                                                         uint32_t* __restrict__ count, uint32_t* __restrict__ rank)
@@ -190,14 +224,29 @@ int launch_cell_keys(tild_ctx* c, const float* x, uint32_t* key, int32_t* base)
 // Counting sort by cell key: histogram (arrival rank per particle) -> exclusive scan -> scatter.
 // Scratch: count = c->cell_fill [M+1]; c->scan_part holds the nbs block sums followed by rank[n]; after the
 // scatter rank[i] is the destination of particle i, i.e. the inverse permutation used by launch_reorder.
-int launch_counting_sort(tild_ctx* c, const uint32_t* key, uint32_t* perm, uint32_t* cell_start)
+int launch_tile_keys(tild_ctx* c, const float* x, uint32_t* key)
 {
     const int n = c->mesh.n;
-    const size_t len = c->M + 1;
+    if (n == 0) return TILD_OK;
+    const int nb = (n + 255) / 256;
+    switch (c->mesh.P) {
+    case 1: tile_key_kernel<1><<<nb, 256, 0, c->stream>>>(c->mesh, c->tile, x, key); break;
+    case 2: tile_key_kernel<2><<<nb, 256, 0, c->stream>>>(c->mesh, c->tile, x, key); break;
+    case 3: tile_key_kernel<3><<<nb, 256, 0, c->stream>>>(c->mesh, c->tile, x, key); break;
+    default: tile_key_kernel<4><<<nb, 256, 0, c->stream>>>(c->mesh, c->tile, x, key); break;
+    }
+    TILD_LAUNCH_CHECK(c, "tile_key_kernel");
+    return TILD_OK;
+}
+
+int launch_counting_sort(tild_ctx* c, const uint32_t* key, size_t nbins, uint32_t* perm, uint32_t* start)
+{
+    const int n = c->mesh.n;
+    const size_t len = nbins + 1;
     const int nbs = (int)((len + SCAN_CHUNK - 1) / SCAN_CHUNK);
     uint32_t* count = c->cell_fill;
     uint32_t* part = c->scan_part;
-    uint32_t* rank = c->scan_part + nbs;
+    uint32_t* rank = c->scan_part + (c->max_bins + 1 + SCAN_CHUNK - 1) / SCAN_CHUNK;  // fixed offset: see launch_reorder
     TILD_CUDA(c, cudaMemsetAsync(count, 0, len * sizeof(uint32_t), c->stream));
     if (n > 0) {
         histogram_kernel<<<(n + 255) / 256, 256, 0, c->stream>>>(n, key, count, rank);
@@ -207,10 +256,10 @@ int launch_counting_sort(tild_ctx* c, const uint32_t* key, uint32_t* perm, uint3
     TILD_LAUNCH_CHECK(c, "scan_reduce_kernel");
     scan_parts_kernel<<<1, 1024, 0, c->stream>>>(nbs, part);
     TILD_LAUNCH_CHECK(c, "scan_parts_kernel");
-    scan_final_kernel<<<nbs, SCAN_THREADS, 0, c->stream>>>(len, count, part, cell_start);
+    scan_final_kernel<<<nbs, SCAN_THREADS, 0, c->stream>>>(len, count, part, start);
     TILD_LAUNCH_CHECK(c, "scan_final_kernel");
     if (n > 0 && perm) {
-        scatter_kernel<<<(n + 255) / 256, 256, 0, c->stream>>>(n, key, cell_start, rank, perm);
+        scatter_kernel<<<(n + 255) / 256, 256, 0, c->stream>>>(n, key, start, rank, perm);
         TILD_LAUNCH_CHECK(c, "scatter_kernel");
     }
     return TILD_OK;
@@ -219,21 +268,31 @@ int launch_counting_sort(tild_ctx* c, const uint32_t* key, uint32_t* perm, uint3
 int launch_reorder(tild_ctx* c)
 {
     const int n = c->mesh.n;
+    int rc = launch_tile_keys(c, c->x[c->cur], c->key);
+    if (rc) return rc;
+    rc = launch_counting_sort(c, c->key, c->tile.nbins, c->perm, c->tile_start);
+    if (rc) return rc;
+    c->steps_since_sort = 0;
     if (n == 0) return TILD_OK;
-    int rc = launch_cell_keys(c, c->x[c->cur], c->key, nullptr);
-    if (rc) return rc;
-    rc = launch_counting_sort(c, c->key, c->perm, c->cell_start);
-    if (rc) return rc;
-    const size_t len = c->M + 1;
-    const int nbs = (int)((len + SCAN_CHUNK - 1) / SCAN_CHUNK);
-    const uint32_t* inv = c->scan_part + nbs;
+    const uint32_t* inv = c->scan_part + (c->max_bins + 1 + SCAN_CHUNK - 1) / SCAN_CHUNK;
     const int a = c->cur, b = 1 - c->cur;
     reorder_kernel<<<(n + 255) / 256, 256, 0, c->stream>>>(n, c->stp.max_bonds, c->perm, inv, c->x[a], c->w[a], c->type[a],
                                                            c->id[a], c->bond[a], c->x[b], c->w[b], c->type[b], c->id[b],
                                                            c->bond[b]);
     TILD_LAUNCH_CHECK(c, "reorder_kernel");
     c->cur = b;
-    c->steps_since_sort = 0;
+    return TILD_OK;
+}
+
+int launch_stage_sort(tild_ctx* c, const float* x, const int32_t* type)
+{
+    const int n = c->mesh.n;
+    int rc = launch_tile_keys(c, x, c->key);
+    if (rc) return rc;
+    rc = launch_counting_sort(c, c->key, c->tile.nbins, c->perm, c->cell_start);
+    if (rc || n == 0) return rc;
+    gather_stage_kernel<<<(n + 255) / 256, 256, 0, c->stream>>>(n, c->perm, x, type, c->stage_x, c->stage_type);
+    TILD_LAUNCH_CHECK(c, "gather_stage_kernel");
     return TILD_OK;
 }
 
@@ -246,8 +305,8 @@ int launch_unpermute(tild_ctx* c, const float* src, float* dst, int ncomp)
     return TILD_OK;
 }
 
-size_t tild_scan_scratch_entries(size_t M, int n)
+size_t tild_scan_scratch_entries(size_t nbins, int n)
 {
-    const size_t len = M + 1;
+    const size_t len = nbins + 1;
     return (len + SCAN_CHUNK - 1) / SCAN_CHUNK + (size_t)n + 16;
 }

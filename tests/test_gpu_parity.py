@@ -267,3 +267,73 @@ def test_run_host_end_to_end_matches_device_path():
     x2, v2, _, _ = eng2.tild_get_state()
     assert np.abs(min_image(xh.numpy().astype(np.float64) - x2.cpu().numpy(), cfg.box)).max() < 2e-5
     assert np.abs(vh.numpy() - v2.cpu().numpy()).max() < 1e-3
+
+
+# ---------------- kernel variants, fallbacks, full-size configs ----------------
+def test_naive_kernel_flags_match_oracle():
+    cfg = small_cfg(order=4)
+    st, eng = make(cfg, flags=tild.FLAG_NAIVE_SPREAD | tild.FLAG_NAIVE_INTERP)
+    p = oracle_params(cfg)
+    g = eng.tild_spread(dev(st.x), dev(st.type)).cpu().numpy()
+    og = orc.spread(p, st.x, st.type)
+    assert np.abs(g - og).max() <= REL * rms(og)
+    eng.tild_set_state(dev(st.x), dev(st.v), dev(st.type), dev(st.bond_partner), 0)
+    _, _, f, _ = eng.tild_get_state(want_v=False, want_f=True)
+    of = orc.force(p, st.x.astype(np.float64), st.type, st.bond_partner)
+    assert np.abs(f.cpu().numpy() - of).max() <= REL * vec_rms(of)
+
+
+@pytest.mark.parametrize("P", [2, 4])
+def test_fixed_point_tile_wrap_is_detected_and_redone(P):
+    """> 256 particles' worth of weight on one node wraps the 2^-24 fixed-point tile; the mass-balance check must
+    catch it and the tile must be redone with fp32 atomics."""
+    from dataclasses import replace
+    n = 6000
+    cfg = replace(small_cfg(order=P), n=n)
+    rng = np.random.default_rng(17)
+    h = np.array(cfg.box) / np.array(cfg.grid)
+    x = ((np.array([5, 7, 3]) + 0.5 + 0.02 * rng.random((n, 3))) * h).astype(np.float32)   # all next to one cell centre
+    x[:50] = (rng.random((50, 3)) * np.array(cfg.box)).astype(np.float32)
+    ty = (np.arange(n) % 2).astype(np.int32)
+    eng = tild.Tild(tild.params_from_config(cfg))
+    p = oracle_params(cfg)
+    g = eng.tild_spread(dev(x), dev(ty)).cpu().numpy()
+    og = orc.spread(p, x, ty)
+    assert og.max() > 300.0
+    assert np.abs(g - og).max() <= 3e-6 * og.max()
+    assert np.allclose(g.sum(axis=(1, 2, 3)), [n / 2, n / 2], rtol=1e-6)
+
+
+def test_particles_that_drift_out_of_their_tile_fall_back_correctly():
+    """No re-sort for 300 steps at a large dt: many particles leave their tile's halo; spread must stay exact."""
+    cfg = small_cfg(order=4, dt=0.02)
+    st, eng = make(cfg, resort_every=100000)
+    p = oracle_params(cfg)
+    eng.tild_set_state(dev(st.x), dev(st.v), dev(st.type), dev(st.bond_partner), 0)
+    eng.tild_step(300)
+    x, _, f, _ = eng.tild_get_state(want_v=False, want_f=True)
+    xn = x.cpu().numpy()
+    moved = np.abs(min_image(xn.astype(np.float64) - st.x, cfg.box)).max()
+    assert moved > 1.5 * max(np.array(cfg.box) / np.array(cfg.grid))          # more than the one-cell margin
+    of = orc.force(p, xn.astype(np.float64), st.type, st.bond_partner)
+    assert np.abs(f.cpu().numpy() - of).max() <= REL * vec_rms(of)
+
+
+@pytest.mark.parametrize("name", ["C2", "C3"])
+def test_full_size_config_force_and_short_trajectory(name):
+    cfg = inputs.CONFIGS[name]
+    st, eng = make(cfg)
+    p = oracle_params(cfg)
+    base, key, perm, start = eng.tild_index_map(dev(st.x))
+    obase, _, okey = orc.index_map(p, st.x)
+    assert np.array_equal(base.cpu().numpy(), obase) and np.array_equal(key.cpu().numpy().view(np.uint32), okey)
+    assert np.array_equal(start.cpu().numpy().view(np.uint32), orc.cell_sort(cfg.n, cfg.M, okey)[1])
+    eng.tild_set_state(dev(st.x), dev(st.v), dev(st.type), dev(st.bond_partner), 0)
+    _, _, f, _ = eng.tild_get_state(want_v=False, want_f=True)
+    of = orc.force(p, st.x.astype(np.float64), st.type, st.bond_partner)
+    assert np.abs(f.cpu().numpy() - of).max() <= REL * vec_rms(of)
+    nst = 20 if name == "C2" else 5
+    eng.tild_step(nst)
+    x, v, _, _ = eng.tild_get_state()
+    ox, ov, _ = orc.run(p, st.x.astype(np.float64), st.v.astype(np.float64), st.type, st.bond_partner, 0, nst)
+    assert np.abs(min_image(x.cpu().numpy().astype(np.float64) - ox, cfg.box)).max() <= 1e-4
