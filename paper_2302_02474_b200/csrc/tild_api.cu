@@ -65,14 +65,12 @@ void configure_tiles(tild_ctx* c)
     const tild_params& p = c->prm;
     TileParams& t = c->tile;
     const int lo_halo = p.order >= 3 ? 1 : 0, hi_halo = p.order >= 3 ? 2 : 1;
-    int margin = 1;
     int T[3] = {8, 8, 64};
-    if (const char* e = getenv("TILD_TILE")) {  // tuning knob: "TX,TY,TZ,margin"
-        int v[4];
-        if (sscanf(e, "%d,%d,%d,%d", &v[0], &v[1], &v[2], &v[3]) == 4 && v[0] > 0 && v[1] > 0 && v[2] > 0 && v[3] >= 0) {
-            T[0] = v[0]; T[1] = v[1]; T[2] = v[2]; margin = v[3];
-        }
+    if (const char* e = getenv("TILD_TILE_Z")) {  // tuning knob: tile length in z (8, 16, 32 or 64)
+        const int v = atoi(e);
+        if (v == 8 || v == 16 || v == 32 || v == 64) T[2] = v;
     }
+    t.enabled = p.grid[0] >= 8 && p.grid[1] >= 8 && p.grid[2] >= 8;
     for (int a = 0; a < 3; ++a) T[a] = T[a] < p.grid[a] ? T[a] : p.grid[a];
     auto ntiles = [&]() {
         long v = 1;
@@ -81,23 +79,26 @@ void configure_tiles(tild_ctx* c)
     };
     auto smem = [&]() {
         size_t v = (size_t)p.n_species * sizeof(uint32_t);
-        for (int a = 0; a < 3; ++a) v *= (size_t)(T[a] + lo_halo + hi_halo + 2 * margin);
-        return v;
+        for (int a = 0; a < 3; ++a) v *= (size_t)(T[a] + lo_halo + hi_halo);
+        return (v + 15) / 16 * 16;
     };
-    while (ntiles() < 2 * 148 && T[2] > 8) T[2] /= 2;
-    while (smem() > 100 * 1024 && T[2] > 8) T[2] /= 2;
-    while (smem() > 200 * 1024 && T[0] > 2) { T[0] /= 2; T[1] = T[1] > 2 ? T[1] / 2 : T[1]; }
-    t.lo = lo_halo + margin;
+    if (t.enabled) {
+        while (T[2] > p.grid[2] || (T[2] & (T[2] - 1))) T[2] = T[2] >= 64 ? 32 : (T[2] >= 32 ? 16 : 8);  // power of two <= Nz
+        while (ntiles() < 2 * 148 && T[2] > 8) T[2] /= 2;
+        while (smem() > 100 * 1024 && T[2] > 8) T[2] /= 2;
+        if (smem() > 200 * 1024) t.enabled = 0;
+    }
+    t.lo = lo_halo;
     t.TV = 1;
     t.ntiles = 1;
     for (int a = 0; a < 3; ++a) {
         t.T[a] = T[a];
         t.nt[a] = (p.grid[a] + T[a] - 1) / T[a];
-        t.E[a] = T[a] + lo_halo + hi_halo + 2 * margin;
+        t.E[a] = T[a] + lo_halo + hi_halo;
         t.TV *= T[a];
         t.ntiles *= t.nt[a];
     }
-    t.nbins = (unsigned)t.ntiles * (unsigned)t.TV;
+    t.nbins = (unsigned)t.ntiles * (unsigned)p.n_species * (unsigned)t.TV;
     t.smem_bytes = smem();
     const size_t M = (size_t)p.grid[0] * p.grid[1] * p.grid[2];
     c->max_bins = M > t.nbins ? M : t.nbins;
@@ -148,12 +149,17 @@ __global__ void iota_kernel(int n, uint32_t* id)
         if (r__ != CUFFT_SUCCESS) return tild_fail((c), TILD_ECUFFT, "%s: cufft error %d", #call, (int)r__); \
     } while (0)
 
-bool naive_spread(const tild_ctx* c) { return (c->prm.flags & TILD_FLAG_NAIVE_SPREAD) != 0; }
+// The tile kernel needs N >= 8 on every axis (8 x 8 x TZ tiles, single conditional wraps); tiny grids use the
+// per-particle kernel.
+bool naive_spread(const tild_ctx* c)
+{
+    return (c->prm.flags & TILD_FLAG_NAIVE_SPREAD) != 0 || !c->tile.enabled;
+}
 
 // spread -> R2C -> k-space -> C2R on the internal (tile-sorted) particle arrays, with optional stage events
 int mesh_pipeline(tild_ctx* c, const float* x, const int32_t* type, cudaEvent_t* ev)
 {
-    int rc = naive_spread(c) ? launch_spread_naive(c, x, type, c->grid) : launch_spread_tiled(c, c->tile_start, x, type, c->grid);
+    int rc = naive_spread(c) ? launch_spread_naive(c, x, type, c->grid) : launch_spread_tiled(c, c->tile_start, x, c->grid);
     if (rc) return rc;
     if (ev) cudaEventRecord(ev[2], c->stream);
     TILD_FFT(c, cufftExecR2C(c->plan_r2c, c->grid, reinterpret_cast<cufftComplex*>(c->nhat)));
@@ -336,7 +342,7 @@ int tild_spread(tild_ctx* c, const float* x, const int32_t* type, float* grid)
     if (naive_spread(c)) return launch_spread_naive(c, x, type, grid);
     int rc = launch_stage_sort(c, x, type);  // tile-major sorted copy of the caller's particles
     if (rc) return rc;
-    return launch_spread_tiled(c, c->cell_start, c->stage_x, c->stage_type, grid);
+    return launch_spread_tiled(c, c->cell_start, c->stage_x, grid);
 }
 
 int tild_kspace_force(tild_ctx* c, const float* grid, float* ffield)

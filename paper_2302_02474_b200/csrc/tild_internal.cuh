@@ -25,10 +25,11 @@ struct TileParams {
     int nt[3];      // tiles per axis = ceil(N/T)
     int E[3];       // shared tile edge in nodes = T + stencil halo + 2*margin
     int lo;         // nodes below the tile's first cell held in shared memory (low halo + margin)
-    int TV;         // T[0]*T[1]*T[2]: sort keys per tile
+    int TV;         // T[0]*T[1]*T[2]: cells per tile; sort key = (tile*S + species)*TV + local cell
     int ntiles;
-    unsigned nbins; // ntiles*TV
+    unsigned nbins; // ntiles*S*TV
     size_t smem_bytes;
+    int enabled;    // 0: grid too small for the tile kernel (any N < 8) -> per-particle spread
 };
 
 struct KspaceParams {
@@ -118,12 +119,12 @@ int tild_fail(tild_ctx* c, int code, const char* fmt, ...);
 
 // ---- stage launchers (each enqueues on c->stream) -----------------------------------------------
 int launch_cell_keys(tild_ctx* c, const float* x, uint32_t* key, int32_t* base /*nullable*/);  // row-major cell keys
-int launch_tile_keys(tild_ctx* c, const float* x, uint32_t* key);                              // tile-major cell keys
+int launch_tile_keys(tild_ctx* c, const float* x, const int32_t* type, uint32_t* key);        // (tile, species, cell) keys
 int launch_counting_sort(tild_ctx* c, const uint32_t* key, size_t nbins, uint32_t* perm, uint32_t* start);
 int launch_reorder(tild_ctx* c);  // sorts the internal state by tile-major cell and flips buffers
 int launch_stage_sort(tild_ctx* c, const float* x, const int32_t* type);  // caller arrays -> stage_x/stage_type + cell_start
 int launch_spread_naive(tild_ctx* c, const float* x, const int32_t* type, float* grid);
-int launch_spread_tiled(tild_ctx* c, const uint32_t* cell_start, const float* x, const int32_t* type, float* grid);
+int launch_spread_tiled(tild_ctx* c, const uint32_t* cell_start, const float* x, float* grid);
 int tild_spread_configure(tild_ctx* c);
 int launch_kspace(tild_ctx* c, const float2* nhat, float2* fhat);
 int launch_interp_force(tild_ctx* c, const float* ffield, const float* x, const int32_t* type, float* f);

@@ -34,7 +34,7 @@ __global__ void __launch_bounds__(256) cell_key_kernel(MeshParams m, const float
 // z-rows of the mesh, which is what the interpolation's loads want)
 template <int P>
 __global__ void __launch_bounds__(256) tile_key_kernel(MeshParams m, TileParams tp, const float* __restrict__ x,
-                                                       uint32_t* __restrict__ key)
+                                                       const int32_t* __restrict__ type, uint32_t* __restrict__ key)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= m.n) return;
@@ -48,7 +48,7 @@ __global__ void __launch_bounds__(256) tile_key_kernel(MeshParams m, TileParams 
         c[a] -= t[a] * tp.T[a];
     }
     const uint32_t tile = (uint32_t)((t[0] * tp.nt[1] + t[1]) * tp.nt[2] + t[2]);
-    key[i] = tile * (uint32_t)tp.TV + (uint32_t)((c[0] * tp.T[1] + c[1]) * tp.T[2] + c[2]);
+    key[i] = (tile * (uint32_t)m.S + (uint32_t)type[i]) * (uint32_t)tp.TV + (uint32_t)((c[0] * tp.T[1] + c[1]) * tp.T[2] + c[2]);
 }
 
 __global__ void __launch_bounds__(256) gather_stage_kernel(int n, const uint32_t* __restrict__ perm,
@@ -224,16 +224,16 @@ int launch_cell_keys(tild_ctx* c, const float* x, uint32_t* key, int32_t* base)
 // Counting sort by cell key: histogram (arrival rank per particle) -> exclusive scan -> scatter.
 // Scratch: count = c->cell_fill [M+1]; c->scan_part holds the nbs block sums followed by rank[n]; after the
 // scatter rank[i] is the destination of particle i, i.e. the inverse permutation used by launch_reorder.
-int launch_tile_keys(tild_ctx* c, const float* x, uint32_t* key)
+int launch_tile_keys(tild_ctx* c, const float* x, const int32_t* type, uint32_t* key)
 {
     const int n = c->mesh.n;
     if (n == 0) return TILD_OK;
     const int nb = (n + 255) / 256;
     switch (c->mesh.P) {
-    case 1: tile_key_kernel<1><<<nb, 256, 0, c->stream>>>(c->mesh, c->tile, x, key); break;
-    case 2: tile_key_kernel<2><<<nb, 256, 0, c->stream>>>(c->mesh, c->tile, x, key); break;
-    case 3: tile_key_kernel<3><<<nb, 256, 0, c->stream>>>(c->mesh, c->tile, x, key); break;
-    default: tile_key_kernel<4><<<nb, 256, 0, c->stream>>>(c->mesh, c->tile, x, key); break;
+    case 1: tile_key_kernel<1><<<nb, 256, 0, c->stream>>>(c->mesh, c->tile, x, type, key); break;
+    case 2: tile_key_kernel<2><<<nb, 256, 0, c->stream>>>(c->mesh, c->tile, x, type, key); break;
+    case 3: tile_key_kernel<3><<<nb, 256, 0, c->stream>>>(c->mesh, c->tile, x, type, key); break;
+    default: tile_key_kernel<4><<<nb, 256, 0, c->stream>>>(c->mesh, c->tile, x, type, key); break;
     }
     TILD_LAUNCH_CHECK(c, "tile_key_kernel");
     return TILD_OK;
@@ -268,7 +268,7 @@ int launch_counting_sort(tild_ctx* c, const uint32_t* key, size_t nbins, uint32_
 int launch_reorder(tild_ctx* c)
 {
     const int n = c->mesh.n;
-    int rc = launch_tile_keys(c, c->x[c->cur], c->key);
+    int rc = launch_tile_keys(c, c->x[c->cur], c->type[c->cur], c->key);
     if (rc) return rc;
     rc = launch_counting_sort(c, c->key, c->tile.nbins, c->perm, c->tile_start);
     if (rc) return rc;
@@ -287,7 +287,7 @@ int launch_reorder(tild_ctx* c)
 int launch_stage_sort(tild_ctx* c, const float* x, const int32_t* type)
 {
     const int n = c->mesh.n;
-    int rc = launch_tile_keys(c, x, c->key);
+    int rc = launch_tile_keys(c, x, type, c->key);
     if (rc) return rc;
     rc = launch_counting_sort(c, c->key, c->tile.nbins, c->perm, c->cell_start);
     if (rc || n == 0) return rc;
