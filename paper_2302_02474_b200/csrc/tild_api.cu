@@ -57,51 +57,67 @@ int validate(const tild_params* p)
     return TILD_OK;
 }
 
-// Tile shape for the shared-memory spread and the tile-major particle order: 8 x 8 x 64 cells (z-long so that a
-// warp of consecutive particles shares z-rows), clipped to the grid, shortened in z while the grid yields fewer
-// than two waves of CTAs, and shrunk until S tiles of (T + halo + 2*margin)^3 u32 fit in shared memory.
+// Tile shape of the slab-transposed layout: TX x TY x TZ cells with TZ = EZ - H so that the
+// shared image is EZ in {32, 64} nodes long in z (bank = z); TX, TY in {8, 16} (template EY = TY + H).  Tuning
+// knobs (environment): TILD_TILE_X, TILD_TILE_Y (8|16), TILD_EZ (32|64), TILD_FILL (rounds cap factor).
 void configure_tiles(tild_ctx* c)
 {
     const tild_params& p = c->prm;
     TileParams& t = c->tile;
-    const int lo_halo = p.order >= 3 ? 1 : 0, hi_halo = p.order >= 3 ? 2 : 1;
-    int T[3] = {8, 8, 64};
-    if (const char* e = getenv("TILD_TILE_Z")) {  // tuning knob: tile length in z (8, 16, 32 or 64)
-        const int v = atoi(e);
-        if (v == 8 || v == 16 || v == 32 || v == 64) T[2] = v;
-    }
+    memset(&t, 0, sizeof(t));
+    auto env_int = [](const char* name, int dflt) {
+        const char* e = getenv(name);
+        return e ? atoi(e) : dflt;
+    };
+    t.H = p.order >= 3 ? 3 : 1;
+    t.lo = p.order >= 3 ? 1 : 0;
     t.enabled = p.grid[0] >= 8 && p.grid[1] >= 8 && p.grid[2] >= 8;
-    for (int a = 0; a < 3; ++a) T[a] = T[a] < p.grid[a] ? T[a] : p.grid[a];
-    auto ntiles = [&]() {
-        long v = 1;
-        for (int a = 0; a < 3; ++a) v *= (p.grid[a] + T[a] - 1) / T[a];
-        return v;
-    };
-    auto smem = [&]() {
-        size_t v = (size_t)p.n_species * sizeof(uint32_t);
-        for (int a = 0; a < 3; ++a) v *= (size_t)(T[a] + lo_halo + hi_halo);
-        return (v + 15) / 16 * 16;
-    };
-    if (t.enabled) {
-        while (T[2] > p.grid[2] || (T[2] & (T[2] - 1))) T[2] = T[2] >= 64 ? 32 : (T[2] >= 32 ? 16 : 8);  // power of two <= Nz
-        while (ntiles() < 2 * 148 && T[2] > 8) T[2] /= 2;
-        while (smem() > 100 * 1024 && T[2] > 8) T[2] /= 2;
-        if (smem() > 200 * 1024) t.enabled = 0;
+    int tx = env_int("TILD_TILE_X", 8), ty = env_int("TILD_TILE_Y", 8), ez = env_int("TILD_EZ", p.grid[2] >= 96 ? 64 : 32);
+    if (tx != 8 && tx != 16) tx = 8;
+    if (ty != 8 && ty != 16) ty = 8;
+    if (ez != 32 && ez != 64) ez = 32;
+    if ((size_t)(tx + t.H) * (ty + t.H) * 3 * ez * sizeof(float) > 200 * 1024) tx = 8;
+    if ((size_t)(tx + t.H) * (ty + t.H) * 3 * ez * sizeof(float) > 200 * 1024) ty = 8;
+    t.EY = ty + t.H;
+    t.EZ = ez;
+    // z: the image starts sh nodes below the stencil's low halo so that it begins on a 16-byte boundary of the mesh
+    // rows (16-byte cp.async staging in the interpolation); TZ is a multiple of 4 with TZ + H + sh <= EZ
+    t.sh = t.lo ? 4 - t.lo : 0;
+    const int tz_max = (ez - t.H - t.sh) / 4 * 4;
+    int tzc = p.grid[2];
+    if (tzc > tz_max) {
+        const int ntz = (p.grid[2] + tz_max - 1) / tz_max;
+        tzc = ((p.grid[2] + ntz - 1) / ntz + 3) / 4 * 4;
     }
-    t.lo = lo_halo;
-    t.TV = 1;
+    const int T[3] = {tx, ty, tzc};
     t.ntiles = 1;
     for (int a = 0; a < 3; ++a) {
-        t.T[a] = T[a];
-        t.nt[a] = (p.grid[a] + T[a] - 1) / T[a];
-        t.E[a] = T[a] + lo_halo + hi_halo;
-        t.TV *= T[a];
+        t.T[a] = T[a] < p.grid[a] ? T[a] : p.grid[a];
+        t.nt[a] = (p.grid[a] + t.T[a] - 1) / t.T[a];
+        t.E[a] = t.T[a] + t.H;
         t.ntiles *= t.nt[a];
     }
-    t.nbins = (unsigned)t.ntiles * (unsigned)p.n_species * (unsigned)t.TV;
-    t.smem_bytes = smem();
+    t.E[2] = ez;
+    if (t.T[2] + t.H + t.sh > ez) t.enabled = 0;   // Nz <= tz_max but not a fit (cannot happen: Nz <= tz_max)
+    t.nseg = t.ntiles * p.n_species;
+    const size_t per_species = (size_t)t.E[0] * t.EY * t.EZ * sizeof(uint32_t);
+    t.sp_group = (int)((100 * 1024) / per_species);
+    if (t.sp_group < 1) t.sp_group = 1;
+    if (t.sp_group > p.n_species) t.sp_group = p.n_species;
+    t.smem_spread = per_species * t.sp_group;
+    t.smem_interp = (size_t)t.E[0] * t.EY * 3 * t.EZ * sizeof(float);
+    t.fill = 1.02f;
+    if (const char* e = getenv("TILD_FILL")) {
+        const float v = (float)atof(e);
+        if (v >= 1.0f && v <= 1.5f) t.fill = v;
+    }
+    t.add = 1;
+    const size_t n = (size_t)p.n;
+    t.cap_ell = (size_t)(1.5 * (double)n) + (size_t)32 * (t.add + 1) * t.nseg + 32;   // >= fill*n + 32*(add+1)*nseg
+    t.cap_ell = (t.cap_ell + 31) / 32 * 32;
+    t.cap = t.cap_ell + n + 32;
     const size_t M = (size_t)p.grid[0] * p.grid[1] * p.grid[2];
-    c->max_bins = M > t.nbins ? M : t.nbins;
+    c->max_bins = M > (size_t)t.nseg * 32 ? M : (size_t)t.nseg * 32;
 }
 
 void carve(tild_ctx* c, void* base, size_t* total)
@@ -111,36 +127,35 @@ void carve(tild_ctx* c, void* base, size_t* total)
     const size_t n = (size_t)p.n, S = (size_t)p.n_species;
     const size_t M = (size_t)p.grid[0] * p.grid[1] * p.grid[2];
     const size_t Mk = (size_t)p.grid[0] * p.grid[1] * (p.grid[2] / 2 + 1);
-    const size_t nb = n * (size_t)(p.max_bonds > 0 ? p.max_bonds : 1);
+    const size_t cap = c->tile.cap;
+    const size_t nb = cap * (size_t)(p.max_bonds > 0 ? p.max_bonds : 1);
     Carver w(base);
     for (int k = 0; k < 2; ++k) {
-        c->x[k] = w.take<float>(3 * n);
-        c->w[k] = w.take<float>(3 * n);
-        c->type[k] = w.take<int32_t>(n);
-        c->id[k] = w.take<uint32_t>(n);
-        c->bond[k] = w.take<int32_t>(nb);
+        c->X4[k] = w.take<float4>(cap);
+        c->W4[k] = w.take<float4>(cap);
+        c->B[k] = w.take<int32_t>(nb);
     }
+    c->F4 = w.take<float4>(cap);
+    c->SX4 = w.take<float4>(cap);
+    c->lay.seg_base = w.take<uint32_t>((size_t)c->tile.nseg + 1);
+    c->lay_stage.seg_base = w.take<uint32_t>((size_t)c->tile.nseg + 1);
     c->grid = w.take<float>(S * M);
     c->nhat = w.take<float2>(S * Mk);
     c->fhat = w.take<float2>(3 * S * Mk);
     c->ffield = w.take<float>(3 * S * M);
-    c->fpart = w.take<float>(3 * n);
-    c->key = w.take<uint32_t>(n);
+    c->key = w.take<uint32_t>(cap);
+    c->rank = w.take<uint32_t>(cap);
+    c->inv = w.take<uint32_t>(cap);
+    c->count = w.take<uint32_t>(c->max_bins + 2);
+    c->start = w.take<uint32_t>(c->max_bins + 2);
+    c->scan_part = w.take<uint32_t>(tild_scan_scratch_entries(c->max_bins + 2));
+    c->holepref = w.take<uint32_t>((size_t)c->tile.nseg * 32);
+    c->segholes = w.take<uint32_t>((size_t)c->tile.nseg);
+    c->segtick = w.take<uint32_t>((size_t)c->tile.nseg);
     c->perm = w.take<uint32_t>(n);
-    c->tile_start = w.take<uint32_t>((size_t)c->tile.nbins + 1);
-    c->cell_start = w.take<uint32_t>(c->max_bins + 1);
-    c->cell_fill = w.take<uint32_t>(c->max_bins + 1);
-    c->scan_part = w.take<uint32_t>(tild_scan_scratch_entries(c->max_bins, p.n));
-    c->stage_x = w.take<float>(3 * n);
-    c->stage_type = w.take<int32_t>(n);
+    c->totals = w.take<uint32_t>(4);
     c->tables = w.take<float>(6 * 4096);
     *total = w.off;
-}
-
-__global__ void iota_kernel(int n, uint32_t* id)
-{
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < n) id[i] = (uint32_t)i;
 }
 
 #define TILD_FFT(c, call)                                                                  \
@@ -149,17 +164,22 @@ __global__ void iota_kernel(int n, uint32_t* id)
         if (r__ != CUFFT_SUCCESS) return tild_fail((c), TILD_ECUFFT, "%s: cufft error %d", #call, (int)r__); \
     } while (0)
 
-// The tile kernel needs N >= 8 on every axis (8 x 8 x TZ tiles, single conditional wraps); tiny grids use the
-// per-particle kernel.
-bool naive_spread(const tild_ctx* c)
+// out[i][0..2] = F4[inv[i]].xyz: per-slot results of a stage call back to caller order (inv: source slot = id -> slot)
+__global__ void __launch_bounds__(256) gather_by_inv_kernel(int n, const uint32_t* __restrict__ inv, const float4* __restrict__ F4,
+                                                            float* __restrict__ out)
 {
-    return (c->prm.flags & TILD_FLAG_NAIVE_SPREAD) != 0 || !c->tile.enabled;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const float4 f = F4[inv[i]];
+    out[3 * (size_t)i + 0] = f.x;
+    out[3 * (size_t)i + 1] = f.y;
+    out[3 * (size_t)i + 2] = f.z;
 }
 
-// spread -> R2C -> k-space -> C2R on the internal (tile-sorted) particle arrays, with optional stage events
-int mesh_pipeline(tild_ctx* c, const float* x, const int32_t* type, cudaEvent_t* ev)
+// spread -> R2C -> k-space -> C2R on slab-ordered particles, with optional stage events
+int mesh_pipeline(tild_ctx* c, const EllLayout& lay, const float4* X4, cudaEvent_t* ev)
 {
-    int rc = naive_spread(c) ? launch_spread_naive(c, x, type, c->grid) : launch_spread_tiled(c, c->tile_start, x, c->grid);
+    int rc = launch_spread(c, lay, X4, c->grid);
     if (rc) return rc;
     if (ev) cudaEventRecord(ev[2], c->stream);
     TILD_FFT(c, cufftExecR2C(c->plan_r2c, c->grid, reinterpret_cast<cufftComplex*>(c->nhat)));
@@ -172,16 +192,21 @@ int mesh_pipeline(tild_ctx* c, const float* x, const int32_t* type, cudaEvent_t*
     return TILD_OK;
 }
 
-// total force at the current internal positions -> c->fpart (internal order); no state change
+// total force at the current internal positions -> c->F4 (per slot); no state change
 int force_current(tild_ctx* c)
 {
     const int a = c->cur;
-    int rc = mesh_pipeline(c, c->x[a], c->type[a], nullptr);
+    int rc = mesh_pipeline(c, c->lay, c->X4[a], nullptr);
     if (rc) return rc;
-    rc = launch_interp_force(c, c->ffield, c->x[a], c->type[a], c->fpart);
+    return launch_interp(c, INTERP_TOTAL_BY_SLOT, c->lay, c->ffield, c->X4[a], c->W4[a], c->B[a], nullptr, nullptr, nullptr);
+}
+
+// caller (x, type) -> slab-ordered copy in c->SX4 described by c->lay_stage; c->inv maps id -> slot
+int stage_layout(tild_ctx* c, const float* x, const int32_t* type)
+{
+    int rc = launch_pack(c, x, nullptr, type, nullptr, c->F4, nullptr, nullptr);
     if (rc) return rc;
-    if (c->stp.max_bonds > 0) rc = launch_bond_force(c, c->x[a], c->bond[a], c->fpart, true);
-    return rc;
+    return launch_build_ell(c, (size_t)c->mesh.n, c->F4, c->SX4, &c->lay_stage);
 }
 
 }  // namespace
@@ -303,7 +328,7 @@ int tild_init(tild_ctx** out, const tild_params* params, void* workspace, size_t
         return TILD_ECUFFT;
     }
     c->plans_ok = true;
-    if ((rc = tild_spread_configure(c)) != TILD_OK) {
+    if ((rc = tild_spread_configure(c)) != TILD_OK || (rc = tild_interp_configure(c)) != TILD_OK) {
         cufftDestroy(c->plan_r2c);
         cufftDestroy(c->plan_c2r);
         delete c;
@@ -336,13 +361,23 @@ void tild_destroy(tild_ctx* c)
 const char* tild_last_error(const tild_ctx* c) { return c ? c->err : "null context"; }
 int64_t tild_launch_count(const tild_ctx* c) { return c ? c->launches : 0; }
 
+int tild_layout_info(const tild_ctx* c, uint64_t info[8])
+{
+    if (!c || !info) return TILD_EINVAL;
+    if (!c->has_state) return TILD_ESTATE;
+    const TileParams& t = c->tile;
+    const uint64_t v[8] = {(uint64_t)t.ntiles, (uint64_t)t.nseg, (uint64_t)t.cap, (uint64_t)c->lay.total_ell, (uint64_t)c->lay.n_ovf,
+                           (uint64_t)t.T[0], (uint64_t)t.T[1], (uint64_t)t.T[2]};
+    for (int k = 0; k < 8; ++k) info[k] = v[k];
+    return TILD_OK;
+}
+
 int tild_spread(tild_ctx* c, const float* x, const int32_t* type, float* grid)
 {
     if (!c || !grid || (c->mesh.n > 0 && (!x || !type))) return tild_fail(c, TILD_EINVAL, "tild_spread: null argument");
-    if (naive_spread(c)) return launch_spread_naive(c, x, type, grid);
-    int rc = launch_stage_sort(c, x, type);  // tile-major sorted copy of the caller's particles
+    int rc = stage_layout(c, x, type);  // slab-ordered copy of the caller's particles
     if (rc) return rc;
-    return launch_spread_tiled(c, c->cell_start, c->stage_x, grid);
+    return launch_spread(c, c->lay_stage, c->SX4, grid);
 }
 
 int tild_kspace_force(tild_ctx* c, const float* grid, float* ffield)
@@ -358,14 +393,22 @@ int tild_kspace_force(tild_ctx* c, const float* grid, float* ffield)
 int tild_interp(tild_ctx* c, const float* ffield, const float* x, const int32_t* type, float* f)
 {
     if (!c || !ffield || (c->mesh.n > 0 && (!x || !type || !f))) return tild_fail(c, TILD_EINVAL, "tild_interp: null argument");
-    return launch_interp_force(c, ffield, x, type, f);
+    const int n = c->mesh.n;
+    if (n == 0) return TILD_OK;
+    int rc = stage_layout(c, x, type);
+    if (rc) return rc;
+    rc = launch_interp(c, INTERP_NONBONDED_BY_ID, c->lay_stage, ffield, c->SX4, nullptr, nullptr, nullptr, nullptr, nullptr);
+    if (rc) return rc;
+    gather_by_inv_kernel<<<(n + 255) / 256, 256, 0, c->stream>>>(n, c->inv, c->F4, f);
+    TILD_LAUNCH_CHECK(c, "gather_by_inv_kernel");
+    return TILD_OK;
 }
 
 int tild_bond_force(tild_ctx* c, const float* x, const int32_t* bond_partner, float* f)
 {
     if (!c || (c->mesh.n > 0 && (!x || !f))) return tild_fail(c, TILD_EINVAL, "tild_bond_force: null argument");
     if (c->stp.max_bonds > 0 && !bond_partner && c->mesh.n > 0) return tild_fail(c, TILD_EINVAL, "tild_bond_force: null partners");
-    return launch_bond_force(c, x, bond_partner, f, false);
+    return launch_bond_force_caller(c, x, bond_partner, f);
 }
 
 int tild_index_map(tild_ctx* c, const float* x, int32_t* base, uint32_t* cell_key, uint32_t* perm, uint32_t* cell_start)
@@ -374,7 +417,7 @@ int tild_index_map(tild_ctx* c, const float* x, int32_t* base, uint32_t* cell_ke
     uint32_t* key = cell_key ? cell_key : c->key;
     int rc = launch_cell_keys(c, x, key, base);
     if (rc) return rc;
-    if (perm || cell_start) rc = launch_counting_sort(c, key, c->M, perm ? perm : c->perm, cell_start ? cell_start : c->cell_start);
+    if (perm || cell_start) rc = launch_counting_sort(c, key, c->M, perm ? perm : c->perm, cell_start ? cell_start : c->start);
     return rc;
 }
 
@@ -391,23 +434,13 @@ int tild_set_state(tild_ctx* c, const float* x, const float* v, const int32_t* t
     if (n > 0 && (!x || !v || !type)) return tild_fail(c, TILD_EINVAL, "tild_set_state: null argument");
     if (n > 0 && c->stp.max_bonds > 0 && !bond_partner) return tild_fail(c, TILD_EINVAL, "tild_set_state: null bond_partner");
     c->cur = 0;
-    if (n > 0) {
-        // cudaMemcpyDefault: the sources may be device (stage API) or host (tild_run_host) pointers
-        TILD_CUDA(c, cudaMemcpyAsync(c->x[0], x, 3 * n * sizeof(float), cudaMemcpyDefault, c->stream));
-        TILD_CUDA(c, cudaMemcpyAsync(c->w[0], v, 3 * n * sizeof(float), cudaMemcpyDefault, c->stream));
-        TILD_CUDA(c, cudaMemcpyAsync(c->type[0], type, n * sizeof(int32_t), cudaMemcpyDefault, c->stream));
-        if (c->stp.max_bonds > 0)
-            TILD_CUDA(c, cudaMemcpyAsync(c->bond[0], bond_partner, n * c->stp.max_bonds * sizeof(int32_t), cudaMemcpyDefault,
-                                         c->stream));
-        iota_kernel<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>((int)n, c->id[0]);
-        TILD_LAUNCH_CHECK(c, "iota_kernel");
-    }
-    int rc = launch_reorder(c);
+    int rc = launch_pack(c, x, v, type, c->stp.max_bonds > 0 ? bond_partner : nullptr, c->X4[0], c->W4[0], c->B[0]);
     if (rc) return rc;
-    rc = force_current(c);
-    if (rc) return rc;
-    rc = launch_make_w(c, c->fpart, c->w[c->cur], -1.0f);  // w = v - (dt/2m) F
-    if (rc) return rc;
+    c->lay.total_ell = 0;   // slots [0, n) in id order: all of it is "tail" until the first re-sort
+    c->lay.n_ovf = n;
+    if ((rc = launch_reorder(c))) return rc;
+    if ((rc = force_current(c))) return rc;
+    if ((rc = launch_make_w(c, c->lay.used(), c->F4, c->W4[c->cur], -1.0f))) return rc;  // w = v - (dt/2m) F
     c->step = step0;
     c->has_state = true;
     c->timed_steps = 0;
@@ -423,14 +456,18 @@ int tild_step(tild_ctx* c, int32_t nsteps)
         cudaEvent_t* ev = (c->ev_ok && c->timed_steps < TILD_MAX_TIMED_STEPS) ? c->ev[c->timed_steps] : nullptr;
         if (ev) cudaEventRecord(ev[0], c->stream);
         if (c->steps_since_sort >= c->resort_every) {
-            int rc = launch_reorder(c);
+            int rc = launch_reorder(c);   // synchronises once (8-byte read-back of the layout totals)
             if (rc) return rc;
         }
         if (ev) cudaEventRecord(ev[1], c->stream);
-        int rc = mesh_pipeline(c, c->x[c->cur], c->type[c->cur], ev);
+        const int a = c->cur;
+        int rc = mesh_pipeline(c, c->lay, c->X4[a], ev);
         if (rc) return rc;
-        rc = launch_fused_step(c);
+        rc = launch_interp(c, INTERP_FUSED_STEP, c->lay, c->ffield, c->X4[a], c->W4[a], c->B[a], c->X4[1 - a], c->W4[1 - a], nullptr);
         if (rc) return rc;
+        // swap only the x/w pointers so that `cur` keeps naming the buffer that holds the bond table
+        float4* t = c->X4[a]; c->X4[a] = c->X4[1 - a]; c->X4[1 - a] = t;
+        t = c->W4[a]; c->W4[a] = c->W4[1 - a]; c->W4[1 - a] = t;
         if (ev) {
             cudaEventRecord(ev[6], c->stream);
             c->timed_steps++;
@@ -450,23 +487,20 @@ int tild_get_state(tild_ctx* c, float* x, float* v, float* f, uint64_t* step)
     if (step) *step = c->step;
     if (n == 0) return TILD_OK;
     const int a = c->cur;
-    float* scratch = c->x[1 - a];  // the inactive position buffer is free between steps
+    float* scratch = reinterpret_cast<float*>(c->SX4);  // [n][3] staging in caller order; x/v/f may be host pointers
     int rc;
     if (x) {
-        if ((rc = launch_unpermute(c, c->x[a], scratch, 3))) return rc;
+        if ((rc = launch_unpermute(c, c->X4[a], scratch))) return rc;
         TILD_CUDA(c, cudaMemcpyAsync(x, scratch, bytes, cudaMemcpyDefault, c->stream));
     }
     if (v || f) {
         if ((rc = force_current(c))) return rc;
         if (f) {
-            if ((rc = launch_unpermute(c, c->fpart, scratch, 3))) return rc;
+            if ((rc = launch_unpermute(c, c->F4, scratch))) return rc;
             TILD_CUDA(c, cudaMemcpyAsync(f, scratch, bytes, cudaMemcpyDefault, c->stream));
         }
         if (v) {
-            float* vs = c->w[1 - a];
-            TILD_CUDA(c, cudaMemcpyAsync(vs, c->w[a], bytes, cudaMemcpyDeviceToDevice, c->stream));
-            if ((rc = launch_make_w(c, c->fpart, vs, +1.0f))) return rc;  // v = w + (dt/2m) F
-            if ((rc = launch_unpermute(c, vs, scratch, 3))) return rc;
+            if ((rc = launch_velocity_out(c, c->lay.used(), c->F4, c->W4[a], scratch))) return rc;  // v = w + (dt/2m) F
             TILD_CUDA(c, cudaMemcpyAsync(v, scratch, bytes, cudaMemcpyDefault, c->stream));
         }
     }
@@ -501,7 +535,23 @@ int tild_get_timings(tild_ctx* c, float ms[8], int32_t* steps_timed)
 int tild_run_host(tild_ctx* c, float* x_host, float* v_host, const int32_t* type_host, const int32_t* bond_partner_host,
                   uint64_t step0, int32_t nsteps)
 {
-    int rc = tild_set_state(c, x_host, v_host, type_host, bond_partner_host, step0);
+    if (!c) return TILD_EINVAL;
+    const size_t n = (size_t)c->mesh.n;
+    const size_t mb = (size_t)c->stp.max_bonds;
+    if (n > 0 && (!x_host || !v_host || !type_host || (mb > 0 && !bond_partner_host)))
+        return tild_fail(c, TILD_EINVAL, "tild_run_host: null argument");
+    // device staging of the host batch: x, v, type in SX4 (28 n bytes <= 16 cap), bond partners in F4
+    float* xs = reinterpret_cast<float*>(c->SX4);
+    float* vs = xs + 3 * n;
+    int32_t* ts = reinterpret_cast<int32_t*>(vs + 3 * n);
+    int32_t* bs = reinterpret_cast<int32_t*>(c->F4);
+    if (n > 0) {
+        TILD_CUDA(c, cudaMemcpyAsync(xs, x_host, 3 * n * sizeof(float), cudaMemcpyHostToDevice, c->stream));
+        TILD_CUDA(c, cudaMemcpyAsync(vs, v_host, 3 * n * sizeof(float), cudaMemcpyHostToDevice, c->stream));
+        TILD_CUDA(c, cudaMemcpyAsync(ts, type_host, n * sizeof(int32_t), cudaMemcpyHostToDevice, c->stream));
+        if (mb > 0) TILD_CUDA(c, cudaMemcpyAsync(bs, bond_partner_host, n * mb * sizeof(int32_t), cudaMemcpyHostToDevice, c->stream));
+    }
+    int rc = tild_set_state(c, xs, vs, ts, bs, step0);
     if (rc) return rc;
     if ((rc = tild_step(c, nsteps))) return rc;
     if ((rc = tild_get_state(c, x_host, v_host, nullptr, nullptr))) return rc;

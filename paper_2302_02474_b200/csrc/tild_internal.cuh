@@ -19,17 +19,29 @@ struct MeshParams {
     long long M;     // Nx*Ny*Nz
 };
 
-// Tiling of the cell grid for the shared-memory spread (tild_spread.cu) and the tile-major particle order.
+// Tiling of the cell grid and the slab-transposed ("ELL") particle layout.
+// A tile is T[0] x T[1] x T[2] cells; its shared-memory image holds E = T + H nodes per axis (H = stencil halo),
+// with E[2] = EZ a multiple of 32 so that the bank of a node depends on its z only.  A "segment" is (tile, species).
+// Inside a segment particle slots are laid out round-major: slot = seg_base[seg] + round*32 + r with
+// r = (local z cell) mod 32, so lane r of a warp always works on a particle whose stencil starts at bank r + const:
+// every shared-memory access of the stencil is bank-conflict free, and a round is one coalesced 512-byte read.
 struct TileParams {
     int T[3];       // tile edge in cells (clipped to the grid)
     int nt[3];      // tiles per axis = ceil(N/T)
-    int E[3];       // shared tile edge in nodes = T + stencil halo + 2*margin
-    int lo;         // nodes below the tile's first cell held in shared memory (low halo + margin)
-    int TV;         // T[0]*T[1]*T[2]: cells per tile; sort key = (tile*S + species)*TV + local cell
+    int E[3];       // shared tile edge in nodes: E[0], E[1] = tile edge + H (template EY >= E[1]); E[2] = EZ
+    int lo;         // nodes below the tile's first cell that a stencil can touch (0 for P <= 2, 1 for P = 3, 4)
+    int sh;         // extra nodes below those so that the image starts on a 16-byte boundary of the mesh rows
+    int H;          // stencil halo in nodes (1 for P <= 2, 3 for P = 3, 4)
+    int EY, EZ;     // template strides the kernels were instantiated with
     int ntiles;
-    unsigned nbins; // ntiles*S*TV
-    size_t smem_bytes;
-    int enabled;    // 0: grid too small for the tile kernel (any N < 8) -> per-particle spread
+    int nseg;       // ntiles * S
+    int sp_group;   // species accumulated per spread CTA (shared-memory budget)
+    size_t cap_ell; // slots reserved for the ELL region
+    size_t cap;     // cap_ell + n + 32: total slots (the tail holds particles that overflow their segment)
+    float fill;     // rounds of a segment are capped at ceil(fill * mean lane length) + add
+    int add;
+    size_t smem_spread, smem_interp;
+    int enabled;    // 0: grid too small for the tile kernels -> per-particle kernels on every slot
 };
 
 struct KspaceParams {
@@ -55,6 +67,14 @@ struct StepParams {
 };
 
 // ---- context -----------------------------------------------------------------------------------
+// One slab-transposed ordering of a particle set: ELL region [0, total_ell), overflow tail [total_ell, used).
+struct EllLayout {
+    uint32_t* seg_base;  // device [nseg+1]: first slot of each segment; seg_base[nseg] = total_ell
+    size_t total_ell;    // host copies, refreshed by launch_build_ell (one 8-byte read-back per re-sort)
+    size_t n_ovf;
+    size_t used() const { return total_ell + n_ovf; }
+};
+
 struct tild_ctx {
     tild_params prm;
     cudaStream_t stream;
@@ -63,29 +83,32 @@ struct tild_ctx {
     StepParams stp;
     size_t M, Mk;
     TileParams tile;
-    size_t max_bins;      // max(M, tile.nbins)
+    size_t max_bins;      // max(M, nseg*32): histogram length
 
-    // carved from the caller's workspace
-    float* x[2];
-    float* w[2];
-    int32_t* type[2];
-    uint32_t* id[2];
-    int32_t* bond[2];
+    // carved from the caller's workspace.  Slot arrays have tile.cap entries.
+    float4* X4[2];        // (x, y, z, type as int bits); type < 0 marks a hole
+    float4* W4[2];        // (w_x, w_y, w_z, original id as uint bits)
+    int32_t* B[2];        // [cap][max_bonds] partner SLOTS, -1 = none
     int cur;
-    float* grid;        // [S][M]
-    float2* nhat;       // [S][Mk]
-    float2* fhat;       // [3S][Mk]
-    float* ffield;      // [3S][M]
-    float* fpart;       // [n][3] scratch forces (internal order)
-    uint32_t* key;      // [n]
-    uint32_t* perm;     // [n]
-    uint32_t* tile_start;  // [tile.nbins+1] tile-major cell offsets of the internal (sorted) state
-    uint32_t* cell_start;  // [max_bins+1] scratch offsets for tild_index_map / stage calls
-    uint32_t* cell_fill;   // [max_bins+1] histogram
-    uint32_t* scan_part;   // block sums for the scan, then rank[n]
-    float* stage_x;        // [n][3] sorted copy of caller positions (stage calls)
-    int32_t* stage_type;   // [n]
-    float* tables;      // k-space tables
+    float4* F4;           // [cap] per-slot force scratch
+    float4* SX4;          // [cap] stage-call scratch: slab-ordered copy of caller particles; caller-order staging
+    EllLayout lay, lay_stage;
+    float* grid;          // [S][M]
+    float2* nhat;         // [S][Mk]
+    float2* fhat;         // [3S][Mk]
+    float* ffield;        // [3S][M]
+    uint32_t* key;        // [cap]
+    uint32_t* rank;       // [cap]
+    uint32_t* inv;        // [cap] old slot -> new slot
+    uint32_t* count;      // [max_bins+1] histogram
+    uint32_t* start;      // [max_bins+1] scan output (cell_start of tild_index_map)
+    uint32_t* scan_part;  // block sums of the scan
+    uint32_t* holepref;   // [nseg*32] holes in the lanes before this one (launch_build_ell)
+    uint32_t* segholes;   // [nseg] holes of the segment
+    uint32_t* segtick;    // [nseg] tickets handed to particles that overflow their own lane
+    uint32_t* perm;       // [n] tild_index_map scratch
+    uint32_t* totals;     // [4] device counters: [0] = overflow count
+    float* tables;        // k-space tables
 
     cufftHandle plan_r2c, plan_c2r;
     bool plans_ok;
@@ -118,23 +141,32 @@ int tild_fail(tild_ctx* c, int code, const char* fmt, ...);
     } while (0)
 
 // ---- stage launchers (each enqueues on c->stream) -----------------------------------------------
+// tild_sort.cu
 int launch_cell_keys(tild_ctx* c, const float* x, uint32_t* key, int32_t* base /*nullable*/);  // row-major cell keys
-int launch_tile_keys(tild_ctx* c, const float* x, const int32_t* type, uint32_t* key);        // (tile, species, cell) keys
 int launch_counting_sort(tild_ctx* c, const uint32_t* key, size_t nbins, uint32_t* perm, uint32_t* start);
-int launch_reorder(tild_ctx* c);  // sorts the internal state by tile-major cell and flips buffers
-int launch_stage_sort(tild_ctx* c, const float* x, const int32_t* type);  // caller arrays -> stage_x/stage_type + cell_start
-int launch_spread_naive(tild_ctx* c, const float* x, const int32_t* type, float* grid);
-int launch_spread_tiled(tild_ctx* c, const uint32_t* cell_start, const float* x, float* grid);
+int launch_pack(tild_ctx* c, const float* x, const float* v, const int32_t* type, const int32_t* bond, float4* X4,
+                float4* W4, int32_t* B);                                  // caller arrays -> slots [0, n), slot i = id i
+// src slots [0, nsrc) -> slab-transposed dst; fills lay (incl. host totals: synchronises) and c->inv
+int launch_build_ell(tild_ctx* c, size_t nsrc, const float4* X4src, float4* X4dst, EllLayout* lay);
+int launch_reorder(tild_ctx* c);  // re-sorts the internal state and flips buffers
+int launch_unpermute(tild_ctx* c, const float4* src, float* dst);        // dst[id[s]][0..2] = src[s].xyz over used slots
+// tild_spread.cu
 int tild_spread_configure(tild_ctx* c);
+int launch_spread(tild_ctx* c, const EllLayout& lay, const float4* X4, float* grid);  // zero fill + tiles + overflow tail
+// tild_kspace.cu
 int launch_kspace(tild_ctx* c, const float2* nhat, float2* fhat);
-int launch_interp_force(tild_ctx* c, const float* ffield, const float* x, const int32_t* type, float* f);
-int launch_bond_force(tild_ctx* c, const float* x, const int32_t* bond, float* f, bool accumulate);
-int launch_fused_step(tild_ctx* c);  // interp + bonds + GJF on the internal state, flips x/w buffers
-int launch_make_w(tild_ctx* c, const float* f, float* w, float sign);  // w += sign*(dt/2m) f
+// tild_interp.cu
+int tild_interp_configure(tild_ctx* c);
+enum { INTERP_NONBONDED_BY_ID = 0, INTERP_TOTAL_BY_SLOT = 1, INTERP_FUSED_STEP = 2 };
+// mode 0: fout[id][3] = interpolated force; mode 1: c->F4[slot] = interpolated + bond force; mode 2: GJF step
+int launch_interp(tild_ctx* c, int mode, const EllLayout& lay, const float* ffield, const float4* X4, const float4* W4,
+                  const int32_t* B, float4* X4o, float4* W4o, float* fout);
+int launch_bond_force_caller(tild_ctx* c, const float* x, const int32_t* bond, float* f);  // caller-order stage call
+int launch_make_w(tild_ctx* c, size_t nslots, const float4* F4, float4* W4, float sign);   // w += sign*(dt/2m) f
+int launch_velocity_out(tild_ctx* c, size_t nslots, const float4* F4, const float4* W4, float* v);  // v[id] = w + (dt/2m) f
 int launch_philox_test(tild_ctx* c, const uint32_t* ctr, const uint32_t* key, uint32_t* out, float* gauss, int m);
-int launch_unpermute(tild_ctx* c, const float* src, float* dst, int ncomp);  // dst[id[i]] = src[i]
 
-size_t tild_scan_scratch_entries(size_t nbins, int n);
+size_t tild_scan_scratch_entries(size_t nbins);
 
 // ---- device helpers ------------------------------------------------------------------------------
 #ifdef __CUDACC__
@@ -162,6 +194,14 @@ __device__ __forceinline__ int wrap_idx(int a, int N)
 {
     a %= N;
     return a < 0 ? a + N : a;
+}
+
+// a in (-N, 2N): one conditional wrap each way (no integer division)
+__device__ __forceinline__ int wrap_near(int a, int N)
+{
+    a += a < 0 ? N : 0;
+    a -= a >= N ? N : 0;
+    return a;
 }
 
 // Order-P assignment weights (P-fold top-hat convolution; PAPER.md L223 -> Deserno & Holm appendix).

@@ -1,29 +1,27 @@
 // a6: mesh -> particle interpolation with the same weights (Fig. 1),
 // harmonic bonds computed per particle without Newton's third law (Eq. 2) and the GJF Langevin
 // update (L352; equations per DESIGN.md A11) fused into one pass over the particles.
+//
+// Hot kernel: one CTA per tile.  For each species present in the tile the three force-field components of the
+// tile (+ stencil halo) are staged into shared memory with coalesced cp.async row copies (periodic wrap applied
+// per row), then the particles of that (tile, species) segment are read round by round from the slab-transposed
+// layout (tild_sort.cu): lane r holds a particle whose z cell is r mod 32 and the shared image has a z extent that
+// is a multiple of 32, so the 3 P^3 shared-memory loads of the stencil are bank-conflict free.
 #include "tild_internal.cuh"
 
 namespace {
 
-// f_a = sum_{stencil} w_x w_y w_z ffield[type][a][g]
-//
+constexpr int INTERP_THREADS = 256;
+constexpr int INTERP_WARPS = INTERP_THREADS / 32;
+
+// ---- per-particle global gather (overflow tail, drifted particles, grids too small for tiles) -------------------
 // VEC = true (Nz % 4 == 0, 16-byte aligned field): the P nodes of one z-row are contiguous in memory but start at
 // an arbitrary z, so each row is read as the one or two ALIGNED float4 that cover it (LDG.128) and dotted with an
-// 8-wide weight vector holding w_z shifted to the row's offset and zeros elsewhere.  That halves the load
-// instructions of the scalar form; with the particles in tile-major cell order (z fastest) the lanes of a warp
-// read neighbouring z of the same rows, so each load touches few cache lines.
+// 8-wide weight vector holding w_z shifted to the row's offset and zeros elsewhere.
 template <int P, bool VEC>
-__device__ __forceinline__ float3 interp_one(const MeshParams& m, const float* __restrict__ ffield, float px, float py,
-                                             float pz, int type)
+__device__ __forceinline__ float3 interp_global(const MeshParams& m, const float* __restrict__ ffield, const int b[3],
+                                                const float w[3][P], int type)
 {
-    int cell, b[3];
-    float t, w[3][P];
-    index_1d<P>(px, m.inv_h[0], cell, b[0], t);
-    weights_1d<P>(t, w[0]);
-    index_1d<P>(py, m.inv_h[1], cell, b[1], t);
-    weights_1d<P>(t, w[1]);
-    index_1d<P>(pz, m.inv_h[2], cell, b[2], t);
-    weights_1d<P>(t, w[2]);
     const float* fx = ffield + (size_t)type * 3 * m.M;
     const float* fy = fx + m.M;
     const float* fz = fy + m.M;
@@ -91,16 +89,18 @@ __device__ __forceinline__ float3 interp_one(const MeshParams& m, const float* _
     return acc;
 }
 
-__device__ __forceinline__ float3 bond_force_one(const MeshParams& m, const StepParams& s, const float* __restrict__ x,
-                                                 const int32_t* __restrict__ bond, size_t i, float px, float py, float pz)
+// Bond force on the particle at p from its partners' positions (slots into X4).
+__device__ __forceinline__ float3 bond_force_slots(const MeshParams& m, const StepParams& s, const float4* __restrict__ X4,
+                                                   const int32_t* __restrict__ B, size_t slot, const float4& p)
 {
     float3 f = make_float3(0.f, 0.f, 0.f);
     for (int k = 0; k < s.max_bonds; ++k) {
-        const int32_t j = bond[i * s.max_bonds + k];
+        const int32_t j = B[slot * s.max_bonds + k];
         if (j < 0) continue;
-        const float dx = min_image(px - x[3 * (size_t)j + 0], m.L[0], m.inv_L[0]);
-        const float dy = min_image(py - x[3 * (size_t)j + 1], m.L[1], m.inv_L[1]);
-        const float dz = min_image(pz - x[3 * (size_t)j + 2], m.L[2], m.inv_L[2]);
+        const float4 q = X4[j];
+        const float dx = min_image(p.x - q.x, m.L[0], m.inv_L[0]);
+        const float dy = min_image(p.y - q.y, m.L[1], m.inv_L[1]);
+        const float dz = min_image(p.z - q.z, m.L[2], m.inv_L[2]);
         float scale = -2.0f * s.k_bond;
         if (s.r0_bond != 0.0f) {
             const float r = sqrtf(dx * dx + dy * dy + dz * dz);
@@ -113,78 +113,257 @@ __device__ __forceinline__ float3 bond_force_one(const MeshParams& m, const Step
     return f;
 }
 
-template <int P, bool VEC>
-__global__ void __launch_bounds__(256) interp_force_kernel(MeshParams m, const float* __restrict__ ffield,
-                                                           const float* __restrict__ x, const int32_t* __restrict__ type,
-                                                           float* __restrict__ f)
+// What happens to one particle once its interpolated force is known.
+//   MODE 0: F4[slot] = interpolated force            (stage call tild_interp)
+//   MODE 1: F4[slot] = interpolated + bond force     (tild_set_state / tild_get_state)
+//   MODE 2: one GJF step: state (r^n, w^n), w^n = v^n - (dt/2m) F^n.
+//     F^n = interp(r^n) + bonds(r^n);  v^n = w^n + (dt/2m) F^n;  beta = beta^{n+1} (Philox: id, step n+1)
+//     r^{n+1} = wrap(r^n + b dt v^n + (b dt^2/2m) F^n + (b dt/2m) beta)
+//     w^{n+1} = a v^n + (dt/2m) a F^n + (b/m) beta
+//   Positions are double-buffered because bonds read the partners' r^n while r^{n+1} is written.
+template <int MODE>
+__device__ __forceinline__ void finish_particle(const MeshParams& m, const StepParams& s, uint64_t step_next, size_t slot,
+                                                const float4& p, float3 F, const float4* __restrict__ X4,
+                                                const float4* __restrict__ W4, const int32_t* __restrict__ B,
+                                                float4* __restrict__ X4o, float4* __restrict__ W4o, float4* __restrict__ F4)
 {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= m.n) return;
-    const float3 a = interp_one<P, VEC>(m, ffield, x[3 * (size_t)i], x[3 * (size_t)i + 1], x[3 * (size_t)i + 2], type[i]);
-    f[3 * (size_t)i + 0] = a.x;
-    f[3 * (size_t)i + 1] = a.y;
-    f[3 * (size_t)i + 2] = a.z;
-}
-
-__global__ void __launch_bounds__(256) bond_force_kernel(MeshParams m, StepParams s, const float* __restrict__ x,
-                                                         const int32_t* __restrict__ bond, float* __restrict__ f,
-                                                         int accumulate)
-{
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= m.n) return;
-    const float3 b = bond_force_one(m, s, x, bond, (size_t)i, x[3 * (size_t)i], x[3 * (size_t)i + 1], x[3 * (size_t)i + 2]);
-    if (accumulate) {
-        f[3 * (size_t)i + 0] += b.x;
-        f[3 * (size_t)i + 1] += b.y;
-        f[3 * (size_t)i + 2] += b.z;
-    } else {
-        f[3 * (size_t)i + 0] = b.x;
-        f[3 * (size_t)i + 1] = b.y;
-        f[3 * (size_t)i + 2] = b.z;
+    if (MODE >= 1) {
+        const float3 fb = bond_force_slots(m, s, X4, B, slot, p);
+        F.x += fb.x;
+        F.y += fb.y;
+        F.z += fb.z;
     }
-}
-
-// One pass per step n: state (r^n, w^n), w^n = v^n - (dt/2m) F^n.
-//   F^n = interp(r^n) + bonds(r^n);  v^n = w^n + (dt/2m) F^n;  beta = beta^{n+1} (Philox: id, step n+1)
-//   r^{n+1} = wrap(r^n + b dt v^n + (b dt^2/2m) F^n + (b dt/2m) beta)
-//   w^{n+1} = a v^n + (dt/2m) a F^n + (b/m) beta
-// Positions are double-buffered because bonds read the partners' r^n while r^{n+1} is written.
-template <int P, bool VEC>
-__global__ void __launch_bounds__(256) fused_step_kernel(MeshParams m, StepParams s, uint64_t step_next,
-                                                         const float* __restrict__ ffield, const float* __restrict__ x0,
-                                                         const float* __restrict__ w0, const int32_t* __restrict__ type,
-                                                         const uint32_t* __restrict__ id, const int32_t* __restrict__ bond,
-                                                         float* __restrict__ x1, float* __restrict__ w1)
-{
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= m.n) return;
-    const float px = x0[3 * (size_t)i], py = x0[3 * (size_t)i + 1], pz = x0[3 * (size_t)i + 2];
-    float3 F = interp_one<P, VEC>(m, ffield, px, py, pz, type[i]);
-    const float3 fb = bond_force_one(m, s, x0, bond, (size_t)i, px, py, pz);
-    F.x += fb.x;
-    F.y += fb.y;
-    F.z += fb.z;
+    if (MODE <= 1) {
+        F4[slot] = make_float4(F.x, F.y, F.z, 0.f);
+        return;
+    }
+    const float4 w0 = W4[slot];
     float3 beta = make_float3(0.f, 0.f, 0.f);
     if (s.noise_amp != 0.0f) {
-        const float3 z = gauss3(id[i], step_next, s.key0, s.key1);
+        const float3 z = gauss3(__float_as_uint(w0.w), step_next, s.key0, s.key1);
         beta = make_float3(s.noise_amp * z.x, s.noise_amp * z.y, s.noise_amp * z.z);
     }
-    const float p[3] = {px, py, pz};
+    const float pp[3] = {p.x, p.y, p.z};
+    const float wv[3] = {w0.x, w0.y, w0.z};
     const float Fv[3] = {F.x, F.y, F.z};
     const float bv[3] = {beta.x, beta.y, beta.z};
+    float xo[3], wo[3];
 #pragma unroll
     for (int a = 0; a < 3; ++a) {
-        const float v = w0[3 * (size_t)i + a] + s.half_dt_over_m * Fv[a];
-        const float r = p[a] + (s.b_dt * v + s.b_dt2_over_2m * Fv[a] + s.b_dt_over_2m * bv[a]);
-        x1[3 * (size_t)i + a] = wrap_pos(r, m.L[a], m.inv_L[a]);
-        w1[3 * (size_t)i + a] = s.a_g * (v + s.half_dt_over_m * Fv[a]) + s.b_over_m * bv[a];
+        const float v = wv[a] + s.half_dt_over_m * Fv[a];
+        const float r = pp[a] + (s.b_dt * v + s.b_dt2_over_2m * Fv[a] + s.b_dt_over_2m * bv[a]);
+        xo[a] = wrap_pos(r, m.L[a], m.inv_L[a]);
+        wo[a] = s.a_g * (v + s.half_dt_over_m * Fv[a]) + s.b_over_m * bv[a];
+    }
+    X4o[slot] = make_float4(xo[0], xo[1], xo[2], p.w);
+    W4o[slot] = make_float4(wo[0], wo[1], wo[2], w0.w);
+}
+
+template <int P>
+__device__ __forceinline__ void index_weights(const MeshParams& m, const float4& p, int b[3], float w[3][P])
+{
+    const float pos[3] = {p.x, p.y, p.z};
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        int cell;
+        float t;
+        index_1d<P>(pos[a], m.inv_h[a], cell, b[a], t);
+        weights_1d<P>(t, w[a]);
     }
 }
 
-__global__ void __launch_bounds__(256) axpy_kernel(size_t len, float alpha, const float* __restrict__ f, float* __restrict__ w)
+// per-particle kernel over the slots [s0, s1)
+template <int P, bool VEC, int MODE>
+__global__ void __launch_bounds__(256) interp_slots_kernel(MeshParams m, StepParams s, uint64_t step_next, size_t s0, size_t s1,
+                                                           const float* __restrict__ ffield, const float4* __restrict__ X4,
+                                                           const float4* __restrict__ W4, const int32_t* __restrict__ B,
+                                                           float4* __restrict__ X4o, float4* __restrict__ W4o,
+                                                           float4* __restrict__ F4)
 {
-    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < len) w[i] += alpha * f[i];
+    const size_t slot = s0 + (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (slot >= s1) return;
+    const float4 p = X4[slot];
+    const int type = __float_as_int(p.w);
+    if (type < 0) return;
+    int b[3];
+    float w[3][P];
+    index_weights<P>(m, p, b, w);
+    const float3 F = interp_global<P, VEC>(m, ffield, b, w, type);
+    finish_particle<MODE>(m, s, step_next, slot, p, F, X4, W4, B, X4o, W4o, F4);
+}
+
+__device__ __forceinline__ void cp_async_f32(float* smem_dst, const float* gsrc)
+{
+    const unsigned sa = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;\n" ::"r"(sa), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cp_async_16(float* smem_dst, const float* gsrc)
+{
+    const unsigned sa = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(sa), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all()
+{
+    asm volatile("cp.async.commit_group;\ncp.async.wait_group 0;\n" ::: "memory");
+}
+
+// Shared image of one species' force field over the tile: fs[((lx*EY + ly)*3 + comp)*EZ + lz].
+template <int P, int EY, int EZ, int MODE>
+__global__ void __launch_bounds__(INTERP_THREADS) interp_tile_kernel(MeshParams m, TileParams tp, StepParams s, uint64_t step_next,
+                                                                     const uint32_t* __restrict__ seg_base,
+                                                                     const float* __restrict__ ffield,
+                                                                     const float4* __restrict__ X4, const float4* __restrict__ W4,
+                                                                     const int32_t* __restrict__ B, float4* __restrict__ X4o,
+                                                                     float4* __restrict__ W4o, float4* __restrict__ F4)
+{
+    extern __shared__ __align__(16) float fs[];
+    __shared__ int goff_x[32], goff_y[32];
+    const int EX = tp.E[0];
+    const int tile = blockIdx.x;
+    const int tz = tile % tp.nt[2], ty = (tile / tp.nt[2]) % tp.nt[1], tx = tile / (tp.nt[2] * tp.nt[1]);
+    const int o[3] = {tx * tp.T[0] - tp.lo, ty * tp.T[1] - tp.lo, tz * tp.T[2] - tp.lo - tp.sh};
+    const int E[3] = {EX, tp.E[1], EZ};
+    const size_t seg0 = (size_t)tile * m.S;
+    if (seg_base[seg0] == seg_base[seg0 + m.S]) return;   // empty tile (uniform)
+    if (threadIdx.x < EX) goff_x[threadIdx.x] = wrap_idx(o[0] + threadIdx.x, m.N[0]);
+    else if (threadIdx.x >= 32 && threadIdx.x < 32 + EY) goff_y[threadIdx.x - 32] = wrap_idx(o[1] + threadIdx.x - 32, m.N[1]);
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const bool vec16 = (m.N[2] % 4 == 0) && ((reinterpret_cast<uintptr_t>(ffield) & 15) == 0) && (m.M % 4 == 0);
+
+    for (int sp = 0; sp < m.S; ++sp) {
+        const uint32_t b0 = seg_base[seg0 + sp], rounds = (seg_base[seg0 + sp + 1] - b0) >> 5;
+        if (rounds == 0) continue;                         // uniform
+        __syncthreads();                                   // previous species' gathers are done; goff_* visible
+        {
+            // stage the field: one (x, y) column of the image per thread group, three components each
+            const float* fsp = ffield + (size_t)sp * 3 * m.M;
+            if (vec16) {
+                // 16-byte copies: the image starts on a 16-byte boundary of the mesh rows (tp.sh) and Nz % 4 == 0,
+                // so every aligned float4 of a row stays inside the row and wraps as a whole
+                constexpr int CPR = EZ / 4;                       // chunks per row
+                const int chunk = threadIdx.x % CPR;
+                const int gz = wrap_idx(o[2] + 4 * chunk, m.N[2]);
+                for (int q = threadIdx.x / CPR; q < EX * EY; q += INTERP_THREADS / CPR) {
+                    const int lx = q / EY, ly = q - lx * EY;
+                    if (ly >= E[1]) continue;
+                    const float* src = fsp + ((size_t)goff_x[lx] * m.N[1] + goff_y[ly]) * m.N[2] + gz;
+                    float* dst = fs + q * 3 * EZ + 4 * chunk;
+#pragma unroll
+                    for (int comp = 0; comp < 3; ++comp) cp_async_16(dst + comp * EZ, src + (size_t)comp * m.M);
+                }
+            } else {
+                const int lz = threadIdx.x % EZ;
+                const int gz = wrap_idx(o[2] + lz, m.N[2]);
+                for (int q = threadIdx.x / EZ; q < EX * EY; q += INTERP_THREADS / EZ) {
+                    const int lx = q / EY, ly = q - lx * EY;
+                    if (ly >= E[1]) continue;
+                    const float* src = fsp + ((size_t)goff_x[lx] * m.N[1] + goff_y[ly]) * m.N[2] + gz;
+                    float* dst = fs + q * 3 * EZ + lz;
+#pragma unroll
+                    for (int comp = 0; comp < 3; ++comp) cp_async_f32(dst + comp * EZ, src + (size_t)comp * m.M);
+                }
+            }
+            cp_async_wait_all();
+        }
+        __syncthreads();
+        for (uint32_t k = wid; k < rounds; k += INTERP_WARPS) {
+            const size_t slot = (size_t)b0 + (size_t)k * 32u + lane;
+            const float4 p = X4[slot];
+            if (__float_as_int(p.w) < 0) continue;         // hole
+            int b[3], d[3];
+            float w[3][P];
+            index_weights<P>(m, p, b, w);
+            bool inside = true;
+#pragma unroll
+            for (int a = 0; a < 3; ++a) {
+                d[a] = wrap_near(b[a] - o[a], m.N[a]);
+                inside = inside && (d[a] + P <= E[a]);
+            }
+            float3 F;
+            if (inside) {
+                const float* base = fs + ((d[0] * EY + d[1]) * 3) * EZ + d[2];
+                F = make_float3(0.f, 0.f, 0.f);
+#pragma unroll
+                for (int jx = 0; jx < P; ++jx) {
+#pragma unroll
+                    for (int jy = 0; jy < P; ++jy) {
+                        const float* row = base + ((jx * EY + jy) * 3) * EZ;
+                        float tx_ = 0.f, ty_ = 0.f, tz_ = 0.f;
+#pragma unroll
+                        for (int jz = 0; jz < P; ++jz) {
+                            tx_ = fmaf(w[2][jz], row[jz], tx_);
+                            ty_ = fmaf(w[2][jz], row[EZ + jz], ty_);
+                            tz_ = fmaf(w[2][jz], row[2 * EZ + jz], tz_);
+                        }
+                        const float wxy = w[0][jx] * w[1][jy];
+                        F.x = fmaf(wxy, tx_, F.x);
+                        F.y = fmaf(wxy, ty_, F.y);
+                        F.z = fmaf(wxy, tz_, F.z);
+                    }
+                }
+            } else {
+                F = interp_global<P, false>(m, ffield, b, w, sp); // drifted out of the tile's halo since the last re-sort
+            }
+            finish_particle<MODE>(m, s, step_next, slot, p, F, X4, W4, B, X4o, W4o, F4);
+        }
+    }
+}
+
+// caller-order bond force (stage call)
+__global__ void __launch_bounds__(256) bond_force_kernel(MeshParams m, StepParams s, const float* __restrict__ x,
+                                                         const int32_t* __restrict__ bond, float* __restrict__ f)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= m.n) return;
+    const float px = x[3 * (size_t)i], py = x[3 * (size_t)i + 1], pz = x[3 * (size_t)i + 2];
+    float3 acc = make_float3(0.f, 0.f, 0.f);
+    for (int k = 0; k < s.max_bonds; ++k) {
+        const int32_t j = bond[(size_t)i * s.max_bonds + k];
+        if (j < 0) continue;
+        const float dx = min_image(px - x[3 * (size_t)j + 0], m.L[0], m.inv_L[0]);
+        const float dy = min_image(py - x[3 * (size_t)j + 1], m.L[1], m.inv_L[1]);
+        const float dz = min_image(pz - x[3 * (size_t)j + 2], m.L[2], m.inv_L[2]);
+        float scale = -2.0f * s.k_bond;
+        if (s.r0_bond != 0.0f) {
+            const float r = sqrtf(dx * dx + dy * dy + dz * dz);
+            scale = r > 0.0f ? scale * (1.0f - s.r0_bond / r) : 0.0f;
+        }
+        acc.x += scale * dx;
+        acc.y += scale * dy;
+        acc.z += scale * dz;
+    }
+    f[3 * (size_t)i + 0] = acc.x;
+    f[3 * (size_t)i + 1] = acc.y;
+    f[3 * (size_t)i + 2] = acc.z;
+}
+
+// w.xyz += alpha * f.xyz on occupied slots
+__global__ void __launch_bounds__(256) axpy_slots_kernel(size_t nslots, float alpha, const float4* __restrict__ F4, float4* __restrict__ W4)
+{
+    const size_t s = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= nslots) return;
+    float4 w = W4[s];
+    if (__float_as_uint(w.w) == 0xFFFFFFFFu) return;
+    const float4 f = F4[s];
+    w.x += alpha * f.x;
+    w.y += alpha * f.y;
+    w.z += alpha * f.z;
+    W4[s] = w;
+}
+
+// v[id] = w + alpha f
+__global__ void __launch_bounds__(256) velocity_out_kernel(size_t nslots, float alpha, const float4* __restrict__ F4,
+                                                           const float4* __restrict__ W4, float* __restrict__ v)
+{
+    const size_t s = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= nslots) return;
+    const float4 w = W4[s];
+    const uint32_t id = __float_as_uint(w.w);
+    if (id == 0xFFFFFFFFu) return;
+    const float4 f = F4[s];
+    v[3 * (size_t)id + 0] = w.x + alpha * f.x;
+    v[3 * (size_t)id + 1] = w.y + alpha * f.y;
+    v[3 * (size_t)id + 2] = w.z + alpha * f.z;
 }
 
 __global__ void philox_test_kernel(int m, const uint32_t* __restrict__ ctr, const uint32_t* __restrict__ key,
@@ -206,81 +385,138 @@ __global__ void philox_test_kernel(int m, const uint32_t* __restrict__ ctr, cons
     }
 }
 
-}  // namespace
-
-static bool can_vectorize(const tild_ctx* c, const float* ffield)
+bool can_vectorize(const tild_ctx* c, const float* ffield)
 {
     return (c->mesh.N[2] % 4 == 0) && (reinterpret_cast<uintptr_t>(ffield) % 16 == 0) && !(c->prm.flags & TILD_FLAG_NAIVE_INTERP);
 }
 
-int launch_interp_force(tild_ctx* c, const float* ffield, const float* x, const int32_t* type, float* f)
+// ---- dispatch ------------------------------------------------------------------------------------------------------
+struct InterpArgs {
+    MeshParams m;
+    TileParams tp;
+    StepParams s;
+    uint64_t step_next;
+    const uint32_t* seg_base;
+    const float* ffield;
+    const float4* X4;
+    const float4* W4;
+    const int32_t* B;
+    float4* X4o;
+    float4* W4o;
+    float4* F4;
+};
+
+template <int P, int EY, int EZ, int MODE>
+void tile_launch(const InterpArgs& a, cudaStream_t st, size_t smem, bool configure_only, cudaError_t* err)
 {
-    const int n = c->mesh.n;
-    if (n == 0) return TILD_OK;
-    const int nb = (n + 255) / 256;
-    const bool vec = can_vectorize(c, ffield);
-#define IF(PP)                                                                                          \
-    if (vec) interp_force_kernel<PP, true><<<nb, 256, 0, c->stream>>>(c->mesh, ffield, x, type, f);     \
-    else interp_force_kernel<PP, false><<<nb, 256, 0, c->stream>>>(c->mesh, ffield, x, type, f)
-    switch (c->mesh.P) {
-    case 1: IF(1); break;
-    case 2: IF(2); break;
-    case 3: IF(3); break;
-    default: IF(4); break;
+    auto kernel = interp_tile_kernel<P, EY, EZ, MODE>;
+    if (configure_only) {
+        const cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) *err = e;
+        return;
     }
-#undef IF
-    TILD_LAUNCH_CHECK(c, "interp_force_kernel");
+    kernel<<<a.tp.ntiles, INTERP_THREADS, smem, st>>>(a.m, a.tp, a.s, a.step_next, a.seg_base, a.ffield, a.X4, a.W4, a.B, a.X4o,
+                                                      a.W4o, a.F4);
+}
+template <int P, int EY, int EZ>
+void tile_launch_m(const InterpArgs& a, int mode, cudaStream_t st, size_t smem, bool cfg, cudaError_t* err)
+{
+    if (cfg || mode == 0) tile_launch<P, EY, EZ, 0>(a, st, smem, cfg, err);
+    if (cfg || mode == 1) tile_launch<P, EY, EZ, 1>(a, st, smem, cfg, err);
+    if (cfg || mode == 2) tile_launch<P, EY, EZ, 2>(a, st, smem, cfg, err);
+}
+template <int P>
+bool tile_launch_p(const InterpArgs& a, int ey, int ez, int mode, cudaStream_t st, size_t smem, bool cfg, cudaError_t* err)
+{
+    constexpr int H = (P >= 3) ? 3 : 1;
+    if (ey == 8 + H && ez == 32) tile_launch_m<P, 8 + H, 32>(a, mode, st, smem, cfg, err);
+    else if (ey == 8 + H && ez == 64) tile_launch_m<P, 8 + H, 64>(a, mode, st, smem, cfg, err);
+    else if (ey == 16 + H && ez == 32) tile_launch_m<P, 16 + H, 32>(a, mode, st, smem, cfg, err);
+    else if (ey == 16 + H && ez == 64) tile_launch_m<P, 16 + H, 64>(a, mode, st, smem, cfg, err);
+    else return false;
+    return true;
+}
+bool tile_launch_any(const InterpArgs& a, int mode, cudaStream_t st, size_t smem, bool cfg, cudaError_t* err)
+{
+    switch (a.m.P) {
+    case 1: return tile_launch_p<1>(a, a.tp.EY, a.tp.EZ, mode, st, smem, cfg, err);
+    case 2: return tile_launch_p<2>(a, a.tp.EY, a.tp.EZ, mode, st, smem, cfg, err);
+    case 3: return tile_launch_p<3>(a, a.tp.EY, a.tp.EZ, mode, st, smem, cfg, err);
+    default: return tile_launch_p<4>(a, a.tp.EY, a.tp.EZ, mode, st, smem, cfg, err);
+    }
+}
+
+template <int P>
+void slots_launch_p(const InterpArgs& a, bool vec, int mode, size_t s0, size_t s1, cudaStream_t st)
+{
+    const unsigned nb = (unsigned)((s1 - s0 + 255) / 256);
+#define TILD_SL(V, M_) interp_slots_kernel<P, V, M_><<<nb, 256, 0, st>>>(a.m, a.s, a.step_next, s0, s1, a.ffield, a.X4, a.W4, a.B, a.X4o, a.W4o, a.F4)
+    if (vec) { if (mode == 0) TILD_SL(true, 0); else if (mode == 1) TILD_SL(true, 1); else TILD_SL(true, 2); }
+    else     { if (mode == 0) TILD_SL(false, 0); else if (mode == 1) TILD_SL(false, 1); else TILD_SL(false, 2); }
+#undef TILD_SL
+}
+
+}  // namespace
+
+int tild_interp_configure(tild_ctx* c)
+{
+    if (!c->tile.enabled) return TILD_OK;
+    InterpArgs a{};
+    a.m = c->mesh;
+    a.tp = c->tile;
+    cudaError_t e = cudaSuccess;
+    if (!tile_launch_any(a, 0, c->stream, c->tile.smem_interp, true, &e))
+        return tild_fail(c, TILD_EINVAL, "no interp tile kernel for P=%d EY=%d EZ=%d", c->mesh.P, c->tile.EY, c->tile.EZ);
+    if (e != cudaSuccess)
+        return tild_fail(c, TILD_ECUDA, "cudaFuncSetAttribute(interp_tile_kernel, %zu B): %s", c->tile.smem_interp, cudaGetErrorString(e));
     return TILD_OK;
 }
 
-int launch_bond_force(tild_ctx* c, const float* x, const int32_t* bond, float* f, bool accumulate)
+int launch_interp(tild_ctx* c, int mode, const EllLayout& lay, const float* ffield, const float4* X4, const float4* W4,
+                  const int32_t* B, float4* X4o, float4* W4o, float* /*unused*/)
+{
+    if (c->mesh.n == 0) return TILD_OK;
+    InterpArgs a{c->mesh, c->tile, c->stp, c->step + 1, lay.seg_base, ffield, X4, W4, B, X4o, W4o, c->F4};
+    const bool vec = can_vectorize(c, ffield);
+    if (c->tile.enabled && lay.total_ell > 0) {
+        cudaError_t e = cudaSuccess;
+        tile_launch_any(a, mode, c->stream, c->tile.smem_interp, false, &e);
+        TILD_LAUNCH_CHECK(c, "interp_tile_kernel");
+    }
+    if (lay.n_ovf > 0) {
+        switch (c->mesh.P) {
+        case 1: slots_launch_p<1>(a, vec, mode, lay.total_ell, lay.used(), c->stream); break;
+        case 2: slots_launch_p<2>(a, vec, mode, lay.total_ell, lay.used(), c->stream); break;
+        case 3: slots_launch_p<3>(a, vec, mode, lay.total_ell, lay.used(), c->stream); break;
+        default: slots_launch_p<4>(a, vec, mode, lay.total_ell, lay.used(), c->stream); break;
+        }
+        TILD_LAUNCH_CHECK(c, "interp_slots_kernel");
+    }
+    return TILD_OK;
+}
+
+int launch_bond_force_caller(tild_ctx* c, const float* x, const int32_t* bond, float* f)
 {
     const int n = c->mesh.n;
     if (n == 0) return TILD_OK;
-    bond_force_kernel<<<(n + 255) / 256, 256, 0, c->stream>>>(c->mesh, c->stp, x, bond, f, accumulate ? 1 : 0);
+    bond_force_kernel<<<(n + 255) / 256, 256, 0, c->stream>>>(c->mesh, c->stp, x, bond, f);
     TILD_LAUNCH_CHECK(c, "bond_force_kernel");
     return TILD_OK;
 }
 
-int launch_fused_step(tild_ctx* c)
+int launch_make_w(tild_ctx* c, size_t nslots, const float4* F4, float4* W4, float sign)
 {
-    const int n = c->mesh.n;
-    const int a = c->cur;
-    // x/w flip between the two buffers; type/id/bond stay in buffer `cur` (they only move on a reorder)
-    float* x0 = c->x[a];
-    float* w0 = c->w[a];
-    float* x1 = c->x[1 - a];
-    float* w1 = c->w[1 - a];
-    if (n > 0) {
-        const int nb = (n + 255) / 256;
-        const uint64_t sn = c->step + 1;
-        const bool vec = can_vectorize(c, c->ffield);
-#define FS(PP)                                                                                                          \
-    if (vec) fused_step_kernel<PP, true><<<nb, 256, 0, c->stream>>>(c->mesh, c->stp, sn, c->ffield, x0, w0, c->type[a], c->id[a], c->bond[a], x1, w1); \
-    else fused_step_kernel<PP, false><<<nb, 256, 0, c->stream>>>(c->mesh, c->stp, sn, c->ffield, x0, w0, c->type[a], c->id[a], c->bond[a], x1, w1)
-        switch (c->mesh.P) {
-        case 1: FS(1); break;
-        case 2: FS(2); break;
-        case 3: FS(3); break;
-        default: FS(4); break;
-        }
-#undef FS
-        TILD_LAUNCH_CHECK(c, "fused_step_kernel");
-    }
-    // swap only the x/w pointers so that `cur` keeps naming the buffer that holds type/id/bond
-    c->x[a] = x1;
-    c->x[1 - a] = x0;
-    c->w[a] = w1;
-    c->w[1 - a] = w0;
+    if (nslots == 0) return TILD_OK;
+    axpy_slots_kernel<<<(unsigned)((nslots + 255) / 256), 256, 0, c->stream>>>(nslots, sign * c->stp.half_dt_over_m, F4, W4);
+    TILD_LAUNCH_CHECK(c, "axpy_slots_kernel");
     return TILD_OK;
 }
 
-int launch_make_w(tild_ctx* c, const float* f, float* w, float sign)
+int launch_velocity_out(tild_ctx* c, size_t nslots, const float4* F4, const float4* W4, float* v)
 {
-    const size_t len = 3 * (size_t)c->mesh.n;
-    if (len == 0) return TILD_OK;
-    axpy_kernel<<<(unsigned)((len + 255) / 256), 256, 0, c->stream>>>(len, sign * c->stp.half_dt_over_m, f, w);
-    TILD_LAUNCH_CHECK(c, "axpy_kernel");
+    if (nslots == 0) return TILD_OK;
+    velocity_out_kernel<<<(unsigned)((nslots + 255) / 256), 256, 0, c->stream>>>(nslots, c->stp.half_dt_over_m, F4, W4, v);
+    TILD_LAUNCH_CHECK(c, "velocity_out_kernel");
     return TILD_OK;
 }
 

@@ -24,7 +24,7 @@ TIMING_NAMES = ("sort", "spread", "fft_fwd", "kspace", "fft_inv", "interp", "oth
 EXPORTS = (
     "tild_workspace_bytes", "tild_init", "tild_set_state", "tild_spread", "tild_kspace_force", "tild_interp",
     "tild_bond_force", "tild_step", "tild_get_state", "tild_index_map", "tild_get_timings", "tild_run_host",
-    "tild_philox_test", "tild_launch_count", "tild_last_error", "tild_destroy", "tild_version",
+    "tild_philox_test", "tild_layout_info", "tild_launch_count", "tild_last_error", "tild_destroy", "tild_version",
 )
 
 
@@ -103,6 +103,7 @@ def load():
     lib.tild_get_timings.argtypes = [vp, C.POINTER(C.c_float * 8), C.POINTER(i32)]
     lib.tild_run_host.argtypes = [vp, vp, vp, vp, vp, u64, i32]
     lib.tild_philox_test.argtypes = [vp, vp, vp, vp, vp, i32]
+    lib.tild_layout_info.argtypes = [vp, C.POINTER(C.c_uint64 * 8)]
     lib.tild_launch_count.argtypes = [vp]
     lib.tild_launch_count.restype = C.c_int64
     lib.tild_last_error.argtypes = [vp]
@@ -243,6 +244,12 @@ class Tild:
         g = self._empty((m, 3), t.float32) if want_gauss else None
         self._check(self.lib.tild_philox_test(self.ctx, _dp(ctr), _dp(key), _dp(out), _dp(g), m), "tild_philox_test")
         return out, g
+
+    def tild_layout_info(self) -> dict:
+        info = (C.c_uint64 * 8)()
+        self._check(self.lib.tild_layout_info(self.ctx, C.byref(info)), "tild_layout_info")
+        names = ("tiles", "segments", "slot_capacity", "ell_slots", "overflow", "tile_x", "tile_y", "tile_z")
+        return dict(zip(names, [int(v) for v in info]))
 
     def tild_launch_count(self) -> int:
         return int(self.lib.tild_launch_count(self.ctx))
