@@ -137,9 +137,8 @@ int tild_run_host(tild_ctx*, float* x_host, float* v_host, const int32_t* type_h
 int tild_philox_test(tild_ctx*, const uint32_t* ctr /*[m][4]*/, const uint32_t* key /*[m][2]*/,
                      uint32_t* out /*[m][4]*/, float* gauss /*[m][3]*/, int32_t m);
 
-/* HOST. The internal slab-transposed particle layout of the current state:
- * info = {tiles, segments, slot capacity, slots in the round-major region, particles in the overflow tail,
- * tile cells x, y, z}.  Needs tild_set_state. */
+/* HOST. The internal tiling: info = {tiles, segments = tiles * species, image nodes in z,
+ * spread kernel shared bytes, interpolation kernel shared bytes, tile cells x, y, z}.  Needs tild_set_state. */
 int tild_layout_info(const tild_ctx*, uint64_t info[8] /*HOST out*/);
 
 /* HOST. Number of kernels of this library launched on the context's stream so far. */

@@ -57,9 +57,9 @@ int validate(const tild_params* p)
     return TILD_OK;
 }
 
-// Tile shape of the slab-transposed layout: TX x TY x TZ cells with TZ = EZ - H so that the
-// shared image is EZ in {32, 64} nodes long in z (bank = z); TX, TY in {8, 16} (template EY = TY + H).  Tuning
-// knobs (environment): TILD_TILE_X, TILD_TILE_Y (8|16), TILD_EZ (32|64), TILD_FILL (rounds cap factor).
+// Tile shape: TX x TY x TZ cells, TX, TY in {8, 16} (template EY = TY + H), TZ in {16, 32};
+// the shared image is EZ = TZ + H + sh nodes long in z, rounded up to a multiple of 4.  Tuning knobs (environment):
+// TILD_TILE_X, TILD_TILE_Y (8|16), TILD_TILE_Z (16|32).
 void configure_tiles(tild_ctx* c)
 {
     const tild_params& p = c->prm;
@@ -71,25 +71,20 @@ void configure_tiles(tild_ctx* c)
     };
     t.H = p.order >= 3 ? 3 : 1;
     t.lo = p.order >= 3 ? 1 : 0;
+    t.sh = t.lo ? 4 - t.lo : 0;   // image starts on a 16-byte boundary of the mesh rows (16-byte cp.async staging)
     t.enabled = p.grid[0] >= 8 && p.grid[1] >= 8 && p.grid[2] >= 8;
-    int tx = env_int("TILD_TILE_X", 8), ty = env_int("TILD_TILE_Y", 8), ez = env_int("TILD_EZ", p.grid[2] >= 96 ? 64 : 32);
+    int tx = env_int("TILD_TILE_X", 8), ty = env_int("TILD_TILE_Y", 16), tz = env_int("TILD_TILE_Z", p.grid[2] >= 32 ? 32 : 16);
     if (tx != 8 && tx != 16) tx = 8;
-    if (ty != 8 && ty != 16) ty = 8;
-    if (ez != 32 && ez != 64) ez = 32;
-    if ((size_t)(tx + t.H) * (ty + t.H) * 3 * ez * sizeof(float) > 200 * 1024) tx = 8;
-    if ((size_t)(tx + t.H) * (ty + t.H) * 3 * ez * sizeof(float) > 200 * 1024) ty = 8;
+    if (ty != 8 && ty != 16) ty = 16;
+    if (tz != 16 && tz != 32) tz = 32;
+    const int ez = (tz + t.H + t.sh + 3) / 4 * 4;
+    const size_t lists_i = (size_t)TILD_INTERP_KCAP * 32 * 2 + (size_t)TILD_INTERP_CHUNK * 2;
+    const size_t lists_s = (size_t)TILD_SPREAD_KCAP * 32 * 2 + (size_t)TILD_SPREAD_CHUNK * 2;
+    auto interp_bytes = [&](int ax, int ay) { return (size_t)(ax + t.H) * (ay + t.H) * 3 * ez * sizeof(float) + lists_i; };
+    if (interp_bytes(tx, ty) > 220 * 1024) tx = 8;
     t.EY = ty + t.H;
     t.EZ = ez;
-    // z: the image starts sh nodes below the stencil's low halo so that it begins on a 16-byte boundary of the mesh
-    // rows (16-byte cp.async staging in the interpolation); TZ is a multiple of 4 with TZ + H + sh <= EZ
-    t.sh = t.lo ? 4 - t.lo : 0;
-    const int tz_max = (ez - t.H - t.sh) / 4 * 4;
-    int tzc = p.grid[2];
-    if (tzc > tz_max) {
-        const int ntz = (p.grid[2] + tz_max - 1) / tz_max;
-        tzc = ((p.grid[2] + ntz - 1) / ntz + 3) / 4 * 4;
-    }
-    const int T[3] = {tx, ty, tzc};
+    const int T[3] = {tx, ty, tz};
     t.ntiles = 1;
     for (int a = 0; a < 3; ++a) {
         t.T[a] = T[a] < p.grid[a] ? T[a] : p.grid[a];
@@ -98,26 +93,15 @@ void configure_tiles(tild_ctx* c)
         t.ntiles *= t.nt[a];
     }
     t.E[2] = ez;
-    if (t.T[2] + t.H + t.sh > ez) t.enabled = 0;   // Nz <= tz_max but not a fit (cannot happen: Nz <= tz_max)
     t.nseg = t.ntiles * p.n_species;
     const size_t per_species = (size_t)t.E[0] * t.EY * t.EZ * sizeof(uint32_t);
-    t.sp_group = (int)((100 * 1024) / per_species);
+    t.sp_group = (int)((100 * 1024 - lists_s) / per_species);
     if (t.sp_group < 1) t.sp_group = 1;
     if (t.sp_group > p.n_species) t.sp_group = p.n_species;
-    t.smem_spread = per_species * t.sp_group;
-    t.smem_interp = (size_t)t.E[0] * t.EY * 3 * t.EZ * sizeof(float);
-    t.fill = 1.02f;
-    if (const char* e = getenv("TILD_FILL")) {
-        const float v = (float)atof(e);
-        if (v >= 1.0f && v <= 1.5f) t.fill = v;
-    }
-    t.add = 1;
-    const size_t n = (size_t)p.n;
-    t.cap_ell = (size_t)(1.5 * (double)n) + (size_t)32 * (t.add + 1) * t.nseg + 32;   // >= fill*n + 32*(add+1)*nseg
-    t.cap_ell = (t.cap_ell + 31) / 32 * 32;
-    t.cap = t.cap_ell + n + 32;
+    t.smem_spread = per_species * t.sp_group + lists_s;
+    t.smem_interp = (size_t)t.E[0] * t.EY * 3 * t.EZ * sizeof(float) + lists_i;
     const size_t M = (size_t)p.grid[0] * p.grid[1] * p.grid[2];
-    c->max_bins = M > (size_t)t.nseg * 32 ? M : (size_t)t.nseg * 32;
+    c->max_bins = M > (size_t)t.nseg ? M : (size_t)t.nseg;
 }
 
 void carve(tild_ctx* c, void* base, size_t* total)
@@ -127,33 +111,28 @@ void carve(tild_ctx* c, void* base, size_t* total)
     const size_t n = (size_t)p.n, S = (size_t)p.n_species;
     const size_t M = (size_t)p.grid[0] * p.grid[1] * p.grid[2];
     const size_t Mk = (size_t)p.grid[0] * p.grid[1] * (p.grid[2] / 2 + 1);
-    const size_t cap = c->tile.cap;
-    const size_t nb = cap * (size_t)(p.max_bonds > 0 ? p.max_bonds : 1);
+    const size_t nb = n * (size_t)(p.max_bonds > 0 ? p.max_bonds : 1);
     Carver w(base);
     for (int k = 0; k < 2; ++k) {
-        c->X4[k] = w.take<float4>(cap);
-        c->W4[k] = w.take<float4>(cap);
+        c->X4[k] = w.take<float4>(n);
+        c->W4[k] = w.take<float4>(n);
         c->B[k] = w.take<int32_t>(nb);
     }
-    c->F4 = w.take<float4>(cap);
-    c->SX4 = w.take<float4>(cap);
-    c->lay.seg_base = w.take<uint32_t>((size_t)c->tile.nseg + 1);
-    c->lay_stage.seg_base = w.take<uint32_t>((size_t)c->tile.nseg + 1);
+    c->F4 = w.take<float4>(n);
+    c->SX4 = w.take<float4>(n);
+    c->lay.seg_base = w.take<uint32_t>((size_t)c->tile.nseg + 2);
+    c->lay_stage.seg_base = w.take<uint32_t>((size_t)c->tile.nseg + 2);
     c->grid = w.take<float>(S * M);
     c->nhat = w.take<float2>(S * Mk);
     c->fhat = w.take<float2>(3 * S * Mk);
     c->ffield = w.take<float>(3 * S * M);
-    c->key = w.take<uint32_t>(cap);
-    c->rank = w.take<uint32_t>(cap);
-    c->inv = w.take<uint32_t>(cap);
+    c->key = w.take<uint32_t>(n);
+    c->rank = w.take<uint32_t>(n);
+    c->inv = w.take<uint32_t>(n);
     c->count = w.take<uint32_t>(c->max_bins + 2);
     c->start = w.take<uint32_t>(c->max_bins + 2);
     c->scan_part = w.take<uint32_t>(tild_scan_scratch_entries(c->max_bins + 2));
-    c->holepref = w.take<uint32_t>((size_t)c->tile.nseg * 32);
-    c->segholes = w.take<uint32_t>((size_t)c->tile.nseg);
-    c->segtick = w.take<uint32_t>((size_t)c->tile.nseg);
     c->perm = w.take<uint32_t>(n);
-    c->totals = w.take<uint32_t>(4);
     c->tables = w.take<float>(6 * 4096);
     *total = w.off;
 }
@@ -177,7 +156,7 @@ __global__ void __launch_bounds__(256) gather_by_inv_kernel(int n, const uint32_
 }
 
 // spread -> R2C -> k-space -> C2R on slab-ordered particles, with optional stage events
-int mesh_pipeline(tild_ctx* c, const EllLayout& lay, const float4* X4, cudaEvent_t* ev)
+int mesh_pipeline(tild_ctx* c, const SegLayout& lay, const float4* X4, cudaEvent_t* ev)
 {
     int rc = launch_spread(c, lay, X4, c->grid);
     if (rc) return rc;
@@ -201,12 +180,12 @@ int force_current(tild_ctx* c)
     return launch_interp(c, INTERP_TOTAL_BY_SLOT, c->lay, c->ffield, c->X4[a], c->W4[a], c->B[a], nullptr, nullptr, nullptr);
 }
 
-// caller (x, type) -> slab-ordered copy in c->SX4 described by c->lay_stage; c->inv maps id -> slot
+// caller (x, type) -> segment-sorted copy in c->SX4 described by c->lay_stage; c->inv maps id -> slot
 int stage_layout(tild_ctx* c, const float* x, const int32_t* type)
 {
     int rc = launch_pack(c, x, nullptr, type, nullptr, c->F4, nullptr, nullptr);
     if (rc) return rc;
-    return launch_build_ell(c, (size_t)c->mesh.n, c->F4, c->SX4, &c->lay_stage);
+    return launch_segment_sort(c, c->F4, c->SX4, &c->lay_stage);
 }
 
 }  // namespace
@@ -366,7 +345,7 @@ int tild_layout_info(const tild_ctx* c, uint64_t info[8])
     if (!c || !info) return TILD_EINVAL;
     if (!c->has_state) return TILD_ESTATE;
     const TileParams& t = c->tile;
-    const uint64_t v[8] = {(uint64_t)t.ntiles, (uint64_t)t.nseg, (uint64_t)t.cap, (uint64_t)c->lay.total_ell, (uint64_t)c->lay.n_ovf,
+    const uint64_t v[8] = {(uint64_t)t.ntiles, (uint64_t)t.nseg, (uint64_t)t.EZ, (uint64_t)t.smem_spread, (uint64_t)t.smem_interp,
                            (uint64_t)t.T[0], (uint64_t)t.T[1], (uint64_t)t.T[2]};
     for (int k = 0; k < 8; ++k) info[k] = v[k];
     return TILD_OK;
@@ -436,11 +415,9 @@ int tild_set_state(tild_ctx* c, const float* x, const float* v, const int32_t* t
     c->cur = 0;
     int rc = launch_pack(c, x, v, type, c->stp.max_bonds > 0 ? bond_partner : nullptr, c->X4[0], c->W4[0], c->B[0]);
     if (rc) return rc;
-    c->lay.total_ell = 0;   // slots [0, n) in id order: all of it is "tail" until the first re-sort
-    c->lay.n_ovf = n;
     if ((rc = launch_reorder(c))) return rc;
     if ((rc = force_current(c))) return rc;
-    if ((rc = launch_make_w(c, c->lay.used(), c->F4, c->W4[c->cur], -1.0f))) return rc;  // w = v - (dt/2m) F
+    if ((rc = launch_make_w(c, c->F4, c->W4[c->cur], -1.0f))) return rc;  // w = v - (dt/2m) F
     c->step = step0;
     c->has_state = true;
     c->timed_steps = 0;
@@ -456,7 +433,7 @@ int tild_step(tild_ctx* c, int32_t nsteps)
         cudaEvent_t* ev = (c->ev_ok && c->timed_steps < TILD_MAX_TIMED_STEPS) ? c->ev[c->timed_steps] : nullptr;
         if (ev) cudaEventRecord(ev[0], c->stream);
         if (c->steps_since_sort >= c->resort_every) {
-            int rc = launch_reorder(c);   // synchronises once (8-byte read-back of the layout totals)
+            int rc = launch_reorder(c);
             if (rc) return rc;
         }
         if (ev) cudaEventRecord(ev[1], c->stream);
@@ -500,7 +477,7 @@ int tild_get_state(tild_ctx* c, float* x, float* v, float* f, uint64_t* step)
             TILD_CUDA(c, cudaMemcpyAsync(f, scratch, bytes, cudaMemcpyDefault, c->stream));
         }
         if (v) {
-            if ((rc = launch_velocity_out(c, c->lay.used(), c->F4, c->W4[a], scratch))) return rc;  // v = w + (dt/2m) F
+            if ((rc = launch_velocity_out(c, c->F4, c->W4[a], scratch))) return rc;  // v = w + (dt/2m) F
             TILD_CUDA(c, cudaMemcpyAsync(v, scratch, bytes, cudaMemcpyDefault, c->stream));
         }
     }
@@ -540,11 +517,11 @@ int tild_run_host(tild_ctx* c, float* x_host, float* v_host, const int32_t* type
     const size_t mb = (size_t)c->stp.max_bonds;
     if (n > 0 && (!x_host || !v_host || !type_host || (mb > 0 && !bond_partner_host)))
         return tild_fail(c, TILD_EINVAL, "tild_run_host: null argument");
-    // device staging of the host batch: x, v, type in SX4 (28 n bytes <= 16 cap), bond partners in F4
+    // device staging of the host batch in scratch that tild_set_state only touches after it has packed the batch
     float* xs = reinterpret_cast<float*>(c->SX4);
-    float* vs = xs + 3 * n;
-    int32_t* ts = reinterpret_cast<int32_t*>(vs + 3 * n);
-    int32_t* bs = reinterpret_cast<int32_t*>(c->F4);
+    float* vs = reinterpret_cast<float*>(c->F4);
+    int32_t* ts = reinterpret_cast<int32_t*>(c->key);
+    int32_t* bs = c->B[1];
     if (n > 0) {
         TILD_CUDA(c, cudaMemcpyAsync(xs, x_host, 3 * n * sizeof(float), cudaMemcpyHostToDevice, c->stream));
         TILD_CUDA(c, cudaMemcpyAsync(vs, v_host, 3 * n * sizeof(float), cudaMemcpyHostToDevice, c->stream));

@@ -19,16 +19,16 @@ struct MeshParams {
     long long M;     // Nx*Ny*Nz
 };
 
-// Tiling of the cell grid and the slab-transposed ("ELL") particle layout.
-// A tile is T[0] x T[1] x T[2] cells; its shared-memory image holds E = T + H nodes per axis (H = stencil halo),
-// with E[2] = EZ a multiple of 32 so that the bank of a node depends on its z only.  A "segment" is (tile, species).
-// Inside a segment particle slots are laid out round-major: slot = seg_base[seg] + round*32 + r with
-// r = (local z cell) mod 32, so lane r of a warp always works on a particle whose stencil starts at bank r + const:
-// every shared-memory access of the stencil is bank-conflict free, and a round is one coalesced 512-byte read.
+// Tiling of the cell grid.  A tile is T[0] x T[1] x T[2] cells; its shared-memory image holds
+// E = T + H nodes per axis (H = stencil halo; in z also `sh` alignment nodes).  A "segment" is (tile, species):
+// the internal particle arrays are kept sorted by segment, dense, in arbitrary order inside a segment.  Every step
+// each tile kernel bins its own particles in shared memory by the BANK of the first stencil node's shared-memory
+// address ("class", 32 of them) and then works in rounds of one particle per class, so that all 32 lanes of every
+// stencil access hit different banks.
 struct TileParams {
     int T[3];       // tile edge in cells (clipped to the grid)
     int nt[3];      // tiles per axis = ceil(N/T)
-    int E[3];       // shared tile edge in nodes: E[0], E[1] = tile edge + H (template EY >= E[1]); E[2] = EZ
+    int E[3];       // shared image edge in nodes: E[0] = T[0] + H, E[1] = T[1] + H (<= template EY), E[2] = EZ
     int lo;         // nodes below the tile's first cell that a stencil can touch (0 for P <= 2, 1 for P = 3, 4)
     int sh;         // extra nodes below those so that the image starts on a 16-byte boundary of the mesh rows
     int H;          // stencil halo in nodes (1 for P <= 2, 3 for P = 3, 4)
@@ -36,13 +36,15 @@ struct TileParams {
     int ntiles;
     int nseg;       // ntiles * S
     int sp_group;   // species accumulated per spread CTA (shared-memory budget)
-    size_t cap_ell; // slots reserved for the ELL region
-    size_t cap;     // cap_ell + n + 32: total slots (the tail holds particles that overflow their segment)
-    float fill;     // rounds of a segment are capped at ceil(fill * mean lane length) + add
-    int add;
     size_t smem_spread, smem_interp;
-    int enabled;    // 0: grid too small for the tile kernels -> per-particle kernels on every slot
+    int enabled;    // 0: grid too small for the tile kernels -> per-particle kernels
 };
+
+// shared-memory particle binning of the tile kernels
+#define TILD_SPREAD_CHUNK 4096   // particles binned at a time by the spread kernel (all species of its group)
+#define TILD_SPREAD_KCAP 160     // rounds of its class lists (1.25 x the mean of a full chunk); the rest overflows
+#define TILD_INTERP_CHUNK 2048   // same for the interpolation kernel (one species at a time)
+#define TILD_INTERP_KCAP 96
 
 struct KspaceParams {
     int S;
@@ -67,12 +69,9 @@ struct StepParams {
 };
 
 // ---- context -----------------------------------------------------------------------------------
-// One slab-transposed ordering of a particle set: ELL region [0, total_ell), overflow tail [total_ell, used).
-struct EllLayout {
-    uint32_t* seg_base;  // device [nseg+1]: first slot of each segment; seg_base[nseg] = total_ell
-    size_t total_ell;    // host copies, refreshed by launch_build_ell (one 8-byte read-back per re-sort)
-    size_t n_ovf;
-    size_t used() const { return total_ell + n_ovf; }
+// One segment-sorted ordering of a particle set: particles of segment g are slots [seg_base[g], seg_base[g+1]).
+struct SegLayout {
+    uint32_t* seg_base;  // device [nseg+1]
 };
 
 struct tild_ctx {
@@ -85,29 +84,25 @@ struct tild_ctx {
     TileParams tile;
     size_t max_bins;      // max(M, nseg*32): histogram length
 
-    // carved from the caller's workspace.  Slot arrays have tile.cap entries.
-    float4* X4[2];        // (x, y, z, type as int bits); type < 0 marks a hole
+    // carved from the caller's workspace.  Slot arrays have n entries.
+    float4* X4[2];        // (x, y, z, type as int bits)
     float4* W4[2];        // (w_x, w_y, w_z, original id as uint bits)
-    int32_t* B[2];        // [cap][max_bonds] partner SLOTS, -1 = none
+    int32_t* B[2];        // [n][max_bonds] partner SLOTS, -1 = none
     int cur;
-    float4* F4;           // [cap] per-slot force scratch
-    float4* SX4;          // [cap] stage-call scratch: slab-ordered copy of caller particles; caller-order staging
-    EllLayout lay, lay_stage;
+    float4* F4;           // [n] per-slot force scratch
+    float4* SX4;          // [n] stage-call scratch: segment-sorted copy of caller particles; caller-order staging
+    SegLayout lay, lay_stage;
     float* grid;          // [S][M]
     float2* nhat;         // [S][Mk]
     float2* fhat;         // [3S][Mk]
     float* ffield;        // [3S][M]
-    uint32_t* key;        // [cap]
-    uint32_t* rank;       // [cap]
-    uint32_t* inv;        // [cap] old slot -> new slot
+    uint32_t* key;        // [n]
+    uint32_t* rank;       // [n]
+    uint32_t* inv;        // [n] old slot -> new slot
     uint32_t* count;      // [max_bins+1] histogram
     uint32_t* start;      // [max_bins+1] scan output (cell_start of tild_index_map)
     uint32_t* scan_part;  // block sums of the scan
-    uint32_t* holepref;   // [nseg*32] holes in the lanes before this one (launch_build_ell)
-    uint32_t* segholes;   // [nseg] holes of the segment
-    uint32_t* segtick;    // [nseg] tickets handed to particles that overflow their own lane
     uint32_t* perm;       // [n] tild_index_map scratch
-    uint32_t* totals;     // [4] device counters: [0] = overflow count
     float* tables;        // k-space tables
 
     cufftHandle plan_r2c, plan_c2r;
@@ -146,24 +141,24 @@ int launch_cell_keys(tild_ctx* c, const float* x, uint32_t* key, int32_t* base /
 int launch_counting_sort(tild_ctx* c, const uint32_t* key, size_t nbins, uint32_t* perm, uint32_t* start);
 int launch_pack(tild_ctx* c, const float* x, const float* v, const int32_t* type, const int32_t* bond, float4* X4,
                 float4* W4, int32_t* B);                                  // caller arrays -> slots [0, n), slot i = id i
-// src slots [0, nsrc) -> slab-transposed dst; fills lay (incl. host totals: synchronises) and c->inv
-int launch_build_ell(tild_ctx* c, size_t nsrc, const float4* X4src, float4* X4dst, EllLayout* lay);
-int launch_reorder(tild_ctx* c);  // re-sorts the internal state and flips buffers
-int launch_unpermute(tild_ctx* c, const float4* src, float* dst);        // dst[id[s]][0..2] = src[s].xyz over used slots
+// src slots [0, n) -> segment-sorted dst; fills lay->seg_base and c->inv (old slot -> new slot)
+int launch_segment_sort(tild_ctx* c, const float4* X4src, float4* X4dst, SegLayout* lay);
+int launch_reorder(tild_ctx* c);  // re-sorts the internal state by segment and flips buffers
+int launch_unpermute(tild_ctx* c, const float4* src, float* dst);        // dst[id[s]][0..2] = src[s].xyz
 // tild_spread.cu
 int tild_spread_configure(tild_ctx* c);
-int launch_spread(tild_ctx* c, const EllLayout& lay, const float4* X4, float* grid);  // zero fill + tiles + overflow tail
+int launch_spread(tild_ctx* c, const SegLayout& lay, const float4* X4, float* grid);  // zero fill + tile kernel
 // tild_kspace.cu
 int launch_kspace(tild_ctx* c, const float2* nhat, float2* fhat);
 // tild_interp.cu
 int tild_interp_configure(tild_ctx* c);
 enum { INTERP_NONBONDED_BY_ID = 0, INTERP_TOTAL_BY_SLOT = 1, INTERP_FUSED_STEP = 2 };
 // mode 0: fout[id][3] = interpolated force; mode 1: c->F4[slot] = interpolated + bond force; mode 2: GJF step
-int launch_interp(tild_ctx* c, int mode, const EllLayout& lay, const float* ffield, const float4* X4, const float4* W4,
+int launch_interp(tild_ctx* c, int mode, const SegLayout& lay, const float* ffield, const float4* X4, const float4* W4,
                   const int32_t* B, float4* X4o, float4* W4o, float* fout);
 int launch_bond_force_caller(tild_ctx* c, const float* x, const int32_t* bond, float* f);  // caller-order stage call
-int launch_make_w(tild_ctx* c, size_t nslots, const float4* F4, float4* W4, float sign);   // w += sign*(dt/2m) f
-int launch_velocity_out(tild_ctx* c, size_t nslots, const float4* F4, const float4* W4, float* v);  // v[id] = w + (dt/2m) f
+int launch_make_w(tild_ctx* c, const float4* F4, float4* W4, float sign);   // w += sign*(dt/2m) f
+int launch_velocity_out(tild_ctx* c, const float4* F4, const float4* W4, float* v);  // v[id] = w + (dt/2m) f
 int launch_philox_test(tild_ctx* c, const uint32_t* ctr, const uint32_t* key, uint32_t* out, float* gauss, int m);
 
 size_t tild_scan_scratch_entries(size_t nbins);

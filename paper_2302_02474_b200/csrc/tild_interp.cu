@@ -3,10 +3,10 @@
 // update (L352; equations per DESIGN.md A11) fused into one pass over the particles.
 //
 // Hot kernel: one CTA per tile.  For each species present in the tile the three force-field components of the
-// tile (+ stencil halo) are staged into shared memory with coalesced cp.async row copies (periodic wrap applied
-// per row), then the particles of that (tile, species) segment are read round by round from the slab-transposed
-// layout (tild_sort.cu): lane r holds a particle whose z cell is r mod 32 and the shared image has a z extent that
-// is a multiple of 32, so the 3 P^3 shared-memory loads of the stencil are bank-conflict free.
+// tile (+ stencil halo) are staged into shared memory with 16-byte cp.async row copies (periodic wrap applied per
+// row).  While those copies are in flight the CTA bins the segment's particles by the bank of their first stencil
+// node in the image ("class", see tild_spread.cu), then works in rounds of one particle per class: lane c takes
+// the k-th particle of class c, so each of the 3 P^3 shared-memory loads of the stencil hits 32 different banks.
 #include "tild_internal.cuh"
 
 namespace {
@@ -184,7 +184,6 @@ __global__ void __launch_bounds__(256) interp_slots_kernel(MeshParams m, StepPar
     if (slot >= s1) return;
     const float4 p = X4[slot];
     const int type = __float_as_int(p.w);
-    if (type < 0) return;
     int b[3];
     float w[3][P];
     index_weights<P>(m, p, b, w);
@@ -202,12 +201,10 @@ __device__ __forceinline__ void cp_async_16(float* smem_dst, const float* gsrc)
     const unsigned sa = (unsigned)__cvta_generic_to_shared(smem_dst);
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(sa), "l"(gsrc) : "memory");
 }
-__device__ __forceinline__ void cp_async_wait_all()
-{
-    asm volatile("cp.async.commit_group;\ncp.async.wait_group 0;\n" ::: "memory");
-}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;\n" ::: "memory"); }
 
-// Shared image of one species' force field over the tile: fs[((lx*EY + ly)*3 + comp)*EZ + lz].
+// Dynamic shared memory: image float[3][EX][EY][EZ] of one species | idx u16[KCAP][32] | ovf u16[CHUNK].
 template <int P, int EY, int EZ, int MODE>
 __global__ void __launch_bounds__(INTERP_THREADS) interp_tile_kernel(MeshParams m, TileParams tp, StepParams s, uint64_t step_next,
                                                                      const uint32_t* __restrict__ seg_base,
@@ -216,23 +213,28 @@ __global__ void __launch_bounds__(INTERP_THREADS) interp_tile_kernel(MeshParams 
                                                                      const int32_t* __restrict__ B, float4* __restrict__ X4o,
                                                                      float4* __restrict__ W4o, float4* __restrict__ F4)
 {
+    constexpr int CHUNK = TILD_INTERP_CHUNK, KCAP = TILD_INTERP_KCAP;
     extern __shared__ __align__(16) float fs[];
     __shared__ int goff_x[32], goff_y[32];
+    __shared__ uint32_t cnt[32], novf;
     const int EX = tp.E[0];
+    const int CS = EX * EY * EZ;                              // component stride of the image
     const int tile = blockIdx.x;
     const int tz = tile % tp.nt[2], ty = (tile / tp.nt[2]) % tp.nt[1], tx = tile / (tp.nt[2] * tp.nt[1]);
     const int o[3] = {tx * tp.T[0] - tp.lo, ty * tp.T[1] - tp.lo, tz * tp.T[2] - tp.lo - tp.sh};
     const int E[3] = {EX, tp.E[1], EZ};
     const size_t seg0 = (size_t)tile * m.S;
     if (seg_base[seg0] == seg_base[seg0 + m.S]) return;   // empty tile (uniform)
+    uint16_t* idx = reinterpret_cast<uint16_t*>(fs + 3 * (size_t)CS);
+    uint16_t* ovf = idx + KCAP * 32;
     if (threadIdx.x < EX) goff_x[threadIdx.x] = wrap_idx(o[0] + threadIdx.x, m.N[0]);
     else if (threadIdx.x >= 32 && threadIdx.x < 32 + EY) goff_y[threadIdx.x - 32] = wrap_idx(o[1] + threadIdx.x - 32, m.N[1]);
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    const bool vec16 = (m.N[2] % 4 == 0) && ((reinterpret_cast<uintptr_t>(ffield) & 15) == 0) && (m.M % 4 == 0);
+    const bool vec16 = (m.N[2] % 4 == 0) && ((reinterpret_cast<uintptr_t>(ffield) & 15) == 0);
 
     for (int sp = 0; sp < m.S; ++sp) {
-        const uint32_t b0 = seg_base[seg0 + sp], rounds = (seg_base[seg0 + sp + 1] - b0) >> 5;
-        if (rounds == 0) continue;                         // uniform
+        const uint32_t p_lo = seg_base[seg0 + sp], p_hi = seg_base[seg0 + sp + 1];
+        if (p_lo == p_hi) continue;                        // uniform
         __syncthreads();                                   // previous species' gathers are done; goff_* visible
         {
             // stage the field: one (x, y) column of the image per thread group, three components each
@@ -241,59 +243,103 @@ __global__ void __launch_bounds__(INTERP_THREADS) interp_tile_kernel(MeshParams 
                 // 16-byte copies: the image starts on a 16-byte boundary of the mesh rows (tp.sh) and Nz % 4 == 0,
                 // so every aligned float4 of a row stays inside the row and wraps as a whole
                 constexpr int CPR = EZ / 4;                       // chunks per row
+                constexpr int RPP = INTERP_THREADS / CPR;         // rows per pass
                 const int chunk = threadIdx.x % CPR;
                 const int gz = wrap_idx(o[2] + 4 * chunk, m.N[2]);
-                for (int q = threadIdx.x / CPR; q < EX * EY; q += INTERP_THREADS / CPR) {
-                    const int lx = q / EY, ly = q - lx * EY;
-                    if (ly >= E[1]) continue;
-                    const float* src = fsp + ((size_t)goff_x[lx] * m.N[1] + goff_y[ly]) * m.N[2] + gz;
-                    float* dst = fs + q * 3 * EZ + 4 * chunk;
+                if (threadIdx.x < RPP * CPR)
+                    for (int q = threadIdx.x / CPR; q < EX * EY; q += RPP) {
+                        const int lx = q / EY, ly = q - lx * EY;
+                        if (ly >= E[1]) continue;
+                        const float* src = fsp + ((size_t)goff_x[lx] * m.N[1] + goff_y[ly]) * m.N[2] + gz;
+                        float* dst = fs + q * EZ + 4 * chunk;
 #pragma unroll
-                    for (int comp = 0; comp < 3; ++comp) cp_async_16(dst + comp * EZ, src + (size_t)comp * m.M);
-                }
+                        for (int comp = 0; comp < 3; ++comp) cp_async_16(dst + comp * CS, src + (size_t)comp * m.M);
+                    }
             } else {
+                constexpr int RPP = INTERP_THREADS / EZ;
                 const int lz = threadIdx.x % EZ;
                 const int gz = wrap_idx(o[2] + lz, m.N[2]);
-                for (int q = threadIdx.x / EZ; q < EX * EY; q += INTERP_THREADS / EZ) {
-                    const int lx = q / EY, ly = q - lx * EY;
-                    if (ly >= E[1]) continue;
-                    const float* src = fsp + ((size_t)goff_x[lx] * m.N[1] + goff_y[ly]) * m.N[2] + gz;
-                    float* dst = fs + q * 3 * EZ + lz;
+                if (threadIdx.x < RPP * EZ)
+                    for (int q = threadIdx.x / EZ; q < EX * EY; q += RPP) {
+                        const int lx = q / EY, ly = q - lx * EY;
+                        if (ly >= E[1]) continue;
+                        const float* src = fsp + ((size_t)goff_x[lx] * m.N[1] + goff_y[ly]) * m.N[2] + gz;
+                        float* dst = fs + q * EZ + lz;
 #pragma unroll
-                    for (int comp = 0; comp < 3; ++comp) cp_async_f32(dst + comp * EZ, src + (size_t)comp * m.M);
+                        for (int comp = 0; comp < 3; ++comp) cp_async_f32(dst + comp * CS, src + (size_t)comp * m.M);
+                    }
+            }
+            cp_async_commit();
+        }
+        for (uint32_t c0 = p_lo; c0 < p_hi; c0 += CHUNK) {
+            const int nchunk = (int)min((uint32_t)CHUNK, p_hi - c0);
+            if (c0 != p_lo) __syncthreads();               // previous chunk's rounds are done
+            if (threadIdx.x < 32) cnt[threadIdx.x] = 0u;
+            if (threadIdx.x == 32) novf = 0u;
+            __syncthreads();
+            // phase A (overlaps the copies in flight): class = bank of the first stencil node in the image
+            for (int i = threadIdx.x; i < nchunk; i += INTERP_THREADS) {
+                const size_t slot = (size_t)c0 + i;
+                const float4 p = X4[slot];
+                int b[3], d[3];
+                float w[3][P];
+                index_weights<P>(m, p, b, w);
+                bool inside = true;
+#pragma unroll
+                for (int a = 0; a < 3; ++a) {
+                    d[a] = wrap_near(b[a] - o[a], m.N[a]);
+                    inside = inside && (d[a] + P <= E[a]);
+                }
+                if (inside) {
+                    const uint32_t cls = (uint32_t)((d[0] * EY + d[1]) * EZ + d[2]) & 31u;
+                    const uint32_t k = atomicAdd(&cnt[cls], 1u);
+                    if (k < (uint32_t)KCAP) idx[k * 32 + cls] = (uint16_t)i;
+                    else ovf[atomicAdd(&novf, 1u)] = (uint16_t)i;
+                } else {
+                    // drifted out of the tile's halo since the last re-sort: rare, gathers from the global mesh
+                    const float3 F = interp_global<P, false>(m, ffield, b, w, sp);
+                    finish_particle<MODE>(m, s, step_next, slot, p, F, X4, W4, B, X4o, W4o, F4);
                 }
             }
             cp_async_wait_all();
-        }
-        __syncthreads();
-        for (uint32_t k = wid; k < rounds; k += INTERP_WARPS) {
-            const size_t slot = (size_t)b0 + (size_t)k * 32u + lane;
-            const float4 p = X4[slot];
-            if (__float_as_int(p.w) < 0) continue;         // hole
-            int b[3], d[3];
-            float w[3][P];
-            index_weights<P>(m, p, b, w);
-            bool inside = true;
+            __syncthreads();
+            // phase B: rounds of one particle per class, then the overflow (any class)
+            const uint32_t mine = cnt[lane];
+            uint32_t rounds = mine;
 #pragma unroll
-            for (int a = 0; a < 3; ++a) {
-                d[a] = wrap_near(b[a] - o[a], m.N[a]);
-                inside = inside && (d[a] + P <= E[a]);
-            }
-            float3 F;
-            if (inside) {
-                const float* base = fs + ((d[0] * EY + d[1]) * 3) * EZ + d[2];
-                F = make_float3(0.f, 0.f, 0.f);
+            for (int dlt = 16; dlt > 0; dlt >>= 1) rounds = max(rounds, __shfl_xor_sync(0xffffffffu, rounds, dlt));
+            rounds = min(rounds, (uint32_t)KCAP);
+            const uint32_t extra = (novf + 31u) >> 5;
+            for (uint32_t k = wid; k < rounds + extra; k += INTERP_WARPS) {
+                int i = -1;
+                if (k < rounds) {
+                    if (k < mine) i = idx[k * 32 + lane];
+                } else {
+                    const uint32_t j = (k - rounds) * 32u + lane;
+                    if (j < novf) i = ovf[j];
+                }
+                if (i < 0) continue;
+                const size_t slot = (size_t)c0 + i;
+                const float4 p = X4[slot];
+                int b[3];
+                float w[3][P];
+                index_weights<P>(m, p, b, w);
+                const float* f0 = fs + (wrap_near(b[0] - o[0], m.N[0]) * EY + wrap_near(b[1] - o[1], m.N[1])) * EZ +
+                                  wrap_near(b[2] - o[2], m.N[2]);
+                const float* f1 = f0 + CS;
+                const float* f2 = f1 + CS;
+                float3 F = make_float3(0.f, 0.f, 0.f);
 #pragma unroll
                 for (int jx = 0; jx < P; ++jx) {
 #pragma unroll
                     for (int jy = 0; jy < P; ++jy) {
-                        const float* row = base + ((jx * EY + jy) * 3) * EZ;
+                        const int off = (jx * EY + jy) * EZ;
                         float tx_ = 0.f, ty_ = 0.f, tz_ = 0.f;
 #pragma unroll
                         for (int jz = 0; jz < P; ++jz) {
-                            tx_ = fmaf(w[2][jz], row[jz], tx_);
-                            ty_ = fmaf(w[2][jz], row[EZ + jz], ty_);
-                            tz_ = fmaf(w[2][jz], row[2 * EZ + jz], tz_);
+                            tx_ = fmaf(w[2][jz], f0[off + jz], tx_);
+                            ty_ = fmaf(w[2][jz], f1[off + jz], ty_);
+                            tz_ = fmaf(w[2][jz], f2[off + jz], tz_);
                         }
                         const float wxy = w[0][jx] * w[1][jy];
                         F.x = fmaf(wxy, tx_, F.x);
@@ -301,10 +347,8 @@ __global__ void __launch_bounds__(INTERP_THREADS) interp_tile_kernel(MeshParams 
                         F.z = fmaf(wxy, tz_, F.z);
                     }
                 }
-            } else {
-                F = interp_global<P, false>(m, ffield, b, w, sp); // drifted out of the tile's halo since the last re-sort
+                finish_particle<MODE>(m, s, step_next, slot, p, F, X4, W4, B, X4o, W4o, F4);
             }
-            finish_particle<MODE>(m, s, step_next, slot, p, F, X4, W4, B, X4o, W4o, F4);
         }
     }
 }
@@ -343,7 +387,6 @@ __global__ void __launch_bounds__(256) axpy_slots_kernel(size_t nslots, float al
     const size_t s = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= nslots) return;
     float4 w = W4[s];
-    if (__float_as_uint(w.w) == 0xFFFFFFFFu) return;
     const float4 f = F4[s];
     w.x += alpha * f.x;
     w.y += alpha * f.y;
@@ -359,7 +402,6 @@ __global__ void __launch_bounds__(256) velocity_out_kernel(size_t nslots, float 
     if (s >= nslots) return;
     const float4 w = W4[s];
     const uint32_t id = __float_as_uint(w.w);
-    if (id == 0xFFFFFFFFu) return;
     const float4 f = F4[s];
     v[3 * (size_t)id + 0] = w.x + alpha * f.x;
     v[3 * (size_t)id + 1] = w.y + alpha * f.y;
@@ -387,7 +429,7 @@ __global__ void philox_test_kernel(int m, const uint32_t* __restrict__ ctr, cons
 
 bool can_vectorize(const tild_ctx* c, const float* ffield)
 {
-    return (c->mesh.N[2] % 4 == 0) && (reinterpret_cast<uintptr_t>(ffield) % 16 == 0) && !(c->prm.flags & TILD_FLAG_NAIVE_INTERP);
+    return (c->mesh.N[2] % 4 == 0) && (reinterpret_cast<uintptr_t>(ffield) % 16 == 0);
 }
 
 // ---- dispatch ------------------------------------------------------------------------------------------------------
@@ -429,10 +471,11 @@ template <int P>
 bool tile_launch_p(const InterpArgs& a, int ey, int ez, int mode, cudaStream_t st, size_t smem, bool cfg, cudaError_t* err)
 {
     constexpr int H = (P >= 3) ? 3 : 1;
-    if (ey == 8 + H && ez == 32) tile_launch_m<P, 8 + H, 32>(a, mode, st, smem, cfg, err);
-    else if (ey == 8 + H && ez == 64) tile_launch_m<P, 8 + H, 64>(a, mode, st, smem, cfg, err);
-    else if (ey == 16 + H && ez == 32) tile_launch_m<P, 16 + H, 32>(a, mode, st, smem, cfg, err);
-    else if (ey == 16 + H && ez == 64) tile_launch_m<P, 16 + H, 64>(a, mode, st, smem, cfg, err);
+    constexpr int EZA = (P >= 3) ? 24 : 20, EZB = (P >= 3) ? 40 : 36;   // TZ = 16 / 32 (+ halo + alignment, % 4 == 0)
+    if (ey == 8 + H && ez == EZA) tile_launch_m<P, 8 + H, EZA>(a, mode, st, smem, cfg, err);
+    else if (ey == 8 + H && ez == EZB) tile_launch_m<P, 8 + H, EZB>(a, mode, st, smem, cfg, err);
+    else if (ey == 16 + H && ez == EZA) tile_launch_m<P, 16 + H, EZA>(a, mode, st, smem, cfg, err);
+    else if (ey == 16 + H && ez == EZB) tile_launch_m<P, 16 + H, EZB>(a, mode, st, smem, cfg, err);
     else return false;
     return true;
 }
@@ -472,26 +515,26 @@ int tild_interp_configure(tild_ctx* c)
     return TILD_OK;
 }
 
-int launch_interp(tild_ctx* c, int mode, const EllLayout& lay, const float* ffield, const float4* X4, const float4* W4,
+int launch_interp(tild_ctx* c, int mode, const SegLayout& lay, const float* ffield, const float4* X4, const float4* W4,
                   const int32_t* B, float4* X4o, float4* W4o, float* /*unused*/)
 {
-    if (c->mesh.n == 0) return TILD_OK;
+    const size_t n = (size_t)c->mesh.n;
+    if (n == 0) return TILD_OK;
     InterpArgs a{c->mesh, c->tile, c->stp, c->step + 1, lay.seg_base, ffield, X4, W4, B, X4o, W4o, c->F4};
-    const bool vec = can_vectorize(c, ffield);
-    if (c->tile.enabled && lay.total_ell > 0) {
+    if (c->tile.enabled && !(c->prm.flags & TILD_FLAG_NAIVE_INTERP)) {
         cudaError_t e = cudaSuccess;
         tile_launch_any(a, mode, c->stream, c->tile.smem_interp, false, &e);
         TILD_LAUNCH_CHECK(c, "interp_tile_kernel");
+        return TILD_OK;
     }
-    if (lay.n_ovf > 0) {
-        switch (c->mesh.P) {
-        case 1: slots_launch_p<1>(a, vec, mode, lay.total_ell, lay.used(), c->stream); break;
-        case 2: slots_launch_p<2>(a, vec, mode, lay.total_ell, lay.used(), c->stream); break;
-        case 3: slots_launch_p<3>(a, vec, mode, lay.total_ell, lay.used(), c->stream); break;
-        default: slots_launch_p<4>(a, vec, mode, lay.total_ell, lay.used(), c->stream); break;
-        }
-        TILD_LAUNCH_CHECK(c, "interp_slots_kernel");
+    const bool vec = can_vectorize(c, ffield);
+    switch (c->mesh.P) {
+    case 1: slots_launch_p<1>(a, vec, mode, 0, n, c->stream); break;
+    case 2: slots_launch_p<2>(a, vec, mode, 0, n, c->stream); break;
+    case 3: slots_launch_p<3>(a, vec, mode, 0, n, c->stream); break;
+    default: slots_launch_p<4>(a, vec, mode, 0, n, c->stream); break;
     }
+    TILD_LAUNCH_CHECK(c, "interp_slots_kernel");
     return TILD_OK;
 }
 
@@ -504,16 +547,18 @@ int launch_bond_force_caller(tild_ctx* c, const float* x, const int32_t* bond, f
     return TILD_OK;
 }
 
-int launch_make_w(tild_ctx* c, size_t nslots, const float4* F4, float4* W4, float sign)
+int launch_make_w(tild_ctx* c, const float4* F4, float4* W4, float sign)
 {
+    const size_t nslots = (size_t)c->mesh.n;
     if (nslots == 0) return TILD_OK;
     axpy_slots_kernel<<<(unsigned)((nslots + 255) / 256), 256, 0, c->stream>>>(nslots, sign * c->stp.half_dt_over_m, F4, W4);
     TILD_LAUNCH_CHECK(c, "axpy_slots_kernel");
     return TILD_OK;
 }
 
-int launch_velocity_out(tild_ctx* c, size_t nslots, const float4* F4, const float4* W4, float* v)
+int launch_velocity_out(tild_ctx* c, const float4* F4, const float4* W4, float* v)
 {
+    const size_t nslots = (size_t)c->mesh.n;
     if (nslots == 0) return TILD_OK;
     velocity_out_kernel<<<(unsigned)((nslots + 255) / 256), 256, 0, c->stream>>>(nslots, c->stp.half_dt_over_m, F4, W4, v);
     TILD_LAUNCH_CHECK(c, "velocity_out_kernel");

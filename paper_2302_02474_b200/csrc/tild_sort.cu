@@ -1,5 +1,5 @@
 // a1: canonical fp32 index map, cell keys, counting sort by cell (the stage call tild_index_map),
-// and the slab-transposed ("ELL") re-ordering of the internal particle state that the tile kernels run on.
+// and the segment (tile, species) ordering of the internal particle state that the tile kernels run on.
 // Not in the paper's PM text; nearest prior art is its neighbour-list cell binning with atomics
 // (PAPER.md L205).  DESIGN.md A15/A16 define what is bit-exact; DESIGN.md section 4 describes the layout.
 #include "tild_internal.cuh"
@@ -157,133 +157,71 @@ __global__ void __launch_bounds__(256) pack_kernel(int n, int max_bonds, const f
         for (int k = 0; k < max_bonds; ++k) B[(size_t)i * max_bonds + k] = bond[(size_t)i * max_bonds + k];
 }
 
-// key = segment * 32 + (local z cell mod 32), segment = tile * S + species; rank = arrival order in that lane list
+// key = segment = tile * S + species; rank = arrival order in the segment (one atomic per distinct key per warp)
 template <int P>
-__global__ void __launch_bounds__(256) ell_key_kernel(MeshParams m, TileParams tp, size_t nsrc, const float4* __restrict__ X4,
+__global__ void __launch_bounds__(256) seg_key_kernel(MeshParams m, TileParams tp, const float4* __restrict__ X4,
                                                       uint32_t* __restrict__ key, uint32_t* __restrict__ rank,
                                                       uint32_t* __restrict__ count)
 {
-    const size_t s = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (s >= nsrc) return;
-    const float4 p = X4[s];
-    const int type = __float_as_int(p.w);
-    if (type < 0) {
-        key[s] = 0xFFFFFFFFu;
-        return;
-    }
-    const float pos[3] = {p.x, p.y, p.z};
-    int t[3], rz = 0;
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    uint32_t k = 0xFFFFFFFFu;
+    if (s < m.n) {
+        const float4 p = X4[s];
+        const float pos[3] = {p.x, p.y, p.z};
+        int t[3];
 #pragma unroll
-    for (int a = 0; a < 3; ++a) {
-        int cell, b;
-        float off;
-        index_1d<P>(pos[a], m.inv_h[a], cell, b, off);
-        cell = wrap_idx(cell, m.N[a]);
-        t[a] = cell / tp.T[a];
-        // lane = z of the stencil's first node relative to the tile (the cell for even P, the nearest node for odd P)
-        if (a == 2) rz = wrap_idx(b + tp.lo, m.N[2]) - t[2] * tp.T[2];
-    }
-    const uint32_t tile = (uint32_t)((t[0] * tp.nt[1] + t[1]) * tp.nt[2] + t[2]);
-    const uint32_t k = ((tile * (uint32_t)m.S + (uint32_t)type) << 5) | (uint32_t)(rz & 31);
-    key[s] = k;
-    rank[s] = atomicAdd(&count[k], 1u);
-}
-
-// one warp per segment: rounds = min(longest lane list, ceil(fill * mean) + add); out[seg] = 32 * rounds.
-// Lanes shorter than `rounds` leave holes; holepref[seg*32 + r] = holes in lanes < r, segholes[seg] = all of them.
-// Particles beyond `rounds` in their own lane are placed into those holes by ell_scatter_kernel (they cost a 2-way
-// bank conflict in the round they land in, instead of an idle lane slot or a trip through the per-particle kernels).
-__global__ void __launch_bounds__(256) ell_rounds_kernel(int nseg, float fill, int add, const uint32_t* __restrict__ count,
-                                                         uint32_t* __restrict__ rounds32, uint32_t* __restrict__ holepref,
-                                                         uint32_t* __restrict__ segholes, uint32_t* __restrict__ segtick)
-{
-    const int seg = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
-    if (seg >= nseg) return;
-    const uint32_t len = count[((size_t)seg << 5) + lane];
-    uint32_t mx = len, sum = len;
-#pragma unroll
-    for (int d = 16; d > 0; d >>= 1) {
-        mx = max(mx, __shfl_xor_sync(0xffffffffu, mx, d));
-        sum += __shfl_xor_sync(0xffffffffu, sum, d);
-    }
-    const uint32_t cap = (sum && fill > 0.0f) ? (uint32_t)ceilf(fill * (float)sum * (1.0f / 32.0f)) + (uint32_t)add : 0u;
-    const uint32_t rounds = min(mx, cap);
-    const uint32_t deficit = rounds > len ? rounds - len : 0u;
-    uint32_t incl = deficit;
-#pragma unroll
-    for (int d = 1; d < 32; d <<= 1) {
-        const uint32_t o = __shfl_up_sync(0xffffffffu, incl, d);
-        if (lane >= d) incl += o;
-    }
-    holepref[((size_t)seg << 5) + lane] = incl - deficit;
-    if (lane == 31) segholes[seg] = incl;
-    if (lane == 0) {
-        rounds32[seg] = 32u * rounds;
-        segtick[seg] = 0u;
-    }
-    if (seg == 0 && lane == 0) rounds32[nseg] = 0u;
-}
-
-// new slot of every source slot: own lane list first, then the holes of the segment, then the overflow tail
-__global__ void __launch_bounds__(256) ell_scatter_kernel(size_t nsrc, int nseg, const uint32_t* __restrict__ key,
-                                                          const uint32_t* __restrict__ rank, const uint32_t* __restrict__ seg_base,
-                                                          const uint32_t* __restrict__ count, const uint32_t* __restrict__ holepref,
-                                                          const uint32_t* __restrict__ segholes, uint32_t* __restrict__ segtick,
-                                                          const float4* __restrict__ X4src, float4* __restrict__ X4dst,
-                                                          uint32_t* __restrict__ inv, uint32_t* __restrict__ totals)
-{
-    const size_t s = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (s >= nsrc) return;
-    const uint32_t k = key[s];
-    if (k == 0xFFFFFFFFu) {
-        inv[s] = 0xFFFFFFFFu;
-        return;
-    }
-    const uint32_t seg = k >> 5, r = k & 31u, b0 = seg_base[seg], rounds = (seg_base[seg + 1] - b0) >> 5, rk = rank[s];
-    uint32_t d;
-    if (rk < rounds) {
-        d = b0 + rk * 32u + r;
-    } else {
-        const uint32_t t = atomicAdd(&segtick[seg], 1u);
-        if (t < segholes[seg]) {
-            const uint32_t* hp = holepref + ((size_t)seg << 5);
-            uint32_t lo = 0;   // largest lane with holepref <= t
-#pragma unroll
-            for (uint32_t step = 16; step > 0; step >>= 1)
-                if (hp[lo + step] <= t) lo += step;
-            d = b0 + (count[((size_t)seg << 5) + lo] + (t - hp[lo])) * 32u + lo;
-        } else {
-            d = seg_base[nseg] + atomicAdd(&totals[0], 1u);
+        for (int a = 0; a < 3; ++a) {
+            int cell, b;
+            float off;
+            index_1d<P>(pos[a], m.inv_h[a], cell, b, off);
+            t[a] = wrap_idx(cell, m.N[a]) / tp.T[a];
         }
+        k = (uint32_t)((t[0] * tp.nt[1] + t[1]) * tp.nt[2] + t[2]) * (uint32_t)m.S + (uint32_t)__float_as_int(p.w);
     }
+    const unsigned peers = __match_any_sync(0xffffffffu, k);
+    const int lane = threadIdx.x & 31, leader = __ffs(peers) - 1;
+    uint32_t base = 0;
+    if (lane == leader && k != 0xFFFFFFFFu) base = atomicAdd(&count[k], (uint32_t)__popc(peers));
+    base = __shfl_sync(0xffffffffu, base, leader);
+    if (s < m.n) {
+        key[s] = k;
+        rank[s] = base + (uint32_t)__popc(peers & ((1u << lane) - 1u));
+    }
+}
+
+__global__ void __launch_bounds__(256) seg_scatter_kernel(int n, const uint32_t* __restrict__ key, const uint32_t* __restrict__ rank,
+                                                          const uint32_t* __restrict__ seg_base, const float4* __restrict__ X4src,
+                                                          float4* __restrict__ X4dst, uint32_t* __restrict__ inv)
+{
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= n) return;
+    const uint32_t d = seg_base[key[s]] + rank[s];
     inv[s] = d;
     X4dst[d] = X4src[s];
 }
 
 // moves the rest of the state (w + id, bond partner slots remapped through inv) to the new slots
-__global__ void __launch_bounds__(256) ell_move_state_kernel(size_t nsrc, int max_bonds, const uint32_t* __restrict__ inv,
-                                                             const float4* __restrict__ W4src, const int32_t* __restrict__ Bsrc,
-                                                             float4* __restrict__ W4dst, int32_t* __restrict__ Bdst)
+__global__ void __launch_bounds__(256) move_state_kernel(int n, int max_bonds, const uint32_t* __restrict__ inv,
+                                                         const float4* __restrict__ W4src, const int32_t* __restrict__ Bsrc,
+                                                         float4* __restrict__ W4dst, int32_t* __restrict__ Bdst)
 {
-    const size_t s = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (s >= nsrc) return;
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= n) return;
     const uint32_t d = inv[s];
-    if (d == 0xFFFFFFFFu) return;
     W4dst[d] = W4src[s];
     for (int k = 0; k < max_bonds; ++k) {
-        const int32_t q = Bsrc[s * max_bonds + k];
+        const int32_t q = Bsrc[(size_t)s * max_bonds + k];
         Bdst[(size_t)d * max_bonds + k] = q < 0 ? -1 : (int32_t)inv[q];
     }
 }
 
-// dst[id[s]][0..2] = src[s].xyz for every occupied slot
-__global__ void __launch_bounds__(256) unpermute_kernel(size_t nslots, const float4* __restrict__ W4, const float4* __restrict__ src,
+// dst[id[s]][0..2] = src[s].xyz
+__global__ void __launch_bounds__(256) unpermute_kernel(int n, const float4* __restrict__ W4, const float4* __restrict__ src,
                                                         float* __restrict__ dst)
 {
-    const size_t s = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (s >= nslots) return;
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= n) return;
     const uint32_t id = __float_as_uint(W4[s].w);
-    if (id == 0xFFFFFFFFu) return;
     const float4 v = src[s];
     dst[3 * (size_t)id + 0] = v.x;
     dst[3 * (size_t)id + 1] = v.y;
@@ -350,73 +288,48 @@ int launch_pack(tild_ctx* c, const float* x, const float* v, const int32_t* type
     return TILD_OK;
 }
 
-int launch_build_ell(tild_ctx* c, size_t nsrc, const float4* X4src, float4* X4dst, EllLayout* lay)
+int launch_segment_sort(tild_ctx* c, const float4* X4src, float4* X4dst, SegLayout* lay)
 {
     const TileParams& tp = c->tile;
-    const int nseg = tp.nseg;
-    const size_t nbins = (size_t)nseg * 32;
-    TILD_CUDA(c, cudaMemsetAsync(c->count, 0, nbins * sizeof(uint32_t), c->stream));
-    TILD_CUDA(c, cudaMemsetAsync(c->totals, 0, 4 * sizeof(uint32_t), c->stream));
-    if (nsrc > 0) {
+    const int n = c->mesh.n, nseg = tp.nseg;
+    TILD_CUDA(c, cudaMemsetAsync(c->count, 0, ((size_t)nseg + 1) * sizeof(uint32_t), c->stream));
+    if (n > 0) {
         switch (c->mesh.P) {
-        case 1: ell_key_kernel<1><<<blocks_for(nsrc), 256, 0, c->stream>>>(c->mesh, tp, nsrc, X4src, c->key, c->rank, c->count); break;
-        case 2: ell_key_kernel<2><<<blocks_for(nsrc), 256, 0, c->stream>>>(c->mesh, tp, nsrc, X4src, c->key, c->rank, c->count); break;
-        case 3: ell_key_kernel<3><<<blocks_for(nsrc), 256, 0, c->stream>>>(c->mesh, tp, nsrc, X4src, c->key, c->rank, c->count); break;
-        default: ell_key_kernel<4><<<blocks_for(nsrc), 256, 0, c->stream>>>(c->mesh, tp, nsrc, X4src, c->key, c->rank, c->count); break;
+        case 1: seg_key_kernel<1><<<blocks_for(n), 256, 0, c->stream>>>(c->mesh, tp, X4src, c->key, c->rank, c->count); break;
+        case 2: seg_key_kernel<2><<<blocks_for(n), 256, 0, c->stream>>>(c->mesh, tp, X4src, c->key, c->rank, c->count); break;
+        case 3: seg_key_kernel<3><<<blocks_for(n), 256, 0, c->stream>>>(c->mesh, tp, X4src, c->key, c->rank, c->count); break;
+        default: seg_key_kernel<4><<<blocks_for(n), 256, 0, c->stream>>>(c->mesh, tp, X4src, c->key, c->rank, c->count); break;
         }
-        TILD_LAUNCH_CHECK(c, "ell_key_kernel");
+        TILD_LAUNCH_CHECK(c, "seg_key_kernel");
     }
-    uint32_t* rounds32 = c->start;  // [nseg+1] scratch
-    ell_rounds_kernel<<<blocks_for((size_t)nseg * 32), 256, 0, c->stream>>>(nseg, tp.enabled ? tp.fill : 0.0f, tp.enabled ? tp.add : 0,
-                                                                             c->count, rounds32, c->holepref, c->segholes, c->segtick);
-    TILD_LAUNCH_CHECK(c, "ell_rounds_kernel");
-    int rc = exclusive_scan(c, rounds32, (size_t)nseg + 1, lay->seg_base);
+    int rc = exclusive_scan(c, c->count, (size_t)nseg + 1, lay->seg_base);
     if (rc) return rc;
-    // holes of the ELL region: type = -1 (all-ones bit pattern); the tail is written densely
-    TILD_CUDA(c, cudaMemsetAsync(X4dst, 0xFF, tp.cap_ell * sizeof(float4), c->stream));
-    if (nsrc > 0) {
-        ell_scatter_kernel<<<blocks_for(nsrc), 256, 0, c->stream>>>(nsrc, nseg, c->key, c->rank, lay->seg_base, c->count, c->holepref,
-                                                                    c->segholes, c->segtick, X4src, X4dst, c->inv, c->totals);
-        TILD_LAUNCH_CHECK(c, "ell_scatter_kernel");
+    if (n > 0) {
+        seg_scatter_kernel<<<blocks_for(n), 256, 0, c->stream>>>(n, c->key, c->rank, lay->seg_base, X4src, X4dst, c->inv);
+        TILD_LAUNCH_CHECK(c, "seg_scatter_kernel");
     }
-    uint32_t h[2] = {0, 0};
-    TILD_CUDA(c, cudaMemcpyAsync(&h[0], lay->seg_base + nseg, sizeof(uint32_t), cudaMemcpyDeviceToHost, c->stream));
-    TILD_CUDA(c, cudaMemcpyAsync(&h[1], c->totals, sizeof(uint32_t), cudaMemcpyDeviceToHost, c->stream));
-    TILD_CUDA(c, cudaStreamSynchronize(c->stream));
-    lay->total_ell = h[0];
-    lay->n_ovf = h[1];
-    if (lay->total_ell > tp.cap_ell || lay->used() > tp.cap)
-        return tild_fail(c, TILD_ENOMEM, "slab layout needs %zu + %zu slots, capacity %zu + %zu", lay->total_ell, lay->n_ovf,
-                         tp.cap_ell, tp.cap - tp.cap_ell);
     return TILD_OK;
 }
 
 int launch_reorder(tild_ctx* c)
 {
-    const int a = c->cur, b = 1 - c->cur;
-    const size_t nsrc = c->lay.used();
-    int rc = launch_build_ell(c, nsrc, c->X4[a], c->X4[b], &c->lay);
+    const int a = c->cur, b = 1 - c->cur, n = c->mesh.n;
+    int rc = launch_segment_sort(c, c->X4[a], c->X4[b], &c->lay);
     if (rc) return rc;
     c->steps_since_sort = 0;
-    const TileParams& tp = c->tile;
-    TILD_CUDA(c, cudaMemsetAsync(c->W4[b], 0xFF, tp.cap_ell * sizeof(float4), c->stream));
-    if (nsrc > 0) {
-        ell_move_state_kernel<<<blocks_for(nsrc), 256, 0, c->stream>>>(nsrc, c->stp.max_bonds, c->inv, c->W4[a], c->B[a], c->W4[b],
-                                                                       c->B[b]);
-        TILD_LAUNCH_CHECK(c, "ell_move_state_kernel");
+    if (n > 0) {
+        move_state_kernel<<<blocks_for(n), 256, 0, c->stream>>>(n, c->stp.max_bonds, c->inv, c->W4[a], c->B[a], c->W4[b], c->B[b]);
+        TILD_LAUNCH_CHECK(c, "move_state_kernel");
     }
-    // the fused step never writes holes, so the other buffer pair must carry the hole markers too
-    TILD_CUDA(c, cudaMemsetAsync(c->X4[a], 0xFF, tp.cap_ell * sizeof(float4), c->stream));
-    TILD_CUDA(c, cudaMemsetAsync(c->W4[a], 0xFF, tp.cap_ell * sizeof(float4), c->stream));
     c->cur = b;
     return TILD_OK;
 }
 
 int launch_unpermute(tild_ctx* c, const float4* src, float* dst)
 {
-    const size_t ns = c->lay.used();
-    if (ns == 0) return TILD_OK;
-    unpermute_kernel<<<blocks_for(ns), 256, 0, c->stream>>>(ns, c->W4[c->cur], src, dst);
+    const int n = c->mesh.n;
+    if (n == 0) return TILD_OK;
+    unpermute_kernel<<<blocks_for(n), 256, 0, c->stream>>>(n, c->W4[c->cur], src, dst);
     TILD_LAUNCH_CHECK(c, "unpermute_kernel");
     return TILD_OK;
 }

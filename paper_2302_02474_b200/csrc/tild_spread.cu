@@ -2,13 +2,17 @@
 // its density contribution to nearby grid points, using a spline interpolation scheme"; Eq. 1 L110.
 // grid[J][g] = sum_{i in J} W_x W_y W_z  (raw weights), g = (ix*Ny + iy)*Nz + iz.
 //
-// Hot kernel: one CTA per tile of TX x TY x TZ cells.  The particles of the tile sit in the slab-transposed
-// layout of tild_sort.cu: a warp reads one round (32 consecutive slots, one coalesced 512-byte load) in which lane r
-// holds a particle whose z cell is r mod 32.  The P^3 stencil of every particle is accumulated into a shared-memory
-// image of the tile whose z extent EZ is a multiple of 32, so the bank of a stencil node is (r + const) mod 32:
-// every shared-memory atomic of a warp instruction hits 32 different banks.  (With particles in plain cell order
-// the same kernel measured 3.5 wavefronts per ATOMS; profiles/r1_before_slab_layout.md.)  The tile is flushed to the
-// global grid once, so global-atomic traffic is per tile node instead of per particle.
+// Hot kernel: one CTA per tile of TX x TY x TZ cells (x a group of species).  The particles of the tile are one
+// contiguous range of the segment-sorted arrays (tild_sort.cu).  The P^3 stencil of every particle is accumulated
+// into a shared-memory image of the tile and the image is flushed to the global grid once, so global-atomic traffic
+// is per tile node instead of per particle.
+//
+// Bank conflicts: 32 particles of a warp in cell order hit the 32 banks at random (measured 3.5 wavefronts per
+// ATOMS, profiles/r1_spread_interp_before.md).  All P^3 stencil offsets are the same for every particle, so the bank
+// of each access is (bank of the first stencil node) + const.  Each step the CTA therefore first bins its particles
+// by that bank ("class") into 32 shared-memory lists (phase A: one shared atomic per particle), then works in rounds
+// of one particle per class (phase B): lane c takes the k-th particle of class c, and every ATOMS of the round hits
+// 32 different banks.  Binning every step makes this independent of how far particles drifted since the last re-sort.
 //
 // sm_100a has no native fp32 shared-memory atomic add (atomicAdd(float*) on shared compiles to an
 // LDS + FADD + ATOMS.CAST.SPIN loop) but does have a native 32-bit integer one (ATOMS.ADD).  The tile is
@@ -24,6 +28,7 @@ constexpr int SPREAD_THREADS = 256;
 constexpr int SPREAD_WARPS = SPREAD_THREADS / 32;
 constexpr int FIX_BITS = 23;                    // tile fixed point: units of 2^-23
 constexpr float FIX_INV = 1.0f / 8388608.0f;
+
 
 // Baseline / fallback: one thread per particle, P^3 global reductions (REDG.E.ADD.F32 resolves in L2).
 template <int P>
@@ -54,7 +59,6 @@ __global__ void __launch_bounds__(256) spread_slots_kernel(MeshParams m, size_t 
     if (s >= s1) return;
     const float4 p = X4[s];
     const int type = __float_as_int(p.w);
-    if (type < 0) return;
     const float pos[3] = {p.x, p.y, p.z};
     int cell, b[3];
     float t, w[3][P];
@@ -100,15 +104,17 @@ __device__ __forceinline__ bool locate(const MeshParams& m, const float4& p, con
 
 // EY, EZ are template parameters so that every shared-memory offset of the stencil is an immediate.
 // One CTA = one tile x one group of up to tp.sp_group species (blockIdx.y).
+// Dynamic shared memory: image u32[nsp][EX][EY][EZ] | idx u16[KCAP][32] | ovf u16[CHUNK].
 template <int P, int EY, int EZ>
 __global__ void __launch_bounds__(SPREAD_THREADS) spread_tile_kernel(MeshParams m, TileParams tp,
                                                                      const uint32_t* __restrict__ seg_base,
                                                                      const float4* __restrict__ X4, float* __restrict__ grid)
 {
+    constexpr int CHUNK = TILD_SPREAD_CHUNK, KCAP = TILD_SPREAD_KCAP;
     extern __shared__ __align__(16) uint32_t sm[];
     __shared__ unsigned long long red[SPREAD_WARPS];
     __shared__ int goff_x[32], goff_y[32];          // wrapped global x / y node of each local x / y
-    __shared__ uint32_t sbase[TILD_MAX_SPECIES + 1], srounds[TILD_MAX_SPECIES + 1];
+    __shared__ uint32_t cnt[32], novf;
     const int EX = tp.E[0];
     const int E3 = EX * EY * EZ;
     const int tile = blockIdx.x;
@@ -118,38 +124,66 @@ __global__ void __launch_bounds__(SPREAD_THREADS) spread_tile_kernel(MeshParams 
     const int o[3] = {tx * tp.T[0] - tp.lo, ty * tp.T[1] - tp.lo, tz * tp.T[2] - tp.lo - tp.sh};
     const int E[3] = {EX, tp.E[1], EZ};
     const size_t seg0 = (size_t)tile * m.S + sp0;
-    if (seg_base[seg0] == seg_base[seg0 + nsp]) return;   // empty tile (uniform)
+    const uint32_t p_lo = seg_base[seg0], p_hi = seg_base[seg0 + nsp];
+    if (p_lo == p_hi) return;                        // empty tile (uniform)
+    uint16_t* idx = reinterpret_cast<uint16_t*>(sm + (size_t)tp.sp_group * E3);
+    uint16_t* ovf = idx + KCAP * 32;
 
     {
         uint4* z4 = reinterpret_cast<uint4*>(sm);
-        const int n4 = nsp * E3 / 4;                 // EZ % 32 == 0
+        const int n4 = nsp * E3 / 4;                 // EZ % 4 == 0
         for (int k = threadIdx.x; k < n4; k += SPREAD_THREADS) z4[k] = make_uint4(0u, 0u, 0u, 0u);
         if (threadIdx.x < EX) goff_x[threadIdx.x] = wrap_idx(o[0] + threadIdx.x, m.N[0]);
         else if (threadIdx.x >= 32 && threadIdx.x < 32 + EY) goff_y[threadIdx.x - 32] = wrap_idx(o[1] + threadIdx.x - 32, m.N[1]);
-        if (threadIdx.x == 64) {                     // prefix of the rounds of this CTA's segments
-            uint32_t acc = 0;
-            for (int sp = 0; sp < nsp; ++sp) {
-                srounds[sp] = acc;
-                sbase[sp] = seg_base[seg0 + sp];
-                acc += (seg_base[seg0 + sp + 1] - sbase[sp]) >> 5;
-            }
-            srounds[nsp] = acc;
-        }
     }
-    __syncthreads();
-
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     uint32_t n_tile = 0;  // particles this thread accumulated through shared memory
-    const uint32_t rounds_total = srounds[nsp];
-    int sp = 0;
-    for (uint32_t j = wid; j < rounds_total; j += SPREAD_WARPS) {
-        while (j >= srounds[sp + 1]) ++sp;           // warp-uniform
-        const float4 p = X4[(size_t)sbase[sp] + (size_t)(j - srounds[sp]) * 32u + lane];
-        if (__float_as_int(p.w) < 0) continue;       // hole
-        int b[3], d[3];
-        float w[3][P];
-        if (locate<P>(m, p, o, E, b, d, w)) {
-            uint32_t* s = sm + sp * E3 + (d[0] * EY + d[1]) * EZ + d[2];
+
+    for (uint32_t c0 = p_lo; c0 < p_hi; c0 += CHUNK) {
+        const int nchunk = (int)min((uint32_t)CHUNK, p_hi - c0);
+        __syncthreads();                             // image zeroed / previous chunk's rounds done
+        if (threadIdx.x < 32) cnt[threadIdx.x] = 0u;
+        if (threadIdx.x == 32) novf = 0u;
+        __syncthreads();
+        // phase A: class of every particle = bank of its first stencil node in the image
+        for (int i = threadIdx.x; i < nchunk; i += SPREAD_THREADS) {
+            const float4 p = X4[c0 + i];
+            const int spl = __float_as_int(p.w) - sp0;
+            int b[3], d[3];
+            float w[3][P];
+            if (locate<P>(m, p, o, E, b, d, w)) {
+                const uint32_t cls = (uint32_t)(spl * E3 + (d[0] * EY + d[1]) * EZ + d[2]) & 31u;
+                const uint32_t k = atomicAdd(&cnt[cls], 1u);
+                if (k < (uint32_t)KCAP) idx[k * 32 + cls] = (uint16_t)i;
+                else ovf[atomicAdd(&novf, 1u)] = (uint16_t)i;
+            } else {
+                // drifted out of the tile's halo since the last re-sort: rare, goes straight to the global grid
+                spread_global_one<P>(m, b, w, grid + (size_t)(sp0 + spl) * m.M);
+            }
+        }
+        __syncthreads();
+        // phase B: rounds of one particle per class, then the overflow (any class)
+        const uint32_t mine = cnt[lane];
+        uint32_t rounds = mine;
+#pragma unroll
+        for (int dlt = 16; dlt > 0; dlt >>= 1) rounds = max(rounds, __shfl_xor_sync(0xffffffffu, rounds, dlt));
+        rounds = min(rounds, (uint32_t)KCAP);
+        const uint32_t extra = (novf + 31u) >> 5;
+        for (uint32_t k = wid; k < rounds + extra; k += SPREAD_WARPS) {
+            int i = -1;
+            if (k < rounds) {
+                if (k < mine) i = idx[k * 32 + lane];
+            } else {
+                const uint32_t j = (k - rounds) * 32u + lane;
+                if (j < novf) i = ovf[j];
+            }
+            if (i < 0) continue;
+            const float4 p = X4[c0 + i];
+            const int spl = __float_as_int(p.w) - sp0;
+            int b[3], d[3];
+            float w[3][P];
+            locate<P>(m, p, o, E, b, d, w);
+            uint32_t* s = sm + spl * E3 + (d[0] * EY + d[1]) * EZ + d[2];
 #pragma unroll
             for (int jx = 0; jx < P; ++jx) {
 #pragma unroll
@@ -161,53 +195,44 @@ __global__ void __launch_bounds__(SPREAD_THREADS) spread_tile_kernel(MeshParams 
                 }
             }
             ++n_tile;
-        } else {
-            // drifted out of the tile's halo since the last re-sort: rare, goes straight to the global grid
-            spread_global_one<P>(m, b, w, grid + (size_t)(sp0 + sp) * m.M);
         }
     }
     __syncthreads();
 
-    // flush: one warp per z-row of the tile so that the global reductions are coalesced along z
+    // flush: consecutive threads take consecutive z of a row so that the global reductions are coalesced along z
     unsigned long long tile_sum = 0;
-    int gz[EZ / 32];
-#pragma unroll
-    for (int it = 0; it < EZ / 32; ++it) gz[it] = wrap_idx(o[2] + lane + 32 * it, m.N[2]);
+    constexpr int RPP = SPREAD_THREADS / EZ;               // rows per pass
+    const int lz = threadIdx.x % EZ, r0 = threadIdx.x / EZ;
+    const int gz = wrap_idx(o[2] + lz, m.N[2]);
     for (int pass = 0; pass < 2; ++pass) {          // pass 1 only runs to undo a wrapped tile
         const float sc = pass == 0 ? FIX_INV : -FIX_INV;
-        for (int spl = 0; spl < nsp; ++spl) {
-            float* gsp = grid + (size_t)(sp0 + spl) * m.M;
-            for (int q = wid; q < EX * EY; q += SPREAD_WARPS) {
-                const int lx = q / EY, ly = q - lx * EY;
-                if (ly >= E[1]) continue;
-                float* grow = gsp + ((size_t)goff_x[lx] * m.N[1] + goff_y[ly]) * m.N[2];
-                const uint32_t* srow = sm + (spl * EX * EY + q) * EZ + lane;
-#pragma unroll
-                for (int it = 0; it < EZ / 32; ++it) {
-                    const uint32_t u = srow[32 * it];
+        if (r0 < RPP) {
+            for (int spl = 0; spl < nsp; ++spl) {
+                float* gsp = grid + (size_t)(sp0 + spl) * m.M + gz;
+                const uint32_t* simg = sm + spl * E3 + lz;
+                for (int q = r0; q < EX * EY; q += RPP) {
+                    const uint32_t u = simg[q * EZ];
                     if (u) {
+                        const int lx = q / EY, ly = q - lx * EY;
                         if (pass == 0) tile_sum += u;
-                        atomicAdd(grow + gz[it], (float)u * sc);
+                        atomicAdd(gsp + ((size_t)goff_x[lx] * m.N[1] + goff_y[ly]) * m.N[2], (float)u * sc);
                     }
                 }
             }
         }
         if (pass == 1) break;
         const unsigned long long total = block_sum_u64(tile_sum, red);
-        const unsigned long long cnt = block_sum_u64((unsigned long long)n_tile, red);
-        const unsigned long long expect = cnt << FIX_BITS, slack = 64ull * cnt + 64ull;
+        const unsigned long long cntp = block_sum_u64((unsigned long long)n_tile, red);
+        const unsigned long long expect = cntp << FIX_BITS, slack = 64ull * cntp + 64ull;
         const bool ok = total + slack >= expect && total <= expect + slack;
         if (ok) return;                               // uniform across the block
     }
     // a node wrapped past 2^32 (>= 512 particles' worth on one node): redo this tile with fp32 global atomics
-    sp = 0;
-    for (uint32_t j = wid; j < rounds_total; j += SPREAD_WARPS) {
-        while (j >= srounds[sp + 1]) ++sp;
-        const float4 p = X4[(size_t)sbase[sp] + (size_t)(j - srounds[sp]) * 32u + lane];
-        if (__float_as_int(p.w) < 0) continue;
+    for (uint32_t i = p_lo + threadIdx.x; i < p_hi; i += SPREAD_THREADS) {
+        const float4 p = X4[i];
         int b[3], d[3];
         float w[3][P];
-        if (locate<P>(m, p, o, E, b, d, w)) spread_global_one<P>(m, b, w, grid + (size_t)(sp0 + sp) * m.M);
+        if (locate<P>(m, p, o, E, b, d, w)) spread_global_one<P>(m, b, w, grid + (size_t)__float_as_int(p.w) * m.M);
     }
 }
 
@@ -225,8 +250,9 @@ template <int P, typename F>
 bool tile_dispatch_p(int p, int ey, int ez, F&& f)
 {
     constexpr int H = (P >= 3) ? 3 : 1;
-    return tile_case<P, 8 + H, 32>(p, ey, ez, f) || tile_case<P, 8 + H, 64>(p, ey, ez, f) ||
-           tile_case<P, 16 + H, 32>(p, ey, ez, f) || tile_case<P, 16 + H, 64>(p, ey, ez, f);
+    constexpr int EZA = (P >= 3) ? 24 : 20, EZB = (P >= 3) ? 40 : 36;   // TZ = 16 / 32 (+ halo + alignment, % 4 == 0)
+    return tile_case<P, 8 + H, EZA>(p, ey, ez, f) || tile_case<P, 8 + H, EZB>(p, ey, ez, f) ||
+           tile_case<P, 16 + H, EZA>(p, ey, ez, f) || tile_case<P, 16 + H, EZB>(p, ey, ez, f);
 }
 template <typename F>
 bool tile_dispatch(int p, int ey, int ez, F&& f)
@@ -264,18 +290,17 @@ int tild_spread_configure(tild_ctx* c)
     return TILD_OK;
 }
 
-// X4 must be in the slab-transposed layout described by lay.
-int launch_spread(tild_ctx* c, const EllLayout& lay, const float4* X4, float* grid)
+// X4 must be segment-sorted with the offsets lay.seg_base.
+int launch_spread(tild_ctx* c, const SegLayout& lay, const float4* X4, float* grid)
 {
     TILD_CUDA(c, cudaMemsetAsync(grid, 0, sizeof(float) * c->M * c->mesh.S, c->stream));
     if (c->mesh.n == 0) return TILD_OK;
     const TileParams& tp = c->tile;
-    if (tp.enabled && lay.total_ell > 0) {
-        const dim3 g((unsigned)tp.ntiles, (unsigned)((c->mesh.S + tp.sp_group - 1) / tp.sp_group));
-        tile_dispatch(c->mesh.P, tp.EY, tp.EZ, [&](auto kernel) {
-            kernel<<<g, SPREAD_THREADS, tp.smem_spread, c->stream>>>(c->mesh, tp, lay.seg_base, X4, grid);
-        });
-        TILD_LAUNCH_CHECK(c, "spread_tile_kernel");
-    }
-    return spread_slots(c, lay.total_ell, lay.used(), X4, grid);
+    if (!tp.enabled || (c->prm.flags & TILD_FLAG_NAIVE_SPREAD)) return spread_slots(c, 0, (size_t)c->mesh.n, X4, grid);
+    const dim3 g((unsigned)tp.ntiles, (unsigned)((c->mesh.S + tp.sp_group - 1) / tp.sp_group));
+    tile_dispatch(c->mesh.P, tp.EY, tp.EZ, [&](auto kernel) {
+        kernel<<<g, SPREAD_THREADS, tp.smem_spread, c->stream>>>(c->mesh, tp, lay.seg_base, X4, grid);
+    });
+    TILD_LAUNCH_CHECK(c, "spread_tile_kernel");
+    return TILD_OK;
 }

@@ -248,7 +248,7 @@ class Tild:
     def tild_layout_info(self) -> dict:
         info = (C.c_uint64 * 8)()
         self._check(self.lib.tild_layout_info(self.ctx, C.byref(info)), "tild_layout_info")
-        names = ("tiles", "segments", "slot_capacity", "ell_slots", "overflow", "tile_x", "tile_y", "tile_z")
+        names = ("tiles", "segments", "image_z", "smem_spread", "smem_interp", "tile_x", "tile_y", "tile_z")
         return dict(zip(names, [int(v) for v in info]))
 
     def tild_launch_count(self) -> int:
