@@ -79,7 +79,7 @@ void configure_tiles(tild_ctx* c)
     if (tz != 16 && tz != 32) tz = 32;
     const int ez = (tz + t.H + t.sh + 3) / 4 * 4;
     const size_t lists_i = (size_t)TILD_INTERP_KCAP * 32 * 2 + (size_t)TILD_INTERP_CHUNK * 2;
-    const size_t lists_s = (size_t)TILD_SPREAD_KCAP * 32 * 2 + (size_t)TILD_SPREAD_CHUNK * 2;
+    const size_t lists_s = (size_t)TILD_SPREAD_KCAP * 32 * 4 + (size_t)TILD_SPREAD_CHUNK * 4;
     auto interp_bytes = [&](int ax, int ay) { return (size_t)(ax + t.H) * (ay + t.H) * 3 * ez * sizeof(float) + lists_i; };
     if (interp_bytes(tx, ty) > 220 * 1024) tx = 8;
     t.EY = ty + t.H;

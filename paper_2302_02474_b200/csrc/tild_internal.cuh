@@ -42,7 +42,7 @@ struct TileParams {
 
 // shared-memory particle binning of the tile kernels
 #define TILD_SPREAD_CHUNK 4096   // particles binned at a time by the spread kernel (all species of its group)
-#define TILD_SPREAD_KCAP 160     // rounds of its class lists (1.25 x the mean of a full chunk); the rest overflows
+#define TILD_SPREAD_KCAP 144     // rounds of its class lists (1.125 x the mean of a full chunk); the rest overflows
 #define TILD_INTERP_CHUNK 2048   // same for the interpolation kernel (one species at a time)
 #define TILD_INTERP_KCAP 96
 

@@ -11,7 +11,7 @@
 
 namespace {
 
-constexpr int INTERP_THREADS = 256;
+constexpr int INTERP_THREADS = 384;
 constexpr int INTERP_WARPS = INTERP_THREADS / 32;
 
 // ---- per-particle global gather (overflow tail, drifted particles, grids too small for tiles) -------------------
@@ -89,6 +89,22 @@ __device__ __forceinline__ float3 interp_global(const MeshParams& m, const float
     return acc;
 }
 
+// f += force on the particle at p from the bond to the particle at q (Eq. 2; minimum image)
+__device__ __forceinline__ void bond_term(const MeshParams& m, const StepParams& s, const float4& p, const float4& q, float3& f)
+{
+    const float dx = min_image(p.x - q.x, m.L[0], m.inv_L[0]);
+    const float dy = min_image(p.y - q.y, m.L[1], m.inv_L[1]);
+    const float dz = min_image(p.z - q.z, m.L[2], m.inv_L[2]);
+    float scale = -2.0f * s.k_bond;
+    if (s.r0_bond != 0.0f) {
+        const float r = sqrtf(dx * dx + dy * dy + dz * dz);
+        scale = r > 0.0f ? scale * (1.0f - s.r0_bond / r) : 0.0f;
+    }
+    f.x += scale * dx;
+    f.y += scale * dy;
+    f.z += scale * dz;
+}
+
 // Bond force on the particle at p from its partners' positions (slots into X4).
 __device__ __forceinline__ float3 bond_force_slots(const MeshParams& m, const StepParams& s, const float4* __restrict__ X4,
                                                    const int32_t* __restrict__ B, size_t slot, const float4& p)
@@ -96,19 +112,7 @@ __device__ __forceinline__ float3 bond_force_slots(const MeshParams& m, const St
     float3 f = make_float3(0.f, 0.f, 0.f);
     for (int k = 0; k < s.max_bonds; ++k) {
         const int32_t j = B[slot * s.max_bonds + k];
-        if (j < 0) continue;
-        const float4 q = X4[j];
-        const float dx = min_image(p.x - q.x, m.L[0], m.inv_L[0]);
-        const float dy = min_image(p.y - q.y, m.L[1], m.inv_L[1]);
-        const float dz = min_image(p.z - q.z, m.L[2], m.inv_L[2]);
-        float scale = -2.0f * s.k_bond;
-        if (s.r0_bond != 0.0f) {
-            const float r = sqrtf(dx * dx + dy * dy + dz * dz);
-            scale = r > 0.0f ? scale * (1.0f - s.r0_bond / r) : 0.0f;
-        }
-        f.x += scale * dx;
-        f.y += scale * dy;
-        f.z += scale * dz;
+        if (j >= 0) bond_term(m, s, p, X4[j], f);
     }
     return f;
 }
@@ -121,23 +125,16 @@ __device__ __forceinline__ float3 bond_force_slots(const MeshParams& m, const St
 //     r^{n+1} = wrap(r^n + b dt v^n + (b dt^2/2m) F^n + (b dt/2m) beta)
 //     w^{n+1} = a v^n + (dt/2m) a F^n + (b/m) beta
 //   Positions are double-buffered because bonds read the partners' r^n while r^{n+1} is written.
+// F already holds the total force; w0 = W4[slot] (MODE 2 only)
 template <int MODE>
-__device__ __forceinline__ void finish_particle(const MeshParams& m, const StepParams& s, uint64_t step_next, size_t slot,
-                                                const float4& p, float3 F, const float4* __restrict__ X4,
-                                                const float4* __restrict__ W4, const int32_t* __restrict__ B,
-                                                float4* __restrict__ X4o, float4* __restrict__ W4o, float4* __restrict__ F4)
+__device__ __forceinline__ void finish_update(const MeshParams& m, const StepParams& s, uint64_t step_next, size_t slot,
+                                              const float4& p, const float3& F, const float4& w0, float4* __restrict__ X4o,
+                                              float4* __restrict__ W4o, float4* __restrict__ F4)
 {
-    if (MODE >= 1) {
-        const float3 fb = bond_force_slots(m, s, X4, B, slot, p);
-        F.x += fb.x;
-        F.y += fb.y;
-        F.z += fb.z;
-    }
     if (MODE <= 1) {
         F4[slot] = make_float4(F.x, F.y, F.z, 0.f);
         return;
     }
-    const float4 w0 = W4[slot];
     float3 beta = make_float3(0.f, 0.f, 0.f);
     if (s.noise_amp != 0.0f) {
         const float3 z = gauss3(__float_as_uint(w0.w), step_next, s.key0, s.key1);
@@ -157,6 +154,23 @@ __device__ __forceinline__ void finish_particle(const MeshParams& m, const StepP
     }
     X4o[slot] = make_float4(xo[0], xo[1], xo[2], p.w);
     W4o[slot] = make_float4(wo[0], wo[1], wo[2], w0.w);
+}
+
+template <int MODE>
+__device__ __forceinline__ void finish_particle(const MeshParams& m, const StepParams& s, uint64_t step_next, size_t slot,
+                                                const float4& p, float3 F, const float4* __restrict__ X4,
+                                                const float4* __restrict__ W4, const int32_t* __restrict__ B,
+                                                float4* __restrict__ X4o, float4* __restrict__ W4o, float4* __restrict__ F4)
+{
+    if (MODE >= 1) {
+        const float3 fb = bond_force_slots(m, s, X4, B, slot, p);
+        F.x += fb.x;
+        F.y += fb.y;
+        F.z += fb.z;
+    }
+    float4 w0 = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (MODE == 2) w0 = W4[slot];
+    finish_update<MODE>(m, s, step_next, slot, p, F, w0, X4o, W4o, F4);
 }
 
 template <int P>
@@ -206,7 +220,7 @@ __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wai
 
 // Dynamic shared memory: image float[3][EX][EY][EZ] of one species | idx u16[KCAP][32] | ovf u16[CHUNK].
 template <int P, int EY, int EZ, int MODE>
-__global__ void __launch_bounds__(INTERP_THREADS) interp_tile_kernel(MeshParams m, TileParams tp, StepParams s, uint64_t step_next,
+__global__ void __launch_bounds__(INTERP_THREADS, 2) interp_tile_kernel(MeshParams m, TileParams tp, StepParams s, uint64_t step_next,
                                                                      const uint32_t* __restrict__ seg_base,
                                                                      const float* __restrict__ ffield,
                                                                      const float4* __restrict__ X4, const float4* __restrict__ W4,
@@ -273,6 +287,8 @@ __global__ void __launch_bounds__(INTERP_THREADS) interp_tile_kernel(MeshParams 
         }
         for (uint32_t c0 = p_lo; c0 < p_hi; c0 += CHUNK) {
             const int nchunk = (int)min((uint32_t)CHUNK, p_hi - c0);
+            // rounds reserved per class: a little above the mean; the rest is worked off in dense mixed rounds
+            const uint32_t kcap = min((uint32_t)KCAP, (uint32_t)(nchunk + 31) / 32u + (uint32_t)(nchunk >> 9) + 1u);
             if (c0 != p_lo) __syncthreads();               // previous chunk's rounds are done
             if (threadIdx.x < 32) cnt[threadIdx.x] = 0u;
             if (threadIdx.x == 32) novf = 0u;
@@ -293,7 +309,7 @@ __global__ void __launch_bounds__(INTERP_THREADS) interp_tile_kernel(MeshParams 
                 if (inside) {
                     const uint32_t cls = (uint32_t)((d[0] * EY + d[1]) * EZ + d[2]) & 31u;
                     const uint32_t k = atomicAdd(&cnt[cls], 1u);
-                    if (k < (uint32_t)KCAP) idx[k * 32 + cls] = (uint16_t)i;
+                    if (k < kcap) idx[k * 32 + cls] = (uint16_t)i;
                     else ovf[atomicAdd(&novf, 1u)] = (uint16_t)i;
                 } else {
                     // drifted out of the tile's halo since the last re-sort: rare, gathers from the global mesh
@@ -308,7 +324,7 @@ __global__ void __launch_bounds__(INTERP_THREADS) interp_tile_kernel(MeshParams 
             uint32_t rounds = mine;
 #pragma unroll
             for (int dlt = 16; dlt > 0; dlt >>= 1) rounds = max(rounds, __shfl_xor_sync(0xffffffffu, rounds, dlt));
-            rounds = min(rounds, (uint32_t)KCAP);
+            rounds = min(rounds, kcap);
             const uint32_t extra = (novf + 31u) >> 5;
             for (uint32_t k = wid; k < rounds + extra; k += INTERP_WARPS) {
                 int i = -1;
@@ -321,9 +337,22 @@ __global__ void __launch_bounds__(INTERP_THREADS) interp_tile_kernel(MeshParams 
                 if (i < 0) continue;
                 const size_t slot = (size_t)c0 + i;
                 const float4 p = X4[slot];
+                // issue the loads the finish needs now, so that their latency hides behind the stencil gather
+                float4 w0 = make_float4(0.f, 0.f, 0.f, 0.f), q0 = p, q1 = p;
+                int bj0 = -1, bj1 = -1;
+                if (MODE == 2) w0 = W4[slot];
+                if (MODE >= 1 && s.max_bonds == 2) {
+                    const int2 bb = *reinterpret_cast<const int2*>(B + 2 * slot);
+                    bj0 = bb.x;
+                    bj1 = bb.y;
+                } else if (MODE >= 1 && s.max_bonds == 1) {
+                    bj0 = B[slot];
+                }
                 int b[3];
                 float w[3][P];
                 index_weights<P>(m, p, b, w);
+                if (MODE >= 1 && bj0 >= 0) q0 = X4[bj0];
+                if (MODE >= 1 && bj1 >= 0) q1 = X4[bj1];
                 const float* f0 = fs + (wrap_near(b[0] - o[0], m.N[0]) * EY + wrap_near(b[1] - o[1], m.N[1])) * EZ +
                                   wrap_near(b[2] - o[2], m.N[2]);
                 const float* f1 = f0 + CS;
@@ -347,7 +376,18 @@ __global__ void __launch_bounds__(INTERP_THREADS) interp_tile_kernel(MeshParams 
                         F.z = fmaf(wxy, tz_, F.z);
                     }
                 }
-                finish_particle<MODE>(m, s, step_next, slot, p, F, X4, W4, B, X4o, W4o, F4);
+                if (MODE >= 1) {
+                    if (s.max_bonds <= 2) {
+                        if (bj0 >= 0) bond_term(m, s, p, q0, F);
+                        if (bj1 >= 0) bond_term(m, s, p, q1, F);
+                    } else {
+                        const float3 fb = bond_force_slots(m, s, X4, B, slot, p);
+                        F.x += fb.x;
+                        F.y += fb.y;
+                        F.z += fb.z;
+                    }
+                }
+                finish_update<MODE>(m, s, step_next, slot, p, F, w0, X4o, W4o, F4);
             }
         }
     }

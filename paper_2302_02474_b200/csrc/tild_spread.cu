@@ -24,7 +24,7 @@
 
 namespace {
 
-constexpr int SPREAD_THREADS = 256;
+constexpr int SPREAD_THREADS = 512;
 constexpr int SPREAD_WARPS = SPREAD_THREADS / 32;
 constexpr int FIX_BITS = 23;                    // tile fixed point: units of 2^-23
 constexpr float FIX_INV = 1.0f / 8388608.0f;
@@ -102,11 +102,26 @@ __device__ __forceinline__ bool locate(const MeshParams& m, const float4& p, con
     return inside;
 }
 
+// weights only (the stencil position is already known): same single-rounded fp32 offsets as index_1d
+template <int P>
+__device__ __forceinline__ void offset_weights(const MeshParams& m, const float4& p, float w[3][P])
+{
+    const float pos[3] = {p.x, p.y, p.z};
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        int cell, b;
+        float t;
+        index_1d<P>(pos[a], m.inv_h[a], cell, b, t);
+        weights_1d<P>(t, w[a]);
+    }
+}
+
 // EY, EZ are template parameters so that every shared-memory offset of the stencil is an immediate.
 // One CTA = one tile x one group of up to tp.sp_group species (blockIdx.y).
-// Dynamic shared memory: image u32[nsp][EX][EY][EZ] | idx u16[KCAP][32] | ovf u16[CHUNK].
+// Dynamic shared memory: image u32[nsp][EX][EY][EZ] | idx u32[KCAP][32] | ovf u32[CHUNK]; a list entry is
+// (image word offset of the first stencil node << 12) | index of the particle in the chunk.
 template <int P, int EY, int EZ>
-__global__ void __launch_bounds__(SPREAD_THREADS) spread_tile_kernel(MeshParams m, TileParams tp,
+__global__ void __launch_bounds__(SPREAD_THREADS, 2) spread_tile_kernel(MeshParams m, TileParams tp,
                                                                      const uint32_t* __restrict__ seg_base,
                                                                      const float4* __restrict__ X4, float* __restrict__ grid)
 {
@@ -115,6 +130,7 @@ __global__ void __launch_bounds__(SPREAD_THREADS) spread_tile_kernel(MeshParams 
     __shared__ unsigned long long red[SPREAD_WARPS];
     __shared__ int goff_x[32], goff_y[32];          // wrapped global x / y node of each local x / y
     __shared__ uint32_t cnt[32], novf;
+    __shared__ uint32_t rowoff[19 * 19];            // mesh offset of image row (lx, ly), z excluded
     const int EX = tp.E[0];
     const int E3 = EX * EY * EZ;
     const int tile = blockIdx.x;
@@ -126,8 +142,8 @@ __global__ void __launch_bounds__(SPREAD_THREADS) spread_tile_kernel(MeshParams 
     const size_t seg0 = (size_t)tile * m.S + sp0;
     const uint32_t p_lo = seg_base[seg0], p_hi = seg_base[seg0 + nsp];
     if (p_lo == p_hi) return;                        // empty tile (uniform)
-    uint16_t* idx = reinterpret_cast<uint16_t*>(sm + (size_t)tp.sp_group * E3);
-    uint16_t* ovf = idx + KCAP * 32;
+    uint32_t* idx = sm + (size_t)tp.sp_group * E3;
+    uint32_t* ovf = idx + KCAP * 32;
 
     {
         uint4* z4 = reinterpret_cast<uint4*>(sm);
@@ -135,12 +151,19 @@ __global__ void __launch_bounds__(SPREAD_THREADS) spread_tile_kernel(MeshParams 
         for (int k = threadIdx.x; k < n4; k += SPREAD_THREADS) z4[k] = make_uint4(0u, 0u, 0u, 0u);
         if (threadIdx.x < EX) goff_x[threadIdx.x] = wrap_idx(o[0] + threadIdx.x, m.N[0]);
         else if (threadIdx.x >= 32 && threadIdx.x < 32 + EY) goff_y[threadIdx.x - 32] = wrap_idx(o[1] + threadIdx.x - 32, m.N[1]);
+        if (threadIdx.x < EX * EY) {                 // EX * EY <= 361 <= SPREAD_THREADS
+            const int lx = threadIdx.x / EY, ly = threadIdx.x - lx * EY;
+            rowoff[threadIdx.x] = (uint32_t)((wrap_idx(o[0] + lx, m.N[0]) * m.N[1] + wrap_idx(o[1] + ly, m.N[1])) * m.N[2]);
+        }
     }
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     uint32_t n_tile = 0;  // particles this thread accumulated through shared memory
 
     for (uint32_t c0 = p_lo; c0 < p_hi; c0 += CHUNK) {
         const int nchunk = (int)min((uint32_t)CHUNK, p_hi - c0);
+        // rounds reserved per class: a little above the mean; what does not fit is worked off in dense rounds of
+        // mixed classes (a few bank conflicts) instead of rounds with idle lanes
+        const uint32_t kcap = min((uint32_t)KCAP, (uint32_t)(nchunk + 31) / 32u + (uint32_t)(nchunk >> 9) + 1u);
         __syncthreads();                             // image zeroed / previous chunk's rounds done
         if (threadIdx.x < 32) cnt[threadIdx.x] = 0u;
         if (threadIdx.x == 32) novf = 0u;
@@ -152,10 +175,11 @@ __global__ void __launch_bounds__(SPREAD_THREADS) spread_tile_kernel(MeshParams 
             int b[3], d[3];
             float w[3][P];
             if (locate<P>(m, p, o, E, b, d, w)) {
-                const uint32_t cls = (uint32_t)(spl * E3 + (d[0] * EY + d[1]) * EZ + d[2]) & 31u;
+                const uint32_t off = (uint32_t)(spl * E3 + (d[0] * EY + d[1]) * EZ + d[2]);
+                const uint32_t cls = off & 31u, ent = (off << 12) | (uint32_t)i;
                 const uint32_t k = atomicAdd(&cnt[cls], 1u);
-                if (k < (uint32_t)KCAP) idx[k * 32 + cls] = (uint16_t)i;
-                else ovf[atomicAdd(&novf, 1u)] = (uint16_t)i;
+                if (k < kcap) idx[k * 32 + cls] = ent;
+                else ovf[atomicAdd(&novf, 1u)] = ent;
             } else {
                 // drifted out of the tile's halo since the last re-sort: rare, goes straight to the global grid
                 spread_global_one<P>(m, b, w, grid + (size_t)(sp0 + spl) * m.M);
@@ -167,23 +191,21 @@ __global__ void __launch_bounds__(SPREAD_THREADS) spread_tile_kernel(MeshParams 
         uint32_t rounds = mine;
 #pragma unroll
         for (int dlt = 16; dlt > 0; dlt >>= 1) rounds = max(rounds, __shfl_xor_sync(0xffffffffu, rounds, dlt));
-        rounds = min(rounds, (uint32_t)KCAP);
+        rounds = min(rounds, kcap);
         const uint32_t extra = (novf + 31u) >> 5;
         for (uint32_t k = wid; k < rounds + extra; k += SPREAD_WARPS) {
-            int i = -1;
+            uint32_t ent = 0xFFFFFFFFu;
             if (k < rounds) {
-                if (k < mine) i = idx[k * 32 + lane];
+                if (k < mine) ent = idx[k * 32 + lane];
             } else {
                 const uint32_t j = (k - rounds) * 32u + lane;
-                if (j < novf) i = ovf[j];
+                if (j < novf) ent = ovf[j];
             }
-            if (i < 0) continue;
-            const float4 p = X4[c0 + i];
-            const int spl = __float_as_int(p.w) - sp0;
-            int b[3], d[3];
+            if (ent == 0xFFFFFFFFu) continue;
+            const float4 p = X4[c0 + (ent & 4095u)];
             float w[3][P];
-            locate<P>(m, p, o, E, b, d, w);
-            uint32_t* s = sm + spl * E3 + (d[0] * EY + d[1]) * EZ + d[2];
+            offset_weights<P>(m, p, w);
+            uint32_t* s = sm + (ent >> 12);
 #pragma unroll
             for (int jx = 0; jx < P; ++jx) {
 #pragma unroll
@@ -213,9 +235,8 @@ __global__ void __launch_bounds__(SPREAD_THREADS) spread_tile_kernel(MeshParams 
                 for (int q = r0; q < EX * EY; q += RPP) {
                     const uint32_t u = simg[q * EZ];
                     if (u) {
-                        const int lx = q / EY, ly = q - lx * EY;
                         if (pass == 0) tile_sum += u;
-                        atomicAdd(gsp + ((size_t)goff_x[lx] * m.N[1] + goff_y[ly]) * m.N[2], (float)u * sc);
+                        atomicAdd(gsp + rowoff[q], (float)u * sc);
                     }
                 }
             }
