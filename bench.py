@@ -79,6 +79,26 @@ def run_oracle(cfg, steps, warmup):
     return cfg.n * steps / dt, 1e3 * dt / steps, orc.get_threads()
 
 
+def replica_seeds(cfg, rank):
+    """Independent replica per rank: same recipe, rank-specific input and Philox seeds."""
+    return cfg.input_seed + 7919 * rank, cfg.philox_seed + rank
+
+
+def max_over_ranks(dist, value, device):
+    """Device time of the slowest replica; `dist` is torch.distributed or None (single process)."""
+    if dist is None:
+        return float(value)
+    import torch
+    t = torch.tensor([float(value)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_value(n, steps, world, ms_total):
+    """Whole-job particle-steps/s: every rank advanced n particles by `steps` steps in ms_total (max over ranks)."""
+    return world * n * steps / (ms_total * 1e-3)
+
+
 class ClockSampler:
     """Samples nvidia-smi clocks and throttle reasons during the timed region."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
@@ -157,8 +177,9 @@ def ours_arm(args, cfg):
         torch.cuda.synchronize()
 
     # independent replica per rank: same recipe, rank-specific seeds
-    st = inputs.make_state(cfg, seed=cfg.input_seed + 7919 * rank)
-    eng = tild.Tild(tild.params_from_config(cfg, flags=tild.FLAG_TIMING | args.flags, seed=cfg.philox_seed + rank,
+    in_seed, ph_seed = replica_seeds(cfg, rank)
+    st = inputs.make_state(cfg, seed=in_seed)
+    eng = tild.Tild(tild.params_from_config(cfg, flags=tild.FLAG_TIMING | args.flags, seed=ph_seed,
                                             resort_every=args.resort_every), device=f"cuda:{local}")
     xd, vd = torch.from_numpy(st.x).cuda(), torch.from_numpy(st.v).cuda()
     td, bd = torch.from_numpy(st.type).cuda(), torch.from_numpy(st.bond_partner).cuda()
@@ -177,13 +198,9 @@ def ours_arm(args, cfg):
     barrier()
     launches = eng.tild_launch_count() - l0
     clocks = sampler.stop()
-    ms_total = e0.elapsed_time(e1)
-    if dist is not None:
-        t = torch.tensor([ms_total], device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t.item())
+    ms_total = max_over_ranks(dist, e0.elapsed_time(e1), "cuda")
     stage_ms, nst = eng.tild_get_timings()
-    value = world * cfg.n * args.steps / (ms_total * 1e-3)
+    value = aggregate_value(cfg.n, args.steps, world, ms_total)
 
     # end to end through the C-ABI with HOST buffers: every step copies the batch in and the result out
     e2e = None
@@ -197,11 +214,7 @@ def ours_arm(args, cfg):
         for r in range(reps):
             eng.tild_run_host(xh, vh, th, bh, r, 1)   # synchronous: H2D + set_state + 1 step + D2H
         barrier()
-        dt = time.perf_counter() - t0
-        if dist is not None:
-            t = torch.tensor([dt], device="cuda")
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            dt = float(t.item())
+        dt = max_over_ranks(dist, time.perf_counter() - t0, "cuda")
         e2e = {"value": world * cfg.n * reps / dt, "unit": UNIT,
                "h2d_bytes_per_step": int(xh.nbytes + vh.nbytes + th.nbytes + bh.nbytes),
                "d2h_bytes_per_step": int(xh.nbytes + vh.nbytes), "steps": reps,
@@ -214,7 +227,8 @@ def ours_arm(args, cfg):
     stages = {}
     for k in ("spread", "kspace", "interp"):
         gbs = alg[k] / (stage_ms[k] * 1e-3) / 1e9 if stage_ms[k] > 0 else 0.0
-        stages[k] = {"ms": stage_ms[k], "alg_bytes": alg[k], "gbs": gbs, "frac": gbs / peak}
+        stages[k] = {"ms": stage_ms[k], "alg_bytes": alg[k], "gbs": gbs, "frac": gbs / peak,
+                     "traffic": NCU_TRAFFIC.get((cfg.name, k))}
     dom = max(stages, key=lambda k: stages[k]["ms"])
     three_ms = sum(stages[k]["ms"] for k in stages)
     three_gbs = sum(alg.values()) / (three_ms * 1e-3) / 1e9 if three_ms > 0 else 0.0
@@ -247,7 +261,11 @@ def ours_arm(args, cfg):
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from `ncu --set full` captures committed under profiles/
 # (key: (workload name, stage)); None until a capture exists.
-NCU_TRAFFIC = {}
+NCU_TRAFFIC = {   # profiles/r1_spread_interp_kspace_c4.md
+    ("C4_diblock_8m", "spread"): 358.1e6,
+    ("C4_diblock_8m", "kspace"): 483.4e6,
+    ("C4_diblock_8m", "interp"): 1038.0e6,
+}
 
 
 def main():

@@ -337,3 +337,46 @@ def test_full_size_config_force_and_short_trajectory(name):
     x, v, _, _ = eng.tild_get_state()
     ox, ov, _ = orc.run(p, st.x.astype(np.float64), st.v.astype(np.float64), st.type, st.bond_partner, 0, nst)
     assert np.abs(min_image(x.cpu().numpy().astype(np.float64) - ox, cfg.box)).max() <= 1e-4
+
+
+def test_layout_info_reports_the_tiling():
+    cfg = inputs.C2
+    st, eng = make(cfg)
+    eng.tild_set_state(dev(st.x), dev(st.v), dev(st.type), dev(st.bond_partner), 0)
+    info = eng.tild_layout_info()
+    assert info["segments"] == info["tiles"] * cfg.n_species
+    assert info["tile_x"] in (8, 16) and info["tile_y"] in (8, 16) and info["tile_z"] in (16, 32)
+    assert info["smem_spread"] <= 113 * 1024 and info["smem_interp"] <= 113 * 1024      # two CTAs per SM
+
+
+def test_c4_full_size_force_and_two_steps():
+    """BASELINE configs[3], the bench workload, in the launch configuration bench.py times (default tiles, default
+    re-sort cadence): total force on every particle against the oracle, zero net force, then two steps."""
+    cfg = inputs.C4
+    st, eng = make(cfg)
+    p = oracle_params(cfg)
+    eng.tild_set_state(dev(st.x), dev(st.v), dev(st.type), dev(st.bond_partner), 0)
+    _, _, f, _ = eng.tild_get_state(want_v=False, want_f=True)
+    f = f.cpu().numpy()
+    of = orc.force(p, st.x.astype(np.float64), st.type, st.bond_partner)
+    scale = vec_rms(of)
+    assert np.abs(f - of).max() <= REL * scale, (np.abs(f - of).max(), scale)
+    assert np.abs(f.astype(np.float64).sum(0)).max() < 1e-4 * scale * np.sqrt(cfg.n)
+    eng.tild_step(2)
+    x, _, _, step = eng.tild_get_state(want_v=False)
+    assert step == 2
+    ox, _, _ = orc.run(p, st.x.astype(np.float64), st.v.astype(np.float64), st.type, st.bond_partner, 0, 2, f=of)
+    dx = min_image(x.cpu().numpy().astype(np.float64) - ox, cfg.box)
+    # A18: fp32 ulp at L = 160 is 1.5e-5; RMS <= 1e-4 and max <= 1e-4 * L / 10
+    assert np.sqrt((dx ** 2).sum(1).mean()) <= 1e-4 and np.abs(dx).max() <= 1e-4 * cfg.box[0] / 10.0
+
+
+@pytest.mark.parametrize("grid,order,memory_order", [(192, 3, "random"), (128, 1, "chain")])
+def test_c5_sweep_point_force(grid, order, memory_order):
+    cfg = inputs.c5(grid=grid, order=order, memory_order=memory_order)
+    st, eng = make(cfg)
+    p = oracle_params(cfg)
+    eng.tild_set_state(dev(st.x), dev(st.v), dev(st.type), dev(st.bond_partner), 0)
+    _, _, f, _ = eng.tild_get_state(want_v=False, want_f=True)
+    of = orc.force(p, st.x.astype(np.float64), st.type, st.bond_partner)
+    assert np.abs(f.cpu().numpy() - of).max() <= REL * vec_rms(of)
