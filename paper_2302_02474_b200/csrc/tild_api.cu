@@ -133,6 +133,7 @@ void carve(tild_ctx* c, void* base, size_t* total)
     c->start = w.take<uint32_t>(c->max_bins + 2);
     c->scan_part = w.take<uint32_t>(tild_scan_scratch_entries(c->max_bins + 2));
     c->perm = w.take<uint32_t>(n);
+    c->drift_count = w.take<uint32_t>(4);
     c->tables = w.take<float>(6 * 4096);
     *total = w.off;
 }
@@ -231,7 +232,7 @@ int tild_init(tild_ctx** out, const tild_params* params, void* workspace, size_t
     const double V = p.box[0] * p.box[1] * p.box[2];
     const double sigma2 = p.sigma2 > 0.0 ? p.sigma2 : 2.0 * p.a * p.a;
     const double rho0 = p.rho0 > 0.0 ? p.rho0 : (double)p.n / V;          // L121
-    c->resort_every = p.resort_every > 0 ? p.resort_every : 20;
+    c->resort_every = p.resort_every > 0 ? p.resort_every : 10;
 
     MeshParams& m = c->mesh;
     m.n = p.n;

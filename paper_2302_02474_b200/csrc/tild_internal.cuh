@@ -96,9 +96,10 @@ struct tild_ctx {
     float2* nhat;         // [S][Mk]
     float2* fhat;         // [3S][Mk]
     float* ffield;        // [3S][M]
-    uint32_t* key;        // [n]
-    uint32_t* rank;       // [n]
+    uint32_t* key;        // [n] sort scratch; between sorts: the drift list of launch_spread
+    uint32_t* rank;       // [n] sort scratch; between sorts: the drift list of launch_interp
     uint32_t* inv;        // [n] old slot -> new slot
+    uint32_t* drift_count;  // [4]
     uint32_t* count;      // [max_bins+1] histogram
     uint32_t* start;      // [max_bins+1] scan output (cell_start of tild_index_map)
     uint32_t* scan_part;  // block sums of the scan

@@ -7,6 +7,8 @@
 // row).  While those copies are in flight the CTA bins the segment's particles by the bank of their first stencil
 // node in the image ("class", see tild_spread.cu), then works in rounds of one particle per class: lane c takes
 // the k-th particle of class c, so each of the 3 P^3 shared-memory loads of the stencil hits 32 different banks.
+#include <stdlib.h>
+
 #include "tild_internal.cuh"
 
 namespace {
@@ -225,12 +227,14 @@ __global__ void __launch_bounds__(INTERP_THREADS, 2) interp_tile_kernel(MeshPara
                                                                      const float* __restrict__ ffield,
                                                                      const float4* __restrict__ X4, const float4* __restrict__ W4,
                                                                      const int32_t* __restrict__ B, float4* __restrict__ X4o,
-                                                                     float4* __restrict__ W4o, float4* __restrict__ F4)
+                                                                     float4* __restrict__ W4o, float4* __restrict__ F4,
+                                                                     uint32_t* __restrict__ drift_list,
+                                                                     uint32_t* __restrict__ drift_count)
 {
     constexpr int CHUNK = TILD_INTERP_CHUNK, KCAP = TILD_INTERP_KCAP;
     extern __shared__ __align__(16) float fs[];
     __shared__ int goff_x[32], goff_y[32];
-    __shared__ uint32_t cnt[32], novf;
+    __shared__ uint32_t cnt[32], novf, ndrift, drift_base;
     const int EX = tp.E[0];
     const int CS = EX * EY * EZ;                              // component stride of the image
     const int tile = blockIdx.x;
@@ -292,6 +296,7 @@ __global__ void __launch_bounds__(INTERP_THREADS, 2) interp_tile_kernel(MeshPara
             if (c0 != p_lo) __syncthreads();               // previous chunk's rounds are done
             if (threadIdx.x < 32) cnt[threadIdx.x] = 0u;
             if (threadIdx.x == 32) novf = 0u;
+            if (threadIdx.x == 33) ndrift = 0u;
             __syncthreads();
             // phase A (overlaps the copies in flight): class = bank of the first stencil node in the image
             for (int i = threadIdx.x; i < nchunk; i += INTERP_THREADS) {
@@ -312,9 +317,9 @@ __global__ void __launch_bounds__(INTERP_THREADS, 2) interp_tile_kernel(MeshPara
                     if (k < kcap) idx[k * 32 + cls] = (uint16_t)i;
                     else ovf[atomicAdd(&novf, 1u)] = (uint16_t)i;
                 } else {
-                    // drifted out of the tile's halo since the last re-sort: rare, gathers from the global mesh
-                    const float3 F = interp_global<P, false>(m, ffield, b, w, sp);
-                    finish_particle<MODE>(m, s, step_next, slot, p, F, X4, W4, B, X4o, W4o, F4);
+                    // drifted out of the tile's halo since the last re-sort: queued (from the top of ovf) and done
+                    // together after the rounds, so that one such particle does not stall the 31 other lanes here
+                    ovf[CHUNK - 1 - atomicAdd(&ndrift, 1u)] = (uint16_t)i;
                 }
             }
             cp_async_wait_all();
@@ -326,17 +331,26 @@ __global__ void __launch_bounds__(INTERP_THREADS, 2) interp_tile_kernel(MeshPara
             for (int dlt = 16; dlt > 0; dlt >>= 1) rounds = max(rounds, __shfl_xor_sync(0xffffffffu, rounds, dlt));
             rounds = min(rounds, kcap);
             const uint32_t extra = (novf + 31u) >> 5;
-            for (uint32_t k = wid; k < rounds + extra; k += INTERP_WARPS) {
-                int i = -1;
+            // software pipeline: the list entry and position of the NEXT round are fetched before this round's work
+            auto fetch = [&](uint32_t k, int& i, float4& p) {
+                i = -1;
                 if (k < rounds) {
                     if (k < mine) i = idx[k * 32 + lane];
-                } else {
+                } else if (k < rounds + extra) {
                     const uint32_t j = (k - rounds) * 32u + lane;
                     if (j < novf) i = ovf[j];
                 }
+                if (i >= 0) p = X4[(size_t)c0 + i];
+            };
+            int i_next;
+            float4 p_next = make_float4(0.f, 0.f, 0.f, 0.f);
+            fetch(wid, i_next, p_next);
+            for (uint32_t k = wid; k < rounds + extra; k += INTERP_WARPS) {
+                const int i = i_next;
+                const float4 p = p_next;
+                fetch(k + INTERP_WARPS, i_next, p_next);
                 if (i < 0) continue;
                 const size_t slot = (size_t)c0 + i;
-                const float4 p = X4[slot];
                 // issue the loads the finish needs now, so that their latency hides behind the stencil gather
                 float4 w0 = make_float4(0.f, 0.f, 0.f, 0.f), q0 = p, q1 = p;
                 int bj0 = -1, bj1 = -1;
@@ -389,8 +403,56 @@ __global__ void __launch_bounds__(INTERP_THREADS, 2) interp_tile_kernel(MeshPara
                 }
                 finish_update<MODE>(m, s, step_next, slot, p, F, w0, X4o, W4o, F4);
             }
+            // drifted particles of this chunk: handed to interp_drift_kernel through a global list (one global
+            // atomic per chunk), so that their long global gathers are off this CTA's critical path
+            if (ndrift > 0) {                              // uniform: ndrift is stable since the sync after phase A
+                if (threadIdx.x == 0) drift_base = atomicAdd(drift_count, ndrift);
+                __syncthreads();
+                for (uint32_t j = threadIdx.x; j < ndrift; j += INTERP_THREADS)
+                    drift_list[drift_base + j] = c0 + ovf[CHUNK - 1 - j];
+            }
         }
     }
+}
+
+// particles that left their tile's image since the last re-sort: per-particle global gather, any order
+template <int P, int MODE>
+__global__ void __launch_bounds__(256) interp_drift_kernel(MeshParams m, StepParams s, uint64_t step_next,
+                                                           const uint32_t* __restrict__ drift_list,
+                                                           const uint32_t* __restrict__ drift_count,
+                                                           const float* __restrict__ ffield, const float4* __restrict__ X4,
+                                                           const float4* __restrict__ W4, const int32_t* __restrict__ B,
+                                                           float4* __restrict__ X4o, float4* __restrict__ W4o,
+                                                           float4* __restrict__ F4)
+{
+    const uint32_t nd = *drift_count;
+    for (uint32_t j = blockIdx.x * blockDim.x + threadIdx.x; j < nd; j += gridDim.x * blockDim.x) {
+        const size_t slot = drift_list[j];
+        const float4 p = X4[slot];
+        int b[3];
+        float w[3][P];
+        index_weights<P>(m, p, b, w);
+        const float3 F = interp_global<P, false>(m, ffield, b, w, __float_as_int(p.w));
+        finish_particle<MODE>(m, s, step_next, slot, p, F, X4, W4, B, X4o, W4o, F4);
+    }
+}
+
+// Split variant of the step (TILD_SPLIT_STEP=1): the tile kernel leaves the interpolated force in F4 and this
+// fully coalesced pass adds the bonds and does the GJF update.
+__global__ void __launch_bounds__(256) gjf_stream_kernel(MeshParams m, StepParams s, uint64_t step_next, const float4* __restrict__ X4,
+                                                         const float4* __restrict__ W4, const int32_t* __restrict__ B,
+                                                         const float4* __restrict__ F4, float4* __restrict__ X4o,
+                                                         float4* __restrict__ W4o)
+{
+    const size_t slot = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (slot >= (size_t)m.n) return;
+    const float4 p = X4[slot], w0 = W4[slot], f = F4[slot];
+    float3 F = make_float3(f.x, f.y, f.z);
+    const float3 fb = bond_force_slots(m, s, X4, B, slot, p);
+    F.x += fb.x;
+    F.y += fb.y;
+    F.z += fb.z;
+    finish_update<2>(m, s, step_next, slot, p, F, w0, X4o, W4o, nullptr);
 }
 
 // caller-order bond force (stage call)
@@ -486,6 +548,8 @@ struct InterpArgs {
     float4* X4o;
     float4* W4o;
     float4* F4;
+    uint32_t* drift_list;
+    uint32_t* drift_count;
 };
 
 template <int P, int EY, int EZ, int MODE>
@@ -498,7 +562,9 @@ void tile_launch(const InterpArgs& a, cudaStream_t st, size_t smem, bool configu
         return;
     }
     kernel<<<a.tp.ntiles, INTERP_THREADS, smem, st>>>(a.m, a.tp, a.s, a.step_next, a.seg_base, a.ffield, a.X4, a.W4, a.B, a.X4o,
-                                                      a.W4o, a.F4);
+                                                      a.W4o, a.F4, a.drift_list, a.drift_count);
+    interp_drift_kernel<P, MODE><<<592, 256, 0, st>>>(a.m, a.s, a.step_next, a.drift_list, a.drift_count, a.ffield, a.X4, a.W4,
+                                                      a.B, a.X4o, a.W4o, a.F4);
 }
 template <int P, int EY, int EZ>
 void tile_launch_m(const InterpArgs& a, int mode, cudaStream_t st, size_t smem, bool cfg, cudaError_t* err)
@@ -560,11 +626,21 @@ int launch_interp(tild_ctx* c, int mode, const SegLayout& lay, const float* ffie
 {
     const size_t n = (size_t)c->mesh.n;
     if (n == 0) return TILD_OK;
-    InterpArgs a{c->mesh, c->tile, c->stp, c->step + 1, lay.seg_base, ffield, X4, W4, B, X4o, W4o, c->F4};
+    InterpArgs a{c->mesh, c->tile, c->stp, c->step + 1, lay.seg_base, ffield, X4, W4, B, X4o, W4o, c->F4, c->rank, c->drift_count};
     if (c->tile.enabled && !(c->prm.flags & TILD_FLAG_NAIVE_INTERP)) {
         cudaError_t e = cudaSuccess;
+        TILD_CUDA(c, cudaMemsetAsync(c->drift_count, 0, sizeof(uint32_t), c->stream));
+        static const bool split = getenv("TILD_SPLIT_STEP") && atoi(getenv("TILD_SPLIT_STEP")) != 0;
+        if (split && mode == INTERP_FUSED_STEP) {
+            tile_launch_any(a, INTERP_NONBONDED_BY_ID, c->stream, c->tile.smem_interp, false, &e);
+            TILD_LAUNCH_CHECK(c, "interp_tile_kernel");
+            gjf_stream_kernel<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(c->mesh, c->stp, c->step + 1, X4, W4, B, c->F4, X4o, W4o);
+            TILD_LAUNCH_CHECK(c, "gjf_stream_kernel");
+            return TILD_OK;
+        }
         tile_launch_any(a, mode, c->stream, c->tile.smem_interp, false, &e);
         TILD_LAUNCH_CHECK(c, "interp_tile_kernel");
+        TILD_LAUNCH_CHECK(c, "interp_drift_kernel");
         return TILD_OK;
     }
     const bool vec = can_vectorize(c, ffield);

@@ -129,7 +129,7 @@ __global__ void __launch_bounds__(SPREAD_THREADS, 2) spread_tile_kernel(MeshPara
     extern __shared__ __align__(16) uint32_t sm[];
     __shared__ unsigned long long red[SPREAD_WARPS];
     __shared__ int goff_x[32], goff_y[32];          // wrapped global x / y node of each local x / y
-    __shared__ uint32_t cnt[32], novf;
+    __shared__ uint32_t cnt[32], novf, ndrift;
     __shared__ uint32_t rowoff[19 * 19];            // mesh offset of image row (lx, ly), z excluded
     const int EX = tp.E[0];
     const int E3 = EX * EY * EZ;
@@ -167,6 +167,7 @@ __global__ void __launch_bounds__(SPREAD_THREADS, 2) spread_tile_kernel(MeshPara
         __syncthreads();                             // image zeroed / previous chunk's rounds done
         if (threadIdx.x < 32) cnt[threadIdx.x] = 0u;
         if (threadIdx.x == 32) novf = 0u;
+        if (threadIdx.x == 33) ndrift = 0u;
         __syncthreads();
         // phase A: class of every particle = bank of its first stencil node in the image
         for (int i = threadIdx.x; i < nchunk; i += SPREAD_THREADS) {
@@ -181,8 +182,9 @@ __global__ void __launch_bounds__(SPREAD_THREADS, 2) spread_tile_kernel(MeshPara
                 if (k < kcap) idx[k * 32 + cls] = ent;
                 else ovf[atomicAdd(&novf, 1u)] = ent;
             } else {
-                // drifted out of the tile's halo since the last re-sort: rare, goes straight to the global grid
-                spread_global_one<P>(m, b, w, grid + (size_t)(sp0 + spl) * m.M);
+                // drifted out of the tile's halo since the last re-sort: queued (from the top of ovf) and done
+                // together after the rounds, so that one such particle does not stall the 31 other lanes here
+                ovf[CHUNK - 1 - atomicAdd(&ndrift, 1u)] = (uint32_t)i;
             }
         }
         __syncthreads();
@@ -217,6 +219,15 @@ __global__ void __launch_bounds__(SPREAD_THREADS, 2) spread_tile_kernel(MeshPara
                 }
             }
             ++n_tile;
+        }
+        // drifted particles of this chunk: straight to the global grid (fp32 reductions resolve in L2).  Kept in
+        // this CTA: a separate kernel for them measured slower (its reductions no longer overlap other tiles' work)
+        for (uint32_t j = threadIdx.x; j < ndrift; j += SPREAD_THREADS) {
+            const float4 p = X4[c0 + ovf[CHUNK - 1 - j]];
+            int b[3], d[3];
+            float w[3][P];
+            locate<P>(m, p, o, E, b, d, w);
+            spread_global_one<P>(m, b, w, grid + (size_t)__float_as_int(p.w) * m.M);
         }
     }
     __syncthreads();
