@@ -253,6 +253,10 @@ __global__ void __launch_bounds__(SPREAD_THREADS, 2) spread_tile_kernel(MeshPara
             }
         }
         if (pass == 1) break;
+        // A node can only wrap past 2^32 if >= 2^9 / (largest single-node weight) particles sit on it: the largest
+        // weight is 1 (P <= 2), (3/4)^3 (P = 3), (23/48)^3 (P = 4).  Tiles with fewer particles skip the check.
+        constexpr uint32_t SAFE = P <= 2 ? 511u : (P == 3 ? 1213u : 4653u);
+        if (p_hi - p_lo <= SAFE) return;              // uniform across the block
         const unsigned long long total = block_sum_u64(tile_sum, red);
         const unsigned long long cntp = block_sum_u64((unsigned long long)n_tile, red);
         const unsigned long long expect = cntp << FIX_BITS, slack = 64ull * cntp + 64ull;
