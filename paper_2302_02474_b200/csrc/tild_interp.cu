@@ -299,9 +299,16 @@ __global__ void __launch_bounds__(INTERP_THREADS, 2) interp_tile_kernel(MeshPara
             if (threadIdx.x == 33) ndrift = 0u;
             __syncthreads();
             // phase A (overlaps the copies in flight): class = bank of the first stencil node in the image
-            for (int i = threadIdx.x; i < nchunk; i += INTERP_THREADS) {
-                const size_t slot = (size_t)c0 + i;
-                const float4 p = X4[slot];
+            for (int i0 = threadIdx.x; i0 < nchunk; i0 += 3 * INTERP_THREADS) {   // three loads in flight per thread
+                float4 pj[3];
+#pragma unroll
+                for (int j = 0; j < 3; ++j)
+                    if (i0 + j * INTERP_THREADS < nchunk) pj[j] = X4[(size_t)c0 + i0 + j * INTERP_THREADS];
+#pragma unroll
+                for (int j = 0; j < 3; ++j) {
+                const int i = i0 + j * INTERP_THREADS;
+                if (i >= nchunk) break;
+                const float4 p = pj[j];
                 int b[3], d[3];
                 float w[3][P];
                 index_weights<P>(m, p, b, w);
@@ -320,6 +327,7 @@ __global__ void __launch_bounds__(INTERP_THREADS, 2) interp_tile_kernel(MeshPara
                     // drifted out of the tile's halo since the last re-sort: queued (from the top of ovf) and done
                     // together after the rounds, so that one such particle does not stall the 31 other lanes here
                     ovf[CHUNK - 1 - atomicAdd(&ndrift, 1u)] = (uint16_t)i;
+                }
                 }
             }
             cp_async_wait_all();

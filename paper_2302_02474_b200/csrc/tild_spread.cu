@@ -17,7 +17,7 @@
 // sm_100a has no native fp32 shared-memory atomic add (atomicAdd(float*) on shared compiles to an
 // LDS + FADD + ATOMS.CAST.SPIN loop) but does have a native 32-bit integer one (ATOMS.ADD).  The tile is
 // therefore accumulated in unsigned 2^-23 fixed point: each contribution is rounded once to 2^-23 (read off the
-// mantissa of 1 + w, so no F2I on the XU pipe), the integer sum is exact and order-independent, and it is
+// bit pattern of the denormal w 2^-126, so no F2I on the XU pipe), the integer sum is exact and order-independent, and it is
 // converted to fp32 at the flush.  A tile node holds < 512; a wrap is detected exactly by the tile's mass balance
 // (sum of the tile == particles * 2^23 up to rounding) and such a tile is redone with fp32 global atomics.
 #include "tild_internal.cuh"
@@ -170,8 +170,16 @@ __global__ void __launch_bounds__(SPREAD_THREADS, 2) spread_tile_kernel(MeshPara
         if (threadIdx.x == 33) ndrift = 0u;
         __syncthreads();
         // phase A: class of every particle = bank of its first stencil node in the image
-        for (int i = threadIdx.x; i < nchunk; i += SPREAD_THREADS) {
-            const float4 p = X4[c0 + i];
+        for (int i0 = threadIdx.x; i0 < nchunk; i0 += 4 * SPREAD_THREADS) {   // four loads in flight per thread
+            float4 pj[4];
+#pragma unroll
+            for (int j = 0; j < 4; ++j)
+                if (i0 + j * SPREAD_THREADS < nchunk) pj[j] = X4[c0 + i0 + j * SPREAD_THREADS];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+            const int i = i0 + j * SPREAD_THREADS;
+            if (i >= nchunk) break;
+            const float4 p = pj[j];
             const int spl = __float_as_int(p.w) - sp0;
             int b[3], d[3];
             float w[3][P];
@@ -185,6 +193,7 @@ __global__ void __launch_bounds__(SPREAD_THREADS, 2) spread_tile_kernel(MeshPara
                 // drifted out of the tile's halo since the last re-sort: queued (from the top of ovf) and done
                 // together after the rounds, so that one such particle does not stall the 31 other lanes here
                 ovf[CHUNK - 1 - atomicAdd(&ndrift, 1u)] = (uint32_t)i;
+            }
             }
         }
         __syncthreads();
@@ -208,14 +217,22 @@ __global__ void __launch_bounds__(SPREAD_THREADS, 2) spread_tile_kernel(MeshPara
             float w[3][P];
             offset_weights<P>(m, p, w);
             uint32_t* s = sm + (ent >> 12);
+            // round(w 2^23) with one FMUL and no F2I: w 2^-126 is a denormal (or the smallest normal for w = 1) whose
+            // bit pattern IS the integer round(w 2^23); the two 2^-63 factors keep both operands normal, so the
+            // product is rounded once, to nearest.  (Denormals are on: the library is built without -ftz.)
+#pragma unroll
+            for (int j = 0; j < P; ++j) {
+                w[0][j] *= 0x1p-63f;
+                w[2][j] *= 0x1p-63f;
+            }
 #pragma unroll
             for (int jx = 0; jx < P; ++jx) {
 #pragma unroll
                 for (int jy = 0; jy < P; ++jy) {
                     const float wxy = w[0][jx] * w[1][jy];
 #pragma unroll
-                    for (int jz = 0; jz < P; ++jz)       // round(w 2^23) without F2I: mantissa of (w + 1), w in [0, 1]
-                        atomicAdd(s + (jx * EY + jy) * EZ + jz, __float_as_uint(fmaf(wxy, w[2][jz], 1.0f)) - 0x3F800000u);
+                    for (int jz = 0; jz < P; ++jz)
+                        atomicAdd(s + (jx * EY + jy) * EZ + jz, __float_as_uint(__fmul_rn(wxy, w[2][jz])));
                 }
             }
             ++n_tile;
