@@ -440,7 +440,9 @@ __global__ void __launch_bounds__(256) interp_drift_kernel(MeshParams m, StepPar
         int b[3];
         float w[3][P];
         index_weights<P>(m, p, b, w);
-        const float3 F = interp_global<P, false>(m, ffield, b, w, __float_as_int(p.w));
+        const bool vec = (m.N[2] % 4 == 0) && ((reinterpret_cast<uintptr_t>(ffield) & 15) == 0);   // uniform
+        const float3 F = vec ? interp_global<P, true>(m, ffield, b, w, __float_as_int(p.w))
+                             : interp_global<P, false>(m, ffield, b, w, __float_as_int(p.w));
         finish_particle<MODE>(m, s, step_next, slot, p, F, X4, W4, B, X4o, W4o, F4);
     }
 }
