@@ -7,8 +7,6 @@
 // row).  While those copies are in flight the CTA bins the segment's particles by the bank of their first stencil
 // node in the image ("class", see tild_spread.cu), then works in rounds of one particle per class: lane c takes
 // the k-th particle of class c, so each of the 3 P^3 shared-memory loads of the stencil hits 32 different banks.
-#include <stdlib.h>
-
 #include "tild_internal.cuh"
 
 namespace {
@@ -447,24 +445,6 @@ __global__ void __launch_bounds__(256) interp_drift_kernel(MeshParams m, StepPar
     }
 }
 
-// Split variant of the step (TILD_SPLIT_STEP=1): the tile kernel leaves the interpolated force in F4 and this
-// fully coalesced pass adds the bonds and does the GJF update.
-__global__ void __launch_bounds__(256) gjf_stream_kernel(MeshParams m, StepParams s, uint64_t step_next, const float4* __restrict__ X4,
-                                                         const float4* __restrict__ W4, const int32_t* __restrict__ B,
-                                                         const float4* __restrict__ F4, float4* __restrict__ X4o,
-                                                         float4* __restrict__ W4o)
-{
-    const size_t slot = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (slot >= (size_t)m.n) return;
-    const float4 p = X4[slot], w0 = W4[slot], f = F4[slot];
-    float3 F = make_float3(f.x, f.y, f.z);
-    const float3 fb = bond_force_slots(m, s, X4, B, slot, p);
-    F.x += fb.x;
-    F.y += fb.y;
-    F.z += fb.z;
-    finish_update<2>(m, s, step_next, slot, p, F, w0, X4o, W4o, nullptr);
-}
-
 // caller-order bond force (stage call)
 __global__ void __launch_bounds__(256) bond_force_kernel(MeshParams m, StepParams s, const float* __restrict__ x,
                                                          const int32_t* __restrict__ bond, float* __restrict__ f)
@@ -640,14 +620,6 @@ int launch_interp(tild_ctx* c, int mode, const SegLayout& lay, const float* ffie
     if (c->tile.enabled && !(c->prm.flags & TILD_FLAG_NAIVE_INTERP)) {
         cudaError_t e = cudaSuccess;
         TILD_CUDA(c, cudaMemsetAsync(c->drift_count, 0, sizeof(uint32_t), c->stream));
-        static const bool split = getenv("TILD_SPLIT_STEP") && atoi(getenv("TILD_SPLIT_STEP")) != 0;
-        if (split && mode == INTERP_FUSED_STEP) {
-            tile_launch_any(a, INTERP_NONBONDED_BY_ID, c->stream, c->tile.smem_interp, false, &e);
-            TILD_LAUNCH_CHECK(c, "interp_tile_kernel");
-            gjf_stream_kernel<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(c->mesh, c->stp, c->step + 1, X4, W4, B, c->F4, X4o, W4o);
-            TILD_LAUNCH_CHECK(c, "gjf_stream_kernel");
-            return TILD_OK;
-        }
         tile_launch_any(a, mode, c->stream, c->tile.smem_interp, false, &e);
         TILD_LAUNCH_CHECK(c, "interp_tile_kernel");
         TILD_LAUNCH_CHECK(c, "interp_drift_kernel");

@@ -380,3 +380,26 @@ def test_c5_sweep_point_force(grid, order, memory_order):
     _, _, f, _ = eng.tild_get_state(want_v=False, want_f=True)
     of = orc.force(p, st.x.astype(np.float64), st.type, st.bond_partner)
     assert np.abs(f.cpu().numpy() - of).max() <= REL * vec_rms(of)
+
+
+@pytest.mark.parametrize("env", [{"TILD_TILE_X": "16", "TILD_TILE_Y": "8"}, {"TILD_TILE_Y": "8", "TILD_TILE_Z": "16"},
+                                 {"TILD_TILE_X": "16", "TILD_TILE_Y": "16", "TILD_TILE_Z": "16"}],
+                         ids=["x16y8", "y8z16", "x16y16z16"])
+@pytest.mark.parametrize("P", [2, 3, 4])
+def test_tile_shape_variants(env, P, monkeypatch):
+    """Every (EY, EZ) instantiation of the tile kernels gives the same forces and trajectories."""
+    for k, v in env.items():
+        monkeypatch.setenv(k, v)
+    cfg = small_cfg(order=P, grid=(40, 24, 48), box=(20.0, 12.0, 24.0), n_chains=900)
+    st, eng = make(cfg, resort_every=3)
+    p = oracle_params(cfg)
+    eng.tild_set_state(dev(st.x), dev(st.v), dev(st.type), dev(st.bond_partner), 0)
+    info = eng.tild_layout_info()
+    assert info["tile_y"] == int(env.get("TILD_TILE_Y", 16)) and info["tile_z"] == int(env.get("TILD_TILE_Z", 32))
+    _, _, f, _ = eng.tild_get_state(want_v=False, want_f=True)
+    of = orc.force(p, st.x.astype(np.float64), st.type, st.bond_partner)
+    assert np.abs(f.cpu().numpy() - of).max() <= REL * vec_rms(of)
+    eng.tild_step(10)
+    x, _, _, _ = eng.tild_get_state(want_v=False)
+    ox, _, _ = orc.run(p, st.x.astype(np.float64), st.v.astype(np.float64), st.type, st.bond_partner, 0, 10, f=of)
+    assert np.abs(min_image(x.cpu().numpy().astype(np.float64) - ox, cfg.box)).max() <= 1e-4
