@@ -268,6 +268,35 @@ NCU_TRAFFIC = {   # profiles/r1_spread_interp_kspace_c4.md
 }
 
 
+def sweep_arm(args):
+    """C5 roofline sweep (BASELINE.json configs[4]): grid x order x memory order, 50 steps per point, per-stage times.
+    Prints one JSON line per point; not the headline bench line."""
+    import torch
+    from paper_2302_02474_b200 import tild
+    peak, _ = measured_peak_gbs()
+    for grid in (128, 192, 256):
+        for order in (1, 2, 3, 4):
+            for mo in ("random", "sorted"):
+                cfg = inputs.c5(grid=grid, order=order, memory_order=mo)
+                st = inputs.make_state(cfg)
+                eng = tild.Tild(tild.params_from_config(cfg, flags=tild.FLAG_TIMING))
+                d = lambda a: torch.from_numpy(a).cuda()
+                eng.tild_set_state(d(st.x), d(st.v), d(st.type), d(st.bond_partner), 0)
+                eng.tild_step(10)
+                eng.tild_get_timings()
+                eng.tild_step(cfg.steps)
+                ms, nst = eng.tild_get_timings()
+                alg = algorithmic_bytes(cfg)
+                three = sum(ms[k] for k in alg)
+                print(json.dumps({"sweep": "C5", "grid": grid, "order": order, "memory_order": mo, "steps": nst,
+                                  "stage_ms": {k: round(v, 4) for k, v in ms.items()},
+                                  "particle_steps_per_sec": cfg.n / (ms["total"] * 1e-3),
+                                  "frac": {k: alg[k] / (ms[k] * 1e-3) / 1e9 / peak for k in alg},
+                                  "spread_kspace_interp_frac": sum(alg.values()) / (three * 1e-3) / 1e9 / peak}), flush=True)
+                eng.close()
+                del eng
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -280,9 +309,12 @@ def main():
     ap.add_argument("--flags", type=int, default=0, help="extra TILD_FLAG_* bits (kernel A/B runs)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--sweep", action="store_true", help="run the C5 roofline sweep instead of the headline bench")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
     cfg = inputs.CONFIGS[args.workload]
+    if args.sweep:
+        return sweep_arm(args)
     if args.impl == "reference":
         reference_arm(args, cfg)
     else:
