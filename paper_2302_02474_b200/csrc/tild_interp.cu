@@ -617,7 +617,7 @@ int launch_interp(tild_ctx* c, int mode, const SegLayout& lay, const float* ffie
     const size_t n = (size_t)c->mesh.n;
     if (n == 0) return TILD_OK;
     InterpArgs a{c->mesh, c->tile, c->stp, c->step + 1, lay.seg_base, ffield, X4, W4, B, X4o, W4o, c->F4, c->rank, c->drift_count};
-    if (c->tile.enabled && !(c->prm.flags & TILD_FLAG_NAIVE_INTERP)) {
+    if (c->tile.enabled && c->mesh.P >= 2 && !(c->prm.flags & TILD_FLAG_NAIVE_INTERP)) {   // P = 1: one node per particle
         cudaError_t e = cudaSuccess;
         TILD_CUDA(c, cudaMemsetAsync(c->drift_count, 0, sizeof(uint32_t), c->stream));
         tile_launch_any(a, mode, c->stream, c->tile.smem_interp, false, &e);

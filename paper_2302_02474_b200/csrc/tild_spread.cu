@@ -349,7 +349,8 @@ int launch_spread(tild_ctx* c, const SegLayout& lay, const float4* X4, float* gr
     TILD_CUDA(c, cudaMemsetAsync(grid, 0, sizeof(float) * c->M * c->mesh.S, c->stream));
     if (c->mesh.n == 0) return TILD_OK;
     const TileParams& tp = c->tile;
-    if (!tp.enabled || (c->prm.flags & TILD_FLAG_NAIVE_SPREAD)) return spread_slots(c, 0, (size_t)c->mesh.n, X4, grid);
+    // P = 1 touches one node per particle: the per-particle kernel is faster than any tiling (profiles/r1_c5_sweep.md)
+    if (!tp.enabled || c->mesh.P == 1 || (c->prm.flags & TILD_FLAG_NAIVE_SPREAD)) return spread_slots(c, 0, (size_t)c->mesh.n, X4, grid);
     const dim3 g((unsigned)tp.ntiles, (unsigned)((c->mesh.S + tp.sp_group - 1) / tp.sp_group));
     tile_dispatch(c->mesh.P, tp.EY, tp.EZ, [&](auto kernel) {
         kernel<<<g, SPREAD_THREADS, tp.smem_spread, c->stream>>>(c->mesh, tp, lay.seg_base, X4, grid);
