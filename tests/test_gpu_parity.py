@@ -403,3 +403,54 @@ def test_tile_shape_variants(env, P, monkeypatch):
     x, _, _, _ = eng.tild_get_state(want_v=False)
     ox, _, _ = orc.run(p, st.x.astype(np.float64), st.v.astype(np.float64), st.type, st.bond_partner, 0, 10, f=of)
     assert np.abs(min_image(x.cpu().numpy().astype(np.float64) - ox, cfg.box)).max() <= 1e-4
+
+
+def test_two_contexts_on_their_own_streams_do_not_interfere():
+    """Contexts share no mutable state (include/tild.h): two engines stepped alternately on two non-default streams
+    give the same trajectories as each of them alone on the default stream."""
+    cfgs = [small_cfg(order=4), small_cfg(order=3, S=3, grid=(18, 12, 30), box=(9.0, 6.0, 15.0))]
+    states = [inputs.make_state(c) for c in cfgs]
+
+    def start(cfg, st, stream=None):
+        ctx = torch.cuda.stream(stream) if stream is not None else None
+        if ctx is not None:
+            ctx.__enter__()
+        try:
+            eng = tild.Tild(tild.params_from_config(cfg, resort_every=4), stream=stream)
+            eng.tild_set_state(dev(st.x), dev(st.v), dev(st.type), dev(st.bond_partner), 0)
+        finally:
+            if ctx is not None:
+                ctx.__exit__(None, None, None)
+        return eng
+
+    alone = []
+    for cfg, st in zip(cfgs, states):
+        eng = start(cfg, st)
+        eng.tild_step(24)
+        alone.append(eng.tild_get_state(want_v=False)[0].cpu().numpy())
+    torch.cuda.synchronize()
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    engs = [start(c, s, t) for c, s, t in zip(cfgs, states, streams)]
+    for _ in range(6):
+        for eng in engs:
+            eng.tild_step(4)
+    outs = []
+    for eng, t in zip(engs, streams):
+        with torch.cuda.stream(t):
+            outs.append(eng.tild_get_state(want_v=False)[0])
+    torch.cuda.synchronize()
+    for cfg, a, b in zip(cfgs, alone, outs):
+        assert np.abs(min_image(a.astype(np.float64) - b.cpu().numpy(), cfg.box)).max() < 2e-5
+
+
+def test_set_state_can_be_called_again_and_restarts_the_step_counter():
+    cfg = small_cfg(order=2)
+    st, eng = make(cfg)
+    eng.tild_set_state(dev(st.x), dev(st.v), dev(st.type), dev(st.bond_partner), 0)
+    eng.tild_step(7)
+    x1 = eng.tild_get_state(want_v=False)[0].cpu().numpy()
+    eng.tild_set_state(dev(st.x), dev(st.v), dev(st.type), dev(st.bond_partner), 0)
+    eng.tild_step(7)
+    x2, _, _, step = eng.tild_get_state(want_v=False)
+    assert step == 7
+    assert np.abs(min_image(x1.astype(np.float64) - x2.cpu().numpy(), cfg.box)).max() < 2e-5
