@@ -50,6 +50,9 @@ typedef enum {
 #define TILD_FLAG_TIMING 1u        /* record CUDA events around every stage of tild_step */
 #define TILD_FLAG_NAIVE_SPREAD 2u  /* per-particle global-atomic spread (baseline kernel) */
 #define TILD_FLAG_NAIVE_INTERP 4u  /* per-particle global-gather interpolation (baseline kernel) */
+#define TILD_FLAG_GRAPH 8u         /* tild_step replays blocks of 2*resort_every steps as one CUDA graph (launch-bound
+                                      small systems); ignored with TILD_FLAG_TIMING, an odd resort_every, or the
+                                      legacy default stream (which cannot be captured) */
 
 typedef struct tild_ctx tild_ctx;
 

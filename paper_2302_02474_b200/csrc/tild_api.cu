@@ -134,6 +134,7 @@ void carve(tild_ctx* c, void* base, size_t* total)
     c->scan_part = w.take<uint32_t>(tild_scan_scratch_entries(c->max_bins + 2));
     c->perm = w.take<uint32_t>(n);
     c->drift_count = w.take<uint32_t>(4);
+    c->d_step = w.take<uint64_t>(2);
     c->tables = w.take<float>(6 * 4096);
     *total = w.off;
 }
@@ -332,6 +333,7 @@ void tild_destroy(tild_ctx* c)
         cufftDestroy(c->plan_r2c);
         cufftDestroy(c->plan_c2r);
     }
+    if (c->graph_ok) cudaGraphExecDestroy(c->graph_exec);
     if (c->ev_ok)
         for (int i = 0; i < TILD_MAX_TIMED_STEPS; ++i)
             for (int k = 0; k < TILD_N_STAGE_EVENTS; ++k) cudaEventDestroy(c->ev[i][k]);
@@ -420,38 +422,111 @@ int tild_set_state(tild_ctx* c, const float* x, const float* v, const int32_t* t
     if ((rc = force_current(c))) return rc;
     if ((rc = launch_make_w(c, c->F4, c->W4[c->cur], -1.0f))) return rc;  // w = v - (dt/2m) F
     c->step = step0;
+    c->h_step_upload = step0;
+    TILD_CUDA(c, cudaMemcpyAsync(c->d_step, &c->h_step_upload, sizeof(uint64_t), cudaMemcpyHostToDevice, c->stream));
     c->has_state = true;
     c->timed_steps = 0;
     return TILD_OK;
 }
+
+}  // extern "C"
+
+namespace {
+
+// one TILD step on the internal state (re-sort when due, mesh pipeline, fused interpolation pass, step counter)
+int enqueue_one_step(tild_ctx* c, cudaEvent_t* ev)
+{
+    if (ev) cudaEventRecord(ev[0], c->stream);
+    if (c->steps_since_sort >= c->resort_every) {
+        int rc = launch_reorder(c);
+        if (rc) return rc;
+    }
+    if (ev) cudaEventRecord(ev[1], c->stream);
+    const int a = c->cur;
+    int rc = mesh_pipeline(c, c->lay, c->X4[a], ev);
+    if (rc) return rc;
+    rc = launch_interp(c, INTERP_FUSED_STEP, c->lay, c->ffield, c->X4[a], c->W4[a], c->B[a], c->X4[1 - a], c->W4[1 - a], nullptr);
+    if (rc) return rc;
+    if ((rc = launch_advance_step(c))) return rc;
+    // swap only the x/w pointers so that `cur` keeps naming the buffer that holds the bond table
+    float4* t = c->X4[a]; c->X4[a] = c->X4[1 - a]; c->X4[1 - a] = t;
+    t = c->W4[a]; c->W4[a] = c->W4[1 - a]; c->W4[1 - a] = t;
+    if (ev) cudaEventRecord(ev[6], c->stream);
+    c->step++;
+    c->steps_since_sort++;
+    return TILD_OK;
+}
+
+// TILD_FLAG_GRAPH: two re-sort cycles (2 * resort_every steps, starting with a re-sort) as one CUDA graph.  After an
+// even number of steps per cycle and two cycles every buffer pointer is back where it started, and the step index
+// lives in device memory, so the instantiated graph can be replayed as it is.
+int launch_graph_block(tild_ctx* c)
+{
+    const int block = 2 * c->resort_every;
+    if (!(c->graph_ok && c->graph_cur == c->cur && c->graph_x0 == c->X4[0])) {
+        if (c->graph_ok) {
+            cudaGraphExecDestroy(c->graph_exec);
+            c->graph_ok = false;
+        }
+        // capture: nothing executes, so the host bookkeeping the enqueue advances is put back afterwards
+        const int cur0 = c->cur, sss0 = c->steps_since_sort;
+        const uint64_t step0 = c->step;
+        const int64_t launches0 = c->launches;
+        float4* const x0[2] = {c->X4[0], c->X4[1]};
+        float4* const w0[2] = {c->W4[0], c->W4[1]};
+        TILD_CUDA(c, cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal));
+        int rc = TILD_OK;
+        for (int i = 0; i < block && rc == TILD_OK; ++i) rc = enqueue_one_step(c, nullptr);
+        cudaGraph_t graph = nullptr;
+        const cudaError_t e = cudaStreamEndCapture(c->stream, &graph);
+        c->graph_launches = c->launches - launches0;
+        const bool same = c->cur == cur0 && c->X4[0] == x0[0] && c->W4[0] == w0[0] && c->steps_since_sort == sss0;
+        c->cur = cur0; c->steps_since_sort = sss0; c->step = step0; c->launches = launches0;
+        c->X4[0] = x0[0]; c->X4[1] = x0[1]; c->W4[0] = w0[0]; c->W4[1] = w0[1];
+        if (rc != TILD_OK || e != cudaSuccess || !graph || !same) {
+            if (graph) cudaGraphDestroy(graph);
+            if (rc != TILD_OK) return rc;
+            return tild_fail(c, TILD_ECUDA, "CUDA graph capture of %d steps failed: %s", block,
+                             e != cudaSuccess ? cudaGetErrorString(e) : "state does not return to its start");
+        }
+        const cudaError_t ei = cudaGraphInstantiate(&c->graph_exec, graph, 0);
+        cudaGraphDestroy(graph);
+        if (ei != cudaSuccess) return tild_fail(c, TILD_ECUDA, "cudaGraphInstantiate: %s", cudaGetErrorString(ei));
+        c->graph_ok = true;
+        c->graph_cur = c->cur;
+        c->graph_x0 = c->X4[0];
+    }
+    TILD_CUDA(c, cudaGraphLaunch(c->graph_exec, c->stream));
+    c->step += (uint64_t)block;          // pointers, cur and steps_since_sort end where they started
+    c->launches += c->graph_launches;
+    return TILD_OK;
+}
+
+}  // namespace
+
+extern "C" {
 
 int tild_step(tild_ctx* c, int32_t nsteps)
 {
     if (!c) return TILD_EINVAL;
     if (!c->has_state) return tild_fail(c, TILD_ESTATE, "tild_step before tild_set_state");
     if (nsteps < 0) return tild_fail(c, TILD_EINVAL, "tild_step: nsteps < 0");
-    for (int32_t s = 0; s < nsteps; ++s) {
-        cudaEvent_t* ev = (c->ev_ok && c->timed_steps < TILD_MAX_TIMED_STEPS) ? c->ev[c->timed_steps] : nullptr;
-        if (ev) cudaEventRecord(ev[0], c->stream);
-        if (c->steps_since_sort >= c->resort_every) {
-            int rc = launch_reorder(c);
+    // stream capture is not available on the legacy default stream (NULL / cudaStreamLegacy)
+    const bool graphs = (c->prm.flags & TILD_FLAG_GRAPH) && !c->ev_ok && c->resort_every % 2 == 0 && c->stream != nullptr &&
+                        c->stream != cudaStreamLegacy;
+    int32_t s = 0;
+    while (s < nsteps) {
+        if (graphs && c->steps_since_sort >= c->resort_every && nsteps - s >= 2 * c->resort_every) {
+            int rc = launch_graph_block(c);
             if (rc) return rc;
+            s += 2 * c->resort_every;
+            continue;
         }
-        if (ev) cudaEventRecord(ev[1], c->stream);
-        const int a = c->cur;
-        int rc = mesh_pipeline(c, c->lay, c->X4[a], ev);
+        cudaEvent_t* ev = (c->ev_ok && c->timed_steps < TILD_MAX_TIMED_STEPS) ? c->ev[c->timed_steps] : nullptr;
+        int rc = enqueue_one_step(c, ev);
         if (rc) return rc;
-        rc = launch_interp(c, INTERP_FUSED_STEP, c->lay, c->ffield, c->X4[a], c->W4[a], c->B[a], c->X4[1 - a], c->W4[1 - a], nullptr);
-        if (rc) return rc;
-        // swap only the x/w pointers so that `cur` keeps naming the buffer that holds the bond table
-        float4* t = c->X4[a]; c->X4[a] = c->X4[1 - a]; c->X4[1 - a] = t;
-        t = c->W4[a]; c->W4[a] = c->W4[1 - a]; c->W4[1 - a] = t;
-        if (ev) {
-            cudaEventRecord(ev[6], c->stream);
-            c->timed_steps++;
-        }
-        c->step++;
-        c->steps_since_sort++;
+        if (ev) c->timed_steps++;
+        ++s;
     }
     return TILD_OK;
 }

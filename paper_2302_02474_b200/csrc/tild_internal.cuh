@@ -100,6 +100,8 @@ struct tild_ctx {
     uint32_t* rank;       // [n] sort scratch; between sorts: the drift list of launch_interp
     uint32_t* inv;        // [n] old slot -> new slot
     uint32_t* drift_count;  // [4]
+    uint64_t* d_step;       // device copy of `step` (read by the fused step kernels, advanced by a kernel)
+    uint64_t h_step_upload; // staging for the asynchronous upload of d_step
     uint32_t* count;      // [max_bins+1] histogram
     uint32_t* start;      // [max_bins+1] scan output (cell_start of tild_index_map)
     uint32_t* scan_part;  // block sums of the scan
@@ -114,6 +116,13 @@ struct tild_ctx {
     int steps_since_sort;
     int resort_every;
     int64_t launches;
+
+    // TILD_FLAG_GRAPH: instantiated graph of two re-sort cycles and the state it was captured in
+    cudaGraphExec_t graph_exec;
+    bool graph_ok;
+    int graph_cur;
+    float4* graph_x0;
+    int64_t graph_launches;
 
     // timing
     cudaEvent_t ev[TILD_MAX_TIMED_STEPS][TILD_N_STAGE_EVENTS];
@@ -160,6 +169,7 @@ int launch_interp(tild_ctx* c, int mode, const SegLayout& lay, const float* ffie
 int launch_bond_force_caller(tild_ctx* c, const float* x, const int32_t* bond, float* f);  // caller-order stage call
 int launch_make_w(tild_ctx* c, const float4* F4, float4* W4, float sign);   // w += sign*(dt/2m) f
 int launch_velocity_out(tild_ctx* c, const float4* F4, const float4* W4, float* v);  // v[id] = w + (dt/2m) f
+int launch_advance_step(tild_ctx* c);
 int launch_philox_test(tild_ctx* c, const uint32_t* ctr, const uint32_t* key, uint32_t* out, float* gauss, int m);
 
 size_t tild_scan_scratch_entries(size_t nbins);

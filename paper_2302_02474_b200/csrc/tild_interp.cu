@@ -188,12 +188,13 @@ __device__ __forceinline__ void index_weights(const MeshParams& m, const float4&
 
 // per-particle kernel over the slots [s0, s1)
 template <int P, bool VEC, int MODE>
-__global__ void __launch_bounds__(256) interp_slots_kernel(MeshParams m, StepParams s, uint64_t step_next, size_t s0, size_t s1,
+__global__ void __launch_bounds__(256) interp_slots_kernel(MeshParams m, StepParams s, const uint64_t* __restrict__ step_ptr, size_t s0, size_t s1,
                                                            const float* __restrict__ ffield, const float4* __restrict__ X4,
                                                            const float4* __restrict__ W4, const int32_t* __restrict__ B,
                                                            float4* __restrict__ X4o, float4* __restrict__ W4o,
                                                            float4* __restrict__ F4)
 {
+    const uint64_t step_next = *step_ptr + 1;   // the step being produced (device-side counter: graph replays see it move)
     const size_t slot = s0 + (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (slot >= s1) return;
     const float4 p = X4[slot];
@@ -220,7 +221,7 @@ __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wai
 
 // Dynamic shared memory: image float[3][EX][EY][EZ] of one species | idx u16[KCAP][32] | ovf u16[CHUNK].
 template <int P, int EY, int EZ, int MODE>
-__global__ void __launch_bounds__(INTERP_THREADS, 2) interp_tile_kernel(MeshParams m, TileParams tp, StepParams s, uint64_t step_next,
+__global__ void __launch_bounds__(INTERP_THREADS, 2) interp_tile_kernel(MeshParams m, TileParams tp, StepParams s, const uint64_t* __restrict__ step_ptr,
                                                                      const uint32_t* __restrict__ seg_base,
                                                                      const float* __restrict__ ffield,
                                                                      const float4* __restrict__ X4, const float4* __restrict__ W4,
@@ -229,6 +230,7 @@ __global__ void __launch_bounds__(INTERP_THREADS, 2) interp_tile_kernel(MeshPara
                                                                      uint32_t* __restrict__ drift_list,
                                                                      uint32_t* __restrict__ drift_count)
 {
+    const uint64_t step_next = *step_ptr + 1;   // the step being produced (device-side counter: graph replays see it move)
     constexpr int CHUNK = TILD_INTERP_CHUNK, KCAP = TILD_INTERP_KCAP;
     extern __shared__ __align__(16) float fs[];
     __shared__ int goff_x[32], goff_y[32];
@@ -423,7 +425,7 @@ __global__ void __launch_bounds__(INTERP_THREADS, 2) interp_tile_kernel(MeshPara
 
 // particles that left their tile's image since the last re-sort: per-particle global gather, any order
 template <int P, int MODE>
-__global__ void __launch_bounds__(256) interp_drift_kernel(MeshParams m, StepParams s, uint64_t step_next,
+__global__ void __launch_bounds__(256) interp_drift_kernel(MeshParams m, StepParams s, const uint64_t* __restrict__ step_ptr,
                                                            const uint32_t* __restrict__ drift_list,
                                                            const uint32_t* __restrict__ drift_count,
                                                            const float* __restrict__ ffield, const float4* __restrict__ X4,
@@ -431,6 +433,7 @@ __global__ void __launch_bounds__(256) interp_drift_kernel(MeshParams m, StepPar
                                                            float4* __restrict__ X4o, float4* __restrict__ W4o,
                                                            float4* __restrict__ F4)
 {
+    const uint64_t step_next = *step_ptr + 1;   // the step being produced (device-side counter: graph replays see it move)
     const uint32_t nd = *drift_count;
     for (uint32_t j = blockIdx.x * blockDim.x + threadIdx.x; j < nd; j += gridDim.x * blockDim.x) {
         const size_t slot = drift_list[j];
@@ -529,7 +532,7 @@ struct InterpArgs {
     MeshParams m;
     TileParams tp;
     StepParams s;
-    uint64_t step_next;
+    const uint64_t* step_ptr;
     const uint32_t* seg_base;
     const float* ffield;
     const float4* X4;
@@ -551,9 +554,9 @@ void tile_launch(const InterpArgs& a, cudaStream_t st, size_t smem, bool configu
         if (e != cudaSuccess) *err = e;
         return;
     }
-    kernel<<<a.tp.ntiles, INTERP_THREADS, smem, st>>>(a.m, a.tp, a.s, a.step_next, a.seg_base, a.ffield, a.X4, a.W4, a.B, a.X4o,
+    kernel<<<a.tp.ntiles, INTERP_THREADS, smem, st>>>(a.m, a.tp, a.s, a.step_ptr, a.seg_base, a.ffield, a.X4, a.W4, a.B, a.X4o,
                                                       a.W4o, a.F4, a.drift_list, a.drift_count);
-    interp_drift_kernel<P, MODE><<<592, 256, 0, st>>>(a.m, a.s, a.step_next, a.drift_list, a.drift_count, a.ffield, a.X4, a.W4,
+    interp_drift_kernel<P, MODE><<<592, 256, 0, st>>>(a.m, a.s, a.step_ptr, a.drift_list, a.drift_count, a.ffield, a.X4, a.W4,
                                                       a.B, a.X4o, a.W4o, a.F4);
 }
 template <int P, int EY, int EZ>
@@ -589,7 +592,7 @@ template <int P>
 void slots_launch_p(const InterpArgs& a, bool vec, int mode, size_t s0, size_t s1, cudaStream_t st)
 {
     const unsigned nb = (unsigned)((s1 - s0 + 255) / 256);
-#define TILD_SL(V, M_) interp_slots_kernel<P, V, M_><<<nb, 256, 0, st>>>(a.m, a.s, a.step_next, s0, s1, a.ffield, a.X4, a.W4, a.B, a.X4o, a.W4o, a.F4)
+#define TILD_SL(V, M_) interp_slots_kernel<P, V, M_><<<nb, 256, 0, st>>>(a.m, a.s, a.step_ptr, s0, s1, a.ffield, a.X4, a.W4, a.B, a.X4o, a.W4o, a.F4)
     if (vec) { if (mode == 0) TILD_SL(true, 0); else if (mode == 1) TILD_SL(true, 1); else TILD_SL(true, 2); }
     else     { if (mode == 0) TILD_SL(false, 0); else if (mode == 1) TILD_SL(false, 1); else TILD_SL(false, 2); }
 #undef TILD_SL
@@ -616,7 +619,7 @@ int launch_interp(tild_ctx* c, int mode, const SegLayout& lay, const float* ffie
 {
     const size_t n = (size_t)c->mesh.n;
     if (n == 0) return TILD_OK;
-    InterpArgs a{c->mesh, c->tile, c->stp, c->step + 1, lay.seg_base, ffield, X4, W4, B, X4o, W4o, c->F4, c->rank, c->drift_count};
+    InterpArgs a{c->mesh, c->tile, c->stp, c->d_step, lay.seg_base, ffield, X4, W4, B, X4o, W4o, c->F4, c->rank, c->drift_count};
     if (c->tile.enabled && c->mesh.P >= 2 && !(c->prm.flags & TILD_FLAG_NAIVE_INTERP)) {   // P = 1: one node per particle
         cudaError_t e = cudaSuccess;
         TILD_CUDA(c, cudaMemsetAsync(c->drift_count, 0, sizeof(uint32_t), c->stream));
@@ -633,6 +636,15 @@ int launch_interp(tild_ctx* c, int mode, const SegLayout& lay, const float* ffie
     default: slots_launch_p<4>(a, vec, mode, 0, n, c->stream); break;
     }
     TILD_LAUNCH_CHECK(c, "interp_slots_kernel");
+    return TILD_OK;
+}
+
+__global__ void advance_step_kernel(uint64_t* step) { *step += 1; }
+
+int launch_advance_step(tild_ctx* c)
+{
+    advance_step_kernel<<<1, 1, 0, c->stream>>>(c->d_step);
+    TILD_LAUNCH_CHECK(c, "advance_step_kernel");
     return TILD_OK;
 }
 

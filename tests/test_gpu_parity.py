@@ -454,3 +454,27 @@ def test_set_state_can_be_called_again_and_restarts_the_step_counter():
     x2, _, _, step = eng.tild_get_state(want_v=False)
     assert step == 7
     assert np.abs(min_image(x1.astype(np.float64) - x2.cpu().numpy(), cfg.box)).max() < 2e-5
+
+
+def test_cuda_graph_blocks_match_eager_stepping():
+    """TILD_FLAG_GRAPH replays 2 * resort_every steps as one CUDA graph; noise still follows (id, step)."""
+    cfg = small_cfg(order=3)
+    st = inputs.make_state(cfg)
+    outs = []
+    side = torch.cuda.Stream()                   # the legacy default stream cannot be captured
+    for flags in (0, tild.FLAG_GRAPH):
+        with torch.cuda.stream(side):
+            eng = tild.Tild(tild.params_from_config(cfg, flags=flags, resort_every=4), stream=side)
+            eng.tild_set_state(dev(st.x), dev(st.v), dev(st.type), dev(st.bond_partner), 3)
+            eng.tild_step(4 + 3 * 8 + 5)        # eager prefix, three graph blocks (one capture + two replays), eager tail
+            x, v, _, step = eng.tild_get_state()
+        side.synchronize()
+        assert step == 3 + 33
+        outs.append((x.cpu().numpy().astype(np.float64), v.cpu().numpy().astype(np.float64)))
+        if flags:
+            assert eng.tild_launch_count() > 33 * 4
+    assert np.abs(min_image(outs[0][0] - outs[1][0], cfg.box)).max() < 2e-5
+    assert np.abs(outs[0][1] - outs[1][1]).max() < 1e-3
+    p = oracle_params(cfg)
+    ox, _, _ = orc.run(p, st.x.astype(np.float64), st.v.astype(np.float64), st.type, st.bond_partner, 3, 33)
+    assert np.abs(min_image(outs[1][0] - ox, cfg.box)).max() <= 1e-4
