@@ -8,7 +8,7 @@
 // is per tile node instead of per particle.
 //
 // Bank conflicts: 32 particles of a warp in cell order hit the 32 banks at random (measured 3.5 wavefronts per
-// ATOMS, profiles/r1_spread_interp_before.md).  All P^3 stencil offsets are the same for every particle, so the bank
+// ATOMS, profiles/r1_before.md).  All P^3 stencil offsets are the same for every particle, so the bank
 // of each access is (bank of the first stencil node) + const.  Each step the CTA therefore first bins its particles
 // by that bank ("class") into 32 shared-memory lists (phase A: one shared atomic per particle), then works in rounds
 // of one particle per class (phase B): lane c takes the k-th particle of class c, and every ATOMS of the round hits
