@@ -316,7 +316,7 @@ __global__ void __launch_bounds__(INTERP_THREADS, 2) interp_tile_kernel(MeshPara
 #pragma unroll
                 for (int a = 0; a < 3; ++a) {
                     d[a] = wrap_near(b[a] - o[a], m.N[a]);
-                    inside = inside && (d[a] + P <= E[a]);
+                    inside = inside && ((unsigned)d[a] + (unsigned)P <= (unsigned)E[a]);   // unsigned: a wild position (d < 0) is not inside
                 }
                 if (inside) {
                     const uint32_t cls = (uint32_t)((d[0] * EY + d[1]) * EZ + d[2]) & 31u;

@@ -97,7 +97,7 @@ __device__ __forceinline__ bool locate(const MeshParams& m, const float4& p, con
         index_1d<P>(pos[a], m.inv_h[a], cell, b[a], t);
         weights_1d<P>(t, w[a]);
         d[a] = wrap_near(b[a] - o[a], m.N[a]);  // a periodic image of the stencil's first node, relative to the tile (N >= 8)
-        inside = inside && (d[a] + P <= E[a]);
+        inside = inside && ((unsigned)d[a] + (unsigned)P <= (unsigned)E[a]);   // unsigned: a wild position (d < 0) is not inside
     }
     return inside;
 }

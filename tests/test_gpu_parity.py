@@ -478,3 +478,20 @@ def test_cuda_graph_blocks_match_eager_stepping():
     p = oracle_params(cfg)
     ox, _, _ = orc.run(p, st.x.astype(np.float64), st.v.astype(np.float64), st.type, st.bond_partner, 3, 33)
     assert np.abs(min_image(outs[1][0] - ox, cfg.box)).max() <= 1e-4
+
+
+def test_positions_outside_the_box_are_wrapped_not_trusted():
+    """tild.h asks for positions in [0, L]; positions several boxes away must still land on the right nodes (periodic
+    images) instead of indexing outside a tile image."""
+    cfg = small_cfg(order=4)
+    st = inputs.make_state(cfg)
+    L = np.array(cfg.box, dtype=np.float32)
+    x = st.x.copy()
+    x[::3] += 3 * L
+    x[1::3] -= 2 * L
+    eng = tild.Tild(tild.params_from_config(cfg))
+    g = eng.tild_spread(dev(x), dev(st.type)).cpu().numpy()
+    assert np.allclose(g.sum(axis=(1, 2, 3)), np.bincount(st.type, minlength=cfg.n_species), rtol=1e-5)
+    p = oracle_params(cfg)
+    og = orc.spread(p, x, st.type)
+    assert np.abs(g - og).max() <= 1e-4 * rms(og)          # fp32 position resolution is coarser 3 boxes out
