@@ -49,6 +49,7 @@ typedef struct {
     int32_t max_bonds;
     double dt, gamma, kT, mass;
     uint64_t seed;
+    int32_t deconvolve; /* 0: kernel is u^(k) (A13); 1: u^(k) / W^(k)^2, W^ = prod_a sinc(k_a h_a / 2)^P */
 } orc_params;
 
 static const double ORC_PI = 3.14159265358979323846264338327950288;
@@ -342,6 +343,26 @@ static double orc_cIJ(const orc_params *p, int I, int J)
     return (p->kappa + p->chi[I * ORC_MAX_SPECIES + J]) / p->rho0;
 }
 
+/* Pair kernel at mode (mx, my, mz).  PAPER.md L121: u^(k) = exp(-sigma2 |k|^2 / 2) (A4, A5).
+ * deconvolve = 1 (reading A13): divided by the squared Fourier transform of the order-P assignment
+ * function, W^(k) = prod_a [sin(x_a) / x_a]^P with x_a = k_a h_a / 2 = pi m~_a / N_a (Hockney & Eastwood; the P-fold
+ * top-hat convolution of O2 has this transform), which undoes the smoothing of spreading and interpolating with W. */
+static double orc_uhat(const orc_params *p, int mx, int my, int mz)
+{
+    const int m[3] = {mx, my, mz};
+    double k2 = 0.0, w2 = 1.0;
+    for (int a = 0; a < 3; ++a) {
+        const double k = orc_k(p, a, m[a]);
+        k2 += k * k;
+        if (p->deconvolve) {
+            const double x = 0.5 * k * p->L[a] / (double)p->N[a];
+            const double sinc = x == 0.0 ? 1.0 : sin(x) / x;
+            w2 *= pow(sinc, 2.0 * p->P);
+        }
+    }
+    return exp(-0.5 * p->sigma2 * k2) / w2;
+}
+
 /* ------------------------------------------------------------------------------------------
  * O4-O6 k-space force.  PAPER.md Eq. 18, "becomes a simple multiplication" L227:
  *   n^_J(m)   = sum_g n_J(g) exp(-2 pi i m.g/N)
@@ -372,7 +393,8 @@ void orc_kspace_force(const orc_params *p, const double *grid, double *ffield)
                     for (int mz = 0; mz < p->N[2]; ++mz) {
                         size_t g = ((size_t)mx * p->N[1] + my) * p->N[2] + mz;
                         double kx = orc_k(p, 0, mx), ky = orc_k(p, 1, my), kz = orc_k(p, 2, mz);
-                        double uhat = exp(-0.5 * p->sigma2 * (kx * kx + ky * ky + kz * kz));
+                        double uhat = orc_uhat(p, mx, my, mz);
+                        (void)kx; (void)ky; (void)kz;
                         int m_a = a == 0 ? mx : (a == 1 ? my : mz);
                         double kg = orc_kgrad(p, a, m_a);
                         double gr = 0.0, gi = 0.0;
@@ -634,7 +656,8 @@ void orc_energy(const orc_params *p, const double *x, const double *v, const int
             for (int mz = 0; mz < p->N[2]; ++mz) {
                 size_t g = ((size_t)mx * p->N[1] + my) * p->N[2] + mz;
                 double kx = orc_k(p, 0, mx), ky = orc_k(p, 1, my), kz = orc_k(p, 2, mz);
-                double uhat = exp(-0.5 * p->sigma2 * (kx * kx + ky * ky + kz * kz));
+                double uhat = orc_uhat(p, mx, my, mz);
+                (void)kx; (void)ky; (void)kz;
                 double acc = 0.0;
                 for (int I = 0; I < S; ++I)
                     for (int J = 0; J < S; ++J) {

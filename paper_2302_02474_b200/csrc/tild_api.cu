@@ -257,6 +257,11 @@ int tild_init(tild_ctx** out, const tild_params* params, void* workspace, size_t
             const double k = 2.0 * PI * (double)mt / p.box[a];
             const double kg = (N % 2 == 0 && mm == N / 2) ? 0.0 : k;
             double u = exp(-0.5 * sigma2 * k * k);
+            if (p.flags & TILD_FLAG_DECONVOLVE) {   // separable: [sinc(k h / 2)]^(-2P) per axis
+                const double xh = 0.5 * k * p.box[a] / (double)N;
+                const double sinc = xh == 0.0 ? 1.0 : sin(xh) / xh;
+                u /= pow(sinc, 2.0 * p.order);
+            }
             if (a == 0) u /= V;
             tab[(size_t)a * 4096 + mm] = (float)kg;
             tab[(size_t)(3 + a) * 4096 + mm] = (float)u;

@@ -18,7 +18,7 @@ MAX_SPECIES = 8
 MAX_BONDS = 4
 
 OK, EINVAL, ENOMEM, ECUDA, ECUFFT, ESTATE = 0, -1, -2, -3, -4, -5
-FLAG_TIMING, FLAG_NAIVE_SPREAD, FLAG_NAIVE_INTERP, FLAG_GRAPH = 1, 2, 4, 8
+FLAG_TIMING, FLAG_NAIVE_SPREAD, FLAG_NAIVE_INTERP, FLAG_GRAPH, FLAG_DECONVOLVE = 1, 2, 4, 8, 16
 TIMING_NAMES = ("sort", "spread", "fft_fwd", "kspace", "fft_inv", "interp", "other", "total")
 
 EXPORTS = (

@@ -495,3 +495,21 @@ def test_positions_outside_the_box_are_wrapped_not_trusted():
     p = oracle_params(cfg)
     og = orc.spread(p, x, st.type)
     assert np.abs(g - og).max() <= 1e-4 * rms(og)          # fp32 position resolution is coarser 3 boxes out
+
+
+@pytest.mark.parametrize("P", [2, 3, 4])
+def test_deconvolved_kernel_parity(P):
+    """TILD_FLAG_DECONVOLVE (SURVEY 8(f) #2): k-space stage and total force against the oracle's deconvolved kernel."""
+    cfg = small_cfg(order=P)
+    st, eng = make(cfg, flags=tild.FLAG_DECONVOLVE)
+    p = oracle_params(cfg, deconvolve=True)
+    og32 = orc.spread(p, st.x, st.type).astype(np.float32)
+    ff = eng.tild_kspace_force(dev(og32)).cpu().numpy()
+    off = orc.kspace_force(p, og32.astype(np.float64))
+    assert np.abs(ff - off).max() <= REL * rms(off)
+    plain = orc.kspace_force(oracle_params(cfg), og32.astype(np.float64))
+    assert np.abs(off - plain).max() > 0.05 * rms(plain)            # the flag really changes the field
+    eng.tild_set_state(dev(st.x), dev(st.v), dev(st.type), dev(st.bond_partner), 0)
+    _, _, f, _ = eng.tild_get_state(want_v=False, want_f=True)
+    of = orc.force(p, st.x.astype(np.float64), st.type, st.bond_partner)
+    assert np.abs(f.cpu().numpy() - of).max() <= REL * vec_rms(of)

@@ -242,3 +242,42 @@ def test_force_is_minus_gradient_of_mesh_energy_up_to_discretisation():
         dE = (orc.energy(p, xp, v, ty, bp)[2] - orc.energy(p, xm, v, ty, bp)[2]) / (2 * eps)
         rel.append(abs(-dE - F[3, 1]) / np.abs(F[3]).max())
     assert rel[1] < 0.02 and rel[1] < rel[0], rel
+
+
+# ---- assignment-function deconvolution (kernel u^(k) / W^(k)^2) --------------------------------------
+def test_deconvolved_kernel_removes_the_assignment_smoothing():
+    """Plain PM smears the pair kernel by W^2 (error vs the bare analytic force: tens of percent at h = 0.625,
+    growing with P).  Dividing the kernel by W^(k)^2 leaves only aliasing: the error against the BARE analytic
+    Gaussian pair force must drop well below the plain error and shrink with the order."""
+    L = (10.0, 10.0, 10.0)
+    x = np.array([[4.1, 5.2, 4.9], [4.9, 4.7, 5.3]], dtype=np.float32)
+    ty = np.array([0, 1], dtype=np.int32)
+    chi = np.array([[0.0, 1.0], [1.0, 0.0]])
+    ref = direct_pair_force(x, ty, L, chi, 0.0, 2.0, 0.5, images=1)
+    plain, dec = {}, {}
+    for P in (2, 3, 4):
+        for store, flag in ((plain, False), (dec, True)):
+            p = orc.OracleParams(2, 2, L, (16,) * 3, P, chi, kappa=0.0, sigma2=0.5, rho0=2.0, deconvolve=flag)
+            F = orc.nonbonded_force(p, x, ty)
+            store[P] = np.abs(F - ref).max() / np.abs(ref).max()
+    assert plain[2] > 0.2 and plain[4] > plain[2]                 # the smoothing error grows with P (A13)
+    assert dec[2] < 0.15 and dec[3] < 0.06 and dec[4] < 0.02      # aliasing only
+    assert dec[4] < dec[3] < dec[2]
+    for P in (2, 3, 4):
+        assert dec[P] < 0.35 * plain[P], (P, plain, dec)
+
+
+def test_deconvolved_kernel_keeps_momentum_and_reduces_to_plain_at_k0():
+    rng = np.random.default_rng(5)
+    L, N = (6.0, 4.5, 7.0), (12, 8, 10)
+    n = 150
+    x = (rng.random((n, 3)) * np.array(L)).astype(np.float32)
+    ty = rng.integers(0, 3, size=n).astype(np.int32)
+    p = orc.OracleParams(n, 3, L, N, 3, CHI3, kappa=5.0, sigma2=0.5, rho0=2.0, deconvolve=True)
+    F = orc.nonbonded_force(p, x, ty)
+    assert np.abs(F.sum(0)).max() < 1e-10 * np.abs(F).max() * n   # the modified kernel is still real and even
+    # a uniform density (only k = 0 populated) feels no force under either kernel
+    q = orc.OracleParams(n, 3, L, N, 3, CHI3, kappa=5.0, sigma2=0.5, rho0=2.0)
+    grid = np.ones((3,) + N)
+    for params in (p, q):
+        assert np.abs(orc.kspace_force(params, grid)).max() < 1e-12
