@@ -120,6 +120,11 @@ int tild_step(tild_ctx*, int32_t nsteps);
  * current positions (no state change).  Any of x, v, f may be NULL.  step is HOST out, nullable. */
 int tild_get_state(tild_ctx*, float* x, float* v, float* f, uint64_t* step /*HOST*/);
 
+/* HOST out, synchronises.  Energies of the current state (diagnostic): e[0] kinetic m/2 sum |v|^2,
+ * e[1] bonds sum k (|d| - r0)^2 (Eq. 2), e[2] non-bonded on the mesh
+ * (1/2V) sum_m u^(k_m) sum_IJ c_IJ Re[n^_I(m) conj(n^_J(m))] (Eq. 3-4).  One force evaluation, no state change. */
+int tild_energy(tild_ctx*, double e[3] /*HOST out*/);
+
 /* a1: index map of arbitrary caller positions.  base[i][a] = first stencil node (unwrapped),
  * cell_key[i] = (cx*Ny+cy)*Nz+cz, perm = particle ids grouped by ascending cell key (order inside
  * a cell unspecified), cell_start[c] = #particles with key < c (M+1 entries).  Any output may be NULL. */

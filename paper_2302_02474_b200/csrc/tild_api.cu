@@ -135,6 +135,7 @@ void carve(tild_ctx* c, void* base, size_t* total)
     c->perm = w.take<uint32_t>(n);
     c->drift_count = w.take<uint32_t>(4);
     c->d_step = w.take<uint64_t>(2);
+    c->d_energy = w.take<double>(4);
     c->tables = w.take<float>(6 * 4096);
     *total = w.off;
 }
@@ -562,6 +563,18 @@ int tild_get_state(tild_ctx* c, float* x, float* v, float* f, uint64_t* step)
             TILD_CUDA(c, cudaMemcpyAsync(v, scratch, bytes, cudaMemcpyDefault, c->stream));
         }
     }
+    return TILD_OK;
+}
+
+int tild_energy(tild_ctx* c, double e[3])
+{
+    if (!c || !e) return TILD_EINVAL;
+    if (!c->has_state) return tild_fail(c, TILD_ESTATE, "tild_energy before tild_set_state");
+    int rc = force_current(c);              // F4 and nhat at the current positions; no state change
+    if (rc) return rc;
+    if ((rc = launch_energy(c, c->d_energy))) return rc;
+    TILD_CUDA(c, cudaMemcpyAsync(e, c->d_energy, 3 * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    TILD_CUDA(c, cudaStreamSynchronize(c->stream));
     return TILD_OK;
 }
 

@@ -1,0 +1,95 @@
+// Energies of the current state (diagnostic, not on the timed path).
+//   e[0] = kinetic  = m/2 sum |v|^2, v = w + (dt/2m) F (the split-kick state of DESIGN.md "GJF in one pass")
+//   e[1] = bonds    = sum_bonds k (|d| - r0)^2, each bond once (Eq. 2)
+//   e[2] = non-bonded on the mesh = (1/2V) sum_m u^(k_m) sum_IJ c_IJ Re[n^_I(m) conj(n^_J(m))] (Eq. 3-4 L119-123 with
+//          the smeared densities of L139-149; the rho0 shift of Eq. 4 touches m = 0 only and is a constant)
+#include "tild_internal.cuh"
+
+namespace {
+
+__device__ __forceinline__ void block_add(double v, double* out)
+{
+    __shared__ double warp_sum[8];
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) v += __shfl_xor_sync(0xffffffffu, v, d);
+    if ((threadIdx.x & 31) == 0) warp_sum[threadIdx.x >> 5] = v;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double s = 0.0;
+        for (int k = 0; k < (int)(blockDim.x >> 5); ++k) s += warp_sum[k];
+        atomicAdd(out, s);
+    }
+}
+
+// half spectrum of the R2C transform: modes with 0 < mz < Nz/2 stand for themselves and their conjugates
+template <int S>
+__global__ void __launch_bounds__(256) kspace_energy_kernel(KspaceParams k, size_t Mk, const float2* __restrict__ nhat,
+                                                            double* __restrict__ out)
+{
+    double e = 0.0;
+    for (size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x; idx < Mk; idx += (size_t)gridDim.x * blockDim.x) {
+        const int mz = (int)(idx % k.Nzc);
+        const size_t r = idx / k.Nzc;
+        const int my = (int)(r % k.N[1]);
+        const int mx = (int)(r / k.N[1]);
+        const double u = (double)__ldg(k.ufac[0] + mx) * (double)__ldg(k.ufac[1] + my) * (double)__ldg(k.ufac[2] + mz);  // 1/V inside
+        float2 nj[S];
+#pragma unroll
+        for (int J = 0; J < S; ++J) nj[J] = nhat[(size_t)J * Mk + idx];
+        double acc = 0.0;
+#pragma unroll
+        for (int I = 0; I < S; ++I)
+#pragma unroll
+            for (int J = 0; J < S; ++J)
+                acc += (double)k.c[I * TILD_MAX_SPECIES + J] * ((double)nj[I].x * nj[J].x + (double)nj[I].y * nj[J].y);
+        const bool self_conjugate = mz == 0 || (k.N[2] % 2 == 0 && mz == k.N[2] / 2);
+        e += (self_conjugate ? 0.5 : 1.0) * u * acc;
+    }
+    block_add(e, out + 2);
+}
+
+__global__ void __launch_bounds__(256) particle_energy_kernel(MeshParams m, StepParams s, double mass, const float4* __restrict__ X4,
+                                                              const float4* __restrict__ W4, const float4* __restrict__ F4,
+                                                              const int32_t* __restrict__ B, double* __restrict__ out)
+{
+    double ke = 0.0, eb = 0.0;
+    for (size_t slot = (size_t)blockIdx.x * blockDim.x + threadIdx.x; slot < (size_t)m.n; slot += (size_t)gridDim.x * blockDim.x) {
+        const float4 p = X4[slot], w = W4[slot], f = F4[slot];
+        const double vx = (double)w.x + (double)s.half_dt_over_m * f.x, vy = (double)w.y + (double)s.half_dt_over_m * f.y,
+                     vz = (double)w.z + (double)s.half_dt_over_m * f.z;
+        ke += 0.5 * mass * (vx * vx + vy * vy + vz * vz);
+        for (int k = 0; k < s.max_bonds; ++k) {
+            const int32_t j = B[slot * s.max_bonds + k];
+            if (j < 0 || (size_t)j <= slot) continue;            // each bond once: from its lower slot
+            const float4 q = X4[j];
+            const double dx = min_image(p.x - q.x, m.L[0], m.inv_L[0]), dy = min_image(p.y - q.y, m.L[1], m.inv_L[1]),
+                         dz = min_image(p.z - q.z, m.L[2], m.inv_L[2]);
+            const double d = sqrt(dx * dx + dy * dy + dz * dz) - (double)s.r0_bond;
+            eb += (double)s.k_bond * d * d;
+        }
+    }
+    block_add(ke, out + 0);
+    __syncthreads();
+    block_add(eb, out + 1);
+}
+
+}  // namespace
+
+// F4 must hold the total force at the current positions and c->nhat their transformed densities (force_current)
+int launch_energy(tild_ctx* c, double* d_out)
+{
+    TILD_CUDA(c, cudaMemsetAsync(d_out, 0, 3 * sizeof(double), c->stream));
+    const unsigned nb = 592;
+#define KE(SS) case SS: kspace_energy_kernel<SS><<<nb, 256, 0, c->stream>>>(c->ksp, c->Mk, c->nhat, d_out); break;
+    switch (c->mesh.S) {
+        KE(1) KE(2) KE(3) KE(4) KE(5) KE(6) KE(7) KE(8)
+    }
+#undef KE
+    TILD_LAUNCH_CHECK(c, "kspace_energy_kernel");
+    if (c->mesh.n > 0) {
+        particle_energy_kernel<<<nb, 256, 0, c->stream>>>(c->mesh, c->stp, c->prm.mass, c->X4[c->cur], c->W4[c->cur], c->F4,
+                                                          c->B[c->cur], d_out);
+        TILD_LAUNCH_CHECK(c, "particle_energy_kernel");
+    }
+    return TILD_OK;
+}

@@ -100,6 +100,7 @@ struct tild_ctx {
     uint32_t* rank;       // [n] sort scratch; between sorts: the drift list of launch_interp
     uint32_t* inv;        // [n] old slot -> new slot
     uint32_t* drift_count;  // [4]
+    double* d_energy;       // [4] reduction targets of tild_energy
     uint64_t* d_step;       // device copy of `step` (read by the fused step kernels, advanced by a kernel)
     uint64_t h_step_upload; // staging for the asynchronous upload of d_step
     uint32_t* count;      // [max_bins+1] histogram
@@ -170,6 +171,7 @@ int launch_bond_force_caller(tild_ctx* c, const float* x, const int32_t* bond, f
 int launch_make_w(tild_ctx* c, const float4* F4, float4* W4, float sign);   // w += sign*(dt/2m) f
 int launch_velocity_out(tild_ctx* c, const float4* F4, const float4* W4, float* v);  // v[id] = w + (dt/2m) f
 int launch_advance_step(tild_ctx* c);
+int launch_energy(tild_ctx* c, double* d_out);   // tild_energy.cu
 int launch_philox_test(tild_ctx* c, const uint32_t* ctr, const uint32_t* key, uint32_t* out, float* gauss, int m);
 
 size_t tild_scan_scratch_entries(size_t nbins);

@@ -23,7 +23,7 @@ TIMING_NAMES = ("sort", "spread", "fft_fwd", "kspace", "fft_inv", "interp", "oth
 
 EXPORTS = (
     "tild_workspace_bytes", "tild_init", "tild_set_state", "tild_spread", "tild_kspace_force", "tild_interp",
-    "tild_bond_force", "tild_step", "tild_get_state", "tild_index_map", "tild_get_timings", "tild_run_host",
+    "tild_bond_force", "tild_step", "tild_get_state", "tild_energy", "tild_index_map", "tild_get_timings", "tild_run_host",
     "tild_philox_test", "tild_layout_info", "tild_launch_count", "tild_last_error", "tild_destroy", "tild_version",
 )
 
@@ -99,6 +99,7 @@ def load():
     lib.tild_bond_force.argtypes = [vp, vp, vp, vp]
     lib.tild_step.argtypes = [vp, i32]
     lib.tild_get_state.argtypes = [vp, vp, vp, vp, C.POINTER(u64)]
+    lib.tild_energy.argtypes = [vp, C.POINTER(C.c_double * 3)]
     lib.tild_index_map.argtypes = [vp, vp, vp, vp, vp, vp]
     lib.tild_get_timings.argtypes = [vp, C.POINTER(C.c_float * 8), C.POINTER(i32)]
     lib.tild_run_host.argtypes = [vp, vp, vp, vp, vp, u64, i32]
@@ -223,6 +224,12 @@ class Tild:
         step = C.c_uint64(0)
         self._check(self.lib.tild_get_state(self.ctx, _dp(x), _dp(v), _dp(f), C.byref(step)), "tild_get_state")
         return x, v, f, step.value
+
+    def tild_energy(self):
+        """(kinetic, bond, non-bonded mesh) energies of the current state as a numpy array."""
+        e = (C.c_double * 3)()
+        self._check(self.lib.tild_energy(self.ctx, C.byref(e)), "tild_energy")
+        return np.array([e[0], e[1], e[2]])
 
     def tild_get_timings(self):
         ms = (C.c_float * 8)()

@@ -513,3 +513,22 @@ def test_deconvolved_kernel_parity(P):
     _, _, f, _ = eng.tild_get_state(want_v=False, want_f=True)
     of = orc.force(p, st.x.astype(np.float64), st.type, st.bond_partner)
     assert np.abs(f.cpu().numpy() - of).max() <= REL * vec_rms(of)
+
+
+@pytest.mark.parametrize("cfg", [small_cfg(order=4), small_cfg(order=3, S=3, grid=(18, 12, 30), box=(9.0, 6.0, 15.0)), inputs.C1],
+                         ids=["P4", "P3_S3_odd_grid", "C1"])
+def test_energy_matches_oracle(cfg):
+    """tild_energy (SURVEY 8(f) #3) against the oracle's O10 on the same state: kinetic, bond, non-bonded mesh energy."""
+    st, eng = make(cfg)
+    p = oracle_params(cfg)
+    eng.tild_set_state(dev(st.x), dev(st.v), dev(st.type), dev(st.bond_partner), 0)
+    e0 = eng.tild_energy()
+    o0 = orc.energy(p, st.x.astype(np.float64), st.v.astype(np.float64), st.type, st.bond_partner)
+    assert np.all(np.abs(e0 - o0) <= 2e-5 * np.abs(o0).max()), (e0, o0)
+    eng.tild_step(15)
+    x, v, _, _ = eng.tild_get_state()
+    e1 = eng.tild_energy()
+    o1 = orc.energy(p, x.cpu().numpy().astype(np.float64), v.cpu().numpy().astype(np.float64), st.type, st.bond_partner)
+    assert np.all(np.abs(e1 - o1) <= 2e-5 * np.abs(o1).max()), (e1, o1)
+    x2 = eng.tild_get_state(want_v=False)[0]
+    assert torch.equal(x, x2)                                        # tild_energy does not change the state
