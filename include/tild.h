@@ -125,6 +125,12 @@ int tild_get_state(tild_ctx*, float* x, float* v, float* f, uint64_t* step /*HOS
  * (1/2V) sum_m u^(k_m) sum_IJ c_IJ Re[n^_I(m) conj(n^_J(m))] (Eq. 3-4).  One force evaluation, no state change. */
 int tild_energy(tild_ctx*, double e[3] /*HOST out*/);
 
+/* Structure factor of the current state (diagnostic; Eq. 23, "Compute" class L332-336):
+ * sk[m] (= or +=, by `accumulate`) |sum_{J in species_mask} n^_J(m)|^2 / N_mask on the half spectrum
+ * [Nx][Ny][Nz/2+1], with n^ the transform of the mesh (spread) density and N_mask the particles of the masked
+ * species.  Averaging over time is the caller's: accumulate, then divide by the number of samples. */
+int tild_structure_factor(tild_ctx*, uint32_t species_mask, float* sk /*DEVICE [Nx][Ny][Nz/2+1]*/, int32_t accumulate);
+
 /* a1: index map of arbitrary caller positions.  base[i][a] = first stencil node (unwrapped),
  * cell_key[i] = (cx*Ny+cy)*Nz+cz, perm = particle ids grouped by ascending cell key (order inside
  * a cell unspecified), cell_start[c] = #particles with key < c (M+1 entries).  Any output may be NULL. */

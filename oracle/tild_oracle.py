@@ -257,3 +257,15 @@ def energy(p: OracleParams, x, v, type_, partner) -> np.ndarray:
     lib().orc_energy(C.byref(cp), _ptr(x, C.c_double), _ptr(v, C.c_double), _ptr(type_, C.c_int32),
                      _ptr(partner, C.c_int32), _ptr(e, C.c_double))
     return e
+
+
+def structure_factor(p: OracleParams, x, type_, species=None) -> np.ndarray:
+    """S(m) = |rho^(m)|^2 / N of the mesh density of the chosen species (all when None), Eq. 23 L334 with
+    rho^ taken from the spread density (the mesh the force path works on): rho^(m) = sum_g n(g) exp(-2 pi i m.g/N).
+    Returned on the half spectrum [Nx][Ny][Nz/2+1] (the other half is its mirror image)."""
+    g = spread(p, x, type_)
+    sel = range(p.S) if species is None else list(species)
+    n = sum(g[J] for J in sel)
+    count = float(n.sum())
+    rho = dft3d(n.astype(np.complex128), -1)
+    return (np.abs(rho) ** 2 / count)[:, :, : int(p.N[2]) // 2 + 1]

@@ -578,6 +578,17 @@ int tild_energy(tild_ctx* c, double e[3])
     return TILD_OK;
 }
 
+int tild_structure_factor(tild_ctx* c, uint32_t species_mask, float* sk, int32_t accumulate)
+{
+    if (!c || !sk) return tild_fail(c, TILD_EINVAL, "tild_structure_factor: null argument");
+    if (!c->has_state) return tild_fail(c, TILD_ESTATE, "tild_structure_factor before tild_set_state");
+    if ((species_mask & ((1u << c->mesh.S) - 1u)) == 0) return tild_fail(c, TILD_EINVAL, "tild_structure_factor: empty species mask");
+    int rc = launch_spread(c, c->lay, c->X4[c->cur], c->grid);
+    if (rc) return rc;
+    TILD_FFT(c, cufftExecR2C(c->plan_r2c, c->grid, reinterpret_cast<cufftComplex*>(c->nhat)));
+    return launch_structure_factor(c, species_mask, sk, accumulate);
+}
+
 int tild_get_timings(tild_ctx* c, float ms[8], int32_t* steps_timed)
 {
     if (!c || !ms) return TILD_EINVAL;

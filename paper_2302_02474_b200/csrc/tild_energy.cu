@@ -1,4 +1,4 @@
-// Energies of the current state (diagnostic, not on the timed path).
+// Diagnostics of the current state (not on the timed path): energies and the structure factor.
 //   e[0] = kinetic  = m/2 sum |v|^2, v = w + (dt/2m) F (the split-kick state of DESIGN.md "GJF in one pass")
 //   e[1] = bonds    = sum_bonds k (|d| - r0)^2, each bond once (Eq. 2)
 //   e[2] = non-bonded on the mesh = (1/2V) sum_m u^(k_m) sum_IJ c_IJ Re[n^_I(m) conj(n^_J(m))] (Eq. 3-4 L119-123 with
@@ -73,7 +73,35 @@ __global__ void __launch_bounds__(256) particle_energy_kernel(MeshParams m, Step
     block_add(eb, out + 1);
 }
 
+// S(m) = |sum_{J in mask} n^_J(m)|^2 / N_mask on the half spectrum; N_mask = the m = 0 mode (Eq. 23)
+__global__ void __launch_bounds__(256) structure_factor_kernel(int S, uint32_t mask, size_t Mk, const float2* __restrict__ nhat,
+                                                               float* __restrict__ sk, int accumulate)
+{
+    float count = 0.f;
+    for (int J = 0; J < S; ++J)
+        if (mask >> J & 1u) count += nhat[(size_t)J * Mk].x;
+    const float inv = count > 0.f ? 1.0f / count : 0.f;
+    for (size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x; idx < Mk; idx += (size_t)gridDim.x * blockDim.x) {
+        float re = 0.f, im = 0.f;
+        for (int J = 0; J < S; ++J)
+            if (mask >> J & 1u) {
+                const float2 v = nhat[(size_t)J * Mk + idx];
+                re += v.x;
+                im += v.y;
+            }
+        const float v = (re * re + im * im) * inv;
+        sk[idx] = accumulate ? sk[idx] + v : v;
+    }
+}
+
 }  // namespace
+
+int launch_structure_factor(tild_ctx* c, uint32_t mask, float* sk, int accumulate)
+{
+    structure_factor_kernel<<<592, 256, 0, c->stream>>>(c->mesh.S, mask, c->Mk, c->nhat, sk, accumulate);
+    TILD_LAUNCH_CHECK(c, "structure_factor_kernel");
+    return TILD_OK;
+}
 
 // F4 must hold the total force at the current positions and c->nhat their transformed densities (force_current)
 int launch_energy(tild_ctx* c, double* d_out)

@@ -172,6 +172,7 @@ int launch_make_w(tild_ctx* c, const float4* F4, float4* W4, float sign);   // w
 int launch_velocity_out(tild_ctx* c, const float4* F4, const float4* W4, float* v);  // v[id] = w + (dt/2m) f
 int launch_advance_step(tild_ctx* c);
 int launch_energy(tild_ctx* c, double* d_out);   // tild_energy.cu
+int launch_structure_factor(tild_ctx* c, uint32_t mask, float* sk, int accumulate);  // c->nhat must be current
 int launch_philox_test(tild_ctx* c, const uint32_t* ctr, const uint32_t* key, uint32_t* out, float* gauss, int m);
 
 size_t tild_scan_scratch_entries(size_t nbins);

@@ -23,7 +23,7 @@ TIMING_NAMES = ("sort", "spread", "fft_fwd", "kspace", "fft_inv", "interp", "oth
 
 EXPORTS = (
     "tild_workspace_bytes", "tild_init", "tild_set_state", "tild_spread", "tild_kspace_force", "tild_interp",
-    "tild_bond_force", "tild_step", "tild_get_state", "tild_energy", "tild_index_map", "tild_get_timings", "tild_run_host",
+    "tild_bond_force", "tild_step", "tild_get_state", "tild_energy", "tild_structure_factor", "tild_index_map", "tild_get_timings", "tild_run_host",
     "tild_philox_test", "tild_layout_info", "tild_launch_count", "tild_last_error", "tild_destroy", "tild_version",
 )
 
@@ -100,6 +100,7 @@ def load():
     lib.tild_step.argtypes = [vp, i32]
     lib.tild_get_state.argtypes = [vp, vp, vp, vp, C.POINTER(u64)]
     lib.tild_energy.argtypes = [vp, C.POINTER(C.c_double * 3)]
+    lib.tild_structure_factor.argtypes = [vp, C.c_uint32, vp, i32]
     lib.tild_index_map.argtypes = [vp, vp, vp, vp, vp, vp]
     lib.tild_get_timings.argtypes = [vp, C.POINTER(C.c_float * 8), C.POINTER(i32)]
     lib.tild_run_host.argtypes = [vp, vp, vp, vp, vp, u64, i32]
@@ -230,6 +231,14 @@ class Tild:
         e = (C.c_double * 3)()
         self._check(self.lib.tild_energy(self.ctx, C.byref(e)), "tild_energy")
         return np.array([e[0], e[1], e[2]])
+
+    def tild_structure_factor(self, species_mask: int, sk=None):
+        """S(m) of the masked species on the half spectrum; pass a previous result as `sk` to accumulate into it."""
+        acc = sk is not None
+        if sk is None:
+            sk = self._empty(self.N[:2] + (self.N[2] // 2 + 1,), self.torch.float32)
+        self._check(self.lib.tild_structure_factor(self.ctx, int(species_mask), _dp(sk), 1 if acc else 0), "tild_structure_factor")
+        return sk
 
     def tild_get_timings(self):
         ms = (C.c_float * 8)()

@@ -532,3 +532,23 @@ def test_energy_matches_oracle(cfg):
     assert np.all(np.abs(e1 - o1) <= 2e-5 * np.abs(o1).max()), (e1, o1)
     x2 = eng.tild_get_state(want_v=False)[0]
     assert torch.equal(x, x2)                                        # tild_energy does not change the state
+
+
+def test_structure_factor_matches_oracle():
+    """tild_structure_factor (Eq. 23) of the state after a few steps, total and per species, and accumulation."""
+    cfg = small_cfg(order=3, S=3, grid=(18, 12, 30), box=(9.0, 6.0, 15.0))
+    st, eng = make(cfg)
+    p = oracle_params(cfg)
+    eng.tild_set_state(dev(st.x), dev(st.v), dev(st.type), dev(st.bond_partner), 0)
+    eng.tild_step(6)
+    x = eng.tild_get_state(want_v=False)[0].cpu().numpy()
+    for mask, species in ((0b111, None), (0b010, [1]), (0b101, [0, 2])):
+        sk = eng.tild_structure_factor(mask).cpu().numpy()
+        osk = orc.structure_factor(p, x, st.type, species)
+        assert sk.shape == osk.shape
+        assert np.abs(sk - osk).max() <= 2e-5 * osk.max(), (mask, np.abs(sk - osk).max(), osk.max())
+    acc = eng.tild_structure_factor(0b111)
+    acc = eng.tild_structure_factor(0b111, acc)
+    assert np.allclose(acc.cpu().numpy(), 2 * orc.structure_factor(p, x, st.type), rtol=1e-4, atol=1e-4 * cfg.n)
+    with pytest.raises(tild.TildError, match="empty species mask"):
+        eng.tild_structure_factor(0b1000)

@@ -281,3 +281,27 @@ def test_deconvolved_kernel_keeps_momentum_and_reduces_to_plain_at_k0():
     grid = np.ones((3,) + N)
     for params in (p, q):
         assert np.abs(orc.kspace_force(params, grid)).max() < 1e-12
+
+
+# ---- structure factor of the mesh density (Eq. 23) ---------------------------------------------
+def test_structure_factor_matches_particle_sum_times_assignment_transform():
+    """S_mesh(k) = |sum_g n(g) e^{-ik.g h}|^2 / N.  For |k| well below the mesh Nyquist the mesh density is the particle
+    density convolved with W, so S_mesh(k) = W^(k)^2 |sum_i e^{-ik.r_i}|^2 / N up to aliasing; S(0) = N."""
+    rng = np.random.default_rng(9)
+    L, N, P = (8.0, 6.0, 10.0), (16, 12, 20), 4
+    n = 300
+    x = (rng.random((n, 3)) * np.array(L)).astype(np.float32)
+    ty = rng.integers(0, 2, size=n).astype(np.int32)
+    p = orc.OracleParams(n, 2, L, N, P, np.zeros((2, 2)), kappa=1.0, sigma2=0.5)
+    S = orc.structure_factor(p, x, ty)
+    assert S.shape == (16, 12, 11)
+    assert abs(S[0, 0, 0] - n) < 1e-9 * n
+    xs = x.astype(np.float64)
+    for m in [(1, 0, 0), (0, 2, 0), (1, 1, 1), (2, 0, 3), (15, 11, 1)]:          # (15, 11, .) = (-1, -1, .)
+        mt = [mi if mi <= Ni // 2 else mi - Ni for mi, Ni in zip(m, N)]
+        k = 2 * np.pi * np.array(mt) / np.array(L)
+        direct = np.abs(np.exp(-1j * xs @ k).sum()) ** 2 / n
+        w2 = np.prod([np.sinc(mi / Ni) ** (2 * P) for mi, Ni in zip(mt, N)])    # np.sinc(x) = sin(pi x)/(pi x)
+        assert abs(S[m] - w2 * direct) < 2e-3 * max(1.0, direct), (m, S[m], w2 * direct)
+    A = orc.structure_factor(p, x, ty, species=[0])
+    assert abs(A[0, 0, 0] - (ty == 0).sum()) < 1e-9 * n
