@@ -56,6 +56,10 @@ typedef enum {
                                       small systems); ignored with TILD_FLAG_TIMING, an odd resort_every, or the
                                       legacy default stream (which cannot be captured) */
 
+/* integrators */
+#define TILD_INTEGRATOR_GJF 0   /* Gronbech-Jensen & Farago, one force evaluation per step */
+#define TILD_INTEGRATOR_EM 1    /* Euler-Maruyama: r' = r + (dt/gamma) F + sqrt(2 kT dt/gamma) xi; velocities unused */
+
 typedef struct tild_ctx tild_ctx;
 
 /* The model statement.  PAPER.md: box L54; grid Nx,Ny,Nz and pmeorder Listing 1 L69-78; species,
@@ -79,6 +83,8 @@ typedef struct {
     uint64_t seed;             /* Philox4x32-10 key (A12) */
     int32_t resort_every;      /* physically re-sort particles by cell every this many steps; <= 0 -> default */
     uint32_t flags;            /* TILD_FLAG_* */
+    int32_t integrator;        /* TILD_INTEGRATOR_GJF (default, A11) or TILD_INTEGRATOR_EM (overdamped, A11b; gamma > 0) */
+    int32_t reserved;          /* 0 */
 } tild_params;
 
 /* HOST. Bytes of device workspace tild_init needs for these parameters. */

@@ -49,6 +49,7 @@ typedef struct {
     int32_t max_bonds;
     double dt, gamma, kT, mass;
     uint64_t seed;
+    int32_t integrator; /* 0: GJF (A11); 1: Euler-Maruyama, overdamped */
     int32_t deconvolve; /* 0: kernel is u^(k) (A13); 1: u^(k) / W^(k)^2, W^ = prod_a sinc(k_a h_a / 2)^P */
 } orc_params;
 
@@ -606,10 +607,36 @@ void orc_gjf_step(const orc_params *p, double *x, double *v, double *f, const in
     free(fnew);
 }
 
+/* ------------------------------------------------------------------------------------------
+ * Euler-Maruyama step (PAPER.md L348-352 lists it next to GJF, "GJF ... time steps up to 10x larger than EM";
+ * equations not in the paper).  Reading A11b: the overdamped Langevin equation gamma dr = F dt + sqrt(2 gamma kT) dW
+ * discretised explicitly, with the same noise beta ~ N(0, 2 gamma kT dt) as GJF (same Philox counters):
+ *   r' = r + (dt/gamma) F + beta/gamma, wrapped;   F' = F(r').   Velocities are not used and are left unchanged.
+ * ---------------------------------------------------------------------------------------- */
+void orc_em_step(const orc_params *p, double *x, double *f, const int32_t *type, const int32_t *partner, uint64_t step)
+{
+    const size_t n3 = 3 * (size_t)p->n;
+    double *fnew = (double *)malloc(sizeof(double) * n3);
+    for (int i = 0; i < p->n; ++i) {
+        double beta[3];
+        orc_noise(p, (uint32_t)i, step + 1, beta);
+        for (int c = 0; c < 3; ++c) {
+            size_t q = 3 * (size_t)i + c;
+            x[q] = orc_wrap(x[q] + (p->dt / p->gamma) * f[q] + beta[c] / p->gamma, p->L[c]);
+        }
+    }
+    orc_force(p, x, type, partner, fnew);
+    memcpy(f, fnew, sizeof(double) * n3);
+    free(fnew);
+}
+
 void orc_run(const orc_params *p, double *x, double *v, double *f, const int32_t *type,
              const int32_t *partner, uint64_t step0, int32_t nsteps)
 {
-    for (int32_t s = 0; s < nsteps; ++s) orc_gjf_step(p, x, v, f, type, partner, step0 + (uint64_t)s);
+    for (int32_t s = 0; s < nsteps; ++s) {
+        if (p->integrator == 1) orc_em_step(p, x, f, type, partner, step0 + (uint64_t)s);
+        else orc_gjf_step(p, x, v, f, type, partner, step0 + (uint64_t)s);
+    }
 }
 
 /* ------------------------------------------------------------------------------------------

@@ -41,6 +41,7 @@ class _Params(C.Structure):
         ("max_bonds", C.c_int32),
         ("dt", C.c_double), ("gamma", C.c_double), ("kT", C.c_double), ("mass", C.c_double),
         ("seed", C.c_uint64),
+        ("integrator", C.c_int32),
         ("deconvolve", C.c_int32),
     ]
 
@@ -65,6 +66,7 @@ class OracleParams:
     kT: float = 1.0
     mass: float = 1.0
     seed: int = 0
+    integrator: int = 0        # 0 GJF (A11), 1 Euler-Maruyama (A11b)
     deconvolve: bool = False   # divide the pair kernel by W^(k)^2; default: plain u^(k) (A13)
     _c: _Params = field(default=None, repr=False)
 
@@ -85,6 +87,7 @@ class OracleParams:
         p.k_bond, p.r0_bond, p.max_bonds = float(self.k_bond), float(self.r0_bond), int(self.max_bonds)
         p.dt, p.gamma, p.kT, p.mass = float(self.dt), float(self.gamma), float(self.kT), float(self.mass)
         p.seed = int(self.seed)
+        p.integrator = int(self.integrator)
         p.deconvolve = 1 if self.deconvolve else 0
         return p
 

@@ -54,6 +54,8 @@ int validate(const tild_params* p)
     if (M > 2.0e9) return TILD_EINVAL;
     if (!(p->sigma2 > 0.0) && !(p->a > 0.0)) return TILD_EINVAL;
     if (!(p->dt > 0.0) || !(p->mass > 0.0) || p->gamma < 0.0 || p->kT < 0.0) return TILD_EINVAL;
+    if (p->integrator != TILD_INTEGRATOR_GJF && p->integrator != TILD_INTEGRATOR_EM) return TILD_EINVAL;
+    if (p->integrator == TILD_INTEGRATOR_EM && !(p->gamma > 0.0)) return TILD_EINVAL;
     return TILD_OK;
 }
 
@@ -296,6 +298,9 @@ int tild_init(tild_ctx** out, const tild_params* params, void* workspace, size_t
     s.k_bond = (float)p.k_bond;
     s.r0_bond = (float)p.r0_bond;
     s.max_bonds = p.max_bonds;
+    s.integrator = p.integrator;
+    s.em_drift = p.gamma > 0.0 ? (float)(p.dt / p.gamma) : 0.0f;
+    s.em_noise = p.gamma > 0.0 ? (float)(1.0 / p.gamma) : 0.0f;
     s.key0 = (uint32_t)(p.seed & 0xffffffffu);
     s.key1 = (uint32_t)(p.seed >> 32);
 

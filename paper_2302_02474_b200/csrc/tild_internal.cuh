@@ -66,6 +66,9 @@ struct StepParams {
     float k_bond, r0_bond;
     int max_bonds;
     uint32_t key0, key1;   // Philox key = seed lo, hi
+    int integrator;        // TILD_INTEGRATOR_*
+    float em_drift;        // dt/gamma
+    float em_noise;        // 1/gamma (times beta = noise_amp * z)
 };
 
 // ---- context -----------------------------------------------------------------------------------

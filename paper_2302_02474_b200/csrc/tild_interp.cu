@@ -140,6 +140,13 @@ __device__ __forceinline__ void finish_update(const MeshParams& m, const StepPar
         const float3 z = gauss3(__float_as_uint(w0.w), step_next, s.key0, s.key1);
         beta = make_float3(s.noise_amp * z.x, s.noise_amp * z.y, s.noise_amp * z.z);
     }
+    if (s.integrator == TILD_INTEGRATOR_EM) {   // r' = r + (dt/gamma) F + beta/gamma; velocities are not used (A11b)
+        X4o[slot] = make_float4(wrap_pos(p.x + (s.em_drift * F.x + s.em_noise * beta.x), m.L[0], m.inv_L[0]),
+                                wrap_pos(p.y + (s.em_drift * F.y + s.em_noise * beta.y), m.L[1], m.inv_L[1]),
+                                wrap_pos(p.z + (s.em_drift * F.z + s.em_noise * beta.z), m.L[2], m.inv_L[2]), p.w);
+        W4o[slot] = w0;
+        return;
+    }
     const float pp[3] = {p.x, p.y, p.z};
     const float wv[3] = {w0.x, w0.y, w0.z};
     const float Fv[3] = {F.x, F.y, F.z};

@@ -18,6 +18,7 @@ MAX_SPECIES = 8
 MAX_BONDS = 4
 
 OK, EINVAL, ENOMEM, ECUDA, ECUFFT, ESTATE = 0, -1, -2, -3, -4, -5
+INTEGRATOR_GJF, INTEGRATOR_EM = 0, 1
 FLAG_TIMING, FLAG_NAIVE_SPREAD, FLAG_NAIVE_INTERP, FLAG_GRAPH, FLAG_DECONVOLVE = 1, 2, 4, 8, 16
 TIMING_NAMES = ("sort", "spread", "fft_fwd", "kspace", "fft_inv", "interp", "other", "total")
 
@@ -40,13 +41,14 @@ class Params(C.Structure):
         ("dt", C.c_double), ("gamma", C.c_double), ("kT", C.c_double), ("mass", C.c_double),
         ("seed", C.c_uint64),
         ("resort_every", C.c_int32), ("flags", C.c_uint32),
+        ("integrator", C.c_int32), ("reserved", C.c_int32),
     ]
 
 
 def make_params(n: int, n_species: int, box: Sequence[float], grid: Sequence[int], order: int, chi, kappa: float,
                 a: float = 0.5, sigma2: float = 0.0, rho0: float = 0.0, k_bond: float = 1.5, r0_bond: float = 0.0,
                 max_bonds: int = 2, dt: float = 0.005, gamma: float = 1.0, kT: float = 1.0, mass: float = 1.0,
-                seed: int = 0, resort_every: int = 0, flags: int = 0) -> Params:
+                seed: int = 0, resort_every: int = 0, flags: int = 0, integrator: int = 0) -> Params:
     p = Params()
     p.struct_size = C.sizeof(Params)
     p.n, p.n_species, p.order = int(n), int(n_species), int(order)
@@ -63,6 +65,7 @@ def make_params(n: int, n_species: int, box: Sequence[float], grid: Sequence[int
     p.dt, p.gamma, p.kT, p.mass = float(dt), float(gamma), float(kT), float(mass)
     p.seed = int(seed)
     p.resort_every, p.flags = int(resort_every), int(flags)
+    p.integrator, p.reserved = int(integrator), 0
     return p
 
 

@@ -552,3 +552,26 @@ def test_structure_factor_matches_oracle():
     assert np.allclose(acc.cpu().numpy(), 2 * orc.structure_factor(p, x, st.type), rtol=1e-4, atol=1e-4 * cfg.n)
     with pytest.raises(tild.TildError, match="empty species mask"):
         eng.tild_structure_factor(0b1000)
+
+
+@pytest.mark.parametrize("cfg", [small_cfg(order=4), inputs.C1], ids=["P4", "C1"])
+def test_euler_maruyama_trajectory_parity(cfg):
+    """TILD_INTEGRATOR_EM (SURVEY 8(f) #3, reading A11b) against the oracle's orc_em_step: same Philox stream."""
+    st = inputs.make_state(cfg)
+    eng = tild.Tild(tild.params_from_config(cfg, resort_every=6, integrator=tild.INTEGRATOR_EM))
+    p = oracle_params(cfg, integrator=1)
+    eng.tild_set_state(dev(st.x), dev(st.v), dev(st.type), dev(st.bond_partner), 0)
+    eng.tild_step(60)
+    x, _, f, step = eng.tild_get_state(want_v=False, want_f=True)
+    assert step == 60
+    ox, _, of = orc.run(p, st.x.astype(np.float64), st.v.astype(np.float64), st.type, st.bond_partner, 0, 60)
+    assert np.abs(min_image(x.cpu().numpy().astype(np.float64) - ox, cfg.box)).max() <= 1e-4
+    # the two integrators really differ
+    gx, _, _ = orc.run(oracle_params(cfg), st.x.astype(np.float64), st.v.astype(np.float64), st.type, st.bond_partner, 0, 60)
+    assert np.abs(min_image(gx - ox, cfg.box)).max() > 1e-2
+
+
+def test_euler_maruyama_needs_friction():
+    cfg = small_cfg(order=2, gamma=0.0)
+    with pytest.raises(tild.TildError):
+        tild.Tild(tild.params_from_config(cfg, integrator=tild.INTEGRATOR_EM))

@@ -201,3 +201,56 @@ def test_philox_matches_curand_header(curand_host):
         ref = np.zeros(4, np.uint32)
         curand_host.curand_philox_host(ctr.ctypes.data_as(U), key.ctypes.data_as(U), ref.ctypes.data_as(U))
         assert np.array_equal(orc.philox4x32_10(ctr, key), ref)
+
+
+# ---- Euler-Maruyama (reading A11b) --------------------------------------------------------------------
+def test_em_one_step_is_the_explicit_formula_with_the_gjf_noise():
+    """r' = r + (dt/gamma) F + beta/gamma with beta the SAME noise GJF would draw for (id, step + 1); v untouched."""
+    rng = np.random.default_rng(4)
+    n, L = 40, (6.0, 5.0, 7.0)
+    x = rng.random((n, 3)) * np.array(L)
+    v = rng.normal(size=(n, 3))
+    ty = rng.integers(0, 2, size=n).astype(np.int32)
+    bp = -np.ones((n, 2), np.int32)
+    bp[1:, 0] = np.arange(n - 1)
+    bp[:-1, 1] = np.arange(1, n)
+    p = orc.OracleParams(n, 2, L, (12, 10, 14), 3, np.array([[0, 1.0], [1.0, 0]]), 5.0, 0.5, gamma=2.0, dt=0.01, seed=7,
+                         integrator=1)
+    f0 = orc.force(p, x.astype(np.float32).astype(np.float64), ty, bp)
+    x0 = x.astype(np.float32).astype(np.float64)
+    x1, v1, f1 = orc.run(p, x0, v, ty, bp, 11, 1)
+    beta = np.array([orc.noise(p, i, 12) for i in range(n)])
+    want = x0 + (p.dt / p.gamma) * f0 + beta / p.gamma
+    want -= np.array(L) * np.floor(want / np.array(L))
+    assert np.abs(x1 - want).max() < 1e-12
+    assert np.array_equal(v1, v)
+    assert np.abs(f1 - orc.force(p, x1, ty, bp)).max() < 1e-12
+
+
+def test_em_free_diffusion_and_dimer_stationary_variance():
+    """No forces: every step adds N(0, 2 kT dt/gamma) per component, so <dr^2> = 6 (kT/gamma) t exactly in expectation.
+    Harmonic dimer U = k d^2: the relative coordinate obeys d' = (1 - 4 k dt/gamma) d + noise of variance 4 kT dt/gamma,
+    whose stationary variance per component is (4 kT dt/gamma) / (1 - (1 - 4 k dt/gamma)^2) (the finite-dt EM bias)."""
+    n = 4000
+    rng = np.random.default_rng(12)
+    L = 1000.0
+    x = np.full((n, 3), 500.0) + rng.random((n, 3))
+    ty = np.zeros(n, np.int32)
+    gamma, dt, nst = 2.0, 0.01, 100
+    p = orc.OracleParams(n, 1, (L,) * 3, (4,) * 3, 1, np.zeros((1, 1)), 0.0, 0.5, k_bond=0.0, gamma=gamma, dt=dt, seed=3,
+                         integrator=1)
+    x1, _, _ = orc.run(p, x, np.zeros_like(x), ty, -np.ones((n, 2), np.int32), 0, nst)
+    msd = ((x1 - x) ** 2).sum(1).mean()
+    assert abs(msd / (6 * dt * nst / gamma) - 1) < 0.04, msd
+    nd, k = 2000, 1.5
+    c = rng.random((nd, 1, 3)) * 900 + 50
+    xd = (c + rng.normal(0, 0.4, size=(nd, 2, 3))).reshape(-1, 3)
+    bp = np.stack([np.arange(2 * nd) ^ 1, -np.ones(2 * nd, int)], axis=1).astype(np.int32)
+    dt = 0.02
+    q = orc.OracleParams(2 * nd, 1, (L,) * 3, (4,) * 3, 1, np.zeros((1, 1)), 0.0, 0.5, k_bond=k, gamma=gamma, dt=dt, seed=8,
+                         integrator=1)
+    xe, _, _ = orc.run(q, xd, np.zeros_like(xd), np.zeros(2 * nd, np.int32), bp, 0, 400)
+    d = (xe[0::2] - xe[1::2])
+    a = 1 - 4 * k * dt / gamma
+    var = (4 * dt / gamma) / (1 - a * a)
+    assert abs((d ** 2).mean() / var - 1) < 0.05, ((d ** 2).mean(), var)
