@@ -52,6 +52,8 @@ typedef enum {
 #define TILD_FLAG_NAIVE_INTERP 4u  /* per-particle global-gather interpolation (baseline kernel) */
 #define TILD_FLAG_DECONVOLVE 16u   /* pair kernel u^(k) / W^(k)^2, W^ = prod_a sinc(k_a h_a/2)^P: undoes the smoothing of the
                                       order-P assignment (A13; default off: the kernel is exactly u^(k)) */
+#define TILD_FLAG_SAMPLED_KERNEL 32u /* pair kernel = DFT of u_G sampled on the mesh (minimum image), as PAPER.md L223
+                                      describes, instead of the analytic u^(k) (A5b); still three 1-D tables */
 #define TILD_FLAG_GRAPH 8u         /* tild_step replays blocks of 2*resort_every steps as one CUDA graph (launch-bound
                                       small systems); ignored with TILD_FLAG_TIMING, an odd resort_every, or the
                                       legacy default stream (which cannot be captured) */

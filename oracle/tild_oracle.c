@@ -50,6 +50,7 @@ typedef struct {
     double dt, gamma, kT, mass;
     uint64_t seed;
     int32_t integrator; /* 0: GJF (A11); 1: Euler-Maruyama, overdamped */
+    int32_t sampled_kernel; /* 0: analytic u^(k) (A5); 1: FFT of u_G sampled on the mesh, as PAPER.md L223 describes (A5b) */
     int32_t deconvolve; /* 0: kernel is u^(k) (A13); 1: u^(k) / W^(k)^2, W^ = prod_a sinc(k_a h_a / 2)^P */
 } orc_params;
 
@@ -364,6 +365,60 @@ static double orc_uhat(const orc_params *p, int mx, int my, int mz)
     return exp(-0.5 * p->sigma2 * k2) / w2;
 }
 
+/* "a Fourier-space representation of the inter-particle potential is calculated using Fast Fourier
+ * Transform (FFT), and is stored".  Reading A5b: u_G(r) = (2 pi sigma2)^(-3/2) exp(-r^2 / 2 sigma2) (L121) is sampled at the
+ * mesh nodes with the minimum-image distance, and u^_s(m) = dV sum_g u_G(r_g) exp(-2 pi i m.g/N) (real: u_G is even).
+ * Returns a malloc'ed [Nx][Ny][Nz] table of u^_s (times 1/W^2 when deconvolve is set), or NULL when the analytic
+ * kernel is in use. */
+static double *orc_sampled_uhat(const orc_params *p)
+{
+    if (!p->sampled_kernel) return NULL;
+    const size_t M = (size_t)p->N[0] * p->N[1] * p->N[2];
+    const double dV = (p->L[0] / p->N[0]) * (p->L[1] / p->N[1]) * (p->L[2] / p->N[2]);
+    const double norm = pow(2.0 * ORC_PI * p->sigma2, -1.5);
+    double *u = (double *)malloc(sizeof(double) * 2 * M);
+    for (int gx = 0; gx < p->N[0]; ++gx)
+        for (int gy = 0; gy < p->N[1]; ++gy)
+            for (int gz = 0; gz < p->N[2]; ++gz) {
+                const int g[3] = {gx, gy, gz};
+                double r2 = 0.0;
+                for (int a = 0; a < 3; ++a) {
+                    double d = g[a] * p->L[a] / p->N[a];
+                    if (d > 0.5 * p->L[a]) d -= p->L[a];      /* minimum image */
+                    r2 += d * d;
+                }
+                const size_t q = ((size_t)gx * p->N[1] + gy) * p->N[2] + gz;
+                u[2 * q] = dV * norm * exp(-0.5 * r2 / p->sigma2);
+                u[2 * q + 1] = 0.0;
+            }
+    orc_dft3d(p->N, u, -1);
+    double *t = (double *)malloc(sizeof(double) * M);
+    for (int mx = 0; mx < p->N[0]; ++mx)
+        for (int my = 0; my < p->N[1]; ++my)
+            for (int mz = 0; mz < p->N[2]; ++mz) {
+                const size_t q = ((size_t)mx * p->N[1] + my) * p->N[2] + mz;
+                /* orc_uhat(...) / exp(...) is the deconvolution factor alone (1 when it is off) */
+                const double kx = orc_k(p, 0, mx), ky = orc_k(p, 1, my), kz = orc_k(p, 2, mz);
+                const double dec = orc_uhat(p, mx, my, mz) / exp(-0.5 * p->sigma2 * (kx * kx + ky * ky + kz * kz));
+                t[q] = u[2 * q] * (p->deconvolve ? dec : 1.0);
+            }
+    free(u);
+    return t;
+}
+
+/* The pair kernel the k-space stage multiplies with, as a table [Nx][Ny][Nz] (for the pins). */
+void orc_uhat_table(const orc_params *p, double *out)
+{
+    double *t = orc_sampled_uhat(p);
+    for (int mx = 0; mx < p->N[0]; ++mx)
+        for (int my = 0; my < p->N[1]; ++my)
+            for (int mz = 0; mz < p->N[2]; ++mz) {
+                const size_t q = ((size_t)mx * p->N[1] + my) * p->N[2] + mz;
+                out[q] = t ? t[q] : orc_uhat(p, mx, my, mz);
+            }
+    free(t);
+}
+
 /* ------------------------------------------------------------------------------------------
  * O4-O6 k-space force.  PAPER.md Eq. 18, "becomes a simple multiplication" L227:
  *   n^_J(m)   = sum_g n_J(g) exp(-2 pi i m.g/N)
@@ -386,6 +441,7 @@ void orc_kspace_force(const orc_params *p, const double *grid, double *ffield)
         }
         orc_dft3d(p->N, d, -1);
     }
+    double *utab = orc_sampled_uhat(p);
     for (int I = 0; I < S; ++I) {
         for (int a = 0; a < 3; ++a) {
 #pragma omp parallel for schedule(static)
@@ -394,7 +450,7 @@ void orc_kspace_force(const orc_params *p, const double *grid, double *ffield)
                     for (int mz = 0; mz < p->N[2]; ++mz) {
                         size_t g = ((size_t)mx * p->N[1] + my) * p->N[2] + mz;
                         double kx = orc_k(p, 0, mx), ky = orc_k(p, 1, my), kz = orc_k(p, 2, mz);
-                        double uhat = orc_uhat(p, mx, my, mz);
+                        double uhat = utab ? utab[g] : orc_uhat(p, mx, my, mz);
                         (void)kx; (void)ky; (void)kz;
                         int m_a = a == 0 ? mx : (a == 1 ? my : mz);
                         double kg = orc_kgrad(p, a, m_a);
@@ -416,6 +472,7 @@ void orc_kspace_force(const orc_params *p, const double *grid, double *ffield)
             for (size_t g = 0; g < M; ++g) out[g] = work[2 * g];
         }
     }
+    free(utab);
     free(nhat);
     free(work);
 }
@@ -678,12 +735,13 @@ void orc_energy(const orc_params *p, const double *x, const double *v, const int
         }
         orc_dft3d(p->N, d, -1);
     }
+    double *utab_e = orc_sampled_uhat(p);
     for (int mx = 0; mx < p->N[0]; ++mx)
         for (int my = 0; my < p->N[1]; ++my)
             for (int mz = 0; mz < p->N[2]; ++mz) {
                 size_t g = ((size_t)mx * p->N[1] + my) * p->N[2] + mz;
                 double kx = orc_k(p, 0, mx), ky = orc_k(p, 1, my), kz = orc_k(p, 2, mz);
-                double uhat = orc_uhat(p, mx, my, mz);
+                double uhat = utab_e ? utab_e[g] : orc_uhat(p, mx, my, mz);
                 (void)kx; (void)ky; (void)kz;
                 double acc = 0.0;
                 for (int I = 0; I < S; ++I)
@@ -696,6 +754,7 @@ void orc_energy(const orc_params *p, const double *x, const double *v, const int
     nb *= 0.5 / V;
     free(xf);
     free(grid);
+    free(utab_e);
     free(nhat);
     e[0] = ke;
     e[1] = be;

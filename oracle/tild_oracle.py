@@ -42,6 +42,7 @@ class _Params(C.Structure):
         ("dt", C.c_double), ("gamma", C.c_double), ("kT", C.c_double), ("mass", C.c_double),
         ("seed", C.c_uint64),
         ("integrator", C.c_int32),
+        ("sampled_kernel", C.c_int32),
         ("deconvolve", C.c_int32),
     ]
 
@@ -67,6 +68,7 @@ class OracleParams:
     mass: float = 1.0
     seed: int = 0
     integrator: int = 0        # 0 GJF (A11), 1 Euler-Maruyama (A11b)
+    sampled_kernel: bool = False  # u^ from the FFT of u_G sampled on the mesh (A5b) instead of analytic (A5)
     deconvolve: bool = False   # divide the pair kernel by W^(k)^2; default: plain u^(k) (A13)
     _c: _Params = field(default=None, repr=False)
 
@@ -88,6 +90,7 @@ class OracleParams:
         p.dt, p.gamma, p.kT, p.mass = float(self.dt), float(self.gamma), float(self.kT), float(self.mass)
         p.seed = int(self.seed)
         p.integrator = int(self.integrator)
+        p.sampled_kernel = 1 if self.sampled_kernel else 0
         p.deconvolve = 1 if self.deconvolve else 0
         return p
 
@@ -178,6 +181,14 @@ def dft1d(a, sign: int) -> np.ndarray:
     out = np.zeros_like(a)
     lib().orc_dft1d(C.c_int(a.shape[0]), C.c_int(1), _ptr(a.view(np.float64), C.c_double),
                     _ptr(out.view(np.float64), C.c_double), C.c_int(sign))
+    return out
+
+
+def uhat_table(p: OracleParams) -> np.ndarray:
+    """The pair kernel u^(m) of the k-space stage on the full spectrum [Nx][Ny][Nz] (analytic or sampled, deconvolved or not)."""
+    out = np.zeros(tuple(int(v) for v in p.N), dtype=np.float64)
+    cp = p.c()
+    lib().orc_uhat_table(C.byref(cp), _ptr(out, C.c_double))
     return out
 
 

@@ -260,6 +260,18 @@ int tild_init(tild_ctx** out, const tild_params* params, void* workspace, size_t
             const double k = 2.0 * PI * (double)mt / p.box[a];
             const double kg = (N % 2 == 0 && mm == N / 2) ? 0.0 : k;
             double u = exp(-0.5 * sigma2 * k * k);
+            if (p.flags & TILD_FLAG_SAMPLED_KERNEL) {
+                // A5b: u_G sampled at the nodes with the minimum-image distance is a product of three 1-D Gaussians, so
+                // its 3-D DFT is the product of three 1-D DFTs: u_a(m) = h sum_g g1(d_g) cos(2 pi m g / N)
+                const double h = p.box[a] / (double)N;
+                u = 0.0;
+                for (int g = 0; g < N; ++g) {
+                    double d = g * h;
+                    if (d > 0.5 * p.box[a]) d -= p.box[a];
+                    u += exp(-0.5 * d * d / sigma2) * cos(2.0 * PI * (double)mm * (double)g / (double)N);
+                }
+                u *= h / sqrt(2.0 * PI * sigma2);
+            }
             if (p.flags & TILD_FLAG_DECONVOLVE) {   // separable: [sinc(k h / 2)]^(-2P) per axis
                 const double xh = 0.5 * k * p.box[a] / (double)N;
                 const double sinc = xh == 0.0 ? 1.0 : sin(xh) / xh;

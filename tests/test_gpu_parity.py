@@ -575,3 +575,23 @@ def test_euler_maruyama_needs_friction():
     cfg = small_cfg(order=2, gamma=0.0)
     with pytest.raises(tild.TildError):
         tild.Tild(tild.params_from_config(cfg, integrator=tild.INTEGRATOR_EM))
+
+
+@pytest.mark.parametrize("deconv", [False, True])
+def test_sampled_kernel_parity(deconv):
+    """TILD_FLAG_SAMPLED_KERNEL (reading A5b): the library's separable 1-D tables against the oracle's
+    3-D DFT of the sampled Gaussian, alone and combined with the deconvolution."""
+    cfg = small_cfg(order=3, S=3, grid=(18, 12, 30), box=(9.0, 6.0, 15.0))
+    flags = tild.FLAG_SAMPLED_KERNEL | (tild.FLAG_DECONVOLVE if deconv else 0)
+    st, eng = make(cfg, flags=flags)
+    p = oracle_params(cfg, sampled_kernel=True, deconvolve=deconv)
+    og32 = orc.spread(p, st.x, st.type).astype(np.float32)
+    ff = eng.tild_kspace_force(dev(og32)).cpu().numpy()
+    off = orc.kspace_force(p, og32.astype(np.float64))
+    assert np.abs(ff - off).max() <= REL * rms(off)
+    ana = orc.kspace_force(oracle_params(cfg, deconvolve=deconv), og32.astype(np.float64))
+    assert np.abs(off - ana).max() > 1e-4 * rms(ana)                  # not the analytic kernel
+    eng.tild_set_state(dev(st.x), dev(st.v), dev(st.type), dev(st.bond_partner), 0)
+    e = eng.tild_energy()
+    oe = orc.energy(p, st.x.astype(np.float64), st.v.astype(np.float64), st.type, st.bond_partner)
+    assert np.all(np.abs(e - oe) <= 2e-5 * np.abs(oe).max())

@@ -305,3 +305,42 @@ def test_structure_factor_matches_particle_sum_times_assignment_transform():
         assert abs(S[m] - w2 * direct) < 2e-3 * max(1.0, direct), (m, S[m], w2 * direct)
     A = orc.structure_factor(p, x, ty, species=[0])
     assert abs(A[0, 0, 0] - (ty == 0).sum()) < 1e-9 * n
+
+
+# ---- pair kernel from the FFT of the sampled real-space potential (reading A5b) -------
+def test_sampled_kernel_is_the_aliased_sum_of_the_analytic_one():
+    """Sampling u_G on the mesh and transforming gives, by Poisson summation, u^_s(m) = sum_G u^(k_m + G) over the mesh's
+    reciprocal vectors G = 2 pi N_a j_a / L_a (box >> sigma, so periodic images of u_G are negligible); it tends to the
+    analytic u^ where that has decayed at the mesh Nyquist, and u^_s(0) -> 1 (u_G is a unit Gaussian, L121)."""
+    L, N, sigma2 = (10.0, 8.0, 12.0), (16, 12, 20), 0.5
+    p = orc.OracleParams(1, 1, L, N, 2, np.zeros((1, 1)), 1.0, sigma2, sampled_kernel=True)
+    t = orc.uhat_table(p)
+    ana = orc.uhat_table(orc.OracleParams(1, 1, L, N, 2, np.zeros((1, 1)), 1.0, sigma2))
+    for m in [(0, 0, 0), (1, 0, 0), (3, 2, 5), (8, 6, 10), (15, 11, 19), (7, 0, 1)]:
+        mt = [mi if mi <= Ni // 2 else mi - Ni for mi, Ni in zip(m, N)]
+        tot = 0.0
+        for jx in range(-3, 4):
+            for jy in range(-3, 4):
+                for jz in range(-3, 4):
+                    k = 2 * np.pi * (np.array(mt) + np.array(N) * np.array([jx, jy, jz])) / np.array(L)
+                    tot += np.exp(-0.5 * sigma2 * (k ** 2).sum())
+        assert abs(t[m] - tot) < 2e-7, (m, t[m], tot)      # the truncated tails of u_G beyond L/2 (5.7 sigma) are ~4e-8
+    assert abs(t[0, 0, 0] - 1.0) < 1e-6
+    assert 1e-6 < np.abs(t - ana).max() < 1e-2                               # h ~ 0.6 = 0.9 sigma: visible aliasing (4e-3)
+    fine = orc.uhat_table(orc.OracleParams(1, 1, L, (40, 32, 48), 2, np.zeros((1, 1)), 1.0, sigma2, sampled_kernel=True))
+    fana = orc.uhat_table(orc.OracleParams(1, 1, L, (40, 32, 48), 2, np.zeros((1, 1)), 1.0, sigma2))
+    assert np.abs(fine - fana).max() < 1e-7                                  # h = 0.25: they coincide up to the truncated tails
+
+
+def test_sampled_kernel_force_is_consistent():
+    rng = np.random.default_rng(3)
+    L, N = (6.0, 4.5, 7.0), (12, 8, 10)
+    n = 120
+    x = (rng.random((n, 3)) * np.array(L)).astype(np.float32)
+    ty = rng.integers(0, 3, size=n).astype(np.int32)
+    p = orc.OracleParams(n, 3, L, N, 3, CHI3, kappa=5.0, sigma2=0.5, rho0=2.0, sampled_kernel=True)
+    q = orc.OracleParams(n, 3, L, N, 3, CHI3, kappa=5.0, sigma2=0.5, rho0=2.0)
+    F, G = orc.nonbonded_force(p, x, ty), orc.nonbonded_force(q, x, ty)
+    assert np.abs(F.sum(0)).max() < 1e-10 * np.abs(F).max() * n               # still momentum conserving
+    rel = np.abs(F - G).max() / np.abs(G).max()
+    assert 1e-5 < rel < 0.1, rel                                              # close to, but not, the analytic kernel
