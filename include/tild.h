@@ -71,7 +71,7 @@ typedef struct {
     uint32_t struct_size;      /* = sizeof(tild_params) */
     int32_t n;                 /* particles, >= 0 */
     int32_t n_species;         /* S, 1..TILD_MAX_SPECIES */
-    int32_t order;             /* P = grid nodes touched per dimension, 1..4 (A1: P=2 is the paper's Fig. 1) */
+    int32_t order;             /* P = grid nodes touched per dimension, 1..5 (A1: P = 2..5 are the paper's orders 1..4) */
     double box[3];             /* L > 0 */
     int32_t grid[3];           /* N >= P, each; any size cuFFT accepts (2,3,5,7 factors are fast) */
     int32_t max_bonds;         /* bond partner slots per particle, 0..TILD_MAX_BONDS */

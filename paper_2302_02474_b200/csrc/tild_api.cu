@@ -44,7 +44,7 @@ int validate(const tild_params* p)
 {
     if (!p || p->struct_size != sizeof(tild_params)) return TILD_EINVAL;
     if (p->n < 0 || p->n_species < 1 || p->n_species > TILD_MAX_SPECIES) return TILD_EINVAL;
-    if (p->order < 1 || p->order > 4) return TILD_EINVAL;
+    if (p->order < 1 || p->order > 5) return TILD_EINVAL;
     if (p->max_bonds < 0 || p->max_bonds > TILD_MAX_BONDS) return TILD_EINVAL;
     double M = 1.0;
     for (int a = 0; a < 3; ++a) {
@@ -71,8 +71,8 @@ void configure_tiles(tild_ctx* c)
         const char* e = getenv(name);
         return e ? atoi(e) : dflt;
     };
-    t.H = p.order >= 3 ? 3 : 1;
-    t.lo = p.order >= 3 ? 1 : 0;
+    t.H = p.order <= 2 ? 1 : (p.order <= 4 ? 3 : 5);
+    t.lo = p.order <= 2 ? 0 : (p.order <= 4 ? 1 : 2);
     t.sh = t.lo ? 4 - t.lo : 0;   // image starts on a 16-byte boundary of the mesh rows (16-byte cp.async staging)
     t.enabled = p.grid[0] >= 8 && p.grid[1] >= 8 && p.grid[2] >= 8;
     int tx = env_int("TILD_TILE_X", 8), ty = env_int("TILD_TILE_Y", 16), tz = env_int("TILD_TILE_Z", p.grid[2] >= 32 ? 32 : 16);

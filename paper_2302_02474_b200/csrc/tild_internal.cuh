@@ -29,9 +29,9 @@ struct TileParams {
     int T[3];       // tile edge in cells (clipped to the grid)
     int nt[3];      // tiles per axis = ceil(N/T)
     int E[3];       // shared image edge in nodes: E[0] = T[0] + H, E[1] = T[1] + H (<= template EY), E[2] = EZ
-    int lo;         // nodes below the tile's first cell that a stencil can touch (0 for P <= 2, 1 for P = 3, 4)
+    int lo;         // nodes below the tile's first cell that a stencil can touch (0 for P <= 2, 1 for P = 3, 4, 2 for P = 5)
     int sh;         // extra nodes below those so that the image starts on a 16-byte boundary of the mesh rows
-    int H;          // stencil halo in nodes (1 for P <= 2, 3 for P = 3, 4)
+    int H;          // stencil halo in nodes (1 for P <= 2, 3 for P = 3, 4, 5 for P = 5)
     int EY, EZ;     // template strides the kernels were instantiated with
     int ntiles;
     int nseg;       // ntiles * S
@@ -230,7 +230,7 @@ __device__ __forceinline__ void weights_1d(float t, float* w)
         w[0] = 0.5f * a * a;
         w[1] = 0.75f - t * t;
         w[2] = 0.5f * b * b;
-    } else {
+    } else if (P == 4) {
         const float a = 1.0f - 2.0f * t, b = 1.0f + 2.0f * t;
         const float t2 = t * t;
         w[0] = a * a * a * (1.0f / 48.0f);
@@ -238,8 +238,24 @@ __device__ __forceinline__ void weights_1d(float t, float* w)
         const float even = 23.0f - 12.0f * t2, odd = t * (24.0f * t2 - 30.0f);
         w[1] = (even + odd) * (1.0f / 48.0f);
         w[2] = (even - odd) * (1.0f / 48.0f);
+    } else {   // P = 5 (the paper's "order 4", A1): quartic B-spline
+        const float a = 1.0f - 2.0f * t, b = 1.0f + 2.0f * t;
+        const float t2 = t * t, a2 = a * a, b2 = b * b;
+        w[0] = a2 * a2 * (1.0f / 384.0f);
+        w[4] = b2 * b2 * (1.0f / 384.0f);
+        const float even = 19.0f + t2 * (24.0f - 16.0f * t2), odd = t * (16.0f * t2 - 44.0f);
+        w[1] = (even + odd) * (1.0f / 96.0f);
+        w[3] = (even - odd) * (1.0f / 96.0f);
+        w[2] = (115.0f + t2 * (48.0f * t2 - 120.0f)) * (1.0f / 192.0f);
     }
 }
+
+// stencil halo of order P relative to the particle's cell: nodes [cell - LO, cell - LO + H + 1)
+template <int P> struct Halo {
+    static constexpr int H = P <= 2 ? 1 : (P <= 4 ? 3 : 5);     // extra nodes a tile image needs per axis
+    static constexpr int LO = P <= 2 ? 0 : (P <= 4 ? 1 : 2);    // of which below the tile's first cell
+    static constexpr int EZA = P <= 2 ? 20 : 24, EZB = P <= 2 ? 36 : 40;   // image z extent for TZ = 16 / 32 (% 4 == 0)
+};
 
 // Philox4x32-10 (Salmon et al., SC'11), written from the published round function.
 __device__ __forceinline__ uint4 philox4x32_10(uint4 c, uint32_t k0, uint32_t k1)

@@ -576,8 +576,7 @@ void tile_launch_m(const InterpArgs& a, int mode, cudaStream_t st, size_t smem, 
 template <int P>
 bool tile_launch_p(const InterpArgs& a, int ey, int ez, int mode, cudaStream_t st, size_t smem, bool cfg, cudaError_t* err)
 {
-    constexpr int H = (P >= 3) ? 3 : 1;
-    constexpr int EZA = (P >= 3) ? 24 : 20, EZB = (P >= 3) ? 40 : 36;   // TZ = 16 / 32 (+ halo + alignment, % 4 == 0)
+    constexpr int H = Halo<P>::H, EZA = Halo<P>::EZA, EZB = Halo<P>::EZB;
     if (ey == 8 + H && ez == EZA) tile_launch_m<P, 8 + H, EZA>(a, mode, st, smem, cfg, err);
     else if (ey == 8 + H && ez == EZB) tile_launch_m<P, 8 + H, EZB>(a, mode, st, smem, cfg, err);
     else if (ey == 16 + H && ez == EZA) tile_launch_m<P, 16 + H, EZA>(a, mode, st, smem, cfg, err);
@@ -591,7 +590,8 @@ bool tile_launch_any(const InterpArgs& a, int mode, cudaStream_t st, size_t smem
     case 1: return tile_launch_p<1>(a, a.tp.EY, a.tp.EZ, mode, st, smem, cfg, err);
     case 2: return tile_launch_p<2>(a, a.tp.EY, a.tp.EZ, mode, st, smem, cfg, err);
     case 3: return tile_launch_p<3>(a, a.tp.EY, a.tp.EZ, mode, st, smem, cfg, err);
-    default: return tile_launch_p<4>(a, a.tp.EY, a.tp.EZ, mode, st, smem, cfg, err);
+    case 4: return tile_launch_p<4>(a, a.tp.EY, a.tp.EZ, mode, st, smem, cfg, err);
+    default: return tile_launch_p<5>(a, a.tp.EY, a.tp.EZ, mode, st, smem, cfg, err);
     }
 }
 
@@ -640,7 +640,8 @@ int launch_interp(tild_ctx* c, int mode, const SegLayout& lay, const float* ffie
     case 1: slots_launch_p<1>(a, vec, mode, 0, n, c->stream); break;
     case 2: slots_launch_p<2>(a, vec, mode, 0, n, c->stream); break;
     case 3: slots_launch_p<3>(a, vec, mode, 0, n, c->stream); break;
-    default: slots_launch_p<4>(a, vec, mode, 0, n, c->stream); break;
+    case 4: slots_launch_p<4>(a, vec, mode, 0, n, c->stream); break;
+    default: slots_launch_p<5>(a, vec, mode, 0, n, c->stream); break;
     }
     TILD_LAUNCH_CHECK(c, "interp_slots_kernel");
     return TILD_OK;

@@ -253,7 +253,8 @@ int launch_cell_keys(tild_ctx* c, const float* x, uint32_t* key, int32_t* base)
     case 1: cell_key_kernel<1><<<nb, 256, 0, c->stream>>>(c->mesh, x, key, base); break;
     case 2: cell_key_kernel<2><<<nb, 256, 0, c->stream>>>(c->mesh, x, key, base); break;
     case 3: cell_key_kernel<3><<<nb, 256, 0, c->stream>>>(c->mesh, x, key, base); break;
-    default: cell_key_kernel<4><<<nb, 256, 0, c->stream>>>(c->mesh, x, key, base); break;
+    case 4: cell_key_kernel<4><<<nb, 256, 0, c->stream>>>(c->mesh, x, key, base); break;
+    default: cell_key_kernel<5><<<nb, 256, 0, c->stream>>>(c->mesh, x, key, base); break;
     }
     TILD_LAUNCH_CHECK(c, "cell_key_kernel");
     return TILD_OK;
@@ -298,7 +299,8 @@ int launch_segment_sort(tild_ctx* c, const float4* X4src, float4* X4dst, SegLayo
         case 1: seg_key_kernel<1><<<blocks_for(n), 256, 0, c->stream>>>(c->mesh, tp, X4src, c->key, c->rank, c->count); break;
         case 2: seg_key_kernel<2><<<blocks_for(n), 256, 0, c->stream>>>(c->mesh, tp, X4src, c->key, c->rank, c->count); break;
         case 3: seg_key_kernel<3><<<blocks_for(n), 256, 0, c->stream>>>(c->mesh, tp, X4src, c->key, c->rank, c->count); break;
-        default: seg_key_kernel<4><<<blocks_for(n), 256, 0, c->stream>>>(c->mesh, tp, X4src, c->key, c->rank, c->count); break;
+        case 4: seg_key_kernel<4><<<blocks_for(n), 256, 0, c->stream>>>(c->mesh, tp, X4src, c->key, c->rank, c->count); break;
+        default: seg_key_kernel<5><<<blocks_for(n), 256, 0, c->stream>>>(c->mesh, tp, X4src, c->key, c->rank, c->count); break;
         }
         TILD_LAUNCH_CHECK(c, "seg_key_kernel");
     }

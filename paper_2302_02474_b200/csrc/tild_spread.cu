@@ -130,7 +130,7 @@ __global__ void __launch_bounds__(SPREAD_THREADS, 2) spread_tile_kernel(MeshPara
     __shared__ unsigned long long red[SPREAD_WARPS];
     __shared__ int goff_x[32], goff_y[32];          // wrapped global x / y node of each local x / y
     __shared__ uint32_t cnt[32], novf, ndrift;
-    __shared__ uint32_t rowoff[19 * 19];            // mesh offset of image row (lx, ly), z excluded
+    __shared__ uint32_t rowoff[21 * 21];            // mesh offset of image row (lx, ly), z excluded
     const int EX = tp.E[0];
     const int E3 = EX * EY * EZ;
     const int tile = blockIdx.x;
@@ -151,7 +151,7 @@ __global__ void __launch_bounds__(SPREAD_THREADS, 2) spread_tile_kernel(MeshPara
         for (int k = threadIdx.x; k < n4; k += SPREAD_THREADS) z4[k] = make_uint4(0u, 0u, 0u, 0u);
         if (threadIdx.x < EX) goff_x[threadIdx.x] = wrap_idx(o[0] + threadIdx.x, m.N[0]);
         else if (threadIdx.x >= 32 && threadIdx.x < 32 + EY) goff_y[threadIdx.x - 32] = wrap_idx(o[1] + threadIdx.x - 32, m.N[1]);
-        if (threadIdx.x < EX * EY) {                 // EX * EY <= 361 <= SPREAD_THREADS
+        if (threadIdx.x < EX * EY) {                 // EX * EY <= 441 <= SPREAD_THREADS
             const int lx = threadIdx.x / EY, ly = threadIdx.x - lx * EY;
             rowoff[threadIdx.x] = (uint32_t)((wrap_idx(o[0] + lx, m.N[0]) * m.N[1] + wrap_idx(o[1] + ly, m.N[1])) * m.N[2]);
         }
@@ -272,7 +272,7 @@ __global__ void __launch_bounds__(SPREAD_THREADS, 2) spread_tile_kernel(MeshPara
         if (pass == 1) break;
         // A node can only wrap past 2^32 if >= 2^9 / (largest single-node weight) particles sit on it: the largest
         // weight is 1 (P <= 2), (3/4)^3 (P = 3), (23/48)^3 (P = 4).  Tiles with fewer particles skip the check.
-        constexpr uint32_t SAFE = P <= 2 ? 511u : (P == 3 ? 1213u : 4653u);
+        constexpr uint32_t SAFE = P <= 2 ? 511u : (P == 3 ? 1213u : (P == 4 ? 4653u : 2381u));   // P = 5: (115/192)^3
         if (p_hi - p_lo <= SAFE) return;              // uniform across the block
         const unsigned long long total = block_sum_u64(tile_sum, red);
         const unsigned long long cntp = block_sum_u64((unsigned long long)n_tile, red);
@@ -302,8 +302,7 @@ bool tile_case(int p, int ey, int ez, F&& f)
 template <int P, typename F>
 bool tile_dispatch_p(int p, int ey, int ez, F&& f)
 {
-    constexpr int H = (P >= 3) ? 3 : 1;
-    constexpr int EZA = (P >= 3) ? 24 : 20, EZB = (P >= 3) ? 40 : 36;   // TZ = 16 / 32 (+ halo + alignment, % 4 == 0)
+    constexpr int H = Halo<P>::H, EZA = Halo<P>::EZA, EZB = Halo<P>::EZB;
     return tile_case<P, 8 + H, EZA>(p, ey, ez, f) || tile_case<P, 8 + H, EZB>(p, ey, ez, f) ||
            tile_case<P, 16 + H, EZA>(p, ey, ez, f) || tile_case<P, 16 + H, EZB>(p, ey, ez, f);
 }
@@ -311,7 +310,7 @@ template <typename F>
 bool tile_dispatch(int p, int ey, int ez, F&& f)
 {
     return tile_dispatch_p<1>(p, ey, ez, f) || tile_dispatch_p<2>(p, ey, ez, f) || tile_dispatch_p<3>(p, ey, ez, f) ||
-           tile_dispatch_p<4>(p, ey, ez, f);
+           tile_dispatch_p<4>(p, ey, ez, f) || tile_dispatch_p<5>(p, ey, ez, f);
 }
 
 int spread_slots(tild_ctx* c, size_t s0, size_t s1, const float4* X4, float* grid)
@@ -322,7 +321,8 @@ int spread_slots(tild_ctx* c, size_t s0, size_t s1, const float4* X4, float* gri
     case 1: spread_slots_kernel<1><<<nb, 256, 0, c->stream>>>(c->mesh, s0, s1, X4, grid); break;
     case 2: spread_slots_kernel<2><<<nb, 256, 0, c->stream>>>(c->mesh, s0, s1, X4, grid); break;
     case 3: spread_slots_kernel<3><<<nb, 256, 0, c->stream>>>(c->mesh, s0, s1, X4, grid); break;
-    default: spread_slots_kernel<4><<<nb, 256, 0, c->stream>>>(c->mesh, s0, s1, X4, grid); break;
+    case 4: spread_slots_kernel<4><<<nb, 256, 0, c->stream>>>(c->mesh, s0, s1, X4, grid); break;
+    default: spread_slots_kernel<5><<<nb, 256, 0, c->stream>>>(c->mesh, s0, s1, X4, grid); break;
     }
     TILD_LAUNCH_CHECK(c, "spread_slots_kernel");
     return TILD_OK;

@@ -42,7 +42,7 @@ def test_params_struct_matches_header(lib):
     assert lib.tild_workspace_bytes(C.byref(p), C.byref(nbytes)) == tild.EINVAL
 
 
-@pytest.mark.parametrize("field,value", [("order", 0), ("order", 5), ("n_species", 0), ("n_species", 9), ("n", -1),
+@pytest.mark.parametrize("field,value", [("order", 0), ("order", 6), ("n_species", 0), ("n_species", 9), ("n", -1),
                                          ("max_bonds", 5), ("dt", 0.0), ("mass", -1.0)])
 def test_invalid_params_are_rejected(lib, field, value):
     p = tild.make_params(1000, 2, (10.0,) * 3, (16,) * 3, 2, [[0, 1], [1, 0]], 50.0)

@@ -38,7 +38,7 @@ def make(cfg, **kw):
     return st, eng
 
 
-CASES = [small_cfg(order=P) for P in (1, 2, 3, 4)] + [small_cfg(order=3, S=3, grid=(18, 12, 30), box=(9.0, 6.0, 15.0))]
+CASES = [small_cfg(order=P) for P in (1, 2, 3, 4, 5)] + [small_cfg(order=3, S=3, grid=(18, 12, 30), box=(9.0, 6.0, 15.0))]
 
 
 def test_philox_bit_exact_and_normals():
@@ -142,8 +142,8 @@ def test_trajectory_c1_100_steps(resort_every):
     assert ev <= 2e-3, ev
 
 
-@pytest.mark.parametrize("cfg", [small_cfg(order=4), small_cfg(order=3, S=3, grid=(18, 12, 30), box=(9.0, 6.0, 15.0))],
-                         ids=["P4", "P3_S3"])
+@pytest.mark.parametrize("cfg", [small_cfg(order=4), small_cfg(order=3, S=3, grid=(18, 12, 30), box=(9.0, 6.0, 15.0)),
+                                 small_cfg(order=5)], ids=["P4", "P3_S3", "P5"])
 def test_trajectory_small_100_steps(cfg):
     ex, ev, _ = run_trajectory(cfg, 100, resort_every=9)
     assert ex <= 1e-4, ex
@@ -198,7 +198,7 @@ def test_empty_system():
     assert step == 3
 
 
-@pytest.mark.parametrize("P", [1, 2, 3, 4])
+@pytest.mark.parametrize("P", [1, 2, 3, 4, 5])
 def test_crowded_cell_and_box_edges(P):
     """All particles in one cell at the periodic corner (maximum atomic contention, wrap on every axis),
     plus particles exactly at 0 and one ulp below L."""
@@ -283,7 +283,7 @@ def test_naive_kernel_flags_match_oracle():
     assert np.abs(f.cpu().numpy() - of).max() <= REL * vec_rms(of)
 
 
-@pytest.mark.parametrize("P", [2, 4])
+@pytest.mark.parametrize("P", [2, 4, 5])
 def test_fixed_point_tile_wrap_is_detected_and_redone(P):
     """> 256 particles' worth of weight on one node wraps the 2^-24 fixed-point tile; the mass-balance check must
     catch it and the tile must be redone with fp32 atomics."""
@@ -292,7 +292,8 @@ def test_fixed_point_tile_wrap_is_detected_and_redone(P):
     cfg = replace(small_cfg(order=P), n=n)
     rng = np.random.default_rng(17)
     h = np.array(cfg.box) / np.array(cfg.grid)
-    x = ((np.array([5, 7, 3]) + 0.5 + 0.02 * rng.random((n, 3))) * h).astype(np.float32)   # all next to one cell centre
+    centre = 0.5 if P % 2 == 0 else 0.0          # the largest single-node weight: cell centre (even P) / node (odd P)
+    x = ((np.array([5, 7, 3]) + centre + 0.02 * rng.random((n, 3))) * h).astype(np.float32)
     x[:50] = (rng.random((50, 3)) * np.array(cfg.box)).astype(np.float32)
     ty = (np.arange(n) % 2).astype(np.int32)
     eng = tild.Tild(tild.params_from_config(cfg))
@@ -385,7 +386,7 @@ def test_c5_sweep_point_force(grid, order, memory_order):
 @pytest.mark.parametrize("env", [{"TILD_TILE_X": "16", "TILD_TILE_Y": "8"}, {"TILD_TILE_Y": "8", "TILD_TILE_Z": "16"},
                                  {"TILD_TILE_X": "16", "TILD_TILE_Y": "16", "TILD_TILE_Z": "16"}],
                          ids=["x16y8", "y8z16", "x16y16z16"])
-@pytest.mark.parametrize("P", [2, 3, 4])
+@pytest.mark.parametrize("P", [2, 3, 4, 5])
 def test_tile_shape_variants(env, P, monkeypatch):
     """Every (EY, EZ) instantiation of the tile kernels gives the same forces and trajectories."""
     for k, v in env.items():
