@@ -87,6 +87,11 @@ typedef struct {
     uint32_t flags;            /* TILD_FLAG_* */
     int32_t integrator;        /* TILD_INTEGRATOR_GJF (default, A11) or TILD_INTEGRATOR_EM (overdamped, A11b; gamma > 0) */
     int32_t reserved;          /* 0 */
+    /* electrostatics on the same path (reading A22): valence per species, Bjerrum length
+     * (0 = off), Gaussian smearing length of a charge; pair kernel 4 pi l_B exp(-k^2 a_q^2) / k^2, k = 0 dropped */
+    double charge[TILD_MAX_SPECIES];
+    double bjerrum;
+    double a_charge;
 } tild_params;
 
 /* HOST. Bytes of device workspace tild_init needs for these parameters. */

@@ -49,6 +49,9 @@ typedef struct {
     int32_t max_bonds;
     double dt, gamma, kT, mass;
     uint64_t seed;
+    double charge[ORC_MAX_SPECIES]; /* valence of each species (reading A22) */
+    double bjerrum;     /* l_B >= 0; 0 switches electrostatics off */
+    double a_charge;    /* Gaussian smearing length of a charge (same form as h) */
     int32_t integrator; /* 0: GJF (A11); 1: Euler-Maruyama, overdamped */
     int32_t sampled_kernel; /* 0: analytic u^(k) (A5); 1: FFT of u_G sampled on the mesh, as PAPER.md L223 describes (A5b) */
     int32_t deconvolve; /* 0: kernel is u^(k) (A13); 1: u^(k) / W^(k)^2, W^ = prod_a sinc(k_a h_a / 2)^P */
@@ -365,6 +368,30 @@ static double orc_uhat(const orc_params *p, int mx, int my, int mz)
     return exp(-0.5 * p->sigma2 * k2) / w2;
 }
 
+/* Electrostatics on the same path ("electrostatic forces acting between the charged monomers ...
+ * use the mass/charge density field"; formulas not in the paper, reading A22).  Charge density rho_c = sum_J z_J rho_J,
+ * each charge smeared by a unit Gaussian of variance a_q^2 per dimension (the h of L139), Coulomb energy
+ * beta U = (l_B / 2) int int rho_c(r) rho_c(r') / |r - r'|.  In Fourier space the pair kernel between unit charges is
+ *   u^_el(k) = 4 pi l_B exp(-k^2 a_q^2) / k^2   (k != 0; the k = 0 mode is dropped: neutralising background),
+ * so the force spectra gain the term -i k_a u^_el(k) z_I sum_J z_J n^_J / V. */
+static double orc_uel(const orc_params *p, int mx, int my, int mz)
+{
+    if (!(p->bjerrum > 0.0)) return 0.0;
+    const int m[3] = {mx, my, mz};
+    double k2 = 0.0, w2 = 1.0;
+    for (int a = 0; a < 3; ++a) {
+        const double k = orc_k(p, a, m[a]);
+        k2 += k * k;
+        if (p->deconvolve) {
+            const double x = 0.5 * k * p->L[a] / (double)p->N[a];
+            const double sinc = x == 0.0 ? 1.0 : sin(x) / x;
+            w2 *= pow(sinc, 2.0 * p->P);
+        }
+    }
+    if (k2 == 0.0) return 0.0;
+    return 4.0 * ORC_PI * p->bjerrum * exp(-k2 * p->a_charge * p->a_charge) / k2 / w2;
+}
+
 /* "a Fourier-space representation of the inter-particle potential is calculated using Fast Fourier
  * Transform (FFT), and is stored".  Reading A5b: u_G(r) = (2 pi sigma2)^(-3/2) exp(-r^2 / 2 sigma2) (L121) is sampled at the
  * mesh nodes with the minimum-image distance, and u^_s(m) = dV sum_g u_G(r_g) exp(-2 pi i m.g/N) (real: u_G is even).
@@ -454,16 +481,18 @@ void orc_kspace_force(const orc_params *p, const double *grid, double *ffield)
                         (void)kx; (void)ky; (void)kz;
                         int m_a = a == 0 ? mx : (a == 1 ? my : mz);
                         double kg = orc_kgrad(p, a, m_a);
-                        double gr = 0.0, gi = 0.0;
+                        double gr = 0.0, gi = 0.0, er = 0.0, ei = 0.0;
                         for (int J = 0; J < S; ++J) {
                             double c = orc_cIJ(p, I, J);
                             gr += c * nhat[2 * (M * (size_t)J + g)];
                             gi += c * nhat[2 * (M * (size_t)J + g) + 1];
+                            er += p->charge[I] * p->charge[J] * nhat[2 * (M * (size_t)J + g)];
+                            ei += p->charge[I] * p->charge[J] * nhat[2 * (M * (size_t)J + g) + 1];
                         }
+                        const double uel = orc_uel(p, mx, my, mz);
                         /* -i * (gr + i gi) = gi - i gr */
-                        double f = kg * uhat / V;
-                        work[2 * g] = f * gi;
-                        work[2 * g + 1] = -f * gr;
+                        work[2 * g] = kg * (uhat * gi + uel * ei) / V;
+                        work[2 * g + 1] = -kg * (uhat * gr + uel * er) / V;
                     }
                 }
             }
@@ -743,13 +772,14 @@ void orc_energy(const orc_params *p, const double *x, const double *v, const int
                 double kx = orc_k(p, 0, mx), ky = orc_k(p, 1, my), kz = orc_k(p, 2, mz);
                 double uhat = utab_e ? utab_e[g] : orc_uhat(p, mx, my, mz);
                 (void)kx; (void)ky; (void)kz;
-                double acc = 0.0;
+                double acc = 0.0, el = 0.0;
                 for (int I = 0; I < S; ++I)
                     for (int J = 0; J < S; ++J) {
                         const double *aI = nhat + 2 * (M * (size_t)I + g), *aJ = nhat + 2 * (M * (size_t)J + g);
                         acc += orc_cIJ(p, I, J) * (aI[0] * aJ[0] + aI[1] * aJ[1]);
+                        el += p->charge[I] * p->charge[J] * (aI[0] * aJ[0] + aI[1] * aJ[1]);
                     }
-                nb += uhat * acc;
+                nb += uhat * acc + orc_uel(p, mx, my, mz) * el;
             }
     nb *= 0.5 / V;
     free(xf);

@@ -41,6 +41,7 @@ class _Params(C.Structure):
         ("max_bonds", C.c_int32),
         ("dt", C.c_double), ("gamma", C.c_double), ("kT", C.c_double), ("mass", C.c_double),
         ("seed", C.c_uint64),
+        ("charge", C.c_double * MAX_SPECIES), ("bjerrum", C.c_double), ("a_charge", C.c_double),
         ("integrator", C.c_int32),
         ("sampled_kernel", C.c_int32),
         ("deconvolve", C.c_int32),
@@ -67,6 +68,9 @@ class OracleParams:
     kT: float = 1.0
     mass: float = 1.0
     seed: int = 0
+    charge: tuple = ()         # valence per species (reading A22); bjerrum = 0 switches electrostatics off
+    bjerrum: float = 0.0
+    a_charge: float = 0.5
     integrator: int = 0        # 0 GJF (A11), 1 Euler-Maruyama (A11b)
     sampled_kernel: bool = False  # u^ from the FFT of u_G sampled on the mesh (A5b) instead of analytic (A5)
     deconvolve: bool = False   # divide the pair kernel by W^(k)^2; default: plain u^(k) (A13)
@@ -89,6 +93,9 @@ class OracleParams:
         p.k_bond, p.r0_bond, p.max_bonds = float(self.k_bond), float(self.r0_bond), int(self.max_bonds)
         p.dt, p.gamma, p.kT, p.mass = float(self.dt), float(self.gamma), float(self.kT), float(self.mass)
         p.seed = int(self.seed)
+        for i, z in enumerate(self.charge):
+            p.charge[i] = float(z)
+        p.bjerrum, p.a_charge = float(self.bjerrum), float(self.a_charge)
         p.integrator = int(self.integrator)
         p.sampled_kernel = 1 if self.sampled_kernel else 0
         p.deconvolve = 1 if self.deconvolve else 0

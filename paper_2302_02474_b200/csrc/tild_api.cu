@@ -56,6 +56,7 @@ int validate(const tild_params* p)
     if (!(p->dt > 0.0) || !(p->mass > 0.0) || p->gamma < 0.0 || p->kT < 0.0) return TILD_EINVAL;
     if (p->integrator != TILD_INTEGRATOR_GJF && p->integrator != TILD_INTEGRATOR_EM) return TILD_EINVAL;
     if (p->integrator == TILD_INTEGRATOR_EM && !(p->gamma > 0.0)) return TILD_EINVAL;
+    if (p->bjerrum < 0.0 || (p->bjerrum > 0.0 && !(p->a_charge > 0.0))) return TILD_EINVAL;
     return TILD_OK;
 }
 
@@ -138,7 +139,7 @@ void carve(tild_ctx* c, void* base, size_t* total)
     c->drift_count = w.take<uint32_t>(4);
     c->d_step = w.take<uint64_t>(2);
     c->d_energy = w.take<double>(4);
-    c->tables = w.take<float>(6 * 4096);
+    c->tables = w.take<float>(12 * 4096);
     *total = w.off;
 }
 
@@ -251,7 +252,7 @@ int tild_init(tild_ctx** out, const tild_params* params, void* workspace, size_t
     }
 
     // a0: k-space tables in double on the host (A4-A6), uploaded as fp32
-    std::vector<float> tab(6 * 4096, 0.0f);
+    std::vector<float> tab(12 * 4096, 0.0f);
     const double PI = 3.14159265358979323846264338327950288;
     for (int a = 0; a < 3; ++a) {
         const int N = p.grid[a];
@@ -280,6 +281,16 @@ int tild_init(tild_ctx** out, const tild_params* params, void* workspace, size_t
             if (a == 0) u /= V;
             tab[(size_t)a * 4096 + mm] = (float)kg;
             tab[(size_t)(3 + a) * 4096 + mm] = (float)u;
+            // electrostatics (A22): separable Gaussian part of 4 pi l_B exp(-k^2 a_q^2) / k^2, and k_a^2
+            double e = exp(-k * k * p.a_charge * p.a_charge);
+            if (p.flags & TILD_FLAG_DECONVOLVE) {
+                const double xh = 0.5 * k * p.box[a] / (double)N;
+                const double sinc = xh == 0.0 ? 1.0 : sin(xh) / xh;
+                e /= pow(sinc, 2.0 * p.order);
+            }
+            if (a == 0) e *= 4.0 * PI * p.bjerrum / V;
+            tab[(size_t)(6 + a) * 4096 + mm] = (float)e;
+            tab[(size_t)(9 + a) * 4096 + mm] = (float)(k * k);
         }
     }
     KspaceParams& ks = c->ksp;
@@ -289,11 +300,15 @@ int tild_init(tild_ctx** out, const tild_params* params, void* workspace, size_t
         ks.N[a] = p.grid[a];
         ks.kgrad[a] = c->tables + (size_t)a * 4096;
         ks.ufac[a] = c->tables + (size_t)(3 + a) * 4096;
+        ks.eel[a] = c->tables + (size_t)(6 + a) * 4096;
+        ks.k2[a] = c->tables + (size_t)(9 + a) * 4096;
     }
+    ks.has_el = p.bjerrum > 0.0 ? 1 : 0;
     for (int I = 0; I < S; ++I)
         for (int J = 0; J < S; ++J) {
             const double cij = (I == J) ? p.kappa / rho0 : (p.kappa + p.chi[I * TILD_MAX_SPECIES + J]) / rho0;  // A9
             ks.c[I * TILD_MAX_SPECIES + J] = (float)cij;
+            ks.qq[I * TILD_MAX_SPECIES + J] = (float)(p.charge[I] * p.charge[J]);
         }
 
     // GJF constants (A11)

@@ -36,14 +36,20 @@ __global__ void __launch_bounds__(256) kspace_energy_kernel(KspaceParams k, size
         float2 nj[S];
 #pragma unroll
         for (int J = 0; J < S; ++J) nj[J] = nhat[(size_t)J * Mk + idx];
+        double uel = 0.0;
+        if (k.has_el) {
+            const double k2 = (double)__ldg(k.k2[0] + mx) + (double)__ldg(k.k2[1] + my) + (double)__ldg(k.k2[2] + mz);
+            if (k2 > 0.0) uel = (double)__ldg(k.eel[0] + mx) * (double)__ldg(k.eel[1] + my) * (double)__ldg(k.eel[2] + mz) / k2;
+        }
         double acc = 0.0;
 #pragma unroll
         for (int I = 0; I < S; ++I)
 #pragma unroll
             for (int J = 0; J < S; ++J)
-                acc += (double)k.c[I * TILD_MAX_SPECIES + J] * ((double)nj[I].x * nj[J].x + (double)nj[I].y * nj[J].y);
+                acc += ((double)k.c[I * TILD_MAX_SPECIES + J] * u + (double)k.qq[I * TILD_MAX_SPECIES + J] * uel) *
+                       ((double)nj[I].x * nj[J].x + (double)nj[I].y * nj[J].y);
         const bool self_conjugate = mz == 0 || (k.N[2] % 2 == 0 && mz == k.N[2] / 2);
-        e += (self_conjugate ? 0.5 : 1.0) * u * acc;
+        e += (self_conjugate ? 0.5 : 1.0) * acc;
     }
     block_add(e, out + 2);
 }

@@ -53,6 +53,11 @@ struct KspaceParams {
     const float* kgrad[3];   // k_a(m), 0 at the Nyquist index of even N (A6)
     const float* ufac[3];    // exp(-sigma2 k_a(m)^2 / 2); ufac[0] also carries 1/V
     float c[TILD_MAX_SPECIES * TILD_MAX_SPECIES];  // c_IJ (1/V folded into ufac[0])
+    // electrostatics (A22): u_el = eel[0] eel[1] eel[2] / (k2[0] + k2[1] + k2[2]), 0 at k = 0; 4 pi l_B / V in eel[0]
+    int has_el;
+    const float* eel[3];     // exp(-k_a^2 a_q^2) (times the deconvolution factor when that is on)
+    const float* k2[3];      // k_a(m)^2, true wave number (Nyquist included)
+    float qq[TILD_MAX_SPECIES * TILD_MAX_SPECIES];  // z_I z_J
 };
 
 struct StepParams {

@@ -42,13 +42,15 @@ class Params(C.Structure):
         ("seed", C.c_uint64),
         ("resort_every", C.c_int32), ("flags", C.c_uint32),
         ("integrator", C.c_int32), ("reserved", C.c_int32),
+        ("charge", C.c_double * MAX_SPECIES), ("bjerrum", C.c_double), ("a_charge", C.c_double),
     ]
 
 
 def make_params(n: int, n_species: int, box: Sequence[float], grid: Sequence[int], order: int, chi, kappa: float,
                 a: float = 0.5, sigma2: float = 0.0, rho0: float = 0.0, k_bond: float = 1.5, r0_bond: float = 0.0,
                 max_bonds: int = 2, dt: float = 0.005, gamma: float = 1.0, kT: float = 1.0, mass: float = 1.0,
-                seed: int = 0, resort_every: int = 0, flags: int = 0, integrator: int = 0) -> Params:
+                seed: int = 0, resort_every: int = 0, flags: int = 0, integrator: int = 0,
+                charge: Sequence[float] = (), bjerrum: float = 0.0, a_charge: float = 0.5) -> Params:
     p = Params()
     p.struct_size = C.sizeof(Params)
     p.n, p.n_species, p.order = int(n), int(n_species), int(order)
@@ -66,6 +68,9 @@ def make_params(n: int, n_species: int, box: Sequence[float], grid: Sequence[int
     p.seed = int(seed)
     p.resort_every, p.flags = int(resort_every), int(flags)
     p.integrator, p.reserved = int(integrator), 0
+    for i, z in enumerate(charge):
+        p.charge[i] = float(z)
+    p.bjerrum, p.a_charge = float(bjerrum), float(a_charge)
     return p
 
 
@@ -74,7 +79,8 @@ def params_from_config(cfg, flags: int = 0, resort_every: int = 0, **overrides) 
     kw = dict(n=cfg.n, n_species=cfg.n_species, box=cfg.box, grid=cfg.grid, order=cfg.order, chi=cfg.chi,
               kappa=cfg.kappa, a=cfg.a, sigma2=cfg.sigma2, k_bond=cfg.k_bond, r0_bond=cfg.r0_bond, max_bonds=2,
               dt=cfg.dt, gamma=cfg.gamma, kT=cfg.kT, mass=cfg.mass, seed=cfg.philox_seed,
-              resort_every=resort_every, flags=flags)
+              resort_every=resort_every, flags=flags, charge=getattr(cfg, "charge", ()),
+              bjerrum=getattr(cfg, "bjerrum", 0.0), a_charge=getattr(cfg, "a_charge", 0.5))
     kw.update(overrides)
     return make_params(**kw)
 

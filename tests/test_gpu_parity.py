@@ -596,3 +596,48 @@ def test_sampled_kernel_parity(deconv):
     e = eng.tild_energy()
     oe = orc.energy(p, st.x.astype(np.float64), st.v.astype(np.float64), st.type, st.bond_partner)
     assert np.all(np.abs(e - oe) <= 2e-5 * np.abs(oe).max())
+
+
+@pytest.mark.parametrize("deconv", [False, True])
+def test_electrostatics_parity(deconv):
+    """SURVEY 8(f) #1 (reading A22): charges per species, Coulomb kernel of Gaussian-smeared charges in the fused k-space
+    kernel.  Stage, total force, energy and a trajectory against the oracle."""
+    cfg = small_cfg(order=4, S=3, grid=(18, 12, 30), box=(9.0, 6.0, 15.0))
+    el = dict(charge=(1.0, -1.0, 0.0), bjerrum=2.0, a_charge=0.45)
+    flags = tild.FLAG_DECONVOLVE if deconv else 0
+    st, eng = make(cfg, flags=flags, resort_every=5, **el)
+    p = oracle_params(cfg, deconvolve=deconv, **el)
+    og32 = orc.spread(p, st.x, st.type).astype(np.float32)
+    ff = eng.tild_kspace_force(dev(og32)).cpu().numpy()
+    off = orc.kspace_force(p, og32.astype(np.float64))
+    assert np.abs(ff - off).max() <= REL * rms(off)
+    neutral = orc.kspace_force(oracle_params(cfg, deconvolve=deconv), og32.astype(np.float64))
+    assert np.abs(off - neutral)[:2].max() > 0.1 * rms(neutral)       # the charged species' fields really change
+    assert np.abs(off - neutral)[2].max() < 1e-12                     # the neutral species' field does not
+    eng.tild_set_state(dev(st.x), dev(st.v), dev(st.type), dev(st.bond_partner), 0)
+    _, _, f, _ = eng.tild_get_state(want_v=False, want_f=True)
+    of = orc.force(p, st.x.astype(np.float64), st.type, st.bond_partner)
+    assert np.abs(f.cpu().numpy() - of).max() <= REL * vec_rms(of)
+    e = eng.tild_energy()
+    oe = orc.energy(p, st.x.astype(np.float64), st.v.astype(np.float64), st.type, st.bond_partner)
+    assert np.all(np.abs(e - oe) <= 2e-5 * np.abs(oe).max()), (e, oe)
+    eng.tild_step(40)
+    x = eng.tild_get_state(want_v=False)[0].cpu().numpy().astype(np.float64)
+    ox, _, _ = orc.run(p, st.x.astype(np.float64), st.v.astype(np.float64), st.type, st.bond_partner, 0, 40, f=of)
+    assert np.abs(min_image(x - ox, cfg.box)).max() <= 1e-4
+
+
+def test_coacervate_sized_charged_melt_force_and_steps():
+    """434 x 82 polycation / polyanion chains (the size of PAPER.md VII.A, L464-466; parameters are this repo's): total
+    force incl. electrostatics against the oracle, then 20 steps."""
+    cfg = inputs.COAC
+    st, eng = make(cfg)
+    p = oracle_params(cfg)
+    eng.tild_set_state(dev(st.x), dev(st.v), dev(st.type), dev(st.bond_partner), 0)
+    _, _, f, _ = eng.tild_get_state(want_v=False, want_f=True)
+    of = orc.force(p, st.x.astype(np.float64), st.type, st.bond_partner)
+    assert np.abs(f.cpu().numpy() - of).max() <= REL * vec_rms(of)
+    eng.tild_step(20)
+    x = eng.tild_get_state(want_v=False)[0].cpu().numpy().astype(np.float64)
+    ox, _, _ = orc.run(p, st.x.astype(np.float64), st.v.astype(np.float64), st.type, st.bond_partner, 0, 20, f=of)
+    assert np.abs(min_image(x - ox, cfg.box)).max() <= 1e-4

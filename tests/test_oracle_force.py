@@ -344,3 +344,88 @@ def test_sampled_kernel_force_is_consistent():
     assert np.abs(F.sum(0)).max() < 1e-10 * np.abs(F).max() * n               # still momentum conserving
     rel = np.abs(F - G).max() / np.abs(G).max()
     assert 1e-5 < rel < 0.1, rel                                              # close to, but not, the analytic kernel
+
+
+# ---- electrostatics on the same path (reading A22) ----------------------------------------------------
+def ewald_smeared_force(x, z, L, lB, aq, alpha, kmax=10, images=2):
+    """Textbook Ewald evaluation of the force between Gaussian-smeared charges, written independently of the oracle.
+    Pair potential phi(r) = lB erf(r / 2 aq) / r, split as lB [erf(r/2aq) - erf(alpha r)] / r (short-ranged, summed over
+    images in real space) + lB erf(alpha r) / r (smooth: k-space, 4 pi / k^2 exp(-k^2 / 4 alpha^2), k != 0).
+    The result must not depend on alpha (alpha = 1 / 2 aq makes the real-space part vanish)."""
+    from scipy.special import erf
+    x = np.asarray(x, dtype=np.float64)
+    L = np.asarray(L, dtype=np.float64)
+    n = len(x)
+    F = np.zeros((n, 3))
+    rng_img = range(-images, images + 1)
+    for i in range(n):
+        for j in range(n):
+            for a in rng_img:
+                for b in rng_img:
+                    for c in rng_img:
+                        if i == j and a == b == c == 0:
+                            continue
+                        d = x[i] - x[j] + L * np.array([a, b, c])
+                        r = np.linalg.norm(d)
+                        # -d/dr {[erf(r/2aq) - erf(alpha r)] / r}
+                        dphi = (erf(r / (2 * aq)) - erf(alpha * r)) / r ** 2 - (
+                            np.exp(-r ** 2 / (4 * aq ** 2)) / (aq * np.sqrt(np.pi)) - 2 * alpha * np.exp(-(alpha * r) ** 2) / np.sqrt(np.pi)) / r
+                        F[i] += lB * z[i] * z[j] * dphi * d / r
+    V = L.prod()
+    ms = np.arange(-kmax, kmax + 1)
+    MX, MY, MZ = np.meshgrid(ms, ms, ms, indexing="ij")
+    KX, KY, KZ = 2 * np.pi * MX / L[0], 2 * np.pi * MY / L[1], 2 * np.pi * MZ / L[2]
+    K2 = KX ** 2 + KY ** 2 + KZ ** 2
+    K2[kmax, kmax, kmax] = 1.0
+    G = 4 * np.pi * lB * np.exp(-K2 / (4 * alpha ** 2)) / K2
+    G[kmax, kmax, kmax] = 0.0
+    S = sum(z[j] * np.exp(-1j * (KX * x[j, 0] + KY * x[j, 1] + KZ * x[j, 2])) for j in range(n))
+    for i in range(n):
+        ph = np.exp(1j * (KX * x[i, 0] + KY * x[i, 1] + KZ * x[i, 2]))
+        for a, K in enumerate((KX, KY, KZ)):
+            F[i, a] += (z[i] * (-1j * K) * G * S * ph).sum().real / V
+    return F
+
+
+def test_electrostatic_force_matches_ewald_of_smeared_charges():
+    """PM electrostatics (charges per species, Coulomb kernel 4 pi lB exp(-k^2 aq^2)/k^2) with the deconvolved kernel on a
+    fine mesh against the Ewald sum with a DIFFERENT splitting parameter (real-space erf differences + k-space)."""
+    rng = np.random.default_rng(11)
+    L = (6.0, 6.0, 6.0)
+    n, lB, aq = 8, 2.5, 0.5
+    x = (rng.random((n, 3)) * 6.0).astype(np.float32)
+    ty = np.array([0, 1] * (n // 2), dtype=np.int32)
+    zsp = (1.0, -1.0)
+    z = np.array([zsp[t] for t in ty])
+    a1 = ewald_smeared_force(x, z, L, lB, aq, alpha=1.0 / (2 * aq))          # real-space part vanishes identically
+    a2 = ewald_smeared_force(x, z, L, lB, aq, alpha=0.7 / (2 * aq))          # genuinely split
+    assert np.abs(a1 - a2).max() < 1e-9 * np.abs(a1).max()
+    assert np.abs(a1.sum(0)).max() < 1e-9 * np.abs(a1).max()
+    errs = []
+    for Ng in (24, 48):
+        p = orc.OracleParams(n, 2, L, (Ng,) * 3, 4, np.zeros((2, 2)), kappa=0.0, sigma2=0.5, rho0=1.0,
+                             charge=zsp, bjerrum=lB, a_charge=aq, deconvolve=True)
+        F = orc.nonbonded_force(p, x, ty)
+        errs.append(np.abs(F - a2).max() / np.abs(a2).max())
+    assert errs[0] < 2e-3 and errs[1] < 1e-4, errs                           # aliasing only; falls fast with h
+    # opposite charges attract, equal charges repel (sign convention)
+    q = orc.OracleParams(2, 2, L, (32,) * 3, 4, np.zeros((2, 2)), kappa=0.0, sigma2=0.5, rho0=1.0, charge=zsp, bjerrum=lB, a_charge=aq)
+    xp = np.array([[2.0, 3.0, 3.0], [3.5, 3.0, 3.0]], dtype=np.float32)
+    Fp = orc.nonbonded_force(q, xp, np.array([0, 1], np.int32))
+    assert Fp[0, 0] > 0 and Fp[1, 0] < 0
+    Fs = orc.nonbonded_force(q, xp, np.array([0, 0], np.int32))
+    assert Fs[0, 0] < 0 and Fs[1, 0] > 0
+
+
+def test_electrostatics_off_and_neutral_species_feel_nothing():
+    rng = np.random.default_rng(2)
+    L, N = (6.0, 4.5, 7.0), (12, 8, 10)
+    n = 90
+    x = (rng.random((n, 3)) * np.array(L)).astype(np.float32)
+    ty = rng.integers(0, 3, size=n).astype(np.int32)
+    base = orc.OracleParams(n, 3, L, N, 3, CHI3, kappa=5.0, sigma2=0.5, rho0=2.0)
+    el = orc.OracleParams(n, 3, L, N, 3, CHI3, kappa=5.0, sigma2=0.5, rho0=2.0, charge=(1.0, -1.0, 0.0), bjerrum=1.7, a_charge=0.4)
+    F0, F1 = orc.nonbonded_force(base, x, ty), orc.nonbonded_force(el, x, ty)
+    assert np.abs(F1 - F0)[ty == 2].max() < 1e-12                             # the neutral species gains no force
+    assert np.abs(F1 - F0)[ty != 2].max() > 1e-3
+    assert np.abs(F1.sum(0)).max() < 1e-10 * np.abs(F1).max() * n            # momentum conservation survives

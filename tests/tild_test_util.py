@@ -8,7 +8,7 @@ from paper_2302_02474_b200 import inputs
 def oracle_params(cfg, **over):
     kw = dict(n=cfg.n, S=cfg.n_species, L=cfg.box, N=cfg.grid, P=cfg.order, chi=np.array(cfg.chi), kappa=cfg.kappa,
               sigma2=cfg.sigma2, k_bond=cfg.k_bond, r0_bond=cfg.r0_bond, max_bonds=2, dt=cfg.dt, gamma=cfg.gamma,
-              kT=cfg.kT, mass=cfg.mass, seed=cfg.philox_seed)
+              kT=cfg.kT, mass=cfg.mass, seed=cfg.philox_seed, charge=cfg.charge, bjerrum=cfg.bjerrum, a_charge=cfg.a_charge)
     kw.update(over)
     return orc.OracleParams(**kw)
 
