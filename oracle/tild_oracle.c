@@ -49,6 +49,7 @@ typedef struct {
     int32_t max_bonds;
     double dt, gamma, kT, mass;
     uint64_t seed;
+    double lambda_wlc;  /* stiffness of the cosine angle potential, Eq. 16; 0 = no angles (A23) */
     double charge[ORC_MAX_SPECIES]; /* valence of each species (reading A22) */
     double bjerrum;     /* l_B >= 0; 0 switches electrostatics off */
     double a_charge;    /* Gaussian smearing length of a charge (same form as h) */
@@ -569,6 +570,32 @@ void orc_bond_force(const orc_params *p, const double *x, const int32_t *partner
             for (int a = 0; a < 3; ++a) f[3 * (size_t)i + a] += scale * d[a];
         }
     }
+    /* Angles, Eq. 16: u_wlc = lambda [1 + cos(theta_ijk)], theta the inside angle at j between the bonds to
+     * i and k.  Reading A23: for linear chains (max_bonds = 2) the triplets are (partner slot 0, j, partner slot 1) of
+     * every bead j that has both.  cos(theta) = d1.d2 / (|d1| |d2|), d1 = r_i - r_j, d2 = r_k - r_j (minimum image);
+     * F_i = -lambda d cos/d r_i, F_k likewise, F_j = -(F_i + F_k).  Serial loop: each angle adds to its three beads. */
+    if (p->lambda_wlc != 0.0 && p->max_bonds == 2) {
+        for (int j = 0; j < p->n; ++j) {
+            int32_t i = partner[2 * (size_t)j], k = partner[2 * (size_t)j + 1];
+            if (i < 0 || k < 0) continue;
+            double d1[3], d2[3], n1 = 0.0, n2 = 0.0, dot = 0.0;
+            for (int a = 0; a < 3; ++a) {
+                d1[a] = orc_min_image(x[3 * (size_t)i + a] - x[3 * (size_t)j + a], p->L[a]);
+                d2[a] = orc_min_image(x[3 * (size_t)k + a] - x[3 * (size_t)j + a], p->L[a]);
+                n1 += d1[a] * d1[a];
+                n2 += d2[a] * d2[a];
+                dot += d1[a] * d2[a];
+            }
+            if (n1 == 0.0 || n2 == 0.0) continue;
+            double inv = 1.0 / sqrt(n1 * n2), c = dot * inv;
+            for (int a = 0; a < 3; ++a) {
+                double gi = d2[a] * inv - c * d1[a] / n1, gk = d1[a] * inv - c * d2[a] / n2;
+                f[3 * (size_t)i + a] -= p->lambda_wlc * gi;
+                f[3 * (size_t)k + a] -= p->lambda_wlc * gk;
+                f[3 * (size_t)j + a] += p->lambda_wlc * (gi + gk);
+            }
+        }
+    }
 }
 
 /* Total force F(x): PM part on the fp32-rounded positions (O1 defines the index map on fp32
@@ -787,6 +814,21 @@ void orc_energy(const orc_params *p, const double *x, const double *v, const int
     free(utab_e);
     free(nhat);
     e[0] = ke;
+    if (p->lambda_wlc != 0.0 && p->max_bonds == 2) {   /* Eq. 16: sum over angles of lambda (1 + cos theta) */
+        for (int j = 0; j < p->n; ++j) {
+            int32_t i = partner[2 * (size_t)j], k = partner[2 * (size_t)j + 1];
+            if (i < 0 || k < 0) continue;
+            double n1 = 0.0, n2 = 0.0, dot = 0.0;
+            for (int a = 0; a < 3; ++a) {
+                double d1 = orc_min_image(x[3 * (size_t)i + a] - x[3 * (size_t)j + a], p->L[a]);
+                double d2 = orc_min_image(x[3 * (size_t)k + a] - x[3 * (size_t)j + a], p->L[a]);
+                n1 += d1 * d1;
+                n2 += d2 * d2;
+                dot += d1 * d2;
+            }
+            if (n1 > 0.0 && n2 > 0.0) be += p->lambda_wlc * (1.0 + dot / sqrt(n1 * n2));
+        }
+    }
     e[1] = be;
     e[2] = nb;
 }

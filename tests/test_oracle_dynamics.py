@@ -254,3 +254,54 @@ def test_em_free_diffusion_and_dimer_stationary_variance():
     a = 1 - 4 * k * dt / gamma
     var = (4 * dt / gamma) / (1 - a * a)
     assert abs((d ** 2).mean() / var - 1) < 0.05, ((d ** 2).mean(), var)
+
+
+# ---- cosine (wormlike-chain) angle potential, Eq. 16 L213 (reading A23) ----------------------
+def _chain_partners(n_chains, nb):
+    ids = np.arange(n_chains * nb).reshape(n_chains, nb)
+    prev, nxt = ids - 1, ids + 1
+    prev[:, 0] = -1
+    nxt[:, -1] = -1
+    return np.stack([prev.reshape(-1), nxt.reshape(-1)], axis=1).astype(np.int32)
+
+
+def test_wlc_angle_force_is_minus_the_energy_gradient_and_conserves_momentum_and_torque():
+    rng = np.random.default_rng(14)
+    n_chains, nb, L = 3, 6, (7.0, 8.0, 9.0)
+    n = n_chains * nb
+    x = (rng.random((n_chains, 1, 3)) * np.array(L) + np.cumsum(rng.normal(0, 0.6, (n_chains, nb, 3)), axis=1)).reshape(-1, 3)
+    x -= np.array(L) * np.floor(x / np.array(L))                       # some chains cross the periodic boundary
+    bp = _chain_partners(n_chains, nb)
+    p = orc.OracleParams(n, 1, L, (8, 8, 8), 2, np.zeros((1, 1)), 0.0, 0.5, k_bond=0.0, lambda_wlc=2.3)
+    F = orc.bond_force(p, x, bp)
+    ty, v = np.zeros(n, np.int32), np.zeros((n, 3))
+    eps = 1e-6
+    for i in (0, 1, 5, 7, 9, 17):
+        for a in range(3):
+            xp, xm = x.copy(), x.copy()
+            xp[i, a] += eps
+            xm[i, a] -= eps
+            dE = (orc.energy(p, xp, v, ty, bp)[1] - orc.energy(p, xm, v, ty, bp)[1]) / (2 * eps)
+            assert abs(F[i, a] + dE) < 1e-6 * max(1.0, np.abs(F).max()), (i, a, F[i, a], -dE)
+    assert np.abs(F.sum(0)).max() < 1e-12 * max(1.0, np.abs(F).max())
+    # torque about the chain's first bead (minimum-image unwrapped chain) vanishes chain by chain
+    for c in range(n_chains):
+        sl = slice(c * nb, (c + 1) * nb)
+        r = x[sl] - x[c * nb]
+        r -= np.array(L) * np.round(r / np.array(L))
+        assert np.abs(np.cross(r, F[sl]).sum(0)).max() < 1e-9
+
+
+def test_wlc_angle_special_cases():
+    """Straight trimer: cos = -1, u = 0, no force.  Right angle with unit bonds: u = lambda; the end beads are pushed
+    so as to open the angle with |F| = lambda / |d| (d cos/d r_i = d2_hat / |d1| at cos = 0)."""
+    L = (20.0,) * 3
+    bp = _chain_partners(1, 3)
+    ty, v = np.zeros(3, np.int32), np.zeros((3, 3))
+    p = orc.OracleParams(3, 1, L, (8, 8, 8), 2, np.zeros((1, 1)), 0.0, 0.5, k_bond=0.0, lambda_wlc=1.7)
+    straight = np.array([[4.0, 5, 5], [5.0, 5, 5], [6.5, 5, 5]])
+    assert np.abs(orc.bond_force(p, straight, bp)).max() < 1e-12 and abs(orc.energy(p, straight, v, ty, bp)[1]) < 1e-12
+    right = np.array([[5.0, 6, 5], [5.0, 5, 5], [6.0, 5, 5]])
+    F = orc.bond_force(p, right, bp)
+    assert abs(orc.energy(p, right, v, ty, bp)[1] - 1.7) < 1e-12
+    assert np.allclose(F[0], [-1.7, 0, 0]) and np.allclose(F[2], [0, -1.7, 0]) and np.allclose(F[1], [1.7, 1.7, 0])
