@@ -92,6 +92,9 @@ typedef struct {
     double charge[TILD_MAX_SPECIES];
     double bjerrum;
     double a_charge;
+    /* cosine (wormlike-chain) angle potential lambda [1 + cos(theta_ijk)], Eq. 16; 0 = none.  Needs
+     * max_bonds == 2: the triplets are (partner slot 0, bead, partner slot 1) of every bead with both (A23) */
+    double lambda_wlc;
 } tild_params;
 
 /* HOST. Bytes of device workspace tild_init needs for these parameters. */

@@ -56,6 +56,7 @@ int validate(const tild_params* p)
     if (!(p->dt > 0.0) || !(p->mass > 0.0) || p->gamma < 0.0 || p->kT < 0.0) return TILD_EINVAL;
     if (p->integrator != TILD_INTEGRATOR_GJF && p->integrator != TILD_INTEGRATOR_EM) return TILD_EINVAL;
     if (p->integrator == TILD_INTEGRATOR_EM && !(p->gamma > 0.0)) return TILD_EINVAL;
+    if (p->lambda_wlc != 0.0 && p->max_bonds != 2) return TILD_EINVAL;
     if (p->bjerrum < 0.0 || (p->bjerrum > 0.0 && !(p->a_charge > 0.0))) return TILD_EINVAL;
     return TILD_OK;
 }
@@ -325,6 +326,7 @@ int tild_init(tild_ctx** out, const tild_params* params, void* workspace, size_t
     s.k_bond = (float)p.k_bond;
     s.r0_bond = (float)p.r0_bond;
     s.max_bonds = p.max_bonds;
+    s.lambda_wlc = (p.max_bonds == 2) ? (float)p.lambda_wlc : 0.0f;
     s.integrator = p.integrator;
     s.em_drift = p.gamma > 0.0 ? (float)(p.dt / p.gamma) : 0.0f;
     s.em_noise = p.gamma > 0.0 ? (float)(1.0 / p.gamma) : 0.0f;

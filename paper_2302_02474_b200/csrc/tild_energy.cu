@@ -73,6 +73,20 @@ __global__ void __launch_bounds__(256) particle_energy_kernel(MeshParams m, Step
             const double d = sqrt(dx * dx + dy * dy + dz * dz) - (double)s.r0_bond;
             eb += (double)s.k_bond * d * d;
         }
+        if (s.lambda_wlc != 0.0f) {   // Eq. 16: lambda (1 + cos theta), counted by the angle's centre bead
+            const int2 bb = *reinterpret_cast<const int2*>(B + 2 * slot);
+            if (bb.x >= 0 && bb.y >= 0) {
+                const float4 a = X4[bb.x], c = X4[bb.y];
+                const float d1[3] = {min_image(a.x - p.x, m.L[0], m.inv_L[0]), min_image(a.y - p.y, m.L[1], m.inv_L[1]),
+                                     min_image(a.z - p.z, m.L[2], m.inv_L[2])};
+                const float d2[3] = {min_image(c.x - p.x, m.L[0], m.inv_L[0]), min_image(c.y - p.y, m.L[1], m.inv_L[1]),
+                                     min_image(c.z - p.z, m.L[2], m.inv_L[2])};
+                const double n1 = (double)d1[0] * d1[0] + (double)d1[1] * d1[1] + (double)d1[2] * d1[2];
+                const double n2 = (double)d2[0] * d2[0] + (double)d2[1] * d2[1] + (double)d2[2] * d2[2];
+                const double dot = (double)d1[0] * d2[0] + (double)d1[1] * d2[1] + (double)d1[2] * d2[2];
+                if (n1 > 0.0 && n2 > 0.0) eb += (double)s.lambda_wlc * (1.0 + dot / sqrt(n1 * n2));
+            }
+        }
     }
     block_add(ke, out + 0);
     __syncthreads();

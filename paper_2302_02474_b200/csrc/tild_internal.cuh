@@ -71,6 +71,7 @@ struct StepParams {
     float k_bond, r0_bond;
     int max_bonds;
     uint32_t key0, key1;   // Philox key = seed lo, hi
+    float lambda_wlc;      // cosine angle potential, Eq. 16 (0 = none; needs max_bonds == 2)
     int integrator;        // TILD_INTEGRATOR_*
     float em_drift;        // dt/gamma
     float em_noise;        // 1/gamma (times beta = noise_amp * z)
@@ -302,6 +303,66 @@ __device__ __forceinline__ float wrap_pos(float x, float L, float inv_L)
 __device__ __forceinline__ float min_image(float d, float L, float inv_L)
 {
     return d - L * rintf(d * inv_L);
+}
+
+// Gradients of cos(theta) = d1.d2 / (|d1| |d2|) with respect to the end points of d1 and d2 (Eq. 16):
+// gi = d cos / d r_i = d2 / (|d1||d2|) - cos d1 / |d1|^2,  gk likewise;  d cos / d r_j = -(gi + gk).  Returns cos.
+__device__ __forceinline__ float cos_gradients(const float d1[3], const float d2[3], float gi[3], float gk[3])
+{
+    const float n1 = d1[0] * d1[0] + d1[1] * d1[1] + d1[2] * d1[2], n2 = d2[0] * d2[0] + d2[1] * d2[1] + d2[2] * d2[2];
+    if (!(n1 > 0.0f) || !(n2 > 0.0f)) {
+        gi[0] = gi[1] = gi[2] = gk[0] = gk[1] = gk[2] = 0.0f;
+        return -1.0f;
+    }
+    const float inv = rsqrtf(n1) * rsqrtf(n2), c = (d1[0] * d2[0] + d1[1] * d2[1] + d1[2] * d2[2]) * inv;
+    const float c1 = c / n1, c2 = c / n2;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        gi[a] = d2[a] * inv - c1 * d1[a];
+        gk[a] = d1[a] * inv - c2 * d2[a];
+    }
+    return c;
+}
+
+// Force of the cosine angle potential on the bead at r with neighbours: prev / next (either may be missing) and their
+// own outer neighbours pprev / nnext.  has_* say which exist.  Each bead computes its own share of the (up to) three
+// angles it belongs to, without Newton's third law (as the paper does for bonds, L209).
+__device__ __forceinline__ void wlc_angle_force(float lambda, const float L[3], const float inv_L[3], const float r[3],
+                                                bool has_prev, const float prev[3], bool has_pprev, const float pprev[3],
+                                                bool has_next, const float next[3], bool has_nnext, const float nnext[3],
+                                                float f[3])
+{
+    float d1[3], d2[3], gi[3], gk[3];
+    if (has_prev && has_next) {          // centre bead of (prev, r, next)
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            d1[a] = min_image(prev[a] - r[a], L[a], inv_L[a]);
+            d2[a] = min_image(next[a] - r[a], L[a], inv_L[a]);
+        }
+        cos_gradients(d1, d2, gi, gk);
+#pragma unroll
+        for (int a = 0; a < 3; ++a) f[a] += lambda * (gi[a] + gk[a]);
+    }
+    if (has_prev && has_pprev) {         // end bead k of (pprev, prev, r)
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            d1[a] = min_image(pprev[a] - prev[a], L[a], inv_L[a]);
+            d2[a] = min_image(r[a] - prev[a], L[a], inv_L[a]);
+        }
+        cos_gradients(d1, d2, gi, gk);
+#pragma unroll
+        for (int a = 0; a < 3; ++a) f[a] -= lambda * gk[a];
+    }
+    if (has_next && has_nnext) {         // end bead i of (r, next, nnext)
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            d1[a] = min_image(r[a] - next[a], L[a], inv_L[a]);
+            d2[a] = min_image(nnext[a] - next[a], L[a], inv_L[a]);
+        }
+        cos_gradients(d1, d2, gi, gk);
+#pragma unroll
+        for (int a = 0; a < 3; ++a) f[a] -= lambda * gi[a];
+    }
 }
 
 #endif  // __CUDACC__

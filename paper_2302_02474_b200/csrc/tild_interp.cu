@@ -105,6 +105,41 @@ __device__ __forceinline__ void bond_term(const MeshParams& m, const StepParams&
     f.z += scale * dz;
 }
 
+// f += cosine angle force (Eq. 16; max_bonds == 2: slot 0 = previous bead, slot 1 = next bead, A23)
+__device__ __forceinline__ void angle_force_slots(const MeshParams& m, const StepParams& s, const float4* __restrict__ X4,
+                                                  const int32_t* __restrict__ B, size_t slot, const float4& p, float3& f)
+{
+    const int2 bb = *reinterpret_cast<const int2*>(B + 2 * slot);
+    const float r[3] = {p.x, p.y, p.z};
+    float prev[3] = {0.f, 0.f, 0.f}, next[3] = {0.f, 0.f, 0.f}, pprev[3] = {0.f, 0.f, 0.f}, nnext[3] = {0.f, 0.f, 0.f};
+    bool has_pprev = false, has_nnext = false;
+    if (bb.x >= 0) {
+        const float4 q = X4[bb.x];
+        prev[0] = q.x; prev[1] = q.y; prev[2] = q.z;
+        const int32_t pp = B[2 * (size_t)bb.x];
+        if (pp >= 0) {
+            const float4 qq = X4[pp];
+            pprev[0] = qq.x; pprev[1] = qq.y; pprev[2] = qq.z;
+            has_pprev = true;
+        }
+    }
+    if (bb.y >= 0) {
+        const float4 q = X4[bb.y];
+        next[0] = q.x; next[1] = q.y; next[2] = q.z;
+        const int32_t nn = B[2 * (size_t)bb.y + 1];
+        if (nn >= 0) {
+            const float4 qq = X4[nn];
+            nnext[0] = qq.x; nnext[1] = qq.y; nnext[2] = qq.z;
+            has_nnext = true;
+        }
+    }
+    float fa[3] = {0.f, 0.f, 0.f};
+    wlc_angle_force(s.lambda_wlc, m.L, m.inv_L, r, bb.x >= 0, prev, has_pprev, pprev, bb.y >= 0, next, has_nnext, nnext, fa);
+    f.x += fa[0];
+    f.y += fa[1];
+    f.z += fa[2];
+}
+
 // Bond force on the particle at p from its partners' positions (slots into X4).
 __device__ __forceinline__ float3 bond_force_slots(const MeshParams& m, const StepParams& s, const float4* __restrict__ X4,
                                                    const int32_t* __restrict__ B, size_t slot, const float4& p)
@@ -114,6 +149,7 @@ __device__ __forceinline__ float3 bond_force_slots(const MeshParams& m, const St
         const int32_t j = B[slot * s.max_bonds + k];
         if (j >= 0) bond_term(m, s, p, X4[j], f);
     }
+    if (s.lambda_wlc != 0.0f) angle_force_slots(m, s, X4, B, slot, p, f);
     return f;
 }
 
@@ -409,6 +445,7 @@ __global__ void __launch_bounds__(INTERP_THREADS, 2) interp_tile_kernel(MeshPara
                     if (s.max_bonds <= 2) {
                         if (bj0 >= 0) bond_term(m, s, p, q0, F);
                         if (bj1 >= 0) bond_term(m, s, p, q1, F);
+                        if (s.lambda_wlc != 0.0f) angle_force_slots(m, s, X4, B, slot, p, F);
                     } else {
                         const float3 fb = bond_force_slots(m, s, X4, B, slot, p);
                         F.x += fb.x;
@@ -477,6 +514,33 @@ __global__ void __launch_bounds__(256) bond_force_kernel(MeshParams m, StepParam
         acc.x += scale * dx;
         acc.y += scale * dy;
         acc.z += scale * dz;
+    }
+    if (s.lambda_wlc != 0.0f) {   // cosine angles, Eq. 16 (max_bonds == 2: slot 0 = previous, slot 1 = next bead)
+        const int32_t jp = bond[2 * (size_t)i], jn = bond[2 * (size_t)i + 1];
+        const float r[3] = {px, py, pz};
+        float prev[3] = {0.f, 0.f, 0.f}, next[3] = {0.f, 0.f, 0.f}, pprev[3] = {0.f, 0.f, 0.f}, nnext[3] = {0.f, 0.f, 0.f};
+        bool has_pprev = false, has_nnext = false;
+        if (jp >= 0) {
+            for (int a = 0; a < 3; ++a) prev[a] = x[3 * (size_t)jp + a];
+            const int32_t pp = bond[2 * (size_t)jp];
+            if (pp >= 0) {
+                for (int a = 0; a < 3; ++a) pprev[a] = x[3 * (size_t)pp + a];
+                has_pprev = true;
+            }
+        }
+        if (jn >= 0) {
+            for (int a = 0; a < 3; ++a) next[a] = x[3 * (size_t)jn + a];
+            const int32_t nn = bond[2 * (size_t)jn + 1];
+            if (nn >= 0) {
+                for (int a = 0; a < 3; ++a) nnext[a] = x[3 * (size_t)nn + a];
+                has_nnext = true;
+            }
+        }
+        float fa[3] = {0.f, 0.f, 0.f};
+        wlc_angle_force(s.lambda_wlc, m.L, m.inv_L, r, jp >= 0, prev, has_pprev, pprev, jn >= 0, next, has_nnext, nnext, fa);
+        acc.x += fa[0];
+        acc.y += fa[1];
+        acc.z += fa[2];
     }
     f[3 * (size_t)i + 0] = acc.x;
     f[3 * (size_t)i + 1] = acc.y;

@@ -43,6 +43,7 @@ class Params(C.Structure):
         ("resort_every", C.c_int32), ("flags", C.c_uint32),
         ("integrator", C.c_int32), ("reserved", C.c_int32),
         ("charge", C.c_double * MAX_SPECIES), ("bjerrum", C.c_double), ("a_charge", C.c_double),
+        ("lambda_wlc", C.c_double),
     ]
 
 
@@ -50,7 +51,8 @@ def make_params(n: int, n_species: int, box: Sequence[float], grid: Sequence[int
                 a: float = 0.5, sigma2: float = 0.0, rho0: float = 0.0, k_bond: float = 1.5, r0_bond: float = 0.0,
                 max_bonds: int = 2, dt: float = 0.005, gamma: float = 1.0, kT: float = 1.0, mass: float = 1.0,
                 seed: int = 0, resort_every: int = 0, flags: int = 0, integrator: int = 0,
-                charge: Sequence[float] = (), bjerrum: float = 0.0, a_charge: float = 0.5) -> Params:
+                charge: Sequence[float] = (), bjerrum: float = 0.0, a_charge: float = 0.5,
+                lambda_wlc: float = 0.0) -> Params:
     p = Params()
     p.struct_size = C.sizeof(Params)
     p.n, p.n_species, p.order = int(n), int(n_species), int(order)
@@ -71,6 +73,7 @@ def make_params(n: int, n_species: int, box: Sequence[float], grid: Sequence[int
     for i, z in enumerate(charge):
         p.charge[i] = float(z)
     p.bjerrum, p.a_charge = float(bjerrum), float(a_charge)
+    p.lambda_wlc = float(lambda_wlc)
     return p
 
 

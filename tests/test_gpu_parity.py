@@ -641,3 +641,33 @@ def test_coacervate_sized_charged_melt_force_and_steps():
     x = eng.tild_get_state(want_v=False)[0].cpu().numpy().astype(np.float64)
     ox, _, _ = orc.run(p, st.x.astype(np.float64), st.v.astype(np.float64), st.type, st.bond_partner, 0, 20, f=of)
     assert np.abs(min_image(x - ox, cfg.box)).max() <= 1e-4
+
+
+def test_wlc_angle_potential_parity():
+    """Cosine angle potential (Eq. 16; reading A23) in the bond stage, the fused step and tild_energy."""
+    cfg = small_cfg(order=3, n_chains=120, nb=12)
+    lam = 2.5
+    st, eng = make(cfg, resort_every=4, lambda_wlc=lam)
+    p = oracle_params(cfg, lambda_wlc=lam)
+    fb = eng.tild_bond_force(dev(st.x), dev(st.bond_partner)).cpu().numpy()
+    ofb = orc.bond_force(p, st.x.astype(np.float64), st.bond_partner)
+    assert np.abs(fb - ofb).max() <= 2e-5 * vec_rms(ofb)        # fp32 cancellation in d/|d|^3 terms of near-straight triplets
+    plain = orc.bond_force(oracle_params(cfg), st.x.astype(np.float64), st.bond_partner)
+    assert np.abs(ofb - plain).max() > 0.1 * vec_rms(plain)      # the angles really contribute
+    eng.tild_set_state(dev(st.x), dev(st.v), dev(st.type), dev(st.bond_partner), 0)
+    _, _, f, _ = eng.tild_get_state(want_v=False, want_f=True)
+    of = orc.force(p, st.x.astype(np.float64), st.type, st.bond_partner)
+    assert np.abs(f.cpu().numpy() - of).max() <= 2e-5 * vec_rms(of)
+    e = eng.tild_energy()
+    oe = orc.energy(p, st.x.astype(np.float64), st.v.astype(np.float64), st.type, st.bond_partner)
+    assert np.all(np.abs(e - oe) <= 2e-5 * np.abs(oe).max()), (e, oe)
+    eng.tild_step(50)
+    x = eng.tild_get_state(want_v=False)[0].cpu().numpy().astype(np.float64)
+    ox, _, _ = orc.run(p, st.x.astype(np.float64), st.v.astype(np.float64), st.type, st.bond_partner, 0, 50, f=of)
+    assert np.abs(min_image(x - ox, cfg.box)).max() <= 1e-4
+
+
+def test_wlc_needs_linear_chain_tables():
+    cfg = small_cfg(order=2)
+    with pytest.raises(tild.TildError):
+        tild.Tild(tild.params_from_config(cfg, lambda_wlc=1.0, max_bonds=3))
