@@ -95,6 +95,9 @@ typedef struct {
     /* cosine (wormlike-chain) angle potential lambda [1 + cos(theta_ijk)], Eq. 16; 0 = none.  Needs
      * max_bonds == 2: the triplets are (partner slot 0, bead, partner slot 1) of every bead with both (A23) */
     double lambda_wlc;
+    /* harmonic angle potential k_theta (theta_ijk - theta0)^2, Eq. 17, on the same triplets; k_theta = 0:
+     * none; theta0 in [0, pi].  The force is singular at sin(theta) = 0 and that term is dropped there */
+    double k_theta, theta0;
 } tild_params;
 
 /* HOST. Bytes of device workspace tild_init needs for these parameters. */

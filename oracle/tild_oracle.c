@@ -50,6 +50,7 @@ typedef struct {
     double dt, gamma, kT, mass;
     uint64_t seed;
     double lambda_wlc;  /* stiffness of the cosine angle potential, Eq. 16; 0 = no angles (A23) */
+    double k_theta, theta0; /* harmonic angle potential k_theta (theta - theta0)^2, Eq. 17; 0 = none */
     double charge[ORC_MAX_SPECIES]; /* valence of each species (reading A22) */
     double bjerrum;     /* l_B >= 0; 0 switches electrostatics off */
     double a_charge;    /* Gaussian smearing length of a charge (same form as h) */
@@ -550,6 +551,29 @@ static double orc_min_image(double d, double L)
     return d - L * floor(d / L + 0.5);
 }
 
+/* Angle potentials as functions of c = cos(theta_ijk), theta the inside angle at j (Eq. 16-17):
+ *   U(c) = lambda (1 + c) + k_theta (acos(c) - theta0)^2,
+ *   dU/dc = lambda - 2 k_theta (theta - theta0) / sin(theta)      (d theta / d c = -1 / sin theta).
+ * At sin(theta) -> 0 the harmonic term is singular unless theta -> theta0 there; it is dropped below 1e-9. */
+static double orc_angle_energy(const orc_params *p, double c)
+{
+    if (c > 1.0) c = 1.0;
+    if (c < -1.0) c = -1.0;
+    const double th = acos(c);
+    return p->lambda_wlc * (1.0 + c) + p->k_theta * (th - p->theta0) * (th - p->theta0);
+}
+static double orc_angle_dUdc(const orc_params *p, double c)
+{
+    if (c > 1.0) c = 1.0;
+    if (c < -1.0) c = -1.0;
+    double coef = p->lambda_wlc;
+    if (p->k_theta != 0.0) {
+        const double sn = sqrt(1.0 - c * c);
+        if (sn > 1e-9) coef -= 2.0 * p->k_theta * (acos(c) - p->theta0) / sn;
+    }
+    return coef;
+}
+
 void orc_bond_force(const orc_params *p, const double *x, const int32_t *partner, double *f)
 {
 #pragma omp parallel for schedule(static)
@@ -574,7 +598,7 @@ void orc_bond_force(const orc_params *p, const double *x, const int32_t *partner
      * i and k.  Reading A23: for linear chains (max_bonds = 2) the triplets are (partner slot 0, j, partner slot 1) of
      * every bead j that has both.  cos(theta) = d1.d2 / (|d1| |d2|), d1 = r_i - r_j, d2 = r_k - r_j (minimum image);
      * F_i = -lambda d cos/d r_i, F_k likewise, F_j = -(F_i + F_k).  Serial loop: each angle adds to its three beads. */
-    if (p->lambda_wlc != 0.0 && p->max_bonds == 2) {
+    if ((p->lambda_wlc != 0.0 || p->k_theta != 0.0) && p->max_bonds == 2) {
         for (int j = 0; j < p->n; ++j) {
             int32_t i = partner[2 * (size_t)j], k = partner[2 * (size_t)j + 1];
             if (i < 0 || k < 0) continue;
@@ -588,11 +612,12 @@ void orc_bond_force(const orc_params *p, const double *x, const int32_t *partner
             }
             if (n1 == 0.0 || n2 == 0.0) continue;
             double inv = 1.0 / sqrt(n1 * n2), c = dot * inv;
+            const double coef = orc_angle_dUdc(p, c);        /* F = -dU/dc * dc/dr */
             for (int a = 0; a < 3; ++a) {
                 double gi = d2[a] * inv - c * d1[a] / n1, gk = d1[a] * inv - c * d2[a] / n2;
-                f[3 * (size_t)i + a] -= p->lambda_wlc * gi;
-                f[3 * (size_t)k + a] -= p->lambda_wlc * gk;
-                f[3 * (size_t)j + a] += p->lambda_wlc * (gi + gk);
+                f[3 * (size_t)i + a] -= coef * gi;
+                f[3 * (size_t)k + a] -= coef * gk;
+                f[3 * (size_t)j + a] += coef * (gi + gk);
             }
         }
     }
@@ -814,7 +839,7 @@ void orc_energy(const orc_params *p, const double *x, const double *v, const int
     free(utab_e);
     free(nhat);
     e[0] = ke;
-    if (p->lambda_wlc != 0.0 && p->max_bonds == 2) {   /* Eq. 16: sum over angles of lambda (1 + cos theta) */
+    if ((p->lambda_wlc != 0.0 || p->k_theta != 0.0) && p->max_bonds == 2) {   /* Eq. 16-17: sum over angles of U(cos theta) */
         for (int j = 0; j < p->n; ++j) {
             int32_t i = partner[2 * (size_t)j], k = partner[2 * (size_t)j + 1];
             if (i < 0 || k < 0) continue;
@@ -826,7 +851,7 @@ void orc_energy(const orc_params *p, const double *x, const double *v, const int
                 n2 += d2 * d2;
                 dot += d1 * d2;
             }
-            if (n1 > 0.0 && n2 > 0.0) be += p->lambda_wlc * (1.0 + dot / sqrt(n1 * n2));
+            if (n1 > 0.0 && n2 > 0.0) be += orc_angle_energy(p, dot / sqrt(n1 * n2));
         }
     }
     e[1] = be;

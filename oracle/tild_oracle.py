@@ -41,7 +41,7 @@ class _Params(C.Structure):
         ("max_bonds", C.c_int32),
         ("dt", C.c_double), ("gamma", C.c_double), ("kT", C.c_double), ("mass", C.c_double),
         ("seed", C.c_uint64),
-        ("lambda_wlc", C.c_double),
+        ("lambda_wlc", C.c_double), ("k_theta", C.c_double), ("theta0", C.c_double),
         ("charge", C.c_double * MAX_SPECIES), ("bjerrum", C.c_double), ("a_charge", C.c_double),
         ("integrator", C.c_int32),
         ("sampled_kernel", C.c_int32),
@@ -70,6 +70,8 @@ class OracleParams:
     mass: float = 1.0
     seed: int = 0
     lambda_wlc: float = 0.0    # cosine angle potential lambda (1 + cos theta), Eq. 16; linear chains (A23)
+    k_theta: float = 0.0       # harmonic angle potential k_theta (theta - theta0)^2, Eq. 17
+    theta0: float = 0.0
     charge: tuple = ()         # valence per species (reading A22); bjerrum = 0 switches electrostatics off
     bjerrum: float = 0.0
     a_charge: float = 0.5
@@ -96,6 +98,7 @@ class OracleParams:
         p.dt, p.gamma, p.kT, p.mass = float(self.dt), float(self.gamma), float(self.kT), float(self.mass)
         p.seed = int(self.seed)
         p.lambda_wlc = float(self.lambda_wlc)
+        p.k_theta, p.theta0 = float(self.k_theta), float(self.theta0)
         for i, z in enumerate(self.charge):
             p.charge[i] = float(z)
         p.bjerrum, p.a_charge = float(self.bjerrum), float(self.a_charge)

@@ -56,7 +56,8 @@ int validate(const tild_params* p)
     if (!(p->dt > 0.0) || !(p->mass > 0.0) || p->gamma < 0.0 || p->kT < 0.0) return TILD_EINVAL;
     if (p->integrator != TILD_INTEGRATOR_GJF && p->integrator != TILD_INTEGRATOR_EM) return TILD_EINVAL;
     if (p->integrator == TILD_INTEGRATOR_EM && !(p->gamma > 0.0)) return TILD_EINVAL;
-    if (p->lambda_wlc != 0.0 && p->max_bonds != 2) return TILD_EINVAL;
+    if ((p->lambda_wlc != 0.0 || p->k_theta != 0.0) && p->max_bonds != 2) return TILD_EINVAL;
+    if (!(p->k_theta >= 0.0) || !(p->theta0 >= 0.0 && p->theta0 <= 3.141592653589794)) return TILD_EINVAL;
     if (p->bjerrum < 0.0 || (p->bjerrum > 0.0 && !(p->a_charge > 0.0))) return TILD_EINVAL;
     return TILD_OK;
 }
@@ -327,6 +328,8 @@ int tild_init(tild_ctx** out, const tild_params* params, void* workspace, size_t
     s.r0_bond = (float)p.r0_bond;
     s.max_bonds = p.max_bonds;
     s.lambda_wlc = (p.max_bonds == 2) ? (float)p.lambda_wlc : 0.0f;
+    s.k_theta = (p.max_bonds == 2) ? (float)p.k_theta : 0.0f;
+    s.theta0 = (float)p.theta0;
     s.integrator = p.integrator;
     s.em_drift = p.gamma > 0.0 ? (float)(p.dt / p.gamma) : 0.0f;
     s.em_noise = p.gamma > 0.0 ? (float)(1.0 / p.gamma) : 0.0f;

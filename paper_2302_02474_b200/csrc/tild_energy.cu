@@ -73,7 +73,7 @@ __global__ void __launch_bounds__(256) particle_energy_kernel(MeshParams m, Step
             const double d = sqrt(dx * dx + dy * dy + dz * dz) - (double)s.r0_bond;
             eb += (double)s.k_bond * d * d;
         }
-        if (s.lambda_wlc != 0.0f) {   // Eq. 16: lambda (1 + cos theta), counted by the angle's centre bead
+        if (s.lambda_wlc != 0.0f || s.k_theta != 0.0f) {   // Eq. 16-17, counted by the angle's centre bead
             const int2 bb = *reinterpret_cast<const int2*>(B + 2 * slot);
             if (bb.x >= 0 && bb.y >= 0) {
                 const float4 a = X4[bb.x], c = X4[bb.y];
@@ -84,7 +84,10 @@ __global__ void __launch_bounds__(256) particle_energy_kernel(MeshParams m, Step
                 const double n1 = (double)d1[0] * d1[0] + (double)d1[1] * d1[1] + (double)d1[2] * d1[2];
                 const double n2 = (double)d2[0] * d2[0] + (double)d2[1] * d2[1] + (double)d2[2] * d2[2];
                 const double dot = (double)d1[0] * d2[0] + (double)d1[1] * d2[1] + (double)d1[2] * d2[2];
-                if (n1 > 0.0 && n2 > 0.0) eb += (double)s.lambda_wlc * (1.0 + dot / sqrt(n1 * n2));
+                if (n1 > 0.0 && n2 > 0.0) {
+                    const double cs = fmin(1.0, fmax(-1.0, dot / sqrt(n1 * n2))), dth = acos(cs) - (double)s.theta0;
+                    eb += (double)s.lambda_wlc * (1.0 + cs) + (double)s.k_theta * dth * dth;
+                }
             }
         }
     }

@@ -72,6 +72,7 @@ struct StepParams {
     int max_bonds;
     uint32_t key0, key1;   // Philox key = seed lo, hi
     float lambda_wlc;      // cosine angle potential, Eq. 16 (0 = none; needs max_bonds == 2)
+    float k_theta, theta0; // harmonic angle potential k_theta (theta - theta0)^2, Eq. 17 (0 = none; same triplets)
     int integrator;        // TILD_INTEGRATOR_*
     float em_drift;        // dt/gamma
     float em_noise;        // 1/gamma (times beta = noise_amp * z)
@@ -307,8 +308,9 @@ __device__ __forceinline__ float min_image(float d, float L, float inv_L)
 
 // Gradients of cos(theta) = d1.d2 / (|d1| |d2|) with respect to the end points of d1 and d2 (Eq. 16):
 // gi = d cos / d r_i = d2 / (|d1||d2|) - cos d1 / |d1|^2,  gk likewise;  d cos / d r_j = -(gi + gk).  Returns cos.
-__device__ __forceinline__ float cos_gradients(const float d1[3], const float d2[3], float gi[3], float gk[3])
+__device__ __forceinline__ float cos_gradients(const float d1[3], const float d2[3], float gi[3], float gk[3], float& sn)
 {
+    sn = 0.0f;
     const float n1 = d1[0] * d1[0] + d1[1] * d1[1] + d1[2] * d1[2], n2 = d2[0] * d2[0] + d2[1] * d2[1] + d2[2] * d2[2];
     if (!(n1 > 0.0f) || !(n2 > 0.0f)) {
         gi[0] = gi[1] = gi[2] = gk[0] = gk[1] = gk[2] = 0.0f;
@@ -316,6 +318,8 @@ __device__ __forceinline__ float cos_gradients(const float d1[3], const float d2
     }
     const float inv = rsqrtf(n1) * rsqrtf(n2), c = (d1[0] * d2[0] + d1[1] * d2[1] + d1[2] * d2[2]) * inv;
     const float c1 = c / n1, c2 = c / n2;
+    const float cx = d1[1] * d2[2] - d1[2] * d2[1], cy = d1[2] * d2[0] - d1[0] * d2[2], cz = d1[0] * d2[1] - d1[1] * d2[0];
+    sn = sqrtf(cx * cx + cy * cy + cz * cz) * inv;    // sin(theta) from the cross product: no cancellation near 0 and pi
 #pragma unroll
     for (int a = 0; a < 3; ++a) {
         gi[a] = d2[a] * inv - c1 * d1[a];
@@ -324,24 +328,35 @@ __device__ __forceinline__ float cos_gradients(const float d1[3], const float d2
     return c;
 }
 
-// Force of the cosine angle potential on the bead at r with neighbours: prev / next (either may be missing) and their
+// dU/d(cos theta) of U = lambda (1 + cos theta) + k_theta (theta - theta0)^2 (Eq. 16-17):
+// lambda - 2 k_theta (theta - theta0) / sin theta, theta = atan2(sin, cos).  The harmonic term is singular at
+// sin theta -> 0 (unless theta0 is that angle) and is dropped there.
+__device__ __forceinline__ float angle_dUdc(float lambda, float k_theta, float theta0, float c, float sn)
+{
+    float coef = lambda;
+    if (k_theta != 0.0f && sn > 1e-6f) coef -= 2.0f * k_theta * (atan2f(sn, c) - theta0) / sn;
+    return coef;
+}
+
+// Force of the angle potentials on the bead at r with neighbours: prev / next (either may be missing) and their
 // own outer neighbours pprev / nnext.  has_* say which exist.  Each bead computes its own share of the (up to) three
 // angles it belongs to, without Newton's third law (as the paper does for bonds, L209).
-__device__ __forceinline__ void wlc_angle_force(float lambda, const float L[3], const float inv_L[3], const float r[3],
+__device__ __forceinline__ void wlc_angle_force(float lambda, float k_theta, float theta0, const float L[3], const float inv_L[3], const float r[3],
                                                 bool has_prev, const float prev[3], bool has_pprev, const float pprev[3],
                                                 bool has_next, const float next[3], bool has_nnext, const float nnext[3],
                                                 float f[3])
 {
-    float d1[3], d2[3], gi[3], gk[3];
+    float d1[3], d2[3], gi[3], gk[3], sn, c, coef;
     if (has_prev && has_next) {          // centre bead of (prev, r, next)
 #pragma unroll
         for (int a = 0; a < 3; ++a) {
             d1[a] = min_image(prev[a] - r[a], L[a], inv_L[a]);
             d2[a] = min_image(next[a] - r[a], L[a], inv_L[a]);
         }
-        cos_gradients(d1, d2, gi, gk);
+        c = cos_gradients(d1, d2, gi, gk, sn);
+        coef = angle_dUdc(lambda, k_theta, theta0, c, sn);
 #pragma unroll
-        for (int a = 0; a < 3; ++a) f[a] += lambda * (gi[a] + gk[a]);
+        for (int a = 0; a < 3; ++a) f[a] += coef * (gi[a] + gk[a]);
     }
     if (has_prev && has_pprev) {         // end bead k of (pprev, prev, r)
 #pragma unroll
@@ -349,9 +364,10 @@ __device__ __forceinline__ void wlc_angle_force(float lambda, const float L[3], 
             d1[a] = min_image(pprev[a] - prev[a], L[a], inv_L[a]);
             d2[a] = min_image(r[a] - prev[a], L[a], inv_L[a]);
         }
-        cos_gradients(d1, d2, gi, gk);
+        c = cos_gradients(d1, d2, gi, gk, sn);
+        coef = angle_dUdc(lambda, k_theta, theta0, c, sn);
 #pragma unroll
-        for (int a = 0; a < 3; ++a) f[a] -= lambda * gk[a];
+        for (int a = 0; a < 3; ++a) f[a] -= coef * gk[a];
     }
     if (has_next && has_nnext) {         // end bead i of (r, next, nnext)
 #pragma unroll
@@ -359,9 +375,10 @@ __device__ __forceinline__ void wlc_angle_force(float lambda, const float L[3], 
             d1[a] = min_image(r[a] - next[a], L[a], inv_L[a]);
             d2[a] = min_image(nnext[a] - next[a], L[a], inv_L[a]);
         }
-        cos_gradients(d1, d2, gi, gk);
+        c = cos_gradients(d1, d2, gi, gk, sn);
+        coef = angle_dUdc(lambda, k_theta, theta0, c, sn);
 #pragma unroll
-        for (int a = 0; a < 3; ++a) f[a] -= lambda * gi[a];
+        for (int a = 0; a < 3; ++a) f[a] -= coef * gi[a];
     }
 }
 

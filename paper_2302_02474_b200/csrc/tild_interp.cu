@@ -134,7 +134,7 @@ __device__ __forceinline__ void angle_force_slots(const MeshParams& m, const Ste
         }
     }
     float fa[3] = {0.f, 0.f, 0.f};
-    wlc_angle_force(s.lambda_wlc, m.L, m.inv_L, r, bb.x >= 0, prev, has_pprev, pprev, bb.y >= 0, next, has_nnext, nnext, fa);
+    wlc_angle_force(s.lambda_wlc, s.k_theta, s.theta0, m.L, m.inv_L, r, bb.x >= 0, prev, has_pprev, pprev, bb.y >= 0, next, has_nnext, nnext, fa);
     f.x += fa[0];
     f.y += fa[1];
     f.z += fa[2];
@@ -149,7 +149,7 @@ __device__ __forceinline__ float3 bond_force_slots(const MeshParams& m, const St
         const int32_t j = B[slot * s.max_bonds + k];
         if (j >= 0) bond_term(m, s, p, X4[j], f);
     }
-    if (s.lambda_wlc != 0.0f) angle_force_slots(m, s, X4, B, slot, p, f);
+    if (s.lambda_wlc != 0.0f || s.k_theta != 0.0f) angle_force_slots(m, s, X4, B, slot, p, f);
     return f;
 }
 
@@ -445,7 +445,7 @@ __global__ void __launch_bounds__(INTERP_THREADS, 2) interp_tile_kernel(MeshPara
                     if (s.max_bonds <= 2) {
                         if (bj0 >= 0) bond_term(m, s, p, q0, F);
                         if (bj1 >= 0) bond_term(m, s, p, q1, F);
-                        if (s.lambda_wlc != 0.0f) angle_force_slots(m, s, X4, B, slot, p, F);
+                        if (s.lambda_wlc != 0.0f || s.k_theta != 0.0f) angle_force_slots(m, s, X4, B, slot, p, F);
                     } else {
                         const float3 fb = bond_force_slots(m, s, X4, B, slot, p);
                         F.x += fb.x;
@@ -515,7 +515,7 @@ __global__ void __launch_bounds__(256) bond_force_kernel(MeshParams m, StepParam
         acc.y += scale * dy;
         acc.z += scale * dz;
     }
-    if (s.lambda_wlc != 0.0f) {   // cosine angles, Eq. 16 (max_bonds == 2: slot 0 = previous, slot 1 = next bead)
+    if (s.lambda_wlc != 0.0f || s.k_theta != 0.0f) {   // angles, Eq. 16-17 (max_bonds == 2: slot 0 = previous, slot 1 = next bead)
         const int32_t jp = bond[2 * (size_t)i], jn = bond[2 * (size_t)i + 1];
         const float r[3] = {px, py, pz};
         float prev[3] = {0.f, 0.f, 0.f}, next[3] = {0.f, 0.f, 0.f}, pprev[3] = {0.f, 0.f, 0.f}, nnext[3] = {0.f, 0.f, 0.f};
@@ -537,7 +537,7 @@ __global__ void __launch_bounds__(256) bond_force_kernel(MeshParams m, StepParam
             }
         }
         float fa[3] = {0.f, 0.f, 0.f};
-        wlc_angle_force(s.lambda_wlc, m.L, m.inv_L, r, jp >= 0, prev, has_pprev, pprev, jn >= 0, next, has_nnext, nnext, fa);
+        wlc_angle_force(s.lambda_wlc, s.k_theta, s.theta0, m.L, m.inv_L, r, jp >= 0, prev, has_pprev, pprev, jn >= 0, next, has_nnext, nnext, fa);
         acc.x += fa[0];
         acc.y += fa[1];
         acc.z += fa[2];

@@ -44,6 +44,8 @@ class Params(C.Structure):
         ("integrator", C.c_int32), ("reserved", C.c_int32),
         ("charge", C.c_double * MAX_SPECIES), ("bjerrum", C.c_double), ("a_charge", C.c_double),
         ("lambda_wlc", C.c_double),
+        ("k_theta", C.c_double),
+        ("theta0", C.c_double),
     ]
 
 
@@ -52,7 +54,7 @@ def make_params(n: int, n_species: int, box: Sequence[float], grid: Sequence[int
                 max_bonds: int = 2, dt: float = 0.005, gamma: float = 1.0, kT: float = 1.0, mass: float = 1.0,
                 seed: int = 0, resort_every: int = 0, flags: int = 0, integrator: int = 0,
                 charge: Sequence[float] = (), bjerrum: float = 0.0, a_charge: float = 0.5,
-                lambda_wlc: float = 0.0) -> Params:
+                lambda_wlc: float = 0.0, k_theta: float = 0.0, theta0: float = 0.0) -> Params:
     p = Params()
     p.struct_size = C.sizeof(Params)
     p.n, p.n_species, p.order = int(n), int(n_species), int(order)
@@ -74,6 +76,7 @@ def make_params(n: int, n_species: int, box: Sequence[float], grid: Sequence[int
         p.charge[i] = float(z)
     p.bjerrum, p.a_charge = float(bjerrum), float(a_charge)
     p.lambda_wlc = float(lambda_wlc)
+    p.k_theta, p.theta0 = float(k_theta), float(theta0)
     return p
 
 

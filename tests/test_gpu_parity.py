@@ -667,7 +667,38 @@ def test_wlc_angle_potential_parity():
     assert np.abs(min_image(x - ox, cfg.box)).max() <= 1e-4
 
 
+def test_harmonic_angle_potential_parity():
+    """Harmonic angle potential k_theta (theta - theta0)^2 (Eq. 17) together with the cosine one, in the
+    bond stage, the fused step and tild_energy.  The 1/sin(theta) factor makes a few near-straight triplets carry forces
+    far above the RMS, so the absolute bound is the relative fp32 error of those: 1e-4 of the RMS."""
+    cfg = small_cfg(order=3, n_chains=120, nb=12)
+    kw = dict(k_theta=1.2, theta0=2.0, lambda_wlc=0.5)
+    st, eng = make(cfg, resort_every=4, **kw)
+    p = oracle_params(cfg, **kw)
+    fb = eng.tild_bond_force(dev(st.x), dev(st.bond_partner)).cpu().numpy()
+    ofb = orc.bond_force(p, st.x.astype(np.float64), st.bond_partner)
+    assert np.abs(fb - ofb).max() <= 1e-4 * vec_rms(ofb)
+    assert np.abs(fb - ofb).max() <= 2e-5 * np.abs(ofb).max()
+    wlc_only = orc.bond_force(oracle_params(cfg, lambda_wlc=0.5), st.x.astype(np.float64), st.bond_partner)
+    assert np.abs(ofb - wlc_only).max() > 0.1 * vec_rms(wlc_only)
+    eng.tild_set_state(dev(st.x), dev(st.v), dev(st.type), dev(st.bond_partner), 0)
+    _, _, f, _ = eng.tild_get_state(want_v=False, want_f=True)
+    of = orc.force(p, st.x.astype(np.float64), st.type, st.bond_partner)
+    assert np.abs(f.cpu().numpy() - of).max() <= 1e-4 * vec_rms(of)
+    e = eng.tild_energy()
+    oe = orc.energy(p, st.x.astype(np.float64), st.v.astype(np.float64), st.type, st.bond_partner)
+    assert np.all(np.abs(e - oe) <= 2e-5 * np.abs(oe).max()), (e, oe)
+    eng.tild_step(30)
+    x = eng.tild_get_state(want_v=False)[0].cpu().numpy().astype(np.float64)
+    ox, _, _ = orc.run(p, st.x.astype(np.float64), st.v.astype(np.float64), st.type, st.bond_partner, 0, 30, f=of)
+    assert np.abs(min_image(x - ox, cfg.box)).max() <= 1e-4
+
+
 def test_wlc_needs_linear_chain_tables():
     cfg = small_cfg(order=2)
+    with pytest.raises(tild.TildError):
+        tild.Tild(tild.params_from_config(cfg, k_theta=1.0, theta0=2.0, max_bonds=3))
+    with pytest.raises(tild.TildError):
+        tild.Tild(tild.params_from_config(cfg, k_theta=1.0, theta0=4.0))
     with pytest.raises(tild.TildError):
         tild.Tild(tild.params_from_config(cfg, lambda_wlc=1.0, max_bonds=3))

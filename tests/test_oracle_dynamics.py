@@ -305,3 +305,35 @@ def test_wlc_angle_special_cases():
     F = orc.bond_force(p, right, bp)
     assert abs(orc.energy(p, right, v, ty, bp)[1] - 1.7) < 1e-12
     assert np.allclose(F[0], [-1.7, 0, 0]) and np.allclose(F[2], [0, -1.7, 0]) and np.allclose(F[1], [1.7, 1.7, 0])
+
+
+def test_harmonic_angle_force_is_minus_the_energy_gradient_and_special_cases():
+    """PAPER.md Eq. 17: u_h = k_theta (theta - theta0)^2.  Gradient check, conservation laws, and a right-angle
+    trimer with theta0 = pi/3: U = k (pi/2 - pi/3)^2, end-bead force magnitude 2 k (theta - theta0) / |d|, opening."""
+    rng = np.random.default_rng(15)
+    n_chains, nb, L = 3, 6, (7.0, 8.0, 9.0)
+    n = n_chains * nb
+    x = (rng.random((n_chains, 1, 3)) * np.array(L) + np.cumsum(rng.normal(0, 0.6, (n_chains, nb, 3)), axis=1)).reshape(-1, 3)
+    x -= np.array(L) * np.floor(x / np.array(L))
+    bp = _chain_partners(n_chains, nb)
+    p = orc.OracleParams(n, 1, L, (8, 8, 8), 2, np.zeros((1, 1)), 0.0, 0.5, k_bond=0.0, k_theta=1.3, theta0=2.0, lambda_wlc=0.4)
+    F = orc.bond_force(p, x, bp)
+    ty, v = np.zeros(n, np.int32), np.zeros((n, 3))
+    eps = 1e-6
+    for i in (0, 2, 6, 8, 11, 16):
+        for a in range(3):
+            xp, xm = x.copy(), x.copy()
+            xp[i, a] += eps
+            xm[i, a] -= eps
+            dE = (orc.energy(p, xp, v, ty, bp)[1] - orc.energy(p, xm, v, ty, bp)[1]) / (2 * eps)
+            assert abs(F[i, a] + dE) < 2e-6 * max(1.0, np.abs(F).max()), (i, a, F[i, a], -dE)
+    assert np.abs(F.sum(0)).max() < 1e-12 * max(1.0, np.abs(F).max())
+    q = orc.OracleParams(3, 1, (20.0,) * 3, (8, 8, 8), 2, np.zeros((1, 1)), 0.0, 0.5, k_bond=0.0, k_theta=1.5, theta0=np.pi / 3)
+    right = np.array([[5.0, 6, 5], [5.0, 5, 5], [6.0, 5, 5]])
+    b3 = _chain_partners(1, 3)
+    assert abs(orc.energy(q, right, np.zeros((3, 3)), np.zeros(3, np.int32), b3)[1] - 1.5 * (np.pi / 6) ** 2) < 1e-12
+    Fr = orc.bond_force(q, right, b3)
+    mag = 2 * 1.5 * (np.pi / 2 - np.pi / 3)
+    assert np.allclose(Fr[0], [mag, 0, 0]) and np.allclose(Fr[2], [0, mag, 0]) and np.allclose(Fr[1], [-mag, -mag, 0])
+    at_rest = orc.OracleParams(3, 1, (20.0,) * 3, (8, 8, 8), 2, np.zeros((1, 1)), 0.0, 0.5, k_bond=0.0, k_theta=1.5, theta0=np.pi / 2)
+    assert np.abs(orc.bond_force(at_rest, right, b3)).max() < 1e-12
