@@ -141,7 +141,7 @@ void carve(tild_ctx* c, void* base, size_t* total)
     c->drift_count = w.take<uint32_t>(4);
     c->d_step = w.take<uint64_t>(2);
     c->d_energy = w.take<double>(4);
-    c->tables = w.take<float>(12 * 4096);
+    c->tables = w.take<float>(14 * 4096);
     *total = w.off;
 }
 
@@ -163,20 +163,39 @@ __global__ void __launch_bounds__(256) gather_by_inv_kernel(int n, const uint32_
     out[3 * (size_t)i + 2] = f.z;
 }
 
+// R2C -> k-space multiplication -> C2R.  With the fused x-transform (xfft_R) cuFFT runs over (y, z) only and
+// kspace_xfft_kernel does the x transforms around the multiplication; otherwise 3-D plans and kspace_kernel.
+int kspace_pipeline(tild_ctx* c, const float* grid, float* ffield, cudaEvent_t* ev)
+{
+    int rc;
+    cufftComplex* nh = reinterpret_cast<cufftComplex*>(c->nhat);
+    cufftComplex* fh = reinterpret_cast<cufftComplex*>(c->fhat);
+    if (c->xfft_R) {
+        TILD_FFT(c, cufftExecR2C(c->plan_r2c_yz, const_cast<float*>(grid), nh));
+        if (ev) cudaEventRecord(ev[3], c->stream);
+        rc = launch_kspace_xfft(c, c->nhat, c->fhat);
+        if (rc) return rc;
+        if (ev) cudaEventRecord(ev[4], c->stream);
+        TILD_FFT(c, cufftExecC2R(c->plan_c2r_yz, fh, ffield));
+    } else {
+        TILD_FFT(c, cufftExecR2C(c->plan_r2c, const_cast<float*>(grid), nh));
+        if (ev) cudaEventRecord(ev[3], c->stream);
+        rc = launch_kspace(c, c->nhat, c->fhat);
+        if (rc) return rc;
+        if (ev) cudaEventRecord(ev[4], c->stream);
+        TILD_FFT(c, cufftExecC2R(c->plan_c2r, fh, ffield));
+    }
+    if (ev) cudaEventRecord(ev[5], c->stream);
+    return TILD_OK;
+}
+
 // spread -> R2C -> k-space -> C2R on slab-ordered particles, with optional stage events
 int mesh_pipeline(tild_ctx* c, const SegLayout& lay, const float4* X4, cudaEvent_t* ev)
 {
     int rc = launch_spread(c, lay, X4, c->grid);
     if (rc) return rc;
     if (ev) cudaEventRecord(ev[2], c->stream);
-    TILD_FFT(c, cufftExecR2C(c->plan_r2c, c->grid, reinterpret_cast<cufftComplex*>(c->nhat)));
-    if (ev) cudaEventRecord(ev[3], c->stream);
-    rc = launch_kspace(c, c->nhat, c->fhat);
-    if (rc) return rc;
-    if (ev) cudaEventRecord(ev[4], c->stream);
-    TILD_FFT(c, cufftExecC2R(c->plan_c2r, reinterpret_cast<cufftComplex*>(c->fhat), c->ffield));
-    if (ev) cudaEventRecord(ev[5], c->stream);
-    return TILD_OK;
+    return kspace_pipeline(c, c->grid, c->ffield, ev);
 }
 
 // total force at the current internal positions -> c->F4 (per slot); no state change
@@ -254,7 +273,7 @@ int tild_init(tild_ctx** out, const tild_params* params, void* workspace, size_t
     }
 
     // a0: k-space tables in double on the host (A4-A6), uploaded as fp32
-    std::vector<float> tab(12 * 4096, 0.0f);
+    std::vector<float> tab(14 * 4096, 0.0f);
     const double PI = 3.14159265358979323846264338327950288;
     for (int a = 0; a < 3; ++a) {
         const int N = p.grid[a];
@@ -294,6 +313,16 @@ int tild_init(tild_ctx** out, const tild_params* params, void* workspace, size_t
             tab[(size_t)(6 + a) * 4096 + mm] = (float)e;
             tab[(size_t)(9 + a) * 4096 + mm] = (float)(k * k);
         }
+    }
+    for (int j = 0; j < p.grid[0]; ++j) {      // x twiddles of the fused x-transform kernel
+        const double ang = 2.0 * PI * (double)j / (double)p.grid[0];
+        tab[(size_t)12 * 4096 + 2 * j] = (float)cos(ang);
+        tab[(size_t)12 * 4096 + 2 * j + 1] = (float)(-sin(ang));
+    }
+    c->xtw = reinterpret_cast<const float2*>(c->tables + (size_t)12 * 4096);
+    {
+        const char* env = getenv("TILD_XFFT");   // 0 forces the 3-D cuFFT plans + separate k-space kernel (A/B runs)
+        c->xfft_R = (env && env[0] == '0') ? 0 : kspace_xfft_radix(p.grid[0], S);
     }
     KspaceParams& ks = c->ksp;
     ks.S = S;
@@ -343,23 +372,40 @@ int tild_init(tild_ctx** out, const tild_params* params, void* workspace, size_t
         return TILD_ECUDA;
     }
     int dims[3] = {p.grid[0], p.grid[1], p.grid[2]};
-    cufftResult r1 = cufftPlanMany(&c->plan_r2c, 3, dims, nullptr, 1, 0, nullptr, 1, 0, CUFFT_R2C, S);
-    cufftResult r2 = r1 == CUFFT_SUCCESS ? cufftPlanMany(&c->plan_c2r, 3, dims, nullptr, 1, 0, nullptr, 1, 0, CUFFT_C2R, 3 * S)
-                                         : CUFFT_INTERNAL_ERROR;
-    if (r1 != CUFFT_SUCCESS || r2 != CUFFT_SUCCESS) {
-        if (r1 == CUFFT_SUCCESS) cufftDestroy(c->plan_r2c);
+    cufftHandle* plans[4] = {&c->plan_r2c, &c->plan_c2r, &c->plan_r2c_yz, &c->plan_c2r_yz};
+    bool made[4] = {false, false, false, false};
+    cufftResult fr = cufftPlanMany(&c->plan_r2c, 3, dims, nullptr, 1, 0, nullptr, 1, 0, CUFFT_R2C, S);
+    made[0] = fr == CUFFT_SUCCESS;
+    if (fr == CUFFT_SUCCESS && !c->xfft_R) {
+        fr = cufftPlanMany(&c->plan_c2r, 3, dims, nullptr, 1, 0, nullptr, 1, 0, CUFFT_C2R, 3 * S);
+        made[1] = fr == CUFFT_SUCCESS;
+    }
+    if (fr == CUFFT_SUCCESS && c->xfft_R) {   // contiguous (y, z) planes: batch = planes of all species / components
+        fr = cufftPlanMany(&c->plan_r2c_yz, 2, dims + 1, nullptr, 1, 0, nullptr, 1, 0, CUFFT_R2C, S * p.grid[0]);
+        made[2] = fr == CUFFT_SUCCESS;
+        if (fr == CUFFT_SUCCESS) {
+            fr = cufftPlanMany(&c->plan_c2r_yz, 2, dims + 1, nullptr, 1, 0, nullptr, 1, 0, CUFFT_C2R, 3 * S * p.grid[0]);
+            made[3] = fr == CUFFT_SUCCESS;
+        }
+    }
+    auto drop_plans = [&]() {
+        for (int i = 0; i < 4; ++i)
+            if (made[i]) cufftDestroy(*plans[i]);
+    };
+    if (fr != CUFFT_SUCCESS) {
+        drop_plans();
         delete c;
         return TILD_ECUFFT;
     }
-    c->plans_ok = true;
-    if ((rc = tild_spread_configure(c)) != TILD_OK || (rc = tild_interp_configure(c)) != TILD_OK) {
-        cufftDestroy(c->plan_r2c);
-        cufftDestroy(c->plan_c2r);
+    if ((rc = tild_spread_configure(c)) != TILD_OK || (rc = tild_interp_configure(c)) != TILD_OK ||
+        (rc = tild_kspace_configure(c)) != TILD_OK) {
+        drop_plans();
         delete c;
         return rc;
     }
-    cufftSetStream(c->plan_r2c, c->stream);
-    cufftSetStream(c->plan_c2r, c->stream);
+    c->plans_ok = true;
+    for (int i = 0; i < 4; ++i)
+        if (made[i]) cufftSetStream(*plans[i], c->stream);
     if (p.flags & TILD_FLAG_TIMING) {
         for (int i = 0; i < TILD_MAX_TIMED_STEPS; ++i)
             for (int k = 0; k < TILD_N_STAGE_EVENTS; ++k) cudaEventCreate(&c->ev[i][k]);
@@ -374,7 +420,12 @@ void tild_destroy(tild_ctx* c)
     if (!c) return;
     if (c->plans_ok) {
         cufftDestroy(c->plan_r2c);
-        cufftDestroy(c->plan_c2r);
+        if (c->xfft_R) {
+            cufftDestroy(c->plan_r2c_yz);
+            cufftDestroy(c->plan_c2r_yz);
+        } else {
+            cufftDestroy(c->plan_c2r);
+        }
     }
     if (c->graph_ok) cudaGraphExecDestroy(c->graph_exec);
     if (c->ev_ok)
@@ -408,11 +459,7 @@ int tild_spread(tild_ctx* c, const float* x, const int32_t* type, float* grid)
 int tild_kspace_force(tild_ctx* c, const float* grid, float* ffield)
 {
     if (!c || !grid || !ffield) return tild_fail(c, TILD_EINVAL, "tild_kspace_force: null argument");
-    TILD_FFT(c, cufftExecR2C(c->plan_r2c, const_cast<float*>(grid), reinterpret_cast<cufftComplex*>(c->nhat)));
-    int rc = launch_kspace(c, c->nhat, c->fhat);
-    if (rc) return rc;
-    TILD_FFT(c, cufftExecC2R(c->plan_c2r, reinterpret_cast<cufftComplex*>(c->fhat), ffield));
-    return TILD_OK;
+    return kspace_pipeline(c, grid, ffield, nullptr);
 }
 
 int tild_interp(tild_ctx* c, const float* ffield, const float* x, const int32_t* type, float* f)
@@ -609,6 +656,8 @@ int tild_energy(tild_ctx* c, double e[3])
     if (!c->has_state) return tild_fail(c, TILD_ESTATE, "tild_energy before tild_set_state");
     int rc = force_current(c);              // F4 and nhat at the current positions; no state change
     if (rc) return rc;
+    if (c->xfft_R)   // the fused x-transform leaves nhat transformed over (y, z) only: redo the full transform of the densities
+        TILD_FFT(c, cufftExecR2C(c->plan_r2c, c->grid, reinterpret_cast<cufftComplex*>(c->nhat)));
     if ((rc = launch_energy(c, c->d_energy))) return rc;
     TILD_CUDA(c, cudaMemcpyAsync(e, c->d_energy, 3 * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
     TILD_CUDA(c, cudaStreamSynchronize(c->stream));

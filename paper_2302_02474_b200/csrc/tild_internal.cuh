@@ -119,7 +119,10 @@ struct tild_ctx {
     uint32_t* perm;       // [n] tild_index_map scratch
     float* tables;        // k-space tables
 
-    cufftHandle plan_r2c, plan_c2r;
+    cufftHandle plan_r2c, plan_c2r;   // 3-D, batched over species / force components (plan_c2r only when !xfft_R)
+    cufftHandle plan_r2c_yz, plan_c2r_yz;   // 2-D over (y, z), batched over the x planes: used with the fused x-transform
+    int xfft_R;           // radix of kspace_xfft_kernel (Nx = R^2), 0 = 3-D cuFFT plans + kspace_kernel
+    const float2* xtw;    // exp(-2 pi i j / Nx), j < Nx
     bool plans_ok;
 
     bool has_state;
@@ -171,6 +174,9 @@ int tild_spread_configure(tild_ctx* c);
 int launch_spread(tild_ctx* c, const SegLayout& lay, const float4* X4, float* grid);  // zero fill + tile kernel
 // tild_kspace.cu
 int launch_kspace(tild_ctx* c, const float2* nhat, float2* fhat);
+int kspace_xfft_radix(int Nx, int S);
+int tild_kspace_configure(tild_ctx* c);
+int launch_kspace_xfft(tild_ctx* c, const float2* nhat, float2* fhat);
 // tild_interp.cu
 int tild_interp_configure(tild_ctx* c);
 enum { INTERP_NONBONDED_BY_ID = 0, INTERP_TOTAL_BY_SLOT = 1, INTERP_FUSED_STEP = 2 };

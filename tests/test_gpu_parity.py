@@ -39,6 +39,13 @@ def make(cfg, **kw):
 
 
 CASES = [small_cfg(order=P) for P in (1, 2, 3, 4, 5)] + [small_cfg(order=3, S=3, grid=(18, 12, 30), box=(9.0, 6.0, 15.0))]
+# Nx = 16, 64, 256: the fused x-transform k-space kernel (R = 4, 8, 16), ragged (y, z) line counts, one and two species
+XFFT_CASES = [small_cfg(order=3, grid=(16, 20, 18), box=(8.0, 10.0, 9.0)),
+              small_cfg(order=4, grid=(64, 12, 10), box=(32.0, 6.0, 5.0)),
+              small_cfg(order=2, grid=(256, 6, 10), box=(128.0, 3.0, 5.0), n_chains=400),
+              small_cfg(order=3, grid=(64, 9, 7), box=(32.0, 4.5, 3.5), chi=((0.0,),), n_species=1,
+                        chains=(inputs.ChainSpec(300, ((0, 5),)),), n=1500)]
+CASES = CASES + XFFT_CASES
 
 
 def test_philox_bit_exact_and_normals():
@@ -120,6 +127,35 @@ def test_total_force_parity_through_set_state(cfg):
     assert err <= REL * vec_rms(of), (err, vec_rms(of))
     # zero net non-bonded + bonded force
     assert np.abs(f.cpu().numpy().astype(np.float64).sum(0)).max() < 1e-4 * vec_rms(of) * np.sqrt(cfg.n)
+
+
+@pytest.mark.parametrize("cfg", XFFT_CASES, ids=lambda c: c.name + f"_{c.grid[0]}_S{c.n_species}")
+def test_fused_x_transform_kspace_path(cfg, monkeypatch):
+    """The fused x-transform kernel (2-D cuFFT over (y, z) + in-kernel FFT along x around the multiplication) against
+    the oracle's plain 3-D DFT definition, with electrostatics on, for the stage, tild_energy, and a short trajectory;
+    and against this library's own 3-D-plan path (TILD_XFFT=0), which it must match to fp32 rounding."""
+    from dataclasses import replace
+    S = cfg.n_species
+    ccfg = replace(cfg, charge=(1.0, -1.0)[:S] if S == 2 else (1.0,), bjerrum=0.7, a_charge=0.6)
+    st, eng = make(ccfg)
+    p = oracle_params(ccfg)
+    og32 = orc.spread(p, st.x, st.type).astype(np.float32)
+    ff = eng.tild_kspace_force(dev(og32)).cpu().numpy()
+    off = orc.kspace_force(p, og32.astype(np.float64))
+    assert np.abs(ff - off).max() <= REL * rms(off)
+    monkeypatch.setenv("TILD_XFFT", "0")
+    _, eng3 = make(ccfg)
+    monkeypatch.delenv("TILD_XFFT")
+    ff3 = eng3.tild_kspace_force(dev(og32)).cpu().numpy()
+    assert np.abs(ff - ff3).max() <= 2e-6 * rms(off)
+    eng.tild_set_state(dev(st.x), dev(st.v), dev(st.type), dev(st.bond_partner), 0)
+    e = eng.tild_energy()
+    oe = orc.energy(p, st.x.astype(np.float64), st.v.astype(np.float64), st.type, st.bond_partner)
+    assert np.all(np.abs(e - oe) <= 2e-5 * np.abs(oe).max()), (e, oe)
+    eng.tild_step(20)
+    x = eng.tild_get_state(want_v=False)[0].cpu().numpy().astype(np.float64)
+    ox, _, _ = orc.run(p, st.x.astype(np.float64), st.v.astype(np.float64), st.type, st.bond_partner, 0, 20)
+    assert np.abs(min_image(x - ox, cfg.box)).max() <= 1e-4
 
 
 def run_trajectory(cfg, nsteps, **kw):
