@@ -131,10 +131,15 @@ __global__ void __launch_bounds__(256, 2) kspace_xfft_kernel(KspaceParams k, siz
 {
     constexpr int N = R * R, LINES = 256 / R, EXN = R * 256;
     extern __shared__ float2 xs[];
-    float2* stw = xs;                   // [N]
-    float2* ex = xs + N;                // [2][R][R][LINES], alternating so that one barrier per transpose is enough
-    for (int j = threadIdx.x; j < N; j += 256) stw[j] = tw[j];
-    __syncthreads();
+    float2* stw = xs;                   // [N] twiddles
+    float2* sxu = xs + N;               // [N] (u^_x(m) / V, k_x(m))
+    float2* sxe = xs + 2 * N;           // [N] (Coulomb x factor, k_x(m)^2)
+    float2* ex = xs + 3 * N;            // [2][R][R][LINES], alternating so that one barrier per transpose is enough
+    for (int j = threadIdx.x; j < N; j += 256) {
+        stw[j] = tw[j];
+        sxu[j] = make_float2(__ldg(k.ufac[0] + j), __ldg(k.kgrad[0] + j));
+        sxe[j] = make_float2(__ldg(k.eel[0] + j), __ldg(k.k2[0] + j));
+    }
     const int ql = threadIdx.x % LINES, me = threadIdx.x / LINES;
     const size_t q = (size_t)blockIdx.x * LINES + ql;
     const bool active = q < Q;
@@ -149,11 +154,6 @@ __global__ void __launch_bounds__(256, 2) kspace_xfft_kernel(KspaceParams k, siz
 #pragma unroll
         for (int j = 0; j < R; ++j) X[J][j] = __ldg(src + (size_t)j * xstride);
     }
-#pragma unroll
-    for (int J = 0; J < S; ++J) {
-        line_fft<R, -1>(X[J], stw, ex + par * EXN, me, ql);
-        par ^= 1;
-    }
     const int my = (int)(qc / k.Nzc), mz = (int)(qc % k.Nzc);
     const float uyz = __ldg(k.ufac[1] + my) * __ldg(k.ufac[2] + mz);
     const float ky = __ldg(k.kgrad[1] + my), kz = __ldg(k.kgrad[2] + mz);
@@ -162,56 +162,65 @@ __global__ void __launch_bounds__(256, 2) kspace_xfft_kernel(KspaceParams k, siz
         eyz = __ldg(k.eel[1] + my) * __ldg(k.eel[2] + mz);
         k2yz = __ldg(k.k2[1] + my) + __ldg(k.k2[2] + mz);
     }
+    __syncthreads();
 #pragma unroll
-    for (int I = 0; I < S; ++I) {
+    for (int J = 0; J < S; ++J) {
+        line_fft<R, -1>(X[J], stw, ex + par * EXN, me, ql);
+        par ^= 1;
+    }
+    // 2S inverse transforms: (I, pass) with pass 0: t_I -> y and z components, pass 1: -i k_x t_I -> x component
+#pragma unroll 1
+    for (int ip = 0; ip < 2 * S; ++ip) {
+        const int I = ip >> 1, pass = ip & 1;
+        float cI[S], qI[S];
 #pragma unroll
-        for (int pass = 0; pass < 2; ++pass) {      // 0: t -> y and z components; 1: -i k_x t -> x component
-            float2 t[R];
+        for (int J = 0; J < S; ++J) {
+            cI[J] = k.c[I * TILD_MAX_SPECIES + J];
+            qI[J] = k.qq[I * TILD_MAX_SPECIES + J];
+        }
+        float2 t[R];
 #pragma unroll
-            for (int j = 0; j < R; ++j) {
-                const int mx = me + R * j;
-                float gr = 0.f, gi = 0.f, er = 0.f, ei = 0.f;
+        for (int j = 0; j < R; ++j) {
+            const int mx = me + R * j;
+            float gr = 0.f, gi = 0.f;
+#pragma unroll
+            for (int J = 0; J < S; ++J) {
+                gr += cI[J] * X[J][j].x;
+                gi += cI[J] * X[J][j].y;
+            }
+            const float2 xu = sxu[mx];
+            const float u = xu.x * uyz;
+            float tr = u * gr, ti = u * gi;
+            if (k.has_el) {
+                float er = 0.f, ei = 0.f;
 #pragma unroll
                 for (int J = 0; J < S; ++J) {
-                    const float cij = k.c[I * TILD_MAX_SPECIES + J];
-                    gr += cij * X[J][j].x;
-                    gi += cij * X[J][j].y;
-                    if (k.has_el) {
-                        const float qq = k.qq[I * TILD_MAX_SPECIES + J];
-                        er += qq * X[J][j].x;
-                        ei += qq * X[J][j].y;
-                    }
+                    er += qI[J] * X[J][j].x;
+                    ei += qI[J] * X[J][j].y;
                 }
-                const float u = __ldg(k.ufac[0] + mx) * uyz;
-                float uel = 0.f;
-                if (k.has_el) {
-                    const float k2 = __ldg(k.k2[0] + mx) + k2yz;
-                    uel = k2 > 0.f ? __ldg(k.eel[0] + mx) * eyz / k2 : 0.f;
-                }
-                const float tr = u * gr + uel * er, ti = u * gi + uel * ei;
-                if (pass == 0) {
-                    t[j] = make_float2(tr, ti);
-                } else {
-                    const float kx = __ldg(k.kgrad[0] + mx);
-                    t[j] = make_float2(kx * ti, -kx * tr);      // -i k_x (tr + i ti)
-                }
+                const float2 xe = sxe[mx];
+                const float k2 = xe.y + k2yz;
+                const float uel = k2 > 0.f ? xe.x * eyz / k2 : 0.f;
+                tr += uel * er;
+                ti += uel * ei;
             }
-            line_fft<R, +1>(t, stw, ex + par * EXN, me, ql);
-            par ^= 1;
-            if (active) {
-                if (pass == 0) {
-                    float2* dy = fhat + (((size_t)I * 3 + 1) * N + me) * Q + q;
-                    float2* dz = fhat + (((size_t)I * 3 + 2) * N + me) * Q + q;
+            t[j] = pass == 0 ? make_float2(tr, ti) : make_float2(xu.y * ti, -xu.y * tr);   // pass 1: -i k_x (tr + i ti)
+        }
+        line_fft<R, +1>(t, stw, ex + par * EXN, me, ql);
+        par ^= 1;
+        if (active) {
+            if (pass == 0) {
+                float2* dy = fhat + (((size_t)I * 3 + 1) * N + me) * Q + q;
+                float2* dz = fhat + (((size_t)I * 3 + 2) * N + me) * Q + q;
 #pragma unroll
-                    for (int j = 0; j < R; ++j) {
-                        dy[(size_t)j * xstride] = make_float2(ky * t[j].y, -ky * t[j].x);
-                        dz[(size_t)j * xstride] = make_float2(kz * t[j].y, -kz * t[j].x);
-                    }
-                } else {
-                    float2* dx = fhat + (((size_t)I * 3 + 0) * N + me) * Q + q;
-#pragma unroll
-                    for (int j = 0; j < R; ++j) dx[(size_t)j * xstride] = t[j];
+                for (int j = 0; j < R; ++j) {
+                    dy[(size_t)j * xstride] = make_float2(ky * t[j].y, -ky * t[j].x);
+                    dz[(size_t)j * xstride] = make_float2(kz * t[j].y, -kz * t[j].x);
                 }
+            } else {
+                float2* dx = fhat + (((size_t)I * 3 + 0) * N + me) * Q + q;
+#pragma unroll
+                for (int j = 0; j < R; ++j) dx[(size_t)j * xstride] = t[j];
             }
         }
     }
@@ -239,7 +248,7 @@ int kspace_xfft_radix(int Nx, int S)
     return Nx == 256 ? 16 : Nx == 64 ? 8 : Nx == 16 ? 4 : 0;
 }
 
-size_t kspace_xfft_smem(int R) { return ((size_t)R * R + 2 * (size_t)R * 256) * sizeof(float2); }
+size_t kspace_xfft_smem(int R) { return (3 * (size_t)R * R + 2 * (size_t)R * 256) * sizeof(float2); }
 
 int tild_kspace_configure(tild_ctx* c)
 {
