@@ -262,9 +262,9 @@ def ours_arm(args, cfg):
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from `ncu --set full` captures committed under profiles/
 # (key: (workload name, stage)); None until a capture exists.
 NCU_TRAFFIC = {   # profiles/r1_spread_interp_kspace_c4.md
-    ("C4_diblock_8m", "spread"): 357.2e6,
-    ("C4_diblock_8m", "kspace"): 483.3e6,
-    ("C4_diblock_8m", "interp"): 1124.5e6,
+    ("C4_diblock_8m", "spread"): 358.0e6,
+    ("C4_diblock_8m", "kspace"): 482.5e6,
+    ("C4_diblock_8m", "interp"): 1172.0e6,
 }
 
 

@@ -121,7 +121,7 @@ struct tild_ctx {
 
     cufftHandle plan_r2c, plan_c2r;   // 3-D, batched over species / force components (plan_c2r only when !xfft_R)
     cufftHandle plan_r2c_yz, plan_c2r_yz;   // 2-D over (y, z), batched over the x planes: used with the fused x-transform
-    int xfft_R;           // radix of kspace_xfft_kernel (Nx = R^2), 0 = 3-D cuFFT plans + kspace_kernel
+    int xfft_R;           // threads per line (R2) of kspace_xfft_kernel (Nx = R1 R2), 0 = 3-D cuFFT plans + kspace_kernel
     const float2* xtw;    // exp(-2 pi i j / Nx), j < Nx
     bool plans_ok;
 

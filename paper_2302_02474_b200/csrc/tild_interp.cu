@@ -231,7 +231,7 @@ __device__ __forceinline__ void index_weights(const MeshParams& m, const float4&
 
 // per-particle kernel over the slots [s0, s1)
 template <int P, bool VEC, int MODE>
-__global__ void __launch_bounds__(256) interp_slots_kernel(MeshParams m, StepParams s, const uint64_t* __restrict__ step_ptr, size_t s0, size_t s1,
+__global__ void __launch_bounds__(256, P == 1 ? 8 : 1) interp_slots_kernel(MeshParams m, StepParams s, const uint64_t* __restrict__ step_ptr, size_t s0, size_t s1,
                                                            const float* __restrict__ ffield, const float4* __restrict__ X4,
                                                            const float4* __restrict__ W4, const int32_t* __restrict__ B,
                                                            float4* __restrict__ X4o, float4* __restrict__ W4o,

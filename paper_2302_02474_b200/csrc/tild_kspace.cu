@@ -53,10 +53,10 @@ __global__ void __launch_bounds__(256) kspace_kernel(KspaceParams k, size_t Mk, 
 
 
 // ---- fused x-transform variant --------------------------------------------------------------------------------------
-// The 3-D transforms are separable.  When Nx = R^2 (R = 4, 8, 16) and S <= 2 the mesh pipeline runs cuFFT only over
+// The 3-D transforms are separable.  When Nx = 16, 32, 64, 128 or 256 and S <= 2 the mesh pipeline runs cuFFT only over
 // (y, z) -- batched 2-D R2C / C2R over the x planes -- and this kernel does, for 256 / R lines (ky, kz) at a time,
 //   forward FFT along x of the S densities -> the multiplication above -> inverse FFT along x of the 3S force spectra,
-// in registers (two R-point transforms per length-N transform, one shared-memory transpose between them).  Against the
+// in registers (Nx = R1 R2: an R1- and an R2-point transform per line, one shared-memory transpose between them).  Against the
 // 3-D plans this drops the x passes of all 4S transforms and the round trip of n^ and f^ through HBM between them:
 // the stage still reads S and writes 3S half-spectra (its algorithmic bytes), nothing else.  Since k_y and k_z are
 // constant along a line, only IFFT_x(t) and IFFT_x(-i k_x t) are computed; the y and z components scale the former.
@@ -105,36 +105,57 @@ struct RegFft<1, SGN> {
     static __device__ __forceinline__ void run(float2 (&)[1]) {}
 };
 
-// One length-N (N = R^2) transform per line, spread over R threads.  On entry thread `me` of a line holds
-// v[j] = in[R j + me] (forward) or in[me + R j] (inverse); on exit out[me + R j] (forward) or out[R j + me] (inverse):
-// N = R^2 Cooley-Tukey with the twiddle exp(SGN 2 pi i me k / N) between the two R-point passes.
-template <int R, int SGN>
-__device__ __forceinline__ void line_fft(float2 (&v)[R], const float2* __restrict__ stw, float2* __restrict__ ex, int me, int ql)
+// One length-N transform per line, N = R1 R2 (R1 <= R2), spread over R2 threads: Cooley-Tukey with the twiddle
+// exp(-/+ 2 pi i n2 k1 / N) between an R1-point and an R2-point pass and one shared-memory transpose.
+// Forward: thread me (< R2) holds a[j] = in[R2 j + me]; on exit thread me < R1 holds b[j] = out[me + R1 j].
+template <int R1, int R2>
+__device__ __forceinline__ void line_fft_fwd(float2 (&a)[R1], float2 (&b)[R2], const float2* __restrict__ stw,
+                                             float2* __restrict__ ex, int me, int ql)
 {
-    constexpr int LINES = 256 / R;
-    RegFft<R, SGN>::run(v);
+    constexpr int LINES = 256 / R2;
+    RegFft<R1, -1>::run(a);
 #pragma unroll
-    for (int j = 0; j < R; ++j) {
-        const float2 w = stw[me * j];              // exp(-2 pi i me j / N); conjugated for the inverse
-        const float wi = SGN < 0 ? w.y : -w.y;
-        ex[(j * R + me) * LINES + ql] = make_float2(v[j].x * w.x - v[j].y * wi, v[j].x * wi + v[j].y * w.x);
+    for (int j = 0; j < R1; ++j) {
+        const float2 w = stw[me * j];              // exp(-2 pi i me j / N)
+        ex[(j * R2 + me) * LINES + ql] = make_float2(a[j].x * w.x - a[j].y * w.y, a[j].x * w.y + a[j].y * w.x);
+    }
+    __syncthreads();
+    if (me < R1) {
+#pragma unroll
+        for (int j = 0; j < R2; ++j) b[j] = ex[(me * R2 + j) * LINES + ql];
+        RegFft<R2, -1>::run(b);
+    }
+}
+// Inverse: thread me < R1 holds b[j] = in[me + R1 j]; on exit thread me (< R2) holds a[j] = out[R2 j + me].
+template <int R1, int R2>
+__device__ __forceinline__ void line_fft_inv(float2 (&b)[R2], float2 (&a)[R1], const float2* __restrict__ stw,
+                                             float2* __restrict__ ex, int me, int ql)
+{
+    constexpr int LINES = 256 / R2;
+    if (me < R1) {
+        RegFft<R2, +1>::run(b);
+#pragma unroll
+        for (int j = 0; j < R2; ++j) {
+            const float2 w = stw[me * j];          // conjugated: exp(+2 pi i me j / N)
+            ex[(j * R1 + me) * LINES + ql] = make_float2(b[j].x * w.x + b[j].y * w.y, b[j].y * w.x - b[j].x * w.y);
+        }
     }
     __syncthreads();
 #pragma unroll
-    for (int j = 0; j < R; ++j) v[j] = ex[(me * R + j) * LINES + ql];
-    RegFft<R, SGN>::run(v);
+    for (int j = 0; j < R1; ++j) a[j] = ex[(me * R1 + j) * LINES + ql];
+    RegFft<R1, +1>::run(a);
 }
 
-template <int R, int S>
+template <int R1, int R2, int S>
 __global__ void __launch_bounds__(256, 2) kspace_xfft_kernel(KspaceParams k, size_t Q, const float2* __restrict__ tw,
                                                              const float2* __restrict__ nhat, float2* __restrict__ fhat)
 {
-    constexpr int N = R * R, LINES = 256 / R, EXN = R * 256;
+    constexpr int N = R1 * R2, LINES = 256 / R2, EXN = R1 * 256;
     extern __shared__ float2 xs[];
     float2* stw = xs;                   // [N] twiddles
     float2* sxu = xs + N;               // [N] (u^_x(m) / V, k_x(m))
     float2* sxe = xs + 2 * N;           // [N] (Coulomb x factor, k_x(m)^2)
-    float2* ex = xs + 3 * N;            // [2][R][R][LINES], alternating so that one barrier per transpose is enough
+    float2* ex = xs + 3 * N;            // [2][R1][R2][LINES], alternating so that one barrier per transpose is enough
     for (int j = threadIdx.x; j < N; j += 256) {
         stw[j] = tw[j];
         sxu[j] = make_float2(__ldg(k.ufac[0] + j), __ldg(k.kgrad[0] + j));
@@ -144,15 +165,15 @@ __global__ void __launch_bounds__(256, 2) kspace_xfft_kernel(KspaceParams k, siz
     const size_t q = (size_t)blockIdx.x * LINES + ql;
     const bool active = q < Q;
     const size_t qc = active ? q : Q - 1;
-    const size_t xstride = (size_t)R * Q;           // between the R points a thread holds
+    const size_t xstride = (size_t)R2 * Q;          // between the R1 points a thread loads and stores
     int par = 0;
 
-    float2 X[S][R];                                 // X[J][j] = n^_J(kx = me + R j) after the forward transform
+    float2 A[S][R1];
 #pragma unroll
     for (int J = 0; J < S; ++J) {
         const float2* src = nhat + ((size_t)J * N + me) * Q + qc;
 #pragma unroll
-        for (int j = 0; j < R; ++j) X[J][j] = __ldg(src + (size_t)j * xstride);
+        for (int j = 0; j < R1; ++j) A[J][j] = __ldg(src + (size_t)j * xstride);
     }
     const int my = (int)(qc / k.Nzc), mz = (int)(qc % k.Nzc);
     const float uyz = __ldg(k.ufac[1] + my) * __ldg(k.ufac[2] + mz);
@@ -163,9 +184,12 @@ __global__ void __launch_bounds__(256, 2) kspace_xfft_kernel(KspaceParams k, siz
         k2yz = __ldg(k.k2[1] + my) + __ldg(k.k2[2] + mz);
     }
     __syncthreads();
+    float2 X[S][R2];                                // threads me < R1: X[J][j] = n^_J(kx = me + R1 j)
 #pragma unroll
     for (int J = 0; J < S; ++J) {
-        line_fft<R, -1>(X[J], stw, ex + par * EXN, me, ql);
+#pragma unroll
+        for (int j = 0; j < R2; ++j) X[J][j] = make_float2(0.f, 0.f);
+        line_fft_fwd<R1, R2>(A[J], X[J], stw, ex + par * EXN, me, ql);
         par ^= 1;
     }
     // 2S inverse transforms: (I, pass) with pass 0: t_I -> y and z components, pass 1: -i k_x t_I -> x component
@@ -178,49 +202,52 @@ __global__ void __launch_bounds__(256, 2) kspace_xfft_kernel(KspaceParams k, siz
             cI[J] = k.c[I * TILD_MAX_SPECIES + J];
             qI[J] = k.qq[I * TILD_MAX_SPECIES + J];
         }
-        float2 t[R];
+        float2 t[R2];
+        if (me < R1) {
 #pragma unroll
-        for (int j = 0; j < R; ++j) {
-            const int mx = me + R * j;
-            float gr = 0.f, gi = 0.f;
-#pragma unroll
-            for (int J = 0; J < S; ++J) {
-                gr += cI[J] * X[J][j].x;
-                gi += cI[J] * X[J][j].y;
-            }
-            const float2 xu = sxu[mx];
-            const float u = xu.x * uyz;
-            float tr = u * gr, ti = u * gi;
-            if (k.has_el) {
-                float er = 0.f, ei = 0.f;
+            for (int j = 0; j < R2; ++j) {
+                const int mx = me + R1 * j;
+                float gr = 0.f, gi = 0.f;
 #pragma unroll
                 for (int J = 0; J < S; ++J) {
-                    er += qI[J] * X[J][j].x;
-                    ei += qI[J] * X[J][j].y;
+                    gr += cI[J] * X[J][j].x;
+                    gi += cI[J] * X[J][j].y;
                 }
-                const float2 xe = sxe[mx];
-                const float k2 = xe.y + k2yz;
-                const float uel = k2 > 0.f ? xe.x * eyz / k2 : 0.f;
-                tr += uel * er;
-                ti += uel * ei;
+                const float2 xu = sxu[mx];
+                const float u = xu.x * uyz;
+                float tr = u * gr, ti = u * gi;
+                if (k.has_el) {
+                    float er = 0.f, ei = 0.f;
+#pragma unroll
+                    for (int J = 0; J < S; ++J) {
+                        er += qI[J] * X[J][j].x;
+                        ei += qI[J] * X[J][j].y;
+                    }
+                    const float2 xe = sxe[mx];
+                    const float k2 = xe.y + k2yz;
+                    const float uel = k2 > 0.f ? xe.x * eyz / k2 : 0.f;
+                    tr += uel * er;
+                    ti += uel * ei;
+                }
+                t[j] = pass == 0 ? make_float2(tr, ti) : make_float2(xu.y * ti, -xu.y * tr);   // pass 1: -i k_x (tr + i ti)
             }
-            t[j] = pass == 0 ? make_float2(tr, ti) : make_float2(xu.y * ti, -xu.y * tr);   // pass 1: -i k_x (tr + i ti)
         }
-        line_fft<R, +1>(t, stw, ex + par * EXN, me, ql);
+        float2 o[R1];
+        line_fft_inv<R1, R2>(t, o, stw, ex + par * EXN, me, ql);
         par ^= 1;
         if (active) {
             if (pass == 0) {
                 float2* dy = fhat + (((size_t)I * 3 + 1) * N + me) * Q + q;
                 float2* dz = fhat + (((size_t)I * 3 + 2) * N + me) * Q + q;
 #pragma unroll
-                for (int j = 0; j < R; ++j) {
-                    dy[(size_t)j * xstride] = make_float2(ky * t[j].y, -ky * t[j].x);
-                    dz[(size_t)j * xstride] = make_float2(kz * t[j].y, -kz * t[j].x);
+                for (int j = 0; j < R1; ++j) {
+                    dy[(size_t)j * xstride] = make_float2(ky * o[j].y, -ky * o[j].x);
+                    dz[(size_t)j * xstride] = make_float2(kz * o[j].y, -kz * o[j].x);
                 }
             } else {
                 float2* dx = fhat + (((size_t)I * 3 + 0) * N + me) * Q + q;
 #pragma unroll
-                for (int j = 0; j < R; ++j) dx[(size_t)j * xstride] = t[j];
+                for (int j = 0; j < R1; ++j) dx[(size_t)j * xstride] = o[j];
             }
         }
     }
@@ -241,25 +268,45 @@ int launch_kspace(tild_ctx* c, const float2* nhat, float2* fhat)
     return TILD_OK;
 }
 
-// the radix R of the fused x-transform kernel for this mesh, 0 when it does not apply
+// R2 of the fused x-transform kernel for this mesh (Nx = R1 R2, R1 = Nx / R2 <= R2), 0 when it does not apply
 int kspace_xfft_radix(int Nx, int S)
 {
     if (S > 2) return 0;
-    return Nx == 256 ? 16 : Nx == 64 ? 8 : Nx == 16 ? 4 : 0;
+    return Nx == 256 || Nx == 128 ? 16 : Nx == 64 || Nx == 32 ? 8 : Nx == 16 ? 4 : 0;
 }
 
-size_t kspace_xfft_smem(int R) { return (3 * (size_t)R * R + 2 * (size_t)R * 256) * sizeof(float2); }
+// dispatch over (Nx, S): OP(R1, R2, S)
+#define TILD_XFFT_DISPATCH(N_, S_, OP)                                              \
+    do {                                                                            \
+        if ((S_) == 1) {                                                            \
+            switch (N_) {                                                           \
+            case 256: OP(16, 16, 1); break;                                         \
+            case 128: OP(8, 16, 1); break;                                          \
+            case 64: OP(8, 8, 1); break;                                            \
+            case 32: OP(4, 8, 1); break;                                            \
+            default: OP(4, 4, 1); break;                                            \
+            }                                                                       \
+        } else {                                                                    \
+            switch (N_) {                                                           \
+            case 256: OP(16, 16, 2); break;                                         \
+            case 128: OP(8, 16, 2); break;                                          \
+            case 64: OP(8, 8, 2); break;                                            \
+            case 32: OP(4, 8, 2); break;                                            \
+            default: OP(4, 4, 2); break;                                            \
+            }                                                                       \
+        }                                                                           \
+    } while (0)
+
+// shared memory: 3 tables of N float2 + two transpose buffers of R1 * 256 float2
+static size_t xfft_smem_bytes(int N, int R2) { return (3 * (size_t)N + 2 * (size_t)(N / R2) * 256) * sizeof(float2); }
 
 int tild_kspace_configure(tild_ctx* c)
 {
     if (!c->xfft_R) return TILD_OK;
-    const int sm = (int)kspace_xfft_smem(c->xfft_R);
-#define XA(RR, SS) TILD_CUDA(c, cudaFuncSetAttribute(kspace_xfft_kernel<RR, SS>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm))
-    if (c->mesh.S == 1) {
-        if (c->xfft_R == 16) XA(16, 1); else if (c->xfft_R == 8) XA(8, 1); else XA(4, 1);
-    } else {
-        if (c->xfft_R == 16) XA(16, 2); else if (c->xfft_R == 8) XA(8, 2); else XA(4, 2);
-    }
+    const int N = c->mesh.N[0];
+    const int sm = (int)xfft_smem_bytes(N, c->xfft_R);
+#define XA(R1_, R2_, SS) TILD_CUDA(c, cudaFuncSetAttribute(kspace_xfft_kernel<R1_, R2_, SS>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm))
+    TILD_XFFT_DISPATCH(N, c->mesh.S, XA);
 #undef XA
     return TILD_OK;
 }
@@ -268,15 +315,11 @@ int tild_kspace_configure(tild_ctx* c)
 int launch_kspace_xfft(tild_ctx* c, const float2* nhat, float2* fhat)
 {
     const size_t Q = (size_t)c->mesh.N[1] * c->ksp.Nzc;
-    const int R = c->xfft_R, lines = 256 / R;
+    const int N = c->mesh.N[0], lines = 256 / c->xfft_R;
     const unsigned nb = (unsigned)((Q + lines - 1) / lines);
-    const size_t sm = kspace_xfft_smem(R);
-#define XL(RR, SS) kspace_xfft_kernel<RR, SS><<<nb, 256, sm, c->stream>>>(c->ksp, Q, c->xtw, nhat, fhat)
-    if (c->mesh.S == 1) {
-        if (R == 16) XL(16, 1); else if (R == 8) XL(8, 1); else XL(4, 1);
-    } else {
-        if (R == 16) XL(16, 2); else if (R == 8) XL(8, 2); else XL(4, 2);
-    }
+    const size_t sm = xfft_smem_bytes(N, c->xfft_R);
+#define XL(R1_, R2_, SS) kspace_xfft_kernel<R1_, R2_, SS><<<nb, 256, sm, c->stream>>>(c->ksp, Q, c->xtw, nhat, fhat)
+    TILD_XFFT_DISPATCH(N, c->mesh.S, XL);
 #undef XL
     TILD_LAUNCH_CHECK(c, "kspace_xfft_kernel");
     return TILD_OK;

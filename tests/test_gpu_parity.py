@@ -39,10 +39,12 @@ def make(cfg, **kw):
 
 
 CASES = [small_cfg(order=P) for P in (1, 2, 3, 4, 5)] + [small_cfg(order=3, S=3, grid=(18, 12, 30), box=(9.0, 6.0, 15.0))]
-# Nx = 16, 64, 256: the fused x-transform k-space kernel (R = 4, 8, 16), ragged (y, z) line counts, one and two species
+# Nx = 16, 32, 64, 128, 256: the fused x-transform k-space kernel (Nx = R1 R2), ragged (y, z) line counts, one and two species
 XFFT_CASES = [small_cfg(order=3, grid=(16, 20, 18), box=(8.0, 10.0, 9.0)),
               small_cfg(order=4, grid=(64, 12, 10), box=(32.0, 6.0, 5.0)),
               small_cfg(order=2, grid=(256, 6, 10), box=(128.0, 3.0, 5.0), n_chains=400),
+              small_cfg(order=3, grid=(32, 14, 12), box=(16.0, 7.0, 6.0)),
+              small_cfg(order=5, grid=(128, 8, 12), box=(64.0, 4.0, 6.0), n_chains=300),
               small_cfg(order=3, grid=(64, 9, 7), box=(32.0, 4.5, 3.5), chi=((0.0,),), n_species=1,
                         chains=(inputs.ChainSpec(300, ((0, 5),)),), n=1500)]
 CASES = CASES + XFFT_CASES
