@@ -53,7 +53,7 @@ __global__ void __launch_bounds__(256) kspace_kernel(KspaceParams k, size_t Mk, 
 
 
 // ---- fused x-transform variant --------------------------------------------------------------------------------------
-// The 3-D transforms are separable.  When Nx = 16, 32, 64, 128 or 256 and S <= 2 the mesh pipeline runs cuFFT only over
+// The 3-D transforms are separable.  When Nx = 16, 32, 64, 128 or 256 and S <= 4 the mesh pipeline runs cuFFT only over
 // (y, z) -- batched 2-D R2C / C2R over the x planes -- and this kernel does, for 256 / R lines (ky, kz) at a time,
 //   forward FFT along x of the S densities -> the multiplication above -> inverse FFT along x of the 3S force spectra,
 // in registers (Nx = R1 R2: an R1- and an R2-point transform per line, one shared-memory transpose between them).  Against the
@@ -147,7 +147,7 @@ __device__ __forceinline__ void line_fft_inv(float2 (&b)[R2], float2 (&a)[R1], c
 }
 
 template <int R1, int R2, int S>
-__global__ void __launch_bounds__(256, 2) kspace_xfft_kernel(KspaceParams k, size_t Q, const float2* __restrict__ tw,
+__global__ void __launch_bounds__(256, S <= 2 ? 2 : 1) kspace_xfft_kernel(KspaceParams k, size_t Q, const float2* __restrict__ tw,
                                                              const float2* __restrict__ nhat, float2* __restrict__ fhat)
 {
     constexpr int N = R1 * R2, LINES = 256 / R2, EXN = R1 * 256;
@@ -271,30 +271,25 @@ int launch_kspace(tild_ctx* c, const float2* nhat, float2* fhat)
 // R2 of the fused x-transform kernel for this mesh (Nx = R1 R2, R1 = Nx / R2 <= R2), 0 when it does not apply
 int kspace_xfft_radix(int Nx, int S)
 {
-    if (S > 2) return 0;
+    if (S > 4) return 0;   // S = 3, 4: one CTA per SM (the spectra of all species stay in registers)
     return Nx == 256 || Nx == 128 ? 16 : Nx == 64 || Nx == 32 ? 8 : Nx == 16 ? 4 : 0;
 }
 
 // dispatch over (Nx, S): OP(R1, R2, S)
+#define TILD_XFFT_DISPATCH_S(N_, SS, OP)                                            \
+    switch (N_) {                                                                   \
+    case 256: OP(16, 16, SS); break;                                                \
+    case 128: OP(8, 16, SS); break;                                                 \
+    case 64: OP(8, 8, SS); break;                                                   \
+    case 32: OP(4, 8, SS); break;                                                   \
+    default: OP(4, 4, SS); break;                                                   \
+    }
 #define TILD_XFFT_DISPATCH(N_, S_, OP)                                              \
     do {                                                                            \
-        if ((S_) == 1) {                                                            \
-            switch (N_) {                                                           \
-            case 256: OP(16, 16, 1); break;                                         \
-            case 128: OP(8, 16, 1); break;                                          \
-            case 64: OP(8, 8, 1); break;                                            \
-            case 32: OP(4, 8, 1); break;                                            \
-            default: OP(4, 4, 1); break;                                            \
-            }                                                                       \
-        } else {                                                                    \
-            switch (N_) {                                                           \
-            case 256: OP(16, 16, 2); break;                                         \
-            case 128: OP(8, 16, 2); break;                                          \
-            case 64: OP(8, 8, 2); break;                                            \
-            case 32: OP(4, 8, 2); break;                                            \
-            default: OP(4, 4, 2); break;                                            \
-            }                                                                       \
-        }                                                                           \
+        if ((S_) == 1) { TILD_XFFT_DISPATCH_S(N_, 1, OP) }                          \
+        else if ((S_) == 2) { TILD_XFFT_DISPATCH_S(N_, 2, OP) }                     \
+        else if ((S_) == 3) { TILD_XFFT_DISPATCH_S(N_, 3, OP) }                     \
+        else { TILD_XFFT_DISPATCH_S(N_, 4, OP) }                                    \
     } while (0)
 
 // shared memory: 3 tables of N float2 + two transpose buffers of R1 * 256 float2

@@ -44,6 +44,8 @@ XFFT_CASES = [small_cfg(order=3, grid=(16, 20, 18), box=(8.0, 10.0, 9.0)),
               small_cfg(order=4, grid=(64, 12, 10), box=(32.0, 6.0, 5.0)),
               small_cfg(order=2, grid=(256, 6, 10), box=(128.0, 3.0, 5.0), n_chains=400),
               small_cfg(order=3, grid=(32, 14, 12), box=(16.0, 7.0, 6.0)),
+              small_cfg(order=3, S=3, grid=(64, 12, 10), box=(32.0, 6.0, 5.0)),
+              small_cfg(order=2, S=3, grid=(256, 6, 6), box=(128.0, 3.0, 3.0)),
               small_cfg(order=5, grid=(128, 8, 12), box=(64.0, 4.0, 6.0), n_chains=300),
               small_cfg(order=3, grid=(64, 9, 7), box=(32.0, 4.5, 3.5), chi=((0.0,),), n_species=1,
                         chains=(inputs.ChainSpec(300, ((0, 5),)),), n=1500)]
@@ -138,7 +140,7 @@ def test_fused_x_transform_kspace_path(cfg, monkeypatch):
     and against this library's own 3-D-plan path (TILD_XFFT=0), which it must match to fp32 rounding."""
     from dataclasses import replace
     S = cfg.n_species
-    ccfg = replace(cfg, charge=(1.0, -1.0)[:S] if S == 2 else (1.0,), bjerrum=0.7, a_charge=0.6)
+    ccfg = replace(cfg, charge=(1.0, -1.0, 0.5)[:S], bjerrum=0.7, a_charge=0.6)
     st, eng = make(ccfg)
     p = oracle_params(ccfg)
     og32 = orc.spread(p, st.x, st.type).astype(np.float32)
