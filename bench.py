@@ -229,7 +229,7 @@ def ours_arm(args, cfg):
         gbs = alg[k] / (stage_ms[k] * 1e-3) / 1e9 if stage_ms[k] > 0 else 0.0
         stages[k] = {"ms": stage_ms[k], "alg_bytes": alg[k], "gbs": gbs, "frac": gbs / peak,
                      "traffic": NCU_TRAFFIC.get((cfg.name, k))}
-    if os.environ.get("TILD_XFFT", "1") != "0" and cfg.n_species <= 4 and cfg.grid[0] in (16, 32, 64, 128, 256):
+    if os.environ.get("TILD_XFFT", "1") != "0" and not (args.flags & tild.FLAG_PLAIN_FFT) and cfg.n_species <= 4 and cfg.grid[0] in (16, 32, 64, 128, 256):
         stages["kspace"]["note"] = ("fused x-transform kernel: this stage also does the x passes of all 4S FFTs; "
                                     "fft_fwd / fft_inv are the (y, z) passes only")
     dom = max(stages, key=lambda k: stages[k]["ms"])

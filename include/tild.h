@@ -54,6 +54,9 @@ typedef enum {
                                       order-P assignment (A13; default off: the kernel is exactly u^(k)) */
 #define TILD_FLAG_SAMPLED_KERNEL 32u /* pair kernel = DFT of u_G sampled on the mesh (minimum image), as PAPER.md L223
                                       describes, instead of the analytic u^(k) (A5b); still three 1-D tables */
+#define TILD_FLAG_PLAIN_FFT 64u    /* 3-D cuFFT plans + the element-wise k-space kernel even where the fused x-transform
+                                      kernel applies (Nx in {16,32,64,128,256}, S <= 4); same as the environment variable
+                                      TILD_XFFT=0.  For A/B runs: the results agree to fp32 rounding */
 #define TILD_FLAG_GRAPH 8u         /* tild_step replays blocks of 2*resort_every steps as one CUDA graph (launch-bound
                                       small systems); ignored with TILD_FLAG_TIMING, an odd resort_every, or the
                                       legacy default stream (which cannot be captured) */

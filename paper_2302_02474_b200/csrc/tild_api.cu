@@ -322,7 +322,7 @@ int tild_init(tild_ctx** out, const tild_params* params, void* workspace, size_t
     c->xtw = reinterpret_cast<const float2*>(c->tables + (size_t)12 * 4096);
     {
         const char* env = getenv("TILD_XFFT");   // 0 forces the 3-D cuFFT plans + separate k-space kernel (A/B runs)
-        c->xfft_R = (env && env[0] == '0') ? 0 : kspace_xfft_radix(p.grid[0], S);
+        c->xfft_R = ((env && env[0] == '0') || (p.flags & TILD_FLAG_PLAIN_FFT)) ? 0 : kspace_xfft_radix(p.grid[0], S);
     }
     KspaceParams& ks = c->ksp;
     ks.S = S;

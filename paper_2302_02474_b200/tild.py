@@ -20,6 +20,7 @@ MAX_BONDS = 4
 OK, EINVAL, ENOMEM, ECUDA, ECUFFT, ESTATE = 0, -1, -2, -3, -4, -5
 INTEGRATOR_GJF, INTEGRATOR_EM = 0, 1
 FLAG_TIMING, FLAG_NAIVE_SPREAD, FLAG_NAIVE_INTERP, FLAG_GRAPH, FLAG_DECONVOLVE, FLAG_SAMPLED_KERNEL = 1, 2, 4, 8, 16, 32
+FLAG_PLAIN_FFT = 64
 TIMING_NAMES = ("sort", "spread", "fft_fwd", "kspace", "fft_inv", "interp", "other", "total")
 
 EXPORTS = (

@@ -134,10 +134,10 @@ def test_total_force_parity_through_set_state(cfg):
 
 
 @pytest.mark.parametrize("cfg", XFFT_CASES, ids=lambda c: c.name + f"_{c.grid[0]}_S{c.n_species}")
-def test_fused_x_transform_kspace_path(cfg, monkeypatch):
+def test_fused_x_transform_kspace_path(cfg):
     """The fused x-transform kernel (2-D cuFFT over (y, z) + in-kernel FFT along x around the multiplication) against
     the oracle's plain 3-D DFT definition, with electrostatics on, for the stage, tild_energy, and a short trajectory;
-    and against this library's own 3-D-plan path (TILD_XFFT=0), which it must match to fp32 rounding."""
+    and against this library's own 3-D-plan path (TILD_FLAG_PLAIN_FFT), which it must match to fp32 rounding."""
     from dataclasses import replace
     S = cfg.n_species
     ccfg = replace(cfg, charge=(1.0, -1.0, 0.5)[:S], bjerrum=0.7, a_charge=0.6)
@@ -147,9 +147,7 @@ def test_fused_x_transform_kspace_path(cfg, monkeypatch):
     ff = eng.tild_kspace_force(dev(og32)).cpu().numpy()
     off = orc.kspace_force(p, og32.astype(np.float64))
     assert np.abs(ff - off).max() <= REL * rms(off)
-    monkeypatch.setenv("TILD_XFFT", "0")
-    _, eng3 = make(ccfg)
-    monkeypatch.delenv("TILD_XFFT")
+    _, eng3 = make(ccfg, flags=tild.FLAG_PLAIN_FFT)
     ff3 = eng3.tild_kspace_force(dev(og32)).cpu().numpy()
     assert np.abs(ff - ff3).max() <= 2e-6 * rms(off)
     eng.tild_set_state(dev(st.x), dev(st.v), dev(st.type), dev(st.bond_partner), 0)
