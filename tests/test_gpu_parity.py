@@ -495,9 +495,12 @@ def test_set_state_can_be_called_again_and_restarts_the_step_counter():
     assert np.abs(min_image(x1.astype(np.float64) - x2.cpu().numpy(), cfg.box)).max() < 2e-5
 
 
-def test_cuda_graph_blocks_match_eager_stepping():
-    """TILD_FLAG_GRAPH replays 2 * resort_every steps as one CUDA graph; noise still follows (id, step)."""
-    cfg = small_cfg(order=3)
+@pytest.mark.parametrize("grid,box", [((24, 20, 16), (12.0, 10.0, 8.0)), ((32, 20, 16), (16.0, 10.0, 8.0))],
+                         ids=["plans3d", "fused_x"])
+def test_cuda_graph_blocks_match_eager_stepping(grid, box):
+    """TILD_FLAG_GRAPH replays 2 * resort_every steps as one CUDA graph; noise still follows (id, step).  Both k-space
+    paths (3-D plans; 2-D plans + fused x-transform kernel) are captured."""
+    cfg = small_cfg(order=3, grid=grid, box=box)
     st = inputs.make_state(cfg)
     outs = []
     side = torch.cuda.Stream()                   # the legacy default stream cannot be captured
