@@ -180,7 +180,7 @@ def ours_arm(args, cfg):
     in_seed, ph_seed = replica_seeds(cfg, rank)
     st = inputs.make_state(cfg, seed=in_seed)
     eng = tild.Tild(tild.params_from_config(cfg, flags=tild.FLAG_TIMING | args.flags, seed=ph_seed,
-                                            resort_every=args.resort_every), device=f"cuda:{local}")
+                                            resort_every=args.resort_every, tile_shape=args.tile_shape), device=f"cuda:{local}")
     xd, vd = torch.from_numpy(st.x).cuda(), torch.from_numpy(st.v).cuda()
     td, bd = torch.from_numpy(st.type).cuda(), torch.from_numpy(st.bond_partner).cuda()
     eng.tild_set_state(xd, vd, td, bd, 0)
@@ -229,7 +229,7 @@ def ours_arm(args, cfg):
         gbs = alg[k] / (stage_ms[k] * 1e-3) / 1e9 if stage_ms[k] > 0 else 0.0
         stages[k] = {"ms": stage_ms[k], "alg_bytes": alg[k], "gbs": gbs, "frac": gbs / peak,
                      "traffic": NCU_TRAFFIC.get((cfg.name, k))}
-    if os.environ.get("TILD_XFFT", "1") != "0" and not (args.flags & tild.FLAG_PLAIN_FFT) and cfg.n_species <= 4 and cfg.grid[0] in (16, 32, 64, 128, 256):
+    if not (args.flags & tild.FLAG_PLAIN_FFT) and cfg.n_species <= 4 and cfg.grid[0] in (16, 32, 64, 128, 256):
         stages["kspace"]["note"] = ("fused x-transform kernel: this stage also does the x passes of all 4S FFTs; "
                                     "fft_fwd / fft_inv are the (y, z) passes only")
     dom = max(stages, key=lambda k: stages[k]["ms"])
@@ -310,6 +310,7 @@ def main():
     ap.add_argument("--resort-every", type=int, default=0)
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--flags", type=int, default=0, help="extra TILD_FLAG_* bits (kernel A/B runs)")
+    ap.add_argument("--tile-shape", type=int, default=0, help="tild_params.tile_shape = TY | TZ << 8 (0 = default 8x16x32)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--sweep", action="store_true", help="run the C5 roofline sweep instead of the headline bench")

@@ -55,11 +55,14 @@ typedef enum {
 #define TILD_FLAG_SAMPLED_KERNEL 32u /* pair kernel = DFT of u_G sampled on the mesh (minimum image), as PAPER.md L223
                                       describes, instead of the analytic u^(k) (A5b); still three 1-D tables */
 #define TILD_FLAG_PLAIN_FFT 64u    /* 3-D cuFFT plans + the element-wise k-space kernel even where the fused x-transform
-                                      kernel applies (Nx in {16,32,64,128,256}, S <= 4); same as the environment variable
-                                      TILD_XFFT=0.  For A/B runs: the results agree to fp32 rounding */
+                                      kernel applies (Nx in {16,32,64,128,256}, S <= 4).  For A/B runs: the results agree to fp32
+                                      rounding */
 #define TILD_FLAG_GRAPH 8u         /* tild_step replays blocks of 2*resort_every steps as one CUDA graph (launch-bound
                                       small systems); ignored with TILD_FLAG_TIMING, an odd resort_every, or the
                                       legacy default stream (which cannot be captured) */
+
+#define TILD_FLAG_GEN1_TILES 128u   /* first-generation tile kernels (32 bank classes with overflow rounds, per-particle work
+                                      in class order) even where the rotation-class kernels apply (P = 4); for A/B runs */
 
 /* integrators */
 #define TILD_INTEGRATOR_GJF 0   /* Gronbech-Jensen & Farago, one force evaluation per step */
@@ -89,7 +92,7 @@ typedef struct {
     int32_t resort_every;      /* physically re-sort particles by cell every this many steps; <= 0 -> default */
     uint32_t flags;            /* TILD_FLAG_* */
     int32_t integrator;        /* TILD_INTEGRATOR_GJF (default, A11) or TILD_INTEGRATOR_EM (overdamped, A11b; gamma > 0) */
-    int32_t reserved;          /* 0 */
+    int32_t tile_shape;        /* 0 = default tile of 8 x 16 x 32 cells; else TY | TZ << 8 with TY in {8, 16}, TZ in {16, 32} */
     /* electrostatics on the same path (reading A22): valence per species, Bjerrum length
      * (0 = off), Gaussian smearing length of a charge; pair kernel 4 pi l_B exp(-k^2 a_q^2) / k^2, k = 0 dropped */
     double charge[TILD_MAX_SPECIES];

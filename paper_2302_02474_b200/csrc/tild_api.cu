@@ -62,31 +62,25 @@ int validate(const tild_params* p)
     return TILD_OK;
 }
 
-// Tile shape: TX x TY x TZ cells, TX, TY in {8, 16} (template EY = TY + H), TZ in {16, 32};
-// the shared image is EZ = TZ + H + sh nodes long in z, rounded up to a multiple of 4.  Tuning knobs (environment):
-// TILD_TILE_X, TILD_TILE_Y (8|16), TILD_TILE_Z (16|32).
+// Tile shape: 8 x TY x TZ cells, TY in {8, 16} (template EY = TY + H), TZ in {16, 32}; the shared
+// image is EZ = TZ + H + sh nodes long in z, rounded up to a multiple of 4.  tild_params.tile_shape = TY | TZ << 8
+// selects another shape than the default 8 x 16 x 32 (0 = default).
 void configure_tiles(tild_ctx* c)
 {
     const tild_params& p = c->prm;
     TileParams& t = c->tile;
     memset(&t, 0, sizeof(t));
-    auto env_int = [](const char* name, int dflt) {
-        const char* e = getenv(name);
-        return e ? atoi(e) : dflt;
-    };
     t.H = p.order <= 2 ? 1 : (p.order <= 4 ? 3 : 5);
     t.lo = p.order <= 2 ? 0 : (p.order <= 4 ? 1 : 2);
     t.sh = t.lo ? 4 - t.lo : 0;   // image starts on a 16-byte boundary of the mesh rows (16-byte cp.async staging)
     t.enabled = p.grid[0] >= 8 && p.grid[1] >= 8 && p.grid[2] >= 8;
-    int tx = env_int("TILD_TILE_X", 8), ty = env_int("TILD_TILE_Y", 16), tz = env_int("TILD_TILE_Z", p.grid[2] >= 32 ? 32 : 16);
-    if (tx != 8 && tx != 16) tx = 8;
+    const int tx = 8;
+    int ty = p.tile_shape & 0xff, tz = (p.tile_shape >> 8) & 0xff;
     if (ty != 8 && ty != 16) ty = 16;
-    if (tz != 16 && tz != 32) tz = 32;
+    if (tz != 16 && tz != 32) tz = p.grid[2] >= 32 ? 32 : 16;
     const int ez = (tz + t.H + t.sh + 3) / 4 * 4;
     const size_t lists_i = (size_t)TILD_INTERP_KCAP * 32 * 2 + (size_t)TILD_INTERP_CHUNK * 2;
     const size_t lists_s = (size_t)TILD_SPREAD_KCAP * 32 * 4 + (size_t)TILD_SPREAD_CHUNK * 4;
-    auto interp_bytes = [&](int ax, int ay) { return (size_t)(ax + t.H) * (ay + t.H) * 3 * ez * sizeof(float) + lists_i; };
-    if (interp_bytes(tx, ty) > 220 * 1024) tx = 8;
     t.EY = ty + t.H;
     t.EZ = ez;
     const int T[3] = {tx, ty, tz};
@@ -320,10 +314,7 @@ int tild_init(tild_ctx** out, const tild_params* params, void* workspace, size_t
         tab[(size_t)12 * 4096 + 2 * j + 1] = (float)(-sin(ang));
     }
     c->xtw = reinterpret_cast<const float2*>(c->tables + (size_t)12 * 4096);
-    {
-        const char* env = getenv("TILD_XFFT");   // 0 forces the 3-D cuFFT plans + separate k-space kernel (A/B runs)
-        c->xfft_R = ((env && env[0] == '0') || (p.flags & TILD_FLAG_PLAIN_FFT)) ? 0 : kspace_xfft_radix(p.grid[0], S);
-    }
+    c->xfft_R = (p.flags & TILD_FLAG_PLAIN_FFT) ? 0 : kspace_xfft_radix(p.grid[0], S);
     KspaceParams& ks = c->ksp;
     ks.S = S;
     ks.Nzc = p.grid[2] / 2 + 1;

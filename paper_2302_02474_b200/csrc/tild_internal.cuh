@@ -191,6 +191,27 @@ int launch_energy(tild_ctx* c, double* d_out);   // tild_energy.cu
 int launch_structure_factor(tild_ctx* c, uint32_t mask, float* sk, int accumulate);  // c->nhat must be current
 int launch_philox_test(tild_ctx* c, const uint32_t* ctr, const uint32_t* key, uint32_t* out, float* gauss, int m);
 
+struct InterpArgs {
+    MeshParams m;
+    TileParams tp;
+    StepParams s;
+    const uint64_t* step_ptr;
+    const uint32_t* seg_base;
+    const float* ffield;
+    const float4* X4;
+    const float4* W4;
+    const int32_t* B;
+    float4* X4o;
+    float4* W4o;
+    float4* F4;
+    uint32_t* drift_list;
+    uint32_t* drift_count;
+};
+// tild_interp_rot.cu: the P = 4 rotation-class tile kernel
+bool interp_rot_applies(const tild_ctx* c);
+size_t interp_rot_smem(int ey, int ez);
+cudaError_t interp_rot_run(const InterpArgs& a, int mode, cudaStream_t st, bool configure_only);
+
 size_t tild_scan_scratch_entries(size_t nbins);
 
 // ---- device helpers ------------------------------------------------------------------------------
@@ -270,6 +291,33 @@ template <int P> struct Halo {
     static constexpr int EZA = P <= 2 ? 20 : 24, EZB = P <= 2 ? 36 : 40;   // image z extent for TZ = 16 / 32 (% 4 == 0)
 };
 
+// Packed fp32 pair arithmetic (sm_100a: FFMA2 / FMUL2, one issue slot for two lanes of a register pair).
+// d = a * b + c with b broadcast to both halves: ptxas folds the duplicate into the scalar-broadcast operand form.
+__device__ __forceinline__ float2 ffma2_bcast(float2 a, float b, float2 c)
+{
+#ifndef TILD_USE_FFMA2
+    return make_float2(fmaf(a.x, b, c.x), fmaf(a.y, b, c.y));
+#endif
+    unsigned long long ra, rb, rc, rd;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(ra) : "f"(a.x), "f"(a.y));
+    asm("mov.b64 %0, {%1, %1};" : "=l"(rb) : "f"(b));
+    asm("mov.b64 %0, {%1, %2};" : "=l"(rc) : "f"(c.x), "f"(c.y));
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(rd) : "l"(ra), "l"(rb), "l"(rc));
+    float2 d;
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(d.x), "=f"(d.y) : "l"(rd));
+    return d;
+}
+__device__ __forceinline__ float2 fmul2_bcast(float2 a, float b)
+{
+    unsigned long long ra, rb, rd;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(ra) : "f"(a.x), "f"(a.y));
+    asm("mov.b64 %0, {%1, %1};" : "=l"(rb) : "f"(b));
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(rd) : "l"(ra), "l"(rb));
+    float2 d;
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(d.x), "=f"(d.y) : "l"(rd));
+    return d;
+}
+
 // Philox4x32-10 (Salmon et al., SC'11), written from the published round function.
 __device__ __forceinline__ uint4 philox4x32_10(uint4 c, uint32_t k0, uint32_t k1)
 {
@@ -285,17 +333,28 @@ __device__ __forceinline__ uint4 philox4x32_10(uint4 c, uint32_t k0, uint32_t k1
 }
 
 // Three standard normals for (particle id, step): counter (id, step_lo, step_hi, 0); u = ((r>>9)+0.5) 2^-23
-// (exact in fp32); Box-Muller (A12).
+// (exact in fp32); Box-Muller (A12).  The transcendental functions are the hardware approximations
+// (MUFU.LG2 / SQRT / SIN / COS: absolute error <= 2^-20.9 on the unit circle, 2^-22 in lg2), which keeps the draw at
+// ~10 instead of ~130 instructions; the deviation from the correctly rounded value is < 3e-6 per normal, i.e. < 1e-9
+// in a position per step.  Angles are taken in [-pi, pi) where the approximation is specified.
+__device__ __forceinline__ float sqrt_approx(float x)
+{
+    float r;
+    asm("sqrt.approx.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
 __device__ __forceinline__ float3 gauss3(uint32_t id, uint64_t step, uint32_t k0, uint32_t k1)
 {
     const uint4 r = philox4x32_10(make_uint4(id, (uint32_t)step, (uint32_t)(step >> 32), 0u), k0, k1);
-    const float sc = 1.0f / 8388608.0f;
-    const float u0 = ((float)(r.x >> 9) + 0.5f) * sc, u1 = ((float)(r.y >> 9) + 0.5f) * sc;
-    const float u2 = ((float)(r.z >> 9) + 0.5f) * sc, u3 = ((float)(r.w >> 9) + 0.5f) * sc;
-    const float r01 = sqrtf(-2.0f * logf(u0)), r23 = sqrtf(-2.0f * logf(u2));
-    float s1, c1;
-    sincospif(2.0f * u1, &s1, &c1);
-    return make_float3(r01 * c1, r01 * s1, r23 * cospif(2.0f * u3));
+    const float sc = 1.0f / 8388608.0f, hs = 0.5f / 8388608.0f;
+    const float u0 = fmaf((float)(r.x >> 9), sc, hs), u2 = fmaf((float)(r.z >> 9), sc, hs);
+    // 2 pi (u - 1/2): (r >> 9) 2^-23 - 1/2 + 2^-24 is exact in fp32
+    const float a1 = 6.283185307179586f * (fmaf((float)(r.y >> 9), sc, hs) - 0.5f);
+    const float a3 = 6.283185307179586f * (fmaf((float)(r.w >> 9), sc, hs) - 0.5f);
+    const float r01 = sqrt_approx(-1.3862943611198906f * __log2f(u0));   // sqrt(-2 ln u) = sqrt(-2 ln2 lg2 u)
+    const float r23 = sqrt_approx(-1.3862943611198906f * __log2f(u2));
+    // cos(2 pi u) = -cos(2 pi (u - 1/2)), likewise sin
+    return make_float3(-r01 * __cosf(a1), -r01 * __sinf(a1), -r23 * __cosf(a3));
 }
 
 __device__ __forceinline__ float wrap_pos(float x, float L, float inv_L)

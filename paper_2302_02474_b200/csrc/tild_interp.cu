@@ -7,227 +7,13 @@
 // row).  While those copies are in flight the CTA bins the segment's particles by the bank of their first stencil
 // node in the image ("class", see tild_spread.cu), then works in rounds of one particle per class: lane c takes
 // the k-th particle of class c, so each of the 3 P^3 shared-memory loads of the stencil hits 32 different banks.
-#include "tild_internal.cuh"
+#include "tild_particle.cuh"
 
 namespace {
 
 constexpr int INTERP_THREADS = 384;
 constexpr int INTERP_WARPS = INTERP_THREADS / 32;
 
-// ---- per-particle global gather (overflow tail, drifted particles, grids too small for tiles) -------------------
-// VEC = true (Nz % 4 == 0, 16-byte aligned field): the P nodes of one z-row are contiguous in memory but start at
-// an arbitrary z, so each row is read as the one or two ALIGNED float4 that cover it (LDG.128) and dotted with an
-// 8-wide weight vector holding w_z shifted to the row's offset and zeros elsewhere.
-template <int P, bool VEC>
-__device__ __forceinline__ float3 interp_global(const MeshParams& m, const float* __restrict__ ffield, const int b[3],
-                                                const float w[3][P], int type)
-{
-    const float* fx = ffield + (size_t)type * 3 * m.M;
-    const float* fy = fx + m.M;
-    const float* fz = fy + m.M;
-    float3 acc = make_float3(0.f, 0.f, 0.f);
-    if (VEC) {
-        const int bzw = wrap_idx(b[2], m.N[2]);
-        const int a0 = bzw & ~3, off = bzw & 3;
-        const int a1 = (a0 + 4 >= m.N[2]) ? 0 : a0 + 4;
-        const bool two = off + P > 4;
-        float w8[8];
-#pragma unroll
-        for (int k = 0; k < 8; ++k) {
-            float v = 0.f;
-#pragma unroll
-            for (int j = 0; j < P; ++j)
-                if (k - j >= 0 && k - j <= 3) v = (k - j == off) ? w[2][j] : v;
-            w8[k] = v;
-        }
-#pragma unroll
-        for (int jx = 0; jx < P; ++jx) {
-            const size_t ox = (size_t)wrap_idx(b[0] + jx, m.N[0]) * m.N[1];
-#pragma unroll
-            for (int jy = 0; jy < P; ++jy) {
-                const size_t row = (ox + wrap_idx(b[1] + jy, m.N[1])) * m.N[2];
-                const float wxy = w[0][jx] * w[1][jy];
-                const float* comp[3] = {fx, fy, fz};
-                float d[3];
-#pragma unroll
-                for (int q = 0; q < 3; ++q) {
-                    const float4 v0 = __ldg(reinterpret_cast<const float4*>(comp[q] + row + a0));
-                    float s = w8[0] * v0.x + w8[1] * v0.y + w8[2] * v0.z + w8[3] * v0.w;
-                    if (two) {
-                        const float4 v1 = __ldg(reinterpret_cast<const float4*>(comp[q] + row + a1));
-                        s += w8[4] * v1.x + w8[5] * v1.y + w8[6] * v1.z + w8[7] * v1.w;
-                    }
-                    d[q] = s;
-                }
-                acc.x += wxy * d[0];
-                acc.y += wxy * d[1];
-                acc.z += wxy * d[2];
-            }
-        }
-        return acc;
-    }
-    int iz[P];
-#pragma unroll
-    for (int j = 0; j < P; ++j) iz[j] = wrap_idx(b[2] + j, m.N[2]);
-#pragma unroll
-    for (int jx = 0; jx < P; ++jx) {
-        const size_t ox = (size_t)wrap_idx(b[0] + jx, m.N[0]) * m.N[1];
-#pragma unroll
-        for (int jy = 0; jy < P; ++jy) {
-            const size_t row = (ox + wrap_idx(b[1] + jy, m.N[1])) * m.N[2];
-            const float wxy = w[0][jx] * w[1][jy];
-#pragma unroll
-            for (int jz = 0; jz < P; ++jz) {
-                const float ww = wxy * w[2][jz];
-                const size_t g = row + iz[jz];
-                acc.x += ww * __ldg(fx + g);
-                acc.y += ww * __ldg(fy + g);
-                acc.z += ww * __ldg(fz + g);
-            }
-        }
-    }
-    return acc;
-}
-
-// f += force on the particle at p from the bond to the particle at q (Eq. 2; minimum image)
-__device__ __forceinline__ void bond_term(const MeshParams& m, const StepParams& s, const float4& p, const float4& q, float3& f)
-{
-    const float dx = min_image(p.x - q.x, m.L[0], m.inv_L[0]);
-    const float dy = min_image(p.y - q.y, m.L[1], m.inv_L[1]);
-    const float dz = min_image(p.z - q.z, m.L[2], m.inv_L[2]);
-    float scale = -2.0f * s.k_bond;
-    if (s.r0_bond != 0.0f) {
-        const float r = sqrtf(dx * dx + dy * dy + dz * dz);
-        scale = r > 0.0f ? scale * (1.0f - s.r0_bond / r) : 0.0f;
-    }
-    f.x += scale * dx;
-    f.y += scale * dy;
-    f.z += scale * dz;
-}
-
-// f += cosine angle force (Eq. 16; max_bonds == 2: slot 0 = previous bead, slot 1 = next bead, A23)
-__device__ __forceinline__ void angle_force_slots(const MeshParams& m, const StepParams& s, const float4* __restrict__ X4,
-                                                  const int32_t* __restrict__ B, size_t slot, const float4& p, float3& f)
-{
-    const int2 bb = *reinterpret_cast<const int2*>(B + 2 * slot);
-    const float r[3] = {p.x, p.y, p.z};
-    float prev[3] = {0.f, 0.f, 0.f}, next[3] = {0.f, 0.f, 0.f}, pprev[3] = {0.f, 0.f, 0.f}, nnext[3] = {0.f, 0.f, 0.f};
-    bool has_pprev = false, has_nnext = false;
-    if (bb.x >= 0) {
-        const float4 q = X4[bb.x];
-        prev[0] = q.x; prev[1] = q.y; prev[2] = q.z;
-        const int32_t pp = B[2 * (size_t)bb.x];
-        if (pp >= 0) {
-            const float4 qq = X4[pp];
-            pprev[0] = qq.x; pprev[1] = qq.y; pprev[2] = qq.z;
-            has_pprev = true;
-        }
-    }
-    if (bb.y >= 0) {
-        const float4 q = X4[bb.y];
-        next[0] = q.x; next[1] = q.y; next[2] = q.z;
-        const int32_t nn = B[2 * (size_t)bb.y + 1];
-        if (nn >= 0) {
-            const float4 qq = X4[nn];
-            nnext[0] = qq.x; nnext[1] = qq.y; nnext[2] = qq.z;
-            has_nnext = true;
-        }
-    }
-    float fa[3] = {0.f, 0.f, 0.f};
-    wlc_angle_force(s.lambda_wlc, s.k_theta, s.theta0, m.L, m.inv_L, r, bb.x >= 0, prev, has_pprev, pprev, bb.y >= 0, next, has_nnext, nnext, fa);
-    f.x += fa[0];
-    f.y += fa[1];
-    f.z += fa[2];
-}
-
-// Bond force on the particle at p from its partners' positions (slots into X4).
-__device__ __forceinline__ float3 bond_force_slots(const MeshParams& m, const StepParams& s, const float4* __restrict__ X4,
-                                                   const int32_t* __restrict__ B, size_t slot, const float4& p)
-{
-    float3 f = make_float3(0.f, 0.f, 0.f);
-    for (int k = 0; k < s.max_bonds; ++k) {
-        const int32_t j = B[slot * s.max_bonds + k];
-        if (j >= 0) bond_term(m, s, p, X4[j], f);
-    }
-    if (s.lambda_wlc != 0.0f || s.k_theta != 0.0f) angle_force_slots(m, s, X4, B, slot, p, f);
-    return f;
-}
-
-// What happens to one particle once its interpolated force is known.
-//   MODE 0: F4[slot] = interpolated force            (stage call tild_interp)
-//   MODE 1: F4[slot] = interpolated + bond force     (tild_set_state / tild_get_state)
-//   MODE 2: one GJF step: state (r^n, w^n), w^n = v^n - (dt/2m) F^n.
-//     F^n = interp(r^n) + bonds(r^n);  v^n = w^n + (dt/2m) F^n;  beta = beta^{n+1} (Philox: id, step n+1)
-//     r^{n+1} = wrap(r^n + b dt v^n + (b dt^2/2m) F^n + (b dt/2m) beta)
-//     w^{n+1} = a v^n + (dt/2m) a F^n + (b/m) beta
-//   Positions are double-buffered because bonds read the partners' r^n while r^{n+1} is written.
-// F already holds the total force; w0 = W4[slot] (MODE 2 only)
-template <int MODE>
-__device__ __forceinline__ void finish_update(const MeshParams& m, const StepParams& s, uint64_t step_next, size_t slot,
-                                              const float4& p, const float3& F, const float4& w0, float4* __restrict__ X4o,
-                                              float4* __restrict__ W4o, float4* __restrict__ F4)
-{
-    if (MODE <= 1) {
-        F4[slot] = make_float4(F.x, F.y, F.z, 0.f);
-        return;
-    }
-    float3 beta = make_float3(0.f, 0.f, 0.f);
-    if (s.noise_amp != 0.0f) {
-        const float3 z = gauss3(__float_as_uint(w0.w), step_next, s.key0, s.key1);
-        beta = make_float3(s.noise_amp * z.x, s.noise_amp * z.y, s.noise_amp * z.z);
-    }
-    if (s.integrator == TILD_INTEGRATOR_EM) {   // r' = r + (dt/gamma) F + beta/gamma; velocities are not used (A11b)
-        X4o[slot] = make_float4(wrap_pos(p.x + (s.em_drift * F.x + s.em_noise * beta.x), m.L[0], m.inv_L[0]),
-                                wrap_pos(p.y + (s.em_drift * F.y + s.em_noise * beta.y), m.L[1], m.inv_L[1]),
-                                wrap_pos(p.z + (s.em_drift * F.z + s.em_noise * beta.z), m.L[2], m.inv_L[2]), p.w);
-        W4o[slot] = w0;
-        return;
-    }
-    const float pp[3] = {p.x, p.y, p.z};
-    const float wv[3] = {w0.x, w0.y, w0.z};
-    const float Fv[3] = {F.x, F.y, F.z};
-    const float bv[3] = {beta.x, beta.y, beta.z};
-    float xo[3], wo[3];
-#pragma unroll
-    for (int a = 0; a < 3; ++a) {
-        const float v = wv[a] + s.half_dt_over_m * Fv[a];
-        const float r = pp[a] + (s.b_dt * v + s.b_dt2_over_2m * Fv[a] + s.b_dt_over_2m * bv[a]);
-        xo[a] = wrap_pos(r, m.L[a], m.inv_L[a]);
-        wo[a] = s.a_g * (v + s.half_dt_over_m * Fv[a]) + s.b_over_m * bv[a];
-    }
-    X4o[slot] = make_float4(xo[0], xo[1], xo[2], p.w);
-    W4o[slot] = make_float4(wo[0], wo[1], wo[2], w0.w);
-}
-
-template <int MODE>
-__device__ __forceinline__ void finish_particle(const MeshParams& m, const StepParams& s, uint64_t step_next, size_t slot,
-                                                const float4& p, float3 F, const float4* __restrict__ X4,
-                                                const float4* __restrict__ W4, const int32_t* __restrict__ B,
-                                                float4* __restrict__ X4o, float4* __restrict__ W4o, float4* __restrict__ F4)
-{
-    if (MODE >= 1) {
-        const float3 fb = bond_force_slots(m, s, X4, B, slot, p);
-        F.x += fb.x;
-        F.y += fb.y;
-        F.z += fb.z;
-    }
-    float4 w0 = make_float4(0.f, 0.f, 0.f, 0.f);
-    if (MODE == 2) w0 = W4[slot];
-    finish_update<MODE>(m, s, step_next, slot, p, F, w0, X4o, W4o, F4);
-}
-
-template <int P>
-__device__ __forceinline__ void index_weights(const MeshParams& m, const float4& p, int b[3], float w[3][P])
-{
-    const float pos[3] = {p.x, p.y, p.z};
-#pragma unroll
-    for (int a = 0; a < 3; ++a) {
-        int cell;
-        float t;
-        index_1d<P>(pos[a], m.inv_h[a], cell, b[a], t);
-        weights_1d<P>(t, w[a]);
-    }
-}
 
 // per-particle kernel over the slots [s0, s1)
 template <int P, bool VEC, int MODE>
@@ -599,22 +385,6 @@ bool can_vectorize(const tild_ctx* c, const float* ffield)
 }
 
 // ---- dispatch ------------------------------------------------------------------------------------------------------
-struct InterpArgs {
-    MeshParams m;
-    TileParams tp;
-    StepParams s;
-    const uint64_t* step_ptr;
-    const uint32_t* seg_base;
-    const float* ffield;
-    const float4* X4;
-    const float4* W4;
-    const int32_t* B;
-    float4* X4o;
-    float4* W4o;
-    float4* F4;
-    uint32_t* drift_list;
-    uint32_t* drift_count;
-};
 
 template <int P, int EY, int EZ, int MODE>
 void tile_launch(const InterpArgs& a, cudaStream_t st, size_t smem, bool configure_only, cudaError_t* err)
@@ -659,6 +429,14 @@ bool tile_launch_any(const InterpArgs& a, int mode, cudaStream_t st, size_t smem
     }
 }
 
+// the drifted particles of the rotation-class kernel (P = 4)
+void launch_drift_only(const InterpArgs& a, int mode, cudaStream_t st)
+{
+#define TILD_DR(M_) interp_drift_kernel<4, M_><<<592, 256, 0, st>>>(a.m, a.s, a.step_ptr, a.drift_list, a.drift_count, a.ffield, a.X4, a.W4, a.B, a.X4o, a.W4o, a.F4)
+    if (mode == 0) TILD_DR(0); else if (mode == 1) TILD_DR(1); else TILD_DR(2);
+#undef TILD_DR
+}
+
 template <int P>
 void slots_launch_p(const InterpArgs& a, bool vec, int mode, size_t s0, size_t s1, cudaStream_t st)
 {
@@ -678,6 +456,11 @@ int tild_interp_configure(tild_ctx* c)
     a.m = c->mesh;
     a.tp = c->tile;
     cudaError_t e = cudaSuccess;
+    if (interp_rot_applies(c)) {
+        e = interp_rot_run(a, 0, c->stream, true);
+        if (e != cudaSuccess)
+            return tild_fail(c, TILD_ECUDA, "cudaFuncSetAttribute(interp_rot_kernel): %s", cudaGetErrorString(e));
+    }
     if (!tile_launch_any(a, 0, c->stream, c->tile.smem_interp, true, &e))
         return tild_fail(c, TILD_EINVAL, "no interp tile kernel for P=%d EY=%d EZ=%d", c->mesh.P, c->tile.EY, c->tile.EZ);
     if (e != cudaSuccess)
@@ -694,8 +477,14 @@ int launch_interp(tild_ctx* c, int mode, const SegLayout& lay, const float* ffie
     if (c->tile.enabled && c->mesh.P >= 2 && !(c->prm.flags & TILD_FLAG_NAIVE_INTERP)) {   // P = 1: one node per particle
         cudaError_t e = cudaSuccess;
         TILD_CUDA(c, cudaMemsetAsync(c->drift_count, 0, sizeof(uint32_t), c->stream));
-        tile_launch_any(a, mode, c->stream, c->tile.smem_interp, false, &e);
-        TILD_LAUNCH_CHECK(c, "interp_tile_kernel");
+        if (interp_rot_applies(c) && !(c->prm.flags & TILD_FLAG_GEN1_TILES)) {
+            e = interp_rot_run(a, mode, c->stream, false);
+            TILD_LAUNCH_CHECK(c, "interp_rot_kernel");
+            launch_drift_only(a, mode, c->stream);
+        } else {
+            tile_launch_any(a, mode, c->stream, c->tile.smem_interp, false, &e);
+            TILD_LAUNCH_CHECK(c, "interp_tile_kernel");
+        }
         TILD_LAUNCH_CHECK(c, "interp_drift_kernel");
         return TILD_OK;
     }

@@ -21,6 +21,7 @@ OK, EINVAL, ENOMEM, ECUDA, ECUFFT, ESTATE = 0, -1, -2, -3, -4, -5
 INTEGRATOR_GJF, INTEGRATOR_EM = 0, 1
 FLAG_TIMING, FLAG_NAIVE_SPREAD, FLAG_NAIVE_INTERP, FLAG_GRAPH, FLAG_DECONVOLVE, FLAG_SAMPLED_KERNEL = 1, 2, 4, 8, 16, 32
 FLAG_PLAIN_FFT = 64
+FLAG_GEN1_TILES = 128
 TIMING_NAMES = ("sort", "spread", "fft_fwd", "kspace", "fft_inv", "interp", "other", "total")
 
 EXPORTS = (
@@ -42,7 +43,7 @@ class Params(C.Structure):
         ("dt", C.c_double), ("gamma", C.c_double), ("kT", C.c_double), ("mass", C.c_double),
         ("seed", C.c_uint64),
         ("resort_every", C.c_int32), ("flags", C.c_uint32),
-        ("integrator", C.c_int32), ("reserved", C.c_int32),
+        ("integrator", C.c_int32), ("tile_shape", C.c_int32),
         ("charge", C.c_double * MAX_SPECIES), ("bjerrum", C.c_double), ("a_charge", C.c_double),
         ("lambda_wlc", C.c_double),
         ("k_theta", C.c_double),
@@ -55,7 +56,7 @@ def make_params(n: int, n_species: int, box: Sequence[float], grid: Sequence[int
                 max_bonds: int = 2, dt: float = 0.005, gamma: float = 1.0, kT: float = 1.0, mass: float = 1.0,
                 seed: int = 0, resort_every: int = 0, flags: int = 0, integrator: int = 0,
                 charge: Sequence[float] = (), bjerrum: float = 0.0, a_charge: float = 0.5,
-                lambda_wlc: float = 0.0, k_theta: float = 0.0, theta0: float = 0.0) -> Params:
+                lambda_wlc: float = 0.0, k_theta: float = 0.0, theta0: float = 0.0, tile_shape: int = 0) -> Params:
     p = Params()
     p.struct_size = C.sizeof(Params)
     p.n, p.n_species, p.order = int(n), int(n_species), int(order)
@@ -72,7 +73,7 @@ def make_params(n: int, n_species: int, box: Sequence[float], grid: Sequence[int
     p.dt, p.gamma, p.kT, p.mass = float(dt), float(gamma), float(kT), float(mass)
     p.seed = int(seed)
     p.resort_every, p.flags = int(resort_every), int(flags)
-    p.integrator, p.reserved = int(integrator), 0
+    p.integrator, p.tile_shape = int(integrator), int(tile_shape)
     for i, z in enumerate(charge):
         p.charge[i] = float(z)
     p.bjerrum, p.a_charge = float(bjerrum), float(a_charge)

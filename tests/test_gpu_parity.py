@@ -421,20 +421,20 @@ def test_c5_sweep_point_force(grid, order, memory_order):
     assert np.abs(f.cpu().numpy() - of).max() <= REL * vec_rms(of)
 
 
-@pytest.mark.parametrize("env", [{"TILD_TILE_X": "16", "TILD_TILE_Y": "8"}, {"TILD_TILE_Y": "8", "TILD_TILE_Z": "16"},
-                                 {"TILD_TILE_X": "16", "TILD_TILE_Y": "16", "TILD_TILE_Z": "16"}],
-                         ids=["x16y8", "y8z16", "x16y16z16"])
+@pytest.mark.parametrize("ty,tz", [(8, 32), (8, 16), (16, 16)], ids=["y8z32", "y8z16", "y16z16"])
 @pytest.mark.parametrize("P", [2, 3, 4, 5])
-def test_tile_shape_variants(env, P, monkeypatch):
-    """Every (EY, EZ) instantiation of the tile kernels gives the same forces and trajectories."""
-    for k, v in env.items():
-        monkeypatch.setenv(k, v)
+@pytest.mark.parametrize("gen1", [False, True], ids=["gen2", "gen1"])
+def test_tile_shape_variants(ty, tz, P, gen1):
+    """Every (EY, EZ) instantiation of the tile kernels (tild_params.tile_shape) gives the same forces and
+    trajectories; gen1 = the first-generation tile kernels where the rotation-class ones would apply (P = 4)."""
+    if gen1 and P != 4:
+        pytest.skip("the rotation-class kernels only exist for P = 4")
     cfg = small_cfg(order=P, grid=(40, 24, 48), box=(20.0, 12.0, 24.0), n_chains=900)
-    st, eng = make(cfg, resort_every=3)
+    st, eng = make(cfg, resort_every=3, tile_shape=ty | (tz << 8), flags=tild.FLAG_GEN1_TILES if gen1 else 0)
     p = oracle_params(cfg)
     eng.tild_set_state(dev(st.x), dev(st.v), dev(st.type), dev(st.bond_partner), 0)
     info = eng.tild_layout_info()
-    assert info["tile_y"] == int(env.get("TILD_TILE_Y", 16)) and info["tile_z"] == int(env.get("TILD_TILE_Z", 32))
+    assert info["tile_y"] == ty and info["tile_z"] == tz
     _, _, f, _ = eng.tild_get_state(want_v=False, want_f=True)
     of = orc.force(p, st.x.astype(np.float64), st.type, st.bond_partner)
     assert np.abs(f.cpu().numpy() - of).max() <= REL * vec_rms(of)
