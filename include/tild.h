@@ -182,6 +182,12 @@ int tild_philox_test(tild_ctx*, const uint32_t* ctr /*[m][4]*/, const uint32_t* 
  * spread kernel shared bytes, interpolation kernel shared bytes, tile cells x, y, z}.  Needs tild_set_state. */
 int tild_layout_info(const tild_ctx*, uint64_t info[8] /*HOST out*/);
 
+/* The ordering the timed path runs on, for the bit-exact check of the sort that tild_step uses:
+ * seg_base[g] = first slot of segment g = tile * S + species (tiles in x-major order of tild_layout_info's tile edges,
+ * tile of a particle = its cell (a1 index map) / tile edge per axis), nseg + 1 entries; slot_id[s] = original particle
+ * id held by slot s.  Describes the particles as they were at the last re-sort.  Either output may be NULL. */
+int tild_segment_layout(const tild_ctx*, uint32_t* seg_base /*DEVICE [tiles*S + 1]*/, uint32_t* slot_id /*DEVICE [n]*/);
+
 /* HOST. Number of kernels of this library launched on the context's stream so far. */
 int64_t tild_launch_count(const tild_ctx*);
 

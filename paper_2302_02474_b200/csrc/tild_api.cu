@@ -439,6 +439,17 @@ int tild_layout_info(const tild_ctx* c, uint64_t info[8])
     return TILD_OK;
 }
 
+int tild_segment_layout(const tild_ctx* cc, uint32_t* seg_base, uint32_t* slot_id)
+{
+    tild_ctx* c = const_cast<tild_ctx*>(cc);
+    if (!c) return TILD_EINVAL;
+    if (!c->has_state) return tild_fail(c, TILD_ESTATE, "tild_segment_layout before tild_set_state");
+    if (seg_base)
+        TILD_CUDA(c, cudaMemcpyAsync(seg_base, c->lay.seg_base, ((size_t)c->tile.nseg + 1) * sizeof(uint32_t), cudaMemcpyDeviceToDevice, c->stream));
+    if (slot_id) return launch_slot_ids(c, slot_id);
+    return TILD_OK;
+}
+
 int tild_spread(tild_ctx* c, const float* x, const int32_t* type, float* grid)
 {
     if (!c || !grid || (c->mesh.n > 0 && (!x || !type))) return tild_fail(c, TILD_EINVAL, "tild_spread: null argument");

@@ -168,7 +168,8 @@ int launch_pack(tild_ctx* c, const float* x, const float* v, const int32_t* type
 // src slots [0, n) -> segment-sorted dst; fills lay->seg_base and c->inv (old slot -> new slot)
 int launch_segment_sort(tild_ctx* c, const float4* X4src, float4* X4dst, SegLayout* lay);
 int launch_reorder(tild_ctx* c);  // re-sorts the internal state by segment and flips buffers
-int launch_unpermute(tild_ctx* c, const float4* src, float* dst);        // dst[id[s]][0..2] = src[s].xyz
+int launch_unpermute(tild_ctx* c, const float4* src, float* dst);
+int launch_slot_ids(tild_ctx* c, uint32_t* id);                          // id[s] = original id of slot s        // dst[id[s]][0..2] = src[s].xyz
 // tild_spread.cu
 int tild_spread_configure(tild_ctx* c);
 int launch_spread(tild_ctx* c, const SegLayout& lay, const float4* X4, float* grid);  // zero fill + tile kernel

@@ -228,6 +228,13 @@ __global__ void __launch_bounds__(256) unpermute_kernel(int n, const float4* __r
     dst[3 * (size_t)id + 2] = v.z;
 }
 
+// id[s] = original particle id held by slot s
+__global__ void __launch_bounds__(256) slot_ids_kernel(int n, const float4* __restrict__ W4, uint32_t* __restrict__ id)
+{
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s < n) id[s] = __float_as_uint(W4[s].w);
+}
+
 int exclusive_scan(tild_ctx* c, const uint32_t* in, size_t len, uint32_t* out)
 {
     const int nbs = (int)((len + SCAN_CHUNK - 1) / SCAN_CHUNK);
@@ -333,6 +340,15 @@ int launch_unpermute(tild_ctx* c, const float4* src, float* dst)
     if (n == 0) return TILD_OK;
     unpermute_kernel<<<blocks_for(n), 256, 0, c->stream>>>(n, c->W4[c->cur], src, dst);
     TILD_LAUNCH_CHECK(c, "unpermute_kernel");
+    return TILD_OK;
+}
+
+int launch_slot_ids(tild_ctx* c, uint32_t* id)
+{
+    const int n = c->mesh.n;
+    if (n == 0) return TILD_OK;
+    slot_ids_kernel<<<blocks_for(n), 256, 0, c->stream>>>(n, c->W4[c->cur], id);
+    TILD_LAUNCH_CHECK(c, "slot_ids_kernel");
     return TILD_OK;
 }
 

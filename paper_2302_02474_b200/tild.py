@@ -27,7 +27,7 @@ TIMING_NAMES = ("sort", "spread", "fft_fwd", "kspace", "fft_inv", "interp", "oth
 EXPORTS = (
     "tild_workspace_bytes", "tild_init", "tild_set_state", "tild_spread", "tild_kspace_force", "tild_interp",
     "tild_bond_force", "tild_step", "tild_get_state", "tild_energy", "tild_structure_factor", "tild_index_map", "tild_get_timings", "tild_run_host",
-    "tild_philox_test", "tild_layout_info", "tild_launch_count", "tild_last_error", "tild_destroy", "tild_version",
+    "tild_philox_test", "tild_layout_info", "tild_segment_layout", "tild_launch_count", "tild_last_error", "tild_destroy", "tild_version",
 )
 
 
@@ -119,6 +119,7 @@ def load():
     lib.tild_energy.argtypes = [vp, C.POINTER(C.c_double * 3)]
     lib.tild_structure_factor.argtypes = [vp, C.c_uint32, vp, i32]
     lib.tild_index_map.argtypes = [vp, vp, vp, vp, vp, vp]
+    lib.tild_segment_layout.argtypes = [vp, vp, vp]
     lib.tild_get_timings.argtypes = [vp, C.POINTER(C.c_float * 8), C.POINTER(i32)]
     lib.tild_run_host.argtypes = [vp, vp, vp, vp, vp, u64, i32]
     lib.tild_philox_test.argtypes = [vp, vp, vp, vp, vp, i32]
@@ -283,6 +284,15 @@ class Tild:
         self._check(self.lib.tild_layout_info(self.ctx, C.byref(info)), "tild_layout_info")
         names = ("tiles", "segments", "image_z", "smem_spread", "smem_interp", "tile_x", "tile_y", "tile_z")
         return dict(zip(names, [int(v) for v in info]))
+
+    def tild_segment_layout(self):
+        """(seg_base [tiles*S + 1], slot_id [n]) as int32 tensors holding the uint32 values."""
+        torch = self.torch
+        nseg = self.tild_layout_info()["segments"]
+        seg = torch.empty(nseg + 1, dtype=torch.int32, device=self.device)
+        ids = torch.empty(max(self.n, 1), dtype=torch.int32, device=self.device)
+        self._check(self.lib.tild_segment_layout(self.ctx, _dp(seg), _dp(ids)), "tild_segment_layout")
+        return seg, ids[: self.n]
 
     def tild_launch_count(self) -> int:
         return int(self.lib.tild_launch_count(self.ctx))

@@ -17,6 +17,18 @@ pytestmark = pytest.mark.gpu
 REL = 1e-5
 
 
+def check(name, value, bound):
+    """assert value <= bound; the measured value is also appended to gpurun_out/margins.jsonl (when that folder exists)
+    so that every tolerance in this file can be read next to its measured margin."""
+    import json
+    import os
+    d = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "gpurun_out")
+    if os.path.isdir(d):
+        with open(os.path.join(d, "margins.jsonl"), "a") as fh:
+            fh.write(json.dumps({"name": name, "value": float(value), "bound": float(bound)}) + "\n")
+    assert value <= bound, (name, value, bound)
+
+
 def dev(a, dtype=None):
     t = torch.from_numpy(np.ascontiguousarray(a))
     if dtype is not None:
@@ -160,6 +172,11 @@ def test_fused_x_transform_kspace_path(cfg):
     assert np.abs(min_image(x - ox, cfg.box)).max() <= 1e-4
 
 
+# velocity after 100 steps, absolute (|v| ~ 1).  v is rebuilt from the split-kick state w + (dt/2m) F in fp32 and carries
+# 100 steps of fp32 force error; measured 1.4e-5 .. 5.6e-5 (C1, small cases, C2 full size): bound = 3.5 x the largest
+TOL_DV = 2e-4
+
+
 def run_trajectory(cfg, nsteps, **kw):
     st, eng = make(cfg, **kw)
     p = oracle_params(cfg)
@@ -176,16 +193,16 @@ def run_trajectory(cfg, nsteps, **kw):
 @pytest.mark.parametrize("resort_every", [1, 7, 1000])
 def test_trajectory_c1_100_steps(resort_every):
     ex, ev, _ = run_trajectory(inputs.C1, 100, resort_every=resort_every)
-    assert ex <= 1e-4, ex
-    assert ev <= 2e-3, ev
+    check(f"c1_100_dx_re{resort_every}", ex, 1e-4)
+    check(f"c1_100_dv_re{resort_every}", ev, TOL_DV)
 
 
 @pytest.mark.parametrize("cfg", [small_cfg(order=4), small_cfg(order=3, S=3, grid=(18, 12, 30), box=(9.0, 6.0, 15.0)),
                                  small_cfg(order=5)], ids=["P4", "P3_S3", "P5"])
 def test_trajectory_small_100_steps(cfg):
     ex, ev, _ = run_trajectory(cfg, 100, resort_every=9)
-    assert ex <= 1e-4, ex
-    assert ev <= 2e-3, ev
+    check(f"small_100_dx_{cfg.name}_S{cfg.n_species}", ex, 1e-4)
+    check(f"small_100_dv_{cfg.name}_S{cfg.n_species}", ev, TOL_DV)
 
 
 def test_noise_is_keyed_by_original_id_not_memory_order():
@@ -236,6 +253,11 @@ def test_empty_system():
     assert step == 3
 
 
+# hundreds of particles in one cell (density peaks ~400x the mean): measured 1.6e-7 .. 4.6e-7 of the RMS force, so the
+# north_star bound applies unchanged
+TOL_CROWDED = REL
+
+
 @pytest.mark.parametrize("P", [1, 2, 3, 4, 5])
 def test_crowded_cell_and_box_edges(P):
     """All particles in one cell at the periodic corner (maximum atomic contention, wrap on every axis),
@@ -266,7 +288,7 @@ def test_crowded_cell_and_box_edges(P):
     eng.tild_set_state(dev(x), dev(np.zeros_like(x)), dev(ty), dev(bp), 0)
     _, _, f, _ = eng.tild_get_state(want_v=False, want_f=True)
     of = orc.force(p, x.astype(np.float64), ty, bp)
-    assert np.abs(f.cpu().numpy() - of).max() <= 2e-5 * vec_rms(of)
+    check(f"crowded_force_P{P}", np.abs(f.cpu().numpy() - of).max() / vec_rms(of), TOL_CROWDED)
 
 
 def test_radix3_grid_and_rest_length():
@@ -358,8 +380,16 @@ def test_particles_that_drift_out_of_their_tile_fall_back_correctly():
     assert np.abs(f.cpu().numpy() - of).max() <= REL * vec_rms(of)
 
 
+def traj_errors(x, ox, box):
+    dx = min_image(x.cpu().numpy().astype(np.float64) - ox, box)
+    return float(np.sqrt((dx ** 2).sum(1).mean())), float(np.abs(dx).max())
+
+
 @pytest.mark.parametrize("name", ["C2", "C3"])
-def test_full_size_config_force_and_short_trajectory(name):
+def test_full_size_config_force_and_100_step_trajectory(name):
+    """BASELINE configs[1], [2] at full size: bit-exact index map, force on every particle, then 100 steps against the
+    oracle on the same Philox stream (north_star: trajectories over 100 steps within 1e-4; A18: max over particles of the
+    minimum-image |dr|).  Default tiles and re-sort cadence, i.e. ten re-sorts and the drift path are on the way."""
     cfg = inputs.CONFIGS[name]
     st, eng = make(cfg)
     p = oracle_params(cfg)
@@ -370,12 +400,52 @@ def test_full_size_config_force_and_short_trajectory(name):
     eng.tild_set_state(dev(st.x), dev(st.v), dev(st.type), dev(st.bond_partner), 0)
     _, _, f, _ = eng.tild_get_state(want_v=False, want_f=True)
     of = orc.force(p, st.x.astype(np.float64), st.type, st.bond_partner)
-    assert np.abs(f.cpu().numpy() - of).max() <= REL * vec_rms(of)
-    nst = 20 if name == "C2" else 5
+    check(f"{name}_force", np.abs(f.cpu().numpy() - of).max() / vec_rms(of), REL)
+    nst = 100
     eng.tild_step(nst)
-    x, v, _, _ = eng.tild_get_state()
-    ox, ov, _ = orc.run(p, st.x.astype(np.float64), st.v.astype(np.float64), st.type, st.bond_partner, 0, nst)
-    assert np.abs(min_image(x.cpu().numpy().astype(np.float64) - ox, cfg.box)).max() <= 1e-4
+    x, v, _, step = eng.tild_get_state()
+    assert step == nst
+    ox, ov, _ = orc.run(p, st.x.astype(np.float64), st.v.astype(np.float64), st.type, st.bond_partner, 0, nst, f=of)
+    erms, emax = traj_errors(x, ox, cfg.box)
+    # A18: positions are fp32 numbers up to L; every step rounds them once (ulp 1.9e-6 at L = 32, 7.6e-6 at L = 80), so
+    # 100 steps leave a random walk of 100 roundings that the double-precision oracle does not have: RMS ~ 2e-5 and a
+    # 5-sigma maximum over 3 M coordinates ~ 1.1e-4 at L = 80 (measured: C2 6.6e-6 / 2.6e-5, C3 2.0e-5 / 1.09e-4).
+    # Bound: RMS <= 1e-4 and max <= 1e-4 * max(1, L / 10 / 4) -- 1e-4 for L <= 40, 2e-4 at L = 80
+    check(f"{name}_100_dx_rms", erms, 1e-4)
+    check(f"{name}_100_dx_max", emax, 1e-4 * max(1.0, cfg.box[0] / 40.0))
+    check(f"{name}_100_dv_max", np.abs(v.cpu().numpy().astype(np.float64) - ov).max(), TOL_DV)
+
+
+@pytest.mark.parametrize("cfg", [small_cfg(order=4), small_cfg(order=3, S=3, grid=(18, 12, 30), box=(9.0, 6.0, 15.0)),
+                                 small_cfg(order=2, grid=(40, 24, 48), box=(20.0, 12.0, 24.0), n_chains=900), inputs.C2, inputs.C3],
+                         ids=["P4", "P3_S3", "P2_big", "C2", "C3"])
+def test_segment_sort_of_the_timed_path_is_bit_exact(cfg):
+    """The sort tild_set_state / tild_step run (by (tile, species) segment, tild_sort.cu: launch_segment_sort) against
+    a histogram built from the ORACLE's index map: seg_base must equal the exclusive prefix sum of the segment
+    histogram bit for bit, the slots must hold a permutation of the ids, and every slot of segment g must hold a
+    particle whose oracle segment is g (north_star: "cell sorting must be bit-exact"; A16: order inside a bin is free)."""
+    st, eng = make(cfg)
+    p = oracle_params(cfg)
+    eng.tild_set_state(dev(st.x), dev(st.v), dev(st.type), dev(st.bond_partner), 0)
+    info = eng.tild_layout_info()
+    seg, ids = eng.tild_segment_layout()
+    seg = seg.cpu().numpy().view(np.uint32).astype(np.int64)
+    ids = ids.cpu().numpy().view(np.uint32).astype(np.int64)
+    _, _, okey = orc.index_map(p, st.x)
+    N = np.array(cfg.grid, dtype=np.int64)
+    T = np.array([info["tile_x"], info["tile_y"], info["tile_z"]], dtype=np.int64)
+    nt = (N + T - 1) // T
+    okey = okey.astype(np.int64)
+    cx, cy, cz = okey // (N[1] * N[2]), (okey // N[2]) % N[1], okey % N[2]
+    tile = ((cx // T[0]) * nt[1] + cy // T[1]) * nt[2] + cz // T[2]
+    oseg = tile * cfg.n_species + st.type.astype(np.int64)
+    nseg = int(nt.prod()) * cfg.n_species
+    assert info["segments"] == nseg
+    expect = np.concatenate([[0], np.cumsum(np.bincount(oseg, minlength=nseg))])
+    assert np.array_equal(seg, expect)
+    assert np.array_equal(np.sort(ids), np.arange(cfg.n))
+    slot_seg = np.searchsorted(seg, np.arange(cfg.n), side="right") - 1
+    assert np.array_equal(oseg[ids], slot_seg)
 
 
 def test_layout_info_reports_the_tiling():
@@ -388,9 +458,11 @@ def test_layout_info_reports_the_tiling():
     assert info["smem_spread"] <= 113 * 1024 and info["smem_interp"] <= 113 * 1024      # two CTAs per SM
 
 
-def test_c4_full_size_force_and_two_steps():
+def test_c4_full_size_force_and_25_step_trajectory():
     """BASELINE configs[3], the bench workload, in the launch configuration bench.py times (default tiles, default
-    re-sort cadence): total force on every particle against the oracle, zero net force, then two steps."""
+    re-sort cadence of 10): total force on every particle against the oracle, zero net force, then 25 steps -- two
+    re-sorts and the drifted-particle path at scale -- on all 8.4 M particles.  A18: the fp32 ulp of a coordinate at
+    L = 160 is 1.5e-5, so the bound is RMS <= 1e-4 and max <= 1e-4 * L / 10; both are recorded."""
     cfg = inputs.C4
     st, eng = make(cfg)
     p = oracle_params(cfg)
@@ -399,15 +471,44 @@ def test_c4_full_size_force_and_two_steps():
     f = f.cpu().numpy()
     of = orc.force(p, st.x.astype(np.float64), st.type, st.bond_partner)
     scale = vec_rms(of)
-    assert np.abs(f - of).max() <= REL * scale, (np.abs(f - of).max(), scale)
+    check("C4_force", np.abs(f - of).max() / scale, REL)
     assert np.abs(f.astype(np.float64).sum(0)).max() < 1e-4 * scale * np.sqrt(cfg.n)
-    eng.tild_step(2)
+    nst = 25
+    eng.tild_step(nst)
     x, _, _, step = eng.tild_get_state(want_v=False)
-    assert step == 2
-    ox, _, _ = orc.run(p, st.x.astype(np.float64), st.v.astype(np.float64), st.type, st.bond_partner, 0, 2, f=of)
-    dx = min_image(x.cpu().numpy().astype(np.float64) - ox, cfg.box)
-    # A18: fp32 ulp at L = 160 is 1.5e-5; RMS <= 1e-4 and max <= 1e-4 * L / 10
-    assert np.sqrt((dx ** 2).sum(1).mean()) <= 1e-4 and np.abs(dx).max() <= 1e-4 * cfg.box[0] / 10.0
+    assert step == nst
+    ox, _, _ = orc.run(p, st.x.astype(np.float64), st.v.astype(np.float64), st.type, st.bond_partner, 0, nst, f=of)
+    erms, emax = traj_errors(x, ox, cfg.box)
+    check("C4_25_dx_rms", erms, TOL_C4_RMS)
+    check("C4_25_dx_max", emax, TOL_C4_MAX)
+
+
+# C4 / C5 trajectories (A18): positions are fp32 numbers up to L = 160 / 128, one ulp is 1.5e-5 / 7.6e-6, rounded once per
+# step.  Measured after 25 steps of C4: RMS 2.1e-5, max 1.09e-4; after 20 steps of C5: RMS 1.3e-5, max 4.9e-5.
+# Bounds = 3 x the measured values (well inside A18's RMS <= 1e-4, max <= 1e-4 * L / 10 for 100 steps)
+TOL_C4_RMS = 6e-5
+TOL_C4_MAX = 3.5e-4
+
+
+@pytest.mark.parametrize("memory_order", ["random", "sorted"])
+def test_c5_headline_point_force_and_20_steps(memory_order):
+    """BASELINE configs[4] at the point the sweep headlines (256^3, P = 4), in both particle memory orders: force on
+    every particle, then 20 steps (one re-sort)."""
+    cfg = inputs.c5(grid=256, order=4, memory_order=memory_order)
+    st, eng = make(cfg)
+    p = oracle_params(cfg)
+    eng.tild_set_state(dev(st.x), dev(st.v), dev(st.type), dev(st.bond_partner), 0)
+    _, _, f, _ = eng.tild_get_state(want_v=False, want_f=True)
+    of = orc.force(p, st.x.astype(np.float64), st.type, st.bond_partner)
+    check(f"C5_{memory_order}_force", np.abs(f.cpu().numpy() - of).max() / vec_rms(of), REL)
+    nst = 20
+    eng.tild_step(nst)
+    x, _, _, step = eng.tild_get_state(want_v=False)
+    assert step == nst
+    ox, _, _ = orc.run(p, st.x.astype(np.float64), st.v.astype(np.float64), st.type, st.bond_partner, 0, nst, f=of)
+    erms, emax = traj_errors(x, ox, cfg.box)
+    check(f"C5_{memory_order}_20_dx_rms", erms, 4e-5)
+    check(f"C5_{memory_order}_20_dx_max", emax, 1.5e-4)
 
 
 @pytest.mark.parametrize("grid,order,memory_order", [(192, 3, "random"), (128, 1, "chain")])
@@ -684,6 +785,12 @@ def test_coacervate_sized_charged_melt_force_and_steps():
     assert np.abs(min_image(x - ox, cfg.box)).max() <= 1e-4
 
 
+# angle potentials: measured 7.8e-7 (cosine) and 1.2e-6 (harmonic, 1/sin(theta) factor) of the RMS force: the
+# north_star bound applies unchanged
+TOL_WLC = REL
+TOL_HARMONIC = REL
+
+
 def test_wlc_angle_potential_parity():
     """Cosine angle potential (Eq. 16; reading A23) in the bond stage, the fused step and tild_energy."""
     cfg = small_cfg(order=3, n_chains=120, nb=12)
@@ -692,13 +799,13 @@ def test_wlc_angle_potential_parity():
     p = oracle_params(cfg, lambda_wlc=lam)
     fb = eng.tild_bond_force(dev(st.x), dev(st.bond_partner)).cpu().numpy()
     ofb = orc.bond_force(p, st.x.astype(np.float64), st.bond_partner)
-    assert np.abs(fb - ofb).max() <= 2e-5 * vec_rms(ofb)        # fp32 cancellation in d/|d|^3 terms of near-straight triplets
+    check("wlc_bond_force", np.abs(fb - ofb).max() / vec_rms(ofb), TOL_WLC)   # fp32 cancellation in near-straight triplets
     plain = orc.bond_force(oracle_params(cfg), st.x.astype(np.float64), st.bond_partner)
     assert np.abs(ofb - plain).max() > 0.1 * vec_rms(plain)      # the angles really contribute
     eng.tild_set_state(dev(st.x), dev(st.v), dev(st.type), dev(st.bond_partner), 0)
     _, _, f, _ = eng.tild_get_state(want_v=False, want_f=True)
     of = orc.force(p, st.x.astype(np.float64), st.type, st.bond_partner)
-    assert np.abs(f.cpu().numpy() - of).max() <= 2e-5 * vec_rms(of)
+    check("wlc_total_force", np.abs(f.cpu().numpy() - of).max() / vec_rms(of), TOL_WLC)
     e = eng.tild_energy()
     oe = orc.energy(p, st.x.astype(np.float64), st.v.astype(np.float64), st.type, st.bond_partner)
     assert np.all(np.abs(e - oe) <= 2e-5 * np.abs(oe).max()), (e, oe)
@@ -718,14 +825,14 @@ def test_harmonic_angle_potential_parity():
     p = oracle_params(cfg, **kw)
     fb = eng.tild_bond_force(dev(st.x), dev(st.bond_partner)).cpu().numpy()
     ofb = orc.bond_force(p, st.x.astype(np.float64), st.bond_partner)
-    assert np.abs(fb - ofb).max() <= 1e-4 * vec_rms(ofb)
-    assert np.abs(fb - ofb).max() <= 2e-5 * np.abs(ofb).max()
+    check("harmonic_bond_force_rms", np.abs(fb - ofb).max() / vec_rms(ofb), TOL_HARMONIC)
+    check("harmonic_bond_force_max", np.abs(fb - ofb).max() / np.abs(ofb).max(), 2e-5)
     wlc_only = orc.bond_force(oracle_params(cfg, lambda_wlc=0.5), st.x.astype(np.float64), st.bond_partner)
     assert np.abs(ofb - wlc_only).max() > 0.1 * vec_rms(wlc_only)
     eng.tild_set_state(dev(st.x), dev(st.v), dev(st.type), dev(st.bond_partner), 0)
     _, _, f, _ = eng.tild_get_state(want_v=False, want_f=True)
     of = orc.force(p, st.x.astype(np.float64), st.type, st.bond_partner)
-    assert np.abs(f.cpu().numpy() - of).max() <= 1e-4 * vec_rms(of)
+    check("harmonic_total_force", np.abs(f.cpu().numpy() - of).max() / vec_rms(of), TOL_HARMONIC)
     e = eng.tild_energy()
     oe = orc.energy(p, st.x.astype(np.float64), st.v.astype(np.float64), st.type, st.bond_partner)
     assert np.all(np.abs(e - oe) <= 2e-5 * np.abs(oe).max()), (e, oe)
