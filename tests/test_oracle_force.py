@@ -96,6 +96,8 @@ def discrete_transfer(P):
             return 0.75 + 0.25 * np.cos(kh)
         if P == 4:
             return (23.0 / 24.0) * np.cos(kh / 2) + (1.0 / 24.0) * np.cos(1.5 * kh)
+        if P == 5:     # weights at t = 0: {1, 76, 230, 76, 1} / 384 on nodes -2..2
+            return 115.0 / 192.0 + (19.0 / 48.0) * np.cos(kh) + (1.0 / 192.0) * np.cos(2 * kh)
         raise ValueError
     return lambda KX, KY, KZ, h: (d1(KX * h[0]) * d1(KY * h[1]) * d1(KZ * h[2])) ** 2
 
@@ -108,7 +110,7 @@ def sinc_transfer(P):
 CHI3 = np.array([[0.0, 1.0, 0.3], [1.0, 0.0, 2.0], [0.3, 2.0, 0.0]])
 
 
-@pytest.mark.parametrize("P", [1, 2, 3, 4])
+@pytest.mark.parametrize("P", [1, 2, 3, 4, 5])
 def test_lattice_particles_equal_closed_form_ksum(P):
     """(a) exact to round-off; non-cubic box and grid so a transposed axis fails."""
     rng = np.random.default_rng(100 + P)
@@ -130,7 +132,7 @@ def test_lattice_particles_equal_closed_form_ksum(P):
     assert np.abs(F - ref).max() < 2e-6 * scale      # fp32 positions: |t| <= 1e-6 instead of exactly 0
 
 
-@pytest.mark.parametrize("P,bound_coarse,bound_fine", [(2, 0.4, 0.08), (3, 0.08, 0.01), (4, 0.03, 0.0015)])
+@pytest.mark.parametrize("P,bound_coarse,bound_fine", [(2, 0.4, 0.08), (3, 0.08, 0.01), (4, 0.03, 0.0015), (5, 0.02, 0.0005)])
 def test_general_positions_vs_sinc_smeared_ksum(P, bound_coarse, bound_fine):
     """(b) PM = k-sum with W^(k)^2 up to aliasing; the error falls by > 2^P when h is halved."""
     rng = np.random.default_rng(7)
@@ -186,7 +188,7 @@ def test_direct_pair_sum_equals_full_ksum():
     assert np.abs(a - b).max() < 1e-9 * np.abs(b).max()
 
 
-@pytest.mark.parametrize("P", [1, 2, 3, 4])
+@pytest.mark.parametrize("P", [1, 2, 3, 4, 5])
 def test_zero_net_force_and_self_force(P):
     """(d) momentum conservation to round-off (needs A6), and a lone particle feels no force."""
     rng = np.random.default_rng(21)
@@ -429,3 +431,91 @@ def test_electrostatics_off_and_neutral_species_feel_nothing():
     assert np.abs(F1 - F0)[ty == 2].max() < 1e-12                             # the neutral species gains no force
     assert np.abs(F1 - F0)[ty != 2].max() > 1e-3
     assert np.abs(F1.sum(0)).max() < 1e-10 * np.abs(F1).max() * n            # momentum conservation survives
+
+
+# ---- energies of the kernel variants (O10 with the sampled kernel / with electrostatics) ------------------------------
+def test_sampled_kernel_mesh_energy_is_the_pair_sum_of_the_sampled_potential():
+    """With P = 1 every particle is one unit of density on its nearest node, and the kernel obtained by transforming
+    u_G sampled on the mesh (reading A5b) turns the mesh energy (1/2V) sum_m u^_s(m) sum_IJ c_IJ Re[n^_I n^_J*]
+    into the plain double sum  1/2 sum_{a, b} c_{I(a) J(b)} u_G(minimum image of node_a - node_b)  (a = b included):
+    the identity sum_m exp(2 pi i m (g - g') / N) = M delta_{g g'} makes it exact.  Written out by brute force here."""
+    rng = np.random.default_rng(12)
+    L, N, sigma2 = (6.0, 4.5, 7.0), (12, 8, 10), 0.5
+    h = np.array(L) / np.array(N)
+    n = 40
+    cells = np.stack([rng.integers(0, N[a], size=n) for a in range(3)], axis=1)
+    jitter = (rng.random((n, 3)) - 0.5) * 0.6                        # anywhere in the cell of the nearest node
+    x = (((cells + jitter) % np.array(N)) * h).astype(np.float32)
+    ty = rng.integers(0, 3, size=n).astype(np.int32)
+    kappa, rho0 = 5.0, 2.0
+    p = orc.OracleParams(n, 3, L, N, 1, CHI3, kappa=kappa, sigma2=sigma2, rho0=rho0, sampled_kernel=True, k_bond=0.0)
+    base, _, _ = orc.index_map(p, x)
+    node = base % np.array(N)
+    c = c_matrix(CHI3, kappa, rho0)
+    E = 0.0
+    norm = (2 * np.pi * sigma2) ** -1.5
+    for a in range(n):
+        for b in range(n):
+            d = (node[a] - node[b]) * h
+            d -= np.array(L) * np.round(d / np.array(L))
+            E += 0.5 * c[ty[a], ty[b]] * norm * np.exp(-(d ** 2).sum() / (2 * sigma2))
+    bp = -np.ones((n, 2), dtype=np.int32)
+    e = orc.energy(p, x.astype(np.float64), np.zeros((n, 3)), ty, bp)
+    assert abs(e[2] - E) < 1e-10 * abs(E), (e[2], E)
+
+
+def ewald_smeared_energy(x, z, L, lB, aq, alpha, kmax=12, images=2):
+    """Energy of Gaussian-smeared point charges in a neutralising background (k = 0 dropped), self terms included:
+    E = 1/2 sum_{i, j, images} z_i z_j phi(r),  phi(r) = lB erf(r / 2 aq) / r,  phi(0) = lB / (aq sqrt(pi)).
+    Ewald split with parameter alpha: [erf(r/2aq) - erf(alpha r)] / r in real space (limit (2/sqrt(pi)) (1/2aq - alpha) at
+    r = 0) + 4 pi exp(-k^2 / 4 alpha^2) / k^2 in k-space.  Independent of alpha; written independently of the oracle."""
+    from scipy.special import erf
+    x = np.asarray(x, dtype=np.float64)
+    L = np.asarray(L, dtype=np.float64)
+    n = len(x)
+    E = 0.0
+    rng_img = range(-images, images + 1)
+    for i in range(n):
+        for j in range(n):
+            for a in rng_img:
+                for b in rng_img:
+                    for c in rng_img:
+                        d = x[i] - x[j] + L * np.array([a, b, c])
+                        r = np.linalg.norm(d)
+                        if r == 0.0:
+                            E += 0.5 * lB * z[i] * z[j] * (2 / np.sqrt(np.pi)) * (1 / (2 * aq) - alpha)
+                        else:
+                            E += 0.5 * lB * z[i] * z[j] * (erf(r / (2 * aq)) - erf(alpha * r)) / r
+    V = L.prod()
+    ms = np.arange(-kmax, kmax + 1)
+    MX, MY, MZ = np.meshgrid(ms, ms, ms, indexing="ij")
+    KX, KY, KZ = 2 * np.pi * MX / L[0], 2 * np.pi * MY / L[1], 2 * np.pi * MZ / L[2]
+    K2 = KX ** 2 + KY ** 2 + KZ ** 2
+    K2[kmax, kmax, kmax] = 1.0
+    G = 4 * np.pi * lB * np.exp(-K2 / (4 * alpha ** 2)) / K2
+    G[kmax, kmax, kmax] = 0.0
+    S = sum(z[j] * np.exp(-1j * (KX * x[j, 0] + KY * x[j, 1] + KZ * x[j, 2])) for j in range(n))
+    return E + 0.5 * (G * np.abs(S) ** 2).sum() / V
+
+
+def test_electrostatic_mesh_energy_matches_ewald_energy_of_smeared_charges():
+    """O10 with a Bjerrum length: the mesh energy (1/2V) sum_{k != 0} u^_el(k) |rho^_c(k)|^2 (self terms included) with
+    the deconvolved kernel against the Ewald ENERGY evaluated with two different splitting parameters."""
+    rng = np.random.default_rng(11)
+    L = (6.0, 6.0, 6.0)
+    n, lB, aq = 8, 2.5, 0.5
+    x = (rng.random((n, 3)) * 6.0).astype(np.float32)
+    ty = np.array([0, 1] * (n // 2), dtype=np.int32)
+    zsp = (1.0, -1.0)
+    z = np.array([zsp[t] for t in ty])
+    e1 = ewald_smeared_energy(x, z, L, lB, aq, alpha=1.0 / (2 * aq))         # real-space part vanishes identically
+    e2 = ewald_smeared_energy(x, z, L, lB, aq, alpha=0.7 / (2 * aq))
+    assert abs(e1 - e2) < 1e-9 * abs(e1), (e1, e2)
+    bp = -np.ones((n, 2), dtype=np.int32)
+    errs = []
+    for Ng in (24, 48):
+        p = orc.OracleParams(n, 2, L, (Ng,) * 3, 4, np.zeros((2, 2)), kappa=0.0, sigma2=0.5, rho0=1.0,
+                             charge=zsp, bjerrum=lB, a_charge=aq, deconvolve=True, k_bond=0.0)
+        e = orc.energy(p, x.astype(np.float64), np.zeros((n, 3)), ty, bp)
+        errs.append(abs(e[2] - e2) / abs(e2))
+    assert errs[0] < 2e-3 and errs[1] < 1e-4, (errs, e2)

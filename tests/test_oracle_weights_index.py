@@ -77,7 +77,7 @@ def _params(n, L, N, P, S=1):
     return orc.OracleParams(n, S, L, N, P, np.zeros((S, S)), 1.0, 0.5)
 
 
-@pytest.mark.parametrize("P", [1, 2, 3, 4])
+@pytest.mark.parametrize("P", [1, 2, 3, 4, 5])
 def test_index_map_definition(P):
     rng = np.random.default_rng(5)
     L, N = (10.0, 7.0, 12.5), (16, 12, 20)
