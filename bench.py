@@ -50,8 +50,8 @@ def algorithmic_bytes(cfg):
 
 
 def sample_config(cfg):
-    """Bounded CPU-baseline sample: the same recipe at 1/64 of the volume and particle count (same density,
-    same h, same P) for the big workloads; the workload itself when it is already small."""
+    """The same recipe at 1/64 of the volume and particle count (same density, same h, same P): used for the ONE-CORE
+    oracle figure of the big workloads, where a full-size single-core step would take about a minute."""
     if cfg.n <= 70000:
         return cfg, "the full workload"
     scale = 1.0 / 64.0
@@ -62,21 +62,55 @@ def sample_config(cfg):
                f"(same density and mesh spacing)")
 
 
-def run_oracle(cfg, steps, warmup):
-    """Times oracle.run on the host cores.  Returns (particle-steps/s, ms/step, cores)."""
+class OracleRun:
+    """The CPU oracle (oracle/, as it stands) on one workload: state kept between calls so that steps can be timed
+    one batch at a time."""
+
+    def __init__(self, cfg, threads=None):
+        from oracle import tild_oracle as orc
+        self.orc, self.cfg = orc, cfg
+        if threads:
+            orc.set_threads(threads)
+        self.cores = orc.get_threads()
+        st = inputs.make_state(cfg)
+        self.st = st
+        self.p = orc.OracleParams(cfg.n, cfg.n_species, cfg.box, cfg.grid, cfg.order, np.array(cfg.chi), cfg.kappa, cfg.sigma2,
+                                  k_bond=cfg.k_bond, r0_bond=cfg.r0_bond, dt=cfg.dt, gamma=cfg.gamma, kT=cfg.kT, mass=cfg.mass,
+                                  seed=cfg.philox_seed)
+        self.x, self.v = st.x.astype(np.float64), st.v.astype(np.float64)
+        self.f = orc.force(self.p, self.x, st.type, st.bond_partner)
+        self.step = 0
+
+    def run(self, nsteps):
+        """Advances nsteps; returns seconds."""
+        t0 = time.perf_counter()
+        self.x, self.v, self.f = self.orc.run(self.p, self.x, self.v, self.st.type, self.st.bond_partner, self.step, nsteps, f=self.f)
+        self.step += nsteps
+        return time.perf_counter() - t0
+
+
+def oracle_rate(cfg, budget_s, max_steps, threads=None):
+    """particle-steps/s of the oracle on cfg: one step to size the run, then as many more as fit in budget_s (at most
+    max_steps in all).  Returns (rate, ms per step, cores, steps timed)."""
+    o = OracleRun(cfg, threads)
+    t1 = o.run(1)
+    more = int(max(0, min(max_steps - 1, (budget_s - t1) // max(t1, 1e-6))))
+    t = t1 + (o.run(more) if more > 0 else 0.0)
+    k = 1 + more
+    return cfg.n * k / t, 1e3 * t / k, o.cores, k
+
+
+def cpu_baseline(cfg):
+    """The oracle timed on the box's host cores: FULL-SIZE workload on all cores (>= 3 steps for the big configs) and a
+    one-core figure (full size when a step takes under ~10 s on one core, else the 1/64-volume sample)."""
+    rate, ms, cores, k = oracle_rate(cfg, budget_s=18.0, max_steps=50 if cfg.n < 2e6 else 3)
+    scfg, what = sample_config(cfg)
+    r1, ms1, _, k1 = oracle_rate(scfg, budget_s=8.0, max_steps=20, threads=1)
     from oracle import tild_oracle as orc
-    st = inputs.make_state(cfg)
-    p = orc.OracleParams(cfg.n, cfg.n_species, cfg.box, cfg.grid, cfg.order, np.array(cfg.chi), cfg.kappa, cfg.sigma2,
-                         k_bond=cfg.k_bond, r0_bond=cfg.r0_bond, dt=cfg.dt, gamma=cfg.gamma, kT=cfg.kT, mass=cfg.mass,
-                         seed=cfg.philox_seed)
-    x, v = st.x.astype(np.float64), st.v.astype(np.float64)
-    f = orc.force(p, x, st.type, st.bond_partner)
-    if warmup > 0:
-        x, v, f = orc.run(p, x, v, st.type, st.bond_partner, 0, warmup, f=f)
-    t0 = time.perf_counter()
-    x, v, f = orc.run(p, x, v, st.type, st.bond_partner, warmup, steps, f=f)
-    dt = time.perf_counter() - t0
-    return cfg.n * steps / dt, 1e3 * dt / steps, orc.get_threads()
+    orc.set_threads(cores)
+    return {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle", "ms_per_step": ms,
+            "sample": f"the full workload ({cfg.n} particles, grid {cfg.grid[0]}^3), {k} steps on {cores} cores",
+            "one_core": {"value": r1, "unit": UNIT, "cores": 1, "ms_per_step": ms1, "sample": f"{what}; {k1} steps"}}
 
 
 def replica_seeds(cfg, rank):
@@ -140,17 +174,27 @@ class ClockSampler:
 
 
 def reference_arm(args, cfg):
+    """--impl reference: the oracle on the FULL-SIZE workload, all host cores.  A C4 step takes ~5 s, so the run is
+    bounded: W' = min(W, 1) warm-up steps and K' = as many of the K steps as fit in ~100 s; the rate is per step."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    scfg, what = sample_config(cfg)
-    value, ms, cores = run_oracle(scfg, max(1, args.steps), max(0, args.warmup))
+    o = OracleRun(cfg)
+    if args.warmup > 0:
+        o.run(1)
+    t1 = o.run(1)
+    more = int(max(0, min(max(1, args.steps) - 1, (100.0 - t1) // max(t1, 1e-6))))
+    t = t1 + (o.run(more) if more > 0 else 0.0)
+    k = 1 + more
+    value, ms = cfg.n * k / t, 1e3 * t / k
+    what = f"the full workload ({cfg.n} particles, grid {cfg.grid[0]}^3); {k} of the {args.steps} steps timed on {o.cores} cores"
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
-        "config": {"workload": cfg.name, "sample": what},
-        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": what},
+        "config": {"workload": cfg.name, "n": cfg.n, "grid": list(cfg.grid), "order": cfg.order, "species": cfg.n_species,
+                   "steps_timed": k},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": o.cores, "kind": "oracle", "sample": what},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }))
@@ -228,7 +272,7 @@ def ours_arm(args, cfg):
     for k in ("spread", "kspace", "interp"):
         gbs = alg[k] / (stage_ms[k] * 1e-3) / 1e9 if stage_ms[k] > 0 else 0.0
         stages[k] = {"ms": stage_ms[k], "alg_bytes": alg[k], "gbs": gbs, "frac": gbs / peak,
-                     "traffic": NCU_TRAFFIC.get((cfg.name, k))}
+                     "traffic": ncu_traffic(cfg.name, k)}
     if not (args.flags & tild.FLAG_PLAIN_FFT) and cfg.n_species <= 4 and cfg.grid[0] in (16, 32, 64, 128, 256):
         stages["kspace"]["note"] = ("fused x-transform kernel: this stage also does the x passes of all 4S FFTs; "
                                     "fft_fwd / fft_inv are the (y, z) passes only")
@@ -236,17 +280,15 @@ def ours_arm(args, cfg):
     three_ms = sum(stages[k]["ms"] for k in stages)
     three_gbs = sum(alg.values()) / (three_ms * 1e-3) / 1e9 if three_ms > 0 else 0.0
     roofline = {"bound": "hbm", "kernel": dom, "achieved": stages[dom]["gbs"], "peak": peak, "unit": "GB/s",
-                "frac": stages[dom]["gbs"] / peak, "traffic": NCU_TRAFFIC.get((cfg.name, dom)), "peak_source": peak_src,
+                "frac": stages[dom]["gbs"] / peak, "traffic": ncu_traffic(cfg.name, dom),
+                "traffic_source": {k: TRAFFIC.get(k) for k in ("commit", "date", "command")} if TRAFFIC else None,
+                "peak_source": peak_src,
                 "stages": stages,
                 "spread_kspace_interp": {"ms": three_ms, "gbs": three_gbs, "frac": three_gbs / peak,
                                          "frac_of_8TBs_nominal": three_gbs / 8000.0}}
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
-        scfg, what = sample_config(cfg)
-        _, ms1, cores = run_oracle(scfg, 1, 0)
-        k = int(min(50, max(2, 12e3 / max(ms1, 1e-3))))
-        val, _, cores = run_oracle(scfg, k, 0)
-        cpu = {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": f"{what}; {k} steps"}
+        cpu = cpu_baseline(cfg)
     print(json.dumps({
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -262,13 +304,27 @@ def ours_arm(args, cfg):
         dist.destroy_process_group()
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch from `ncu --set full` captures committed under profiles/
-# (key: (workload name, stage)); None until a capture exists.
-NCU_TRAFFIC = {   # profiles/r1_spread_interp_kspace_c4.md
-    ("C4_diblock_8m", "spread"): 358.0e6,
-    ("C4_diblock_8m", "kspace"): 482.5e6,
-    ("C4_diblock_8m", "interp"): 1172.0e6,
-}
+def load_traffic():
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch from the `ncu --set full` capture recorded in
+    profiles/traffic_c4.json (commit, date and command are in the file and echoed into the bench line, so a figure
+    that is older than the kernels is visible).  {} when the file is missing."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic_c4.json")) as f:
+            return json.load(f)
+    except Exception:
+        return {}
+
+
+TRAFFIC = load_traffic()
+
+
+def ncu_traffic(workload, stage):
+    if TRAFFIC.get("workload") != workload:
+        return None
+    ks = TRAFFIC.get("stages", {}).get(stage)
+    if not ks:
+        return None
+    return float(sum(k["dram_bytes_read"] + k["dram_bytes_write"] for k in ks))
 
 
 def sweep_arm(args):

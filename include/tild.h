@@ -21,7 +21,11 @@
  *    grids [species][Nx][Ny][Nz] float, z fastest, linear node index g = (ix*Ny + iy)*Nz + iz;
  *    force fields [species][3][Nx][Ny][Nz].  Box is [0,L) per axis, periodic, node g at g*h.
  *  - Return value: 0 on success, negative tild_status on failure; tild_last_error() gives text.
- *    No exceptions, no output to stdout/stderr, no global mutable state.
+ *    No exceptions, no output to stdout/stderr, no environment variables.  The only process-wide state is the
+ *    per-kernel shared-memory limit, which is only ever raised.  A context is bound to the CUDA device that was
+ *    current at tild_init; its entry points switch to that device and back.
+ *  - type[i] must be in [0, S) and bond_partner entries in [-1, n): tild_set_state checks both (synchronising once) and
+ *    returns TILD_EINVAL; the stage calls trust their arguments.
  *  - There is no CPU fallback: every entry point that computes needs a CUDA device.
  */
 #ifndef TILD_H
@@ -57,10 +61,11 @@ typedef enum {
 #define TILD_FLAG_PLAIN_FFT 64u    /* 3-D cuFFT plans + the element-wise k-space kernel even where the fused x-transform
                                       kernel applies (Nx in {16,32,64,128,256}, S <= 4).  For A/B runs: the results agree to fp32
                                       rounding */
-#define TILD_FLAG_GRAPH 8u         /* tild_step replays blocks of 2*resort_every steps as one CUDA graph (launch-bound
-                                      small systems); ignored with TILD_FLAG_TIMING, an odd resort_every, or the
-                                      legacy default stream (which cannot be captured) */
-
+#define TILD_FLAG_GRAPH 8u         /* accepted for compatibility: graph replay is the default (see TILD_FLAG_EAGER) */
+#define TILD_FLAG_EAGER 256u       /* launch every kernel of every step individually.  Default: tild_step replays blocks of
+                                      2*resort_every steps as one CUDA graph (launch-bound small systems: C1 0.066 -> 0.044 ms
+                                      per step) whenever it can -- no TILD_FLAG_TIMING, an even resort_every, and a stream
+                                      that can be captured (not the legacy default stream); otherwise it launches eagerly */
 #define TILD_FLAG_GEN1_TILES 128u   /* first-generation tile kernels (32 bank classes with overflow rounds, per-particle work
                                       in class order) even where the rotation-class kernels apply (P = 4); for A/B runs */
 
@@ -146,7 +151,9 @@ int tild_step(tild_ctx*, int32_t nsteps);
 int tild_get_state(tild_ctx*, float* x, float* v, float* f, uint64_t* step /*HOST*/);
 
 /* HOST out, synchronises.  Energies of the current state (diagnostic): e[0] kinetic m/2 sum |v|^2,
- * e[1] bonds sum k (|d| - r0)^2 (Eq. 2), e[2] non-bonded on the mesh
+ * e[1] bonded: sum over bonds k (|d| - r0)^2 (Eq. 2; every bond counted once, from its lower slot, so the partner
+ * table must list a bond on both of its particles -- the force path does not need that) plus the angle energies
+ * lambda (1 + cos theta) and k_theta (theta - theta0)^2 (Eq. 16-17) of every centre bead; e[2] non-bonded on the mesh
  * (1/2V) sum_m u^(k_m) sum_IJ c_IJ Re[n^_I(m) conj(n^_J(m))] (Eq. 3-4).  One force evaluation, no state change. */
 int tild_energy(tild_ctx*, double e[3] /*HOST out*/);
 

@@ -5,7 +5,10 @@
 #include <stdlib.h>
 #include <string.h>
 
+#include <map>
+#include <mutex>
 #include <new>
+#include <utility>
 #include <vector>
 
 #include "tild_internal.cuh"
@@ -21,7 +24,39 @@ int tild_fail(tild_ctx* c, int code, const char* fmt, ...)
     return code;
 }
 
+// cudaFuncAttributeMaxDynamicSharedMemorySize is per FUNCTION and process-wide: contexts with different needs for the same
+// kernel instantiation must never lower it (a later tild_init would otherwise break an earlier context's launches).
+// Raises the limit of `func` to at least `bytes`; keeps the maximum asked for so far per (device, function).
+cudaError_t tild_raise_smem_limit(const void* func, size_t bytes)
+{
+    static std::mutex mu;
+    static std::map<std::pair<int, const void*>, size_t> limit;
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    std::lock_guard<std::mutex> lock(mu);
+    size_t& cur = limit[std::make_pair(dev, func)];
+    if (bytes <= cur) return cudaSuccess;
+    e = cudaFuncSetAttribute(func, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+    if (e == cudaSuccess) cur = bytes;
+    return e;
+}
+
 namespace {
+
+// Every entry point runs on the device that was current at tild_init, whatever is current on the calling thread.
+struct DevGuard {
+    int prev = 0;
+    bool switched = false;
+    explicit DevGuard(const tild_ctx* c)
+    {
+        if (c && cudaGetDevice(&prev) == cudaSuccess && prev != c->device) switched = cudaSetDevice(c->device) == cudaSuccess;
+    }
+    ~DevGuard()
+    {
+        if (switched) cudaSetDevice(prev);
+    }
+};
 
 constexpr size_t ALIGN = 256;
 inline size_t up(size_t b) { return (b + ALIGN - 1) / ALIGN * ALIGN; }
@@ -166,20 +201,20 @@ int kspace_pipeline(tild_ctx* c, const float* grid, float* ffield, cudaEvent_t* 
     cufftComplex* fh = reinterpret_cast<cufftComplex*>(c->fhat);
     if (c->xfft_R) {
         TILD_FFT(c, cufftExecR2C(c->plan_r2c_yz, const_cast<float*>(grid), nh));
-        if (ev) cudaEventRecord(ev[3], c->stream);
+        if (ev) TILD_CUDA(c, cudaEventRecord(ev[3], c->stream));
         rc = launch_kspace_xfft(c, c->nhat, c->fhat);
         if (rc) return rc;
-        if (ev) cudaEventRecord(ev[4], c->stream);
+        if (ev) TILD_CUDA(c, cudaEventRecord(ev[4], c->stream));
         TILD_FFT(c, cufftExecC2R(c->plan_c2r_yz, fh, ffield));
     } else {
         TILD_FFT(c, cufftExecR2C(c->plan_r2c, const_cast<float*>(grid), nh));
-        if (ev) cudaEventRecord(ev[3], c->stream);
+        if (ev) TILD_CUDA(c, cudaEventRecord(ev[3], c->stream));
         rc = launch_kspace(c, c->nhat, c->fhat);
         if (rc) return rc;
-        if (ev) cudaEventRecord(ev[4], c->stream);
+        if (ev) TILD_CUDA(c, cudaEventRecord(ev[4], c->stream));
         TILD_FFT(c, cufftExecC2R(c->plan_c2r, fh, ffield));
     }
-    if (ev) cudaEventRecord(ev[5], c->stream);
+    if (ev) TILD_CUDA(c, cudaEventRecord(ev[5], c->stream));
     return TILD_OK;
 }
 
@@ -188,7 +223,7 @@ int mesh_pipeline(tild_ctx* c, const SegLayout& lay, const float4* X4, cudaEvent
 {
     int rc = launch_spread(c, lay, X4, c->grid);
     if (rc) return rc;
-    if (ev) cudaEventRecord(ev[2], c->stream);
+    if (ev) TILD_CUDA(c, cudaEventRecord(ev[2], c->stream));
     return kspace_pipeline(c, c->grid, c->ffield, ev);
 }
 
@@ -239,6 +274,10 @@ int tild_init(tild_ctx** out, const tild_params* params, void* workspace, size_t
     memset(c, 0, sizeof(*c));
     c->prm = *params;
     c->stream = static_cast<cudaStream_t>(cuda_stream);
+    if (cudaGetDevice(&c->device) != cudaSuccess) {
+        delete c;
+        return TILD_ECUDA;
+    }
     size_t need = 0;
     carve(c, workspace, &need);
     if (need > workspace_bytes) {
@@ -251,7 +290,7 @@ int tild_init(tild_ctx** out, const tild_params* params, void* workspace, size_t
     c->Mk = (size_t)p.grid[0] * p.grid[1] * (p.grid[2] / 2 + 1);
     const double V = p.box[0] * p.box[1] * p.box[2];
     const double sigma2 = p.sigma2 > 0.0 ? p.sigma2 : 2.0 * p.a * p.a;
-    const double rho0 = p.rho0 > 0.0 ? p.rho0 : (double)p.n / V;          // L121
+    const double rho0 = p.rho0 > 0.0 ? p.rho0 : (p.n > 0 ? (double)p.n / V : 1.0);   // L121; an empty system has no density scale
     c->resort_every = p.resort_every > 0 ? p.resort_every : 10;
 
     MeshParams& m = c->mesh;
@@ -338,6 +377,7 @@ int tild_init(tild_ctx** out, const tild_params* params, void* workspace, size_t
     const double gh = p.gamma * p.dt / (2.0 * p.mass);
     const double bg = 1.0 / (1.0 + gh), ag = (1.0 - gh) / (1.0 + gh);
     s.half_dt_over_m = (float)(p.dt / (2.0 * p.mass));
+    s.kick_in = s.half_dt_over_m;
     s.a_g = (float)ag;
     s.b_dt = (float)(bg * p.dt);
     s.b_dt2_over_2m = (float)(bg * p.dt * p.dt / (2.0 * p.mass));
@@ -356,7 +396,8 @@ int tild_init(tild_ctx** out, const tild_params* params, void* workspace, size_t
     s.key0 = (uint32_t)(p.seed & 0xffffffffu);
     s.key1 = (uint32_t)(p.seed >> 32);
 
-    cudaError_t e = cudaMemcpyAsync(c->tables, tab.data(), tab.size() * sizeof(float), cudaMemcpyHostToDevice, c->stream);
+    cudaError_t e = cudaMemsetAsync(c->drift_count, 0, 4 * sizeof(uint32_t), c->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(c->tables, tab.data(), tab.size() * sizeof(float), cudaMemcpyHostToDevice, c->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);  // tab is a stack-owned host buffer
     if (e != cudaSuccess) {
         delete c;
@@ -398,8 +439,19 @@ int tild_init(tild_ctx** out, const tild_params* params, void* workspace, size_t
     for (int i = 0; i < 4; ++i)
         if (made[i]) cufftSetStream(*plans[i], c->stream);
     if (p.flags & TILD_FLAG_TIMING) {
-        for (int i = 0; i < TILD_MAX_TIMED_STEPS; ++i)
-            for (int k = 0; k < TILD_N_STAGE_EVENTS; ++k) cudaEventCreate(&c->ev[i][k]);
+        cudaError_t ee = cudaSuccess;
+        int made_ev = 0;
+        for (int i = 0; i < TILD_MAX_TIMED_STEPS && ee == cudaSuccess; ++i)
+            for (int k = 0; k < TILD_N_STAGE_EVENTS && ee == cudaSuccess; ++k) {
+                ee = cudaEventCreate(&c->ev[i][k]);
+                if (ee == cudaSuccess) ++made_ev;
+            }
+        if (ee != cudaSuccess) {
+            for (int j = 0; j < made_ev; ++j) cudaEventDestroy(c->ev[j / TILD_N_STAGE_EVENTS][j % TILD_N_STAGE_EVENTS]);
+            drop_plans();
+            delete c;
+            return TILD_ECUDA;
+        }
         c->ev_ok = true;
     }
     *out = c;
@@ -409,6 +461,7 @@ int tild_init(tild_ctx** out, const tild_params* params, void* workspace, size_t
 void tild_destroy(tild_ctx* c)
 {
     if (!c) return;
+    DevGuard dg(c);
     if (c->plans_ok) {
         cufftDestroy(c->plan_r2c);
         if (c->xfft_R) {
@@ -443,6 +496,7 @@ int tild_segment_layout(const tild_ctx* cc, uint32_t* seg_base, uint32_t* slot_i
 {
     tild_ctx* c = const_cast<tild_ctx*>(cc);
     if (!c) return TILD_EINVAL;
+    DevGuard dg(c);
     if (!c->has_state) return tild_fail(c, TILD_ESTATE, "tild_segment_layout before tild_set_state");
     if (seg_base)
         TILD_CUDA(c, cudaMemcpyAsync(seg_base, c->lay.seg_base, ((size_t)c->tile.nseg + 1) * sizeof(uint32_t), cudaMemcpyDeviceToDevice, c->stream));
@@ -452,6 +506,7 @@ int tild_segment_layout(const tild_ctx* cc, uint32_t* seg_base, uint32_t* slot_i
 
 int tild_spread(tild_ctx* c, const float* x, const int32_t* type, float* grid)
 {
+    DevGuard dg(c);
     if (!c || !grid || (c->mesh.n > 0 && (!x || !type))) return tild_fail(c, TILD_EINVAL, "tild_spread: null argument");
     int rc = stage_layout(c, x, type);  // slab-ordered copy of the caller's particles
     if (rc) return rc;
@@ -460,12 +515,14 @@ int tild_spread(tild_ctx* c, const float* x, const int32_t* type, float* grid)
 
 int tild_kspace_force(tild_ctx* c, const float* grid, float* ffield)
 {
+    DevGuard dg(c);
     if (!c || !grid || !ffield) return tild_fail(c, TILD_EINVAL, "tild_kspace_force: null argument");
     return kspace_pipeline(c, grid, ffield, nullptr);
 }
 
 int tild_interp(tild_ctx* c, const float* ffield, const float* x, const int32_t* type, float* f)
 {
+    DevGuard dg(c);
     if (!c || !ffield || (c->mesh.n > 0 && (!x || !type || !f))) return tild_fail(c, TILD_EINVAL, "tild_interp: null argument");
     const int n = c->mesh.n;
     if (n == 0) return TILD_OK;
@@ -480,6 +537,7 @@ int tild_interp(tild_ctx* c, const float* ffield, const float* x, const int32_t*
 
 int tild_bond_force(tild_ctx* c, const float* x, const int32_t* bond_partner, float* f)
 {
+    DevGuard dg(c);
     if (!c || (c->mesh.n > 0 && (!x || !f))) return tild_fail(c, TILD_EINVAL, "tild_bond_force: null argument");
     if (c->stp.max_bonds > 0 && !bond_partner && c->mesh.n > 0) return tild_fail(c, TILD_EINVAL, "tild_bond_force: null partners");
     return launch_bond_force_caller(c, x, bond_partner, f);
@@ -487,6 +545,7 @@ int tild_bond_force(tild_ctx* c, const float* x, const int32_t* bond_partner, fl
 
 int tild_index_map(tild_ctx* c, const float* x, int32_t* base, uint32_t* cell_key, uint32_t* perm, uint32_t* cell_start)
 {
+    DevGuard dg(c);
     if (!c || (c->mesh.n > 0 && !x)) return tild_fail(c, TILD_EINVAL, "tild_index_map: null argument");
     uint32_t* key = cell_key ? cell_key : c->key;
     int rc = launch_cell_keys(c, x, key, base);
@@ -497,27 +556,40 @@ int tild_index_map(tild_ctx* c, const float* x, int32_t* base, uint32_t* cell_ke
 
 int tild_philox_test(tild_ctx* c, const uint32_t* ctr, const uint32_t* key, uint32_t* out, float* gauss, int32_t m)
 {
+    DevGuard dg(c);
     if (!c || (m > 0 && (!ctr || !key || !out))) return tild_fail(c, TILD_EINVAL, "tild_philox_test: null argument");
     return launch_philox_test(c, ctr, key, out, gauss, m);
 }
 
 int tild_set_state(tild_ctx* c, const float* x, const float* v, const int32_t* type, const int32_t* bond_partner, uint64_t step0)
 {
+    DevGuard dg(c);
     if (!c) return TILD_EINVAL;
     const size_t n = (size_t)c->mesh.n;
     if (n > 0 && (!x || !v || !type)) return tild_fail(c, TILD_EINVAL, "tild_set_state: null argument");
     if (n > 0 && c->stp.max_bonds > 0 && !bond_partner) return tild_fail(c, TILD_EINVAL, "tild_set_state: null bond_partner");
     c->cur = 0;
+    c->has_state = false;
+    TILD_CUDA(c, cudaMemsetAsync(c->drift_count, 0, 4 * sizeof(uint32_t), c->stream));
     int rc = launch_pack(c, x, v, type, c->stp.max_bonds > 0 ? bond_partner : nullptr, c->X4[0], c->W4[0], c->B[0]);
     if (rc) return rc;
+    if (n > 0) {   // argument check (include/tild.h): one 4-byte read-back and a synchronisation per tild_set_state
+        uint32_t bad = 0;
+        TILD_CUDA(c, cudaMemcpyAsync(&bad, c->drift_count + 2, sizeof(uint32_t), cudaMemcpyDeviceToHost, c->stream));
+        TILD_CUDA(c, cudaStreamSynchronize(c->stream));
+        if (bad) return tild_fail(c, TILD_EINVAL, "tild_set_state: a type is outside [0, %d) or a bond partner outside [-1, %d)", c->mesh.S, c->mesh.n);
+    }
     if ((rc = launch_reorder(c))) return rc;
-    if ((rc = force_current(c))) return rc;
-    if ((rc = launch_make_w(c, c->F4, c->W4[c->cur], -1.0f))) return rc;  // w = v - (dt/2m) F
+    // The state array holds v itself until the first step: that step takes v^0 as it is (kick_in = 0) and leaves the
+    // split-kick state w^1 = v^1 - (dt/2m) F^1 behind, so loading a state costs a sort and no force evaluation.
+    c->stp.kick_in = 0.0f;
     c->step = step0;
     c->h_step_upload = step0;
     TILD_CUDA(c, cudaMemcpyAsync(c->d_step, &c->h_step_upload, sizeof(uint64_t), cudaMemcpyHostToDevice, c->stream));
     c->has_state = true;
     c->timed_steps = 0;
+    c->ms_steps = 0;
+    for (int k = 0; k < 8; ++k) c->ms_sum[k] = 0.0;
     return TILD_OK;
 }
 
@@ -525,25 +597,48 @@ int tild_set_state(tild_ctx* c, const float* x, const float* v, const int32_t* t
 
 namespace {
 
+// Synchronises and adds the recorded stage events of the last `timed_steps` steps to the running sums, so that the
+// event ring (TILD_MAX_TIMED_STEPS steps) never limits how many steps are timed.
+int fold_timings(tild_ctx* c)
+{
+    if (!c->ev_ok || c->timed_steps == 0) return TILD_OK;
+    TILD_CUDA(c, cudaStreamSynchronize(c->stream));
+    for (int i = 0; i < c->timed_steps; ++i) {
+        for (int k = 0; k < 6; ++k) {
+            float t = 0.0f;
+            TILD_CUDA(c, cudaEventElapsedTime(&t, c->ev[i][k], c->ev[i][k + 1]));
+            c->ms_sum[k] += t;
+        }
+        float tot = 0.0f;
+        TILD_CUDA(c, cudaEventElapsedTime(&tot, c->ev[i][0], c->ev[i][6]));
+        c->ms_sum[7] += tot;
+    }
+    c->ms_steps += c->timed_steps;
+    c->timed_steps = 0;
+    return TILD_OK;
+}
+
 // one TILD step on the internal state (re-sort when due, mesh pipeline, fused interpolation pass, step counter)
 int enqueue_one_step(tild_ctx* c, cudaEvent_t* ev)
 {
-    if (ev) cudaEventRecord(ev[0], c->stream);
+    if (ev) TILD_CUDA(c, cudaEventRecord(ev[0], c->stream));
     if (c->steps_since_sort >= c->resort_every) {
         int rc = launch_reorder(c);
         if (rc) return rc;
     }
-    if (ev) cudaEventRecord(ev[1], c->stream);
+    if (ev) TILD_CUDA(c, cudaEventRecord(ev[1], c->stream));
     const int a = c->cur;
     int rc = mesh_pipeline(c, c->lay, c->X4[a], ev);
     if (rc) return rc;
     rc = launch_interp(c, INTERP_FUSED_STEP, c->lay, c->ffield, c->X4[a], c->W4[a], c->B[a], c->X4[1 - a], c->W4[1 - a], nullptr);
     if (rc) return rc;
-    if ((rc = launch_advance_step(c))) return rc;
+    // from here on the state is w = v - (dt/2m) F (Euler-Maruyama never touches the velocities: the state stays v)
+    c->stp.kick_in = c->stp.integrator == TILD_INTEGRATOR_EM ? 0.0f : c->stp.half_dt_over_m;
+    if (!c->step_advanced && (rc = launch_advance_step(c))) return rc;   // per-particle path: no drift kernel to do it
     // swap only the x/w pointers so that `cur` keeps naming the buffer that holds the bond table
     float4* t = c->X4[a]; c->X4[a] = c->X4[1 - a]; c->X4[1 - a] = t;
     t = c->W4[a]; c->W4[a] = c->W4[1 - a]; c->W4[1 - a] = t;
-    if (ev) cudaEventRecord(ev[6], c->stream);
+    if (ev) TILD_CUDA(c, cudaEventRecord(ev[6], c->stream));
     c->step++;
     c->steps_since_sort++;
     return TILD_OK;
@@ -600,11 +695,12 @@ extern "C" {
 
 int tild_step(tild_ctx* c, int32_t nsteps)
 {
+    DevGuard dg(c);
     if (!c) return TILD_EINVAL;
     if (!c->has_state) return tild_fail(c, TILD_ESTATE, "tild_step before tild_set_state");
     if (nsteps < 0) return tild_fail(c, TILD_EINVAL, "tild_step: nsteps < 0");
     // stream capture is not available on the legacy default stream (NULL / cudaStreamLegacy)
-    const bool graphs = (c->prm.flags & TILD_FLAG_GRAPH) && !c->ev_ok && c->resort_every % 2 == 0 && c->stream != nullptr &&
+    const bool graphs = !(c->prm.flags & TILD_FLAG_EAGER) && !c->ev_ok && c->resort_every % 2 == 0 && c->stream != nullptr &&
                         c->stream != cudaStreamLegacy;
     int32_t s = 0;
     while (s < nsteps) {
@@ -614,7 +710,11 @@ int tild_step(tild_ctx* c, int32_t nsteps)
             s += 2 * c->resort_every;
             continue;
         }
-        cudaEvent_t* ev = (c->ev_ok && c->timed_steps < TILD_MAX_TIMED_STEPS) ? c->ev[c->timed_steps] : nullptr;
+        if (c->ev_ok && c->timed_steps == TILD_MAX_TIMED_STEPS) {   // ring full: fold it into the sums (synchronises)
+            int rcf = fold_timings(c);
+            if (rcf) return rcf;
+        }
+        cudaEvent_t* ev = c->ev_ok ? c->ev[c->timed_steps] : nullptr;
         int rc = enqueue_one_step(c, ev);
         if (rc) return rc;
         if (ev) c->timed_steps++;
@@ -625,6 +725,7 @@ int tild_step(tild_ctx* c, int32_t nsteps)
 
 int tild_get_state(tild_ctx* c, float* x, float* v, float* f, uint64_t* step)
 {
+    DevGuard dg(c);
     if (!c) return TILD_EINVAL;
     if (!c->has_state) return tild_fail(c, TILD_ESTATE, "tild_get_state before tild_set_state");
     const size_t n = (size_t)c->mesh.n;
@@ -638,8 +739,10 @@ int tild_get_state(tild_ctx* c, float* x, float* v, float* f, uint64_t* step)
         if ((rc = launch_unpermute(c, c->X4[a], scratch))) return rc;
         TILD_CUDA(c, cudaMemcpyAsync(x, scratch, bytes, cudaMemcpyDefault, c->stream));
     }
-    if (v || f) {
+    if (f || (v && c->stp.kick_in != 0.0f)) {   // v = w + (dt/2m) F needs F(x); right after tild_set_state the state is v itself
         if ((rc = force_current(c))) return rc;
+    }
+    if (v || f) {
         if (f) {
             if ((rc = launch_unpermute(c, c->F4, scratch))) return rc;
             TILD_CUDA(c, cudaMemcpyAsync(f, scratch, bytes, cudaMemcpyDefault, c->stream));
@@ -654,6 +757,7 @@ int tild_get_state(tild_ctx* c, float* x, float* v, float* f, uint64_t* step)
 
 int tild_energy(tild_ctx* c, double e[3])
 {
+    DevGuard dg(c);
     if (!c || !e) return TILD_EINVAL;
     if (!c->has_state) return tild_fail(c, TILD_ESTATE, "tild_energy before tild_set_state");
     int rc = force_current(c);              // F4 and nhat at the current positions; no state change
@@ -668,6 +772,7 @@ int tild_energy(tild_ctx* c, double e[3])
 
 int tild_structure_factor(tild_ctx* c, uint32_t species_mask, float* sk, int32_t accumulate)
 {
+    DevGuard dg(c);
     if (!c || !sk) return tild_fail(c, TILD_EINVAL, "tild_structure_factor: null argument");
     if (!c->has_state) return tild_fail(c, TILD_ESTATE, "tild_structure_factor before tild_set_state");
     if ((species_mask & ((1u << c->mesh.S) - 1u)) == 0) return tild_fail(c, TILD_EINVAL, "tild_structure_factor: empty species mask");
@@ -679,25 +784,20 @@ int tild_structure_factor(tild_ctx* c, uint32_t species_mask, float* sk, int32_t
 
 int tild_get_timings(tild_ctx* c, float ms[8], int32_t* steps_timed)
 {
+    DevGuard dg(c);
     if (!c || !ms) return TILD_EINVAL;
     for (int k = 0; k < 8; ++k) ms[k] = 0.0f;
     if (steps_timed) *steps_timed = 0;
     TILD_CUDA(c, cudaStreamSynchronize(c->stream));
-    if (!c->ev_ok || c->timed_steps == 0) return TILD_OK;
-    const int T = c->timed_steps;
-    for (int i = 0; i < T; ++i) {
-        for (int k = 0; k < 6; ++k) {
-            float t = 0.0f;
-            TILD_CUDA(c, cudaEventElapsedTime(&t, c->ev[i][k], c->ev[i][k + 1]));
-            ms[k] += t;
-        }
-        float tot = 0.0f;
-        TILD_CUDA(c, cudaEventElapsedTime(&tot, c->ev[i][0], c->ev[i][6]));
-        ms[7] += tot;
-    }
-    for (int k = 0; k < 8; ++k) ms[k] /= (float)T;
+    int rc = fold_timings(c);
+    if (rc) return rc;
+    if (!c->ev_ok || c->ms_steps == 0) return TILD_OK;
+    const double T = (double)c->ms_steps;
+    for (int k = 0; k < 8; ++k) ms[k] = (float)(c->ms_sum[k] / T);
     ms[6] = ms[7] - (ms[0] + ms[1] + ms[2] + ms[3] + ms[4] + ms[5]);
-    if (steps_timed) *steps_timed = T;
+    if (steps_timed) *steps_timed = (int32_t)c->ms_steps;
+    for (int k = 0; k < 8; ++k) c->ms_sum[k] = 0.0;
+    c->ms_steps = 0;
     c->timed_steps = 0;
     return TILD_OK;
 }
@@ -705,6 +805,7 @@ int tild_get_timings(tild_ctx* c, float ms[8], int32_t* steps_timed)
 int tild_run_host(tild_ctx* c, float* x_host, float* v_host, const int32_t* type_host, const int32_t* bond_partner_host,
                   uint64_t step0, int32_t nsteps)
 {
+    DevGuard dg(c);
     if (!c) return TILD_EINVAL;
     const size_t n = (size_t)c->mesh.n;
     const size_t mb = (size_t)c->stp.max_bonds;

@@ -61,8 +61,8 @@ __global__ void __launch_bounds__(256) particle_energy_kernel(MeshParams m, Step
     double ke = 0.0, eb = 0.0;
     for (size_t slot = (size_t)blockIdx.x * blockDim.x + threadIdx.x; slot < (size_t)m.n; slot += (size_t)gridDim.x * blockDim.x) {
         const float4 p = X4[slot], w = W4[slot], f = F4[slot];
-        const double vx = (double)w.x + (double)s.half_dt_over_m * f.x, vy = (double)w.y + (double)s.half_dt_over_m * f.y,
-                     vz = (double)w.z + (double)s.half_dt_over_m * f.z;
+        const double vx = (double)w.x + (double)s.kick_in * f.x, vy = (double)w.y + (double)s.kick_in * f.y,
+                     vz = (double)w.z + (double)s.kick_in * f.z;
         ke += 0.5 * mass * (vx * vx + vy * vy + vz * vz);
         for (int k = 0; k < s.max_bonds; ++k) {
             const int32_t j = B[slot * s.max_bonds + k];

@@ -62,6 +62,7 @@ struct KspaceParams {
 
 struct StepParams {
     float half_dt_over_m;  // dt/2m
+    float kick_in;         // v^n = w^n + kick_in F^n: dt/2m, or 0 while the state still holds v itself (first step after tild_set_state)
     float a_g;             // (1 - gamma dt/2m)/(1 + gamma dt/2m)
     float b_dt;            // b dt
     float b_dt2_over_2m;   // b dt^2/2m
@@ -87,6 +88,7 @@ struct SegLayout {
 struct tild_ctx {
     tild_params prm;
     cudaStream_t stream;
+    int device;           // the CUDA device that was current at tild_init: every entry point runs on it
     MeshParams mesh;
     KspaceParams ksp;
     StepParams stp;
@@ -106,7 +108,7 @@ struct tild_ctx {
     float2* nhat;         // [S][Mk]
     float2* fhat;         // [3S][Mk]
     float* ffield;        // [3S][M]
-    uint32_t* key;        // [n] sort scratch; between sorts: the drift list of launch_spread
+    uint32_t* key;        // [n] sort scratch
     uint32_t* rank;       // [n] sort scratch; between sorts: the drift list of launch_interp
     uint32_t* inv;        // [n] old slot -> new slot
     uint32_t* drift_count;  // [4]
@@ -126,6 +128,7 @@ struct tild_ctx {
     bool plans_ok;
 
     bool has_state;
+    bool step_advanced;   // the last launch_interp advanced the device step counter itself (tile path)
     uint64_t step;
     int steps_since_sort;
     int resort_every;
@@ -141,12 +144,15 @@ struct tild_ctx {
     // timing
     cudaEvent_t ev[TILD_MAX_TIMED_STEPS][TILD_N_STAGE_EVENTS];
     bool ev_ok;
-    int timed_steps;
+    int timed_steps;          // steps whose events are recorded and not yet folded
+    double ms_sum[8];         // folded stage times (sums over ms_steps steps): any number of steps can be timed
+    long long ms_steps;
 
     char err[512];
 };
 
 int tild_fail(tild_ctx* c, int code, const char* fmt, ...);
+cudaError_t tild_raise_smem_limit(const void* func, size_t bytes);   // tild_api.cu
 #define TILD_CUDA(c, call)                                                                          \
     do {                                                                                            \
         cudaError_t e__ = (call);                                                                   \
@@ -206,7 +212,8 @@ struct InterpArgs {
     float4* W4o;
     float4* F4;
     uint32_t* drift_list;
-    uint32_t* drift_count;
+    uint32_t* drift_count;   // [0] entries of drift_list, [1] blocks of the drift kernel that are done
+    uint64_t* step_adv;      // device step counter, advanced by the last block of the drift kernel in the fused step
 };
 // tild_interp_rot.cu: the P = 4 rotation-class tile kernel
 bool interp_rot_applies(const tild_ctx* c);

@@ -253,11 +253,13 @@ __global__ void __launch_bounds__(INTERP_THREADS, 2) interp_tile_kernel(MeshPara
     }
 }
 
-// particles that left their tile's image since the last re-sort: per-particle global gather, any order
+// particles that left their tile's image since the last re-sort: per-particle global gather, any order.
+// Last kernel of the fused pass: the block that finishes last resets the drift counter for the next pass and, in the
+// fused step (step_adv != nullptr), advances the device-side step counter -- no extra launches for either.
 template <int P, int MODE>
-__global__ void __launch_bounds__(256) interp_drift_kernel(MeshParams m, StepParams s, const uint64_t* __restrict__ step_ptr,
+__global__ void __launch_bounds__(256) interp_drift_kernel(MeshParams m, StepParams s, const uint64_t* step_ptr,
                                                            const uint32_t* __restrict__ drift_list,
-                                                           const uint32_t* __restrict__ drift_count,
+                                                           uint32_t* __restrict__ drift_count, uint64_t* __restrict__ step_adv,
                                                            const float* __restrict__ ffield, const float4* __restrict__ X4,
                                                            const float4* __restrict__ W4, const int32_t* __restrict__ B,
                                                            float4* __restrict__ X4o, float4* __restrict__ W4o,
@@ -275,6 +277,15 @@ __global__ void __launch_bounds__(256) interp_drift_kernel(MeshParams m, StepPar
         const float3 F = vec ? interp_global<P, true>(m, ffield, b, w, __float_as_int(p.w))
                              : interp_global<P, false>(m, ffield, b, w, __float_as_int(p.w));
         finish_particle<MODE>(m, s, step_next, slot, p, F, X4, W4, B, X4o, W4o, F4);
+    }
+    __syncthreads();                            // every thread of this block has read the step and the drift count
+    if (threadIdx.x == 0) {
+        __threadfence();
+        if (atomicAdd(drift_count + 1, 1u) == gridDim.x - 1) {   // all blocks are past their reads
+            drift_count[0] = 0u;
+            drift_count[1] = 0u;
+            if (step_adv) *step_adv = step_next;
+        }
     }
 }
 
@@ -354,7 +365,7 @@ __global__ void __launch_bounds__(256) velocity_out_kernel(size_t nslots, float 
     if (s >= nslots) return;
     const float4 w = W4[s];
     const uint32_t id = __float_as_uint(w.w);
-    const float4 f = F4[s];
+    const float4 f = alpha != 0.0f ? F4[s] : make_float4(0.f, 0.f, 0.f, 0.f);
     v[3 * (size_t)id + 0] = w.x + alpha * f.x;
     v[3 * (size_t)id + 1] = w.y + alpha * f.y;
     v[3 * (size_t)id + 2] = w.z + alpha * f.z;
@@ -391,14 +402,14 @@ void tile_launch(const InterpArgs& a, cudaStream_t st, size_t smem, bool configu
 {
     auto kernel = interp_tile_kernel<P, EY, EZ, MODE>;
     if (configure_only) {
-        const cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        const cudaError_t e = tild_raise_smem_limit(reinterpret_cast<const void*>(kernel), smem);
         if (e != cudaSuccess) *err = e;
         return;
     }
     kernel<<<a.tp.ntiles, INTERP_THREADS, smem, st>>>(a.m, a.tp, a.s, a.step_ptr, a.seg_base, a.ffield, a.X4, a.W4, a.B, a.X4o,
                                                       a.W4o, a.F4, a.drift_list, a.drift_count);
-    interp_drift_kernel<P, MODE><<<592, 256, 0, st>>>(a.m, a.s, a.step_ptr, a.drift_list, a.drift_count, a.ffield, a.X4, a.W4,
-                                                      a.B, a.X4o, a.W4o, a.F4);
+    interp_drift_kernel<P, MODE><<<592, 256, 0, st>>>(a.m, a.s, a.step_ptr, a.drift_list, a.drift_count, MODE == 2 ? a.step_adv : nullptr,
+                                                      a.ffield, a.X4, a.W4, a.B, a.X4o, a.W4o, a.F4);
 }
 template <int P, int EY, int EZ>
 void tile_launch_m(const InterpArgs& a, int mode, cudaStream_t st, size_t smem, bool cfg, cudaError_t* err)
@@ -432,7 +443,7 @@ bool tile_launch_any(const InterpArgs& a, int mode, cudaStream_t st, size_t smem
 // the drifted particles of the rotation-class kernel (P = 4)
 void launch_drift_only(const InterpArgs& a, int mode, cudaStream_t st)
 {
-#define TILD_DR(M_) interp_drift_kernel<4, M_><<<592, 256, 0, st>>>(a.m, a.s, a.step_ptr, a.drift_list, a.drift_count, a.ffield, a.X4, a.W4, a.B, a.X4o, a.W4o, a.F4)
+#define TILD_DR(M_) interp_drift_kernel<4, M_><<<592, 256, 0, st>>>(a.m, a.s, a.step_ptr, a.drift_list, a.drift_count, M_ == 2 ? a.step_adv : nullptr, a.ffield, a.X4, a.W4, a.B, a.X4o, a.W4o, a.F4)
     if (mode == 0) TILD_DR(0); else if (mode == 1) TILD_DR(1); else TILD_DR(2);
 #undef TILD_DR
 }
@@ -473,10 +484,12 @@ int launch_interp(tild_ctx* c, int mode, const SegLayout& lay, const float* ffie
 {
     const size_t n = (size_t)c->mesh.n;
     if (n == 0) return TILD_OK;
-    InterpArgs a{c->mesh, c->tile, c->stp, c->d_step, lay.seg_base, ffield, X4, W4, B, X4o, W4o, c->F4, c->rank, c->drift_count};
+    InterpArgs a{c->mesh, c->tile, c->stp, c->d_step, lay.seg_base, ffield, X4, W4, B, X4o, W4o, c->F4, c->rank, c->drift_count, c->d_step};
+    c->step_advanced = false;
     if (c->tile.enabled && c->mesh.P >= 2 && !(c->prm.flags & TILD_FLAG_NAIVE_INTERP)) {   // P = 1: one node per particle
         cudaError_t e = cudaSuccess;
-        TILD_CUDA(c, cudaMemsetAsync(c->drift_count, 0, sizeof(uint32_t), c->stream));
+        // drift_count[0..1] are zero here: cleared at tild_init and again by the last block of every drift kernel
+        c->step_advanced = mode == INTERP_FUSED_STEP;
         if (interp_rot_applies(c) && !(c->prm.flags & TILD_FLAG_GEN1_TILES)) {
             e = interp_rot_run(a, mode, c->stream, false);
             TILD_LAUNCH_CHECK(c, "interp_rot_kernel");
@@ -531,7 +544,7 @@ int launch_velocity_out(tild_ctx* c, const float4* F4, const float4* W4, float* 
 {
     const size_t nslots = (size_t)c->mesh.n;
     if (nslots == 0) return TILD_OK;
-    velocity_out_kernel<<<(unsigned)((nslots + 255) / 256), 256, 0, c->stream>>>(nslots, c->stp.half_dt_over_m, F4, W4, v);
+    velocity_out_kernel<<<(unsigned)((nslots + 255) / 256), 256, 0, c->stream>>>(nslots, c->stp.kick_in, F4, W4, v);
     TILD_LAUNCH_CHECK(c, "velocity_out_kernel");
     return TILD_OK;
 }

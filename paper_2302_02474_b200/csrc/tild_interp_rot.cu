@@ -361,7 +361,7 @@ template <int EY, int EZ, int MODE>
 cudaError_t rot_launch(const InterpArgs& a, cudaStream_t st, size_t smem, bool configure_only)
 {
     auto kernel = interp_rot_kernel<EY, EZ, MODE>;
-    if (configure_only) return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (configure_only) return tild_raise_smem_limit(reinterpret_cast<const void*>(kernel), smem);
     kernel<<<a.tp.ntiles, RT, smem, st>>>(a.m, a.tp, a.s, a.step_ptr, a.seg_base, a.ffield, a.X4, a.W4, a.B, a.X4o, a.W4o, a.F4,
                                           a.drift_list, a.drift_count);
     return cudaSuccess;

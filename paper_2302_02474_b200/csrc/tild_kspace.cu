@@ -300,7 +300,7 @@ int tild_kspace_configure(tild_ctx* c)
     if (!c->xfft_R) return TILD_OK;
     const int N = c->mesh.N[0];
     const int sm = (int)xfft_smem_bytes(N, c->xfft_R);
-#define XA(R1_, R2_, SS) TILD_CUDA(c, cudaFuncSetAttribute(kspace_xfft_kernel<R1_, R2_, SS>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm))
+#define XA(R1_, R2_, SS) TILD_CUDA(c, tild_raise_smem_limit(reinterpret_cast<const void*>(kspace_xfft_kernel<R1_, R2_, SS>), (size_t)sm))
     TILD_XFFT_DISPATCH(N, c->mesh.S, XA);
 #undef XA
     return TILD_OK;

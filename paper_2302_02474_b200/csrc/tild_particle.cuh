@@ -182,7 +182,7 @@ __device__ __forceinline__ void finish_update(const MeshParams& m, const StepPar
     float xo[3], wo[3];
 #pragma unroll
     for (int a = 0; a < 3; ++a) {
-        const float v = wv[a] + s.half_dt_over_m * Fv[a];
+        const float v = wv[a] + s.kick_in * Fv[a];
         const float r = pp[a] + (s.b_dt * v + s.b_dt2_over_2m * Fv[a] + s.b_dt_over_2m * bv[a]);
         xo[a] = wrap_pos(r, m.L[a], m.inv_L[a]);
         wo[a] = s.a_g * (v + s.half_dt_over_m * Fv[a]) + s.b_over_m * bv[a];

@@ -136,14 +136,19 @@ __global__ void __launch_bounds__(256) scatter_perm_kernel(int n, const uint32_t
 
 // ---- slab-transposed layout ---------------------------------------------------------------------------------------
 
-// caller arrays -> slots [0, n): slot i holds particle id i
-__global__ void __launch_bounds__(256) pack_kernel(int n, int max_bonds, const float* __restrict__ x, const float* __restrict__ v,
+// caller arrays -> slots [0, n): slot i holds particle id i.  A type outside [0, S) or a partner outside [-1, n) is
+// replaced by 0 / -1 (so that no later kernel indexes out of bounds) and reported through *bad.
+__global__ void __launch_bounds__(256) pack_kernel(int n, int S, int max_bonds, const float* __restrict__ x, const float* __restrict__ v,
                                                    const int32_t* __restrict__ type, const int32_t* __restrict__ bond,
-                                                   float4* __restrict__ X4, float4* __restrict__ W4, int32_t* __restrict__ B)
+                                                   float4* __restrict__ X4, float4* __restrict__ W4, int32_t* __restrict__ B,
+                                                   uint32_t* __restrict__ bad)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
-    X4[i] = make_float4(x[3 * (size_t)i], x[3 * (size_t)i + 1], x[3 * (size_t)i + 2], __int_as_float(type[i]));
+    int32_t ty = type[i];
+    bool wrong = ty < 0 || ty >= S;
+    if (wrong) ty = 0;
+    X4[i] = make_float4(x[3 * (size_t)i], x[3 * (size_t)i + 1], x[3 * (size_t)i + 2], __int_as_float(ty));
     if (W4) {
         float4 w = make_float4(0.f, 0.f, 0.f, __uint_as_float((uint32_t)i));
         if (v) {
@@ -154,7 +159,15 @@ __global__ void __launch_bounds__(256) pack_kernel(int n, int max_bonds, const f
         W4[i] = w;
     }
     if (B)
-        for (int k = 0; k < max_bonds; ++k) B[(size_t)i * max_bonds + k] = bond[(size_t)i * max_bonds + k];
+        for (int k = 0; k < max_bonds; ++k) {
+            int32_t q = bond[(size_t)i * max_bonds + k];
+            if (q < -1 || q >= n) {
+                wrong = true;
+                q = -1;
+            }
+            B[(size_t)i * max_bonds + k] = q;
+        }
+    if (wrong) atomicOr(bad, 1u);
 }
 
 // key = segment = tile * S + species; rank = arrival order in the segment (one atomic per distinct key per warp)
@@ -291,7 +304,8 @@ int launch_pack(tild_ctx* c, const float* x, const float* v, const int32_t* type
 {
     const int n = c->mesh.n;
     if (n == 0) return TILD_OK;
-    pack_kernel<<<(n + 255) / 256, 256, 0, c->stream>>>(n, c->stp.max_bonds, x, v, type, bond, X4, W4, bond ? B : nullptr);
+    pack_kernel<<<(n + 255) / 256, 256, 0, c->stream>>>(n, c->mesh.S, c->stp.max_bonds, x, v, type, bond, X4, W4, bond ? B : nullptr,
+                                                          c->drift_count + 2);
     TILD_LAUNCH_CHECK(c, "pack_kernel");
     return TILD_OK;
 }

@@ -336,7 +336,7 @@ int tild_spread_configure(tild_ctx* c)
     const size_t bytes = c->tile.smem_spread;
     cudaError_t e = cudaSuccess;
     const bool found = tile_dispatch(c->mesh.P, c->tile.EY, c->tile.EZ, [&](auto kernel) {
-        e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+        e = tild_raise_smem_limit(reinterpret_cast<const void*>(kernel), bytes);
     });
     if (!found) return tild_fail(c, TILD_EINVAL, "no spread tile kernel for P=%d EY=%d EZ=%d", c->mesh.P, c->tile.EY, c->tile.EZ);
     if (e != cudaSuccess) return tild_fail(c, TILD_ECUDA, "cudaFuncSetAttribute(spread_tile_kernel, %zu B): %s", bytes, cudaGetErrorString(e));

@@ -22,6 +22,7 @@ INTEGRATOR_GJF, INTEGRATOR_EM = 0, 1
 FLAG_TIMING, FLAG_NAIVE_SPREAD, FLAG_NAIVE_INTERP, FLAG_GRAPH, FLAG_DECONVOLVE, FLAG_SAMPLED_KERNEL = 1, 2, 4, 8, 16, 32
 FLAG_PLAIN_FFT = 64
 FLAG_GEN1_TILES = 128
+FLAG_EAGER = 256
 TIMING_NAMES = ("sort", "spread", "fft_fwd", "kspace", "fft_inv", "interp", "other", "total")
 
 EXPORTS = (

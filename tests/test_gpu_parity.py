@@ -247,6 +247,8 @@ def test_empty_system():
     ei = torch.empty((0,), dtype=torch.int32, device="cuda")
     g = eng.tild_spread(e, ei)
     assert float(g.abs().max()) == 0.0
+    ff = eng.tild_kspace_force(g)
+    assert bool(torch.isfinite(ff).all()) and float(ff.abs().max()) == 0.0     # rho0 = n / V would be 0 here
     eng.tild_set_state(e, e, ei, torch.empty((0, 2), dtype=torch.int32, device="cuda"), 0)
     eng.tild_step(3)
     _, _, _, step = eng.tild_get_state()
@@ -599,13 +601,13 @@ def test_set_state_can_be_called_again_and_restarts_the_step_counter():
 @pytest.mark.parametrize("grid,box", [((24, 20, 16), (12.0, 10.0, 8.0)), ((32, 20, 16), (16.0, 10.0, 8.0))],
                          ids=["plans3d", "fused_x"])
 def test_cuda_graph_blocks_match_eager_stepping(grid, box):
-    """TILD_FLAG_GRAPH replays 2 * resort_every steps as one CUDA graph; noise still follows (id, step).  Both k-space
-    paths (3-D plans; 2-D plans + fused x-transform kernel) are captured."""
+    """By default tild_step replays 2 * resort_every steps as one CUDA graph (TILD_FLAG_EAGER switches that off); noise
+    still follows (id, step).  Both k-space paths (3-D plans; 2-D plans + fused x-transform kernel) are captured."""
     cfg = small_cfg(order=3, grid=grid, box=box)
     st = inputs.make_state(cfg)
     outs = []
     side = torch.cuda.Stream()                   # the legacy default stream cannot be captured
-    for flags in (0, tild.FLAG_GRAPH):
+    for flags in (tild.FLAG_EAGER, 0):
         with torch.cuda.stream(side):
             eng = tild.Tild(tild.params_from_config(cfg, flags=flags, resort_every=4), stream=side)
             eng.tild_set_state(dev(st.x), dev(st.v), dev(st.type), dev(st.bond_partner), 3)
@@ -614,13 +616,70 @@ def test_cuda_graph_blocks_match_eager_stepping(grid, box):
         side.synchronize()
         assert step == 3 + 33
         outs.append((x.cpu().numpy().astype(np.float64), v.cpu().numpy().astype(np.float64)))
-        if flags:
+        if not flags:
             assert eng.tild_launch_count() > 33 * 4
     assert np.abs(min_image(outs[0][0] - outs[1][0], cfg.box)).max() < 2e-5
     assert np.abs(outs[0][1] - outs[1][1]).max() < 1e-3
     p = oracle_params(cfg)
     ox, _, _ = orc.run(p, st.x.astype(np.float64), st.v.astype(np.float64), st.type, st.bond_partner, 3, 33)
     assert np.abs(min_image(outs[1][0] - ox, cfg.box)).max() <= 1e-4
+
+
+def test_contexts_sharing_a_kernel_instantiation_keep_their_shared_memory_limits():
+    """the dynamic shared-memory limit is per kernel function, process-wide.  An S = 2 engine needs more for
+    the spread kernel than an S = 1 engine with the same P and tile: creating the second must not break the first."""
+    big = small_cfg(order=4, grid=(40, 24, 48), box=(20.0, 12.0, 24.0), n_chains=600)
+    one = small_cfg(order=4, grid=(40, 24, 48), box=(20.0, 12.0, 24.0), chi=((0.0,),), n_species=1,
+                    chains=(inputs.ChainSpec(500, ((0, 6),)),), n=3000)
+    st2, eng2 = make(big)
+    eng2.tild_set_state(dev(st2.x), dev(st2.v), dev(st2.type), dev(st2.bond_partner), 0)
+    st1, eng1 = make(one)
+    eng1.tild_set_state(dev(st1.x), dev(st1.v), dev(st1.type), dev(st1.bond_partner), 0)
+    eng1.tild_step(3)
+    eng2.tild_step(3)                              # used to fail with "invalid argument" at the spread launch
+    g = eng2.tild_spread(dev(st2.x), dev(st2.type)).cpu().numpy()
+    og = orc.spread(oracle_params(big), st2.x, st2.type)
+    assert np.abs(g - og).max() <= REL * max(og.max(), 1.0)
+    x, _, _, step = eng2.tild_get_state(want_v=False)
+    ox, _, _ = orc.run(oracle_params(big), st2.x.astype(np.float64), st2.v.astype(np.float64), st2.type, st2.bond_partner, 0, 3)
+    assert step == 3 and np.abs(min_image(x.cpu().numpy().astype(np.float64) - ox, big.box)).max() <= 1e-5
+
+
+def test_set_state_rejects_types_and_partners_out_of_range():
+    cfg = small_cfg(order=3)
+    st, eng = make(cfg)
+    ty = st.type.copy()
+    ty[5] = cfg.n_species
+    with pytest.raises(tild.TildError):
+        eng.tild_set_state(dev(st.x), dev(st.v), dev(ty), dev(st.bond_partner), 0)
+    bp = st.bond_partner.copy()
+    bp[7, 1] = cfg.n
+    with pytest.raises(tild.TildError):
+        eng.tild_set_state(dev(st.x), dev(st.v), dev(st.type), dev(bp), 0)
+    with pytest.raises(tild.TildError):
+        eng.tild_step(1)                            # no state was loaded
+    eng.tild_set_state(dev(st.x), dev(st.v), dev(st.type), dev(st.bond_partner), 0)
+    eng.tild_step(2)
+
+
+def test_set_state_costs_no_force_evaluation_and_returns_the_velocities_unchanged():
+    """The first step takes v^0 as loaded (no F(x^0) at load time); reading the state back before any step returns the
+    input bit for bit."""
+    cfg = small_cfg(order=4)
+    st, eng = make(cfg)
+    eng.tild_set_state(dev(st.x), dev(st.v), dev(st.type), dev(st.bond_partner), 0)
+    x, v, _, step = eng.tild_get_state()
+    assert step == 0
+    assert np.array_equal(x.cpu().numpy(), st.x) and np.array_equal(v.cpu().numpy(), st.v)
+
+
+def test_more_timed_steps_than_the_event_ring_holds():
+    cfg = small_cfg(order=2)
+    st, eng = make(cfg, flags=tild.FLAG_TIMING)
+    eng.tild_set_state(dev(st.x), dev(st.v), dev(st.type), dev(st.bond_partner), 0)
+    eng.tild_step(300)
+    ms, nst = eng.tild_get_timings()
+    assert nst == 300 and ms["total"] > 0 and abs(sum(ms[k] for k in tild.TIMING_NAMES[:7]) - ms["total"]) < 1e-3 * ms["total"] + 1e-4
 
 
 def test_positions_outside_the_box_are_wrapped_not_trusted():
