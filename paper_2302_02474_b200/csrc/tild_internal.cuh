@@ -215,6 +215,9 @@ struct InterpArgs {
     uint32_t* drift_count;   // [0] entries of drift_list, [1] blocks of the drift kernel that are done
     uint64_t* step_adv;      // device step counter, advanced by the last block of the drift kernel in the fused step
 };
+// tild_spread_rot.cu: the P = 4 rotation-class spread kernel
+bool spread_rot_applies(const tild_ctx* c);
+cudaError_t spread_rot_run(const tild_ctx* c, const uint32_t* seg_base, const float4* X4, float* grid, bool configure_only);
 // tild_interp_rot.cu: the P = 4 rotation-class tile kernel
 bool interp_rot_applies(const tild_ctx* c);
 size_t interp_rot_smem(int ey, int ez);

@@ -338,6 +338,7 @@ int tild_spread_configure(tild_ctx* c)
     const bool found = tile_dispatch(c->mesh.P, c->tile.EY, c->tile.EZ, [&](auto kernel) {
         e = tild_raise_smem_limit(reinterpret_cast<const void*>(kernel), bytes);
     });
+    if (found && e == cudaSuccess && spread_rot_applies(c)) e = spread_rot_run(c, nullptr, nullptr, nullptr, true);
     if (!found) return tild_fail(c, TILD_EINVAL, "no spread tile kernel for P=%d EY=%d EZ=%d", c->mesh.P, c->tile.EY, c->tile.EZ);
     if (e != cudaSuccess) return tild_fail(c, TILD_ECUDA, "cudaFuncSetAttribute(spread_tile_kernel, %zu B): %s", bytes, cudaGetErrorString(e));
     return TILD_OK;
@@ -351,6 +352,11 @@ int launch_spread(tild_ctx* c, const SegLayout& lay, const float4* X4, float* gr
     const TileParams& tp = c->tile;
     // P = 1 touches one node per particle: the per-particle kernel is faster than any tiling (profiles/r1_c5_sweep.md)
     if (!tp.enabled || c->mesh.P == 1 || (c->prm.flags & TILD_FLAG_NAIVE_SPREAD)) return spread_slots(c, 0, (size_t)c->mesh.n, X4, grid);
+    if (spread_rot_applies(c) && !(c->prm.flags & TILD_FLAG_GEN1_TILES)) {
+        spread_rot_run(c, lay.seg_base, X4, grid, false);
+        TILD_LAUNCH_CHECK(c, "spread_rot_kernel");
+        return TILD_OK;
+    }
     const dim3 g((unsigned)tp.ntiles, (unsigned)((c->mesh.S + tp.sp_group - 1) / tp.sp_group));
     tile_dispatch(c->mesh.P, tp.EY, tp.EZ, [&](auto kernel) {
         kernel<<<g, SPREAD_THREADS, tp.smem_spread, c->stream>>>(c->mesh, tp, lay.seg_base, X4, grid);
