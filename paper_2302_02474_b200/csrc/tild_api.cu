@@ -298,6 +298,9 @@ int tild_init(tild_ctx** out, const tild_params* params, void* workspace, size_t
     m.S = S;
     m.P = p.order;
     m.M = (long long)c->M;
+    m.FN[0] = p.grid[1];
+    m.FN[1] = p.grid[2];
+    m.FM = (long long)c->M;
     for (int a = 0; a < 3; ++a) {
         m.N[a] = p.grid[a];
         m.inv_h[a] = (float)((double)p.grid[a] / p.box[a]);

@@ -17,6 +17,11 @@ struct MeshParams {
     float L[3];
     float inv_L[3];
     long long M;     // Nx*Ny*Nz
+    // layout of the force field the interpolation kernels read: node (x, y, z) of component c is at
+    // ffield[c * FM + (x * FN[0] + y) * FN[1] + z].  Plain arrays: FN = (Ny, Nz), FM = M.  (A ghost-padded layout for TMA
+    // staging was measured and dropped: cuFFT's C2R into padded rows costs more than the staging saves.)
+    int FN[2];
+    long long FM;
 };
 
 // Tiling of the cell grid.  A tile is T[0] x T[1] x T[2] cells; its shared-memory image holds

@@ -101,7 +101,7 @@ __global__ void __launch_bounds__(RT, TILD_ROT_CTAS) interp_rot_kernel(MeshParam
 
     auto stage = [&](int sp) {   // three components of species sp -> image (periodic wrap per row); asynchronous
         if (TILD_ROT_ABL & 1) return;
-        const float* fsp = ffield + (size_t)sp * 3 * m.M;
+        const float* fsp = ffield + (size_t)sp * 3 * m.FM;
         if (vec16) {
             // 16-byte copies: the image starts on a 16-byte boundary of the mesh rows (tp.sh) and Nz % 4 == 0,
             // so every aligned float4 of a row stays inside the row and wraps as a whole
@@ -112,10 +112,10 @@ __global__ void __launch_bounds__(RT, TILD_ROT_CTAS) interp_rot_kernel(MeshParam
                 for (int q = threadIdx.x / CPR; q < REX * EY; q += RPP) {
                     const int lx = q / EY, ly = q - lx * EY;
                     if (ly >= E[1]) continue;
-                    const float* src = fsp + ((size_t)goff_x[lx] * m.N[1] + goff_y[ly]) * m.N[2] + gz;
+                    const float* src = fsp + ((size_t)goff_x[lx] * m.FN[0] + goff_y[ly]) * m.FN[1] + gz;
                     float* dst = fs + q * EZ + 4 * chunk;
 #pragma unroll
-                    for (int comp = 0; comp < 3; ++comp) cp_async_16(dst + comp * CS, src + (size_t)comp * m.M);
+                    for (int comp = 0; comp < 3; ++comp) cp_async_16(dst + comp * CS, src + (size_t)comp * m.FM);
                 }
         } else {
             constexpr int RPP = RT / EZ;
@@ -125,10 +125,10 @@ __global__ void __launch_bounds__(RT, TILD_ROT_CTAS) interp_rot_kernel(MeshParam
                 for (int q = threadIdx.x / EZ; q < REX * EY; q += RPP) {
                     const int lx = q / EY, ly = q - lx * EY;
                     if (ly >= E[1]) continue;
-                    const float* src = fsp + ((size_t)goff_x[lx] * m.N[1] + goff_y[ly]) * m.N[2] + gz;
+                    const float* src = fsp + ((size_t)goff_x[lx] * m.FN[0] + goff_y[ly]) * m.FN[1] + gz;
                     float* dst = fs + q * EZ + lz;
 #pragma unroll
-                    for (int comp = 0; comp < 3; ++comp) cp_async_f32(dst + comp * CS, src + (size_t)comp * m.M);
+                    for (int comp = 0; comp < 3; ++comp) cp_async_f32(dst + comp * CS, src + (size_t)comp * m.FM);
                 }
         }
         cp_async_commit();

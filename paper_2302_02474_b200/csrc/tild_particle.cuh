@@ -14,9 +14,9 @@ template <int P, bool VEC>
 __device__ __forceinline__ float3 interp_global(const MeshParams& m, const float* __restrict__ ffield, const int b[3],
                                                 const float w[3][P], int type)
 {
-    const float* fx = ffield + (size_t)type * 3 * m.M;
-    const float* fy = fx + m.M;
-    const float* fz = fy + m.M;
+    const float* fx = ffield + (size_t)type * 3 * m.FM;
+    const float* fy = fx + m.FM;
+    const float* fz = fy + m.FM;
     float3 acc = make_float3(0.f, 0.f, 0.f);
     if (VEC) {
         const int bzw = wrap_idx(b[2], m.N[2]);
@@ -34,10 +34,10 @@ __device__ __forceinline__ float3 interp_global(const MeshParams& m, const float
         }
 #pragma unroll
         for (int jx = 0; jx < P; ++jx) {
-            const size_t ox = (size_t)wrap_idx(b[0] + jx, m.N[0]) * m.N[1];
+            const size_t ox = (size_t)wrap_idx(b[0] + jx, m.N[0]) * m.FN[0];
 #pragma unroll
             for (int jy = 0; jy < P; ++jy) {
-                const size_t row = (ox + wrap_idx(b[1] + jy, m.N[1])) * m.N[2];
+                const size_t row = (ox + wrap_idx(b[1] + jy, m.N[1])) * m.FN[1];
                 const float wxy = w[0][jx] * w[1][jy];
                 const float* comp[3] = {fx, fy, fz};
                 float d[3];
@@ -63,10 +63,10 @@ __device__ __forceinline__ float3 interp_global(const MeshParams& m, const float
     for (int j = 0; j < P; ++j) iz[j] = wrap_idx(b[2] + j, m.N[2]);
 #pragma unroll
     for (int jx = 0; jx < P; ++jx) {
-        const size_t ox = (size_t)wrap_idx(b[0] + jx, m.N[0]) * m.N[1];
+        const size_t ox = (size_t)wrap_idx(b[0] + jx, m.N[0]) * m.FN[0];
 #pragma unroll
         for (int jy = 0; jy < P; ++jy) {
-            const size_t row = (ox + wrap_idx(b[1] + jy, m.N[1])) * m.N[2];
+            const size_t row = (ox + wrap_idx(b[1] + jy, m.N[1])) * m.FN[1];
             const float wxy = w[0][jx] * w[1][jy];
 #pragma unroll
             for (int jz = 0; jz < P; ++jz) {
