@@ -57,6 +57,11 @@ typedef struct {
     int32_t integrator; /* 0: GJF (A11); 1: Euler-Maruyama, overdamped */
     int32_t sampled_kernel; /* 0: analytic u^(k) (A5); 1: FFT of u_G sampled on the mesh, as PAPER.md L223 describes (A5b) */
     int32_t deconvolve; /* 0: kernel is u^(k) (A13); 1: u^(k) / W^(k)^2, W^ = prod_a sinc(k_a h_a / 2)^P */
+    /* SURVEY 8(f) remainder (round 2).  integrator 2 = velocity Verlet + Langevin ExtraForce (A24) */
+    int32_t dim2;       /* 1: two-dimensional system (Listing 1 L65): N[2] must be 1; z forces, noise and velocities are 0 (A27) */
+    double mu_ms;       /* Maier-Saupe parameter mu of PAPER.md Eq. 20 L241 (0 = off); needs ms_partner (A26) */
+    const double *q_pp; /* per-particle charges [n] or NULL: rho_c = sum_i q_i W(r - r_i) replaces sum_J z_J rho_J (A25) */
+    const int32_t *ms_partner; /* [n]: partner j that defines u_i = (r_i - r_j)/|r_i - r_j| of LC centre i, -1 = not a centre */
 } orc_params;
 
 static const double ORC_PI = 3.14159265358979323846264338327950288;
@@ -376,7 +381,14 @@ static double orc_uhat(const orc_params *p, int mx, int my, int mz)
  * beta U = (l_B / 2) int int rho_c(r) rho_c(r') / |r - r'|.  In Fourier space the pair kernel between unit charges is
  *   u^_el(k) = 4 pi l_B exp(-k^2 a_q^2) / k^2   (k != 0; the k = 0 mode is dropped: neutralising background),
  * so the force spectra gain the term -i k_a u^_el(k) z_I sum_J z_J n^_J / V. */
+static double orc_uel_any(const orc_params *p, int mx, int my, int mz);
+/* kernel of the PER-SPECIES charges; zero when electrostatics is off or when per-particle charges replace them (A25) */
 static double orc_uel(const orc_params *p, int mx, int my, int mz)
+{
+    if (p->q_pp) return 0.0;
+    return orc_uel_any(p, mx, my, mz);
+}
+static double orc_uel_any(const orc_params *p, int mx, int my, int mz)
 {
     if (!(p->bjerrum > 0.0)) return 0.0;
     const int m[3] = {mx, my, mz};
@@ -625,6 +637,243 @@ void orc_bond_force(const orc_params *p, const double *x, const int32_t *partner
 
 /* Total force F(x): PM part on the fp32-rounded positions (O1 defines the index map on fp32
  * input), bonds on the double positions. */
+/* ------------------------------------------------------------------------------------------
+ * helpers shared by the per-particle-charge and Maier-Saupe paths.
+ * mesh[g] = sum_i a_i W(g; r_i) (same weights and index map as O3), and its adjoint, the gather.
+ * ---------------------------------------------------------------------------------------- */
+static void orc_spread_scalar(const orc_params *p, const float *x, const double *a, double *mesh)
+{
+    const int P = p->P;
+    const size_t M = (size_t)p->N[0] * p->N[1] * p->N[2];
+    memset(mesh, 0, sizeof(double) * M);
+    for (int i = 0; i < p->n; ++i) {
+        if (a[i] == 0.0) continue;
+        int32_t b[3], c[3];
+        float t[3];
+        double w[3][ORC_MAX_ORDER];
+        orc_index_1(p, x + 3 * (size_t)i, b, t, c);
+        for (int d = 0; d < 3; ++d) orc_weights(P, (double)t[d], w[d]);
+        for (int jx = 0; jx < P; ++jx)
+            for (int jy = 0; jy < P; ++jy)
+                for (int jz = 0; jz < P; ++jz) {
+                    size_t g = ((size_t)orc_mod(b[0] + jx, p->N[0]) * p->N[1] + orc_mod(b[1] + jy, p->N[1])) * p->N[2] + orc_mod(b[2] + jz, p->N[2]);
+                    mesh[g] += a[i] * w[0][jx] * w[1][jy] * w[2][jz];
+                }
+    }
+}
+static double orc_gather_scalar(const orc_params *p, const double *mesh, const float *xi)
+{
+    const int P = p->P;
+    int32_t b[3], c[3];
+    float t[3];
+    double w[3][ORC_MAX_ORDER];
+    orc_index_1(p, xi, b, t, c);
+    for (int d = 0; d < 3; ++d) orc_weights(P, (double)t[d], w[d]);
+    double acc = 0.0;
+    for (int jx = 0; jx < P; ++jx)
+        for (int jy = 0; jy < P; ++jy)
+            for (int jz = 0; jz < P; ++jz) {
+                size_t g = ((size_t)orc_mod(b[0] + jx, p->N[0]) * p->N[1] + orc_mod(b[1] + jy, p->N[1])) * p->N[2] + orc_mod(b[2] + jz, p->N[2]);
+                acc += w[0][jx] * w[1][jy] * w[2][jz] * mesh[g];
+            }
+    return acc;
+}
+/* real mesh -> complex spectrum (unnormalised forward DFT, O4) */
+static void orc_forward(const orc_params *p, const double *mesh, double *hat)
+{
+    const size_t M = (size_t)p->N[0] * p->N[1] * p->N[2];
+    for (size_t g = 0; g < M; ++g) {
+        hat[2 * g] = mesh[g];
+        hat[2 * g + 1] = 0.0;
+    }
+    orc_dft3d(p->N, hat, -1);
+}
+
+/* Per-particle charges (reading A25).  PAPER.md L223: the electrostatic forces "use the ... charge density field".
+ * rho_c(g) = sum_i q_i W(g; r_i); E_a(m) = -i k_a u^_el(k_m) rho^_c(m) / V with the Coulomb kernel of A22; the force on
+ * particle i is q_i sum_g W(g; r_i) E(g).  ADDS into f. */
+static void orc_charge_force(const orc_params *p, const float *xf, double *f)
+{
+    const size_t M = (size_t)p->N[0] * p->N[1] * p->N[2];
+    const double V = p->L[0] * p->L[1] * p->L[2];
+    double *rho = (double *)malloc(sizeof(double) * M);
+    double *hat = (double *)malloc(sizeof(double) * 2 * M);
+    double *work = (double *)malloc(sizeof(double) * 2 * M);
+    orc_spread_scalar(p, xf, p->q_pp, rho);
+    orc_forward(p, rho, hat);
+    for (int a = 0; a < 3; ++a) {
+        for (int mx = 0; mx < p->N[0]; ++mx)
+            for (int my = 0; my < p->N[1]; ++my)
+                for (int mz = 0; mz < p->N[2]; ++mz) {
+                    size_t g = ((size_t)mx * p->N[1] + my) * p->N[2] + mz;
+                    double kg = orc_kgrad(p, a, a == 0 ? mx : (a == 1 ? my : mz));
+                    double uel = orc_uel_any(p, mx, my, mz);
+                    work[2 * g] = kg * uel * hat[2 * g + 1] / V;          /* -i (re + i im) = im - i re */
+                    work[2 * g + 1] = -kg * uel * hat[2 * g] / V;
+                }
+        orc_dft3d(p->N, work, +1);
+        for (size_t g = 0; g < M; ++g) rho[g] = work[2 * g];              /* reuse: E_a(g) */
+        for (int i = 0; i < p->n; ++i)
+            if (p->q_pp[i] != 0.0) f[3 * (size_t)i + a] += p->q_pp[i] * orc_gather_scalar(p, rho, xf + 3 * (size_t)i);
+    }
+    free(rho);
+    free(hat);
+    free(work);
+}
+/* its energy: (1/2V) sum_{k != 0} u^_el(k) |rho^_c(k)|^2 */
+static double orc_charge_energy(const orc_params *p, const float *xf)
+{
+    const size_t M = (size_t)p->N[0] * p->N[1] * p->N[2];
+    const double V = p->L[0] * p->L[1] * p->L[2];
+    double *rho = (double *)malloc(sizeof(double) * M);
+    double *hat = (double *)malloc(sizeof(double) * 2 * M);
+    orc_spread_scalar(p, xf, p->q_pp, rho);
+    orc_forward(p, rho, hat);
+    double e = 0.0;
+    for (int mx = 0; mx < p->N[0]; ++mx)
+        for (int my = 0; my < p->N[1]; ++my)
+            for (int mz = 0; mz < p->N[2]; ++mz) {
+                size_t g = ((size_t)mx * p->N[1] + my) * p->N[2] + mz;
+                e += orc_uel_any(p, mx, my, mz) * (hat[2 * g] * hat[2 * g] + hat[2 * g + 1] * hat[2 * g + 1]);
+            }
+    free(rho);
+    free(hat);
+    return 0.5 * e / V;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * Maier-Saupe interaction (PAPER.md IV.D L233-247, Eq. 19-20; reading A26).  Every LC centre i has a partner j and the
+ * orientation u_i = d / |d|, d = minimum image of r_i - r_j (L235), the tensor S_i = u_i u_i - I/3 (L235, D = 3), and
+ * the orientation field S(r) = sum_i S_i delta(r - r_i) (Eq. 19) is spread on the mesh with the density weights.
+ * beta U_MS = -(mu/rho0) int int S(r) : S(r') u_G(|r - r'|) (Eq. 20), on the mesh
+ *   U = -(mu / rho0) (1/V) sum_m u^(k_m) sum_ab |S^_ab(m)|^2            (same u^ as the density kernel, L241).
+ * "The forces are derived by explicit differentiation" (L241, not printed).  With Phi_ab = u_G * S_ab, i.e.
+ * Phi^_ab(m) = u^(k_m) S^_ab(m) / V:
+ *   dU = -(2 mu / rho0) sum_i [ dS_i : Phi(r_i) + S_i : grad Phi(r_i) . dr_i ],
+ *   dS_i : Phi = 2 (Phi u_i) . du_i,   du_i = (I - u_i u_i)(dr_i - dr_j) / |d|,
+ * so  F_i = (2 mu/rho0) S_i : grad Phi(r_i) + G_i,  F_j = -G_i,  G_i = (4 mu/rho0) (I - u_i u_i) Phi(r_i) u_i / |d|.
+ * Phi and its ik-gradient (Nyquist rule A6) are interpolated to r_i with the spread weights, exactly as the density
+ * forces are (L227).  6 independent components ab = xx, yy, zz, xy, xz, yz.
+ * ---------------------------------------------------------------------------------------- */
+static const int ORC_MS_A[6] = {0, 1, 2, 0, 0, 1}, ORC_MS_B[6] = {0, 1, 2, 1, 2, 2};
+static int orc_ms_tensor(const orc_params *p, const double *x, int i, double u[3], double *len, double S6[6])
+{
+    const int32_t j = p->ms_partner ? p->ms_partner[i] : -1;
+    if (j < 0) return 0;
+    double d[3], r2 = 0.0;
+    for (int a = 0; a < 3; ++a) {
+        d[a] = orc_min_image(x[3 * (size_t)i + a] - x[3 * (size_t)j + a], p->L[a]);
+        r2 += d[a] * d[a];
+    }
+    if (!(r2 > 0.0)) return 0;
+    *len = sqrt(r2);
+    for (int a = 0; a < 3; ++a) u[a] = d[a] / *len;
+    for (int q = 0; q < 6; ++q) S6[q] = u[ORC_MS_A[q]] * u[ORC_MS_B[q]] - (q < 3 ? 1.0 / 3.0 : 0.0);
+    return 1;
+}
+/* spectra S^_ab of the six components: hat[q] complex [M] */
+static double *orc_ms_spectra(const orc_params *p, const double *x, const float *xf)
+{
+    const size_t M = (size_t)p->N[0] * p->N[1] * p->N[2];
+    double *hat = (double *)malloc(sizeof(double) * 2 * M * 6);
+    double *a = (double *)malloc(sizeof(double) * (size_t)p->n);
+    double *mesh = (double *)malloc(sizeof(double) * M);
+    for (int q = 0; q < 6; ++q) {
+        for (int i = 0; i < p->n; ++i) {
+            double u[3], len, S6[6];
+            a[i] = orc_ms_tensor(p, x, i, u, &len, S6) ? S6[q] : 0.0;
+        }
+        orc_spread_scalar(p, xf, a, mesh);
+        orc_forward(p, mesh, hat + 2 * M * (size_t)q);
+    }
+    free(a);
+    free(mesh);
+    return hat;
+}
+static double orc_ms_energy(const orc_params *p, const double *x, const float *xf)
+{
+    const size_t M = (size_t)p->N[0] * p->N[1] * p->N[2];
+    const double V = p->L[0] * p->L[1] * p->L[2];
+    double *hat = orc_ms_spectra(p, x, xf);
+    double *utab = orc_sampled_uhat(p);
+    double e = 0.0;
+    for (int mx = 0; mx < p->N[0]; ++mx)
+        for (int my = 0; my < p->N[1]; ++my)
+            for (int mz = 0; mz < p->N[2]; ++mz) {
+                size_t g = ((size_t)mx * p->N[1] + my) * p->N[2] + mz;
+                double uhat = utab ? utab[g] : orc_uhat(p, mx, my, mz), s2 = 0.0;
+                for (int q = 0; q < 6; ++q) {
+                    const double *h = hat + 2 * (M * (size_t)q + g);
+                    s2 += (q < 3 ? 1.0 : 2.0) * (h[0] * h[0] + h[1] * h[1]);       /* off-diagonal entries occur twice in S : S */
+                }
+                e += uhat * s2;
+            }
+    free(hat);
+    free(utab);
+    return -(p->mu_ms / p->rho0) * e / V;
+}
+/* ADDS the Maier-Saupe forces into f */
+static void orc_ms_force(const orc_params *p, const double *x, const float *xf, double *f)
+{
+    const size_t M = (size_t)p->N[0] * p->N[1] * p->N[2];
+    const double V = p->L[0] * p->L[1] * p->L[2], pref = p->mu_ms / p->rho0;
+    double *hat = orc_ms_spectra(p, x, xf);
+    double *utab = orc_sampled_uhat(p);
+    double *work = (double *)malloc(sizeof(double) * 2 * M);
+    double *field = (double *)malloc(sizeof(double) * M);
+    double *phi = (double *)calloc((size_t)p->n * 6, sizeof(double));            /* Phi_ab(r_i) */
+    for (int q = 0; q < 6; ++q) {
+        for (int a = -1; a < 3; ++a) {                                           /* a = -1: Phi itself; 0..2: d Phi / d x_a */
+            for (int mx = 0; mx < p->N[0]; ++mx)
+                for (int my = 0; my < p->N[1]; ++my)
+                    for (int mz = 0; mz < p->N[2]; ++mz) {
+                        size_t g = ((size_t)mx * p->N[1] + my) * p->N[2] + mz;
+                        double uhat = (utab ? utab[g] : orc_uhat(p, mx, my, mz)) / V;
+                        const double *h = hat + 2 * (M * (size_t)q + g);
+                        if (a < 0) {
+                            work[2 * g] = uhat * h[0];
+                            work[2 * g + 1] = uhat * h[1];
+                        } else {                                                 /* i k (re + i im) = -k im + i k re */
+                            double kg = orc_kgrad(p, a, a == 0 ? mx : (a == 1 ? my : mz));
+                            work[2 * g] = -kg * uhat * h[1];
+                            work[2 * g + 1] = kg * uhat * h[0];
+                        }
+                    }
+            orc_dft3d(p->N, work, +1);
+            for (size_t g = 0; g < M; ++g) field[g] = work[2 * g];
+            for (int i = 0; i < p->n; ++i) {
+                double u[3], len, S6[6];
+                if (!orc_ms_tensor(p, x, i, u, &len, S6)) continue;
+                double val = orc_gather_scalar(p, field, xf + 3 * (size_t)i);
+                if (a < 0) phi[(size_t)i * 6 + q] = val;
+                else f[3 * (size_t)i + a] += 2.0 * pref * (q < 3 ? 1.0 : 2.0) * S6[q] * val;     /* S_i : d_a Phi */
+            }
+        }
+    }
+    for (int i = 0; i < p->n; ++i) {
+        double u[3], len, S6[6];
+        if (!orc_ms_tensor(p, x, i, u, &len, S6)) continue;
+        const double *ph = phi + (size_t)i * 6;
+        const double Pm[3][3] = {{ph[0], ph[3], ph[4]}, {ph[3], ph[1], ph[5]}, {ph[4], ph[5], ph[2]}};
+        double pu[3], upu = 0.0;
+        for (int a = 0; a < 3; ++a) {
+            pu[a] = Pm[a][0] * u[0] + Pm[a][1] * u[1] + Pm[a][2] * u[2];
+            upu += u[a] * pu[a];
+        }
+        const int32_t j = p->ms_partner[i];
+        for (int a = 0; a < 3; ++a) {
+            const double G = 4.0 * pref * (pu[a] - u[a] * upu) / len;             /* (I - u u) Phi u / |d| */
+            f[3 * (size_t)i + a] += G;
+            f[3 * (size_t)j + a] -= G;
+        }
+    }
+    free(hat);
+    free(utab);
+    free(work);
+    free(field);
+    free(phi);
+}
+
 void orc_force(const orc_params *p, const double *x, const int32_t *type, const int32_t *partner, double *f)
 {
     const size_t M = (size_t)p->N[0] * p->N[1] * p->N[2];
@@ -636,6 +885,10 @@ void orc_force(const orc_params *p, const double *x, const int32_t *type, const 
     orc_kspace_force(p, grid, ff);
     orc_interp(p, ff, xf, type, f);
     orc_bond_force(p, x, partner, f);
+    if (p->q_pp && p->bjerrum > 0.0) orc_charge_force(p, xf, f);
+    if (p->mu_ms != 0.0 && p->ms_partner) orc_ms_force(p, x, xf, f);
+    if (p->dim2)
+        for (int i = 0; i < p->n; ++i) f[3 * (size_t)i + 2] = 0.0;          /* A27: no motion along z */
     free(xf);
     free(grid);
     free(ff);
@@ -729,6 +982,7 @@ void orc_gjf_step(const orc_params *p, double *x, double *v, double *f, const in
     for (int i = 0; i < p->n; ++i) {
         if (p->gamma > 0.0) orc_noise(p, (uint32_t)i, step + 1, beta + 3 * (size_t)i);
         else beta[3 * (size_t)i] = beta[3 * (size_t)i + 1] = beta[3 * (size_t)i + 2] = 0.0;
+        if (p->dim2) beta[3 * (size_t)i + 2] = v[3 * (size_t)i + 2] = 0.0;     /* A27 */
     }
     for (int i = 0; i < p->n; ++i)
         for (int c = 0; c < 3; ++c) {
@@ -758,6 +1012,7 @@ void orc_em_step(const orc_params *p, double *x, double *f, const int32_t *type,
     for (int i = 0; i < p->n; ++i) {
         double beta[3];
         orc_noise(p, (uint32_t)i, step + 1, beta);
+        if (p->dim2) beta[2] = 0.0;                                            /* A27 */
         for (int c = 0; c < 3; ++c) {
             size_t q = 3 * (size_t)i + c;
             x[q] = orc_wrap(x[q] + (p->dt / p->gamma) * f[q] + beta[c] / p->gamma, p->L[c]);
@@ -768,11 +1023,49 @@ void orc_em_step(const orc_params *p, double *x, double *f, const int32_t *type,
     free(fnew);
 }
 
+/* ------------------------------------------------------------------------------------------
+ * Velocity Verlet + Langevin ExtraForce (VV "needs to be coupled with additional thermostat ...
+ * Langevin noise ... part of the ExtraForce class"; L320: "Langevin: adds random noise to the selected group of particles.
+ * Can be used with Velocity Verlet integrator"; no equations).  Reading A24: the ExtraForce adds -gamma v + beta/dt to the
+ * force that the two half kicks of velocity Verlet use, evaluated with the velocity at hand and ONE noise per step,
+ * beta ~ N(0, 2 gamma kT dt) from the same Philox counters as GJF:
+ *   v+ = v + (dt/2m)(F - gamma v + beta/dt);  r' = r + dt v+ (wrapped);  F' = F(r');
+ *   v' = v+ + (dt/2m)(F' - gamma v+ + beta/dt).
+ * gamma = 0 is plain velocity Verlet.  One force evaluation per step; f holds F(r) on entry and F(r') on exit.
+ * ---------------------------------------------------------------------------------------- */
+void orc_vv_step(const orc_params *p, double *x, double *v, double *f, const int32_t *type,
+                 const int32_t *partner, uint64_t step)
+{
+    const double m = p->mass, dt = p->dt, h = dt / (2.0 * m);
+    const size_t n3 = 3 * (size_t)p->n;
+    double *beta = (double *)malloc(sizeof(double) * n3);
+    double *fnew = (double *)malloc(sizeof(double) * n3);
+    for (int i = 0; i < p->n; ++i) {
+        if (p->gamma > 0.0) orc_noise(p, (uint32_t)i, step + 1, beta + 3 * (size_t)i);
+        else beta[3 * (size_t)i] = beta[3 * (size_t)i + 1] = beta[3 * (size_t)i + 2] = 0.0;
+        if (p->dim2) beta[3 * (size_t)i + 2] = v[3 * (size_t)i + 2] = 0.0;     /* A27 */
+    }
+    for (int i = 0; i < p->n; ++i)
+        for (int c = 0; c < 3; ++c) {
+            size_t q = 3 * (size_t)i + c;
+            v[q] += h * (f[q] - p->gamma * v[q] + beta[q] / dt);
+            x[q] = orc_wrap(x[q] + dt * v[q], p->L[c]);
+        }
+    orc_force(p, x, type, partner, fnew);
+    for (size_t q = 0; q < n3; ++q) {
+        v[q] += h * (fnew[q] - p->gamma * v[q] + beta[q] / dt);
+        f[q] = fnew[q];
+    }
+    free(beta);
+    free(fnew);
+}
+
 void orc_run(const orc_params *p, double *x, double *v, double *f, const int32_t *type,
              const int32_t *partner, uint64_t step0, int32_t nsteps)
 {
     for (int32_t s = 0; s < nsteps; ++s) {
-        if (p->integrator == 1) orc_em_step(p, x, f, type, partner, step0 + (uint64_t)s);
+        if (p->integrator == 2) orc_vv_step(p, x, v, f, type, partner, step0 + (uint64_t)s);
+        else if (p->integrator == 1) orc_em_step(p, x, f, type, partner, step0 + (uint64_t)s);
         else orc_gjf_step(p, x, v, f, type, partner, step0 + (uint64_t)s);
     }
 }
@@ -834,6 +1127,8 @@ void orc_energy(const orc_params *p, const double *x, const double *v, const int
                 nb += uhat * acc + orc_uel(p, mx, my, mz) * el;
             }
     nb *= 0.5 / V;
+    if (p->q_pp && p->bjerrum > 0.0) nb += orc_charge_energy(p, xf);
+    if (p->mu_ms != 0.0 && p->ms_partner) nb += orc_ms_energy(p, x, xf);
     free(xf);
     free(grid);
     free(utab_e);
@@ -856,4 +1151,84 @@ void orc_energy(const orc_params *p, const double *x, const double *v, const int
     }
     e[1] = be;
     e[2] = nb;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * Pressure virial ("the contribution the bonded interactions make to the pressure virial coefficient";
+ * non-bonded virial from the k-space kernel).  W = -dU/d(ln lambda) under the affine scaling
+ * r -> lambda r, L -> lambda L (mesh scaled with the box, so weights and n^ are unchanged); the excess pressure is
+ * W / (3 V).
+ *   w[0] bonds: sum over bonds of -dU/dr r = -2 k (r - r0) r (angles are scale invariant: no contribution);
+ *   w[1] non-bonded on the mesh: U = (1/2V) sum_m u^(k_m) A_m with A_m independent of lambda, k -> k / lambda, V -> lambda^3 V:
+ *        W = 3 U + (1/2V) sum_m (k . grad_k u^)(k_m) A_m,   k . grad u^ = -sigma2 k^2 u^ for the Gaussian kernel
+ *        (the deconvolution factor depends on k h only: invariant), (-2 k^2 a_q^2 - 2) u^_el for the Coulomb kernel.
+ *        Per-particle charges and the Maier-Saupe term have the same form.  Not defined for the sampled kernel (NaN).
+ * ---------------------------------------------------------------------------------------- */
+void orc_virial(const orc_params *p, const double *x, const int32_t *type, const int32_t *partner, double w[2])
+{
+    const int S = p->S;
+    const size_t M = (size_t)p->N[0] * p->N[1] * p->N[2];
+    const double V = p->L[0] * p->L[1] * p->L[2];
+    double wb = 0.0;
+    for (int i = 0; i < p->n; ++i)
+        for (int s = 0; s < p->max_bonds; ++s) {
+            int32_t j = partner[(size_t)i * p->max_bonds + s];
+            if (j < 0 || j < i) continue;
+            double r2 = 0.0;
+            for (int a = 0; a < 3; ++a) {
+                double d = orc_min_image(x[3 * (size_t)i + a] - x[3 * (size_t)j + a], p->L[a]);
+                r2 += d * d;
+            }
+            double r = sqrt(r2);
+            wb += -2.0 * p->k_bond * (r - p->r0_bond) * r;
+        }
+    w[0] = wb;
+    if (p->sampled_kernel) {
+        w[1] = NAN;
+        return;
+    }
+    float *xf = (float *)malloc(sizeof(float) * 3 * (size_t)p->n);
+    double *grid = (double *)malloc(sizeof(double) * M * (size_t)S);
+    double *nhat = (double *)malloc(sizeof(double) * 2 * M * (size_t)S);
+    for (size_t q = 0; q < 3 * (size_t)p->n; ++q) xf[q] = (float)x[q];
+    orc_spread(p, xf, type, grid);
+    for (int J = 0; J < S; ++J) orc_forward(p, grid + (size_t)J * M, nhat + 2 * M * (size_t)J);
+    double *qhat = NULL, *shat = NULL;
+    if (p->q_pp && p->bjerrum > 0.0) {
+        qhat = (double *)malloc(sizeof(double) * 2 * M);
+        orc_spread_scalar(p, xf, p->q_pp, grid);
+        orc_forward(p, grid, qhat);
+    }
+    if (p->mu_ms != 0.0 && p->ms_partner) shat = orc_ms_spectra(p, x, xf);
+    double acc = 0.0;
+    for (int mx = 0; mx < p->N[0]; ++mx)
+        for (int my = 0; my < p->N[1]; ++my)
+            for (int mz = 0; mz < p->N[2]; ++mz) {
+                size_t g = ((size_t)mx * p->N[1] + my) * p->N[2] + mz;
+                double kx = orc_k(p, 0, mx), ky = orc_k(p, 1, my), kz = orc_k(p, 2, mz), k2 = kx * kx + ky * ky + kz * kz;
+                double A = 0.0, Ael = 0.0;
+                for (int I = 0; I < S; ++I)
+                    for (int J = 0; J < S; ++J) {
+                        const double *aI = nhat + 2 * (M * (size_t)I + g), *aJ = nhat + 2 * (M * (size_t)J + g);
+                        A += orc_cIJ(p, I, J) * (aI[0] * aJ[0] + aI[1] * aJ[1]);
+                        Ael += p->charge[I] * p->charge[J] * (aI[0] * aJ[0] + aI[1] * aJ[1]);
+                    }
+                if (qhat) Ael = qhat[2 * g] * qhat[2 * g] + qhat[2 * g + 1] * qhat[2 * g + 1];
+                if (shat) {
+                    double s2 = 0.0;
+                    for (int q = 0; q < 6; ++q) {
+                        const double *h = shat + 2 * (M * (size_t)q + g);
+                        s2 += (q < 3 ? 1.0 : 2.0) * (h[0] * h[0] + h[1] * h[1]);
+                    }
+                    A += -2.0 * (p->mu_ms / p->rho0) * s2;                   /* U_MS = (1/2V) sum u^ (-2 mu/rho0) |S^|^2 */
+                }
+                acc += orc_uhat(p, mx, my, mz) * A * (3.0 - p->sigma2 * k2) +
+                       orc_uel_any(p, mx, my, mz) * Ael * (3.0 - 2.0 * k2 * p->a_charge * p->a_charge - 2.0);
+            }
+    w[1] = 0.5 * acc / V;
+    free(xf);
+    free(grid);
+    free(nhat);
+    free(qhat);
+    free(shat);
 }

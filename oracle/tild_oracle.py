@@ -46,6 +46,10 @@ class _Params(C.Structure):
         ("integrator", C.c_int32),
         ("sampled_kernel", C.c_int32),
         ("deconvolve", C.c_int32),
+        ("dim2", C.c_int32),
+        ("mu_ms", C.c_double),
+        ("q_pp", C.c_void_p),
+        ("ms_partner", C.c_void_p),
     ]
 
 
@@ -75,9 +79,13 @@ class OracleParams:
     charge: tuple = ()         # valence per species (reading A22); bjerrum = 0 switches electrostatics off
     bjerrum: float = 0.0
     a_charge: float = 0.5
-    integrator: int = 0        # 0 GJF (A11), 1 Euler-Maruyama (A11b)
+    integrator: int = 0        # 0 GJF (A11), 1 Euler-Maruyama (A11b), 2 velocity Verlet + Langevin ExtraForce (A24)
     sampled_kernel: bool = False  # u^ from the FFT of u_G sampled on the mesh (A5b) instead of analytic (A5)
     deconvolve: bool = False   # divide the pair kernel by W^(k)^2; default: plain u^(k) (A13)
+    dim2: bool = False         # two-dimensional system: N[2] = 1, no motion along z (A27)
+    mu_ms: float = 0.0         # Maier-Saupe mu (Eq. 20); needs ms_partner (A26)
+    q_pp: np.ndarray = None    # per-particle charges [n] (A25); None = charges per species
+    ms_partner: np.ndarray = None  # [n] orientation partner of every LC centre, -1 = not a centre
     _c: _Params = field(default=None, repr=False)
 
     def c(self) -> _Params:
@@ -105,6 +113,15 @@ class OracleParams:
         p.integrator = int(self.integrator)
         p.sampled_kernel = 1 if self.sampled_kernel else 0
         p.deconvolve = 1 if self.deconvolve else 0
+        p.dim2 = 1 if self.dim2 else 0
+        p.mu_ms = float(self.mu_ms)
+        # the arrays must outlive the C call: keep contiguous copies on the dataclass
+        if self.q_pp is not None:
+            self._q = np.ascontiguousarray(self.q_pp, dtype=np.float64)
+            p.q_pp = self._q.ctypes.data
+        if self.ms_partner is not None:
+            self._msp = np.ascontiguousarray(self.ms_partner, dtype=np.int32)
+            p.ms_partner = self._msp.ctypes.data
         return p
 
     @property
@@ -284,6 +301,15 @@ def energy(p: OracleParams, x, v, type_, partner) -> np.ndarray:
     lib().orc_energy(C.byref(cp), _ptr(x, C.c_double), _ptr(v, C.c_double), _ptr(type_, C.c_int32),
                      _ptr(partner, C.c_int32), _ptr(e, C.c_double))
     return e
+
+
+def virial(p: OracleParams, x, type_, partner) -> np.ndarray:
+    """(bonded, non-bonded) pressure virial W = -dU/d ln(lambda) of the affine scaling; excess pressure = W / 3V."""
+    x, type_, partner = _f64(x), _i32(type_), _i32(partner)
+    w = np.zeros(2, dtype=np.float64)
+    cp = p.c()
+    lib().orc_virial(C.byref(cp), _ptr(x, C.c_double), _ptr(type_, C.c_int32), _ptr(partner, C.c_int32), _ptr(w, C.c_double))
+    return w
 
 
 def structure_factor(p: OracleParams, x, type_, species=None) -> np.ndarray:

@@ -495,6 +495,11 @@ def ewald_smeared_energy(x, z, L, lB, aq, alpha, kmax=12, images=2):
     G = 4 * np.pi * lB * np.exp(-K2 / (4 * alpha ** 2)) / K2
     G[kmax, kmax, kmax] = 0.0
     S = sum(z[j] * np.exp(-1j * (KX * x[j, 0] + KY * x[j, 1] + KZ * x[j, 2])) for j in range(n))
+    # net charge Q: the definition drops the k = 0 mode of the WHOLE pair potential (neutralising background), but the
+    # real-space sum above contains the k = 0 component of its short-ranged part,
+    # int d^3r lB [erf(r/2aq) - erf(alpha r)] / r = pi lB (1/alpha^2 - 4 aq^2): take it out again (zero for Q = 0)
+    Q = float(np.sum(z))
+    E -= 0.5 * Q * Q * np.pi * lB * (1.0 / alpha ** 2 - 4.0 * aq ** 2) / V
     return E + 0.5 * (G * np.abs(S) ** 2).sum() / V
 
 
