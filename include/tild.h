@@ -66,12 +66,18 @@ typedef enum {
                                       2*resort_every steps as one CUDA graph (launch-bound small systems: C1 0.066 -> 0.044 ms
                                       per step) whenever it can -- no TILD_FLAG_TIMING, an even resort_every, and a stream
                                       that can be captured (not the legacy default stream); otherwise it launches eagerly */
+#define TILD_FLAG_2D 512u          /* two-dimensional system (Listing 1 L65; A27): grid[2] must be 1; the z
+                                      coordinates are carried along unchanged, no force, noise or velocity along z.  box[2] is
+                                      the thickness that turns the areal density into rho0 = n / V */
 #define TILD_FLAG_GEN1_TILES 128u   /* first-generation tile kernels (32 bank classes with overflow rounds, per-particle work
                                       in class order) even where the rotation-class kernels apply (P = 4); for A/B runs */
 
 /* integrators */
 #define TILD_INTEGRATOR_GJF 0   /* Gronbech-Jensen & Farago, one force evaluation per step */
 #define TILD_INTEGRATOR_EM 1    /* Euler-Maruyama: r' = r + (dt/gamma) F + sqrt(2 kT dt/gamma) xi; velocities unused */
+#define TILD_INTEGRATOR_VV 2    /* velocity Verlet with the Langevin ExtraForce -gamma v + beta/dt in both half kicks, one noise
+                                   per step (A24); gamma = 0: plain velocity Verlet;
+                                   needs gamma dt / 2m < 1 */
 
 typedef struct tild_ctx tild_ctx;
 
@@ -96,7 +102,8 @@ typedef struct {
     uint64_t seed;             /* Philox4x32-10 key (A12) */
     int32_t resort_every;      /* physically re-sort particles by cell every this many steps; <= 0 -> default */
     uint32_t flags;            /* TILD_FLAG_* */
-    int32_t integrator;        /* TILD_INTEGRATOR_GJF (default, A11) or TILD_INTEGRATOR_EM (overdamped, A11b; gamma > 0) */
+    int32_t integrator;        /* TILD_INTEGRATOR_GJF (default, A11), TILD_INTEGRATOR_EM (overdamped, A11b; gamma > 0) or
+                                  TILD_INTEGRATOR_VV (velocity Verlet + Langevin ExtraForce, A24) */
     int32_t tile_shape;        /* 0 = default tile of 8 x 16 x 32 cells; else TY | TZ << 8 with TY in {8, 16}, TZ in {16, 32} */
     /* electrostatics on the same path (reading A22): valence per species, Bjerrum length
      * (0 = off), Gaussian smearing length of a charge; pair kernel 4 pi l_B exp(-k^2 a_q^2) / k^2, k = 0 dropped */
@@ -156,6 +163,12 @@ int tild_get_state(tild_ctx*, float* x, float* v, float* f, uint64_t* step /*HOS
  * lambda (1 + cos theta) and k_theta (theta - theta0)^2 (Eq. 16-17) of every centre bead; e[2] non-bonded on the mesh
  * (1/2V) sum_m u^(k_m) sum_IJ c_IJ Re[n^_I(m) conj(n^_J(m))] (Eq. 3-4).  One force evaluation, no state change. */
 int tild_energy(tild_ctx*, double e[3] /*HOST out*/);
+
+/* HOST out, synchronises.  Pressure virial of the current state, W = -dU/d ln(lambda) under the affine scaling r -> lambda r,
+ * L -> lambda L (excess pressure = W / 3V): w[0] bonds, sum over bonds of -2 k (|d| - r0) |d| (the angle
+ * potentials are scale invariant); w[1] non-bonded on the mesh, (1/2V) sum_m (3 - sigma2 k_m^2) u^(k_m) sum_IJ c_IJ Re[n^_I n^_J*]
+ * plus (1 - 2 k^2 a_q^2) times the Coulomb term; NaN with TILD_FLAG_SAMPLED_KERNEL. */
+int tild_virial(tild_ctx*, double w[2] /*HOST out*/);
 
 /* Structure factor of the current state (diagnostic; Eq. 23, "Compute" class L332-336):
  * sk[m] (= or +=, by `accumulate`) |sum_{J in species_mask} n^_J(m)|^2 / N_mask on the half spectrum

@@ -83,13 +83,16 @@ int validate(const tild_params* p)
     if (p->max_bonds < 0 || p->max_bonds > TILD_MAX_BONDS) return TILD_EINVAL;
     double M = 1.0;
     for (int a = 0; a < 3; ++a) {
-        if (!(p->box[a] > 0.0) || p->grid[a] < p->order || p->grid[a] < 2 || p->grid[a] > 4096) return TILD_EINVAL;
+        const bool flat = a == 2 && (p->flags & TILD_FLAG_2D);          // 2-D mode: one plane of nodes, any order
+        if (flat && p->grid[a] != 1) return TILD_EINVAL;
+        if (!(p->box[a] > 0.0) || (!flat && (p->grid[a] < p->order || p->grid[a] < 2)) || p->grid[a] > 4096) return TILD_EINVAL;
         M *= p->grid[a];
     }
     if (M > 2.0e9) return TILD_EINVAL;
     if (!(p->sigma2 > 0.0) && !(p->a > 0.0)) return TILD_EINVAL;
     if (!(p->dt > 0.0) || !(p->mass > 0.0) || p->gamma < 0.0 || p->kT < 0.0) return TILD_EINVAL;
-    if (p->integrator != TILD_INTEGRATOR_GJF && p->integrator != TILD_INTEGRATOR_EM) return TILD_EINVAL;
+    if (p->integrator != TILD_INTEGRATOR_GJF && p->integrator != TILD_INTEGRATOR_EM && p->integrator != TILD_INTEGRATOR_VV) return TILD_EINVAL;
+    if (p->integrator == TILD_INTEGRATOR_VV && !(p->gamma * p->dt / (2.0 * p->mass) < 1.0)) return TILD_EINVAL;   // c = 1 - gamma dt/2m > 0
     if (p->integrator == TILD_INTEGRATOR_EM && !(p->gamma > 0.0)) return TILD_EINVAL;
     if ((p->lambda_wlc != 0.0 || p->k_theta != 0.0) && p->max_bonds != 2) return TILD_EINVAL;
     if (!(p->k_theta >= 0.0) || !(p->theta0 >= 0.0 && p->theta0 <= 3.141592653589794)) return TILD_EINVAL;
@@ -169,7 +172,7 @@ void carve(tild_ctx* c, void* base, size_t* total)
     c->perm = w.take<uint32_t>(n);
     c->drift_count = w.take<uint32_t>(4);
     c->d_step = w.take<uint64_t>(2);
-    c->d_energy = w.take<double>(4);
+    c->d_energy = w.take<double>(8);
     c->tables = w.take<float>(14 * 4096);
     *total = w.off;
 }
@@ -356,7 +359,7 @@ int tild_init(tild_ctx** out, const tild_params* params, void* workspace, size_t
         tab[(size_t)12 * 4096 + 2 * j + 1] = (float)(-sin(ang));
     }
     c->xtw = reinterpret_cast<const float2*>(c->tables + (size_t)12 * 4096);
-    c->xfft_R = (p.flags & TILD_FLAG_PLAIN_FFT) ? 0 : kspace_xfft_radix(p.grid[0], S);
+    c->xfft_R = (p.flags & (TILD_FLAG_PLAIN_FFT | TILD_FLAG_2D)) ? 0 : kspace_xfft_radix(p.grid[0], S);
     KspaceParams& ks = c->ksp;
     ks.S = S;
     ks.Nzc = p.grid[2] / 2 + 1;
@@ -368,6 +371,8 @@ int tild_init(tild_ctx** out, const tild_params* params, void* workspace, size_t
         ks.k2[a] = c->tables + (size_t)(9 + a) * 4096;
     }
     ks.has_el = p.bjerrum > 0.0 ? 1 : 0;
+    ks.sigma2 = (float)sigma2;
+    ks.aq2 = (float)(p.a_charge * p.a_charge);
     for (int I = 0; I < S; ++I)
         for (int J = 0; J < S; ++J) {
             const double cij = (I == J) ? p.kappa / rho0 : (p.kappa + p.chi[I * TILD_MAX_SPECIES + J]) / rho0;  // A9
@@ -382,10 +387,21 @@ int tild_init(tild_ctx** out, const tild_params* params, void* workspace, size_t
     s.half_dt_over_m = (float)(p.dt / (2.0 * p.mass));
     s.kick_in = s.half_dt_over_m;
     s.a_g = (float)ag;
+    s.w_fr = s.half_dt_over_m;
     s.b_dt = (float)(bg * p.dt);
     s.b_dt2_over_2m = (float)(bg * p.dt * p.dt / (2.0 * p.mass));
     s.b_dt_over_2m = (float)(bg * p.dt / (2.0 * p.mass));
     s.b_over_m = (float)(bg / p.mass);
+    if (p.integrator == TILD_INTEGRATOR_VV) {   // velocity Verlet + Langevin ExtraForce (A24), c = 1 - gamma dt/2m
+        const double cc = 1.0 - gh;
+        s.a_g = (float)(cc * cc);
+        s.w_fr = (float)(p.dt / (2.0 * p.mass * cc));
+        s.b_dt = (float)(cc * p.dt);
+        s.b_dt2_over_2m = (float)(p.dt * p.dt / (2.0 * p.mass));
+        s.b_dt_over_2m = (float)(p.dt / (2.0 * p.mass));
+        s.b_over_m = (float)((1.0 + cc) / (2.0 * p.mass));
+    }
+    s.dim2 = (p.flags & TILD_FLAG_2D) ? 1 : 0;
     s.noise_amp = (float)sqrt(2.0 * p.gamma * p.kT * p.dt);
     s.k_bond = (float)p.k_bond;
     s.r0_bond = (float)p.r0_bond;
@@ -770,6 +786,19 @@ int tild_energy(tild_ctx* c, double e[3])
     if ((rc = launch_energy(c, c->d_energy))) return rc;
     TILD_CUDA(c, cudaMemcpyAsync(e, c->d_energy, 3 * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
     TILD_CUDA(c, cudaStreamSynchronize(c->stream));
+    return TILD_OK;
+}
+
+int tild_virial(tild_ctx* c, double w[2])
+{
+    DevGuard dg(c);
+    if (!c || !w) return TILD_EINVAL;
+    double e[3];
+    int rc = tild_energy(c, e);             // fills d_energy[0..4]
+    if (rc) return rc;
+    TILD_CUDA(c, cudaMemcpyAsync(w, c->d_energy + 3, 2 * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    TILD_CUDA(c, cudaStreamSynchronize(c->stream));
+    if (c->prm.flags & TILD_FLAG_SAMPLED_KERNEL) w[1] = NAN;   // k . grad u^ of the sampled kernel has no closed form
     return TILD_OK;
 }
 

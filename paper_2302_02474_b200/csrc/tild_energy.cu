@@ -26,7 +26,7 @@ template <int S>
 __global__ void __launch_bounds__(256) kspace_energy_kernel(KspaceParams k, size_t Mk, const float2* __restrict__ nhat,
                                                             double* __restrict__ out)
 {
-    double e = 0.0;
+    double e = 0.0, w = 0.0;
     for (size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x; idx < Mk; idx += (size_t)gridDim.x * blockDim.x) {
         const int mz = (int)(idx % k.Nzc);
         const size_t r = idx / k.Nzc;
@@ -50,15 +50,30 @@ __global__ void __launch_bounds__(256) kspace_energy_kernel(KspaceParams k, size
                        ((double)nj[I].x * nj[J].x + (double)nj[I].y * nj[J].y);
         const bool self_conjugate = mz == 0 || (k.N[2] % 2 == 0 && mz == k.N[2] / 2);
         e += (self_conjugate ? 0.5 : 1.0) * acc;
+        // pressure virial W = -dU/d ln(lambda) of the affine scaling: k -> k / lambda,
+        // V -> lambda^3 V, n^ unchanged: every mode contributes its energy times 3 + k . grad_k ln u^, i.e.
+        // 3 - sigma2 k^2 for the Gaussian kernel and 3 - 2 k^2 a_q^2 - 2 for the Coulomb kernel (deconvolution: invariant)
+        const double k2 = (double)__ldg(k.k2[0] + mx) + (double)__ldg(k.k2[1] + my) + (double)__ldg(k.k2[2] + mz);
+        double vacc = 0.0;
+#pragma unroll
+        for (int I = 0; I < S; ++I)
+#pragma unroll
+            for (int J = 0; J < S; ++J)
+                vacc += ((double)k.c[I * TILD_MAX_SPECIES + J] * u * (3.0 - (double)k.sigma2 * k2) +
+                         (double)k.qq[I * TILD_MAX_SPECIES + J] * uel * (1.0 - 2.0 * k2 * (double)k.aq2)) *
+                        ((double)nj[I].x * nj[J].x + (double)nj[I].y * nj[J].y);
+        w += (self_conjugate ? 0.5 : 1.0) * vacc;
     }
     block_add(e, out + 2);
+    __syncthreads();
+    block_add(w, out + 4);
 }
 
 __global__ void __launch_bounds__(256) particle_energy_kernel(MeshParams m, StepParams s, double mass, const float4* __restrict__ X4,
                                                               const float4* __restrict__ W4, const float4* __restrict__ F4,
                                                               const int32_t* __restrict__ B, double* __restrict__ out)
 {
-    double ke = 0.0, eb = 0.0;
+    double ke = 0.0, eb = 0.0, wb = 0.0;
     for (size_t slot = (size_t)blockIdx.x * blockDim.x + threadIdx.x; slot < (size_t)m.n; slot += (size_t)gridDim.x * blockDim.x) {
         const float4 p = X4[slot], w = W4[slot], f = F4[slot];
         const double vx = (double)w.x + (double)s.kick_in * f.x, vy = (double)w.y + (double)s.kick_in * f.y,
@@ -70,8 +85,9 @@ __global__ void __launch_bounds__(256) particle_energy_kernel(MeshParams m, Step
             const float4 q = X4[j];
             const double dx = min_image(p.x - q.x, m.L[0], m.inv_L[0]), dy = min_image(p.y - q.y, m.L[1], m.inv_L[1]),
                          dz = min_image(p.z - q.z, m.L[2], m.inv_L[2]);
-            const double d = sqrt(dx * dx + dy * dy + dz * dz) - (double)s.r0_bond;
+            const double r = sqrt(dx * dx + dy * dy + dz * dz), d = r - (double)s.r0_bond;
             eb += (double)s.k_bond * d * d;
+            wb += -2.0 * (double)s.k_bond * d * r;             // bonded virial -dU/dr r (angles are scale invariant)
         }
         if (s.lambda_wlc != 0.0f || s.k_theta != 0.0f) {   // Eq. 16-17, counted by the angle's centre bead
             const int2 bb = *reinterpret_cast<const int2*>(B + 2 * slot);
@@ -94,6 +110,8 @@ __global__ void __launch_bounds__(256) particle_energy_kernel(MeshParams m, Step
     block_add(ke, out + 0);
     __syncthreads();
     block_add(eb, out + 1);
+    __syncthreads();
+    block_add(wb, out + 3);
 }
 
 // S(m) = |sum_{J in mask} n^_J(m)|^2 / N_mask on the half spectrum; N_mask = the m = 0 mode (Eq. 23)
@@ -129,7 +147,7 @@ int launch_structure_factor(tild_ctx* c, uint32_t mask, float* sk, int accumulat
 // F4 must hold the total force at the current positions and c->nhat their transformed densities (force_current)
 int launch_energy(tild_ctx* c, double* d_out)
 {
-    TILD_CUDA(c, cudaMemsetAsync(d_out, 0, 3 * sizeof(double), c->stream));
+    TILD_CUDA(c, cudaMemsetAsync(d_out, 0, 5 * sizeof(double), c->stream));   // e[0..2], bonded and mesh virial
     const unsigned nb = 592;
 #define KE(SS) case SS: kspace_energy_kernel<SS><<<nb, 256, 0, c->stream>>>(c->ksp, c->Mk, c->nhat, d_out); break;
     switch (c->mesh.S) {

@@ -63,16 +63,23 @@ struct KspaceParams {
     const float* eel[3];     // exp(-k_a^2 a_q^2) (times the deconvolution factor when that is on)
     const float* k2[3];      // k_a(m)^2, true wave number (Nyquist included)
     float qq[TILD_MAX_SPECIES * TILD_MAX_SPECIES];  // z_I z_J
+    float sigma2, aq2;       // variance of u_G and a_q^2 (virial)
 };
 
 struct StepParams {
     float half_dt_over_m;  // dt/2m
     float kick_in;         // v^n = w^n + kick_in F^n: dt/2m, or 0 while the state still holds v itself (first step after tild_set_state)
-    float a_g;             // (1 - gamma dt/2m)/(1 + gamma dt/2m)
-    float b_dt;            // b dt
-    float b_dt2_over_2m;   // b dt^2/2m
-    float b_dt_over_2m;    // b dt/2m
-    float b_over_m;        // b/m
+    // One step of every inertial integrator is linear in (v, F, beta) (A24):
+    //   r' = r + b_dt v + b_dt2_over_2m F + b_dt_over_2m beta,   w' = a_g (v + w_fr F) + b_over_m beta
+    // GJF (A11):            b dt, b dt^2/2m, b dt/2m;  a, dt/2m, b/m        (a, b of Gronbech-Jensen & Farago)
+    // VV + Langevin (A24):  c dt, dt^2/2m,   dt/2m;    c^2, dt/(2m c), (1 + c)/2m,   c = 1 - gamma dt/2m
+    float a_g;
+    float w_fr;
+    float b_dt;
+    float b_dt2_over_2m;
+    float b_dt_over_2m;
+    float b_over_m;
+    int dim2;              // TILD_FLAG_2D: no force, noise or motion along z (A27)
     float noise_amp;       // sqrt(2 gamma kT dt); 0 disables the draw
     float k_bond, r0_bond;
     int max_bonds;
@@ -117,7 +124,7 @@ struct tild_ctx {
     uint32_t* rank;       // [n] sort scratch; between sorts: the drift list of launch_interp
     uint32_t* inv;        // [n] old slot -> new slot
     uint32_t* drift_count;  // [4]
-    double* d_energy;       // [4] reduction targets of tild_energy
+    double* d_energy;       // [8] reduction targets of tild_energy / tild_virial
     uint64_t* d_step;       // device copy of `step` (read by the fused step kernels, advanced by a kernel)
     uint64_t h_step_upload; // staging for the asynchronous upload of d_step
     uint32_t* count;      // [max_bins+1] histogram

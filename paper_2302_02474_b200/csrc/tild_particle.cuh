@@ -156,9 +156,11 @@ __device__ __noinline__ float3 bond_force_slots(const MeshParams& m, const StepP
 // F already holds the total force; w0 = W4[slot] (MODE 2 only)
 template <int MODE>
 __device__ __forceinline__ void finish_update(const MeshParams& m, const StepParams& s, uint64_t step_next, size_t slot,
-                                              const float4& p, const float3& F, const float4& w0, float4* __restrict__ X4o,
+                                              const float4& p, const float3& Fin, const float4& w0, float4* __restrict__ X4o,
                                               float4* __restrict__ W4o, float4* __restrict__ F4)
 {
+    float3 F = Fin;
+    if (s.dim2) F.z = 0.0f;                      // A27: two-dimensional system, nothing acts or moves along z
     if (MODE <= 1) {
         F4[slot] = make_float4(F.x, F.y, F.z, 0.f);
         return;
@@ -166,12 +168,12 @@ __device__ __forceinline__ void finish_update(const MeshParams& m, const StepPar
     float3 beta = make_float3(0.f, 0.f, 0.f);
     if (s.noise_amp != 0.0f) {
         const float3 z = gauss3(__float_as_uint(w0.w), step_next, s.key0, s.key1);
-        beta = make_float3(s.noise_amp * z.x, s.noise_amp * z.y, s.noise_amp * z.z);
+        beta = make_float3(s.noise_amp * z.x, s.noise_amp * z.y, s.dim2 ? 0.f : s.noise_amp * z.z);
     }
     if (s.integrator == TILD_INTEGRATOR_EM) {   // r' = r + (dt/gamma) F + beta/gamma; velocities are not used (A11b)
         X4o[slot] = make_float4(wrap_pos(p.x + (s.em_drift * F.x + s.em_noise * beta.x), m.L[0], m.inv_L[0]),
                                 wrap_pos(p.y + (s.em_drift * F.y + s.em_noise * beta.y), m.L[1], m.inv_L[1]),
-                                wrap_pos(p.z + (s.em_drift * F.z + s.em_noise * beta.z), m.L[2], m.inv_L[2]), p.w);
+                                s.dim2 ? p.z : wrap_pos(p.z + (s.em_drift * F.z + s.em_noise * beta.z), m.L[2], m.inv_L[2]), p.w);
         W4o[slot] = w0;
         return;
     }
@@ -185,7 +187,11 @@ __device__ __forceinline__ void finish_update(const MeshParams& m, const StepPar
         const float v = wv[a] + s.kick_in * Fv[a];
         const float r = pp[a] + (s.b_dt * v + s.b_dt2_over_2m * Fv[a] + s.b_dt_over_2m * bv[a]);
         xo[a] = wrap_pos(r, m.L[a], m.inv_L[a]);
-        wo[a] = s.a_g * (v + s.half_dt_over_m * Fv[a]) + s.b_over_m * bv[a];
+        wo[a] = s.a_g * (v + s.w_fr * Fv[a]) + s.b_over_m * bv[a];
+    }
+    if (s.dim2) {
+        xo[2] = p.z;
+        wo[2] = 0.0f;
     }
     X4o[slot] = make_float4(xo[0], xo[1], xo[2], p.w);
     W4o[slot] = make_float4(wo[0], wo[1], wo[2], w0.w);

@@ -18,16 +18,17 @@ MAX_SPECIES = 8
 MAX_BONDS = 4
 
 OK, EINVAL, ENOMEM, ECUDA, ECUFFT, ESTATE = 0, -1, -2, -3, -4, -5
-INTEGRATOR_GJF, INTEGRATOR_EM = 0, 1
+INTEGRATOR_GJF, INTEGRATOR_EM, INTEGRATOR_VV = 0, 1, 2
 FLAG_TIMING, FLAG_NAIVE_SPREAD, FLAG_NAIVE_INTERP, FLAG_GRAPH, FLAG_DECONVOLVE, FLAG_SAMPLED_KERNEL = 1, 2, 4, 8, 16, 32
 FLAG_PLAIN_FFT = 64
 FLAG_GEN1_TILES = 128
 FLAG_EAGER = 256
+FLAG_2D = 512
 TIMING_NAMES = ("sort", "spread", "fft_fwd", "kspace", "fft_inv", "interp", "other", "total")
 
 EXPORTS = (
     "tild_workspace_bytes", "tild_init", "tild_set_state", "tild_spread", "tild_kspace_force", "tild_interp",
-    "tild_bond_force", "tild_step", "tild_get_state", "tild_energy", "tild_structure_factor", "tild_index_map", "tild_get_timings", "tild_run_host",
+    "tild_bond_force", "tild_step", "tild_get_state", "tild_energy", "tild_virial", "tild_structure_factor", "tild_index_map", "tild_get_timings", "tild_run_host",
     "tild_philox_test", "tild_layout_info", "tild_segment_layout", "tild_launch_count", "tild_last_error", "tild_destroy", "tild_version",
 )
 
@@ -118,6 +119,7 @@ def load():
     lib.tild_step.argtypes = [vp, i32]
     lib.tild_get_state.argtypes = [vp, vp, vp, vp, C.POINTER(u64)]
     lib.tild_energy.argtypes = [vp, C.POINTER(C.c_double * 3)]
+    lib.tild_virial.argtypes = [vp, C.POINTER(C.c_double * 2)]
     lib.tild_structure_factor.argtypes = [vp, C.c_uint32, vp, i32]
     lib.tild_index_map.argtypes = [vp, vp, vp, vp, vp, vp]
     lib.tild_segment_layout.argtypes = [vp, vp, vp]
@@ -250,6 +252,12 @@ class Tild:
         e = (C.c_double * 3)()
         self._check(self.lib.tild_energy(self.ctx, C.byref(e)), "tild_energy")
         return np.array([e[0], e[1], e[2]])
+
+    def tild_virial(self):
+        """(bonded, non-bonded mesh) pressure virial of the current state as a numpy array; excess pressure = sum / 3V."""
+        w = (C.c_double * 2)()
+        self._check(self.lib.tild_virial(self.ctx, C.byref(w)), "tild_virial")
+        return np.array([w[0], w[1]])
 
     def tild_structure_factor(self, species_mask: int, sk=None):
         """S(m) of the masked species on the half spectrum; pass a previous result as `sk` to accumulate into it."""

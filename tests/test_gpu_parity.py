@@ -773,6 +773,77 @@ def test_euler_maruyama_trajectory_parity(cfg):
     assert np.abs(min_image(gx - ox, cfg.box)).max() > 1e-2
 
 
+@pytest.mark.parametrize("gamma", [1.0, 0.0])
+def test_velocity_verlet_langevin_trajectory_parity(gamma):
+    """TILD_INTEGRATOR_VV (PAPER.md L320, L346-349; reading A24): 100 steps against the oracle's orc_vv_step on the same
+    Philox stream; gamma = 0 is plain velocity Verlet."""
+    cfg = small_cfg(order=4, gamma=gamma)
+    st, eng = make(cfg, integrator=tild.INTEGRATOR_VV, resort_every=6)
+    p = oracle_params(cfg, integrator=2)
+    eng.tild_set_state(dev(st.x), dev(st.v), dev(st.type), dev(st.bond_partner), 0)
+    eng.tild_step(100)
+    x, v, _, step = eng.tild_get_state()
+    ox, ov, _ = orc.run(p, st.x.astype(np.float64), st.v.astype(np.float64), st.type, st.bond_partner, 0, 100)
+    assert step == 100
+    check(f"vv_100_dx_g{gamma}", np.abs(min_image(x.cpu().numpy().astype(np.float64) - ox, cfg.box)).max(), 1e-4)
+    check(f"vv_100_dv_g{gamma}", np.abs(v.cpu().numpy().astype(np.float64) - ov).max(), TOL_DV)
+    # it is a different integrator from GJF: the trajectories differ at O(gamma dt)
+    if gamma > 0:
+        gx, _, _ = orc.run(oracle_params(cfg), st.x.astype(np.float64), st.v.astype(np.float64), st.type, st.bond_partner, 0, 100)
+        assert np.abs(min_image(gx - ox, cfg.box)).max() > 1e-3
+    with pytest.raises(tild.TildError):
+        tild.Tild(tild.params_from_config(cfg, integrator=tild.INTEGRATOR_VV, gamma=500.0))     # gamma dt / 2m >= 1
+
+
+@pytest.mark.parametrize("variant", ["plain", "electrostatics", "rest_length"])
+def test_virial_matches_oracle(variant):
+    """tild_virial (PAPER.md L209; SURVEY 8(f) #3) against the oracle's orc_virial, which is pinned as -dE/dln(lambda)."""
+    kw, okw = {}, {}
+    cfg = small_cfg(order=4)
+    if variant == "electrostatics":
+        cfg = small_cfg(order=3, S=3, grid=(18, 12, 30), box=(9.0, 6.0, 15.0), charge=(1.0, -1.0, 0.0), bjerrum=1.5, a_charge=0.45)
+        kw = dict(flags=tild.FLAG_DECONVOLVE)
+        okw = dict(deconvolve=True)
+    if variant == "rest_length":
+        cfg = small_cfg(order=2, r0_bond=0.6, k_bond=2.0)
+    st, eng = make(cfg, **kw)
+    p = oracle_params(cfg, **okw)
+    eng.tild_set_state(dev(st.x), dev(st.v), dev(st.type), dev(st.bond_partner), 0)
+    w = eng.tild_virial()
+    ow = orc.virial(p, st.x.astype(np.float64), st.type, st.bond_partner)
+    check(f"virial_bond_{variant}", abs(w[0] - ow[0]) / abs(ow[0]), 1e-6)
+    check(f"virial_mesh_{variant}", abs(w[1] - ow[1]) / abs(ow[1]), 2e-5)
+    eng.tild_step(7)
+    x, _, _, _ = eng.tild_get_state(want_v=False)
+    w = eng.tild_virial()
+    ow = orc.virial(p, x.cpu().numpy().astype(np.float64), st.type, st.bond_partner)
+    assert abs(w[0] - ow[0]) <= 1e-6 * abs(ow[0]) and abs(w[1] - ow[1]) <= 2e-5 * abs(ow[1])
+
+
+@pytest.mark.parametrize("P", [2, 4])
+def test_two_dimensional_mode_parity(P):
+    """TILD_FLAG_2D (PAPER.md L54, Listing 1 L65; reading A27): one plane of nodes, forces and 50 steps against the oracle."""
+    cfg = small_cfg(order=P, grid=(24, 20, 1), box=(12.0, 10.0, 1.0), n_chains=60)
+    st = inputs.make_state(cfg)
+    st.v[:, 2] = 0.0
+    eng = tild.Tild(tild.params_from_config(cfg, flags=tild.FLAG_2D, resort_every=5))
+    p = oracle_params(cfg, dim2=True)
+    eng.tild_set_state(dev(st.x), dev(st.v), dev(st.type), dev(st.bond_partner), 0)
+    _, _, f, _ = eng.tild_get_state(want_v=False, want_f=True)
+    of = orc.force(p, st.x.astype(np.float64), st.type, st.bond_partner)
+    f = f.cpu().numpy()
+    assert np.abs(f[:, 2]).max() == 0.0 and np.abs(of[:, 2]).max() == 0.0
+    check(f"dim2_force_P{P}", np.abs(f - of).max() / vec_rms(of), REL)
+    eng.tild_step(50)
+    x, v, _, _ = eng.tild_get_state()
+    ox, ov, _ = orc.run(p, st.x.astype(np.float64), st.v.astype(np.float64), st.type, st.bond_partner, 0, 50, f=of)
+    x = x.cpu().numpy()
+    assert np.array_equal(x[:, 2], st.x[:, 2]) and np.abs(v.cpu().numpy()[:, 2]).max() == 0.0
+    check(f"dim2_50_dx_P{P}", np.abs(min_image(x.astype(np.float64) - ox, cfg.box)).max(), 1e-4)
+    with pytest.raises(tild.TildError):
+        tild.Tild(tild.params_from_config(small_cfg(order=P), flags=tild.FLAG_2D))        # needs grid[2] == 1
+
+
 def test_euler_maruyama_needs_friction():
     cfg = small_cfg(order=2, gamma=0.0)
     with pytest.raises(tild.TildError):
