@@ -69,6 +69,8 @@ typedef enum {
 #define TILD_FLAG_2D 512u          /* two-dimensional system (Listing 1 L65; A27): grid[2] must be 1; the z
                                       coordinates are carried along unchanged, no force, noise or velocity along z.  box[2] is
                                       the thickness that turns the areal density into rho0 = n / V */
+#define TILD_FLAG_EXTRAS 1024u     /* reserve workspace and plans for the extra mesh interactions: per-particle charges
+                                      (tild_set_charges) and the Maier-Saupe interaction (mu_ms, tild_set_ms_partners) */
 #define TILD_FLAG_GEN1_TILES 128u   /* first-generation tile kernels (32 bank classes with overflow rounds, per-particle work
                                       in class order) even where the rotation-class kernels apply (P = 4); for A/B runs */
 
@@ -116,6 +118,9 @@ typedef struct {
     /* harmonic angle potential k_theta (theta_ijk - theta0)^2, Eq. 17, on the same triplets; k_theta = 0:
      * none; theta0 in [0, pi].  The force is singular at sin(theta) = 0 and that term is dropped there */
     double k_theta, theta0;
+    /* Maier-Saupe parameter mu of PAPER.md Eq. 20 L241 (0 = off): beta U = -(mu/rho0) int int S(r) : S(r') u_G(|r - r'|) with the
+     * orientation tensors S_i = u_i u_i - I/3 of the LC centres named by tild_set_ms_partners (A26) */
+    double mu_ms;
 } tild_params;
 
 /* HOST. Bytes of device workspace tild_init needs for these parameters. */
@@ -163,6 +168,20 @@ int tild_get_state(tild_ctx*, float* x, float* v, float* f, uint64_t* step /*HOS
  * lambda (1 + cos theta) and k_theta (theta - theta0)^2 (Eq. 16-17) of every centre bead; e[2] non-bonded on the mesh
  * (1/2V) sum_m u^(k_m) sum_IJ c_IJ Re[n^_I(m) conj(n^_J(m))] (Eq. 3-4).  One force evaluation, no state change. */
 int tild_energy(tild_ctx*, double e[3] /*HOST out*/);
+
+/* Per-particle charges (the electrostatic forces "use the ... charge density field"; A25): q[i] is
+ * the charge of particle i (original numbering).  While set, the charge mesh rho_c = sum_i q_i W(r - r_i) replaces the
+ * charges per species of tild_params.charge in the Coulomb term (bjerrum, a_charge as before; k = 0 dropped).  q = NULL
+ * switches back.  Costs one extra spread, one R2C and three C2R per step.  Needs TILD_FLAG_EXTRAS.  The energies and the
+ * virial of tild_energy / tild_virial do not include this term. */
+int tild_set_charges(tild_ctx*, const float* q /*DEVICE [n] or NULL*/);
+
+/* Maier-Saupe interaction (PAPER.md IV.D L233-247, Eq. 19-20; A26): partner[i] = j names the particle that
+ * defines the orientation u_i = (r_i - r_j)/|r_i - r_j| of LC centre i (-1: i is not a centre), as in the paper's list of
+ * pairs (L245).  Forces: (2 mu/rho0) S_i : grad Phi(r_i) on the centre plus +-(4 mu/rho0)(I - u u) Phi u / |d| on centre and
+ * partner, Phi = u_G * S on the mesh.  NULL switches it off.  Costs 6 spreads, 6 R2C and 24 C2R per step.  Needs
+ * TILD_FLAG_EXTRAS and mu_ms != 0.  Not included in tild_energy / tild_virial. */
+int tild_set_ms_partners(tild_ctx*, const int32_t* partner /*DEVICE [n] or NULL*/);
 
 /* HOST out, synchronises.  Pressure virial of the current state, W = -dU/d ln(lambda) under the affine scaling r -> lambda r,
  * L -> lambda L (excess pressure = W / 3V): w[0] bonds, sum over bonds of -2 k (|d| - r0) |d| (the angle

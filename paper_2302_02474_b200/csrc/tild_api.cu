@@ -174,6 +174,15 @@ void carve(tild_ctx* c, void* base, size_t* total)
     c->d_step = w.take<uint64_t>(2);
     c->d_energy = w.take<double>(8);
     c->tables = w.take<float>(14 * 4096);
+    if (p.flags & TILD_FLAG_EXTRAS) {   // per-particle charges / Maier-Saupe (tild_extra.cu)
+        c->q_id = w.take<float>(n);
+        c->msp_id = w.take<int32_t>(n);
+        c->slot_of_id = w.take<uint32_t>(n);
+        c->Fext = w.take<float4>(n);
+        c->xacc = w.take<float4>(n);
+        c->xr = w.take<float>(4 * M);
+        c->xh = w.take<float2>(5 * Mk);
+    }
     *total = w.off;
 }
 
@@ -236,6 +245,7 @@ int force_current(tild_ctx* c)
     const int a = c->cur;
     int rc = mesh_pipeline(c, c->lay, c->X4[a], nullptr);
     if (rc) return rc;
+    if ((rc = launch_extra_forces(c, c->X4[a], c->W4[a]))) return rc;
     return launch_interp(c, INTERP_TOTAL_BY_SLOT, c->lay, c->ffield, c->X4[a], c->W4[a], c->B[a], nullptr, nullptr, nullptr);
 }
 
@@ -295,6 +305,7 @@ int tild_init(tild_ctx** out, const tild_params* params, void* workspace, size_t
     const double sigma2 = p.sigma2 > 0.0 ? p.sigma2 : 2.0 * p.a * p.a;
     const double rho0 = p.rho0 > 0.0 ? p.rho0 : (p.n > 0 ? (double)p.n / V : 1.0);   // L121; an empty system has no density scale
     c->resort_every = p.resort_every > 0 ? p.resort_every : 10;
+    c->rho0 = rho0;
 
     MeshParams& m = c->mesh;
     m.n = p.n;
@@ -448,6 +459,22 @@ int tild_init(tild_ctx** out, const tild_params* params, void* workspace, size_t
         delete c;
         return TILD_ECUFFT;
     }
+    if (fr == CUFFT_SUCCESS && (p.flags & TILD_FLAG_EXTRAS)) {
+        fr = cufftPlanMany(&c->plan_x_r2c, 3, dims, nullptr, 1, 0, nullptr, 1, 0, CUFFT_R2C, 1);
+        if (fr == CUFFT_SUCCESS) {
+            fr = cufftPlanMany(&c->plan_x_c2r, 3, dims, nullptr, 1, 0, nullptr, 1, 0, CUFFT_C2R, 1);
+            if (fr != CUFFT_SUCCESS) cufftDestroy(c->plan_x_r2c);
+        }
+        if (fr == CUFFT_SUCCESS) {
+            c->xplans_ok = true;
+            cufftSetStream(c->plan_x_r2c, c->stream);
+            cufftSetStream(c->plan_x_c2r, c->stream);
+        } else {
+            drop_plans();
+            delete c;
+            return TILD_ECUFFT;
+        }
+    }
     if ((rc = tild_spread_configure(c)) != TILD_OK || (rc = tild_interp_configure(c)) != TILD_OK ||
         (rc = tild_kspace_configure(c)) != TILD_OK) {
         drop_plans();
@@ -489,6 +516,10 @@ void tild_destroy(tild_ctx* c)
         } else {
             cufftDestroy(c->plan_c2r);
         }
+    }
+    if (c->xplans_ok) {
+        cufftDestroy(c->plan_x_r2c);
+        cufftDestroy(c->plan_x_c2r);
     }
     if (c->graph_ok) cudaGraphExecDestroy(c->graph_exec);
     if (c->ev_ok)
@@ -649,6 +680,7 @@ int enqueue_one_step(tild_ctx* c, cudaEvent_t* ev)
     const int a = c->cur;
     int rc = mesh_pipeline(c, c->lay, c->X4[a], ev);
     if (rc) return rc;
+    if ((rc = launch_extra_forces(c, c->X4[a], c->W4[a]))) return rc;   // per-particle charges / Maier-Saupe -> stp.fext
     rc = launch_interp(c, INTERP_FUSED_STEP, c->lay, c->ffield, c->X4[a], c->W4[a], c->B[a], c->X4[1 - a], c->W4[1 - a], nullptr);
     if (rc) return rc;
     // from here on the state is w = v - (dt/2m) F (Euler-Maruyama never touches the velocities: the state stays v)
@@ -786,6 +818,37 @@ int tild_energy(tild_ctx* c, double e[3])
     if ((rc = launch_energy(c, c->d_energy))) return rc;
     TILD_CUDA(c, cudaMemcpyAsync(e, c->d_energy, 3 * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
     TILD_CUDA(c, cudaStreamSynchronize(c->stream));
+    return TILD_OK;
+}
+
+int tild_set_charges(tild_ctx* c, const float* q)
+{
+    DevGuard dg(c);
+    if (!c) return TILD_EINVAL;
+    if (!c->Fext) return tild_fail(c, TILD_EINVAL, "tild_set_charges needs TILD_FLAG_EXTRAS at tild_init");
+    c->has_q = q != nullptr;
+    c->ksp.has_el = (c->prm.bjerrum > 0.0 && !c->has_q) ? 1 : 0;     // A25: the charge mesh replaces the charges per species
+    if (c->graph_ok) {                                               // a captured block has the old choice baked in
+        cudaGraphExecDestroy(c->graph_exec);
+        c->graph_ok = false;
+    }
+    if (q && c->mesh.n > 0)
+        TILD_CUDA(c, cudaMemcpyAsync(c->q_id, q, sizeof(float) * (size_t)c->mesh.n, cudaMemcpyDeviceToDevice, c->stream));
+    return TILD_OK;
+}
+
+int tild_set_ms_partners(tild_ctx* c, const int32_t* partner)
+{
+    DevGuard dg(c);
+    if (!c) return TILD_EINVAL;
+    if (!c->Fext) return tild_fail(c, TILD_EINVAL, "tild_set_ms_partners needs TILD_FLAG_EXTRAS at tild_init");
+    c->has_ms = partner != nullptr;
+    if (c->graph_ok) {
+        cudaGraphExecDestroy(c->graph_exec);
+        c->graph_ok = false;
+    }
+    if (partner && c->mesh.n > 0)
+        TILD_CUDA(c, cudaMemcpyAsync(c->msp_id, partner, sizeof(int32_t) * (size_t)c->mesh.n, cudaMemcpyDeviceToDevice, c->stream));
     return TILD_OK;
 }
 

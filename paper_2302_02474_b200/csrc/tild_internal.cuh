@@ -80,6 +80,7 @@ struct StepParams {
     float b_dt_over_2m;
     float b_over_m;
     int dim2;              // TILD_FLAG_2D: no force, noise or motion along z (A27)
+    const float4* fext;    // per-slot force of the extra mesh interactions (tild_extra.cu), added to every total force; nullptr = none
     float noise_amp;       // sqrt(2 gamma kT dt); 0 disables the draw
     float k_bond, r0_bond;
     int max_bonds;
@@ -132,6 +133,19 @@ struct tild_ctx {
     uint32_t* scan_part;  // block sums of the scan
     uint32_t* perm;       // [n] tild_index_map scratch
     float* tables;        // k-space tables
+
+    // extra mesh interactions (TILD_FLAG_EXTRAS; tild_extra.cu): per-particle charges and Maier-Saupe partners by particle id
+    float* q_id;          // [n]
+    int32_t* msp_id;      // [n] partner id of every LC centre, -1 = not a centre
+    uint32_t* slot_of_id; // [n], refreshed at every re-sort
+    float4* Fext;         // [n] per-slot extra force
+    float4* xacc;         // [n] Phi u accumulator of the Maier-Saupe orientation force
+    float* xr;            // [4][M] real meshes
+    float2* xh;           // [5][Mk] spectra
+    bool has_q, has_ms;
+    double rho0;
+    cufftHandle plan_x_r2c, plan_x_c2r;   // 3-D, one field
+    bool xplans_ok;
 
     cufftHandle plan_r2c, plan_c2r;   // 3-D, batched over species / force components (plan_c2r only when !xfft_R)
     cufftHandle plan_r2c_yz, plan_c2r_yz;   // 2-D over (y, z), batched over the x planes: used with the fused x-transform
@@ -207,6 +221,9 @@ int launch_make_w(tild_ctx* c, const float4* F4, float4* W4, float sign);   // w
 int launch_velocity_out(tild_ctx* c, const float4* F4, const float4* W4, float* v);  // v[id] = w + (dt/2m) f
 int launch_advance_step(tild_ctx* c);
 int launch_energy(tild_ctx* c, double* d_out);   // tild_energy.cu
+// tild_extra.cu
+int launch_slot_of_id(tild_ctx* c);
+int launch_extra_forces(tild_ctx* c, const float4* X4, const float4* W4);
 int launch_structure_factor(tild_ctx* c, uint32_t mask, float* sk, int accumulate);  // c->nhat must be current
 int launch_philox_test(tild_ctx* c, const uint32_t* ctr, const uint32_t* key, uint32_t* out, float* gauss, int m);
 

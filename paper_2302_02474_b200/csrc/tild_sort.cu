@@ -345,7 +345,7 @@ int launch_reorder(tild_ctx* c)
         TILD_LAUNCH_CHECK(c, "move_state_kernel");
     }
     c->cur = b;
-    return TILD_OK;
+    return launch_slot_of_id(c);   // id -> slot map of the extra mesh interactions (no-op without TILD_FLAG_EXTRAS)
 }
 
 int launch_unpermute(tild_ctx* c, const float4* src, float* dst)

@@ -24,11 +24,12 @@ FLAG_PLAIN_FFT = 64
 FLAG_GEN1_TILES = 128
 FLAG_EAGER = 256
 FLAG_2D = 512
+FLAG_EXTRAS = 1024
 TIMING_NAMES = ("sort", "spread", "fft_fwd", "kspace", "fft_inv", "interp", "other", "total")
 
 EXPORTS = (
     "tild_workspace_bytes", "tild_init", "tild_set_state", "tild_spread", "tild_kspace_force", "tild_interp",
-    "tild_bond_force", "tild_step", "tild_get_state", "tild_energy", "tild_virial", "tild_structure_factor", "tild_index_map", "tild_get_timings", "tild_run_host",
+    "tild_bond_force", "tild_step", "tild_get_state", "tild_energy", "tild_virial", "tild_set_charges", "tild_set_ms_partners", "tild_structure_factor", "tild_index_map", "tild_get_timings", "tild_run_host",
     "tild_philox_test", "tild_layout_info", "tild_segment_layout", "tild_launch_count", "tild_last_error", "tild_destroy", "tild_version",
 )
 
@@ -50,6 +51,7 @@ class Params(C.Structure):
         ("lambda_wlc", C.c_double),
         ("k_theta", C.c_double),
         ("theta0", C.c_double),
+        ("mu_ms", C.c_double),
     ]
 
 
@@ -58,7 +60,7 @@ def make_params(n: int, n_species: int, box: Sequence[float], grid: Sequence[int
                 max_bonds: int = 2, dt: float = 0.005, gamma: float = 1.0, kT: float = 1.0, mass: float = 1.0,
                 seed: int = 0, resort_every: int = 0, flags: int = 0, integrator: int = 0,
                 charge: Sequence[float] = (), bjerrum: float = 0.0, a_charge: float = 0.5,
-                lambda_wlc: float = 0.0, k_theta: float = 0.0, theta0: float = 0.0, tile_shape: int = 0) -> Params:
+                lambda_wlc: float = 0.0, k_theta: float = 0.0, theta0: float = 0.0, tile_shape: int = 0, mu_ms: float = 0.0) -> Params:
     p = Params()
     p.struct_size = C.sizeof(Params)
     p.n, p.n_species, p.order = int(n), int(n_species), int(order)
@@ -81,6 +83,7 @@ def make_params(n: int, n_species: int, box: Sequence[float], grid: Sequence[int
     p.bjerrum, p.a_charge = float(bjerrum), float(a_charge)
     p.lambda_wlc = float(lambda_wlc)
     p.k_theta, p.theta0 = float(k_theta), float(theta0)
+    p.mu_ms = float(mu_ms)
     return p
 
 
@@ -120,6 +123,8 @@ def load():
     lib.tild_get_state.argtypes = [vp, vp, vp, vp, C.POINTER(u64)]
     lib.tild_energy.argtypes = [vp, C.POINTER(C.c_double * 3)]
     lib.tild_virial.argtypes = [vp, C.POINTER(C.c_double * 2)]
+    lib.tild_set_charges.argtypes = [vp, vp]
+    lib.tild_set_ms_partners.argtypes = [vp, vp]
     lib.tild_structure_factor.argtypes = [vp, C.c_uint32, vp, i32]
     lib.tild_index_map.argtypes = [vp, vp, vp, vp, vp, vp]
     lib.tild_segment_layout.argtypes = [vp, vp, vp]
@@ -252,6 +257,14 @@ class Tild:
         e = (C.c_double * 3)()
         self._check(self.lib.tild_energy(self.ctx, C.byref(e)), "tild_energy")
         return np.array([e[0], e[1], e[2]])
+
+    def tild_set_charges(self, q=None):
+        """Per-particle charges (float32 [n], original numbering) or None to go back to the charges per species."""
+        self._check(self.lib.tild_set_charges(self.ctx, _dp(q) if q is not None else None), "tild_set_charges")
+
+    def tild_set_ms_partners(self, partner=None):
+        """Maier-Saupe orientation partners (int32 [n], -1 = not an LC centre) or None to switch the interaction off."""
+        self._check(self.lib.tild_set_ms_partners(self.ctx, _dp(partner) if partner is not None else None), "tild_set_ms_partners")
 
     def tild_virial(self):
         """(bonded, non-bonded mesh) pressure virial of the current state as a numpy array; excess pressure = sum / 3V."""

@@ -972,6 +972,62 @@ def test_harmonic_angle_potential_parity():
     assert np.abs(min_image(x - ox, cfg.box)).max() <= 1e-4
 
 
+def test_per_particle_charges_parity():
+    """tild_set_charges (reading A25): arbitrary charges per particle on an extra charge mesh, force and
+    40 steps against the oracle (pinned against an Ewald sum with arbitrary charges); switching back restores the
+    charges per species."""
+    cfg = small_cfg(order=4, bjerrum=1.2, a_charge=0.5, charge=(1.0, -1.0))
+    st = inputs.make_state(cfg)
+    q = np.random.default_rng(5).normal(size=cfg.n).astype(np.float32)
+    q[::3] = 0.0
+    eng = tild.Tild(tild.params_from_config(cfg, flags=tild.FLAG_EXTRAS, resort_every=7))
+    eng.tild_set_charges(dev(q))
+    eng.tild_set_state(dev(st.x), dev(st.v), dev(st.type), dev(st.bond_partner), 0)
+    p = oracle_params(cfg, q_pp=q.astype(np.float64))
+    _, _, f, _ = eng.tild_get_state(want_v=False, want_f=True)
+    of = orc.force(p, st.x.astype(np.float64), st.type, st.bond_partner)
+    check("pp_charge_force", np.abs(f.cpu().numpy() - of).max() / vec_rms(of), REL)
+    plain = orc.force(oracle_params(cfg), st.x.astype(np.float64), st.type, st.bond_partner)
+    assert np.abs(of - plain).max() > 0.05 * vec_rms(plain)                      # the charges really differ
+    eng.tild_step(40)
+    x, _, _, _ = eng.tild_get_state(want_v=False)
+    ox, _, _ = orc.run(p, st.x.astype(np.float64), st.v.astype(np.float64), st.type, st.bond_partner, 0, 40, f=of)
+    check("pp_charge_40_dx", np.abs(min_image(x.cpu().numpy().astype(np.float64) - ox, cfg.box)).max(), 1e-4)
+    eng.tild_set_charges(None)
+    eng.tild_set_state(dev(st.x), dev(st.v), dev(st.type), dev(st.bond_partner), 0)
+    _, _, f, _ = eng.tild_get_state(want_v=False, want_f=True)
+    assert np.abs(f.cpu().numpy() - plain).max() <= REL * vec_rms(plain)
+    with pytest.raises(tild.TildError):
+        tild.Tild(tild.params_from_config(cfg)).tild_set_charges(dev(q))          # needs TILD_FLAG_EXTRAS
+
+
+@pytest.mark.parametrize("P", [3, 4])
+def test_maier_saupe_parity(P):
+    """Maier-Saupe interaction (Eq. 19-20; reading A26): every second bead of a chain is an LC centre
+    oriented along the bond to its next bead; force and 40 steps against the oracle (whose orientation force is pinned as
+    the exact energy gradient and whose pair energy against the continuum expression)."""
+    cfg = small_cfg(order=P)
+    st = inputs.make_state(cfg)
+    msp = -np.ones(cfg.n, dtype=np.int32)
+    has_next = st.bond_partner[:, 1] >= 0
+    centres = np.where(has_next)[0][::2]
+    msp[centres] = st.bond_partner[centres, 1]
+    mu = 2.5
+    eng = tild.Tild(tild.params_from_config(cfg, flags=tild.FLAG_EXTRAS, resort_every=6, mu_ms=mu))
+    eng.tild_set_ms_partners(dev(msp))
+    eng.tild_set_state(dev(st.x), dev(st.v), dev(st.type), dev(st.bond_partner), 0)
+    p = oracle_params(cfg, mu_ms=mu, ms_partner=msp)
+    _, _, f, _ = eng.tild_get_state(want_v=False, want_f=True)
+    of = orc.force(p, st.x.astype(np.float64), st.type, st.bond_partner)
+    plain = orc.force(oracle_params(cfg), st.x.astype(np.float64), st.type, st.bond_partner)
+    assert np.abs(of - plain).max() > 0.05 * vec_rms(plain)                      # the interaction really acts
+    check(f"ms_force_P{P}", np.abs(f.cpu().numpy() - of).max() / vec_rms(of), REL)
+    eng.tild_step(40)
+    x, _, _, _ = eng.tild_get_state(want_v=False)
+    ox, _, _ = orc.run(p, st.x.astype(np.float64), st.v.astype(np.float64), st.type, st.bond_partner, 0, 40, f=of)
+    check(f"ms_40_dx_P{P}", np.abs(min_image(x.cpu().numpy().astype(np.float64) - ox, cfg.box)).max(), 1e-4)
+
+
 def test_wlc_needs_linear_chain_tables():
     cfg = small_cfg(order=2)
     with pytest.raises(tild.TildError):
