@@ -246,7 +246,8 @@ int force_current(tild_ctx* c)
     int rc = mesh_pipeline(c, c->lay, c->X4[a], nullptr);
     if (rc) return rc;
     if ((rc = launch_extra_forces(c, c->X4[a], c->W4[a]))) return rc;
-    return launch_interp(c, INTERP_TOTAL_BY_SLOT, c->lay, c->ffield, c->X4[a], c->W4[a], c->B[a], nullptr, nullptr, nullptr);
+    if ((rc = launch_interp(c, INTERP_TOTAL_BY_SLOT, c->lay, c->ffield, c->X4[a], c->W4[a], c->B[a], nullptr, nullptr, nullptr))) return rc;
+    return launch_extra_apply(c, 1, 0.0f, nullptr, nullptr);
 }
 
 // caller (x, type) -> segment-sorted copy in c->SX4 described by c->lay_stage; c->inv maps id -> slot
@@ -680,9 +681,10 @@ int enqueue_one_step(tild_ctx* c, cudaEvent_t* ev)
     const int a = c->cur;
     int rc = mesh_pipeline(c, c->lay, c->X4[a], ev);
     if (rc) return rc;
-    if ((rc = launch_extra_forces(c, c->X4[a], c->W4[a]))) return rc;   // per-particle charges / Maier-Saupe -> stp.fext
+    if ((rc = launch_extra_forces(c, c->X4[a], c->W4[a]))) return rc;   // per-particle charges / Maier-Saupe -> Fext
     rc = launch_interp(c, INTERP_FUSED_STEP, c->lay, c->ffield, c->X4[a], c->W4[a], c->B[a], c->X4[1 - a], c->W4[1 - a], nullptr);
     if (rc) return rc;
+    if ((rc = launch_extra_apply(c, 2, c->stp.kick_in, c->X4[1 - a], c->W4[1 - a]))) return rc;
     // from here on the state is w = v - (dt/2m) F (Euler-Maruyama never touches the velocities: the state stays v)
     c->stp.kick_in = c->stp.integrator == TILD_INTEGRATOR_EM ? 0.0f : c->stp.half_dt_over_m;
     if (!c->step_advanced && (rc = launch_advance_step(c))) return rc;   // per-particle path: no drift kernel to do it

@@ -1,9 +1,9 @@
 // Extra mesh interactions that ride on the particle-mesh path (SURVEY 8(f) #1 remainder and #4): per-particle charges
 // (reading A25) and the Maier-Saupe orientation interaction (PAPER.md IV.D L233-247, Eq. 19-20, reading
 // A26).  Both spread a per-particle quantity with the density weights, multiply by a kernel in k-space and interpolate a
-// field (and its ik-gradient) back with the same weights.  They write a per-slot force Fext that the fused
-// interpolation pass adds to the force of every particle (StepParams::fext), so the hot path is untouched when they are
-// off.  These are not the headline kernels: one thread per particle, global fp32 reductions and gathers, 3-D cuFFT plans.
+// field (and its ik-gradient) back with the same weights.  They write a per-slot force Fext; because the fused
+// pass is linear in the force, its effect is added to the outputs of that pass by a small kernel afterwards
+// (extra_apply_kernel), so the hot kernels are untouched.  These are not the headline kernels: one thread per particle, global fp32 reductions and gathers, 3-D cuFFT plans.
 #include "tild_particle.cuh"
 
 namespace {
@@ -182,6 +182,41 @@ __global__ void __launch_bounds__(XT) ms_orient_kernel(MeshParams m, float pref,
     }
 }
 
+// The fused pass is linear in the force: r' = r + b_dt v + b_dt2_over_2m F + ..., w' = a_g (v + w_fr F) + ..., v = w + kick_in F.
+// An extra force dF therefore moves its outputs by dr = (b_dt kick_in + b_dt2_over_2m) dF and dw' = a_g (kick_in + w_fr) dF
+// (Euler-Maruyama: dr = (dt/gamma) dF), which this kernel applies after the pass -- the hot kernels carry no branch for it.
+__global__ void __launch_bounds__(XT) extra_apply_kernel(MeshParams m, StepParams s, int mode, float kick_in, const float4* __restrict__ Fext,
+                                                         float4* __restrict__ F4, float4* __restrict__ X4o, float4* __restrict__ W4o)
+{
+    const size_t slot = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (slot >= (size_t)m.n) return;
+    float4 e = Fext[slot];
+    if (s.dim2) e.z = 0.0f;
+    if (mode == 1) {
+        float4 f = F4[slot];
+        f.x += e.x;
+        f.y += e.y;
+        f.z += e.z;
+        F4[slot] = f;
+        return;
+    }
+    const bool em = s.integrator == TILD_INTEGRATOR_EM;
+    const float cr = em ? s.em_drift : s.b_dt * kick_in + s.b_dt2_over_2m;
+    float4 x = X4o[slot];
+    x.x = wrap_pos(x.x + cr * e.x, m.L[0], m.inv_L[0]);
+    x.y = wrap_pos(x.y + cr * e.y, m.L[1], m.inv_L[1]);
+    if (!s.dim2) x.z = wrap_pos(x.z + cr * e.z, m.L[2], m.inv_L[2]);
+    X4o[slot] = x;
+    if (!em) {
+        const float cw = s.a_g * (kick_in + s.w_fr);
+        float4 w = W4o[slot];
+        w.x += cw * e.x;
+        w.y += cw * e.y;
+        w.z += cw * e.z;
+        W4o[slot] = w;
+    }
+}
+
 __global__ void __launch_bounds__(XT) slot_of_id_kernel(int n, const float4* __restrict__ W4, uint32_t* __restrict__ slot_of_id)
 {
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
@@ -244,12 +279,12 @@ static int extra_forces_p(tild_ctx* c, const float4* X4, const float4* W4)
     return TILD_OK;
 }
 
-// Fext[slot] = force of the extra mesh interactions at the positions X4 (slot order W4); sets c->stp.fext for the fused pass
+// Fext[slot] = force of the extra mesh interactions at the positions X4 (slot order W4)
 int launch_extra_forces(tild_ctx* c, const float4* X4, const float4* W4)
 {
     const bool active = c->Fext && ((c->has_q && c->prm.bjerrum > 0.0) || (c->has_ms && c->prm.mu_ms != 0.0));
-    c->stp.fext = active ? c->Fext : nullptr;
-    if (!active || c->mesh.n == 0) return TILD_OK;
+    c->x_active = active && c->mesh.n > 0;
+    if (!c->x_active) return TILD_OK;
     switch (c->mesh.P) {
     case 1: return extra_forces_p<1>(c, X4, W4);
     case 2: return extra_forces_p<2>(c, X4, W4);
@@ -257,4 +292,13 @@ int launch_extra_forces(tild_ctx* c, const float4* X4, const float4* W4)
     case 4: return extra_forces_p<4>(c, X4, W4);
     default: return extra_forces_p<5>(c, X4, W4);
     }
+}
+
+int launch_extra_apply(tild_ctx* c, int mode, float kick_in, float4* X4o, float4* W4o)
+{
+    if (!c->x_active) return TILD_OK;
+    const int n = c->mesh.n;
+    extra_apply_kernel<<<(n + XT - 1) / XT, XT, 0, c->stream>>>(c->mesh, c->stp, mode, kick_in, c->Fext, c->F4, X4o, W4o);
+    TILD_LAUNCH_CHECK(c, "extra_apply_kernel");
+    return TILD_OK;
 }

@@ -80,7 +80,6 @@ struct StepParams {
     float b_dt_over_2m;
     float b_over_m;
     int dim2;              // TILD_FLAG_2D: no force, noise or motion along z (A27)
-    const float4* fext;    // per-slot force of the extra mesh interactions (tild_extra.cu), added to every total force; nullptr = none
     float noise_amp;       // sqrt(2 gamma kT dt); 0 disables the draw
     float k_bond, r0_bond;
     int max_bonds;
@@ -142,7 +141,7 @@ struct tild_ctx {
     float4* xacc;         // [n] Phi u accumulator of the Maier-Saupe orientation force
     float* xr;            // [4][M] real meshes
     float2* xh;           // [5][Mk] spectra
-    bool has_q, has_ms;
+    bool has_q, has_ms, x_active;   // x_active: the last launch_extra_forces filled Fext
     double rho0;
     cufftHandle plan_x_r2c, plan_x_c2r;   // 3-D, one field
     bool xplans_ok;
@@ -224,6 +223,8 @@ int launch_energy(tild_ctx* c, double* d_out);   // tild_energy.cu
 // tild_extra.cu
 int launch_slot_of_id(tild_ctx* c);
 int launch_extra_forces(tild_ctx* c, const float4* X4, const float4* W4);
+// adds the effect of Fext to what launch_interp produced: mode 1 the per-slot force F4, mode 2 the new state (X4o, W4o)
+int launch_extra_apply(tild_ctx* c, int mode, float kick_in, float4* X4o, float4* W4o);
 int launch_structure_factor(tild_ctx* c, uint32_t mask, float* sk, int accumulate);  // c->nhat must be current
 int launch_philox_test(tild_ctx* c, const uint32_t* ctr, const uint32_t* key, uint32_t* out, float* gauss, int m);
 

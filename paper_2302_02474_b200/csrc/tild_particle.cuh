@@ -160,12 +160,6 @@ __device__ __forceinline__ void finish_update(const MeshParams& m, const StepPar
                                               float4* __restrict__ W4o, float4* __restrict__ F4)
 {
     float3 F = Fin;
-    if (MODE >= 1 && s.fext) {                   // per-particle charges / Maier-Saupe (tild_extra.cu), when they are on
-        const float4 e = s.fext[slot];
-        F.x += e.x;
-        F.y += e.y;
-        F.z += e.z;
-    }
     if (s.dim2) F.z = 0.0f;                      // A27: two-dimensional system, nothing acts or moves along z
     if (MODE <= 1) {
         F4[slot] = make_float4(F.x, F.y, F.z, 0.f);
