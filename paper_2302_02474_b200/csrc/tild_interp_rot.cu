@@ -71,8 +71,11 @@ __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commi
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;\n" ::: "memory"); }
 
 // Dynamic shared memory: image float[3][REX][EY][EZ] of one species | ent u32[3][RSLOTS].
-template <int EY, int EZ, int MODE>
-__global__ void __launch_bounds__(RT, TILD_ROT_CTAS) interp_rot_kernel(MeshParams m, TileParams tp, StepParams s, const uint64_t* __restrict__ step_ptr,
+// FAST (MODE 2 only): the plain model of BASELINE configs -- two bond slots, no rest length, no angle potentials, three
+// dimensions, an inertial integrator.  The fields that select the other paths become compile-time constants, which removes
+// their (never taken, but scheduling-relevant) branches from the hot kernel.
+template <int EY, int EZ, int MODE, bool FAST>
+__global__ void __launch_bounds__(RT, TILD_ROT_CTAS) interp_rot_kernel(MeshParams m, TileParams tp, StepParams s_in, const uint64_t* __restrict__ step_ptr,
                                                           const uint32_t* __restrict__ seg_base, const float* __restrict__ ffield,
                                                           const float4* __restrict__ X4, const float4* __restrict__ W4,
                                                           const int32_t* __restrict__ B, float4* __restrict__ X4o,
@@ -81,6 +84,16 @@ __global__ void __launch_bounds__(RT, TILD_ROT_CTAS) interp_rot_kernel(MeshParam
 {
     constexpr int P = 4, CS = REX * EY * EZ;
     static_assert(EZ % 32 == 8 || EZ % 32 == 24, "row rotation needs the P rows of a stencil to tile the 32 banks");
+    static_assert(!FAST || MODE == 2, "FAST is a specialisation of the fused step");
+    StepParams s = s_in;
+    if (FAST) {
+        s.max_bonds = 2;
+        s.r0_bond = 0.0f;
+        s.lambda_wlc = 0.0f;
+        s.k_theta = 0.0f;
+        s.dim2 = 0;
+        s.integrator = TILD_INTEGRATOR_GJF;     // GJF and VV + Langevin share one code path (coefficients differ)
+    }
     extern __shared__ __align__(16) float fs[];
     __shared__ int goff_x[16], goff_y[32];
     __shared__ uint32_t gcnt[8], ndrift, drift_base, dl[RDCAP];
@@ -216,8 +229,9 @@ __global__ void __launch_bounds__(RT, TILD_ROT_CTAS) interp_rot_kernel(MeshParam
         for (int j = 0; j < RPT; ++j) {
             if (myslot[j] < 0) continue;
             if (MODE == 2) wj[j] = W4[(size_t)c0 + threadIdx.x + j * RT];
-            if (!(TILD_ROT_ABL & 4) && ba[j].x >= 0) q0[j] = X4[ba[j].x];
-            if (!(TILD_ROT_ABL & 4) && ba[j].y >= 0) q1[j] = X4[ba[j].y];
+            // a missing partner reads the particle itself: zero separation, zero bond force, no branch in the tail
+            q0[j] = X4[ba[j].x >= 0 ? (size_t)ba[j].x : (size_t)c0 + threadIdx.x + j * RT];
+            q1[j] = X4[ba[j].y >= 0 ? (size_t)ba[j].y : (size_t)c0 + threadIdx.x + j * RT];
         }
         {   // L2 prefetch of the next chunk's lines (positions, partners, velocity state)
             const size_t nx = (size_t)c0 + nchunk + 8 * (size_t)threadIdx.x;
@@ -326,8 +340,8 @@ __global__ void __launch_bounds__(RT, TILD_ROT_CTAS) interp_rot_kernel(MeshParam
                 const float4 p = pa[j];
                 if (MODE >= 1) {
                     if (s.max_bonds <= 2) {
-                        if (ba[j].x >= 0) bond_term(m, s, p, q0[j], F);
-                        if (ba[j].y >= 0) bond_term(m, s, p, q1[j], F);
+                        bond_term(m, s, p, q0[j], F);
+                        bond_term(m, s, p, q1[j], F);
                         if (s.lambda_wlc != 0.0f || s.k_theta != 0.0f) angle_force_slots(m, s, X4, B, slot, p, F);
                     } else {
                         const float3 fb = bond_force_slots(m, s, X4, B, slot, p);
@@ -357,10 +371,10 @@ __global__ void __launch_bounds__(RT, TILD_ROT_CTAS) interp_rot_kernel(MeshParam
     if (threadIdx.x < nd) drift_list[drift_base + threadIdx.x] = dl[threadIdx.x];
 }
 
-template <int EY, int EZ, int MODE>
+template <int EY, int EZ, int MODE, bool FAST>
 cudaError_t rot_launch(const InterpArgs& a, cudaStream_t st, size_t smem, bool configure_only)
 {
-    auto kernel = interp_rot_kernel<EY, EZ, MODE>;
+    auto kernel = interp_rot_kernel<EY, EZ, MODE, FAST>;
     if (configure_only) return tild_raise_smem_limit(reinterpret_cast<const void*>(kernel), smem);
     kernel<<<a.tp.ntiles, RT, smem, st>>>(a.m, a.tp, a.s, a.step_ptr, a.seg_base, a.ffield, a.X4, a.W4, a.B, a.X4o, a.W4o, a.F4,
                                           a.drift_list, a.drift_count);
@@ -369,10 +383,14 @@ cudaError_t rot_launch(const InterpArgs& a, cudaStream_t st, size_t smem, bool c
 template <int EY, int EZ>
 cudaError_t rot_launch_m(const InterpArgs& a, int mode, cudaStream_t st, size_t smem, bool cfg)
 {
+    const StepParams& s = a.s;
+    const bool fast = s.max_bonds == 2 && s.r0_bond == 0.0f && s.lambda_wlc == 0.0f && s.k_theta == 0.0f && !s.dim2 &&
+                      s.integrator != TILD_INTEGRATOR_EM;
     cudaError_t e = cudaSuccess, e2;
-    if (cfg || mode == 0) { e2 = rot_launch<EY, EZ, 0>(a, st, smem, cfg); if (e2 != cudaSuccess) e = e2; }
-    if (cfg || mode == 1) { e2 = rot_launch<EY, EZ, 1>(a, st, smem, cfg); if (e2 != cudaSuccess) e = e2; }
-    if (cfg || mode == 2) { e2 = rot_launch<EY, EZ, 2>(a, st, smem, cfg); if (e2 != cudaSuccess) e = e2; }
+    if (cfg || mode == 0) { e2 = rot_launch<EY, EZ, 0, false>(a, st, smem, cfg); if (e2 != cudaSuccess) e = e2; }
+    if (cfg || mode == 1) { e2 = rot_launch<EY, EZ, 1, false>(a, st, smem, cfg); if (e2 != cudaSuccess) e = e2; }
+    if (cfg || (mode == 2 && !fast)) { e2 = rot_launch<EY, EZ, 2, false>(a, st, smem, cfg); if (e2 != cudaSuccess) e = e2; }
+    if (cfg || (mode == 2 && fast)) { e2 = rot_launch<EY, EZ, 2, true>(a, st, smem, cfg); if (e2 != cudaSuccess) e = e2; }
     return e;
 }
 
