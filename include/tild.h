@@ -71,6 +71,7 @@ typedef enum {
                                       the thickness that turns the areal density into rho0 = n / V */
 #define TILD_FLAG_EXTRAS 1024u     /* reserve workspace and plans for the extra mesh interactions: per-particle charges
                                       (tild_set_charges) and the Maier-Saupe interaction (mu_ms, tild_set_ms_partners) */
+#define TILD_FLAG_NO_TMA 2048u     /* stage every tile image with cp.async, also where a TMA box applies (A/B runs) */
 #define TILD_FLAG_GEN1_TILES 128u   /* first-generation tile kernels (32 bank classes with overflow rounds, per-particle work
                                       in class order) even where the rotation-class kernels apply (P = 4); for A/B runs */
 

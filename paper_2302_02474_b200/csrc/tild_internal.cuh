@@ -152,6 +152,9 @@ struct tild_ctx {
     const float2* xtw;    // exp(-2 pi i j / Nx), j < Nx
     bool plans_ok;
 
+    alignas(64) unsigned char fmap[128];   // CUtensorMap of c->ffield with the image box of the rotation-class kernel
+    bool tma_ok;
+
     bool has_state;
     bool step_advanced;   // the last launch_interp advanced the device step counter itself (tile path)
     uint64_t step;
@@ -244,12 +247,15 @@ struct InterpArgs {
     uint32_t* drift_list;
     uint32_t* drift_count;   // [0] entries of drift_list, [1] blocks of the drift kernel that are done
     uint64_t* step_adv;      // device step counter, advanced by the last block of the drift kernel in the fused step
+    const void* fmap;        // CUtensorMap of the force field (tild_interp_rot.cu) when use_tma
+    int use_tma;
 };
 // tild_spread_rot.cu: the P = 4 rotation-class spread kernel
 bool spread_rot_applies(const tild_ctx* c);
 cudaError_t spread_rot_run(const tild_ctx* c, const uint32_t* seg_base, const float4* X4, float* grid, bool configure_only);
 // tild_interp_rot.cu: the P = 4 rotation-class tile kernel
 bool interp_rot_applies(const tild_ctx* c);
+bool interp_rot_make_tmap(tild_ctx* c);
 size_t interp_rot_smem(int ey, int ez);
 cudaError_t interp_rot_run(const InterpArgs& a, int mode, cudaStream_t st, bool configure_only);
 

@@ -468,6 +468,7 @@ int tild_interp_configure(tild_ctx* c)
     a.tp = c->tile;
     cudaError_t e = cudaSuccess;
     if (interp_rot_applies(c)) {
+        interp_rot_make_tmap(c);
         e = interp_rot_run(a, 0, c->stream, true);
         if (e != cudaSuccess)
             return tild_fail(c, TILD_ECUDA, "cudaFuncSetAttribute(interp_rot_kernel): %s", cudaGetErrorString(e));
@@ -484,7 +485,8 @@ int launch_interp(tild_ctx* c, int mode, const SegLayout& lay, const float* ffie
 {
     const size_t n = (size_t)c->mesh.n;
     if (n == 0) return TILD_OK;
-    InterpArgs a{c->mesh, c->tile, c->stp, c->d_step, lay.seg_base, ffield, X4, W4, B, X4o, W4o, c->F4, c->rank, c->drift_count, c->d_step};
+    InterpArgs a{c->mesh, c->tile, c->stp, c->d_step, lay.seg_base, ffield, X4, W4, B, X4o, W4o, c->F4, c->rank, c->drift_count, c->d_step,
+                 c->fmap, (c->tma_ok && ffield == c->ffield) ? 1 : 0};   // the tensor map describes the library's own field
     c->step_advanced = false;
     if (c->tile.enabled && c->mesh.P >= 2 && !(c->prm.flags & TILD_FLAG_NAIVE_INTERP)) {   // P = 1: one node per particle
         cudaError_t e = cudaSuccess;

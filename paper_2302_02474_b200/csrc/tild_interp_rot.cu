@@ -22,6 +22,8 @@
 //    7 % slower (0.695 vs 0.650 ms) and is kept behind TILD_USE_FFMA2.
 //  * Software pipeline over the chunks of a tile: the next chunk's positions and partners are loaded while this
 //    chunk's tail computes; this chunk's velocity state and partner positions are loaded before its rounds.
+#include <cuda.h>   // CUtensorMap (types only: the encoder is fetched with cudaGetDriverEntryPoint, libcuda is not linked)
+
 #include "tild_particle.cuh"
 
 namespace {
@@ -70,7 +72,33 @@ __device__ __forceinline__ void cp_async_16(float* smem_dst, const float* gsrc)
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;\n" ::: "memory"); }
 
-// Dynamic shared memory: image float[3][REX][EY][EZ] of one species | ent u32[3][RSLOTS].
+// ---- TMA (cp.async.bulk.tensor) staging of a tile image, for tiles whose image does not cross the periodic boundary ------
+__device__ __forceinline__ void mbar_init(uint64_t* bar, unsigned count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, unsigned bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, unsigned parity)
+{
+    const unsigned a = (unsigned)__cvta_generic_to_shared(bar);
+    unsigned done = 0;
+    while (!done)
+        asm volatile("{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\nselp.u32 %0, 1, 0, p;\n}" : "=r"(done) : "r"(a), "r"(parity) : "memory");
+}
+// one box {EZ, EY, REX, 1} of the 4-D field [3S][Nx][Ny][Nz] -> dense image of one component
+__device__ __forceinline__ void tma_load_box(float* smem_dst, const CUtensorMap* map, int z, int y, int x, int f, uint64_t* bar)
+{
+    asm volatile("cp.async.bulk.tensor.4d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];" ::
+                     "r"((unsigned)__cvta_generic_to_shared(smem_dst)), "l"(map), "r"(z), "r"(y), "r"(x), "r"(f),
+                 "r"((unsigned)__cvta_generic_to_shared(bar))
+                 : "memory");
+}
+
+// Dynamic shared memory: (128-byte aligned) image float[3][CSP] of one species, CSP = REX EY EZ rounded up to 32 words so that
+// every component starts on a 128-byte boundary (TMA destination) | ent u32[3][RSLOTS].
 // FAST (MODE 2 only): the plain model of BASELINE configs -- two bond slots, no rest length, no angle potentials, three
 // dimensions, an inertial integrator.  The fields that select the other paths become compile-time constants, which removes
 // their (never taken, but scheduling-relevant) branches from the hot kernel.
@@ -80,9 +108,10 @@ __global__ void __launch_bounds__(RT, TILD_ROT_CTAS) interp_rot_kernel(MeshParam
                                                           const float4* __restrict__ X4, const float4* __restrict__ W4,
                                                           const int32_t* __restrict__ B, float4* __restrict__ X4o,
                                                           float4* __restrict__ W4o, float4* __restrict__ F4,
-                                                          uint32_t* __restrict__ drift_list, uint32_t* __restrict__ drift_count)
+                                                          uint32_t* __restrict__ drift_list, uint32_t* __restrict__ drift_count,
+                                                          const __grid_constant__ CUtensorMap fmap, int use_tma)
 {
-    constexpr int P = 4, CS = REX * EY * EZ;
+    constexpr int P = 4, CS = (REX * EY * EZ + 31) / 32 * 32;
     static_assert(EZ % 32 == 8 || EZ % 32 == 24, "row rotation needs the P rows of a stencil to tile the 32 banks");
     static_assert(!FAST || MODE == 2, "FAST is a specialisation of the fused step");
     StepParams s = s_in;
@@ -94,9 +123,11 @@ __global__ void __launch_bounds__(RT, TILD_ROT_CTAS) interp_rot_kernel(MeshParam
         s.dim2 = 0;
         s.integrator = TILD_INTEGRATOR_GJF;     // GJF and VV + Langevin share one code path (coefficients differ)
     }
-    extern __shared__ __align__(16) float fs[];
+    extern __shared__ __align__(16) float fs_raw[];
+    float* fs = reinterpret_cast<float*>((reinterpret_cast<uintptr_t>(fs_raw) + 127) & ~(uintptr_t)127);
     __shared__ int goff_x[16], goff_y[32];
     __shared__ uint32_t gcnt[8], ndrift, drift_base, dl[RDCAP];
+    __shared__ __align__(8) uint64_t mbar;
     uint32_t* ent = reinterpret_cast<uint32_t*>(fs + 3 * CS);
     const uint64_t step_next = *step_ptr + 1;   // the step being produced (device-side counter: graph replays see it move)
     const int tile = blockIdx.x;
@@ -109,11 +140,28 @@ __global__ void __launch_bounds__(RT, TILD_ROT_CTAS) interp_rot_kernel(MeshParam
     else if (threadIdx.x >= 32 && threadIdx.x < 32 + EY) goff_y[threadIdx.x - 32] = wrap_idx(o[1] + threadIdx.x - 32, m.N[1]);
     if (threadIdx.x >= 64 && threadIdx.x < 72) gcnt[threadIdx.x - 64] = 0u;
     if (threadIdx.x == 72) ndrift = 0u;
+    // TMA staging when the whole image lies inside the mesh (61 % of the tiles at 256^3): one box per component, issued by
+    // one thread, completion on an mbarrier; the other tiles wrap per row with cp.async below
+    const bool tma_tile = use_tma && o[0] >= 0 && o[0] + REX <= m.N[0] && o[1] >= 0 && o[1] + EY <= m.N[1] && o[2] >= 0 && o[2] + EZ <= m.N[2];
+    unsigned tma_parity = 0;
+    if (tma_tile && threadIdx.x == 0) {
+        mbar_init(&mbar, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     const bool vec16 = (m.N[2] % 4 == 0) && ((reinterpret_cast<uintptr_t>(ffield) & 15) == 0);
 
     auto stage = [&](int sp) {   // three components of species sp -> image (periodic wrap per row); asynchronous
         if (TILD_ROT_ABL & 1) return;
+        if (tma_tile) {
+            if (threadIdx.x == 0) {
+                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // the image was read through the generic proxy
+                mbar_expect_tx(&mbar, 3u * REX * EY * EZ * (unsigned)sizeof(float));
+#pragma unroll
+                for (int comp = 0; comp < 3; ++comp) tma_load_box(fs + comp * CS, &fmap, o[2], o[1], o[0], sp * 3 + comp, &mbar);
+            }
+            return;
+        }
         const float* fsp = ffield + (size_t)sp * 3 * m.FM;
         if (vec16) {
             // 16-byte copies: the image starts on a 16-byte boundary of the mesh rows (tp.sh) and Nz % 4 == 0,
@@ -173,7 +221,8 @@ __global__ void __launch_bounds__(RT, TILD_ROT_CTAS) interp_rot_kernel(MeshParam
     float4 pa[RPT];
     int2 ba[RPT];
     load_chunk(c0, (int)min(per, p_hi - c0), pa, ba);
-    __syncthreads();                                              // goff_*, gcnt visible
+    __syncthreads();                                              // goff_*, gcnt, mbarrier visible
+    bool staged = true;                                           // an image is on its way (uniform)
     stage(sp);
     PROF_MARK(0);                                                 // 0: prologue + staging issue
     while (true) {
@@ -244,6 +293,11 @@ __global__ void __launch_bounds__(RT, TILD_ROT_CTAS) interp_rot_kernel(MeshParam
         }
         PROF_MARK(1);                                                 // 1: binning
         cp_async_wait_all();
+        if (tma_tile && staged) {                                     // the boxes of this species have landed
+            mbar_wait(&mbar, tma_parity);
+            tma_parity ^= 1u;
+        }
+        staged = false;
         PROF_MARK(2);                                                 // 2: wait for the image
         __syncthreads();
         PROF_MARK(3);                                                 // 3: barrier after binning
@@ -320,6 +374,7 @@ __global__ void __launch_bounds__(RT, TILD_ROT_CTAS) interp_rot_kernel(MeshParam
                 per = (p_hi - p_lo + RCHUNK - 1) / RCHUNK;
                 per = ((p_hi - p_lo + per - 1) / per + 31u) & ~31u;
                 c0 = p_lo;
+                staged = true;
                 stage(sp);
             } else {
                 more = false;
@@ -376,8 +431,11 @@ cudaError_t rot_launch(const InterpArgs& a, cudaStream_t st, size_t smem, bool c
 {
     auto kernel = interp_rot_kernel<EY, EZ, MODE, FAST>;
     if (configure_only) return tild_raise_smem_limit(reinterpret_cast<const void*>(kernel), smem);
+    static const CUtensorMap no_map{};
+    const bool tma = a.use_tma && a.tp.E[1] == EY;     // the box of the tensor map is the template image
+    const CUtensorMap* map = tma ? static_cast<const CUtensorMap*>(a.fmap) : &no_map;
     kernel<<<a.tp.ntiles, RT, smem, st>>>(a.m, a.tp, a.s, a.step_ptr, a.seg_base, a.ffield, a.X4, a.W4, a.B, a.X4o, a.W4o, a.F4,
-                                          a.drift_list, a.drift_count);
+                                          a.drift_list, a.drift_count, *map, tma ? 1 : 0);
     return cudaSuccess;
 }
 template <int EY, int EZ>
@@ -396,7 +454,37 @@ cudaError_t rot_launch_m(const InterpArgs& a, int mode, cudaStream_t st, size_t 
 
 }  // namespace
 
-size_t interp_rot_smem(int ey, int ez) { return (size_t)REX * ey * ez * 3 * sizeof(float) + (size_t)3 * RSLOTS * sizeof(uint32_t); }
+size_t interp_rot_smem(int ey, int ez)
+{
+    const size_t csp = ((size_t)REX * ey * ez + 31) / 32 * 32;      // component stride, 128-byte multiple
+    return csp * 3 * sizeof(float) + (size_t)3 * RSLOTS * sizeof(uint32_t) + 128;   // + alignment slack
+}
+
+// Tensor map of the library's force field [3S][Nx][Ny][Nz] (float, z fastest) with the box of one component image.
+// Returns false when TMA cannot be used (rows not 16-byte multiples, driver entry point missing): cp.async staging then.
+bool interp_rot_make_tmap(tild_ctx* c)
+{
+    c->tma_ok = false;
+    if (!interp_rot_applies(c) || c->mesh.N[2] % 4 != 0 || (c->prm.flags & TILD_FLAG_NO_TMA)) return false;
+    typedef CUresult (*encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
+                                  const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn || qres != cudaDriverEntryPointSuccess) {
+        cudaGetLastError();
+        return false;
+    }
+    const cuuint64_t dims[4] = {(cuuint64_t)c->mesh.N[2], (cuuint64_t)c->mesh.N[1], (cuuint64_t)c->mesh.N[0], (cuuint64_t)(3 * c->mesh.S)};
+    const cuuint64_t strides[3] = {(cuuint64_t)c->mesh.N[2] * 4, (cuuint64_t)c->mesh.N[2] * c->mesh.N[1] * 4, (cuuint64_t)c->M * 4};
+    const cuuint32_t box[4] = {(cuuint32_t)c->tile.EZ, (cuuint32_t)c->tile.EY, (cuuint32_t)REX, 1u};
+    const cuuint32_t estr[4] = {1u, 1u, 1u, 1u};
+    static_assert(sizeof(CUtensorMap) <= sizeof(c->fmap), "tensor map storage");
+    const CUresult r = reinterpret_cast<encode_fn>(fn)(reinterpret_cast<CUtensorMap*>(c->fmap), CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, c->ffield, dims,
+                                                       strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                                       CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    c->tma_ok = r == CUDA_SUCCESS;
+    return c->tma_ok;
+}
 
 // P = 4 with an image whose rows tile the banks (EZ = 24 or 40) and the default tile width in x
 bool interp_rot_applies(const tild_ctx* c)

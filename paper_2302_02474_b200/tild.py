@@ -25,6 +25,7 @@ FLAG_GEN1_TILES = 128
 FLAG_EAGER = 256
 FLAG_2D = 512
 FLAG_EXTRAS = 1024
+FLAG_NO_TMA = 2048
 TIMING_NAMES = ("sort", "spread", "fft_fwd", "kspace", "fft_inv", "interp", "other", "total")
 
 EXPORTS = (
