@@ -97,6 +97,24 @@ __device__ __forceinline__ void tma_load_box(float* smem_dst, const CUtensorMap*
                  : "memory");
 }
 
+#ifdef TILD_ROT_DRIFT_IN_CTA
+// one drifted particle: global gather of its stencil + the tail (experiment, see the end of the kernel)
+template <int MODE>
+__device__ __noinline__ void drifted_particle(const MeshParams& m, const StepParams& s, uint64_t step_next, size_t slot,
+                                              const float* __restrict__ ffield, const float4* __restrict__ X4,
+                                              const float4* __restrict__ W4, const int32_t* __restrict__ B, float4* __restrict__ X4o,
+                                              float4* __restrict__ W4o, float4* __restrict__ F4)
+{
+    const float4 p = X4[slot];
+    int b[3];
+    float w[3][4];
+    index_weights<4>(m, p, b, w);
+    const bool vec = (m.N[2] % 4 == 0) && ((reinterpret_cast<uintptr_t>(ffield) & 15) == 0);
+    const float3 F = vec ? interp_global<4, true>(m, ffield, b, w, __float_as_int(p.w)) : interp_global<4, false>(m, ffield, b, w, __float_as_int(p.w));
+    finish_particle<MODE>(m, s, step_next, slot, p, F, X4, W4, B, X4o, W4o, F4);
+}
+#endif
+
 // Dynamic shared memory: (128-byte aligned) image float[3][CSP] of one species, CSP = REX EY EZ rounded up to 32 words so that
 // every component starts on a 128-byte boundary (TMA destination) | ent u32[3][RSLOTS].
 // FAST (MODE 2 only): the plain model of BASELINE configs -- two bond slots, no rest length, no angle potentials, three
@@ -421,9 +439,15 @@ __global__ void __launch_bounds__(RT, TILD_ROT_CTAS) interp_rot_kernel(MeshParam
     __syncthreads();
     const uint32_t nd = min(ndrift, (uint32_t)RDCAP);                  // uniform
     if (nd == 0) return;
+#ifndef TILD_ROT_DRIFT_IN_CTA
+    // handed to interp_drift_kernel.  (Doing them here, one per thread from the global field while it is L2-hot, measured
+    // 0.837 instead of 0.582 ms: the gather's latency sits at the end of every CTA and holds its SM slot.)
     if (threadIdx.x == 0) drift_base = atomicAdd(drift_count, nd);
     __syncthreads();
     if (threadIdx.x < nd) drift_list[drift_base + threadIdx.x] = dl[threadIdx.x];
+#else
+    if (threadIdx.x < nd) drifted_particle<MODE>(m, s, step_next, dl[threadIdx.x], ffield, X4, W4, B, X4o, W4o, F4);
+#endif
 }
 
 template <int EY, int EZ, int MODE, bool FAST>
