@@ -16,13 +16,15 @@ constexpr int INTERP_WARPS = INTERP_THREADS / 32;
 
 
 // per-particle kernel over the slots [s0, s1)
-template <int P, bool VEC, int MODE>
-__global__ void __launch_bounds__(256, P == 1 ? 8 : 1) interp_slots_kernel(MeshParams m, StepParams s, const uint64_t* __restrict__ step_ptr, size_t s0, size_t s1,
+template <int P, bool VEC, int MODE, bool FAST>
+__global__ void __launch_bounds__(256, P == 1 ? (FAST ? 8 : 4) : 1) interp_slots_kernel(MeshParams m, StepParams s_in, const uint64_t* __restrict__ step_ptr, size_t s0, size_t s1,
                                                            const float* __restrict__ ffield, const float4* __restrict__ X4,
                                                            const float4* __restrict__ W4, const int32_t* __restrict__ B,
                                                            float4* __restrict__ X4o, float4* __restrict__ W4o,
                                                            float4* __restrict__ F4)
 {
+    StepParams s = s_in;
+    fold_plain_model<FAST>(s);
     const uint64_t step_next = *step_ptr + 1;   // the step being produced (device-side counter: graph replays see it move)
     const size_t slot = s0 + (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (slot >= s1) return;
@@ -49,8 +51,10 @@ __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commi
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;\n" ::: "memory"); }
 
 // Dynamic shared memory: image float[3][EX][EY][EZ] of one species | idx u16[KCAP][32] | ovf u16[CHUNK].
-template <int P, int EY, int EZ, int MODE>
-__global__ void __launch_bounds__(INTERP_THREADS, 2) interp_tile_kernel(MeshParams m, TileParams tp, StepParams s, const uint64_t* __restrict__ step_ptr,
+// FAST (MODE 2): the plain model (two bond slots, no rest length, no angles, 3-D, inertial integrator) with those facts
+// folded in at compile time: no call sites of the generic bond / angle routines, hence no registers saved around them.
+template <int P, int EY, int EZ, int MODE, bool FAST>
+__global__ void __launch_bounds__(INTERP_THREADS, 2) interp_tile_kernel(MeshParams m, TileParams tp, StepParams s_in, const uint64_t* __restrict__ step_ptr,
                                                                      const uint32_t* __restrict__ seg_base,
                                                                      const float* __restrict__ ffield,
                                                                      const float4* __restrict__ X4, const float4* __restrict__ W4,
@@ -59,6 +63,8 @@ __global__ void __launch_bounds__(INTERP_THREADS, 2) interp_tile_kernel(MeshPara
                                                                      uint32_t* __restrict__ drift_list,
                                                                      uint32_t* __restrict__ drift_count)
 {
+    StepParams s = s_in;
+    fold_plain_model<FAST>(s);
     const uint64_t step_next = *step_ptr + 1;   // the step being produced (device-side counter: graph replays see it move)
     constexpr int CHUNK = TILD_INTERP_CHUNK, KCAP = TILD_INTERP_KCAP;
     extern __shared__ __align__(16) float fs[];
@@ -256,8 +262,8 @@ __global__ void __launch_bounds__(INTERP_THREADS, 2) interp_tile_kernel(MeshPara
 // particles that left their tile's image since the last re-sort: per-particle global gather, any order.
 // Last kernel of the fused pass: the block that finishes last resets the drift counter for the next pass and, in the
 // fused step (step_adv != nullptr), advances the device-side step counter -- no extra launches for either.
-template <int P, int MODE>
-__global__ void __launch_bounds__(256) interp_drift_kernel(MeshParams m, StepParams s, const uint64_t* step_ptr,
+template <int P, int MODE, bool FAST>
+__global__ void __launch_bounds__(256) interp_drift_kernel(MeshParams m, StepParams s_in, const uint64_t* step_ptr,
                                                            const uint32_t* __restrict__ drift_list,
                                                            uint32_t* __restrict__ drift_count, uint64_t* __restrict__ step_adv,
                                                            const float* __restrict__ ffield, const float4* __restrict__ X4,
@@ -265,6 +271,8 @@ __global__ void __launch_bounds__(256) interp_drift_kernel(MeshParams m, StepPar
                                                            float4* __restrict__ X4o, float4* __restrict__ W4o,
                                                            float4* __restrict__ F4)
 {
+    StepParams s = s_in;
+    fold_plain_model<FAST>(s);
     const uint64_t step_next = *step_ptr + 1;   // the step being produced (device-side counter: graph replays see it move)
     const uint32_t nd = *drift_count;
     for (uint32_t j = blockIdx.x * blockDim.x + threadIdx.x; j < nd; j += gridDim.x * blockDim.x) {
@@ -397,10 +405,10 @@ bool can_vectorize(const tild_ctx* c, const float* ffield)
 
 // ---- dispatch ------------------------------------------------------------------------------------------------------
 
-template <int P, int EY, int EZ, int MODE>
+template <int P, int EY, int EZ, int MODE, bool FAST>
 void tile_launch(const InterpArgs& a, cudaStream_t st, size_t smem, bool configure_only, cudaError_t* err)
 {
-    auto kernel = interp_tile_kernel<P, EY, EZ, MODE>;
+    auto kernel = interp_tile_kernel<P, EY, EZ, MODE, FAST>;
     if (configure_only) {
         const cudaError_t e = tild_raise_smem_limit(reinterpret_cast<const void*>(kernel), smem);
         if (e != cudaSuccess) *err = e;
@@ -408,15 +416,17 @@ void tile_launch(const InterpArgs& a, cudaStream_t st, size_t smem, bool configu
     }
     kernel<<<a.tp.ntiles, INTERP_THREADS, smem, st>>>(a.m, a.tp, a.s, a.step_ptr, a.seg_base, a.ffield, a.X4, a.W4, a.B, a.X4o,
                                                       a.W4o, a.F4, a.drift_list, a.drift_count);
-    interp_drift_kernel<P, MODE><<<592, 256, 0, st>>>(a.m, a.s, a.step_ptr, a.drift_list, a.drift_count, MODE == 2 ? a.step_adv : nullptr,
-                                                      a.ffield, a.X4, a.W4, a.B, a.X4o, a.W4o, a.F4);
+    interp_drift_kernel<P, MODE, FAST><<<592, 256, 0, st>>>(a.m, a.s, a.step_ptr, a.drift_list, a.drift_count, MODE == 2 ? a.step_adv : nullptr,
+                                                            a.ffield, a.X4, a.W4, a.B, a.X4o, a.W4o, a.F4);
 }
 template <int P, int EY, int EZ>
 void tile_launch_m(const InterpArgs& a, int mode, cudaStream_t st, size_t smem, bool cfg, cudaError_t* err)
 {
-    if (cfg || mode == 0) tile_launch<P, EY, EZ, 0>(a, st, smem, cfg, err);
-    if (cfg || mode == 1) tile_launch<P, EY, EZ, 1>(a, st, smem, cfg, err);
-    if (cfg || mode == 2) tile_launch<P, EY, EZ, 2>(a, st, smem, cfg, err);
+    const bool fast = plain_model(a.s);
+    if (cfg || mode == 0) tile_launch<P, EY, EZ, 0, false>(a, st, smem, cfg, err);
+    if (cfg || mode == 1) tile_launch<P, EY, EZ, 1, false>(a, st, smem, cfg, err);
+    if (cfg || (mode == 2 && !fast)) tile_launch<P, EY, EZ, 2, false>(a, st, smem, cfg, err);
+    if (cfg || (mode == 2 && fast)) tile_launch<P, EY, EZ, 2, true>(a, st, smem, cfg, err);
 }
 template <int P>
 bool tile_launch_p(const InterpArgs& a, int ey, int ez, int mode, cudaStream_t st, size_t smem, bool cfg, cudaError_t* err)
@@ -443,8 +453,8 @@ bool tile_launch_any(const InterpArgs& a, int mode, cudaStream_t st, size_t smem
 // the drifted particles of the rotation-class kernel (P = 4)
 void launch_drift_only(const InterpArgs& a, int mode, cudaStream_t st)
 {
-#define TILD_DR(M_) interp_drift_kernel<4, M_><<<592, 256, 0, st>>>(a.m, a.s, a.step_ptr, a.drift_list, a.drift_count, M_ == 2 ? a.step_adv : nullptr, a.ffield, a.X4, a.W4, a.B, a.X4o, a.W4o, a.F4)
-    if (mode == 0) TILD_DR(0); else if (mode == 1) TILD_DR(1); else TILD_DR(2);
+#define TILD_DR(M_, F_) interp_drift_kernel<4, M_, F_><<<592, 256, 0, st>>>(a.m, a.s, a.step_ptr, a.drift_list, a.drift_count, M_ == 2 ? a.step_adv : nullptr, a.ffield, a.X4, a.W4, a.B, a.X4o, a.W4o, a.F4)
+    if (mode == 0) TILD_DR(0, false); else if (mode == 1) TILD_DR(1, false); else if (plain_model(a.s)) TILD_DR(2, true); else TILD_DR(2, false);
 #undef TILD_DR
 }
 
@@ -452,9 +462,10 @@ template <int P>
 void slots_launch_p(const InterpArgs& a, bool vec, int mode, size_t s0, size_t s1, cudaStream_t st)
 {
     const unsigned nb = (unsigned)((s1 - s0 + 255) / 256);
-#define TILD_SL(V, M_) interp_slots_kernel<P, V, M_><<<nb, 256, 0, st>>>(a.m, a.s, a.step_ptr, s0, s1, a.ffield, a.X4, a.W4, a.B, a.X4o, a.W4o, a.F4)
-    if (vec) { if (mode == 0) TILD_SL(true, 0); else if (mode == 1) TILD_SL(true, 1); else TILD_SL(true, 2); }
-    else     { if (mode == 0) TILD_SL(false, 0); else if (mode == 1) TILD_SL(false, 1); else TILD_SL(false, 2); }
+#define TILD_SL(V, M_, F_) interp_slots_kernel<P, V, M_, F_><<<nb, 256, 0, st>>>(a.m, a.s, a.step_ptr, s0, s1, a.ffield, a.X4, a.W4, a.B, a.X4o, a.W4o, a.F4)
+    const bool fast = plain_model(a.s);
+    if (vec) { if (mode == 0) TILD_SL(true, 0, false); else if (mode == 1) TILD_SL(true, 1, false); else if (fast) TILD_SL(true, 2, true); else TILD_SL(true, 2, false); }
+    else     { if (mode == 0) TILD_SL(false, 0, false); else if (mode == 1) TILD_SL(false, 1, false); else if (fast) TILD_SL(false, 2, true); else TILD_SL(false, 2, false); }
 #undef TILD_SL
 }
 

@@ -133,14 +133,7 @@ __global__ void __launch_bounds__(RT, TILD_ROT_CTAS) interp_rot_kernel(MeshParam
     static_assert(EZ % 32 == 8 || EZ % 32 == 24, "row rotation needs the P rows of a stencil to tile the 32 banks");
     static_assert(!FAST || MODE == 2, "FAST is a specialisation of the fused step");
     StepParams s = s_in;
-    if (FAST) {
-        s.max_bonds = 2;
-        s.r0_bond = 0.0f;
-        s.lambda_wlc = 0.0f;
-        s.k_theta = 0.0f;
-        s.dim2 = 0;
-        s.integrator = TILD_INTEGRATOR_GJF;     // GJF and VV + Langevin share one code path (coefficients differ)
-    }
+    fold_plain_model<FAST>(s);
     extern __shared__ __align__(16) float fs_raw[];
     float* fs = reinterpret_cast<float*>((reinterpret_cast<uintptr_t>(fs_raw) + 127) & ~(uintptr_t)127);
     __shared__ int goff_x[16], goff_y[32];
@@ -465,9 +458,7 @@ cudaError_t rot_launch(const InterpArgs& a, cudaStream_t st, size_t smem, bool c
 template <int EY, int EZ>
 cudaError_t rot_launch_m(const InterpArgs& a, int mode, cudaStream_t st, size_t smem, bool cfg)
 {
-    const StepParams& s = a.s;
-    const bool fast = s.max_bonds == 2 && s.r0_bond == 0.0f && s.lambda_wlc == 0.0f && s.k_theta == 0.0f && !s.dim2 &&
-                      s.integrator != TILD_INTEGRATOR_EM;
+    const bool fast = plain_model(a.s);
     cudaError_t e = cudaSuccess, e2;
     if (cfg || mode == 0) { e2 = rot_launch<EY, EZ, 0, false>(a, st, smem, cfg); if (e2 != cudaSuccess) e = e2; }
     if (cfg || mode == 1) { e2 = rot_launch<EY, EZ, 1, false>(a, st, smem, cfg); if (e2 != cudaSuccess) e = e2; }

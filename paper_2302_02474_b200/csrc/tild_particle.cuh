@@ -81,6 +81,26 @@ __device__ __forceinline__ float3 interp_global(const MeshParams& m, const float
     return acc;
 }
 
+// The plain model of the BASELINE configs: two bond slots, no rest length, no angle potentials, three dimensions, an inertial
+// integrator (GJF or VV + Langevin: one code path, other coefficients).  Kernels instantiated with FAST fold these facts in
+// at compile time (fold_plain_model), which removes the call sites of the generic routines and their never-taken branches.
+inline bool plain_model(const StepParams& s)
+{
+    return s.max_bonds == 2 && s.r0_bond == 0.0f && s.lambda_wlc == 0.0f && s.k_theta == 0.0f && !s.dim2 && s.integrator != TILD_INTEGRATOR_EM;
+}
+template <bool FAST>
+__device__ __forceinline__ void fold_plain_model(StepParams& s)
+{
+    if (FAST) {
+        s.max_bonds = 2;
+        s.r0_bond = 0.0f;
+        s.lambda_wlc = 0.0f;
+        s.k_theta = 0.0f;
+        s.dim2 = 0;
+        s.integrator = TILD_INTEGRATOR_GJF;
+    }
+}
+
 // f += force on the particle at p from the bond to the particle at q (Eq. 2; minimum image)
 __device__ __forceinline__ void bond_term(const MeshParams& m, const StepParams& s, const float4& p, const float4& q, float3& f)
 {
@@ -203,14 +223,21 @@ __device__ __forceinline__ void finish_particle(const MeshParams& m, const StepP
                                                 const float4* __restrict__ W4, const int32_t* __restrict__ B,
                                                 float4* __restrict__ X4o, float4* __restrict__ W4o, float4* __restrict__ F4)
 {
-    if (MODE >= 1) {
-        const float3 fb = bond_force_slots(m, s, X4, B, slot, p);
-        F.x += fb.x;
-        F.y += fb.y;
-        F.z += fb.z;
-    }
     float4 w0 = make_float4(0.f, 0.f, 0.f, 0.f);
     if (MODE == 2) w0 = W4[slot];
+    if (MODE >= 1) {
+        if (s.max_bonds == 2 && s.lambda_wlc == 0.0f && s.k_theta == 0.0f) {   // linear chains without angles: inline, no call
+            const int2 bb = *reinterpret_cast<const int2*>(B + 2 * slot);
+            const float4 q0 = X4[bb.x >= 0 ? (size_t)bb.x : slot], q1 = X4[bb.y >= 0 ? (size_t)bb.y : slot];   // self: zero force
+            bond_term(m, s, p, q0, F);
+            bond_term(m, s, p, q1, F);
+        } else if (s.max_bonds > 0) {
+            const float3 fb = bond_force_slots(m, s, X4, B, slot, p);          // generic tables, angle potentials (not inlined)
+            F.x += fb.x;
+            F.y += fb.y;
+            F.z += fb.z;
+        }
+    }
     finish_update<MODE>(m, s, step_next, slot, p, F, w0, X4o, W4o, F4);
 }
 
