@@ -135,7 +135,9 @@ __global__ void __launch_bounds__(RT, TILD_ROT_CTAS) interp_rot_kernel(MeshParam
     StepParams s = s_in;
     fold_plain_model<FAST>(s);
     extern __shared__ __align__(16) float fs_raw[];
-    float* fs = reinterpret_cast<float*>((reinterpret_cast<uintptr_t>(fs_raw) + 127) & ~(uintptr_t)127);
+    // 128-byte alignment for the TMA boxes, as an offset in the shared window: a round trip through uintptr_t would lose the
+    // address space and turn every stencil LDS into a generic LD with 64-bit address arithmetic
+    float* fs = fs_raw + (((128u - ((unsigned)__cvta_generic_to_shared(fs_raw) & 127u)) & 127u) >> 2);
     __shared__ int goff_x[16], goff_y[32];
     __shared__ uint32_t gcnt[8], ndrift, drift_base, dl[RDCAP];
     __shared__ __align__(8) uint64_t mbar;
