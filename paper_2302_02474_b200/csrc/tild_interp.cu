@@ -275,16 +275,32 @@ __global__ void __launch_bounds__(256) interp_drift_kernel(MeshParams m, StepPar
     fold_plain_model<FAST>(s);
     const uint64_t step_next = *step_ptr + 1;   // the step being produced (device-side counter: graph replays see it move)
     const uint32_t nd = *drift_count;
-    for (uint32_t j = blockIdx.x * blockDim.x + threadIdx.x; j < nd; j += gridDim.x * blockDim.x) {
-        const size_t slot = drift_list[j];
-        const float4 p = X4[slot];
-        int b[3];
-        float w[3][P];
-        index_weights<P>(m, p, b, w);
-        const bool vec = (m.N[2] % 4 == 0) && ((reinterpret_cast<uintptr_t>(ffield) & 15) == 0);   // uniform
-        const float3 F = vec ? interp_global<P, true>(m, ffield, b, w, __float_as_int(p.w))
-                             : interp_global<P, false>(m, ffield, b, w, __float_as_int(p.w));
-        finish_particle<MODE>(m, s, step_next, slot, p, F, X4, W4, B, X4o, W4o, F4);
+    // G lanes share a particle (its P P stencil rows dealt round-robin): the kernel is bound by the latency of the gathers
+    // (the field left L2 long ago), so what counts is how many of them are in flight
+    constexpr int G = P >= 3 ? 8 : P == 2 ? 4 : 1;
+    const bool vec = (m.N[2] % 4 == 0) && ((reinterpret_cast<uintptr_t>(ffield) & 15) == 0);   // uniform
+    const uint32_t g = threadIdx.x % G, per_pass = gridDim.x * (blockDim.x / G);
+    for (uint32_t j0 = 0; j0 < nd; j0 += per_pass) {                  // uniform trip count: the shuffles below are full-warp
+        const uint32_t j = j0 + blockIdx.x * (blockDim.x / G) + threadIdx.x / G;
+        const bool act = j < nd;
+        const size_t slot = act ? drift_list[j] : 0;
+        float4 p = make_float4(0.f, 0.f, 0.f, 0.f);
+        float3 F = make_float3(0.f, 0.f, 0.f);
+        if (act) {
+            p = X4[slot];
+            int b[3];
+            float w[3][P];
+            index_weights<P>(m, p, b, w);
+            F = vec ? interp_global_rows<P, true, G>(m, ffield, b, w, __float_as_int(p.w), (int)g)
+                    : interp_global_rows<P, false, G>(m, ffield, b, w, __float_as_int(p.w), (int)g);
+        }
+#pragma unroll
+        for (int d = G / 2; d > 0; d >>= 1) {
+            F.x += __shfl_xor_sync(0xffffffffu, F.x, d);
+            F.y += __shfl_xor_sync(0xffffffffu, F.y, d);
+            F.z += __shfl_xor_sync(0xffffffffu, F.z, d);
+        }
+        if (act && g == 0) finish_particle<MODE>(m, s, step_next, slot, p, F, X4, W4, B, X4o, W4o, F4);
     }
     __syncthreads();                            // every thread of this block has read the step and the drift count
     if (threadIdx.x == 0) {
@@ -416,7 +432,7 @@ void tile_launch(const InterpArgs& a, cudaStream_t st, size_t smem, bool configu
     }
     kernel<<<a.tp.ntiles, INTERP_THREADS, smem, st>>>(a.m, a.tp, a.s, a.step_ptr, a.seg_base, a.ffield, a.X4, a.W4, a.B, a.X4o,
                                                       a.W4o, a.F4, a.drift_list, a.drift_count);
-    interp_drift_kernel<P, MODE, FAST><<<592, 256, 0, st>>>(a.m, a.s, a.step_ptr, a.drift_list, a.drift_count, MODE == 2 ? a.step_adv : nullptr,
+    interp_drift_kernel<P, MODE, FAST><<<1184, 256, 0, st>>>(a.m, a.s, a.step_ptr, a.drift_list, a.drift_count, MODE == 2 ? a.step_adv : nullptr,
                                                             a.ffield, a.X4, a.W4, a.B, a.X4o, a.W4o, a.F4);
 }
 template <int P, int EY, int EZ>
@@ -453,7 +469,7 @@ bool tile_launch_any(const InterpArgs& a, int mode, cudaStream_t st, size_t smem
 // the drifted particles of the rotation-class kernel (P = 4)
 void launch_drift_only(const InterpArgs& a, int mode, cudaStream_t st)
 {
-#define TILD_DR(M_, F_) interp_drift_kernel<4, M_, F_><<<592, 256, 0, st>>>(a.m, a.s, a.step_ptr, a.drift_list, a.drift_count, M_ == 2 ? a.step_adv : nullptr, a.ffield, a.X4, a.W4, a.B, a.X4o, a.W4o, a.F4)
+#define TILD_DR(M_, F_) interp_drift_kernel<4, M_, F_><<<1184, 256, 0, st>>>(a.m, a.s, a.step_ptr, a.drift_list, a.drift_count, M_ == 2 ? a.step_adv : nullptr, a.ffield, a.X4, a.W4, a.B, a.X4o, a.W4o, a.F4)
     if (mode == 0) TILD_DR(0, false); else if (mode == 1) TILD_DR(1, false); else if (plain_model(a.s)) TILD_DR(2, true); else TILD_DR(2, false);
 #undef TILD_DR
 }

@@ -81,6 +81,66 @@ __device__ __forceinline__ float3 interp_global(const MeshParams& m, const float
     return acc;
 }
 
+// The (x, y) rows r0, r0 + G, ... (< P P) of one particle's stencil: one lane of a group of G lanes that share a particle
+// (interp_drift_kernel); the group's partial sums are added by the caller.
+template <int P, bool VEC, int G>
+__device__ __forceinline__ float3 interp_global_rows(const MeshParams& m, const float* __restrict__ ffield, const int b[3],
+                                                     const float w[3][P], int type, int r0)
+{
+    const float* comp[3];
+    comp[0] = ffield + (size_t)type * 3 * m.FM;
+    comp[1] = comp[0] + m.FM;
+    comp[2] = comp[1] + m.FM;
+    float acc[3] = {0.f, 0.f, 0.f};
+    const int bzw = wrap_idx(b[2], m.N[2]);
+    const int a0 = bzw & ~3, off = bzw & 3;
+    const int a1 = (a0 + 4 >= m.N[2]) ? 0 : a0 + 4;
+    const bool two = off + P > 4;
+    float w8[8];
+    int iz[P];
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+        float v = 0.f;
+#pragma unroll
+        for (int j = 0; j < P; ++j)
+            if (k - j >= 0 && k - j <= 3) v = (k - j == off) ? w[2][j] : v;
+        w8[k] = v;
+    }
+#pragma unroll
+    for (int j = 0; j < P; ++j) iz[j] = wrap_idx(b[2] + j, m.N[2]);
+#pragma unroll
+    for (int i = 0; i < (P * P + G - 1) / G; ++i) {
+        const int r = r0 + i * G;
+        if (r >= P * P) break;
+        const int jx = r / P, jy = r - jx * P;
+        float wx = w[0][0], wy = w[1][0];
+#pragma unroll
+        for (int j = 1; j < P; ++j) {
+            wx = jx == j ? w[0][j] : wx;
+            wy = jy == j ? w[1][j] : wy;
+        }
+        const size_t row = ((size_t)wrap_idx(b[0] + jx, m.N[0]) * m.FN[0] + wrap_idx(b[1] + jy, m.N[1])) * m.FN[1];
+        const float wxy = wx * wy;
+#pragma unroll
+        for (int q = 0; q < 3; ++q) {
+            float sum = 0.f;
+            if (VEC) {
+                const float4 v0 = __ldg(reinterpret_cast<const float4*>(comp[q] + row + a0));
+                sum = w8[0] * v0.x + w8[1] * v0.y + w8[2] * v0.z + w8[3] * v0.w;
+                if (two) {
+                    const float4 v1 = __ldg(reinterpret_cast<const float4*>(comp[q] + row + a1));
+                    sum += w8[4] * v1.x + w8[5] * v1.y + w8[6] * v1.z + w8[7] * v1.w;
+                }
+            } else {
+#pragma unroll
+                for (int jz = 0; jz < P; ++jz) sum += w[2][jz] * __ldg(comp[q] + row + iz[jz]);
+            }
+            acc[q] += wxy * sum;
+        }
+    }
+    return make_float3(acc[0], acc[1], acc[2]);
+}
+
 // The plain model of the BASELINE configs: two bond slots, no rest length, no angle potentials, three dimensions, an inertial
 // integrator (GJF or VV + Langevin: one code path, other coefficients).  Kernels instantiated with FAST fold these facts in
 // at compile time (fold_plain_model), which removes the call sites of the generic routines and their never-taken branches.

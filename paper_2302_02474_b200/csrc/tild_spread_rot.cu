@@ -11,6 +11,8 @@
 //    first-generation kernel's re-load of every position in class order was an L2 round trip per particle.
 #include "tild_internal.cuh"
 
+#include <type_traits>
+
 namespace {
 
 #ifndef TILD_SROT_THREADS
@@ -100,6 +102,8 @@ __global__ void __launch_bounds__(ST, 2) spread_rot_kernel(MeshParams m, TilePar
     const uint32_t p_lo = seg_base[seg0], p_hi = seg_base[seg0 + nsp];
     if (p_lo == p_hi) return;                        // empty tile (uniform)
     uint32_t* ent = sm + (size_t)sp_group * E3;
+    // the tile's positions on their way to L2 while the image is zeroed (8 particles per 128-byte line)
+    for (uint32_t i = p_lo + 8u * threadIdx.x; i < p_hi; i += 8u * ST) asm volatile("prefetch.global.L2 [%0];" ::"l"(X4 + i));
     {
         uint4* z4 = reinterpret_cast<uint4*>(sm);
         const int n4 = nsp * E3 / 4;                 // EZ % 4 == 0
@@ -233,31 +237,35 @@ __global__ void __launch_bounds__(ST, 2) spread_rot_kernel(MeshParams m, TilePar
     constexpr int RPP = ST / EZ;                     // rows per pass
     const int lz = threadIdx.x % EZ, r0 = threadIdx.x / EZ;
     const int gz = wrap_idx(o[2] + lz, m.N[2]);
-    for (int pass = 0; pass < 2; ++pass) {           // pass 1 only runs to undo a wrapped tile
-        const float sc = pass == 0 ? FIX_INV : -FIX_INV;
-        if (r0 < RPP) {
-            for (int spl = 0; spl < nsp; ++spl) {
-                float* gsp = grid + (size_t)(sp0 + spl) * m.M + gz;
-                const uint32_t* simg = sm + spl * E3 + lz;
-                for (int q = r0; q < SEX * EY; q += RPP) {
-                    const uint32_t u = simg[q * EZ];
-                    if (u) {
-                        if (pass == 0) tile_sum += u;
-                        atomicAdd(gsp + rowoff[q], (float)u * sc);
-                    }
+    // A node can only wrap past 2^32 if >= 2^9 / (largest single-node weight) particles sit on it; the largest weight of
+    // the cubic spline is (23/48)^3.  Tiles with fewer particles skip the check and the sum that feeds it.
+    const bool check = p_hi - p_lo > 4653u;          // uniform across the block
+    auto flush = [&](auto sum, const float sc) {
+        if (r0 >= RPP) return;
+        for (int spl = 0; spl < nsp; ++spl) {
+            float* gsp = grid + (size_t)(sp0 + spl) * m.M + gz;
+            const uint32_t* simg = sm + spl * E3 + lz;
+            for (int q = r0; q < SEX * EY; q += RPP) {
+                const uint32_t u = simg[q * EZ];
+                if (u) {
+                    if (decltype(sum)::value) tile_sum += u;
+                    atomicAdd(gsp + rowoff[q], (float)u * sc);
                 }
             }
         }
-        if (pass == 1) break;
-        // A node can only wrap past 2^32 if >= 2^9 / (largest single-node weight) particles sit on it; the largest
-        // weight of the cubic spline is (23/48)^3.  Tiles with fewer particles skip the check.
-        if (p_hi - p_lo <= 4653u) return;             // uniform across the block
+    };
+    if (!check) {
+        flush(std::false_type(), FIX_INV);
+        return;
+    }
+    flush(std::true_type(), FIX_INV);
+    {
         const unsigned long long total = block_sum_u64(tile_sum, red);
         const unsigned long long cntp = block_sum_u64((unsigned long long)n_tile, red);
         const unsigned long long expect = cntp << FIX_BITS, slack = 64ull * cntp + 64ull;
-        const bool ok = total + slack >= expect && total <= expect + slack;
-        if (ok) return;                               // uniform across the block
+        if (total + slack >= expect && total <= expect + slack) return;   // uniform across the block
     }
+    flush(std::false_type(), -FIX_INV);              // undo the wrapped tile
     // a node wrapped past 2^32 (>= 512 particles' worth on one node): redo this tile with fp32 global atomics
     for (uint32_t i = p_lo + threadIdx.x; i < p_hi; i += ST) {
         const float4 p = X4[i];
