@@ -703,6 +703,10 @@ int enqueue_one_step(tild_ctx* c, cudaEvent_t* ev)
 int launch_graph_block(tild_ctx* c)
 {
     const int block = 2 * c->resort_every;
+    if (!c->grid_clean) {   // the captured block starts from a cleared density grid (its steps clear it for one another)
+        TILD_CUDA(c, cudaMemsetAsync(c->grid, 0, sizeof(float) * c->M * c->mesh.S, c->stream));
+        c->grid_clean = true;
+    }
     if (!(c->graph_ok && c->graph_cur == c->cur && c->graph_x0 == c->X4[0])) {
         if (c->graph_ok) {
             cudaGraphExecDestroy(c->graph_exec);
@@ -720,6 +724,8 @@ int launch_graph_block(tild_ctx* c)
         cudaGraph_t graph = nullptr;
         const cudaError_t e = cudaStreamEndCapture(c->stream, &graph);
         c->graph_launches = c->launches - launches0;
+        c->graph_leaves_clean = c->grid_clean;
+        c->grid_clean = true;   // nothing ran
         const bool same = c->cur == cur0 && c->X4[0] == x0[0] && c->W4[0] == w0[0] && c->steps_since_sort == sss0;
         c->cur = cur0; c->steps_since_sort = sss0; c->step = step0; c->launches = launches0;
         c->X4[0] = x0[0]; c->X4[1] = x0[1]; c->W4[0] = w0[0]; c->W4[1] = w0[1];
@@ -737,6 +743,7 @@ int launch_graph_block(tild_ctx* c)
         c->graph_x0 = c->X4[0];
     }
     TILD_CUDA(c, cudaGraphLaunch(c->graph_exec, c->stream));
+    c->grid_clean = c->graph_leaves_clean;
     c->step += (uint64_t)block;          // pointers, cur and steps_since_sort end where they started
     c->launches += c->graph_launches;
     return TILD_OK;

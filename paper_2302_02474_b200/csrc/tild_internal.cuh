@@ -157,6 +157,8 @@ struct tild_ctx {
 
     bool has_state;
     bool step_advanced;   // the last launch_interp advanced the device step counter itself (tile path)
+    bool grid_clean = false;        // c->grid is all zero: the drift kernel of the fused step cleared it for the next spread
+    bool graph_leaves_clean = false;
     uint64_t step;
     int steps_since_sort;
     int resort_every;
@@ -249,6 +251,8 @@ struct InterpArgs {
     uint64_t* step_adv;      // device step counter, advanced by the last block of the drift kernel in the fused step
     const void* fmap;        // CUtensorMap of the force field (tild_interp_rot.cu) when use_tma
     int use_tma;
+    float4* zgrid;           // fused step: the density grid, cleared by the drift kernel for the next step's spread (or null)
+    size_t zcount4;
 };
 // tild_spread_rot.cu: the P = 4 rotation-class spread kernel
 bool spread_rot_applies(const tild_ctx* c);

@@ -269,10 +269,15 @@ __global__ void __launch_bounds__(256) interp_drift_kernel(MeshParams m, StepPar
                                                            const float* __restrict__ ffield, const float4* __restrict__ X4,
                                                            const float4* __restrict__ W4, const int32_t* __restrict__ B,
                                                            float4* __restrict__ X4o, float4* __restrict__ W4o,
-                                                           float4* __restrict__ F4)
+                                                           float4* __restrict__ F4, float4* __restrict__ zgrid, size_t zcount4)
 {
     StepParams s = s_in;
     fold_plain_model<FAST>(s);
+    // The density grid of the next step, cleared here instead of by a memset in front of the spread: this kernel waits on
+    // gather latency and leaves HBM idle, so the stores are free (they drain while the gathers below are in flight).
+    if (zgrid)
+        for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < zcount4; i += (size_t)gridDim.x * blockDim.x)
+            zgrid[i] = make_float4(0.f, 0.f, 0.f, 0.f);
     const uint64_t step_next = *step_ptr + 1;   // the step being produced (device-side counter: graph replays see it move)
     const uint32_t nd = *drift_count;
     // G lanes share a particle (its P P stencil rows dealt round-robin): the kernel is bound by the latency of the gathers
@@ -433,7 +438,7 @@ void tile_launch(const InterpArgs& a, cudaStream_t st, size_t smem, bool configu
     kernel<<<a.tp.ntiles, INTERP_THREADS, smem, st>>>(a.m, a.tp, a.s, a.step_ptr, a.seg_base, a.ffield, a.X4, a.W4, a.B, a.X4o,
                                                       a.W4o, a.F4, a.drift_list, a.drift_count);
     interp_drift_kernel<P, MODE, FAST><<<1184, 256, 0, st>>>(a.m, a.s, a.step_ptr, a.drift_list, a.drift_count, MODE == 2 ? a.step_adv : nullptr,
-                                                            a.ffield, a.X4, a.W4, a.B, a.X4o, a.W4o, a.F4);
+                                                            a.ffield, a.X4, a.W4, a.B, a.X4o, a.W4o, a.F4, MODE == 2 ? a.zgrid : nullptr, a.zcount4);
 }
 template <int P, int EY, int EZ>
 void tile_launch_m(const InterpArgs& a, int mode, cudaStream_t st, size_t smem, bool cfg, cudaError_t* err)
@@ -469,7 +474,7 @@ bool tile_launch_any(const InterpArgs& a, int mode, cudaStream_t st, size_t smem
 // the drifted particles of the rotation-class kernel (P = 4)
 void launch_drift_only(const InterpArgs& a, int mode, cudaStream_t st)
 {
-#define TILD_DR(M_, F_) interp_drift_kernel<4, M_, F_><<<1184, 256, 0, st>>>(a.m, a.s, a.step_ptr, a.drift_list, a.drift_count, M_ == 2 ? a.step_adv : nullptr, a.ffield, a.X4, a.W4, a.B, a.X4o, a.W4o, a.F4)
+#define TILD_DR(M_, F_) interp_drift_kernel<4, M_, F_><<<1184, 256, 0, st>>>(a.m, a.s, a.step_ptr, a.drift_list, a.drift_count, M_ == 2 ? a.step_adv : nullptr, a.ffield, a.X4, a.W4, a.B, a.X4o, a.W4o, a.F4, M_ == 2 ? a.zgrid : nullptr, a.zcount4)
     if (mode == 0) TILD_DR(0, false); else if (mode == 1) TILD_DR(1, false); else if (plain_model(a.s)) TILD_DR(2, true); else TILD_DR(2, false);
 #undef TILD_DR
 }
@@ -513,21 +518,30 @@ int launch_interp(tild_ctx* c, int mode, const SegLayout& lay, const float* ffie
     const size_t n = (size_t)c->mesh.n;
     if (n == 0) return TILD_OK;
     InterpArgs a{c->mesh, c->tile, c->stp, c->d_step, lay.seg_base, ffield, X4, W4, B, X4o, W4o, c->F4, c->rank, c->drift_count, c->d_step,
-                 c->fmap, (c->tma_ok && ffield == c->ffield) ? 1 : 0};   // the tensor map describes the library's own field
+                 c->fmap, (c->tma_ok && ffield == c->ffield) ? 1 : 0,    // the tensor map describes the library's own field
+                 nullptr, 0};
     c->step_advanced = false;
     if (c->tile.enabled && c->mesh.P >= 2 && !(c->prm.flags & TILD_FLAG_NAIVE_INTERP)) {   // P = 1: one node per particle
         cudaError_t e = cudaSuccess;
         // drift_count[0..1] are zero here: cleared at tild_init and again by the last block of every drift kernel
         c->step_advanced = mode == INTERP_FUSED_STEP;
+        const size_t gridf = c->M * (size_t)c->mesh.S;
+        if (mode == INTERP_FUSED_STEP && gridf % 4 == 0 && (reinterpret_cast<uintptr_t>(c->grid) & 15) == 0) {
+            a.zgrid = reinterpret_cast<float4*>(c->grid);   // dead since the forward transform of this step
+            a.zcount4 = gridf / 4;
+        }
         if (interp_rot_applies(c) && !(c->prm.flags & TILD_FLAG_GEN1_TILES)) {
             e = interp_rot_run(a, mode, c->stream, false);
             TILD_LAUNCH_CHECK(c, "interp_rot_kernel");
-            launch_drift_only(a, mode, c->stream);
+            InterpArgs ad = a;
+            ad.zgrid = nullptr;                            // the tile kernel has cleared the grid
+            launch_drift_only(ad, mode, c->stream);
         } else {
             tile_launch_any(a, mode, c->stream, c->tile.smem_interp, false, &e);
             TILD_LAUNCH_CHECK(c, "interp_tile_kernel");
         }
         TILD_LAUNCH_CHECK(c, "interp_drift_kernel");
+        if (a.zgrid) c->grid_clean = true;
         return TILD_OK;
     }
     const bool vec = can_vectorize(c, ffield);

@@ -127,9 +127,16 @@ __global__ void __launch_bounds__(RT, TILD_ROT_CTAS) interp_rot_kernel(MeshParam
                                                           const int32_t* __restrict__ B, float4* __restrict__ X4o,
                                                           float4* __restrict__ W4o, float4* __restrict__ F4,
                                                           uint32_t* __restrict__ drift_list, uint32_t* __restrict__ drift_count,
-                                                          const __grid_constant__ CUtensorMap fmap, int use_tma)
+                                                          const __grid_constant__ CUtensorMap fmap, int use_tma,
+                                                          float4* __restrict__ zgrid, size_t zcount4)
 {
     constexpr int P = 4, CS = (REX * EY * EZ + 31) / 32 * 32;
+    // The density grid of the next step, cleared here (an equal share per CTA) instead of by a memset in front of the spread:
+    // this kernel is bound by the shared-memory pipe and leaves most of the HBM bandwidth unused.
+    if (MODE == 2 && zgrid) {
+        const size_t per = (zcount4 + gridDim.x - 1) / gridDim.x, z0 = blockIdx.x * per, z1 = min(z0 + per, zcount4);
+        for (size_t i = z0 + threadIdx.x; i < z1; i += RT) zgrid[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    }
     static_assert(EZ % 32 == 8 || EZ % 32 == 24, "row rotation needs the P rows of a stencil to tile the 32 banks");
     static_assert(!FAST || MODE == 2, "FAST is a specialisation of the fused step");
     StepParams s = s_in;
@@ -454,7 +461,7 @@ cudaError_t rot_launch(const InterpArgs& a, cudaStream_t st, size_t smem, bool c
     const bool tma = a.use_tma && a.tp.E[1] == EY;     // the box of the tensor map is the template image
     const CUtensorMap* map = tma ? static_cast<const CUtensorMap*>(a.fmap) : &no_map;
     kernel<<<a.tp.ntiles, RT, smem, st>>>(a.m, a.tp, a.s, a.step_ptr, a.seg_base, a.ffield, a.X4, a.W4, a.B, a.X4o, a.W4o, a.F4,
-                                          a.drift_list, a.drift_count, *map, tma ? 1 : 0);
+                                          a.drift_list, a.drift_count, *map, tma ? 1 : 0, MODE == 2 ? a.zgrid : nullptr, a.zcount4);
     return cudaSuccess;
 }
 template <int EY, int EZ>

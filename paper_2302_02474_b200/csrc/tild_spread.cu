@@ -347,8 +347,13 @@ int tild_spread_configure(tild_ctx* c)
 // X4 must be segment-sorted with the offsets lay.seg_base.
 int launch_spread(tild_ctx* c, const SegLayout& lay, const float4* X4, float* grid)
 {
-    TILD_CUDA(c, cudaMemsetAsync(grid, 0, sizeof(float) * c->M * c->mesh.S, c->stream));
-    if (c->mesh.n == 0) return TILD_OK;
+    // the library's own grid comes back cleared from the fused step (interp_drift_kernel); anything else is cleared here
+    if (!(grid == c->grid && c->grid_clean)) TILD_CUDA(c, cudaMemsetAsync(grid, 0, sizeof(float) * c->M * c->mesh.S, c->stream));
+    if (grid == c->grid) c->grid_clean = false;
+    if (c->mesh.n == 0) {
+        if (grid == c->grid) c->grid_clean = true;
+        return TILD_OK;
+    }
     const TileParams& tp = c->tile;
     // P = 1 touches one node per particle: the per-particle kernel is faster than any tiling (profiles/r1_c5_sweep.md)
     if (!tp.enabled || c->mesh.P == 1 || (c->prm.flags & TILD_FLAG_NAIVE_SPREAD)) return spread_slots(c, 0, (size_t)c->mesh.n, X4, grid);

@@ -625,6 +625,39 @@ def test_cuda_graph_blocks_match_eager_stepping(grid, box):
     assert np.abs(min_image(outs[1][0] - ox, cfg.box)).max() <= 1e-4
 
 
+@pytest.mark.parametrize("eager", [True, False], ids=["eager", "graph"])
+def test_queries_between_steps_do_not_disturb_the_cleared_density_grid(eager):
+    """The fused step hands the density grid back cleared (the P = 4 tile kernel clears it for the next spread, so no
+    memset runs in front of the spread); tild_energy / tild_structure_factor / tild_get_state(f) spread into the same grid
+    in between.  A trajectory with such calls in it must agree with one without to the rounding noise of the fp32 global
+    reductions (halo nodes are flushed by several tiles in any order), and with the oracle."""
+    cfg = small_cfg(order=4, grid=(32, 32, 48), box=(16.0, 16.0, 24.0), n_chains=600)
+    st = inputs.make_state(cfg)
+    side = torch.cuda.Stream()
+    outs = []
+    for probe in (False, True):
+        with torch.cuda.stream(side):
+            eng = tild.Tild(tild.params_from_config(cfg, flags=tild.FLAG_EAGER if eager else 0, resort_every=4), stream=side)
+            eng.tild_set_state(dev(st.x), dev(st.v), dev(st.type), dev(st.bond_partner), 0)
+            for k in range(3):
+                eng.tild_step(11)
+                if probe:
+                    eng.tild_energy()
+                    eng.tild_structure_factor(1)
+                    eng.tild_get_state()
+            x, v, _, step = eng.tild_get_state()
+        side.synchronize()
+        assert step == 33
+        assert eng.tild_layout_info()["tiles"] > 1
+        outs.append((x.cpu().numpy(), v.cpu().numpy()))
+    assert np.abs(min_image(outs[0][0].astype(np.float64) - outs[1][0], cfg.box)).max() < 2e-5
+    assert np.abs(outs[0][1].astype(np.float64) - outs[1][1]).max() < 1e-3
+    p = oracle_params(cfg)
+    ox, _, _ = orc.run(p, st.x.astype(np.float64), st.v.astype(np.float64), st.type, st.bond_partner, 0, 33)
+    for x, _ in outs:
+        assert np.abs(min_image(x.astype(np.float64) - ox, cfg.box)).max() <= 1e-4
+
+
 def test_contexts_sharing_a_kernel_instantiation_keep_their_shared_memory_limits():
     """the dynamic shared-memory limit is per kernel function, process-wide.  An S = 2 engine needs more for
     the spread kernel than an S = 1 engine with the same P and tile: creating the second must not break the first."""
