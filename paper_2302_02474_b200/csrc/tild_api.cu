@@ -523,6 +523,12 @@ void tild_destroy(tild_ctx* c)
         cufftDestroy(c->plan_x_c2r);
     }
     if (c->graph_ok) cudaGraphExecDestroy(c->graph_exec);
+    if (c->copy_stream) {
+        cudaStreamSynchronize(c->copy_stream);
+        for (int k = 0; k < 2; ++k)
+            if (c->copy_ev[k]) cudaEventDestroy(c->copy_ev[k]);
+        cudaStreamDestroy(c->copy_stream);
+    }
     if (c->ev_ok)
         for (int i = 0; i < TILD_MAX_TIMED_STEPS; ++i)
             for (int k = 0; k < TILD_N_STAGE_EVENTS; ++k) cudaEventDestroy(c->ev[i][k]);
@@ -795,13 +801,28 @@ int tild_get_state(tild_ctx* c, float* x, float* v, float* f, uint64_t* step)
     const int a = c->cur;
     float* scratch = reinterpret_cast<float*>(c->SX4);  // [n][3] staging in caller order; x/v/f may be host pointers
     int rc;
+    const bool need_force = f || (v && c->stp.kick_in != 0.0f);   // v = w + (dt/2m) F needs F(x); right after tild_set_state the state is v itself
+    bool x_in_flight = false;
     if (x) {
         if ((rc = launch_unpermute(c, c->X4[a], scratch))) return rc;
-        TILD_CUDA(c, cudaMemcpyAsync(x, scratch, bytes, cudaMemcpyDefault, c->stream));
+        // large systems: the copy of x (PCIe when x is a host pointer) runs on a second stream under the force evaluation
+        if (need_force && n >= (size_t)1 << 18 && c->stream != nullptr && c->stream != cudaStreamLegacy) {
+            if (!c->copy_stream) {
+                TILD_CUDA(c, cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
+                for (int k = 0; k < 2; ++k) TILD_CUDA(c, cudaEventCreateWithFlags(&c->copy_ev[k], cudaEventDisableTiming));
+            }
+            TILD_CUDA(c, cudaEventRecord(c->copy_ev[0], c->stream));
+            TILD_CUDA(c, cudaStreamWaitEvent(c->copy_stream, c->copy_ev[0], 0));
+            TILD_CUDA(c, cudaMemcpyAsync(x, scratch, bytes, cudaMemcpyDefault, c->copy_stream));
+            TILD_CUDA(c, cudaEventRecord(c->copy_ev[1], c->copy_stream));
+            x_in_flight = true;
+        } else {
+            TILD_CUDA(c, cudaMemcpyAsync(x, scratch, bytes, cudaMemcpyDefault, c->stream));
+        }
     }
-    if (f || (v && c->stp.kick_in != 0.0f)) {   // v = w + (dt/2m) F needs F(x); right after tild_set_state the state is v itself
-        if ((rc = force_current(c))) return rc;
-    }
+    if (need_force) rc = force_current(c);
+    if (x_in_flight) TILD_CUDA(c, cudaStreamWaitEvent(c->stream, c->copy_ev[1], 0));   // scratch is reused below; stream order for the caller
+    if (rc) return rc;
     if (v || f) {
         if (f) {
             if ((rc = launch_unpermute(c, c->F4, scratch))) return rc;

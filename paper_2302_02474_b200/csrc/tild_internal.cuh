@@ -157,6 +157,8 @@ struct tild_ctx {
 
     bool has_state;
     bool step_advanced;   // the last launch_interp advanced the device step counter itself (tile path)
+    cudaStream_t copy_stream = nullptr;   // tild_get_state: x goes to the host while F(x) is evaluated for v
+    cudaEvent_t copy_ev[2] = {nullptr, nullptr};
     bool grid_clean = false;        // c->grid is all zero: the drift kernel of the fused step cleared it for the next spread
     bool graph_leaves_clean = false;
     uint64_t step;
