@@ -254,18 +254,64 @@ __global__ void __launch_bounds__(ST, 2) spread_rot_kernel(MeshParams m, TilePar
             }
         }
     };
-    if (!check) {
-        flush(std::false_type(), FIX_INV);
-        return;
-    }
-    flush(std::true_type(), FIX_INV);
-    {
+#ifdef TILD_SROT_BULK_FLUSH
+    // Bulk flush (measured, not the default): the image is converted to fp32 in place and every row goes to the mesh as one
+    // (two across the periodic boundary in z) cp.reduce.async.bulk -- an fp32 add of 160 contiguous bytes done by the copy
+    // engine in L2 -- instead of one RED per node issued by the SM.  Needs 16-byte rows: Nz % 4 == 0 (the image then starts
+    // on a 16-byte boundary of the mesh rows, TileParams::sh) and an aligned grid.  C4: spread 0.2416 ms against 0.2382 ms for
+    // the RED loop below, and 0.1887 ms with no flush at all: the flush is bound by the fp32 adds in L2 (137 M per step) and
+    // the read-modify-write of the grid lines, not by who issues them (profiles/r2_variants.md).
+    if (m.N[2] % 4 == 0 && EZ <= m.N[2] && (reinterpret_cast<uintptr_t>(grid) & 15) == 0) {   // uniform
+        const int n4 = nsp * E3 / 4;
+        uint4* v4 = reinterpret_cast<uint4*>(sm);
+        for (int k = threadIdx.x; k < n4; k += ST) {
+            const uint4 u = v4[k];
+            if (check) tile_sum += (unsigned long long)u.x + u.y + u.z + u.w;
+            reinterpret_cast<float4*>(sm)[k] = make_float4((float)u.x * FIX_INV, (float)u.y * FIX_INV, (float)u.z * FIX_INV, (float)u.w * FIX_INV);
+        }
+        const int gz0 = wrap_idx(o[2], m.N[2]);
+        const int len1 = min(EZ, m.N[2] - gz0);      // floats before the periodic boundary; a multiple of 4
+        auto bulk_rows = [&]() {
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // the image was written through the generic proxy
+            __syncthreads();
+            for (int r = threadIdx.x; r < nsp * SEX * EY; r += ST) {
+                const int spl = r / (SEX * EY), q = r - spl * (SEX * EY);
+                if (q % EY >= E[1]) continue;        // rows of the template image this tile shape does not use
+                float* g = grid + (size_t)(sp0 + spl) * m.M + rowoff[q];
+                const unsigned src = (unsigned)__cvta_generic_to_shared(sm + spl * E3 + q * EZ);
+                asm volatile("cp.reduce.async.bulk.global.shared::cta.bulk_group.add.f32 [%0], [%1], %2;" ::"l"(g + gz0), "r"(src), "r"(4 * len1)
+                             : "memory");
+                if (len1 < EZ)
+                    asm volatile("cp.reduce.async.bulk.global.shared::cta.bulk_group.add.f32 [%0], [%1], %2;" ::"l"(g), "r"(src + 4u * len1),
+                                 "r"(4 * (EZ - len1))
+                                 : "memory");
+            }
+            asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+            asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");   // the engine has read the image
+        };
+        bulk_rows();
+        if (!check) return;
         const unsigned long long total = block_sum_u64(tile_sum, red);
         const unsigned long long cntp = block_sum_u64((unsigned long long)n_tile, red);
         const unsigned long long expect = cntp << FIX_BITS, slack = 64ull * cntp + 64ull;
         if (total + slack >= expect && total <= expect + slack) return;   // uniform across the block
+        __syncthreads();
+        for (int k = threadIdx.x; k < nsp * E3; k += ST) sm[k] ^= 0x80000000u;   // undo the wrapped tile: add the negated image
+        bulk_rows();
+    } else
+#endif
+    {
+        if (!check) {
+            flush(std::false_type(), FIX_INV);
+            return;
+        }
+        flush(std::true_type(), FIX_INV);
+        const unsigned long long total = block_sum_u64(tile_sum, red);
+        const unsigned long long cntp = block_sum_u64((unsigned long long)n_tile, red);
+        const unsigned long long expect = cntp << FIX_BITS, slack = 64ull * cntp + 64ull;
+        if (total + slack >= expect && total <= expect + slack) return;   // uniform across the block
+        flush(std::false_type(), -FIX_INV);              // undo the wrapped tile
     }
-    flush(std::false_type(), -FIX_INV);              // undo the wrapped tile
     // a node wrapped past 2^32 (>= 512 particles' worth on one node): redo this tile with fp32 global atomics
     for (uint32_t i = p_lo + threadIdx.x; i < p_hi; i += ST) {
         const float4 p = X4[i];
