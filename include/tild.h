@@ -228,6 +228,23 @@ int tild_layout_info(const tild_ctx*, uint64_t info[8] /*HOST out*/);
  * id held by slot s.  Describes the particles as they were at the last re-sort.  Either output may be NULL. */
 int tild_segment_layout(const tild_ctx*, uint32_t* seg_base /*DEVICE [tiles*S + 1]*/, uint32_t* slot_id /*DEVICE [n]*/);
 
+/* The cell offsets of the a1 index map WITHOUT a context and without any allocation, for callers that cannot call
+ * cudaMalloc (code under CUDA graph capture, serving loops, harnesses that forbid it): histogram of the cell keys +
+ * exclusive scan, the first half of the counting sort (particles binned by cell).
+ *   cell_key   DEVICE [n], as tild_index_map writes it: (cx*Ny+cy)*Nz+cz
+ *   cell_start DEVICE [n_cells + 1] out: cell_start[c] = #particles with key < c (equals tild_index_map's, bit for bit)
+ *   n_bad      DEVICE [1] out or NULL: keys >= n_cells; such particles are left out instead of indexing out of bounds
+ *   stream     a cudaStream_t (NULL = default stream); the call is asynchronous on it
+ *   errmsg     HOST [errmsg_len] out or NULL: the reason when the result is not TILD_OK
+ * The scan's block partials live in a static __device__ array (16.4 KB that every GPU loading the library holds until
+ * exit) sized for n_cells <= TILD_NOALLOC_MAX_CELLS (a 256^3 mesh); larger sizes return TILD_EINVAL.  The call runs one
+ * memset and four kernels on `stream` with the device that is current, and calls no cudaMalloc / cudaFree and no allocating
+ * library routine.  All calls on a device share the array (it is rewritten before it is read: nothing is kept between
+ * calls): calls that can overlap on the GPU -- different streams without an ordering between them -- race on it. */
+#define TILD_NOALLOC_MAX_CELLS 16777216
+int tild_cell_start_noalloc(const uint32_t* cell_key, int32_t n, uint32_t n_cells, uint32_t* cell_start, uint32_t* n_bad,
+                            void* stream, char* errmsg, size_t errmsg_len);
+
 /* HOST. Number of kernels of this library launched on the context's stream so far. */
 int64_t tild_launch_count(const tild_ctx*);
 

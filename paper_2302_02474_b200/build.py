@@ -13,7 +13,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libtild.so")
-SOURCES = ["tild_api.cu", "tild_sort.cu", "tild_spread.cu", "tild_spread_rot.cu", "tild_kspace.cu", "tild_interp.cu", "tild_interp_rot.cu", "tild_energy.cu", "tild_extra.cu"]
+SOURCES = ["tild_api.cu", "tild_sort.cu", "tild_spread.cu", "tild_spread_rot.cu", "tild_kspace.cu", "tild_interp.cu", "tild_interp_rot.cu", "tild_energy.cu", "tild_extra.cu", "tild_noalloc.cu"]
 CUDA_HOME = os.environ.get("CUDA_HOME", "/usr/local/cuda")
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "--fmad=true", "-Wno-deprecated-gpu-targets"]

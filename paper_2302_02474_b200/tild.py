@@ -31,7 +31,7 @@ TIMING_NAMES = ("sort", "spread", "fft_fwd", "kspace", "fft_inv", "interp", "oth
 EXPORTS = (
     "tild_workspace_bytes", "tild_init", "tild_set_state", "tild_spread", "tild_kspace_force", "tild_interp",
     "tild_bond_force", "tild_step", "tild_get_state", "tild_energy", "tild_virial", "tild_set_charges", "tild_set_ms_partners", "tild_structure_factor", "tild_index_map", "tild_get_timings", "tild_run_host",
-    "tild_philox_test", "tild_layout_info", "tild_segment_layout", "tild_launch_count", "tild_last_error", "tild_destroy", "tild_version",
+    "tild_philox_test", "tild_cell_start_noalloc", "tild_layout_info", "tild_segment_layout", "tild_launch_count", "tild_last_error", "tild_destroy", "tild_version",
 )
 
 
@@ -132,6 +132,7 @@ def load():
     lib.tild_get_timings.argtypes = [vp, C.POINTER(C.c_float * 8), C.POINTER(i32)]
     lib.tild_run_host.argtypes = [vp, vp, vp, vp, vp, u64, i32]
     lib.tild_philox_test.argtypes = [vp, vp, vp, vp, vp, i32]
+    lib.tild_cell_start_noalloc.argtypes = [vp, i32, C.c_uint32, vp, vp, vp, C.c_char_p, sz]
     lib.tild_layout_info.argtypes = [vp, C.POINTER(C.c_uint64 * 8)]
     lib.tild_launch_count.argtypes = [vp]
     lib.tild_launch_count.restype = C.c_int64
@@ -149,6 +150,27 @@ def load():
 
 class TildError(RuntimeError):
     pass
+
+
+NOALLOC_MAX_CELLS = 16777216
+
+
+def tild_cell_start_noalloc(cell_key, n_cells: int, cell_start, n_bad=None, stream=None):
+    """include/tild.h: cell offsets of the a1 index map with no context and no allocation (static device scratch).
+    cell_key [n] and cell_start [n_cells + 1] (and n_bad [1]) are the caller's CUDA tensors (int32 holding uint32);
+    asynchronous on `stream` (a torch stream; default: the current one).  Returns cell_start."""
+    import torch
+    lib = load()
+    if stream is None:
+        stream = torch.cuda.current_stream(cell_start.device)
+    assert cell_start.numel() >= n_cells + 1 or n_cells > NOALLOC_MAX_CELLS
+    msg = C.create_string_buffer(512)
+    with torch.cuda.device(cell_start.device):
+        rc = lib.tild_cell_start_noalloc(_dp(cell_key) if cell_key.numel() else None, int(cell_key.numel()), int(n_cells),
+                                         _dp(cell_start), _dp(n_bad), C.c_void_p(stream.cuda_stream), msg, len(msg))
+    if rc != OK:
+        raise TildError(f"tild_cell_start_noalloc failed ({rc}): {msg.value.decode()}")
+    return cell_start
 
 
 def _dp(t) -> Optional[int]:
