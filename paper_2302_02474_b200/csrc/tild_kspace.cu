@@ -53,7 +53,7 @@ __global__ void __launch_bounds__(256) kspace_kernel(KspaceParams k, size_t Mk, 
 
 
 // ---- fused x-transform variant --------------------------------------------------------------------------------------
-// The 3-D transforms are separable.  When Nx = 16, 32, 64, 128 or 256 and S <= 4 the mesh pipeline runs cuFFT only over
+// The 3-D transforms are separable.  When Nx = 16, 32, 48, 64, 96, 128, 192 or 256 and S <= 4 the mesh pipeline runs cuFFT only over
 // (y, z) -- batched 2-D R2C / C2R over the x planes -- and this kernel does, for 256 / R lines (ky, kz) at a time,
 //   forward FFT along x of the S densities -> the multiplication above -> inverse FFT along x of the 3S force spectra,
 // in registers (Nx = R1 R2: an R1- and an R2-point transform per line, one shared-memory transpose between them).  Against the
@@ -104,6 +104,56 @@ template <int SGN>
 struct RegFft<1, SGN> {
     static __device__ __forceinline__ void run(float2 (&)[1]) {}
 };
+
+// cos / sin of 2 pi j / 24, j = 0 .. 23 (twiddles of the radix-3 splits below)
+__host__ __device__ constexpr float cos24q(int j)   // first quadrant, j = 0 .. 6
+{
+    return j == 0 ? 1.0f : j == 1 ? 0.96592582628906829f : j == 2 ? 0.86602540378443865f : j == 3 ? 0.70710678118654752f
+         : j == 4 ? 0.5f : j == 5 ? 0.25881904510252076f : 0.0f;
+}
+__host__ __device__ constexpr float cos24(int j)
+{
+    return j <= 6 ? cos24q(j) : j <= 12 ? -cos24q(12 - j) : j <= 18 ? -cos24q(j - 12) : cos24q(24 - j);
+}
+__host__ __device__ constexpr float sin24(int j) { return cos24((j + 18) % 24); }   // sin x = cos(x - pi/2)
+
+// R = 3 * 2^m points (3, 6, 12, 24): three interleaved power-of-two transforms and a radix-3 butterfly,
+//   X[q + (R/3) s] = E0[q] + w3^s W_R^q E1[q] + w3^(2s) W_R^(2q) E2[q],  E_r = DFT of x[3 m + r],  w3 = exp(SGN 2 pi i / 3)
+template <int R, int SGN>
+struct RegFft3 {
+    static __device__ __forceinline__ void run(float2 (&v)[R])
+    {
+        constexpr int Q = R / 3;
+        float2 e[3][Q];
+#pragma unroll
+        for (int m = 0; m < Q; ++m) {
+            e[0][m] = v[3 * m];
+            e[1][m] = v[3 * m + 1];
+            e[2][m] = v[3 * m + 2];
+        }
+        RegFft<Q, SGN>::run(e[0]);
+        RegFft<Q, SGN>::run(e[1]);
+        RegFft<Q, SGN>::run(e[2]);
+        constexpr float C3 = -0.5f, S3 = (float)SGN * 0.86602540378443865f;   // w3 = C3 + i S3
+#pragma unroll
+        for (int q = 0; q < Q; ++q) {
+            const float c1 = cos24(q * (24 / R)), s1 = (float)SGN * sin24(q * (24 / R));
+            const float c2 = cos24(2 * q * (24 / R)), s2 = (float)SGN * sin24(2 * q * (24 / R));
+            const float2 t1 = q == 0 ? e[1][q] : make_float2(c1 * e[1][q].x - s1 * e[1][q].y, c1 * e[1][q].y + s1 * e[1][q].x);
+            const float2 t2 = q == 0 ? e[2][q] : make_float2(c2 * e[2][q].x - s2 * e[2][q].y, c2 * e[2][q].y + s2 * e[2][q].x);
+            const float2 sum = make_float2(t1.x + t2.x, t1.y + t2.y), dif = make_float2(t1.x - t2.x, t1.y - t2.y);
+            // E0 + w3 t1 + conj(w3) t2 = E0 + C3 (t1 + t2) + i S3 (t1 - t2); the third output has -S3
+            const float2 m = make_float2(e[0][q].x + C3 * sum.x, e[0][q].y + C3 * sum.y);
+            const float2 r = make_float2(-S3 * dif.y, S3 * dif.x);
+            v[q] = make_float2(e[0][q].x + sum.x, e[0][q].y + sum.y);
+            v[q + Q] = make_float2(m.x + r.x, m.y + r.y);
+            v[q + 2 * Q] = make_float2(m.x - r.x, m.y - r.y);
+        }
+    }
+};
+template <int SGN> struct RegFft<3, SGN> : RegFft3<3, SGN> {};
+template <int SGN> struct RegFft<6, SGN> : RegFft3<6, SGN> {};
+template <int SGN> struct RegFft<12, SGN> : RegFft3<12, SGN> {};
 
 // One length-N transform per line, N = R1 R2 (R1 <= R2), spread over R2 threads: Cooley-Tukey with the twiddle
 // exp(-/+ 2 pi i n2 k1 / N) between an R1-point and an R2-point pass and one shared-memory transpose.
@@ -272,14 +322,17 @@ int launch_kspace(tild_ctx* c, const float2* nhat, float2* fhat)
 int kspace_xfft_radix(int Nx, int S)
 {
     if (S > 4) return 0;   // S = 3, 4: one CTA per SM (the spectra of all species stay in registers)
-    return Nx == 256 || Nx == 128 ? 16 : Nx == 64 || Nx == 32 ? 8 : Nx == 16 ? 4 : 0;
+    return Nx == 256 || Nx == 128 || Nx == 192 || Nx == 96 ? 16 : Nx == 64 || Nx == 32 || Nx == 48 ? 8 : Nx == 16 ? 4 : 0;
 }
 
 // dispatch over (Nx, S): OP(R1, R2, S)
 #define TILD_XFFT_DISPATCH_S(N_, SS, OP)                                            \
     switch (N_) {                                                                   \
     case 256: OP(16, 16, SS); break;                                                \
+    case 192: OP(12, 16, SS); break;                                                \
     case 128: OP(8, 16, SS); break;                                                 \
+    case 96: OP(6, 16, SS); break;                                                  \
+    case 48: OP(6, 8, SS); break;                                                   \
     case 64: OP(8, 8, SS); break;                                                   \
     case 32: OP(4, 8, SS); break;                                                   \
     default: OP(4, 4, SS); break;                                                   \

@@ -51,7 +51,7 @@ def make(cfg, **kw):
 
 
 CASES = [small_cfg(order=P) for P in (1, 2, 3, 4, 5)] + [small_cfg(order=3, S=3, grid=(18, 12, 30), box=(9.0, 6.0, 15.0))]
-# Nx = 16, 32, 64, 128, 256: the fused x-transform k-space kernel (Nx = R1 R2), ragged (y, z) line counts, one and two species
+# Nx = 16, 32, 48, 64, 96, 128, 192, 256: the fused x-transform k-space kernel (Nx = R1 R2), ragged (y, z) line counts, one and two species
 XFFT_CASES = [small_cfg(order=3, grid=(16, 20, 18), box=(8.0, 10.0, 9.0)),
               small_cfg(order=4, grid=(64, 12, 10), box=(32.0, 6.0, 5.0)),
               small_cfg(order=2, grid=(256, 6, 10), box=(128.0, 3.0, 5.0), n_chains=400),
@@ -59,6 +59,11 @@ XFFT_CASES = [small_cfg(order=3, grid=(16, 20, 18), box=(8.0, 10.0, 9.0)),
               small_cfg(order=3, S=3, grid=(64, 12, 10), box=(32.0, 6.0, 5.0)),
               small_cfg(order=2, S=3, grid=(256, 6, 6), box=(128.0, 3.0, 3.0)),
               small_cfg(order=5, grid=(128, 8, 12), box=(64.0, 4.0, 6.0), n_chains=300),
+              # Nx = 48, 96, 192: radix-3 register transforms (6 x 8, 6 x 16, 12 x 16)
+              small_cfg(order=3, grid=(48, 10, 12), box=(24.0, 5.0, 6.0)),
+              small_cfg(order=4, grid=(96, 8, 10), box=(48.0, 4.0, 5.0), n_chains=300),
+              small_cfg(order=2, grid=(192, 6, 10), box=(96.0, 3.0, 5.0), n_chains=400),
+              small_cfg(order=3, S=3, grid=(192, 6, 8), box=(96.0, 3.0, 4.0)),
               small_cfg(order=3, grid=(64, 9, 7), box=(32.0, 4.5, 3.5), chi=((0.0,),), n_species=1,
                         chains=(inputs.ChainSpec(300, ((0, 5),)),), n=1500)]
 CASES = CASES + XFFT_CASES
