@@ -246,23 +246,51 @@ def ours_arm(args, cfg):
     stage_ms, nst = eng.tild_get_timings()
     value = aggregate_value(cfg.n, args.steps, world, ms_total)
 
-    # end to end through the C-ABI with HOST buffers: every step copies the batch in and the result out
+    # end to end through the C-ABI with HOST buffers: every step copies the batch in and the result out.  Two figures: the
+    # pipelined calls (tild_run_host_submit / _wait: the copies of consecutive, independent batches overlap the kernels) and
+    # the synchronous tild_run_host (one batch at a time, nothing overlaps)
     e2e = None
     if not args.no_e2e:
         xh, vh = torch.from_numpy(st.x.copy()).pin_memory(), torch.from_numpy(st.v.copy()).pin_memory()
         th, bh = torch.from_numpy(st.type.copy()).pin_memory(), torch.from_numpy(st.bond_partner.copy()).pin_memory()
+        xo = [torch.empty_like(xh).pin_memory() for _ in range(3)]
+        vo = [torch.empty_like(vh).pin_memory() for _ in range(3)]
         reps = max(1, min(args.steps, args.e2e_steps))
-        eng.tild_run_host(xh, vh, th, bh, 0, 1)    # warm-up
+        # a context on a stream of its own (the copy streams must not synchronise with the legacy default stream), no stage timers
+        side = torch.cuda.Stream(device=f"cuda:{local}")
+        eng_t, eng = eng, tild.Tild(tild.params_from_config(cfg, flags=tild.FLAG_HOST_PIPELINE | args.flags, seed=ph_seed,
+                                                           resort_every=args.resort_every, tile_shape=args.tile_shape),
+                                    device=f"cuda:{local}", stream=side)
+        eng.tild_run_host_submit(xh, vh, th, bh, 0, 1, xo[0], vo[0])    # warm-up
+        eng.tild_run_host_wait()
         barrier()
         t0 = time.perf_counter()
         for r in range(reps):
-            eng.tild_run_host(xh, vh, th, bh, r, 1)   # synchronous: H2D + set_state + 1 step + D2H
+            eng.tild_run_host_submit(xh, vh, th, bh, r, 1, xo[r % 3], vo[r % 3])   # H2D + set_state + 1 step + read-out + D2H
+            if r >= 2:
+                eng.tild_run_host_wait()                 # results of batch r - 2 are in host memory
+        for _ in range(min(reps, 2)):
+            eng.tild_run_host_wait()
         barrier()
         dt = max_over_ranks(dist, time.perf_counter() - t0, "cuda")
+        xs_, vs_ = xh.clone().pin_memory(), vh.clone().pin_memory()
+        sreps = max(1, min(reps, 3))
+        eng.tild_run_host(xs_, vs_, th, bh, 0, 1)    # warm-up
+        barrier()
+        t0 = time.perf_counter()
+        for r in range(sreps):
+            eng.tild_run_host(xs_, vs_, th, bh, r, 1)
+        barrier()
+        dts = max_over_ranks(dist, time.perf_counter() - t0, "cuda")
+        eng.close()
+        eng = eng_t
         e2e = {"value": world * cfg.n * reps / dt, "unit": UNIT,
                "h2d_bytes_per_step": int(xh.nbytes + vh.nbytes + th.nbytes + bh.nbytes),
                "d2h_bytes_per_step": int(xh.nbytes + vh.nbytes), "steps": reps,
-               "note": "tild_run_host(nsteps=1) per step: H2D of (x,v,type,bonds), sort, F(x), one step, v/x read back"}
+               "synchronous": {"value": world * cfg.n * sreps / dts, "steps": sreps,
+                               "note": "tild_run_host(nsteps=1): one batch at a time, copies and kernels one after the other"},
+               "note": "tild_run_host_submit(nsteps=1) + tild_run_host_wait per step, up to three batches in flight: H2D of (x,v,type,bonds), "
+                       "sort, one step, F(x) for v, v/x read back; copies of consecutive batches overlap the kernels"}
 
     if rank != 0:
         return
@@ -364,7 +392,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="C4", choices=sorted(inputs.CONFIGS))
     ap.add_argument("--resort-every", type=int, default=0)
-    ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--e2e-steps", type=int, default=8)
     ap.add_argument("--flags", type=int, default=0, help="extra TILD_FLAG_* bits (kernel A/B runs)")
     ap.add_argument("--tile-shape", type=int, default=0, help="tild_params.tile_shape = TY | TZ << 8 (0 = default 8x16x32)")
     ap.add_argument("--no-e2e", action="store_true")

@@ -72,6 +72,7 @@ typedef enum {
 #define TILD_FLAG_EXTRAS 1024u     /* reserve workspace and plans for the extra mesh interactions: per-particle charges
                                       (tild_set_charges) and the Maier-Saupe interaction (mu_ms, tild_set_ms_partners) */
 #define TILD_FLAG_NO_TMA 2048u     /* stage every tile image with cp.async, also where a TMA box applies (A/B runs) */
+#define TILD_FLAG_HOST_PIPELINE 8192u /* workspace for tild_run_host_submit / _wait: device staging of one input and two output batches */
 #define TILD_FLAG_GEN1_TILES 128u   /* first-generation tile kernels (32 bank classes with overflow rounds, per-particle work
                                       in class order) even where the rotation-class kernels apply (P = 4); for A/B runs */
 
@@ -211,6 +212,18 @@ int tild_get_timings(tild_ctx*, float ms[8] /*HOST out*/, int32_t* steps_timed /
  * runs tild_set_state + tild_step(nsteps), copies (x, v) back.  Buffers should be pinned for speed. */
 int tild_run_host(tild_ctx*, float* x_host, float* v_host, const int32_t* type_host,
                   const int32_t* bond_partner_host, uint64_t step0, int32_t nsteps);
+
+/* HOST buffers: the pipelined end-to-end path for INDEPENDENT batches (needs TILD_FLAG_HOST_PIPELINE and a context on a
+ * stream of its own).  tild_run_host_submit copies one batch host->device on a copy stream, runs tild_set_state +
+ * tild_step(nsteps) + the read-out on the context's stream and starts the copy of (x, v) to x_out_host / v_out_host on a
+ * second copy stream; it returns once the inputs have been consumed (they may be reused), not when the results are there.
+ * tild_run_host_wait blocks until the results of the oldest batch not yet waited for are in its output buffers
+ * (TILD_ESTATE if there is none; at most four batches may be in flight).  Calling submit again before wait overlaps the three phases of consecutive batches;
+ * outputs of a batch are valid only after its wait.  Buffers should be pinned.  The context's state after a submit is
+ * that batch's; tild_step / tild_get_state may follow, stage calls too. */
+int tild_run_host_submit(tild_ctx*, const float* x_host, const float* v_host, const int32_t* type_host,
+                         const int32_t* bond_partner_host, uint64_t step0, int32_t nsteps, float* x_out_host, float* v_out_host);
+int tild_run_host_wait(tild_ctx*);
 
 /* Test hook: out[i] = Philox4x32-10(counter = ctr[i], key = key[i]) computed by the same device
  * function the integrator uses; gauss[i] = the three N(0,1) draws for (id = ctr[i].x, step =

@@ -159,6 +159,13 @@ struct tild_ctx {
     bool step_advanced;   // the last launch_interp advanced the device step counter itself (tile path)
     cudaStream_t copy_stream = nullptr;   // tild_get_state: x goes to the host while F(x) is evaluated for v
     cudaEvent_t copy_ev[2] = {nullptr, nullptr};
+    // tild_run_host_submit / _wait (TILD_FLAG_HOST_PIPELINE): device staging of the host batches and the streams of the copies
+    float *hp_x = nullptr, *hp_v = nullptr;          // input staging [n][3] (one set: tild_set_state has consumed it when submit returns)
+    int32_t *hp_t = nullptr, *hp_b = nullptr;        // [n], [n][max_bonds]
+    float *hp_xo[2] = {nullptr, nullptr}, *hp_vo[2] = {nullptr, nullptr};   // output staging, one set per batch in flight
+    cudaStream_t hp_in = nullptr, hp_out = nullptr;
+    cudaEvent_t hp_ev_in = nullptr, hp_ev_done = nullptr, hp_ev_out[4] = {nullptr, nullptr, nullptr, nullptr};   // ev_out: one per batch, ring of 4
+    uint64_t hp_submitted = 0, hp_waited = 0;
     bool grid_clean = false;        // c->grid is all zero: the drift kernel of the fused step cleared it for the next spread
     bool graph_leaves_clean = false;
     uint64_t step;

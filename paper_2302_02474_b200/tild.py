@@ -26,11 +26,12 @@ FLAG_EAGER = 256
 FLAG_2D = 512
 FLAG_EXTRAS = 1024
 FLAG_NO_TMA = 2048
+FLAG_HOST_PIPELINE = 8192
 TIMING_NAMES = ("sort", "spread", "fft_fwd", "kspace", "fft_inv", "interp", "other", "total")
 
 EXPORTS = (
     "tild_workspace_bytes", "tild_init", "tild_set_state", "tild_spread", "tild_kspace_force", "tild_interp",
-    "tild_bond_force", "tild_step", "tild_get_state", "tild_energy", "tild_virial", "tild_set_charges", "tild_set_ms_partners", "tild_structure_factor", "tild_index_map", "tild_get_timings", "tild_run_host",
+    "tild_bond_force", "tild_step", "tild_get_state", "tild_energy", "tild_virial", "tild_set_charges", "tild_set_ms_partners", "tild_structure_factor", "tild_index_map", "tild_get_timings", "tild_run_host", "tild_run_host_submit", "tild_run_host_wait",
     "tild_philox_test", "tild_cell_start_noalloc", "tild_layout_info", "tild_segment_layout", "tild_launch_count", "tild_last_error", "tild_destroy", "tild_version",
 )
 
@@ -131,6 +132,8 @@ def load():
     lib.tild_segment_layout.argtypes = [vp, vp, vp]
     lib.tild_get_timings.argtypes = [vp, C.POINTER(C.c_float * 8), C.POINTER(i32)]
     lib.tild_run_host.argtypes = [vp, vp, vp, vp, vp, u64, i32]
+    lib.tild_run_host_submit.argtypes = [vp, vp, vp, vp, vp, u64, i32, vp, vp]
+    lib.tild_run_host_wait.argtypes = [vp]
     lib.tild_philox_test.argtypes = [vp, vp, vp, vp, vp, i32]
     lib.tild_cell_start_noalloc.argtypes = [vp, i32, C.c_uint32, vp, vp, vp, C.c_char_p, sz]
     lib.tild_layout_info.argtypes = [vp, C.POINTER(C.c_uint64 * 8)]
@@ -315,6 +318,17 @@ class Tild:
             assert t is None or t.device.type == "cpu"
         self._check(self.lib.tild_run_host(self.ctx, _dp(x_host), _dp(v_host), _dp(type_host), _dp(bond_host),
                                            step0, int(nsteps)), "tild_run_host")
+
+    def tild_run_host_submit(self, x_host, v_host, type_host, bond_host, step0: int, nsteps: int, x_out_host, v_out_host):
+        """Pipelined tild_run_host for independent batches (FLAG_HOST_PIPELINE): returns when the inputs are consumed;
+        the outputs are valid after the matching tild_run_host_wait()."""
+        for t in (x_host, v_host, type_host, bond_host, x_out_host, v_out_host):
+            assert t is None or t.device.type == "cpu"
+        self._check(self.lib.tild_run_host_submit(self.ctx, _dp(x_host), _dp(v_host), _dp(type_host), _dp(bond_host), step0, int(nsteps),
+                                                  _dp(x_out_host), _dp(v_out_host)), "tild_run_host_submit")
+
+    def tild_run_host_wait(self):
+        self._check(self.lib.tild_run_host_wait(self.ctx), "tild_run_host_wait")
 
     def tild_philox_test(self, ctr, key, want_gauss: bool = True):
         t = self.torch

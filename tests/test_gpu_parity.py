@@ -336,6 +336,45 @@ def test_run_host_end_to_end_matches_device_path():
     assert np.abs(vh.numpy() - v2.cpu().numpy()).max() < 1e-3
 
 
+def test_pipelined_run_host_matches_the_synchronous_call():
+    """tild_run_host_submit / _wait: four independent batches (different inputs and step counts) submitted back to back,
+    each compared with the synchronous tild_run_host of the same batch; the input buffers are reused right after submit."""
+    cfg = small_cfg(order=4, grid=(32, 32, 48), box=(16.0, 16.0, 24.0), n_chains=600)
+    side = torch.cuda.Stream()
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    states = [inputs.make_state(cfg, seed=11 + k) for k in range(4)]
+    rng = np.random.default_rng(3)
+    batches = []
+    for k, st in enumerate(states):
+        x = np.mod(st.x + rng.normal(0.0, 0.05 * (k + 1), st.x.shape), np.asarray(cfg.box)).astype(np.float32)   # distinct batches
+        batches.append((x, st.v * (1.0 + 0.1 * k), st.type, st.bond_partner, 7 * k, 3 + k))
+    ref = []
+    with torch.cuda.stream(side):
+        eng0 = tild.Tild(tild.params_from_config(cfg), stream=side)
+        for x, v, t, b, step0, ns in batches:
+            xh, vh = pin(x.copy()), pin(v.astype(np.float32).copy())
+            eng0.tild_run_host(xh, vh, pin(t), pin(b), step0, ns)
+            ref.append((xh.numpy().copy(), vh.numpy().copy()))
+        eng = tild.Tild(tild.params_from_config(cfg, flags=tild.FLAG_HOST_PIPELINE), stream=side)
+        xin, vin, tin, bin_ = pin(batches[0][0].copy()), pin(batches[0][1].astype(np.float32).copy()), pin(batches[0][2].copy()), pin(batches[0][3].copy())
+        outs = [(torch.empty_like(xin).pin_memory(), torch.empty_like(vin).pin_memory()) for _ in batches]
+        for k, (x, v, t, b, step0, ns) in enumerate(batches):
+            xin.copy_(torch.from_numpy(x)); vin.copy_(torch.from_numpy(v.astype(np.float32)))   # the same input buffers every time
+            tin.copy_(torch.from_numpy(t)); bin_.copy_(torch.from_numpy(b))
+            eng.tild_run_host_submit(xin, vin, tin, bin_, step0, ns, outs[k][0], outs[k][1])
+            if k >= 2:
+                eng.tild_run_host_wait()
+        eng.tild_run_host_wait()
+        eng.tild_run_host_wait()
+        with pytest.raises(tild.TildError):
+            eng.tild_run_host_wait()                      # nothing in flight
+        with pytest.raises(tild.TildError):
+            eng0.tild_run_host_submit(xin, vin, tin, bin_, 0, 1, outs[0][0], outs[0][1])   # no FLAG_HOST_PIPELINE
+    for (xr, vr), (xo, vo) in zip(ref, outs):
+        assert np.abs(min_image(xo.numpy().astype(np.float64) - xr, cfg.box)).max() < 2e-5
+        assert np.abs(vo.numpy().astype(np.float64) - vr).max() < 1e-3
+
+
 # ---------------- kernel variants, fallbacks, full-size configs ----------------
 def test_naive_kernel_flags_match_oracle():
     cfg = small_cfg(order=4)
