@@ -139,6 +139,7 @@ void configure_tiles(tild_ctx* c)
     t.smem_interp = (size_t)t.E[0] * t.EY * 3 * t.EZ * sizeof(float) + lists_i;
     const size_t M = (size_t)p.grid[0] * p.grid[1] * p.grid[2];
     c->max_bins = M > (size_t)t.nseg ? M : (size_t)t.nseg;
+    if (c->max_bins < 2 * (size_t)t.nseg + 4) c->max_bins = 2 * (size_t)t.nseg + 4;   // re-sort: two arrays per segment in count / start
 }
 
 void carve(tild_ctx* c, void* base, size_t* total)
@@ -645,6 +646,7 @@ int tild_set_state(tild_ctx* c, const float* x, const float* v, const int32_t* t
     if (n > 0 && (!x || !v || !type)) return tild_fail(c, TILD_EINVAL, "tild_set_state: null argument");
     if (n > 0 && c->stp.max_bonds > 0 && !bond_partner) return tild_fail(c, TILD_EINVAL, "tild_set_state: null bond_partner");
     c->cur = 0;
+    c->lay_valid = false;                       // the first sort of a state has no order to keep
     c->has_state = false;
     TILD_CUDA(c, cudaMemsetAsync(c->drift_count, 0, 4 * sizeof(uint32_t), c->stream));
     int rc = launch_pack(c, x, v, type, c->stp.max_bonds > 0 ? bond_partner : nullptr, c->X4[0], c->W4[0], c->B[0]);

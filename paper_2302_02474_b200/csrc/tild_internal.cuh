@@ -166,6 +166,7 @@ struct tild_ctx {
     cudaStream_t hp_in = nullptr, hp_out = nullptr;
     cudaEvent_t hp_ev_in = nullptr, hp_ev_done = nullptr, hp_ev_out[4] = {nullptr, nullptr, nullptr, nullptr};   // ev_out: one per batch, ring of 4
     uint64_t hp_submitted = 0, hp_waited = 0;
+    bool lay_valid = false;         // c->lay describes the buffer X4[cur] (set by the first sort of a state): re-sorts keep the stayers' order
     bool grid_clean = false;        // c->grid is all zero: the drift kernel of the fused step cleared it for the next spread
     bool graph_leaves_clean = false;
     uint64_t step;

@@ -494,6 +494,58 @@ def test_segment_sort_of_the_timed_path_is_bit_exact(cfg):
     assert np.array_equal(oseg[ids], slot_seg)
 
 
+@pytest.mark.parametrize("arrival", [False, True], ids=["stable", "arrival"])
+def test_resort_keeps_the_order_of_particles_that_stay_in_their_segment(arrival):
+    """Re-sorts of the timed path (tild_sort.cu: launch_segment_resort): after every re-sort the layout must again be a
+    valid segment sort of the current positions (seg_base = prefix sums of the segment histogram, every slot in its
+    segment), and -- unless TILD_FLAG_ARRIVAL_SORT -- the particles that were in a segment before and after must keep
+    their relative order, with the ones that moved in behind them.  Large time step so that many particles change tiles."""
+    cfg = small_cfg(order=4, grid=(32, 32, 64), box=(8.0, 8.0, 16.0), n_chains=900)
+    st = inputs.make_state(cfg)
+    eng = tild.Tild(tild.params_from_config(cfg, resort_every=2, dt=0.02, flags=tild.FLAG_EAGER | (tild.FLAG_ARRIVAL_SORT if arrival else 0)))
+    eng.tild_set_state(dev(st.x), dev(st.v * 3.0), dev(st.type), dev(st.bond_partner), 0)
+    info = eng.tild_layout_info()
+    N = np.array(cfg.grid, dtype=np.int64)
+    T = np.array([info["tile_x"], info["tile_y"], info["tile_z"]], dtype=np.int64)
+    nt = (N + T - 1) // T
+    nseg = int(nt.prod()) * cfg.n_species
+    assert nseg >= 16
+
+    def layout():
+        seg, ids = eng.tild_segment_layout()
+        seg = seg.cpu().numpy().view(np.uint32).astype(np.int64)
+        ids = ids.cpu().numpy().view(np.uint32).astype(np.int64)
+        return seg, ids, np.searchsorted(seg, np.arange(cfg.n), side="right") - 1
+
+    seg0, ids0, sseg0 = layout()
+    moved_total = 0
+    for cycle in range(6):
+        eng.tild_step(3 if cycle == 0 else 2)        # the re-sort runs at the start of the step after resort_every steps
+        seg1, ids1, sseg1 = layout()
+        assert np.array_equal(np.sort(ids1), np.arange(cfg.n))
+        assert seg1[0] == 0 and seg1[-1] == cfg.n and np.all(np.diff(seg1) >= 0)
+        seg_of_id0 = np.empty(cfg.n, dtype=np.int64); seg_of_id0[ids0] = sseg0
+        slot_of_id0 = np.empty(cfg.n, dtype=np.int64); slot_of_id0[ids0] = np.arange(cfg.n)
+        stay = seg_of_id0[ids1] == sseg1             # per new slot: was this particle in the same segment before?
+        moved_total += int((~stay).sum())
+        if not arrival:
+            for g in range(nseg):
+                a, b = seg1[g], seg1[g + 1]
+                sl = slice(a, b)
+                old = slot_of_id0[ids1[sl]][stay[sl]]
+                assert np.all(np.diff(old) > 0), g                          # stayers in their old order
+                nstay = int(stay[sl].sum())
+                assert np.all(stay[a:a + nstay]) and not np.any(stay[a + nstay:b]), g   # movers behind them
+        seg0, ids0, sseg0 = seg1, ids1, sseg1
+    assert moved_total > 50                          # the test did exercise particles changing segments
+    # and the trajectory is the oracle's whatever the order in memory
+    x = eng.tild_get_state(want_v=False)[0].cpu().numpy().astype(np.float64)
+    from dataclasses import replace
+    p = oracle_params(replace(cfg, dt=0.02))
+    ox, _, _ = orc.run(p, st.x.astype(np.float64), (st.v * 3.0).astype(np.float64), st.type, st.bond_partner, 0, 13)
+    assert np.abs(min_image(x - ox, cfg.box)).max() <= 1e-4
+
+
 def test_layout_info_reports_the_tiling():
     cfg = inputs.C2
     st, eng = make(cfg)
