@@ -254,9 +254,32 @@ __global__ void __launch_bounds__(SPREAD_THREADS, 2) spread_tile_kernel(MeshPara
     constexpr int RPP = SPREAD_THREADS / EZ;               // rows per pass
     const int lz = threadIdx.x % EZ, r0 = threadIdx.x / EZ;
     const int gz = wrap_idx(o[2] + lz, m.N[2]);
+    // 16-byte rows (Nz % 4 == 0: the image starts on a 16-byte boundary of the mesh rows, TileParams::sh, and every aligned
+    // float4 of a row wraps as a whole): one vector reduction (red.global.add.v4.f32, REDG.E.ADD.F32x4) per four nodes
+    static_assert(EZ % 4 == 0, "image rows are whole float4s");
+    const bool vec4 = m.N[2] % 4 == 0 && (reinterpret_cast<uintptr_t>(grid) & 15) == 0 && (m.M % 4) == 0;
     for (int pass = 0; pass < 2; ++pass) {          // pass 1 only runs to undo a wrapped tile
         const float sc = pass == 0 ? FIX_INV : -FIX_INV;
-        if (r0 < RPP) {
+        if (vec4) {
+            constexpr int CPR = EZ / 4, RPP4 = SPREAD_THREADS / CPR;
+            const int c4 = threadIdx.x % CPR, rr = threadIdx.x / CPR;
+            const int gz4 = wrap_idx(o[2] + 4 * c4, m.N[2]);
+            if (rr < RPP4) {
+                for (int spl = 0; spl < nsp; ++spl) {
+                    float* gsp = grid + (size_t)(sp0 + spl) * m.M + gz4;
+                    const uint4* simg = reinterpret_cast<const uint4*>(sm + spl * E3) + c4;
+                    for (int q = rr; q < EX * EY; q += RPP4) {
+                        const uint4 u = simg[q * CPR];
+                        if (u.x | u.y | u.z | u.w) {
+                            if (pass == 0) tile_sum += (unsigned long long)u.x + u.y + u.z + u.w;
+                            asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(gsp + rowoff[q]), "f"((float)u.x * sc),
+                                         "f"((float)u.y * sc), "f"((float)u.z * sc), "f"((float)u.w * sc)
+                                         : "memory");
+                        }
+                    }
+                }
+            }
+        } else if (r0 < RPP) {
             for (int spl = 0; spl < nsp; ++spl) {
                 float* gsp = grid + (size_t)(sp0 + spl) * m.M + gz;
                 const uint32_t* simg = sm + spl * E3 + lz;

@@ -15,6 +15,9 @@
 
 namespace {
 
+#ifndef TILD_SROT_SCALAR_FLUSH
+#define TILD_SROT_SCALAR_FLUSH 0   // 1: one scalar RED per node also where the vector reduction applies (A/B)
+#endif
 #ifndef TILD_SROT_THREADS
 #define TILD_SROT_THREADS 512
 #define TILD_SROT_CHUNK 2048
@@ -240,7 +243,30 @@ __global__ void __launch_bounds__(ST, 2) spread_rot_kernel(MeshParams m, TilePar
     // A node can only wrap past 2^32 if >= 2^9 / (largest single-node weight) particles sit on it; the largest weight of
     // the cubic spline is (23/48)^3.  Tiles with fewer particles skip the check and the sum that feeds it.
     const bool check = p_hi - p_lo > 4653u;          // uniform across the block
+    // 16-byte rows (Nz % 4 == 0: the image starts on a 16-byte boundary of the mesh rows, TileParams::sh, and every aligned
+    // float4 of a row wraps as a whole): one vector reduction (red.global.add.v4.f32, REDG.E.ADD.F32x4) per four nodes
+    const bool vec4 = !TILD_SROT_SCALAR_FLUSH && m.N[2] % 4 == 0 && (reinterpret_cast<uintptr_t>(grid) & 15) == 0 && (m.M % 4) == 0;
     auto flush = [&](auto sum, const float sc) {
+        if (vec4) {
+            constexpr int CPR = EZ / 4, RPP4 = ST / CPR;
+            const int c4 = threadIdx.x % CPR, rr = threadIdx.x / CPR;
+            if (rr >= RPP4) return;
+            const int gz4 = wrap_idx(o[2] + 4 * c4, m.N[2]);
+            for (int spl = 0; spl < nsp; ++spl) {
+                float* gsp = grid + (size_t)(sp0 + spl) * m.M + gz4;
+                const uint4* simg = reinterpret_cast<const uint4*>(sm + spl * E3) + c4;
+                for (int q = rr; q < SEX * EY; q += RPP4) {
+                    const uint4 u = simg[q * CPR];
+                    if (u.x | u.y | u.z | u.w) {
+                        if (decltype(sum)::value) tile_sum += (unsigned long long)u.x + u.y + u.z + u.w;
+                        asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(gsp + rowoff[q]), "f"((float)u.x * sc),
+                                     "f"((float)u.y * sc), "f"((float)u.z * sc), "f"((float)u.w * sc)
+                                     : "memory");
+                    }
+                }
+            }
+            return;
+        }
         if (r0 >= RPP) return;
         for (int spl = 0; spl < nsp; ++spl) {
             float* gsp = grid + (size_t)(sp0 + spl) * m.M + gz;
