@@ -71,6 +71,31 @@ __host__ __device__ constexpr float sin16(int j)
          : j == 4 ? 1.0f : j == 5 ? 0.92387953251128674f : j == 6 ? 0.70710678118654752f : 0.38268343236508977f;
 }
 
+// complex add / subtract as one packed fp32 pair instruction (sm_100a FADD2: 384 of them replace 768 FADD in the 16 x 16
+// kernel; same rounding; C4 k-space stage 0.1265 -> 0.1251 ms).  TILD_KSPACE_NO_F32X2 builds the scalar form.
+__device__ __forceinline__ float2 cadd(float2 a, float2 b)
+{
+#ifndef TILD_KSPACE_NO_F32X2
+    float2 d;
+    asm("{.reg .b64 ra, rb, rd;\n mov.b64 ra, {%2, %3};\n mov.b64 rb, {%4, %5};\n add.rn.f32x2 rd, ra, rb;\n mov.b64 {%0, %1}, rd;}"
+        : "=f"(d.x), "=f"(d.y) : "f"(a.x), "f"(a.y), "f"(b.x), "f"(b.y));
+    return d;
+#else
+    return make_float2(a.x + b.x, a.y + b.y);
+#endif
+}
+__device__ __forceinline__ float2 csub(float2 a, float2 b)
+{
+#ifndef TILD_KSPACE_NO_F32X2
+    float2 d;
+    asm("{.reg .b64 ra, rb, rd;\n mov.b64 ra, {%2, %3};\n mov.b64 rb, {%4, %5};\n sub.rn.f32x2 rd, ra, rb;\n mov.b64 {%0, %1}, rd;}"
+        : "=f"(d.x), "=f"(d.y) : "f"(a.x), "f"(a.y), "f"(b.x), "f"(b.y));
+    return d;
+#else
+    return make_float2(a.x - b.x, a.y - b.y);
+#endif
+}
+
 // R-point DFT on registers, decimation in time: v[k] <- sum_n v[n] exp(SGN 2 pi i n k / R)
 template <int R, int SGN>
 struct RegFft {
@@ -95,8 +120,8 @@ struct RegFft {
                 const float wr = cos16(k * (16 / R)), wi = (float)SGN * sin16(k * (16 / R));
                 t = make_float2(wr * o[k].x - wi * o[k].y, wr * o[k].y + wi * o[k].x);
             }
-            v[k] = make_float2(e[k].x + t.x, e[k].y + t.y);
-            v[k + R / 2] = make_float2(e[k].x - t.x, e[k].y - t.y);
+            v[k] = cadd(e[k], t);
+            v[k + R / 2] = csub(e[k], t);
         }
     }
 };
@@ -141,13 +166,13 @@ struct RegFft3 {
             const float c2 = cos24(2 * q * (24 / R)), s2 = (float)SGN * sin24(2 * q * (24 / R));
             const float2 t1 = q == 0 ? e[1][q] : make_float2(c1 * e[1][q].x - s1 * e[1][q].y, c1 * e[1][q].y + s1 * e[1][q].x);
             const float2 t2 = q == 0 ? e[2][q] : make_float2(c2 * e[2][q].x - s2 * e[2][q].y, c2 * e[2][q].y + s2 * e[2][q].x);
-            const float2 sum = make_float2(t1.x + t2.x, t1.y + t2.y), dif = make_float2(t1.x - t2.x, t1.y - t2.y);
+            const float2 sum = cadd(t1, t2), dif = csub(t1, t2);
             // E0 + w3 t1 + conj(w3) t2 = E0 + C3 (t1 + t2) + i S3 (t1 - t2); the third output has -S3
             const float2 m = make_float2(e[0][q].x + C3 * sum.x, e[0][q].y + C3 * sum.y);
             const float2 r = make_float2(-S3 * dif.y, S3 * dif.x);
-            v[q] = make_float2(e[0][q].x + sum.x, e[0][q].y + sum.y);
-            v[q + Q] = make_float2(m.x + r.x, m.y + r.y);
-            v[q + 2 * Q] = make_float2(m.x - r.x, m.y - r.y);
+            v[q] = cadd(e[0][q], sum);
+            v[q + Q] = cadd(m, r);
+            v[q + 2 * Q] = csub(m, r);
         }
     }
 };
