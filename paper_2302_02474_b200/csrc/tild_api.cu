@@ -658,6 +658,7 @@ int tild_set_state(tild_ctx* c, const float* x, const float* v, const int32_t* t
         if (bad) return tild_fail(c, TILD_EINVAL, "tild_set_state: a type is outside [0, %d) or a bond partner outside [-1, %d)", c->mesh.S, c->mesh.n);
     }
     if ((rc = launch_reorder(c))) return rc;
+    c->resorts_since_defrag = 0;
     // The state array holds v itself until the first step: that step takes v^0 as it is (kick_in = 0) and leaves the
     // split-kick state w^1 = v^1 - (dt/2m) F^1 behind, so loading a state costs a sort and no force evaluation.
     c->stp.kick_in = 0.0f;
@@ -697,11 +698,12 @@ int fold_timings(tild_ctx* c)
 }
 
 // one TILD step on the internal state (re-sort when due, mesh pipeline, fused interpolation pass, step counter)
-int enqueue_one_step(tild_ctx* c, cudaEvent_t* ev)
+int enqueue_one_step(tild_ctx* c, cudaEvent_t* ev, bool allow_defrag)
 {
     if (ev) TILD_CUDA(c, cudaEventRecord(ev[0], c->stream));
     if (c->steps_since_sort >= c->resort_every) {
-        int rc = launch_reorder(c);
+        const bool defrag = allow_defrag && c->resorts_since_defrag >= TILD_DEFRAG_EVERY && !(c->prm.flags & TILD_FLAG_NO_DEFRAG);
+        int rc = defrag ? launch_defrag(c) : launch_reorder(c);
         if (rc) return rc;
     }
     if (ev) TILD_CUDA(c, cudaEventRecord(ev[1], c->stream));
@@ -740,21 +742,21 @@ int launch_graph_block(tild_ctx* c)
             c->graph_ok = false;
         }
         // capture: nothing executes, so the host bookkeeping the enqueue advances is put back afterwards
-        const int cur0 = c->cur, sss0 = c->steps_since_sort;
+        const int cur0 = c->cur, sss0 = c->steps_since_sort, rsd0 = c->resorts_since_defrag;
         const uint64_t step0 = c->step;
         const int64_t launches0 = c->launches;
         float4* const x0[2] = {c->X4[0], c->X4[1]};
         float4* const w0[2] = {c->W4[0], c->W4[1]};
         TILD_CUDA(c, cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal));
         int rc = TILD_OK;
-        for (int i = 0; i < block && rc == TILD_OK; ++i) rc = enqueue_one_step(c, nullptr);
+        for (int i = 0; i < block && rc == TILD_OK; ++i) rc = enqueue_one_step(c, nullptr, false);
         cudaGraph_t graph = nullptr;
         const cudaError_t e = cudaStreamEndCapture(c->stream, &graph);
         c->graph_launches = c->launches - launches0;
         c->graph_leaves_clean = c->grid_clean;
         c->grid_clean = true;   // nothing ran
         const bool same = c->cur == cur0 && c->X4[0] == x0[0] && c->W4[0] == w0[0] && c->steps_since_sort == sss0;
-        c->cur = cur0; c->steps_since_sort = sss0; c->step = step0; c->launches = launches0;
+        c->cur = cur0; c->steps_since_sort = sss0; c->step = step0; c->launches = launches0; c->resorts_since_defrag = rsd0;
         c->X4[0] = x0[0]; c->X4[1] = x0[1]; c->W4[0] = w0[0]; c->W4[1] = w0[1];
         if (rc != TILD_OK || e != cudaSuccess || !graph || !same) {
             if (graph) cudaGraphDestroy(graph);
@@ -772,6 +774,7 @@ int launch_graph_block(tild_ctx* c)
     TILD_CUDA(c, cudaGraphLaunch(c->graph_exec, c->stream));
     c->grid_clean = c->graph_leaves_clean;
     c->step += (uint64_t)block;          // pointers, cur and steps_since_sort end where they started
+    c->resorts_since_defrag += 2;
     c->launches += c->graph_launches;
     return TILD_OK;
 }
@@ -791,7 +794,11 @@ int tild_step(tild_ctx* c, int32_t nsteps)
                         c->stream != cudaStreamLegacy;
     int32_t s = 0;
     while (s < nsteps) {
-        if (graphs && c->steps_since_sort >= c->resort_every && nsteps - s >= 2 * c->resort_every) {
+        // a return to particle-id order that is due takes the place of the re-sort of an EAGER step (a captured block replays
+        // plain re-sorts only)
+        const bool defrag_due = c->steps_since_sort >= c->resort_every && c->resorts_since_defrag >= TILD_DEFRAG_EVERY &&
+                                !(c->prm.flags & TILD_FLAG_NO_DEFRAG);
+        if (graphs && !defrag_due && c->steps_since_sort >= c->resort_every && nsteps - s >= 2 * c->resort_every) {
             int rc = launch_graph_block(c);
             if (rc) return rc;
             s += 2 * c->resort_every;
@@ -802,7 +809,7 @@ int tild_step(tild_ctx* c, int32_t nsteps)
             if (rcf) return rcf;
         }
         cudaEvent_t* ev = c->ev_ok ? c->ev[c->timed_steps] : nullptr;
-        int rc = enqueue_one_step(c, ev);
+        int rc = enqueue_one_step(c, ev, true);
         if (rc) return rc;
         if (ev) c->timed_steps++;
         ++s;

@@ -171,6 +171,7 @@ struct tild_ctx {
     bool graph_leaves_clean = false;
     uint64_t step;
     int steps_since_sort;
+    int resorts_since_defrag;   // re-sorts since the state was last sorted from particle-id order (launch_defrag)
     int resort_every;
     int64_t launches;
 
@@ -214,6 +215,8 @@ int launch_pack(tild_ctx* c, const float* x, const float* v, const int32_t* type
 // src slots [0, n) -> segment-sorted dst; fills lay->seg_base and c->inv (old slot -> new slot)
 int launch_segment_sort(tild_ctx* c, const float4* X4src, float4* X4dst, SegLayout* lay);
 int launch_reorder(tild_ctx* c);  // re-sorts the internal state by segment and flips buffers
+int launch_defrag(tild_ctx* c);   // back to particle-id order + first sort (every TILD_DEFRAG_EVERY re-sorts)
+#define TILD_DEFRAG_EVERY 5
 int launch_unpermute(tild_ctx* c, const float4* src, float* dst);
 int launch_slot_ids(tild_ctx* c, uint32_t* id);                          // id[s] = original id of slot s        // dst[id[s]][0..2] = src[s].xyz
 // tild_spread.cu

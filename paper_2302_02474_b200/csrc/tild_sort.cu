@@ -437,12 +437,48 @@ int launch_reorder(tild_ctx* c)
     c->lay_valid = true;
     if (rc) return rc;
     c->steps_since_sort = 0;
+    c->resorts_since_defrag++;
     if (n > 0) {
         move_state_kernel<<<blocks_for(n), 256, 0, c->stream>>>(n, c->stp.max_bonds, c->inv, c->W4[a], c->B[a], c->W4[b], c->B[b]);
         TILD_LAUNCH_CHECK(c, "move_state_kernel");
     }
     c->cur = b;
     return launch_slot_of_id(c);   // id -> slot map of the extra mesh interactions (no-op without TILD_FLAG_EXTRAS)
+}
+
+// slot s -> slot id(s): the state in the order tild_set_state packs it (particle id = slot)
+__global__ void __launch_bounds__(256) to_id_order_kernel(int n, int max_bonds, const float4* __restrict__ X4src, const float4* __restrict__ W4src,
+                                                          const int32_t* __restrict__ Bsrc, float4* __restrict__ X4dst,
+                                                          float4* __restrict__ W4dst, int32_t* __restrict__ Bdst)
+{
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= n) return;
+    const float4 w = W4src[s];
+    const uint32_t id = __float_as_uint(w.w);
+    X4dst[id] = X4src[s];
+    W4dst[id] = w;
+    for (int k = 0; k < max_bonds; ++k) {
+        const int32_t q = Bsrc[(size_t)s * max_bonds + k];
+        Bdst[(size_t)id * max_bonds + k] = q < 0 ? -1 : (int32_t)__float_as_uint(W4src[q].w);
+    }
+}
+
+// Every TILD_DEFRAG_EVERY re-sorts the state is put back into particle-id order and sorted from there, as tild_set_state
+// does: the order-preserving re-sorts keep chain neighbours together only until they cross a tile boundary (they come back
+// to the end of their segment), and this restores the order of a fresh state (C4: interp 0.577 -> 0.543 ms after 300 steps).
+// Leaves cur where it was (two buffer flips).
+int launch_defrag(tild_ctx* c)
+{
+    const int a = c->cur, b = 1 - c->cur, n = c->mesh.n;
+    if (n > 0) {
+        to_id_order_kernel<<<blocks_for(n), 256, 0, c->stream>>>(n, c->stp.max_bonds, c->X4[a], c->W4[a], c->B[a], c->X4[b], c->W4[b], c->B[b]);
+        TILD_LAUNCH_CHECK(c, "to_id_order_kernel");
+    }
+    c->cur = b;
+    c->lay_valid = false;
+    const int rc = launch_reorder(c);
+    c->resorts_since_defrag = 0;
+    return rc;
 }
 
 int launch_unpermute(tild_ctx* c, const float4* src, float* dst)

@@ -28,6 +28,7 @@ FLAG_EXTRAS = 1024
 FLAG_NO_TMA = 2048
 FLAG_HOST_PIPELINE = 8192
 FLAG_ARRIVAL_SORT = 16384
+FLAG_NO_DEFRAG = 32768
 TIMING_NAMES = ("sort", "spread", "fft_fwd", "kspace", "fft_inv", "interp", "other", "total")
 
 EXPORTS = (
