@@ -299,8 +299,8 @@ __global__ void __launch_bounds__(RT, TILD_ROT_CTAS) interp_rot_kernel(MeshParam
             if (myslot[j] < 0) continue;
             if (MODE == 2) wj[j] = W4[(size_t)c0 + threadIdx.x + j * RT];
             // a missing partner reads the particle itself: zero separation, zero bond force, no branch in the tail
-            q0[j] = X4[ba[j].x >= 0 ? (size_t)ba[j].x : (size_t)c0 + threadIdx.x + j * RT];
-            q1[j] = X4[ba[j].y >= 0 ? (size_t)ba[j].y : (size_t)c0 + threadIdx.x + j * RT];
+            q0[j] = X4[(ba[j].x >= 0 && !(TILD_ROT_ABL & 4)) ? (size_t)ba[j].x : (size_t)c0 + threadIdx.x + j * RT];
+            q1[j] = X4[(ba[j].y >= 0 && !(TILD_ROT_ABL & 4)) ? (size_t)ba[j].y : (size_t)c0 + threadIdx.x + j * RT];
         }
         {   // L2 prefetch of the next chunk's lines (positions, partners, velocity state)
             const size_t nx = (size_t)c0 + nchunk + 8 * (size_t)threadIdx.x;
