@@ -502,7 +502,7 @@ def test_resort_keeps_the_order_of_particles_that_stay_in_their_segment(arrival)
     their relative order, with the ones that moved in behind them.  Large time step so that many particles change tiles."""
     cfg = small_cfg(order=4, grid=(32, 32, 64), box=(8.0, 8.0, 16.0), n_chains=900)
     st = inputs.make_state(cfg)
-    eng = tild.Tild(tild.params_from_config(cfg, resort_every=2, dt=0.02, flags=tild.FLAG_EAGER | (tild.FLAG_ARRIVAL_SORT if arrival else 0)))
+    eng = tild.Tild(tild.params_from_config(cfg, resort_every=2, dt=0.02, flags=tild.FLAG_EAGER | tild.FLAG_NO_DEFRAG | (tild.FLAG_ARRIVAL_SORT if arrival else 0)))   # no return to id order in between
     eng.tild_set_state(dev(st.x), dev(st.v * 3.0), dev(st.type), dev(st.bond_partner), 0)
     info = eng.tild_layout_info()
     N = np.array(cfg.grid, dtype=np.int64)
