@@ -222,10 +222,14 @@ __device__ __forceinline__ void line_fft_inv(float2 (&b)[R2], float2 (&a)[R1], c
 }
 
 template <int R1, int R2, int S>
-__global__ void __launch_bounds__(256, S <= 2 ? 2 : 1) kspace_xfft_kernel(KspaceParams k, size_t Q, const float2* __restrict__ tw,
+__global__ void __launch_bounds__(256, (S <= 2 || R1 <= 8) ? 2 : 1) kspace_xfft_kernel(KspaceParams k, size_t Q, const float2* __restrict__ tw,
                                                              const float2* __restrict__ nhat, float2* __restrict__ fhat)
 {
     constexpr int N = R1 * R2, LINES = 256 / R2, EXN = R1 * 256;
+    // S >= 3: the transformed densities X of a line live in shared memory (each thread its own S R2 entries), not in registers:
+    // 128 registers and two CTAs per SM where the shared memory allows (Nx <= 128), instead of 249 registers and one CTA
+    constexpr bool XS = S >= 3;
+    constexpr int XSTR = R1 * LINES;    // threads that hold spectra (me < R1)
     extern __shared__ float2 xs[];
     float2* stw = xs;                   // [N] twiddles
     float2* sxu = xs + N;               // [N] (u^_x(m) / V, k_x(m))
@@ -259,13 +263,19 @@ __global__ void __launch_bounds__(256, S <= 2 ? 2 : 1) kspace_xfft_kernel(Kspace
         k2yz = __ldg(k.k2[1] + my) + __ldg(k.k2[2] + mz);
     }
     __syncthreads();
-    float2 X[S][R2];                                // threads me < R1: X[J][j] = n^_J(kx = me + R1 j)
+    float2 X[XS ? 1 : S][R2];                       // threads me < R1: X[J][j] = n^_J(kx = me + R1 j)
+    float2* Xs = ex + 2 * EXN + threadIdx.x;        // XS: entry (J, j) of this thread at Xs[(J * R2 + j) * XSTR]
 #pragma unroll
     for (int J = 0; J < S; ++J) {
+        float2(&Xt)[R2] = X[XS ? 0 : J];
 #pragma unroll
-        for (int j = 0; j < R2; ++j) X[J][j] = make_float2(0.f, 0.f);
-        line_fft_fwd<R1, R2>(A[J], X[J], stw, ex + par * EXN, me, ql);
+        for (int j = 0; j < R2; ++j) Xt[j] = make_float2(0.f, 0.f);
+        line_fft_fwd<R1, R2>(A[J], Xt, stw, ex + par * EXN, me, ql);
         par ^= 1;
+        if (XS && me < R1) {
+#pragma unroll
+            for (int j = 0; j < R2; ++j) Xs[(J * R2 + j) * XSTR] = Xt[j];
+        }
     }
     // 2S inverse transforms: (I, pass) with pass 0: t_I -> y and z components, pass 1: -i k_x t_I -> x component
 #pragma unroll 1
@@ -283,10 +293,13 @@ __global__ void __launch_bounds__(256, S <= 2 ? 2 : 1) kspace_xfft_kernel(Kspace
             for (int j = 0; j < R2; ++j) {
                 const int mx = me + R1 * j;
                 float gr = 0.f, gi = 0.f;
+                float2 xj[S];
+#pragma unroll
+                for (int J = 0; J < S; ++J) xj[J] = XS ? Xs[(J * R2 + j) * XSTR] : X[XS ? 0 : J][j];
 #pragma unroll
                 for (int J = 0; J < S; ++J) {
-                    gr += cI[J] * X[J][j].x;
-                    gi += cI[J] * X[J][j].y;
+                    gr += cI[J] * xj[J].x;
+                    gi += cI[J] * xj[J].y;
                 }
                 const float2 xu = sxu[mx];
                 const float u = xu.x * uyz;
@@ -295,8 +308,8 @@ __global__ void __launch_bounds__(256, S <= 2 ? 2 : 1) kspace_xfft_kernel(Kspace
                     float er = 0.f, ei = 0.f;
 #pragma unroll
                     for (int J = 0; J < S; ++J) {
-                        er += qI[J] * X[J][j].x;
-                        ei += qI[J] * X[J][j].y;
+                        er += qI[J] * xj[J].x;
+                        ei += qI[J] * xj[J].y;
                     }
                     const float2 xe = sxe[mx];
                     const float k2 = xe.y + k2yz;
@@ -371,13 +384,18 @@ int kspace_xfft_radix(int Nx, int S)
     } while (0)
 
 // shared memory: 3 tables of N float2 + two transpose buffers of R1 * 256 float2
-static size_t xfft_smem_bytes(int N, int R2) { return (3 * (size_t)N + 2 * (size_t)(N / R2) * 256) * sizeof(float2); }
+// + S >= 3: the spectra of the S densities, S R2 entries for each of the R1 * (256 / R2) threads that hold them
+static size_t xfft_smem_bytes(int N, int R2, int S)
+{
+    const size_t xs = S >= 3 ? (size_t)S * R2 * (N / R2) * (256 / R2) : 0;
+    return (3 * (size_t)N + 2 * (size_t)(N / R2) * 256 + xs) * sizeof(float2);
+}
 
 int tild_kspace_configure(tild_ctx* c)
 {
     if (!c->xfft_R) return TILD_OK;
     const int N = c->mesh.N[0];
-    const int sm = (int)xfft_smem_bytes(N, c->xfft_R);
+    const int sm = (int)xfft_smem_bytes(N, c->xfft_R, c->mesh.S);
 #define XA(R1_, R2_, SS) TILD_CUDA(c, tild_raise_smem_limit(reinterpret_cast<const void*>(kspace_xfft_kernel<R1_, R2_, SS>), (size_t)sm))
     TILD_XFFT_DISPATCH(N, c->mesh.S, XA);
 #undef XA
@@ -390,7 +408,7 @@ int launch_kspace_xfft(tild_ctx* c, const float2* nhat, float2* fhat)
     const size_t Q = (size_t)c->mesh.N[1] * c->ksp.Nzc;
     const int N = c->mesh.N[0], lines = 256 / c->xfft_R;
     const unsigned nb = (unsigned)((Q + lines - 1) / lines);
-    const size_t sm = xfft_smem_bytes(N, c->xfft_R);
+    const size_t sm = xfft_smem_bytes(N, c->xfft_R, c->mesh.S);
 #define XL(R1_, R2_, SS) kspace_xfft_kernel<R1_, R2_, SS><<<nb, 256, sm, c->stream>>>(c->ksp, Q, c->xtw, nhat, fhat)
     TILD_XFFT_DISPATCH(N, c->mesh.S, XL);
 #undef XL
