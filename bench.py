@@ -223,10 +223,28 @@ def ours_arm(args, cfg):
     # independent replica per rank: same recipe, rank-specific seeds
     in_seed, ph_seed = replica_seeds(cfg, rank)
     st = inputs.make_state(cfg, seed=in_seed)
-    eng = tild.Tild(tild.params_from_config(cfg, flags=tild.FLAG_TIMING | args.flags, seed=ph_seed,
-                                            resort_every=args.resort_every, tile_shape=args.tile_shape), device=f"cuda:{local}")
+    # --extras: the SURVEY 8(f) rows that ride on extra meshes (per-particle charges: 1 mesh; Maier-Saupe: 5 tensor meshes)
+    xkw, xflags = {}, 0
+    if args.extras != "none":
+        xflags = tild.FLAG_EXTRAS
+        if args.extras in ("charges", "both"):
+            xkw.update(bjerrum=1.0, a_charge=0.5)
+        if args.extras in ("ms", "both"):
+            xkw.update(mu_ms=2.5)
+    eng = tild.Tild(tild.params_from_config(cfg, flags=tild.FLAG_TIMING | args.flags | xflags, seed=ph_seed,
+                                            resort_every=args.resort_every, tile_shape=args.tile_shape, **xkw), device=f"cuda:{local}")
     xd, vd = torch.from_numpy(st.x).cuda(), torch.from_numpy(st.v).cuda()
     td, bd = torch.from_numpy(st.type).cuda(), torch.from_numpy(st.bond_partner).cuda()
+    if args.extras in ("charges", "both"):      # zero-mean random charges, a third of the particles neutral
+        q = np.random.default_rng(in_seed + 5).normal(size=cfg.n).astype(np.float32)
+        q[::3] = 0.0
+        q -= q.mean()
+        eng.tild_set_charges(torch.from_numpy(q).cuda())
+    if args.extras in ("ms", "both"):           # every second bead with a next bead is an LC centre oriented along that bond
+        msp = -np.ones(cfg.n, dtype=np.int32)
+        centres = np.where(st.bond_partner[:, 1] >= 0)[0][::2]
+        msp[centres] = st.bond_partner[centres, 1]
+        eng.tild_set_ms_partners(torch.from_numpy(msp).cuda())
     eng.tild_set_state(xd, vd, td, bd, 0)
     eng.tild_step(args.warmup)
     eng.tild_get_timings()                         # synchronises and clears the stage timers
@@ -322,7 +340,7 @@ def ours_arm(args, cfg):
         "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32", "data": "synthetic",
         "config": {"workload": cfg.name, "n": cfg.n, "grid": list(cfg.grid), "order": cfg.order, "species": cfg.n_species,
-                   "resort_every": args.resort_every, "l2": "inputs larger than L2 (no flush needed)"
+                   "resort_every": args.resort_every, "extras": args.extras, "l2": "inputs larger than L2 (no flush needed)"
                    if sum(alg.values()) > 2 * 126e6 else "working set fits L2; steady-state numbers",
                    "parallelism": "replicas only" if world > 1 else "single GPU"},
         "stage_ms": stage_ms, "stage_steps_timed": nst,
@@ -395,6 +413,8 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=8)
     ap.add_argument("--flags", type=int, default=0, help="extra TILD_FLAG_* bits (kernel A/B runs)")
     ap.add_argument("--tile-shape", type=int, default=0, help="tild_params.tile_shape = TY | TZ << 8 (0 = default 8x16x32)")
+    ap.add_argument("--extras", default="none", choices=["none", "charges", "ms", "both"],
+                    help="per-particle charges and / or Maier-Saupe on their extra meshes (not the headline workload)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--sweep", action="store_true", help="run the C5 roofline sweep instead of the headline bench")
