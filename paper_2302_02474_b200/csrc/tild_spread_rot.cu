@@ -18,6 +18,9 @@ namespace {
 #ifndef TILD_SROT_SCALAR_FLUSH
 #define TILD_SROT_SCALAR_FLUSH 0   // 1: one scalar RED per node also where the vector reduction applies (A/B)
 #endif
+#ifndef TILD_SROT_FMUL2
+#define TILD_SROT_FMUL2 1   // packed FMUL2 for the 64 weight products of a particle (0.2291 -> 0.2277 ms on C4)
+#endif
 #ifndef TILD_SROT_THREADS
 #define TILD_SROT_THREADS 512
 #define TILD_SROT_CHUNK 2048
@@ -222,8 +225,18 @@ __global__ void __launch_bounds__(ST, 2) spread_rot_kernel(MeshParams m, TilePar
                 for (int jy = 0; jy < P; ++jy) {
                     const float wxy = wx[jx] * wyr[jy];
                     uint32_t* s = row[jy] + jx * EY * EZ;
+#if TILD_SROT_FMUL2
+                    {   // two packed multiplies (FMUL2, round to nearest, denormals kept) instead of four FMUL
+                        const float2 v01 = fmul2_bcast(make_float2(wz[0], wz[1]), wxy), v23 = fmul2_bcast(make_float2(wz[2], wz[3]), wxy);
+                        atomicAdd(s + 0, __float_as_uint(v01.x));
+                        atomicAdd(s + 1, __float_as_uint(v01.y));
+                        atomicAdd(s + 2, __float_as_uint(v23.x));
+                        atomicAdd(s + 3, __float_as_uint(v23.y));
+                    }
+#else
 #pragma unroll
                     for (int jz = 0; jz < P; ++jz) atomicAdd(s + jz, __float_as_uint(__fmul_rn(wxy, wz[jz])));
+#endif
                 }
             }
             ++n_tile;
