@@ -22,9 +22,11 @@ namespace {
 #define TILD_SROT_FMUL2 1   // packed FMUL2 for the 64 weight products of a particle (0.2291 -> 0.2277 ms on C4)
 #endif
 #ifndef TILD_SROT_THREADS
+// chunk of 3072 > the ~2048 particles of a C4 tile: a tile just above a chunk of 2048 was split into two chunks of ~1030,
+// whose 33-36 rounds fill the 16 warps' third turn only to a fifth (spread 0.2277 -> 0.2135 ms)
 #define TILD_SROT_THREADS 512
-#define TILD_SROT_CHUNK 2048
-#define TILD_SROT_KCAP 76
+#define TILD_SROT_CHUNK 3072
+#define TILD_SROT_KCAP 110
 #endif
 constexpr int ST = TILD_SROT_THREADS;   // threads per CTA
 constexpr int SW = ST / 32;
