@@ -75,7 +75,8 @@ typedef enum {
 #define TILD_FLAG_HOST_PIPELINE 8192u /* workspace for tild_run_host_submit / _wait: device staging of one input and two output batches */
 #define TILD_FLAG_ARRIVAL_SORT 16384u /* A/B: re-sorts hand out slots in arrival order (atomics) instead of keeping the order of the particles
                                         that stay in their segment */
-#define TILD_FLAG_NO_DEFRAG 32768u  /* A/B: never put the state back into particle-id order (done every 20 re-sorts otherwise) */
+#define TILD_FLAG_NO_DEFRAG 32768u  /* A/B: never put the state back into particle-id order (done every 5th re-sort for n >= 2^20 otherwise) */
+#define TILD_FLAG_DEFRAG_SMALL 65536u /* ... also for smaller systems (tests) */
 #define TILD_FLAG_GEN1_TILES 128u   /* first-generation tile kernels (32 bank classes with overflow rounds, per-particle work
                                       in class order) even where the rotation-class kernels apply (P = 4); for A/B runs */
 

@@ -702,7 +702,8 @@ int enqueue_one_step(tild_ctx* c, cudaEvent_t* ev, bool allow_defrag)
 {
     if (ev) TILD_CUDA(c, cudaEventRecord(ev[0], c->stream));
     if (c->steps_since_sort >= c->resort_every) {
-        const bool defrag = allow_defrag && c->resorts_since_defrag >= TILD_DEFRAG_EVERY && !(c->prm.flags & TILD_FLAG_NO_DEFRAG);
+        const bool defrag = allow_defrag && c->resorts_since_defrag >= TILD_DEFRAG_EVERY && !(c->prm.flags & TILD_FLAG_NO_DEFRAG) &&
+                            (c->mesh.n >= TILD_DEFRAG_MIN_N || (c->prm.flags & TILD_FLAG_DEFRAG_SMALL));
         int rc = defrag ? launch_defrag(c) : launch_reorder(c);
         if (rc) return rc;
     }
@@ -797,7 +798,7 @@ int tild_step(tild_ctx* c, int32_t nsteps)
         // a return to particle-id order that is due takes the place of the re-sort of an EAGER step (a captured block replays
         // plain re-sorts only)
         const bool defrag_due = c->steps_since_sort >= c->resort_every && c->resorts_since_defrag >= TILD_DEFRAG_EVERY &&
-                                !(c->prm.flags & TILD_FLAG_NO_DEFRAG);
+                                !(c->prm.flags & TILD_FLAG_NO_DEFRAG) && (c->mesh.n >= TILD_DEFRAG_MIN_N || (c->prm.flags & TILD_FLAG_DEFRAG_SMALL));
         if (graphs && !defrag_due && c->steps_since_sort >= c->resort_every && nsteps - s >= 2 * c->resort_every) {
             int rc = launch_graph_block(c);
             if (rc) return rc;

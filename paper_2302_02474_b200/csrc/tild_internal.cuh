@@ -217,6 +217,7 @@ int launch_segment_sort(tild_ctx* c, const float4* X4src, float4* X4dst, SegLayo
 int launch_reorder(tild_ctx* c);  // re-sorts the internal state by segment and flips buffers
 int launch_defrag(tild_ctx* c);   // back to particle-id order + first sort (every TILD_DEFRAG_EVERY re-sorts)
 #define TILD_DEFRAG_EVERY 5
+#define TILD_DEFRAG_MIN_N (1 << 20)   // smaller states live in L2 whatever their order, and their steps are launch-bound
 int launch_unpermute(tild_ctx* c, const float4* src, float* dst);
 int launch_slot_ids(tild_ctx* c, uint32_t* id);                          // id[s] = original id of slot s        // dst[id[s]][0..2] = src[s].xyz
 // tild_spread.cu

@@ -29,6 +29,7 @@ FLAG_NO_TMA = 2048
 FLAG_HOST_PIPELINE = 8192
 FLAG_ARRIVAL_SORT = 16384
 FLAG_NO_DEFRAG = 32768
+FLAG_DEFRAG_SMALL = 65536
 TIMING_NAMES = ("sort", "spread", "fft_fwd", "kspace", "fft_inv", "interp", "other", "total")
 
 EXPORTS = (

@@ -547,18 +547,19 @@ def test_resort_keeps_the_order_of_particles_that_stay_in_their_segment(arrival)
 
 
 def test_periodic_return_to_id_order_keeps_the_trajectory():
-    """Every 20 re-sorts tild_step puts the state back into particle-id order and sorts from there (tild_sort.cu:
-    launch_defrag).  With a re-sort every step that happens at steps 21 and 41: the trajectory must be the oracle's, and the
+    """Every 5th re-sort tild_step puts the state back into particle-id order and sorts from there (tild_sort.cu:
+    launch_defrag; TILD_FLAG_DEFRAG_SMALL: by default only for n >= 2^20).  With a re-sort every step that happens every
+    fifth step: the trajectory must be the oracle's, and the
     same as with TILD_FLAG_NO_DEFRAG up to the rounding noise of the fp32 reductions; the layout stays a valid segment sort."""
     cfg = small_cfg(order=4, grid=(32, 32, 48), box=(16.0, 16.0, 24.0), n_chains=600)
     st = inputs.make_state(cfg)
     xs = []
-    for flags in (tild.FLAG_EAGER, tild.FLAG_EAGER | tild.FLAG_NO_DEFRAG, 0):
+    for flags in (tild.FLAG_EAGER | tild.FLAG_DEFRAG_SMALL, tild.FLAG_EAGER | tild.FLAG_NO_DEFRAG, tild.FLAG_DEFRAG_SMALL):
         side = torch.cuda.Stream()
         with torch.cuda.stream(side):
-            eng = tild.Tild(tild.params_from_config(cfg, flags=flags, resort_every=1 if flags else 2), stream=side)
+            eng = tild.Tild(tild.params_from_config(cfg, flags=flags, resort_every=1 if flags & tild.FLAG_EAGER else 2), stream=side)
             eng.tild_set_state(dev(st.x), dev(st.v), dev(st.type), dev(st.bond_partner), 0)
-            eng.tild_step(45 if flags else 90)       # the graph path: 4-step blocks, defrag at re-sorts 20 and 40
+            eng.tild_step(45 if flags & tild.FLAG_EAGER else 90)   # the graph path: 4-step blocks, a return to id order every 6 re-sorts
             x = eng.tild_get_state(want_v=False)[0]
             seg, ids = eng.tild_segment_layout()
         side.synchronize()
