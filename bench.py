@@ -373,6 +373,24 @@ def ncu_traffic(workload, stage):
     return float(sum(k["dram_bytes_read"] + k["dram_bytes_write"] for k in ks))
 
 
+def windows_arm(args, cfg):
+    """Per-stage times over successive windows of 20 steps of one run (how the step time evolves with the length of the
+    run: the memory order of chain neighbours between re-sorts, profiles/r2_variants.md).  One JSON line per window."""
+    import torch
+    from paper_2302_02474_b200 import tild
+    st = inputs.make_state(cfg)
+    eng = tild.Tild(tild.params_from_config(cfg, flags=tild.FLAG_TIMING | args.flags, resort_every=args.resort_every))
+    d = lambda a: torch.from_numpy(a).cuda()
+    eng.tild_set_state(d(st.x), d(st.v), d(st.type), d(st.bond_partner), 0)
+    eng.tild_step(max(args.warmup, 0))
+    eng.tild_get_timings()
+    for w in range(args.windows):
+        eng.tild_step(20)
+        ms, nst = eng.tild_get_timings()
+        print(json.dumps({"window": w, "steps": nst, "workload": cfg.name, "flags": args.flags,
+                          "stage_ms": {k: round(v, 4) for k, v in ms.items()}}), flush=True)
+
+
 def sweep_arm(args):
     """C5 roofline sweep (BASELINE.json configs[4]): grid x order x memory order, 50 steps per point, per-stage times.
     Prints one JSON line per point; not the headline bench line."""
@@ -417,12 +435,15 @@ def main():
                     help="per-particle charges and / or Maier-Saupe on their extra meshes (not the headline workload)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--windows", type=int, default=0, help="print per-stage times for this many successive windows of 20 steps")
     ap.add_argument("--sweep", action="store_true", help="run the C5 roofline sweep instead of the headline bench")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
     cfg = inputs.CONFIGS[args.workload]
     if args.sweep:
         return sweep_arm(args)
+    if args.windows > 0:
+        return windows_arm(args, cfg)
     if args.impl == "reference":
         reference_arm(args, cfg)
     else:
