@@ -617,6 +617,37 @@ TOL_C4_RMS = 6e-5
 TOL_C4_MAX = 3.5e-4
 
 
+def test_c4_full_size_2000_steps_thermalise_and_do_not_depend_on_the_memory_order():
+    """Properties that hold at any size (no oracle run this long at 8.4 M particles): after 2000 steps of C4 every
+    coordinate is finite and inside the box, the kinetic temperature is kT (equipartition, <v^2> = kT/m per degree of
+    freedom within 1 %), the centre of mass does not drift, and two runs that only differ in how the particles are ordered
+    in memory (default: order-preserving re-sorts + returns to id order; arrival-order re-sorts) stay together: the same
+    noise (keyed by id and step) and the same forces up to fp32 rounding, which the chaotic dynamics amplify to an RMS
+    difference of ~6e-5 (max ~3e-3) by step 2000."""
+    cfg = inputs.C4
+    st = inputs.make_state(cfg)
+    side = torch.cuda.Stream()
+    xs = []
+    for flags in (0, tild.FLAG_NO_DEFRAG | tild.FLAG_ARRIVAL_SORT):
+        with torch.cuda.stream(side):
+            eng = tild.Tild(tild.params_from_config(cfg, flags=flags), stream=side)
+            eng.tild_set_state(dev(st.x), dev(st.v), dev(st.type), dev(st.bond_partner), 0)
+            eng.tild_step(2000)
+            x, v, _, step = eng.tild_get_state()
+        side.synchronize()
+        assert step == 2000
+        xn, vn = x.cpu().numpy(), v.cpu().numpy().astype(np.float64)
+        assert np.isfinite(xn).all() and np.isfinite(vn).all()
+        assert xn.min() >= 0.0 and np.all(xn.max(0) <= np.asarray(cfg.box, dtype=np.float32))
+        check(f"c4_2000_temperature_flags{flags}", abs((vn ** 2).mean() * cfg.mass / cfg.kT - 1.0), 0.01)
+        check(f"c4_2000_com_velocity_flags{flags}", np.abs(vn.mean(0)).max(), 5e-3)
+        xs.append(xn.astype(np.float64))
+        eng.close()
+    dx = min_image(xs[0] - xs[1], cfg.box)
+    check("c4_2000_orderings_rms_dx", np.sqrt((dx ** 2).mean()), 1e-3)
+    check("c4_2000_orderings_max_dx", np.abs(dx).max(), 0.05)
+
+
 @pytest.mark.parametrize("memory_order", ["random", "sorted"])
 def test_c5_headline_point_force_and_20_steps(memory_order):
     """BASELINE configs[4] at the point the sweep headlines (256^3, P = 4), in both particle memory orders: force on
