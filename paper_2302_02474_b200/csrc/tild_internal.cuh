@@ -301,18 +301,20 @@ __device__ __forceinline__ void index_1d(float x, float inv_h, int& cell, int& b
     }
 }
 
-__device__ __forceinline__ int wrap_idx(int a, int N)
-{
-    a %= N;
-    return a < 0 ? a + N : a;
-}
-
-// a in (-N, 2N): one conditional wrap each way (no integer division)
+// a in [-N, 2N): one conditional wrap each way (no integer division)
 __device__ __forceinline__ int wrap_near(int a, int N)
 {
     a += a < 0 ? N : 0;
     a -= a >= N ? N : 0;
     return a;
+}
+
+// any a; the integer division only runs for indices more than one period away (images wider than a tiny mesh)
+__device__ __forceinline__ int wrap_idx(int a, int N)
+{
+    if ((unsigned)(a + N) < 3u * (unsigned)N) return wrap_near(a, N);
+    a %= N;
+    return a < 0 ? a + N : a;
 }
 
 // Order-P assignment weights (P-fold top-hat convolution; PAPER.md L223 -> Deserno & Holm appendix).

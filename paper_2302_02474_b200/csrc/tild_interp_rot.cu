@@ -32,7 +32,7 @@ namespace {
 #ifdef TILD_ROT_PROFILE
 #define PROF_DECL long long pt_[8] = {0, 0, 0, 0, 0, 0, 0, 0}, pc_ = clock64();
 #define PROF_MARK(k) do { if (threadIdx.x == 0) { const long long n_ = clock64(); pt_[k] += n_ - pc_; pc_ = n_; } } while (0)
-#define PROF_DUMP() do { if (threadIdx.x == 0 && MODE == 2) { F4[2 * blockIdx.x] = make_float4((float)pt_[0], (float)pt_[1], (float)pt_[2], (float)pt_[3]); F4[2 * blockIdx.x + 1] = make_float4((float)pt_[4], (float)pt_[5], (float)pt_[6], (float)pt_[7]); } } while (0)
+#define PROF_DUMP() do { if (threadIdx.x == 0 && MODE == 2) { F4[2 * tile] = make_float4((float)pt_[0], (float)pt_[1], (float)pt_[2], (float)pt_[3]); F4[2 * tile + 1] = make_float4((float)pt_[4], (float)pt_[5], (float)pt_[6], (float)pt_[7]); } } while (0)
 #else
 #define PROF_DECL
 #define PROF_MARK(k)
@@ -128,13 +128,16 @@ __global__ void __launch_bounds__(RT, TILD_ROT_CTAS) interp_rot_kernel(MeshParam
                                                           float4* __restrict__ W4o, float4* __restrict__ F4,
                                                           uint32_t* __restrict__ drift_list, uint32_t* __restrict__ drift_count,
                                                           const __grid_constant__ CUtensorMap fmap, int use_tma,
-                                                          float4* __restrict__ zgrid, size_t zcount4)
+                                                          float4* __restrict__ zgrid, size_t zcount4, size_t zper)
 {
     constexpr int P = 4, CS = (REX * EY * EZ + 31) / 32 * 32;
+    // grid (nt_z, nt_y, nt_x): the tile coordinates are the block indices (no integer divisions), launch order = tile order
+    const int tz = blockIdx.x, ty = blockIdx.y, tx = blockIdx.z;
+    const int tile = (tx * tp.nt[1] + ty) * tp.nt[2] + tz;
     // The density grid of the next step, cleared here (an equal share per CTA) instead of by a memset in front of the spread:
     // this kernel is bound by the shared-memory pipe and leaves most of the HBM bandwidth unused.
     if (MODE == 2 && zgrid) {
-        const size_t per = (zcount4 + gridDim.x - 1) / gridDim.x, z0 = blockIdx.x * per, z1 = min(z0 + per, zcount4);
+        const size_t z0 = (size_t)tile * zper, z1 = min(z0 + zper, zcount4);   // zper = ceil(zcount4 / tiles), from the host
         for (size_t i = z0 + threadIdx.x; i < z1; i += RT) zgrid[i] = make_float4(0.f, 0.f, 0.f, 0.f);
     }
     static_assert(EZ % 32 == 8 || EZ % 32 == 24, "row rotation needs the P rows of a stencil to tile the 32 banks");
@@ -150,8 +153,6 @@ __global__ void __launch_bounds__(RT, TILD_ROT_CTAS) interp_rot_kernel(MeshParam
     __shared__ __align__(8) uint64_t mbar;
     uint32_t* ent = reinterpret_cast<uint32_t*>(fs + 3 * CS);
     const uint64_t step_next = *step_ptr + 1;   // the step being produced (device-side counter: graph replays see it move)
-    const int tile = blockIdx.x;
-    const int tz = tile % tp.nt[2], ty = (tile / tp.nt[2]) % tp.nt[1], tx = tile / (tp.nt[2] * tp.nt[1]);
     const int o[3] = {tx * tp.T[0] - tp.lo, ty * tp.T[1] - tp.lo, tz * tp.T[2] - tp.lo - tp.sh};
     const int E[3] = {REX, tp.E[1], EZ};
     const size_t seg0 = (size_t)tile * m.S;
@@ -460,8 +461,10 @@ cudaError_t rot_launch(const InterpArgs& a, cudaStream_t st, size_t smem, bool c
     static const CUtensorMap no_map{};
     const bool tma = a.use_tma && a.tp.E[1] == EY;     // the box of the tensor map is the template image
     const CUtensorMap* map = tma ? static_cast<const CUtensorMap*>(a.fmap) : &no_map;
-    kernel<<<a.tp.ntiles, RT, smem, st>>>(a.m, a.tp, a.s, a.step_ptr, a.seg_base, a.ffield, a.X4, a.W4, a.B, a.X4o, a.W4o, a.F4,
-                                          a.drift_list, a.drift_count, *map, tma ? 1 : 0, MODE == 2 ? a.zgrid : nullptr, a.zcount4);
+    const dim3 g((unsigned)a.tp.nt[2], (unsigned)a.tp.nt[1], (unsigned)a.tp.nt[0]);
+    kernel<<<g, RT, smem, st>>>(a.m, a.tp, a.s, a.step_ptr, a.seg_base, a.ffield, a.X4, a.W4, a.B, a.X4o, a.W4o, a.F4,
+                                a.drift_list, a.drift_count, *map, tma ? 1 : 0, MODE == 2 ? a.zgrid : nullptr, a.zcount4,
+                                (a.zcount4 + (size_t)a.tp.ntiles - 1) / (size_t)a.tp.ntiles);
     return cudaSuccess;
 }
 template <int EY, int EZ>

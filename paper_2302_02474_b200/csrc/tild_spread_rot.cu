@@ -87,7 +87,8 @@ __device__ __forceinline__ unsigned long long block_sum_u64(unsigned long long v
     return s;
 }
 
-// One CTA = one tile x one group of up to sp_group species (blockIdx.y).
+// One CTA = one tile x one group of up to sp_group species.  Grid (nt_z, nt_y, nt_x x groups): the tile coordinates are the
+// block indices (no integer divisions in the prologue of 4096 x 16 warps), launch order = linear tile order.
 // Dynamic shared memory: image u32[sp_group][SEX][EY][EZ] | ent u32[3][SSLOTS].
 template <int EY, int EZ>
 __global__ void __launch_bounds__(ST, 2) spread_rot_kernel(MeshParams m, TileParams tp, int sp_group, const uint32_t* __restrict__ seg_base,
@@ -100,22 +101,30 @@ __global__ void __launch_bounds__(ST, 2) spread_rot_kernel(MeshParams m, TilePar
     __shared__ uint32_t gcnt[2][8], nq[2];
     __shared__ uint16_t dq[SDCAP];                  // drifted particles of the chunk, done densely after the rounds
     __shared__ uint32_t rowoff[SEX * EY];           // mesh offset of image row (lx, ly), z excluded
-    const int tile = blockIdx.x;
-    const int sp0 = blockIdx.y * sp_group;
+    const int tz = blockIdx.x, ty = blockIdx.y;
+    int tx = blockIdx.z, grp = 0;
+    if (sp_group < m.S) {                            // more than one species group (uniform): blockIdx.z = group * nt_x + tx
+        grp = tx / tp.nt[0];
+        tx -= grp * tp.nt[0];
+    }
+    const int tile = (tx * tp.nt[1] + ty) * tp.nt[2] + tz;
+    const int sp0 = grp * sp_group;
     const int nsp = min(sp_group, m.S - sp0);
-    const int tz = tile % tp.nt[2], ty = (tile / tp.nt[2]) % tp.nt[1], tx = tile / (tp.nt[2] * tp.nt[1]);
     const int o[3] = {tx * tp.T[0] - tp.lo, ty * tp.T[1] - tp.lo, tz * tp.T[2] - tp.lo - tp.sh};
     const int E[3] = {SEX, tp.E[1], EZ};
     const size_t seg0 = (size_t)tile * m.S + sp0;
-    const uint32_t p_lo = seg_base[seg0], p_hi = seg_base[seg0 + nsp];
-    if (p_lo == p_hi) return;                        // empty tile (uniform)
+    const uint32_t p_lo = seg_base[seg0], p_hi = seg_base[seg0 + nsp];   // used after the first half of the zeroing: their
+                                                                         // L2 / DRAM round trip runs under it
     uint32_t* ent = sm + (size_t)sp_group * E3;
-    // the tile's positions on their way to L2 while the image is zeroed (8 particles per 128-byte line)
+    uint4* z4 = reinterpret_cast<uint4*>(sm);
+    const int n4 = nsp * E3 / 4;                     // EZ % 4 == 0
+    const int n4a = (n4 / 2 + ST - 1) / ST * ST;     // first half: whole passes of the CTA
+    for (int k = threadIdx.x; k < min(n4a, n4); k += ST) z4[k] = make_uint4(0u, 0u, 0u, 0u);
+    if (p_lo == p_hi) return;                        // empty tile (uniform)
+    // the tile's positions on their way to L2 while the rest of the image is zeroed (8 particles per 128-byte line)
     for (uint32_t i = p_lo + 8u * threadIdx.x; i < p_hi; i += 8u * ST) asm volatile("prefetch.global.L2 [%0];" ::"l"(X4 + i));
     {
-        uint4* z4 = reinterpret_cast<uint4*>(sm);
-        const int n4 = nsp * E3 / 4;                 // EZ % 4 == 0
-        for (int k = threadIdx.x; k < n4; k += ST) z4[k] = make_uint4(0u, 0u, 0u, 0u);
+        for (int k = n4a + threadIdx.x; k < n4; k += ST) z4[k] = make_uint4(0u, 0u, 0u, 0u);
         if (threadIdx.x < SEX * EY) {
             const int lx = threadIdx.x / EY, ly = threadIdx.x - lx * EY;
             rowoff[threadIdx.x] = (uint32_t)((wrap_idx(o[0] + lx, m.N[0]) * m.N[1] + wrap_idx(o[1] + ly, m.N[1])) * m.N[2]);
@@ -140,13 +149,19 @@ __global__ void __launch_bounds__(ST, 2) spread_rot_kernel(MeshParams m, TilePar
         for (int j = 0; j < SPT; ++j)
             if (threadIdx.x + j * ST < nchunk) pa[j] = X4[(size_t)c0 + threadIdx.x + j * ST];
 #endif
+#ifndef TILD_SROT_BATCH
+        // one load ahead: the position of particle j + 1 is on its way while particle j is binned
+        float4 pnext = make_float4(0.f, 0.f, 0.f, 0.f);
+        if ((int)threadIdx.x < nchunk) pnext = X4[(size_t)c0 + threadIdx.x];
+#endif
 #pragma unroll
         for (int j = 0; j < SPT; ++j) {
-            if (threadIdx.x + j * ST >= nchunk) continue;
+            if (threadIdx.x + j * ST >= nchunk) break;       // later j are beyond the chunk too
 #ifdef TILD_SROT_BATCH
             const float4 p = pa[j];
 #else
-            const float4 p = X4[(size_t)c0 + threadIdx.x + j * ST];
+            const float4 p = pnext;
+            if (j + 1 < SPT && threadIdx.x + (j + 1) * ST < nchunk) pnext = X4[(size_t)c0 + threadIdx.x + (j + 1) * ST];
 #endif
             const float pos[3] = {p.x, p.y, p.z};
             int d[3];
@@ -243,9 +258,11 @@ __global__ void __launch_bounds__(ST, 2) spread_rot_kernel(MeshParams m, TilePar
             }
             ++n_tile;
         }
-        {   // the queued drifted particles, one per thread (their fp32 reductions resolve in L2)
+        {   // the queued drifted particles, one per thread (their fp32 reductions resolve in L2), taken by the LAST warps:
+            // warp 0 always has the most rounds (k = wid, wid + SW, ...), the last ones the fewest
             const uint32_t nd = min(nq[par], (uint32_t)SDCAP);           // stable since the barrier after phase A
-            if (threadIdx.x < nd) spread_particle_global(m, X4[(size_t)c0 + dq[threadIdx.x]], grid);
+            const uint32_t td = (uint32_t)(ST - 1) - threadIdx.x;
+            if (td < nd) spread_particle_global(m, X4[(size_t)c0 + dq[td]], grid);
         }
         __syncthreads();                             // the rounds are done: the lists are free, the image is complete so far
     }
@@ -376,7 +393,7 @@ cudaError_t spread_rot_launch(const tild_ctx* c, int sp_group, size_t smem, cons
 {
     auto kernel = spread_rot_kernel<EY, EZ>;
     if (configure_only) return tild_raise_smem_limit(reinterpret_cast<const void*>(kernel), smem);
-    const dim3 g((unsigned)c->tile.ntiles, (unsigned)((c->mesh.S + sp_group - 1) / sp_group));
+    const dim3 g((unsigned)c->tile.nt[2], (unsigned)c->tile.nt[1], (unsigned)(c->tile.nt[0] * ((c->mesh.S + sp_group - 1) / sp_group)));
     kernel<<<g, ST, smem, c->stream>>>(c->mesh, c->tile, sp_group, seg_base, X4, grid);
     return cudaSuccess;
 }
