@@ -112,7 +112,9 @@ typedef struct {
     uint32_t flags;            /* TILD_FLAG_* */
     int32_t integrator;        /* TILD_INTEGRATOR_GJF (default, A11), TILD_INTEGRATOR_EM (overdamped, A11b; gamma > 0) or
                                   TILD_INTEGRATOR_VV (velocity Verlet + Langevin ExtraForce, A24) */
-    int32_t tile_shape;        /* 0 = default tile of 8 x 16 x 32 cells; else TY | TZ << 8 with TY in {8, 16}, TZ in {16, 32} */
+    int32_t tile_shape;        /* 0 = automatic: tiles of 8 x 16 x 32 cells, halved in y and then in z while there are fewer than
+                                  296 tiles or more than 4096 particles per tile; else TY | TZ << 8 with TY in {8, 16}, TZ in {16, 32}
+                                  (a zero byte leaves that edge automatic) */
     /* electrostatics on the same path (reading A22): valence per species, Bjerrum length
      * (0 = off), Gaussian smearing length of a charge; pair kernel 4 pi l_B exp(-k^2 a_q^2) / k^2, k = 0 dropped */
     double charge[TILD_MAX_SPECIES];

@@ -114,8 +114,21 @@ void configure_tiles(tild_ctx* c)
     t.enabled = p.grid[0] >= 8 && p.grid[1] >= 8 && p.grid[2] >= 8;
     const int tx = 8;
     int ty = p.tile_shape & 0xff, tz = (p.tile_shape >> 8) & 0xff;
-    if (ty != 8 && ty != 16) ty = 16;
-    if (tz != 16 && tz != 32) tz = p.grid[2] >= 32 ? 32 : 16;
+    const bool auto_y = ty != 8 && ty != 16, auto_z = tz != 16 && tz != 32;
+    if (auto_y) ty = 16;
+    if (auto_z) tz = p.grid[2] >= 32 ? 32 : 16;
+    // Default shape 8 x 16 x 32, halved in y and then in z while the tiles are too few to fill the GPU (two CTAs per SM on
+    // 148 SMs) or hold more than 4096 particles each (several chunks per species and image, and few, long CTAs: measured on
+    // the C5 sweep at 128^3, 8192 particles per tile: step 0.600 -> 0.475 ms at P = 4, 0.540 -> 0.397 ms at P = 3; C2 at 64^3,
+    // 64 tiles: 0.082 -> 0.075 ms; C3 and C4 with 2048 particles in each of 512 / 4096 tiles keep the default)
+    if (auto_y || auto_z) {
+        auto crowded = [&](int y, int z) {
+            const long long nt = (long long)((p.grid[0] + tx - 1) / tx) * ((p.grid[1] + y - 1) / y) * ((p.grid[2] + z - 1) / z);
+            return nt < 296 || (long long)p.n > 4096 * nt;
+        };
+        if (auto_y && crowded(ty, tz)) ty = 8;
+        if (auto_z && tz == 32 && crowded(ty, tz)) tz = 16;
+    }
     const int ez = (tz + t.H + t.sh + 3) / 4 * 4;
     const size_t lists_i = (size_t)TILD_INTERP_KCAP * 32 * 2 + (size_t)TILD_INTERP_CHUNK * 2;
     const size_t lists_s = (size_t)TILD_SPREAD_KCAP * 32 * 4 + (size_t)TILD_SPREAD_CHUNK * 4;
