@@ -309,7 +309,7 @@ def test_wlc_angle_special_cases():
 
 def test_harmonic_angle_force_is_minus_the_energy_gradient_and_special_cases():
     """PAPER.md Eq. 17: u_h = k_theta (theta - theta0)^2.  Gradient check, conservation laws, and a right-angle
-    trimer with theta0 = pi/3: U = k (pi/2 - pi/3)^2, end-bead force magnitude 2 k (theta - theta0) / |d|, opening."""
+    trimer with theta0 = pi/3: U = k (pi/2 - pi/3)^2, end-bead force magnitude 2 k (theta - theta0) / |d|, closing the angle (theta > theta0: each end bead is pushed towards the other arm)."""
     rng = np.random.default_rng(15)
     n_chains, nb, L = 3, 6, (7.0, 8.0, 9.0)
     n = n_chains * nb
