@@ -19,7 +19,8 @@
  * convolutions, partition of unity, first moment; grid mass; DFT vs naive O(M^2) DFT and
  * numpy.fft; PM force vs a mesh-free k-space sum and vs the direct periodic Gaussian pair sum;
  * zero net force; bonds vs closed form; GJF(gamma=0) == velocity Verlet; dt^2 energy scaling;
- * Philox vs cuRAND's host-compiled header.  End-to-end trajectory: "parity unpinned" beyond
+ * Philox vs cuRAND's host-compiled header; the uniform -> normal map (A12) through its inverse (the
+ * normals give back the Philox words' top 23 bits).  End-to-end trajectory: "parity unpinned" beyond
  * those (no reference trajectory exists).
  *
  * Build: gcc -O2 -std=c99 -ffp-contract=off -fopenmp -shared -fPIC tild_oracle.c -lm

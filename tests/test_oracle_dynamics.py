@@ -135,6 +135,39 @@ def test_noise_is_keyed_by_id_and_step_and_has_gjf_variance():
     assert abs(b.var() / (2 * 2.0 * 1.5 * 0.01) - 1) < 0.03
 
 
+def test_normals_invert_to_the_philox_words_they_were_drawn_from():
+    """Reading A12 / SURVEY O9, pinned through the INVERSE of the map (no forward Box-Muller is retyped here): from the
+    oracle's normals (z0, z1, z2) of (seed, id, step) the radius gives back u0 = exp(-(z0^2 + z1^2)/2), the polar angle gives
+    u1 = atan2(z1, z0) / 2 pi (mod 1), and z2 / sqrt(-2 ln u2) = cos 2 pi u3 gives u3 up to the reflection u -> 1 - u that
+    the cosine cannot see.  Every u must be ((x >> 9) + 0.5) 2^-23 of the matching word x of Philox4x32-10 (itself pinned
+    bit for bit against cuRAND's header) with counter (id, step lo, step hi, 0) and key (seed lo, seed hi): the top 23 bits
+    of the words come back EXACTLY.  A swapped sine / cosine, another word order, a 24-bit or unshifted uniform, a missing
+    half, a wrong counter layout: each fails."""
+    rng = np.random.default_rng(2302)
+    two23 = float(1 << 23)
+    for _ in range(400):
+        seed = int(rng.integers(0, 2 ** 63))
+        pid = int(rng.integers(0, 2 ** 32))
+        step = int(rng.integers(0, 2 ** 40))
+        z = orc.normals(seed, pid, step)
+        x = orc.philox4x32_10([pid, step & 0xFFFFFFFF, step >> 32, 0], [seed & 0xFFFFFFFF, seed >> 32]).astype(np.int64)
+        k = x >> 9                                                      # the 23 bits the reading keeps
+        u0 = np.exp(-0.5 * (z[0] ** 2 + z[1] ** 2))
+        u1 = (np.arctan2(z[1], z[0]) / (2 * np.pi)) % 1.0
+        assert abs(u0 * two23 - (k[0] + 0.5)) < 1e-3, (seed, pid, step)
+        assert abs(u1 * two23 - (k[1] + 0.5)) < 1e-3, (seed, pid, step)
+        u2 = (k[2] + 0.5) / two23
+        c = z[2] / np.sqrt(-2.0 * np.log(u2))
+        assert abs(c) <= 1.0 + 1e-12
+        u3 = np.arccos(min(1.0, max(-1.0, c))) / (2 * np.pi)            # in [0, 1/2]
+        want = (k[3] + 0.5) / two23
+        want = min(want, 1.0 - want)
+        assert abs(u3 - want) * two23 < 0.05, (seed, pid, step)
+    # the amplitude of the thermostat noise: beta = sqrt(2 gamma kT dt) z, component by component
+    p = _p(4, gamma=2.0, kT=1.5, dt=0.01, seed=987654321987)
+    assert np.allclose(orc.noise(p, 11, 5), np.sqrt(2 * 2.0 * 1.5 * 0.01) * orc.normals(987654321987, 11, 5), rtol=1e-14, atol=0)
+
+
 def test_free_particle_diffusion():
     """No forces (kappa = chi = k_bond = 0): <dr^2> = 6 (kT/gamma) [t - (1 - e^{-gamma t})/gamma] for thermal v0."""
     n = 3000
