@@ -680,7 +680,7 @@ def test_c5_sweep_point_force(grid, order, memory_order):
     assert np.abs(f.cpu().numpy() - of).max() <= REL * vec_rms(of)
 
 
-@pytest.mark.parametrize("ty,tz", [(8, 32), (8, 16), (16, 16)], ids=["y8z32", "y8z16", "y16z16"])
+@pytest.mark.parametrize("ty,tz", [(16, 32), (8, 32), (8, 16), (16, 16)], ids=["y16z32", "y8z32", "y8z16", "y16z16"])
 @pytest.mark.parametrize("P", [2, 3, 4, 5])
 @pytest.mark.parametrize("gen1", [False, True], ids=["gen2", "gen1"])
 def test_tile_shape_variants(ty, tz, P, gen1):
@@ -701,6 +701,37 @@ def test_tile_shape_variants(ty, tz, P, gen1):
     x, _, _, _ = eng.tild_get_state(want_v=False)
     ox, _, _ = orc.run(p, st.x.astype(np.float64), st.v.astype(np.float64), st.type, st.bond_partner, 0, 10, f=of)
     assert np.abs(min_image(x.cpu().numpy().astype(np.float64) - ox, cfg.box)).max() <= 1e-4
+
+
+def test_automatic_tile_shape_and_species_groups_of_the_spread():
+    """tile_shape = 0: the default 8 x 16 x 32 tile is halved in y, then in z, while there are fewer than 296 tiles or more than
+    4096 particles per tile; an explicit shape is taken as given.  With P = 4, three species and the 8 x 16 x 32 tile the spread
+    runs TWO species groups per tile (two images of 33 KB fit beside the lists, the third species goes to a second CTA:
+    blockIdx.z = group * nt_x + tile_x): spread, total force and a few steps against the oracle."""
+    small = small_cfg(order=4, grid=(40, 24, 48), box=(20.0, 12.0, 24.0), n_chains=900)
+    st, eng = make(small)
+    eng.tild_set_state(dev(st.x), dev(st.v), dev(st.type), dev(st.bond_partner), 0)
+    info = eng.tild_layout_info()
+    assert (info["tile_y"], info["tile_z"]) == (8, 16)                # 5 x 2 x 2 default tiles would leave most SMs idle
+    eng.close()
+    cfg = small_cfg(order=4, S=3, grid=(32, 32, 64), box=(16.0, 16.0, 32.0), n_chains=2500, nb=10)
+    st, eng = make(cfg, resort_every=3, tile_shape=16 | (32 << 8))
+    p = oracle_params(cfg)
+    g = eng.tild_spread(dev(st.x), dev(st.type)).cpu().numpy()
+    og = orc.spread(p, st.x, st.type)
+    assert np.abs(g - og).max() <= REL * rms(og)
+    assert np.allclose(g.sum(axis=(1, 2, 3)), np.bincount(st.type, minlength=3), rtol=1e-6)
+    eng.tild_set_state(dev(st.x), dev(st.v), dev(st.type), dev(st.bond_partner), 0)
+    info = eng.tild_layout_info()
+    assert (info["tile_y"], info["tile_z"]) == (16, 32) and info["tiles"] == 4 * 2 * 2
+    _, _, f, _ = eng.tild_get_state(want_v=False, want_f=True)
+    of = orc.force(p, st.x.astype(np.float64), st.type, st.bond_partner)
+    assert np.abs(f.cpu().numpy() - of).max() <= REL * vec_rms(of)
+    eng.tild_step(7)
+    x, _, _, _ = eng.tild_get_state(want_v=False)
+    ox, _, _ = orc.run(p, st.x.astype(np.float64), st.v.astype(np.float64), st.type, st.bond_partner, 0, 7, f=of)
+    assert np.abs(min_image(x.cpu().numpy().astype(np.float64) - ox, cfg.box)).max() <= 1e-4
+    eng.close()
 
 
 def test_two_contexts_on_their_own_streams_do_not_interfere():
