@@ -7,6 +7,10 @@
 // 1-D table look-ups (built in double on the host at tild_init; 1/V folded into the x table).
 #include "tild_internal.cuh"
 
+#ifndef TILD_XFFT_AHEAD
+#define TILD_XFFT_AHEAD 148   // L2 prefetch distance in CTAs (0: off)
+#endif
+
 namespace {
 
 template <int S>
@@ -254,6 +258,14 @@ __global__ void __launch_bounds__(256, (S <= 2 || R1 <= 8) ? 2 : 1) kspace_xfft_
 #pragma unroll
         for (int j = 0; j < R1; ++j) A[J][j] = __ldg(src + (size_t)j * xstride);
     }
+#if TILD_XFFT_AHEAD
+    {   // the lines of the CTA that follows in this CTA's slot (two CTAs per SM resident) on their way to L2: per species and
+        // x one 128-byte piece (LINES consecutive (k_y, k_z) points), S N pieces over 256 threads
+        const size_t q0n = ((size_t)blockIdx.x + TILD_XFFT_AHEAD) * LINES;
+        if (LINES * sizeof(float2) == 128 && q0n + LINES <= Q)
+            for (int i = threadIdx.x; i < S * N; i += 256) asm volatile("prefetch.global.L2 [%0];" ::"l"(nhat + (size_t)i * Q + q0n));
+    }
+#endif
     const int my = (int)(qc / k.Nzc), mz = (int)(qc % k.Nzc);
     const float uyz = __ldg(k.ufac[1] + my) * __ldg(k.ufac[2] + mz);
     const float ky = __ldg(k.kgrad[1] + my), kz = __ldg(k.kgrad[2] + mz);
