@@ -64,7 +64,8 @@ typedef enum {
 #define TILD_FLAG_GRAPH 8u         /* accepted for compatibility: graph replay is the default (see TILD_FLAG_EAGER) */
 #define TILD_FLAG_EAGER 256u       /* launch every kernel of every step individually.  Default: tild_step replays blocks of
                                       2*resort_every steps as one CUDA graph (launch-bound small systems: C1 0.066 -> 0.044 ms
-                                      per step) whenever it can -- no TILD_FLAG_TIMING, an even resort_every, and a stream
+                                      per step; a cycle that starts with the periodic return to particle-id order is a block of
+                                      resort_every steps) whenever it can -- no TILD_FLAG_TIMING, an even resort_every, and a stream
                                       that can be captured (not the legacy default stream); otherwise it launches eagerly */
 #define TILD_FLAG_2D 512u          /* two-dimensional system (Listing 1 L65; A27): grid[2] must be 1; the z
                                       coordinates are carried along unchanged, no force, noise or velocity along z.  box[2] is

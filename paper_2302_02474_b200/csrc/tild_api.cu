@@ -282,6 +282,16 @@ int stage_layout(tild_ctx* c, const float* x, const int32_t* type)
     return launch_segment_sort(c, c->F4, c->SX4, &c->lay_stage);
 }
 
+// the instantiated graphs have the current choice of extra interactions baked in
+void drop_graphs(tild_ctx* c)
+{
+    for (int g = 0; g < 2; ++g)
+        if (c->graph_ok[g]) {
+            cudaGraphExecDestroy(c->graph_exec[g]);
+            c->graph_ok[g] = false;
+        }
+}
+
 }  // namespace
 
 extern "C" {
@@ -546,7 +556,7 @@ void tild_destroy(tild_ctx* c)
         cufftDestroy(c->plan_x_r2c);
         cufftDestroy(c->plan_x_c2r);
     }
-    if (c->graph_ok) cudaGraphExecDestroy(c->graph_exec);
+    drop_graphs(c);
     if (c->hp_in) {
         cudaStreamSynchronize(c->hp_in);
         cudaStreamSynchronize(c->hp_out);
@@ -740,37 +750,42 @@ int enqueue_one_step(tild_ctx* c, cudaEvent_t* ev, bool allow_defrag)
     return TILD_OK;
 }
 
-// TILD_FLAG_GRAPH: two re-sort cycles (2 * resort_every steps, starting with a re-sort) as one CUDA graph.  After an
-// even number of steps per cycle and two cycles every buffer pointer is back where it started, and the step index
-// lives in device memory, so the instantiated graph can be replayed as it is.
-int launch_graph_block(tild_ctx* c)
+// Graph replay.  Block 0: two re-sort cycles (2 * resort_every steps, starting with a re-sort).  After an even number of
+// steps per cycle and two cycles every buffer pointer is back where it started, and the step index lives in device
+// memory, so the instantiated graph can be replayed as it is.  Block 1 (with_defrag): ONE cycle that starts with the return
+// to particle-id order -- launch_defrag flips the buffers twice (to id order, then the sort), so one cycle already ends where
+// it started; without it the step at which the return is due and the rest of its cycle ran as single launches.
+int launch_graph_block(tild_ctx* c, bool with_defrag)
 {
-    const int block = 2 * c->resort_every;
+    const int g = with_defrag ? 1 : 0;
+    const int block = (with_defrag ? 1 : 2) * c->resort_every;
     if (!c->grid_clean) {   // the captured block starts from a cleared density grid (its steps clear it for one another)
         TILD_CUDA(c, cudaMemsetAsync(c->grid, 0, sizeof(float) * c->M * c->mesh.S, c->stream));
         c->grid_clean = true;
     }
-    if (!(c->graph_ok && c->graph_cur == c->cur && c->graph_x0 == c->X4[0])) {
-        if (c->graph_ok) {
-            cudaGraphExecDestroy(c->graph_exec);
-            c->graph_ok = false;
+    if (!(c->graph_ok[g] && c->graph_cur[g] == c->cur && c->graph_x0[g] == c->X4[0])) {
+        if (c->graph_ok[g]) {
+            cudaGraphExecDestroy(c->graph_exec[g]);
+            c->graph_ok[g] = false;
         }
         // capture: nothing executes, so the host bookkeeping the enqueue advances is put back afterwards
         const int cur0 = c->cur, sss0 = c->steps_since_sort, rsd0 = c->resorts_since_defrag;
+        const bool lay_valid0 = c->lay_valid;
         const uint64_t step0 = c->step;
         const int64_t launches0 = c->launches;
         float4* const x0[2] = {c->X4[0], c->X4[1]};
         float4* const w0[2] = {c->W4[0], c->W4[1]};
         TILD_CUDA(c, cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal));
         int rc = TILD_OK;
-        for (int i = 0; i < block && rc == TILD_OK; ++i) rc = enqueue_one_step(c, nullptr, false);
+        for (int i = 0; i < block && rc == TILD_OK; ++i) rc = enqueue_one_step(c, nullptr, with_defrag && i == 0);
         cudaGraph_t graph = nullptr;
         const cudaError_t e = cudaStreamEndCapture(c->stream, &graph);
-        c->graph_launches = c->launches - launches0;
-        c->graph_leaves_clean = c->grid_clean;
+        c->graph_launches[g] = c->launches - launches0;
+        c->graph_leaves_clean2[g] = c->grid_clean;
         c->grid_clean = true;   // nothing ran
         const bool same = c->cur == cur0 && c->X4[0] == x0[0] && c->W4[0] == w0[0] && c->steps_since_sort == sss0;
         c->cur = cur0; c->steps_since_sort = sss0; c->step = step0; c->launches = launches0; c->resorts_since_defrag = rsd0;
+        c->lay_valid = lay_valid0;
         c->X4[0] = x0[0]; c->X4[1] = x0[1]; c->W4[0] = w0[0]; c->W4[1] = w0[1];
         if (rc != TILD_OK || e != cudaSuccess || !graph || !same) {
             if (graph) cudaGraphDestroy(graph);
@@ -778,18 +793,23 @@ int launch_graph_block(tild_ctx* c)
             return tild_fail(c, TILD_ECUDA, "CUDA graph capture of %d steps failed: %s", block,
                              e != cudaSuccess ? cudaGetErrorString(e) : "state does not return to its start");
         }
-        const cudaError_t ei = cudaGraphInstantiate(&c->graph_exec, graph, 0);
+        const cudaError_t ei = cudaGraphInstantiate(&c->graph_exec[g], graph, 0);
         cudaGraphDestroy(graph);
         if (ei != cudaSuccess) return tild_fail(c, TILD_ECUDA, "cudaGraphInstantiate: %s", cudaGetErrorString(ei));
-        c->graph_ok = true;
-        c->graph_cur = c->cur;
-        c->graph_x0 = c->X4[0];
+        c->graph_ok[g] = true;
+        c->graph_cur[g] = c->cur;
+        c->graph_x0[g] = c->X4[0];
     }
-    TILD_CUDA(c, cudaGraphLaunch(c->graph_exec, c->stream));
-    c->grid_clean = c->graph_leaves_clean;
+    TILD_CUDA(c, cudaGraphLaunch(c->graph_exec[g], c->stream));
+    c->grid_clean = c->graph_leaves_clean2[g];
     c->step += (uint64_t)block;          // pointers, cur and steps_since_sort end where they started
-    c->resorts_since_defrag += 2;
-    c->launches += c->graph_launches;
+    if (with_defrag) {
+        c->resorts_since_defrag = 0;
+        c->lay_valid = true;             // the sort inside the block was the sort of a fresh state: c->lay describes X4[cur]
+    } else {
+        c->resorts_since_defrag += 2;
+    }
+    c->launches += c->graph_launches[g];
     return TILD_OK;
 }
 
@@ -808,14 +828,14 @@ int tild_step(tild_ctx* c, int32_t nsteps)
                         c->stream != cudaStreamLegacy;
     int32_t s = 0;
     while (s < nsteps) {
-        // a return to particle-id order that is due takes the place of the re-sort of an EAGER step (a captured block replays
-        // plain re-sorts only)
+        // a return to particle-id order that is due takes the place of the re-sort that starts a cycle: as a captured block of
+        // one cycle where graphs replay, as the re-sort of an eager step otherwise
         const bool defrag_due = c->steps_since_sort >= c->resort_every && c->resorts_since_defrag >= TILD_DEFRAG_EVERY &&
                                 !(c->prm.flags & TILD_FLAG_NO_DEFRAG) && (c->mesh.n >= TILD_DEFRAG_MIN_N || (c->prm.flags & TILD_FLAG_DEFRAG_SMALL));
-        if (graphs && !defrag_due && c->steps_since_sort >= c->resort_every && nsteps - s >= 2 * c->resort_every) {
-            int rc = launch_graph_block(c);
+        if (graphs && c->steps_since_sort >= c->resort_every && nsteps - s >= (defrag_due ? 1 : 2) * c->resort_every) {
+            int rc = launch_graph_block(c, defrag_due);
             if (rc) return rc;
-            s += 2 * c->resort_every;
+            s += (defrag_due ? 1 : 2) * c->resort_every;
             continue;
         }
         if (c->ev_ok && c->timed_steps == TILD_MAX_TIMED_STEPS) {   // ring full: fold it into the sums (synchronises)
@@ -900,10 +920,7 @@ int tild_set_charges(tild_ctx* c, const float* q)
     if (!c->Fext) return tild_fail(c, TILD_EINVAL, "tild_set_charges needs TILD_FLAG_EXTRAS at tild_init");
     c->has_q = q != nullptr;
     c->ksp.has_el = (c->prm.bjerrum > 0.0 && !c->has_q) ? 1 : 0;     // A25: the charge mesh replaces the charges per species
-    if (c->graph_ok) {                                               // a captured block has the old choice baked in
-        cudaGraphExecDestroy(c->graph_exec);
-        c->graph_ok = false;
-    }
+    drop_graphs(c);                                                  // a captured block has the old choice baked in
     if (q && c->mesh.n > 0)
         TILD_CUDA(c, cudaMemcpyAsync(c->q_id, q, sizeof(float) * (size_t)c->mesh.n, cudaMemcpyDeviceToDevice, c->stream));
     return TILD_OK;
@@ -915,10 +932,7 @@ int tild_set_ms_partners(tild_ctx* c, const int32_t* partner)
     if (!c) return TILD_EINVAL;
     if (!c->Fext) return tild_fail(c, TILD_EINVAL, "tild_set_ms_partners needs TILD_FLAG_EXTRAS at tild_init");
     c->has_ms = partner != nullptr;
-    if (c->graph_ok) {
-        cudaGraphExecDestroy(c->graph_exec);
-        c->graph_ok = false;
-    }
+    drop_graphs(c);                                                  // a captured block has the old choice baked in
     if (partner && c->mesh.n > 0)
         TILD_CUDA(c, cudaMemcpyAsync(c->msp_id, partner, sizeof(int32_t) * (size_t)c->mesh.n, cudaMemcpyDeviceToDevice, c->stream));
     return TILD_OK;

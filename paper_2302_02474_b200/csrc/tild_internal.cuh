@@ -175,12 +175,14 @@ struct tild_ctx {
     int resort_every;
     int64_t launches;
 
-    // TILD_FLAG_GRAPH: instantiated graph of two re-sort cycles and the state it was captured in
-    cudaGraphExec_t graph_exec;
-    bool graph_ok;
-    int graph_cur;
-    float4* graph_x0;
-    int64_t graph_launches;
+    // Graph replay: [0] the instantiated graph of two re-sort cycles, [1] of one cycle that starts with the return to
+    // particle-id order (launch_defrag), each with the state it was captured in
+    cudaGraphExec_t graph_exec[2];
+    bool graph_ok[2];
+    int graph_cur[2];
+    float4* graph_x0[2];
+    int64_t graph_launches[2];
+    bool graph_leaves_clean2[2];
 
     // timing
     cudaEvent_t ev[TILD_MAX_TIMED_STEPS][TILD_N_STAGE_EVENTS];
